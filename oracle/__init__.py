@@ -1,0 +1,283 @@
+"""CPU oracle for the LO-AFQMC local energy -- TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Thin ctypes wrapper around oracle/lo_oracle.cpp (plain fp64 loops written from the paper) plus the
+glue that strings its steps together.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It shares nothing with the CUDA path
+(paper_2202_00832_b200) and never imports it.  Pins: tests/test_oracle_*.py; beyond them the
+energies are "parity unpinned" to any number printed by the paper (it prints none).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lo_oracle.cpp")
+_LIB = os.path.join(_HERE, "liblo_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/lo_oracle.cpp with g++ (OpenMP) into oracle/liblo_oracle.so."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _l():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def num_threads() -> int:
+    return int(_l().orc_num_threads())
+
+
+# ------------------------------------------------------------------ single steps
+def theta(psi, phi):
+    """Eq. 15: Theta = Phi (Psi^T Phi)^-1.  Returns (theta [N,O], det(Psi^T Phi), status)."""
+    psi, phi = _f64(psi), _c128(phi)
+    N, O = psi.shape
+    th = np.empty((N, O), dtype=np.complex128)
+    det = np.zeros(1, dtype=np.complex128)
+    st = _l().orc_theta(C.c_int(N), C.c_int(O), _p(psi), _p(phi), _p(th), _p(det))
+    return th, det[0], int(st)
+
+
+def green(psi, th):
+    """Eq. 14: G[p,q] = sum_i Theta[q,i] Psi[p,i]."""
+    psi, th = _f64(psi), _c128(th)
+    N, O = psi.shape
+    G = np.empty((N, N), dtype=np.complex128)
+    _l().orc_green(C.c_int(N), C.c_int(O), _p(psi), _p(th), _p(G))
+    return G
+
+
+def energy_bruteforce(h, L, Ga, Gb=None):
+    """O1: (E1, E_J, E_K) from Eq. 8 + Eq. 10 with explicit spin sums; closed shell when Gb is None."""
+    h, L, Ga = _f64(h), _f64(L), _c128(Ga)
+    Gb = Ga if Gb is None else _c128(Gb)
+    out = np.zeros(3, dtype=np.complex128)
+    _l().orc_energy_bruteforce(C.c_int(h.shape[0]), C.c_int(L.shape[0]), _p(h), _p(L), _p(Ga), _p(Gb), _p(out))
+    return out
+
+
+def half_rotate(L, h, psi):
+    """Lbar[g,i,p] = sum_q L[g,p,q] psi[q,i]; hbar[i,p] = sum_q psi[q,i] h[q,p]."""
+    L, h, psi = _f64(L), _f64(h), _f64(psi)
+    X, N, _ = L.shape
+    O = psi.shape[1]
+    Lbar = np.empty((X, O, N))
+    hbar = np.empty((O, N))
+    _l().orc_half_rotate(C.c_int(N), C.c_int(X), C.c_int(O), _p(L), _p(h), _p(psi), _p(Lbar), _p(hbar))
+    return Lbar, hbar
+
+
+def _ptr_array(arrs):
+    return (C.c_void_p * len(arrs))(*[a.ctypes.data for a in arrs])
+
+
+def onebody_coulomb(Lbars, hbars, thetas, want_X=False):
+    """(E1, E_J) by the Cholesky route for 1 (closed shell) or 2 (unrestricted) spins; optionally X^g."""
+    Lbars = [_f64(a) for a in Lbars]
+    hbars = [_f64(a) for a in hbars]
+    thetas = [_c128(a) for a in thetas]
+    ns = len(Lbars)
+    X, _, N = Lbars[0].shape
+    O = (C.c_int * ns)(*[a.shape[1] for a in Lbars])
+    out = np.zeros(2, dtype=np.complex128)
+    Xg = np.zeros(X, dtype=np.complex128)
+    _l().orc_onebody_coulomb(C.c_int(N), C.c_int(X), C.c_int(ns), O, _ptr_array(Lbars), _ptr_array(hbars),
+                             _ptr_array(thetas), _p(out), _p(Xg))
+    return (out[0], out[1], Xg) if want_X else (out[0], out[1])
+
+
+def exchange_cholesky(Lbar, th):
+    """O2 single-spin exchange sum, Eq. 16."""
+    Lbar, th = _f64(Lbar), _c128(th)
+    X, O, N = Lbar.shape
+    out = np.zeros(1, dtype=np.complex128)
+    _l().orc_exchange_cholesky(C.c_int(N), C.c_int(X), C.c_int(O), _p(Lbar), _p(th), _p(out))
+    return out[0]
+
+
+def pair_eri(Lbar, i, j):
+    """Y^{ij}[p,q] = sum_g Lbar[g,i,p] Lbar[g,j,q]."""
+    Lbar = _f64(Lbar)
+    X, O, N = Lbar.shape
+    Y = np.empty((N, N))
+    _l().orc_pair_eri(C.c_int(N), C.c_int(X), C.c_int(O), _p(Lbar), C.c_int(i), C.c_int(j), _p(Y))
+    return Y
+
+
+def exchange_full_eri(Lbar, th):
+    """O3 single-spin exchange sum from on-the-fly pair ERI blocks, Eq. 17."""
+    Lbar, th = _f64(Lbar), _c128(th)
+    X, O, N = Lbar.shape
+    out = np.zeros(1, dtype=np.complex128)
+    _l().orc_exchange_full_eri(C.c_int(N), C.c_int(X), C.c_int(O), _p(Lbar), _p(th), _p(out))
+    return out[0]
+
+
+def svd(A):
+    """One-sided Jacobi SVD.  Returns (Ut [n,n] rows = left vectors, s descending, Wt [n,n] rows = right vectors)."""
+    A = _f64(A)
+    n = A.shape[0]
+    Ut, s, Wt = np.empty((n, n)), np.empty(n), np.empty((n, n))
+    _l().orc_svd(C.c_int(n), _p(A), _p(Ut), _p(s), _p(Wt))
+    return Ut, s, Wt
+
+
+# ------------------------------------------------------------------ factor sets
+@dataclass
+class FactorSet:
+    """Truncated factors of one spin: pairs (pi[k] <= pj[k]) with rank r[k]; rows of pair k start at off[k]."""
+    N: int
+    O: int
+    pi: np.ndarray
+    pj: np.ndarray
+    r: np.ndarray
+    off: np.ndarray
+    U: np.ndarray        # [sum r, N]
+    sigma: np.ndarray    # [sum r]
+    W: np.ndarray        # [sum r, N]
+
+    @property
+    def sum_rank(self):
+        return int(self.r.sum())
+
+
+def all_pairs(O):
+    pi, pj = np.triu_indices(O)
+    return pi.astype(np.int32), pj.astype(np.int32)
+
+
+def full_svd_pairs(Lbar, pi, pj):
+    """O4 first half: full sorted SVD of the listed pair blocks (OpenMP over pairs)."""
+    Lbar = _f64(Lbar)
+    X, O, N = Lbar.shape
+    pi = np.ascontiguousarray(pi, dtype=np.int32)
+    pj = np.ascontiguousarray(pj, dtype=np.int32)
+    n = len(pi)
+    Ut, s, Wt = np.empty((n, N, N)), np.empty((n, N)), np.empty((n, N, N))
+    _l().orc_factor_pairs(C.c_int(N), C.c_int(X), C.c_int(O), _p(Lbar), C.c_int(n), _p(pi), _p(pj), _p(Ut), _p(s), _p(Wt))
+    return Ut, s, Wt
+
+
+def truncate(N, O, pi, pj, Ut, s, Wt, T) -> FactorSet:
+    """O4 second half (Eq. 18): keep the K with sigma_K > T (strict, absolute)."""
+    r = (s > T).sum(axis=1).astype(np.int32)
+    off = np.zeros(len(r), dtype=np.int64)
+    off[1:] = np.cumsum(r)[:-1]
+    R = int(r.sum())
+    U, W, sg = np.empty((R, N)), np.empty((R, N)), np.empty(R)
+    for k in range(len(r)):
+        U[off[k]:off[k] + r[k]] = Ut[k, :r[k]]
+        W[off[k]:off[k] + r[k]] = Wt[k, :r[k]]
+        sg[off[k]:off[k] + r[k]] = s[k, :r[k]]
+    return FactorSet(N, O, np.asarray(pi, np.int32), np.asarray(pj, np.int32), r, off, U, sg, W)
+
+
+def own_factors(Lbar, T) -> FactorSet:
+    """O4: the oracle's own factor set of one spin at threshold T, all pairs i<=j."""
+    X, O, N = Lbar.shape
+    pi, pj = all_pairs(O)
+    Ut, s, Wt = full_svd_pairs(Lbar, pi, pj)
+    return truncate(N, O, pi, pj, Ut, s, Wt, T)
+
+
+def make_factor_set(N, O, pi, pj, r, U, sigma, W) -> FactorSet:
+    """Wrap factors obtained elsewhere (e.g. lo_factor_pair of the library under test) for O5."""
+    r = np.ascontiguousarray(r, dtype=np.int32)
+    off = np.zeros(len(r), dtype=np.int64)
+    off[1:] = np.cumsum(r)[:-1]
+    return FactorSet(N, O, np.ascontiguousarray(pi, np.int32), np.ascontiguousarray(pj, np.int32), r, off,
+                     _f64(U).reshape(-1, N), _f64(sigma).reshape(-1), _f64(W).reshape(-1, N))
+
+
+def _fs_args(fs: FactorSet):
+    return (C.c_int(fs.N), C.c_int(fs.O), C.c_int(len(fs.r)), _p(fs.pi), _p(fs.pj), _p(fs.r), _p(fs.off),
+            _p(fs.U), _p(fs.sigma), _p(fs.W))
+
+
+def exchange_lo(fs: FactorSet, th):
+    """O5 single-spin truncated exchange sum, Eq. 19/22."""
+    th = _c128(th)
+    out = np.zeros(1, dtype=np.complex128)
+    _l().orc_exchange_lo(*_fs_args(fs), _p(th), _p(out))
+    return out[0]
+
+
+def coulomb_lo(fs: FactorSet, th):
+    """Paper-literal compressed Coulomb double sum S (closed shell E_J^LO = 2 S), Eq. 19/22."""
+    th = _c128(th)
+    out = np.zeros(1, dtype=np.complex128)
+    _l().orc_coulomb_lo(*_fs_args(fs), _p(th), _p(out))
+    return out[0]
+
+
+# ------------------------------------------------------------------ whole energies
+def local_energy_exact(h, L, psis, phis, route="cholesky"):
+    """Exact (untruncated) local energy of ONE walker: returns (E_L, E1, E_J, E_K).
+    route: 'bruteforce' (O1), 'cholesky' (O2), 'full_eri' (O3).  psis/phis: per-spin lists."""
+    ns = len(psis)
+    ths = []
+    for psi, phi in zip(psis, phis):
+        th, _, st = theta(psi, phi)
+        if st:
+            nan = complex(np.nan, np.nan)
+            return nan, nan, nan, nan
+        ths.append(th)
+    if route == "bruteforce":
+        Gs = [green(psi, th) for psi, th in zip(psis, ths)]
+        e1, ej, ek = energy_bruteforce(h, L, Gs[0], Gs[1] if ns == 2 else None)
+        return e1 + ej + ek, e1, ej, ek
+    hr = [half_rotate(L, h, psi) for psi in psis]
+    e1, ej = onebody_coulomb([a for a, _ in hr], [b for _, b in hr], ths)
+    fn = exchange_cholesky if route == "cholesky" else exchange_full_eri
+    ek = sum(fn(hr[s][0], ths[s]) for s in range(ns))
+    if ns == 2:
+        ek *= 0.5
+    return e1 + ej + ek, e1, ej, ek
+
+
+def local_energy_lo(psis, Lbars, hbars, fsets, phis):
+    """The LO local energy of a batch of walkers on given factor sets (one per spin):
+    returns (E [n_w,4] = E_L,E1,E_J,E_K ; status [n_w]).  OpenMP over walkers; bench.py's cpu_baseline."""
+    ns = len(psis)
+    psis = [_f64(a) for a in psis]
+    Lbars = [_f64(a) for a in Lbars]
+    hbars = [_f64(a) for a in hbars]
+    phis = [_c128(a) for a in phis]
+    n_w, N, _ = phis[0].shape
+    X = Lbars[0].shape[0]
+    O = (C.c_int * ns)(*[a.shape[1] for a in psis])
+    npairs = (C.c_int * ns)(*[len(f.r) for f in fsets])
+    out = np.zeros((n_w, 4), dtype=np.complex128)
+    status = np.zeros(n_w, dtype=np.int32)
+    _l().orc_local_energy_lo(C.c_int(n_w), C.c_int(N), C.c_int(X), C.c_int(ns), O, _ptr_array(psis), _ptr_array(Lbars),
+                             _ptr_array(hbars), npairs, _ptr_array([f.pi for f in fsets]), _ptr_array([f.pj for f in fsets]),
+                             _ptr_array([f.r for f in fsets]), _ptr_array([f.off for f in fsets]),
+                             _ptr_array([f.U for f in fsets]), _ptr_array([f.sigma for f in fsets]),
+                             _ptr_array([f.W for f in fsets]), _ptr_array(phis), _p(out), _p(status))
+    return out, status

@@ -1,0 +1,303 @@
+"""Pins of the CPU oracle: the oracle is checked against what the paper and the
+mathematics fix -- four algebraically equal routes (Eq. 10/16/17/19 at T=0), the closed-form HF energy,
+invariances, projector identities, degenerate cases, Eckart-Young, the truncation bound, textbook SVDs and
+numpy's LAPACK SVD.  CPU only."""
+import math
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+
+RTOL = 1e-11
+
+
+def rel(a, b):
+    return abs(a - b) / max(abs(b), 1e-300)
+
+
+def exact(P, phis, w, route):
+    return np.array(oracle.local_energy_exact(P.h, P.L, P.psi, [ph[w] for ph in phis], route))
+
+
+# ---------------------------------------------------------------- P1 / P2: four routes agree at T=0
+def test_p1_routes_agree_c0(c0, c0_walkers):
+    Lbar, hbar = oracle.half_rotate(c0.L, c0.h, c0.psi[0])
+    fs0 = oracle.own_factors(Lbar, 0.0)
+    assert (fs0.r == c0.N).all()                      # T=0 keeps every sigma>0
+    E_lo, st = oracle.local_energy_lo(c0.psi, [Lbar], [hbar], [fs0], c0_walkers)
+    assert (st == 0).all()
+    for w in range(c0.n_w):
+        e_bf = exact(c0, c0_walkers, w, "bruteforce")     # Eq. 10
+        e_ch = exact(c0, c0_walkers, w, "cholesky")       # Eq. 16
+        e_fe = exact(c0, c0_walkers, w, "full_eri")       # Eq. 17
+        scale = abs(e_bf[0])
+        for k in range(4):
+            assert abs(e_ch[k] - e_bf[k]) <= RTOL * max(scale, abs(e_bf[k]))
+            assert abs(e_fe[k] - e_bf[k]) <= RTOL * max(scale, abs(e_bf[k]))
+            assert abs(E_lo[w, k] - e_bf[k]) <= RTOL * max(scale, abs(e_bf[k]))   # Eq. 19 at T=0
+
+
+def test_p2_untruncated_svd_exact_c1(c1, c1_walkers):
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, c1.psi[0])
+    fs0 = oracle.own_factors(Lbar, 0.0)
+    E_lo, _ = oracle.local_energy_lo(c1.psi, [Lbar], [hbar], [fs0], [c1_walkers[0][:3]])
+    for w in range(3):
+        th, _, _ = oracle.theta(c1.psi[0], c1_walkers[0][w])
+        ek = oracle.exchange_cholesky(Lbar, th)
+        assert abs(E_lo[w, 3] - ek) <= 1e-11 * abs(ek)
+        assert abs(oracle.exchange_full_eri(Lbar, th) - ek) <= 1e-11 * abs(ek)
+
+
+# ---------------------------------------------------------------- P3: closed-form HF energy
+@pytest.mark.parametrize("cfg", ["c0", "c1"])
+def test_p3_hf_closed_form(cfg, request):
+    P = request.getfixturevalue(cfg)
+    psi = P.psi[0]
+    D = psi @ psi.T
+    LD = np.einsum("gpq,qr->gpr", P.L, D)
+    e_hf = 2 * np.trace(P.h @ D) + 2 * (np.trace(LD, axis1=1, axis2=2) ** 2).sum() - np.einsum("gpr,grp->", LD, LD)
+    routes = ["bruteforce", "cholesky", "full_eri"] if cfg == "c0" else ["cholesky", "full_eri"]
+    for route in routes:
+        e = oracle.local_energy_exact(P.h, P.L, P.psi, [psi.astype(np.complex128)], route)[0]
+        assert e.imag == 0.0
+        assert rel(e.real, e_hf) < 1e-11
+    th, det, st = oracle.theta(psi, psi.astype(np.complex128))
+    assert st == 0 and np.abs(th - psi).max() < 1e-13 and abs(det - 1) < 1e-12
+
+
+# ---------------------------------------------------------------- P4: occupied rotation
+def test_p4_occupied_rotation(c1, c1_walkers):
+    psi = c1.psi[0]
+    R = gen.random_orthogonal(psi.shape[1], 7)
+    psi_r = psi @ R
+    phi = c1_walkers[0][1]
+    e0 = np.array(oracle.local_energy_exact(c1.h, c1.L, [psi], [phi], "cholesky"))
+    e1 = np.array(oracle.local_energy_exact(c1.h, c1.L, [psi_r], [phi], "cholesky"))
+    assert np.abs(e0 - e1).max() <= 1e-10 * abs(e0[0])
+    # LO at T=0 with the rotated (delocalised) trial is still exact
+    Lb_r, hb_r = oracle.half_rotate(c1.L, c1.h, psi_r)
+    pi, pj = np.array([0, 0, 3], np.int32), np.array([0, 5, 17], np.int32)
+    Ut, s, Wt = oracle.full_svd_pairs(Lb_r, pi, pj)
+    th, _, _ = oracle.theta(psi_r, phi)
+    for k in range(3):
+        Y = oracle.pair_eri(Lb_r, pi[k], pj[k])
+        exact_e = th[:, pj[k]] @ Y @ th[:, pi[k]]
+        lo = ((Ut[k] @ th[:, pj[k]]) * s[k] * (Wt[k] @ th[:, pi[k]])).sum()
+        assert abs(lo - exact_e) <= 1e-11 * abs(exact_e)
+
+
+def test_p4_localised_compresses_better():
+    # delocalising the trial raises the ranks at fixed T>0.  Use the rank-structured
+    # "vector" reading where distance decay drives the ranks.
+    P = gen.make_problem(1, reading="vector")
+    psi = P.psi[0]
+    Lb, _ = oracle.half_rotate(P.L, P.h, psi)
+    Lb_r, _ = oracle.half_rotate(P.L, P.h, psi @ gen.random_orthogonal(psi.shape[1], 3))
+    pi, pj = oracle.all_pairs(psi.shape[1])
+    sel = slice(0, None, 7)
+    _, s, _ = oracle.full_svd_pairs(Lb, pi[sel], pj[sel])
+    _, s_r, _ = oracle.full_svd_pairs(Lb_r, pi[sel], pj[sel])
+    T = 1e-2
+    assert (s_r > T).sum() > (s > T).sum()
+
+
+# ---------------------------------------------------------------- P5: walker gauge invariance
+def test_p5_gauge(c0, c0_walkers):
+    rng = np.random.default_rng(5)
+    O = c0.n_occ[0]
+    Cm = rng.standard_normal((O, O)) + 1j * rng.standard_normal((O, O))
+    phi = c0_walkers[0][2]
+    e0 = np.array(oracle.local_energy_exact(c0.h, c0.L, c0.psi, [phi], "cholesky"))
+    e1 = np.array(oracle.local_energy_exact(c0.h, c0.L, c0.psi, [phi @ Cm], "cholesky"))
+    assert np.abs(e0 - e1).max() <= 1e-9 * abs(e0[0]) * np.linalg.cond(Cm)
+
+
+# ---------------------------------------------------------------- P6: projector identities
+@pytest.mark.parametrize("cfg", ["c0", "c1"])
+def test_p6_projector(cfg, request):
+    P = request.getfixturevalue(cfg)
+    W = request.getfixturevalue(cfg + "_walkers")
+    psi, phi = P.psi[0], W[0][0]
+    th, det, st = oracle.theta(psi, phi)
+    O = psi.shape[1]
+    assert st == 0
+    assert np.abs(psi.T @ th - np.eye(O)).max() < 1e-11
+    G = oracle.green(psi, th)
+    assert abs(np.trace(G) - O) < 1e-10
+    assert np.abs(G @ G - G).max() < 1e-10
+    assert rel(det, np.linalg.det(psi.T @ phi)) < 1e-11
+    assert np.abs(th - phi @ np.linalg.inv(psi.T @ phi)).max() < 1e-10       # library routine (LAPACK)
+
+
+def test_singular_overlap_flagged(c0):
+    psi = c0.psi[0]
+    phi = psi.astype(np.complex128).copy()
+    phi[:, 1] = phi[:, 0]
+    _, _, st = oracle.theta(psi, phi)
+    assert st == 1
+
+
+# ---------------------------------------------------------------- P7: degenerate cases
+def test_p7_single_orbital():
+    xyz, fns = gen.site_geometry(0)
+    P = gen.make_problem_from_geometry(xyz, fns, (1,), 40, seed=11)
+    phi = gen.make_walkers(P, 3)[0]
+    for w in range(3):
+        _, _, ej, ek = oracle.local_energy_exact(P.h, P.L, P.psi, [phi[w]], "cholesky")
+        assert abs(ek + ej / 2) <= 1e-12 * abs(ej)
+
+
+def test_p7_single_cholesky_vector():
+    xyz, fns = gen.site_geometry(0)
+    P = gen.make_problem_from_geometry(xyz, fns, (4,), 1, seed=12)
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, P.psi[0])
+    pi, pj = oracle.all_pairs(4)
+    Ut, s, Wt = oracle.full_svd_pairs(Lbar, pi, pj)
+    assert (s[:, 1] <= 1e-12 * s[:, 0]).all()                 # every Y^{ij} has rank <= 1
+    fs = oracle.truncate(P.N, 4, pi, pj, Ut, s, Wt, 0.5 * s[:, 0].min())
+    assert (fs.r == 1).all()
+    phi = gen.make_walkers(P, 2)
+    E, _ = oracle.local_energy_lo(P.psi, [Lbar], [hbar], [fs], phi)
+    for w in range(2):
+        e = oracle.local_energy_exact(P.h, P.L, P.psi, [phi[0][w]], "bruteforce")
+        assert abs(E[w, 3] - e[3]) <= 1e-12 * abs(e[3])
+
+
+# ---------------------------------------------------------------- P8: Eckart-Young, orthonormality, monotone ranks, bound
+def test_p8_eckart_young_and_bound(c1, c1_walkers):
+    psi = c1.psi[0]
+    O, N = psi.shape[1], c1.N
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, psi)
+    pi, pj = oracle.all_pairs(O)
+    Ut, s, Wt = oracle.full_svd_pairs(Lbar, pi, pj)
+    assert (np.diff(s, axis=1) <= 0).all()
+    for k in (0, 5, 100, len(pi) - 1):
+        assert np.abs(Ut[k] @ Ut[k].T - np.eye(N)).max() < 1e-12
+        assert np.abs(Wt[k] @ Wt[k].T - np.eye(N)).max() < 1e-12
+        Y = oracle.pair_eri(Lbar, pi[k], pj[k])
+        for r in (0, 3, N // 2, N):
+            err2 = np.linalg.norm(Y - (Ut[k, :r].T * s[k, :r]) @ Wt[k, :r]) ** 2
+            assert abs(err2 - (s[k, r:] ** 2).sum()) <= 1e-10 * (s[k] ** 2).sum()
+    ranks = [int((s > T).sum()) for T in (0.0, 1e-6, 1e-4, 1e-2, 1.0, 10.0)]
+    assert all(a >= b for a, b in zip(ranks, ranks[1:])) and ranks[0] > ranks[-1]
+    # truncation bound: |E_K^LO - E_K| <= sum_{i<=j} m_ij sigma_{r+1} |Theta_i| |Theta_j|
+    m = np.where(pi == pj, 1.0, 2.0)
+    for T in (1.0, 5.0):
+        fs = oracle.truncate(N, O, pi, pj, Ut, s, Wt, T)
+        assert 0 < fs.sum_rank < N * len(pi)
+        for w in range(2):
+            th, _, _ = oracle.theta(psi, c1_walkers[0][w])
+            nrm = np.linalg.norm(th, axis=0)
+            s_next = np.array([s[k, fs.r[k]] if fs.r[k] < N else 0.0 for k in range(len(pi))])
+            bound = (m * s_next * nrm[pi] * nrm[pj]).sum()
+            err = abs(oracle.exchange_lo(fs, th) - oracle.exchange_cholesky(Lbar, th))
+            assert 0 < err <= bound <= T * nrm.sum() ** 2
+
+
+# ---------------------------------------------------------------- P9: real walkers, unrestricted = closed shell
+def test_p9_real_walker_real_energy(c0):
+    phi = gen.make_walkers(c0, 2, real=True)
+    for route in ("bruteforce", "cholesky", "full_eri"):
+        e = oracle.local_energy_exact(c0.h, c0.L, c0.psi, [phi[0][0]], route)
+        assert all(x.imag == 0.0 for x in e)
+
+
+def test_p9_unrestricted_equals_closed_shell(c0, c0_walkers):
+    phi = c0_walkers[0][3]
+    for route in ("bruteforce", "cholesky", "full_eri"):
+        e_r = np.array(oracle.local_energy_exact(c0.h, c0.L, c0.psi, [phi], route))
+        e_u = np.array(oracle.local_energy_exact(c0.h, c0.L, [c0.psi[0], c0.psi[0]], [phi, phi], route))
+        assert np.abs(e_r - e_u).max() <= 1e-12 * np.abs(e_r).max()
+
+
+def test_o6_unrestricted_routes_agree():
+    xyz, fns = gen.site_geometry(0)
+    P = gen.make_problem_from_geometry(xyz, fns, (5, 3), 60, seed=21)
+    phis = gen.make_walkers(P, 3)
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+    fsets = [oracle.own_factors(a, 0.0) for a, _ in hr]
+    E, st = oracle.local_energy_lo(P.psi, [a for a, _ in hr], [b for _, b in hr], fsets, phis)
+    for w in range(3):
+        ph = [phis[0][w], phis[1][w]]
+        e_bf = np.array(oracle.local_energy_exact(P.h, P.L, P.psi, ph, "bruteforce"))
+        for route in ("cholesky", "full_eri"):
+            e = np.array(oracle.local_energy_exact(P.h, P.L, P.psi, ph, route))
+            assert np.abs(e - e_bf).max() <= 1e-11 * np.abs(e_bf).max()
+        assert np.abs(E[w] - e_bf).max() <= 1e-11 * np.abs(e_bf).max()
+
+
+# ---------------------------------------------------------------- P10: the Jacobi SVD itself
+def hilbert(n):
+    i = np.arange(n)
+    return 1.0 / (i[:, None] + i[None, :] + 1.0)
+
+
+def test_p10_svd_diagonal_and_rank1():
+    d = np.array([3.0, 0.5, 7.0, 1e-3, 2.0])
+    Ut, s, Wt = oracle.svd(np.diag(d))
+    assert np.allclose(s, np.sort(d)[::-1], rtol=1e-15)
+    u, v = np.arange(1.0, 7.0), np.array([1.0, -2.0, 0.5, 3.0, 0.0, 1.0])
+    Ut, s, Wt = oracle.svd(np.outer(u, v))
+    assert rel(s[0], np.linalg.norm(u) * np.linalg.norm(v)) < 1e-14 and (s[1:] < 1e-13).all()
+    assert np.abs(np.abs(Ut[0]) - u / np.linalg.norm(u)).max() < 1e-14
+    assert np.abs(np.abs(Wt[0]) - np.abs(v) / np.linalg.norm(v)).max() < 1e-14
+    Ut, s, Wt = oracle.svd(np.zeros((4, 4)))
+    assert (s == 0).all()
+
+
+@pytest.mark.parametrize("n", [3, 5, 8])
+def test_p10_svd_hilbert(n):
+    # Hilbert matrix: SPD, so singular values = eigenvalues; sum = trace = sum 1/(2i-1),
+    # product = det(H_n) = c_n^4 / c_{2n}, c_n = prod_{i<n} i!  (textbook closed forms)
+    H = hilbert(n)
+    Ut, s, Wt = oracle.svd(H)
+    assert rel(s.sum(), sum(1.0 / (2 * i + 1) for i in range(n))) < 1e-14
+    c = lambda m: math.prod(math.factorial(i) for i in range(1, m))
+    det = c(n) ** 4 / c(2 * n)
+    assert rel(np.prod(s), det) < 1e-12 * np.linalg.cond(H) ** 0.5
+    s_np = np.linalg.svd(H, compute_uv=False)
+    assert np.abs(s - s_np).max() <= 1e-15 * s[0] * n
+    assert (np.abs(s - s_np) <= 1e-10 * s_np + 4e-16 * s[0]).all()    # LAPACK's small sigmas are only abs-accurate
+    assert np.abs((Ut.T * s) @ Wt - H).max() < 1e-15 * n
+
+
+def test_p10_svd_vs_lapack_random_and_pair_block(c1):
+    rng = np.random.default_rng(0)
+    A = rng.standard_normal((40, 40)) * np.exp(-0.3 * np.arange(40))[None, :]
+    Lbar, _ = oracle.half_rotate(c1.L, c1.h, c1.psi[0])
+    for M in (A, oracle.pair_eri(Lbar, 2, 9)):
+        Ut, s, Wt = oracle.svd(M)
+        s_np = np.linalg.svd(M, compute_uv=False)
+        assert np.abs(s - s_np).max() <= 1e-13 * s_np[0]
+        assert np.abs((Ut.T * s) @ Wt - M).max() <= 1e-13 * s_np[0]
+        assert np.abs(Ut @ Ut.T - np.eye(len(s))).max() < 1e-12
+
+
+def test_pair_eri_symmetry_and_definition(c0):
+    Lbar, hbar = oracle.half_rotate(c0.L, c0.h, c0.psi[0])
+    assert np.abs(Lbar - np.einsum("gpq,qi->gip", c0.L, c0.psi[0])).max() < 1e-12
+    assert np.abs(hbar - c0.psi[0].T @ c0.h).max() < 1e-12
+    Y = oracle.pair_eri(Lbar, 1, 4)
+    assert np.abs(Y - oracle.pair_eri(Lbar, 4, 1).T).max() == 0.0                         # Y^{ji} = (Y^{ij})^T
+    assert np.abs(Y - np.einsum("gp,gq->pq", Lbar[:, 1], Lbar[:, 4])).max() < 1e-11
+
+
+# ---------------------------------------------------------------- D9: paper-literal compressed Coulomb
+def test_coulomb_lo_equals_cholesky_route_at_t0(c0, c0_walkers):
+    Lbar, hbar = oracle.half_rotate(c0.L, c0.h, c0.psi[0])
+    fs0 = oracle.own_factors(Lbar, 0.0)
+    th, _, _ = oracle.theta(c0.psi[0], c0_walkers[0][0])
+    _, ej = oracle.onebody_coulomb([Lbar], [hbar], [th])
+    assert abs(2 * oracle.coulomb_lo(fs0, th) - ej) <= 1e-11 * abs(ej)
+
+
+# ---------------------------------------------------------------- regression anchor (written by tests/golden/make_golden.py)
+def test_golden_c0_regression(c0, c0_walkers):
+    import os
+    ref = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "c0_exact_energies.txt"))
+    for w in range(c0.n_w):
+        e = exact(c0, c0_walkers, w, "cholesky")
+        got = np.array([x for z in e for x in (z.real, z.imag)])
+        assert np.abs(got - ref[w]).max() <= 1e-11 * np.abs(ref[w]).max()
