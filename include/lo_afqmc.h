@@ -1,0 +1,138 @@
+/* lo_afqmc.h -- C ABI of the B200-native LO-AFQMC local-energy library (liblo_afqmc.so).
+ *
+ * The library evaluates, for a batch of walkers, the phaseless-AFQMC local energy with a
+ * single-determinant trial (arxiv 2202.00832; citations are /root/reference/PAPER.md lines):
+ *
+ *   Theta_w = Phi_w (Psi^T Phi_w)^-1                                  Eq. 15
+ *   E1      = c1 sum_{i,p} hbar_ip Theta_pi                           Eq. 8 one-body part
+ *   X^g     = sum_{i,p} Lbar^g_ip Theta_pi ;  E_J = cJ sum_g (X^g)^2  Eq. 16 Coulomb part
+ *   E_K     = -cK sum_{i<=j} m_ij sum_{K<=r_ij} sigma_K (U^{ij T} Theta_j)_K (W^{ij} Theta_i)_K
+ *                                                                     Eq. 18, 19/22 exchange part
+ *   E_L     = E1 + E_J + E_K
+ *
+ * with Lbar^g_ip = sum_q L^g_pq Psi_qi, Y^{ij}_pq = sum_g Lbar^g_ip Lbar^g_jq
+ * = U sigma W truncated to the r_ij singular values > threshold (Eq. 18), m_ij = 1 (i=j) or 2 (i<j).
+ * Closed shell (n_spin=1): c1=2, cJ=2, cK=1.  Unrestricted (n_spin=2): c1=1, cJ=1/2 with X summed over both
+ * spins, cK=1/2 with same-spin pairs only (Eq. 10 with explicit spin sums).  Readings of the paper's silent
+ * points are listed in DESIGN.md.
+ *
+ * Conventions: all matrices row-major (C order); complex128 = two doubles (re, im) interleaved.
+ * "host" / "device" is stated for every pointer.  No call throws; every call returns a lo_status and
+ * lo_last_error() gives a thread-local message for the last failure.  The library never frees or keeps
+ * caller memory.  There is no CPU fallback: lo_local_energy* need a factor set built with device >= 0.
+ */
+#ifndef LO_AFQMC_H
+#define LO_AFQMC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lo_factors lo_factors; /* opaque; owns every host and device allocation it makes */
+
+typedef enum {
+    LO_OK = 0,
+    LO_EINVAL = 1,    /* bad shape / NULL / misaligned pointer / n_w > max_walkers: nothing was launched */
+    LO_ENOMEM = 2,    /* host or device allocation failed */
+    LO_ECUDA = 3,     /* a CUDA call failed, or the factor set has no device (built with device < 0) */
+    LO_ESINGULAR = 4, /* reserved (singular overlaps are per-walker data, see walker_status) */
+    LO_EINTERNAL = 5
+} lo_status;
+
+typedef struct {
+    int N, n_chol, n_spin, n_occ[2];
+    int N_pad;                       /* N rounded up to the K tile (16) */
+    long long n_pairs[2];            /* pairs i<=j per spin */
+    long long sum_rank[2];           /* sum of r_ij per spin (R of SURVEY 8d) */
+    long long sum_rank_padded;       /* rows of the packed factor arrays (ranks padded to x8) */
+    int max_rank, min_rank;
+    unsigned long long factor_bytes; /* device bytes of packed U, W, weights and the tile table */
+    unsigned long long lbar_bytes;   /* device bytes of the half-rotated Cholesky operand [Lbar; hbar] */
+    unsigned long long workspace_bytes;
+    double threshold;
+    int device, max_walkers;
+    int setup_on_gpu;                /* 1 when pair Gram + SVD ran on the device */
+    long long n_tiles;               /* row tiles of the exchange grouped GEMM */
+} lo_info;
+
+/* Kernel indices for lo_timing_get */
+enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_K_EXCHANGE = 4, LO_K_FINAL = 5, LO_K_COUNT = 6 };
+
+/* S0 setup (untimed, deterministic): half-rotation, per-pair Y^{ij}, SVD,
+ * truncation sigma_K > threshold (strict, absolute; Eq. 18), sorting pairs by rank, padding
+ * ranks to multiples of 8, packing and upload.
+ *   h      host [N][N] symmetric.         L      host [n_chol][N][N], every slice symmetric.
+ *   psi_a  host [N][n_occ[0]], orthonormal columns (real trial).   psi_b  host [N][n_occ[1]] or NULL if n_spin==1.
+ *   threshold >= 0 (T_SVD, same units as the integrals).
+ *   device >= 0: CUDA device that will hold the factor set and workspace for up to max_walkers walkers.
+ *   device <  0: host-only factor set (accessors work; lo_local_energy* return LO_ECUDA).
+ *   flags  bit 0 (LO_SETUP_GPU_SVD): run the half-rotation, pair Gram matrices and Jacobi SVDs on the device
+ *          (needs device >= 0); otherwise they run on the host with OpenMP.
+ * On success *out owns everything; release with lo_free. */
+#define LO_SETUP_GPU_SVD 1
+lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const double* h, const double* L,
+                   const double* psi_a, const double* psi_b, double threshold, int device, int max_walkers,
+                   unsigned flags, lo_factors** out);
+
+lo_status lo_info_get(const lo_factors* f, lo_info* info);
+
+/* r[k] = r_ij for the pairs of one spin in row-major i<=j order ((0,0),(0,1),...,(0,O-1),(1,1),...); host [n_pairs]. */
+lo_status lo_ranks(const lo_factors* f, int spin, int* r);
+
+/* Host copy of the factors of pair (i<=j) of one spin, so that a checker can evaluate on THIS factor set:
+ * U host [r][N] (row K = left singular vector over p), sigma host [r] (descending), W host [r][N]. Any may be NULL. */
+lo_status lo_factor_pair(const lo_factors* f, int spin, int i, int j, double* U, double* sigma, double* W);
+
+/* All factors of one spin in lo_ranks order, rows back to back: U,W host [sum_rank][N], sigma host [sum_rank]. */
+lo_status lo_factor_all(const lo_factors* f, int spin, double* U, double* sigma, double* W);
+
+/* New factor set with a looser threshold (>= the one f was built with): prefix truncation of every pair,
+ * re-sorted and re-packed; Lbar/hbar are shared by reference counting.  Used for threshold sweeps. */
+lo_status lo_retruncate(const lo_factors* f, double looser_threshold, lo_factors** out);
+
+/* S1-S5: local energies of n_w walkers.  Asynchronous on `stream`; allocates nothing; no host sync.
+ *   phi_a  device complex128 [n_w][N][n_occ[0]] (walker-major; columns = orbitals), 16-byte aligned.
+ *   phi_b  device complex128 [n_w][N][n_occ[1]] or NULL when n_spin==1.
+ *   E_L, E1, E_J, E_K  device complex128 [n_w]; E_L required, parts may be NULL.
+ *   walker_status  device int32 [n_w] or NULL; nonzero = singular overlap Psi^T Phi, that walker's energies are NaN.
+ *   stream  cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+lo_status lo_local_energy(const lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1,
+                          void* E_J, void* E_K, int* walker_status, void* stream);
+
+/* Same computation with HOST buffers: copies phi to the device, runs lo_local_energy, copies
+ * E[n_w][4] = {E_L, E1, E_J, E_K} (complex128) and status back, and synchronises.  Pinned host memory makes the
+ * copies asynchronous with respect to each other; pageable memory works too. */
+lo_status lo_local_energy_host(const lo_factors* f, int n_w, const void* phi_a_host, const void* phi_b_host,
+                               void* E_host, int* status_host, void* stream);
+
+/* X^g_w = sum_{ip} Lbar^g_ip Theta_pi of the last lo_local_energy call (the force-bias contraction of
+ * PAPER.md:34): device complex128 [n_chol][ld] with ld returned in *ld (walker index fastest).
+ * Valid until the next call on this factor set. */
+lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld);
+
+/* Theta of the last call, for tests: host complex128 [n_w][N][n_occ[spin]] (walker-major, same layout as phi). */
+lo_status lo_theta_host(const lo_factors* f, int spin, int n_w, void* theta_host);
+
+/* Per-kernel device timing: when enabled, every lo_local_energy call brackets each of its kernels with CUDA
+ * events on `stream`; lo_timing_get synchronises those events and returns the accumulated milliseconds and launch
+ * counts per kernel (LO_K_*), then resets them. */
+lo_status lo_timing_enable(lo_factors* f, int enable);
+lo_status lo_timing_get(lo_factors* f, double ms[LO_K_COUNT], long long launches[LO_K_COUNT]);
+
+/* Algorithmic FP64 flops of ONE walker's local energy on this factor set: per step S1..S4. */
+lo_status lo_flops_per_walker(const lo_factors* f, double flops[LO_K_COUNT]);
+
+/* In-run roofline denominators (microbenchmarks on `device`):
+ *   kind 0: FP64 tensor pipe, register-resident DMMA.8x8x4 loop  -> *value in TFLOP/s
+ *   kind 1: FP64 FMA pipe, register-resident DFMA loop           -> *value in TFLOP/s
+ *   kind 2: HBM stream copy (read+write bytes)                   -> *value in GB/s */
+lo_status lo_measure_peak(int device, int kind, double* value);
+
+void lo_free(lo_factors* f);
+const char* lo_last_error(void);
+const char* lo_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LO_AFQMC_H */

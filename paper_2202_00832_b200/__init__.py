@@ -1,0 +1,209 @@
+"""paper_2202_00832_b200 -- Python binding of liblo_afqmc.so (B200-native LO-AFQMC local energy).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the C ABI declared in
+include/lo_afqmc.h.  torch is used for device memory and streams.  There is no CPU fallback: if the
+library cannot be built or loaded, importing works but every call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+LO_SETUP_GPU_SVD = 1
+K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize")
+_STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 4: "LO_ESINGULAR", 5: "LO_EINTERNAL"}
+EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_local_energy",
+           "lo_local_energy_host", "lo_coulomb_x", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
+           "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
+
+
+class LoError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("%s: %s" % (_STATUS.get(status, status), msg))
+        self.status = status
+
+
+class LoInfo(C.Structure):
+    _fields_ = [("N", C.c_int), ("n_chol", C.c_int), ("n_spin", C.c_int), ("n_occ", C.c_int * 2), ("N_pad", C.c_int),
+                ("n_pairs", C.c_longlong * 2), ("sum_rank", C.c_longlong * 2), ("sum_rank_padded", C.c_longlong),
+                ("max_rank", C.c_int), ("min_rank", C.c_int), ("factor_bytes", C.c_ulonglong), ("lbar_bytes", C.c_ulonglong),
+                ("workspace_bytes", C.c_ulonglong), ("threshold", C.c_double), ("device", C.c_int), ("max_walkers", C.c_int),
+                ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong)]
+
+
+_lib = None
+
+
+def lib():
+    """Load (building first if needed) liblo_afqmc.so.  Raises if it cannot be built: there is no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, ci, cd = C.c_void_p, C.c_int, C.c_double
+        L.lo_setup.argtypes = [ci, ci, ci, C.POINTER(ci), vp, vp, vp, vp, cd, ci, ci, C.c_uint, C.POINTER(vp)]
+        L.lo_info_get.argtypes = [vp, C.POINTER(LoInfo)]
+        L.lo_ranks.argtypes = [vp, ci, vp]
+        L.lo_factor_pair.argtypes = [vp, ci, ci, ci, vp, vp, vp]
+        L.lo_factor_all.argtypes = [vp, ci, vp, vp, vp]
+        L.lo_retruncate.argtypes = [vp, cd, C.POINTER(vp)]
+        L.lo_local_energy.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.lo_local_energy_host.argtypes = [vp, ci, vp, vp, vp, vp, vp]
+        L.lo_coulomb_x.argtypes = [vp, C.POINTER(vp), C.POINTER(ci)]
+        L.lo_theta_host.argtypes = [vp, ci, ci, vp]
+        L.lo_timing_enable.argtypes = [vp, ci]
+        L.lo_timing_get.argtypes = [vp, C.POINTER(cd), C.POINTER(C.c_longlong)]
+        L.lo_flops_per_walker.argtypes = [vp, C.POINTER(cd)]
+        L.lo_measure_peak.argtypes = [ci, ci, C.POINTER(cd)]
+        L.lo_free.argtypes = [vp]
+        L.lo_free.restype = None
+        L.lo_last_error.restype = C.c_char_p
+        L.lo_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _check(st):
+    if st != 0:
+        raise LoError(st, lib().lo_last_error().decode())
+
+
+def _np(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def measure_peak(kind: str, device: int = 0) -> float:
+    """In-run roofline denominators: 'dmma' / 'dfma' in TFLOP/s, 'hbm' in GB/s."""
+    v = C.c_double(0)
+    _check(lib().lo_measure_peak(device, {"dmma": 0, "dfma": 1, "hbm": 2}[kind], C.byref(v)))
+    return v.value
+
+
+class Factors:
+    """Owner of a lo_factors handle (lo_setup ... lo_free)."""
+
+    def __init__(self, handle):
+        self._h = C.c_void_p(handle)
+
+    @classmethod
+    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False):
+        """lo_setup: h [N,N], L [n_chol,N,N], psis = [psi] (closed shell) or [psi_a, psi_b]; host numpy arrays."""
+        h, L = _np(h, np.float64), _np(L, np.float64)
+        psis = [_np(p, np.float64) for p in psis]
+        N, n_chol = h.shape[0], L.shape[0]
+        n_occ = (C.c_int * 2)(*([p.shape[1] for p in psis] + [0])[:2])
+        out = C.c_void_p()
+        st = lib().lo_setup(N, n_chol, len(psis), n_occ, h.ctypes.data, L.ctypes.data, psis[0].ctypes.data,
+                            psis[1].ctypes.data if len(psis) == 2 else None, float(threshold), int(device), int(max_walkers),
+                            LO_SETUP_GPU_SVD if gpu_svd else 0, C.byref(out))
+        _check(st)
+        return cls(out.value)
+
+    def free(self):
+        if self._h:
+            lib().lo_free(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+    def info(self) -> LoInfo:
+        info = LoInfo()
+        _check(lib().lo_info_get(self._h, C.byref(info)))
+        return info
+
+    def ranks(self, spin=0) -> np.ndarray:
+        r = np.zeros(self.info().n_pairs[spin], dtype=np.int32)
+        _check(lib().lo_ranks(self._h, spin, r.ctypes.data))
+        return r
+
+    def factor_pair(self, spin, i, j):
+        info = self.info()
+        O = info.n_occ[spin]
+        k = i * O - i * (i - 1) // 2 + (j - i)
+        r = int(self.ranks(spin)[k])
+        U, s, W = np.zeros((r, info.N)), np.zeros(r), np.zeros((r, info.N))
+        _check(lib().lo_factor_pair(self._h, spin, i, j, U.ctypes.data, s.ctypes.data, W.ctypes.data))
+        return U, s, W
+
+    def factor_all(self, spin=0):
+        info = self.info()
+        R = int(info.sum_rank[spin])
+        U, s, W = np.zeros((R, info.N)), np.zeros(R), np.zeros((R, info.N))
+        _check(lib().lo_factor_all(self._h, spin, U.ctypes.data, s.ctypes.data, W.ctypes.data))
+        return U, s, W
+
+    def retruncate(self, threshold) -> "Factors":
+        out = C.c_void_p()
+        _check(lib().lo_retruncate(self._h, float(threshold), C.byref(out)))
+        return Factors(out.value)
+
+    def local_energy(self, phis, parts=True, status=True, stream=None):
+        """lo_local_energy on torch CUDA tensors phis = [phi_a(, phi_b)], complex128 [n_w,N,O].  Asynchronous on the
+        current (or given) torch stream.  Returns (E_L, E1, E_J, E_K, status) torch tensors (None where not requested)."""
+        import torch
+        phis = [p if p.is_contiguous() else p.contiguous() for p in phis]
+        for p in phis:
+            if p.dtype != torch.complex128 or not p.is_cuda:
+                raise LoError(1, "phi must be a CUDA complex128 tensor")
+        n_w, dev = phis[0].shape[0], phis[0].device
+        s = torch.cuda.current_stream(dev) if stream is None else stream
+        E = torch.empty((4 if parts else 1, n_w), dtype=torch.complex128, device=dev)
+        st_t = torch.empty(n_w, dtype=torch.int32, device=dev) if status else None
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        _check(lib().lo_local_energy(self._h, n_w, ptr(phis[0]), ptr(phis[1]) if len(phis) == 2 else None, ptr(E[0]),
+                                     ptr(E[1]) if parts else None, ptr(E[2]) if parts else None, ptr(E[3]) if parts else None,
+                                     ptr(st_t), C.c_void_p(s.cuda_stream)))
+        return (E[0], E[1], E[2], E[3], st_t) if parts else (E[0], None, None, None, st_t)
+
+    def local_energy_host(self, phis_host, E_host=None, status_host=None, stream=None):
+        """lo_local_energy_host: numpy (or pinned torch CPU) complex128 inputs [n_w,N,O]; copies in, runs, copies
+        E [n_w,4] = (E_L,E1,E_J,E_K) and status back, synchronises."""
+        import torch
+        n_w = phis_host[0].shape[0]
+        if E_host is None:
+            E_host = np.empty((n_w, 4), dtype=np.complex128)
+        if status_host is None:
+            status_host = np.empty(n_w, dtype=np.int32)
+        dp = lambda a: C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(lib().lo_local_energy_host(self._h, n_w, dp(phis_host[0]), dp(phis_host[1]) if len(phis_host) == 2 else None,
+                                          dp(E_host), dp(status_host), C.c_void_p(s.cuda_stream)))
+        return E_host, status_host
+
+    def theta_host(self, spin, n_w) -> np.ndarray:
+        info = self.info()
+        th = np.empty((n_w, info.N, info.n_occ[spin]), dtype=np.complex128)
+        _check(lib().lo_theta_host(self._h, spin, n_w, th.ctypes.data))
+        return th
+
+    def coulomb_x(self):
+        """Device pointer and leading dimension of X[g][w] (complex128) from the last call."""
+        p, ld = C.c_void_p(), C.c_int()
+        _check(lib().lo_coulomb_x(self._h, C.byref(p), C.byref(ld)))
+        return p.value, ld.value
+
+    def timing_enable(self, on=True):
+        _check(lib().lo_timing_enable(self._h, 1 if on else 0))
+
+    def timing_get(self):
+        ms = (C.c_double * len(K_NAMES))()
+        n = (C.c_longlong * len(K_NAMES))()
+        _check(lib().lo_timing_get(self._h, ms, n))
+        return {k: (ms[i], n[i]) for i, k in enumerate(K_NAMES)}
+
+    def flops_per_walker(self):
+        fl = (C.c_double * len(K_NAMES))()
+        _check(lib().lo_flops_per_walker(self._h, fl))
+        return {k: fl[i] for i, k in enumerate(K_NAMES)}

@@ -1,0 +1,711 @@
+// lo_api.cu -- C ABI entry points of liblo_afqmc.so and the host side of lo_setup
+// (half-rotation PAPER.md:127, pair blocks PAPER.md:133, SVD + truncation Eq. 18, rank sort, padding, packing).
+#include <omp.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+#include "lo_internal.h"
+
+namespace lo {
+
+std::string& err_buf() {
+    static thread_local std::string s;
+    return s;
+}
+void set_error(const std::string& s) { err_buf() = s; }
+
+SharedOps::~SharedOps() {
+    if (device >= 0) {
+        cudaSetDevice(device);
+        if (dLbar) cudaFree(dLbar);
+        for (int s = 0; s < 2; ++s)
+            if (dPsi[s]) cudaFree(dPsi[s]);
+    }
+}
+
+namespace {
+
+#define CK(call)                                                                                          \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) {                                                                          \
+            set_error(std::string(#call) + ": " + cudaGetErrorString(e_));                                \
+            return (e_ == cudaErrorMemoryAllocation) ? LO_ENOMEM : LO_ECUDA;                              \
+        }                                                                                                 \
+    } while (0)
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// ---- host half-rotation: Lbar[g][o][p] = sum_q L[g][p][q] psi_s[q][i], hbar[o][p] = sum_q psi[q][i] h[q][p]  (row n_chol)
+void host_half_rotate(int N, int n_chol, int n_spin, const int* n_occ, const int* o_base, int O_tot, const double* h, const double* L,
+                      const double* const* psi, std::vector<double>& out) {
+    out.assign((size_t)(n_chol + 1) * O_tot * N, 0.0);
+#pragma omp parallel
+    {
+        std::vector<double> row(O_tot);
+#pragma omp for schedule(static)
+        for (int g = 0; g <= n_chol; ++g) {
+            const double* M = (g < n_chol) ? L + (size_t)g * N * N : h;
+            double* dst = out.data() + (size_t)g * O_tot * N;
+            for (int p = 0; p < N; ++p) {
+                std::fill(row.begin(), row.end(), 0.0);
+                const double* mp = M + (size_t)p * N;   // symmetric: row p == column p
+                for (int q = 0; q < N; ++q) {
+                    const double a = mp[q];
+                    for (int s = 0; s < n_spin; ++s) {
+                        const double* ps = psi[s] + (size_t)q * n_occ[s];
+                        double* r = row.data() + o_base[s];
+                        for (int i = 0; i < n_occ[s]; ++i) r[i] += a * ps[i];
+                    }
+                }
+                for (int o = 0; o < O_tot; ++o) dst[(size_t)o * N + p] = row[o];
+            }
+        }
+    }
+}
+
+// ---- host pair block: Y[q][p] layout chosen so that row q of `G` is COLUMN q of Y^{ij}:  G[q][p] = Y^{ij}_pq
+void host_pair_gram_t(int N, int n_chol, int O_tot, const double* Lbar, int oi, int oj, double* G) {
+    std::fill(G, G + (size_t)N * N, 0.0);
+    for (int g = 0; g < n_chol; ++g) {
+        const double* li = Lbar + ((size_t)g * O_tot + oi) * N;
+        const double* lj = Lbar + ((size_t)g * O_tot + oj) * N;
+        for (int q = 0; q < N; ++q) {
+            const double b = lj[q];
+            double* row = G + (size_t)q * N;
+            for (int p = 0; p < N; ++p) row[p] += b * li[p];
+        }
+    }
+}
+
+// ---- host one-sided Jacobi SVD (Hestenes) with round-robin (tournament) ordering.
+// In: G[q][:] = column q of Y (n vectors of length n).  Rotations orthogonalise the vectors; V accumulates them.
+// Out: order[] sorts the vectors by norm (descending); sigma[K] = |G[order[K]]|; U row K = G[order[K]]/sigma;
+//      W row K = V[order[K]]  (Y v_K = sigma_K u_K).
+void host_jacobi(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order) {
+    std::fill(V, V + (size_t)n * n, 0.0);
+    for (int c = 0; c < n; ++c) V[(size_t)c * n + c] = 1.0;
+    double fro2 = 0;
+    for (size_t k = 0; k < (size_t)n * n; ++k) fro2 += G[k] * G[k];
+    const double tiny2 = fro2 * 1e-30, tol = 1e-15;
+    const int m = n + (n & 1);   // players (one dummy if n is odd)
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        int rotations = 0;
+        for (int round = 0; round < m - 1; ++round) {
+            for (int k = 0; k < m / 2; ++k) {
+                int p, q;
+                if (k == 0) { p = m - 1; q = round; }
+                else { p = (round + k) % (m - 1); q = (round - k + (m - 1)) % (m - 1); }
+                if (p >= n || q >= n) continue;
+                if (p > q) std::swap(p, q);
+                double* gp = G + (size_t)p * n;
+                double* gq = G + (size_t)q * n;
+                double a = 0, b = 0, c = 0;
+                for (int e = 0; e < n; ++e) { a += gp[e] * gp[e]; b += gq[e] * gq[e]; c += gp[e] * gq[e]; }
+                if (a <= tiny2 || b <= tiny2) continue;
+                if (std::fabs(c) <= tol * std::sqrt(a * b)) continue;
+                ++rotations;
+                const double zeta = (b - a) / (2.0 * c);
+                const double t = (zeta >= 0 ? 1.0 : -1.0) / (std::fabs(zeta) + std::sqrt(1.0 + zeta * zeta));
+                const double cs = 1.0 / std::sqrt(1.0 + t * t), sn = cs * t;
+                for (int e = 0; e < n; ++e) {
+                    const double x = gp[e], y = gq[e];
+                    gp[e] = cs * x - sn * y;
+                    gq[e] = sn * x + cs * y;
+                }
+                double* vp = V + (size_t)p * n;
+                double* vq = V + (size_t)q * n;
+                for (int e = 0; e < n; ++e) {
+                    const double x = vp[e], y = vq[e];
+                    vp[e] = cs * x - sn * y;
+                    vq[e] = sn * x + cs * y;
+                }
+            }
+        }
+        if (rotations == 0) break;
+    }
+    std::vector<double> nrm(n);
+    for (int c = 0; c < n; ++c) {
+        double a = 0;
+        for (int e = 0; e < n; ++e) a += G[(size_t)c * n + e] * G[(size_t)c * n + e];
+        nrm[c] = std::sqrt(a);
+    }
+    order.resize(n);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return nrm[x] > nrm[y]; });
+    sigma.resize(n);
+    for (int K = 0; K < n; ++K) sigma[K] = nrm[order[K]];
+}
+
+struct PairRec {
+    int spin, i, j, r;
+    long long src;   // offset (rows) of this pair's kept rows in the staging arrays
+};
+
+// Sort pairs by rank (descending; ties by spin, i, j), assign padded row offsets, cut row tiles.
+void plan_layout(lo_factors* f, std::vector<PairRec>& pairs, std::vector<int>& sorted) {
+    sorted.resize(pairs.size());
+    std::iota(sorted.begin(), sorted.end(), 0);
+    std::stable_sort(sorted.begin(), sorted.end(), [&](int a, int b) { return pairs[a].r > pairs[b].r; });
+    for (int s = 0; s < f->n_spin; ++s) {
+        size_t np = (size_t)f->n_occ[s] * (f->n_occ[s] + 1) / 2;
+        f->rank[s].assign(np, 0);
+        f->row_off[s].assign(np, 0);
+    }
+    long long row = 0;
+    f->hTiles.clear();
+    for (int idx : sorted) {
+        const PairRec& pr = pairs[idx];
+        const int O = f->n_occ[pr.spin];
+        const size_t k = (size_t)pr.i * O - (size_t)pr.i * (pr.i - 1) / 2 + (pr.j - pr.i);
+        f->rank[pr.spin][k] = pr.r;
+        f->row_off[pr.spin][k] = row;
+        const int r_pad = round_up(pr.r, 8);
+        if (r_pad > 0) {
+            const int F = r_pad / 8, nt = (F + 7) / 8;
+            int done = 0;
+            for (int t = 0; t < nt; ++t) {
+                int nf = F / nt + (t < F % nt ? 1 : 0);
+                ExTile T;
+                T.row0 = (int)(row + (long long)done * 8);
+                T.nfrag = nf;
+                T.pi = f->o_base[pr.spin] + pr.i;
+                T.pj = f->o_base[pr.spin] + pr.j;
+                f->hTiles.push_back(T);
+                done += nf;
+            }
+        }
+        row += r_pad;
+    }
+    f->rows = row;
+    f->n_tiles = (long long)f->hTiles.size();
+}
+
+lo_status alloc_device(lo_factors* f) {
+    CK(cudaSetDevice(f->device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, f->device));
+    f->num_sms = prop.multiProcessorCount;
+    const size_t rows_alloc = (size_t)f->rows + EX_BM;
+    CK(cudaMalloc(&f->dU, rows_alloc * f->N_pad * 8));
+    CK(cudaMalloc(&f->dW, rows_alloc * f->N_pad * 8));
+    CK(cudaMalloc(&f->dWgt, rows_alloc * 8));
+    CK(cudaMalloc(&f->dTiles, std::max<size_t>(1, f->hTiles.size()) * sizeof(ExTile)));
+    CK(cudaMemset(f->dU, 0, rows_alloc * f->N_pad * 8));
+    CK(cudaMemset(f->dW, 0, rows_alloc * f->N_pad * 8));
+    CK(cudaMemset(f->dWgt, 0, rows_alloc * 8));
+    f->factor_bytes = 2 * rows_alloc * f->N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
+    return LO_OK;
+}
+
+lo_status alloc_workspace(lo_factors* f) {
+    CK(cudaSetDevice(f->device));
+    const size_t Wcap = f->Wcap, ldw = f->ldw;
+    size_t total = 0;
+    auto al = [&](void** p, size_t bytes) -> cudaError_t {
+        total += bytes;
+        cudaError_t e = cudaMalloc(p, bytes);
+        if (e == cudaSuccess) e = cudaMemset(*p, 0, bytes);
+        return e;
+    };
+    CK(al((void**)&f->dThT, (size_t)f->O_tot * ldw * f->N_pad * 8));
+    for (int s = 0; s < f->n_spin; ++s) {
+        CK(al((void**)&f->dA[s], Wcap * f->n_occ[s] * f->n_occ[s] * 16));
+        CK(al((void**)&f->dPhi[s], Wcap * f->N * f->n_occ[s] * 16));
+    }
+    CK(al((void**)&f->dXpart, (size_t)MAX_SPLIT * f->Xp * ldw * 8));
+    CK(al((void**)&f->dEJpart, (size_t)(f->Xp / CO_BM + 1) * Wcap * 16));
+    CK(al((void**)&f->dEKpart, (size_t)f->num_sms * Wcap * 16));
+    CK(al((void**)&f->dStatus, 2 * Wcap * 4));
+    CK(al((void**)&f->dEout, Wcap * 4 * 16));
+    CK(al((void**)&f->dStatusOut, Wcap * 4));
+    f->workspace_bytes = total;
+    return configure_kernels();
+}
+
+lo_status upload_lbar(lo_factors* f) {
+    SharedOps& ops = *f->ops;
+    CK(cudaSetDevice(f->device));
+    const size_t K = (size_t)f->O_tot * f->N_pad;
+    CK(cudaMalloc(&ops.dLbar, (size_t)f->Xp * K * 8));
+    CK(cudaMemset(ops.dLbar, 0, (size_t)f->Xp * K * 8));
+    // host [g][o][N] -> device [g][o][N_pad]
+    CK(cudaMemcpy2D(ops.dLbar, (size_t)f->N_pad * 8, ops.hLbar.data(), (size_t)f->N * 8, (size_t)f->N * 8,
+                    (size_t)(f->n_chol + 1) * f->O_tot, cudaMemcpyHostToDevice));
+    f->lbar_bytes = (size_t)f->Xp * K * 8;
+    return LO_OK;
+}
+
+void free_all(lo_factors* f) {
+    if (!f) return;
+    if (f->device >= 0) {
+        cudaSetDevice(f->device);
+        for (auto& ev : f->events) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
+        for (auto& ev : f->pool) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
+        void* ptrs[] = {f->dU, f->dW, f->dWgt, f->dTiles, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
+                        f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1]};
+        for (void* p : ptrs)
+            if (p) cudaFree(p);
+    }
+    delete f;
+}
+
+// common tail of lo_setup / lo_retruncate: staging rows (hUs/hWs/hSig in `pairs[].src` order, row pitch N) -> packed + upload
+lo_status pack_and_upload(lo_factors* f, std::vector<PairRec>& pairs, const std::vector<double>& sU, const std::vector<double>& sW,
+                          const std::vector<double>& sSig) {
+    std::vector<int> sorted;
+    plan_layout(f, pairs, sorted);
+    const size_t rows_alloc = (size_t)f->rows + EX_BM;
+    const double cK = f->n_spin == 1 ? 1.0 : 0.5;
+    const int N = f->N, N_pad = f->N_pad;
+    f->hU.assign(rows_alloc * N_pad, 0.0);
+    f->hW.assign(rows_alloc * N_pad, 0.0);
+    f->hWgt.assign(rows_alloc, 0.0);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (size_t x = 0; x < pairs.size(); ++x) {
+        const PairRec& pr = pairs[x];
+        const int O = f->n_occ[pr.spin];
+        const size_t k = (size_t)pr.i * O - (size_t)pr.i * (pr.i - 1) / 2 + (pr.j - pr.i);
+        const long long row0 = f->row_off[pr.spin][k];
+        const double m = pr.i == pr.j ? 1.0 : 2.0;
+        for (int K = 0; K < pr.r; ++K) {
+            std::memcpy(&f->hU[(size_t)(row0 + K) * N_pad], &sU[(size_t)(pr.src + K) * N], (size_t)N * 8);
+            std::memcpy(&f->hW[(size_t)(row0 + K) * N_pad], &sW[(size_t)(pr.src + K) * N], (size_t)N * 8);
+            f->hWgt[row0 + K] = -cK * m * sSig[pr.src + K];
+        }
+    }
+    if (f->device >= 0) {
+        lo_status st = alloc_device(f);
+        if (st != LO_OK) return st;
+        CK(cudaMemcpy(f->dU, f->hU.data(), rows_alloc * N_pad * 8, cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(f->dW, f->hW.data(), rows_alloc * N_pad * 8, cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(f->dWgt, f->hWgt.data(), rows_alloc * 8, cudaMemcpyHostToDevice));
+        if (!f->hTiles.empty())
+            CK(cudaMemcpy(f->dTiles, f->hTiles.data(), f->hTiles.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
+        std::vector<double>().swap(f->hU);
+        std::vector<double>().swap(f->hW);
+        st = alloc_workspace(f);
+        if (st != LO_OK) return st;
+    } else {
+        f->factor_bytes = 2 * rows_alloc * N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
+    }
+    return LO_OK;
+}
+
+// fetch packed rows [row0,row0+r) of U or W to a host buffer with pitch N
+lo_status fetch_rows(const lo_factors* f, bool isU, long long row0, int r, double* dst) {
+    if (r <= 0) return LO_OK;
+    if (f->device >= 0) {
+        CK(cudaSetDevice(f->device));
+        const double* src = (isU ? f->dU : f->dW) + (size_t)row0 * f->N_pad;
+        CK(cudaMemcpy2D(dst, (size_t)f->N * 8, src, (size_t)f->N_pad * 8, (size_t)f->N * 8, (size_t)r, cudaMemcpyDeviceToHost));
+    } else {
+        const std::vector<double>& v = isU ? f->hU : f->hW;
+        for (int K = 0; K < r; ++K) std::memcpy(dst + (size_t)K * f->N, &v[(size_t)(row0 + K) * f->N_pad], (size_t)f->N * 8);
+    }
+    return LO_OK;
+}
+
+}  // namespace
+}  // namespace lo
+
+using namespace lo;
+
+extern "C" {
+
+const char* lo_last_error(void) { return err_buf().c_str(); }
+const char* lo_version(void) { return "lo_afqmc_b200 0.1 (sm_100a)"; }
+
+lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const double* h, const double* L, const double* psi_a,
+                   const double* psi_b, double threshold, int device, int max_walkers, unsigned flags, lo_factors** out) {
+    if (!out) { set_error("lo_setup: out is NULL"); return LO_EINVAL; }
+    *out = nullptr;
+    if (N <= 0 || n_chol <= 0 || (n_spin != 1 && n_spin != 2) || !n_occ || !h || !L || !psi_a || (n_spin == 2 && !psi_b) ||
+        !(threshold >= 0.0) || max_walkers <= 0) {
+        set_error("lo_setup: invalid argument (shape, NULL pointer, negative threshold or max_walkers <= 0)");
+        return LO_EINVAL;
+    }
+    for (int s = 0; s < n_spin; ++s)
+        if (n_occ[s] <= 0 || n_occ[s] > N) { set_error("lo_setup: n_occ out of range"); return LO_EINVAL; }
+    if ((flags & LO_SETUP_GPU_SVD) && device < 0) { set_error("lo_setup: LO_SETUP_GPU_SVD needs device >= 0"); return LO_EINVAL; }
+
+    lo_factors* f = new (std::nothrow) lo_factors();
+    if (!f) { set_error("lo_setup: out of host memory"); return LO_ENOMEM; }
+    f->N = N; f->N_pad = round_up(N, KTILE); f->n_chol = n_chol; f->Xp = round_up(n_chol + 1, CO_BM);
+    f->n_spin = n_spin; f->threshold = threshold; f->device = device; f->max_walkers = max_walkers;
+    f->Wcap = round_up(max_walkers, WALKER_TILE); f->ldw = 2 * f->Wcap;
+    for (int s = 0; s < n_spin; ++s) { f->n_occ[s] = n_occ[s]; f->o_base[s] = f->O_tot; f->O_tot += n_occ[s]; }
+    f->ops = std::make_shared<SharedOps>();
+    f->ops->device = device;
+    const double* psi[2] = {psi_a, psi_b};
+    lo_status st = LO_OK;
+    try {
+        if (device >= 0) {
+            cudaError_t e = cudaSetDevice(device);
+            if (e != cudaSuccess) { set_error(std::string("cudaSetDevice: ") + cudaGetErrorString(e)); free_all(f); return LO_ECUDA; }
+            cudaDeviceProp prop;
+            cudaGetDeviceProperties(&prop, device);
+            f->num_sms = prop.multiProcessorCount;
+            for (int s = 0; s < n_spin; ++s) {
+                size_t b = (size_t)N * n_occ[s] * 8;
+                if (cudaMalloc(&f->ops->dPsi[s], b) != cudaSuccess || cudaMemcpy(f->ops->dPsi[s], psi[s], b, cudaMemcpyHostToDevice) != cudaSuccess) {
+                    set_error("lo_setup: cannot upload psi"); free_all(f); return LO_ECUDA;
+                }
+            }
+        }
+        // ---- half rotation (always kept on the host as well: lo_retruncate / accessors / host-only sets)
+        host_half_rotate(N, n_chol, n_spin, f->n_occ, f->o_base, f->O_tot, h, L, psi, f->ops->hLbar);
+        if (device >= 0) {
+            st = upload_lbar(f);
+            if (st != LO_OK) { free_all(f); return st; }
+        }
+        // ---- per-pair SVD + truncation
+        std::vector<PairRec> pairs;
+        for (int s = 0; s < n_spin; ++s)
+            for (int i = 0; i < n_occ[s]; ++i)
+                for (int j = i; j < n_occ[s]; ++j) pairs.push_back({s, i, j, 0, 0});
+        const size_t np = pairs.size();
+        std::vector<std::vector<double>> pU(np), pW(np), pS(np);
+        std::vector<double> snext(np, 0.0);
+        if (flags & LO_SETUP_GPU_SVD) {
+            f->setup_on_gpu = 1;
+            // batches of pairs on the device
+            const size_t per_pair = gpu_pair_svd_bytes_per_pair(N, f->N_pad);
+            size_t free_b = 0, total_b = 0;
+            cudaMemGetInfo(&free_b, &total_b);
+            size_t B = std::max<size_t>(1, std::min<size_t>({np, (size_t)(f->num_sms * 4), (free_b / 4) / per_pair}));
+            double *tY = nullptr, *tV = nullptr, *tU = nullptr, *tW = nullptr, *dSig = nullptr;
+            int* dOrd = nullptr;
+            const size_t mat = (size_t)N * f->N_pad * 8;
+            if (cudaMalloc(&tY, B * mat) != cudaSuccess || cudaMalloc(&tV, B * mat) != cudaSuccess || cudaMalloc(&tU, B * mat) != cudaSuccess ||
+                cudaMalloc(&tW, B * mat) != cudaSuccess || cudaMalloc(&dSig, B * N * 8) != cudaSuccess || cudaMalloc(&dOrd, B * N * 4) != cudaSuccess) {
+                set_error("lo_setup: cannot allocate GPU SVD workspace"); free_all(f); return LO_ENOMEM;
+            }
+            std::vector<double> hSig(B * N), hRow((size_t)N * f->N_pad);
+            std::vector<int> bi(B), bj(B);
+            for (size_t k0 = 0; k0 < np && st == LO_OK;) {
+                const int spin = pairs[k0].spin;
+                size_t k1 = k0;
+                while (k1 < np && k1 - k0 < B && pairs[k1].spin == spin) ++k1;
+                const int n = (int)(k1 - k0);
+                for (int x = 0; x < n; ++x) { bi[x] = pairs[k0 + x].i; bj[x] = pairs[k0 + x].j; }
+                st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data());
+                if (st != LO_OK) break;
+                for (int x = 0; x < n; ++x) {
+                    const double* sg = &hSig[(size_t)x * N];
+                    int r = 0;
+                    while (r < N && sg[r] > threshold) ++r;
+                    pairs[k0 + x].r = r;
+                    snext[k0 + x] = r < N ? sg[r] : 0.0;
+                    pS[k0 + x].assign(sg, sg + r);
+                    pU[k0 + x].resize((size_t)r * N);
+                    pW[k0 + x].resize((size_t)r * N);
+                    if (r > 0) {
+                        cudaMemcpy2D(pU[k0 + x].data(), (size_t)N * 8, tU + (size_t)x * N * f->N_pad, (size_t)f->N_pad * 8, (size_t)N * 8, r,
+                                     cudaMemcpyDeviceToHost);
+                        cudaMemcpy2D(pW[k0 + x].data(), (size_t)N * 8, tW + (size_t)x * N * f->N_pad, (size_t)f->N_pad * 8, (size_t)N * 8, r,
+                                     cudaMemcpyDeviceToHost);
+                    }
+                }
+                k0 = k1;
+            }
+            cudaFree(tY); cudaFree(tV); cudaFree(tU); cudaFree(tW); cudaFree(dSig); cudaFree(dOrd);
+            if (st != LO_OK) { free_all(f); return st; }
+        } else {
+            const double* Lbar = f->ops->hLbar.data();
+#pragma omp parallel
+            {
+                std::vector<double> G((size_t)N * N), V((size_t)N * N), sg;
+                std::vector<int> order;
+#pragma omp for schedule(dynamic, 1)
+                for (long long x = 0; x < (long long)np; ++x) {
+                    PairRec& pr = pairs[x];
+                    host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[pr.spin] + pr.i, f->o_base[pr.spin] + pr.j, G.data());
+                    host_jacobi(N, G.data(), V.data(), sg, order);
+                    int r = 0;
+                    while (r < N && sg[r] > threshold) ++r;
+                    pr.r = r;
+                    snext[x] = r < N ? sg[r] : 0.0;
+                    pS[x].assign(sg.begin(), sg.begin() + r);
+                    pU[x].resize((size_t)r * N);
+                    pW[x].resize((size_t)r * N);
+                    for (int K = 0; K < r; ++K) {
+                        const double* g = &G[(size_t)order[K] * N];
+                        const double inv = 1.0 / sg[K];
+                        for (int e = 0; e < N; ++e) pU[x][(size_t)K * N + e] = g[e] * inv;
+                        std::memcpy(&pW[x][(size_t)K * N], &V[(size_t)order[K] * N], (size_t)N * 8);
+                    }
+                }
+            }
+        }
+        // ---- staging in natural order
+        long long src = 0;
+        for (size_t x = 0; x < np; ++x) { pairs[x].src = src; src += pairs[x].r; }
+        std::vector<double> sU((size_t)src * N), sW((size_t)src * N), sS((size_t)src);
+        for (size_t x = 0; x < np; ++x) {
+            if (pairs[x].r == 0) continue;
+            std::memcpy(&sU[(size_t)pairs[x].src * N], pU[x].data(), pU[x].size() * 8);
+            std::memcpy(&sW[(size_t)pairs[x].src * N], pW[x].data(), pW[x].size() * 8);
+            std::memcpy(&sS[(size_t)pairs[x].src], pS[x].data(), pS[x].size() * 8);
+            std::vector<double>().swap(pU[x]);
+            std::vector<double>().swap(pW[x]);
+        }
+        st = pack_and_upload(f, pairs, sU, sW, sS);
+        if (st != LO_OK) { free_all(f); return st; }
+        size_t off = 0;
+        for (int s = 0; s < n_spin; ++s) {
+            size_t cnt = (size_t)n_occ[s] * (n_occ[s] + 1) / 2;
+            f->sigma_next[s].assign(snext.begin() + off, snext.begin() + off + cnt);
+            off += cnt;
+        }
+    } catch (const std::bad_alloc&) {
+        set_error("lo_setup: out of host memory");
+        free_all(f);
+        return LO_ENOMEM;
+    }
+    *out = f;
+    return LO_OK;
+}
+
+lo_status lo_info_get(const lo_factors* f, lo_info* info) {
+    if (!f || !info) { set_error("lo_info_get: NULL argument"); return LO_EINVAL; }
+    std::memset(info, 0, sizeof(*info));
+    info->N = f->N; info->n_chol = f->n_chol; info->n_spin = f->n_spin; info->N_pad = f->N_pad;
+    int mx = 0, mn = f->N;
+    for (int s = 0; s < f->n_spin; ++s) {
+        info->n_occ[s] = f->n_occ[s];
+        info->n_pairs[s] = (long long)f->rank[s].size();
+        long long sum = 0;
+        for (int r : f->rank[s]) { sum += r; mx = std::max(mx, r); mn = std::min(mn, r); }
+        info->sum_rank[s] = sum;
+    }
+    info->sum_rank_padded = f->rows; info->max_rank = mx; info->min_rank = mn;
+    info->factor_bytes = f->factor_bytes; info->lbar_bytes = f->lbar_bytes; info->workspace_bytes = f->workspace_bytes;
+    info->threshold = f->threshold; info->device = f->device; info->max_walkers = f->max_walkers;
+    info->setup_on_gpu = f->setup_on_gpu; info->n_tiles = f->n_tiles;
+    return LO_OK;
+}
+
+lo_status lo_ranks(const lo_factors* f, int spin, int* r) {
+    if (!f || !r || spin < 0 || spin >= f->n_spin) { set_error("lo_ranks: invalid argument"); return LO_EINVAL; }
+    std::copy(f->rank[spin].begin(), f->rank[spin].end(), r);
+    return LO_OK;
+}
+
+lo_status lo_factor_pair(const lo_factors* f, int spin, int i, int j, double* U, double* sigma, double* W) {
+    if (!f || spin < 0 || spin >= f->n_spin || i < 0 || j < i || j >= f->n_occ[spin]) { set_error("lo_factor_pair: invalid argument"); return LO_EINVAL; }
+    const int O = f->n_occ[spin];
+    const size_t k = (size_t)i * O - (size_t)i * (i - 1) / 2 + (j - i);
+    const int r = f->rank[spin][k];
+    const long long row0 = f->row_off[spin][k];
+    lo_status st;
+    if (U && (st = fetch_rows(f, true, row0, r, U)) != LO_OK) return st;
+    if (W && (st = fetch_rows(f, false, row0, r, W)) != LO_OK) return st;
+    if (sigma && r > 0) {
+        std::vector<double> w(r);
+        if (f->device >= 0) {
+            CK(cudaSetDevice(f->device));
+            CK(cudaMemcpy(w.data(), f->dWgt + row0, (size_t)r * 8, cudaMemcpyDeviceToHost));
+        } else {
+            std::copy(f->hWgt.begin() + row0, f->hWgt.begin() + row0 + r, w.begin());
+        }
+        const double scale = -(f->n_spin == 1 ? 1.0 : 0.5) * (i == j ? 1.0 : 2.0);   // power of two: exact
+        for (int K = 0; K < r; ++K) sigma[K] = w[K] / scale;
+    }
+    return LO_OK;
+}
+
+lo_status lo_factor_all(const lo_factors* f, int spin, double* U, double* sigma, double* W) {
+    if (!f || spin < 0 || spin >= f->n_spin) { set_error("lo_factor_all: invalid argument"); return LO_EINVAL; }
+    const int O = f->n_occ[spin];
+    size_t off = 0, k = 0;
+    for (int i = 0; i < O; ++i)
+        for (int j = i; j < O; ++j, ++k) {
+            lo_status st = lo_factor_pair(f, spin, i, j, U ? U + off * f->N : nullptr, sigma ? sigma + off : nullptr, W ? W + off * f->N : nullptr);
+            if (st != LO_OK) return st;
+            off += f->rank[spin][k];
+        }
+    return LO_OK;
+}
+
+lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
+    if (!f || !out || !(looser >= f->threshold)) { set_error("lo_retruncate: invalid argument (threshold must be >= the original)"); return LO_EINVAL; }
+    *out = nullptr;
+    lo_factors* g = new (std::nothrow) lo_factors();
+    if (!g) { set_error("lo_retruncate: out of host memory"); return LO_ENOMEM; }
+    g->N = f->N; g->N_pad = f->N_pad; g->n_chol = f->n_chol; g->Xp = f->Xp; g->n_spin = f->n_spin; g->O_tot = f->O_tot;
+    for (int s = 0; s < 2; ++s) { g->n_occ[s] = f->n_occ[s]; g->o_base[s] = f->o_base[s]; }
+    g->threshold = looser; g->device = f->device; g->max_walkers = f->max_walkers; g->Wcap = f->Wcap; g->ldw = f->ldw;
+    g->num_sms = f->num_sms; g->setup_on_gpu = f->setup_on_gpu; g->ops = f->ops; g->lbar_bytes = f->lbar_bytes;
+    try {
+        std::vector<PairRec> pairs;
+        std::vector<double> snext;
+        long long src = 0;
+        std::vector<std::vector<double>> sig;
+        for (int s = 0; s < f->n_spin; ++s) {
+            const int O = f->n_occ[s];
+            size_t k = 0;
+            for (int i = 0; i < O; ++i)
+                for (int j = i; j < O; ++j, ++k) {
+                    const int r0 = f->rank[s][k];
+                    std::vector<double> sg(r0);
+                    lo_status st = lo_factor_pair(f, s, i, j, nullptr, sg.data(), nullptr);
+                    if (st != LO_OK) { free_all(g); return st; }
+                    int r = 0;
+                    while (r < r0 && sg[r] > looser) ++r;
+                    pairs.push_back({s, i, j, r, src});
+                    snext.push_back(r < r0 ? sg[r] : f->sigma_next[s][k]);
+                    src += r;
+                    sg.resize(r);
+                    sig.push_back(std::move(sg));
+                }
+        }
+        std::vector<double> sU((size_t)src * f->N), sW((size_t)src * f->N), sS((size_t)src);
+        for (size_t x = 0; x < pairs.size(); ++x) {
+            const PairRec& pr = pairs[x];
+            if (pr.r == 0) continue;
+            const int O = f->n_occ[pr.spin];
+            const size_t k = (size_t)pr.i * O - (size_t)pr.i * (pr.i - 1) / 2 + (pr.j - pr.i);
+            lo_status st = fetch_rows(f, true, f->row_off[pr.spin][k], pr.r, &sU[(size_t)pr.src * f->N]);
+            if (st == LO_OK) st = fetch_rows(f, false, f->row_off[pr.spin][k], pr.r, &sW[(size_t)pr.src * f->N]);
+            if (st != LO_OK) { free_all(g); return st; }
+            std::copy(sig[x].begin(), sig[x].end(), sS.begin() + pr.src);
+        }
+        lo_status st = pack_and_upload(g, pairs, sU, sW, sS);
+        if (st != LO_OK) { free_all(g); return st; }
+        size_t off = 0;
+        for (int s = 0; s < f->n_spin; ++s) {
+            size_t cnt = f->rank[s].size();
+            g->sigma_next[s].assign(snext.begin() + off, snext.begin() + off + cnt);
+            off += cnt;
+        }
+    } catch (const std::bad_alloc&) {
+        set_error("lo_retruncate: out of host memory");
+        free_all(g);
+        return LO_ENOMEM;
+    }
+    *out = g;
+    return LO_OK;
+}
+
+static lo_status check_call(const lo_factors* f, int n_w, const void* phi_a, const void* phi_b) {
+    if (!f) { set_error("lo_local_energy: factors is NULL"); return LO_EINVAL; }
+    if (f->device < 0) { set_error("lo_local_energy: factor set was built without a device (device < 0); there is no CPU path"); return LO_ECUDA; }
+    if (n_w <= 0 || n_w > f->max_walkers) { set_error("lo_local_energy: n_w out of range (1..max_walkers)"); return LO_EINVAL; }
+    if (!phi_a || (f->n_spin == 2 && !phi_b)) { set_error("lo_local_energy: phi is NULL"); return LO_EINVAL; }
+    if (((uintptr_t)phi_a & 15) || ((uintptr_t)phi_b & 15)) { set_error("lo_local_energy: phi must be 16-byte aligned"); return LO_EINVAL; }
+    return LO_OK;
+}
+
+lo_status lo_local_energy(const lo_factors* fc, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
+                          int* walker_status, void* stream) {
+    lo_status st = check_call(fc, n_w, phi_a, phi_b);
+    if (st != LO_OK) return st;
+    if (!E_L) { set_error("lo_local_energy: E_L is NULL"); return LO_EINVAL; }
+    if (((uintptr_t)E_L & 15) || ((uintptr_t)E1 & 15) || ((uintptr_t)E_J & 15) || ((uintptr_t)E_K & 15)) {
+        set_error("lo_local_energy: outputs must be 16-byte aligned");
+        return LO_EINVAL;
+    }
+    lo_factors* f = const_cast<lo_factors*>(fc);
+    CK(cudaSetDevice(f->device));
+    return launch_local_energy(f, n_w, phi_a, phi_b, E_L, E1, E_J, E_K, walker_status, nullptr, (cudaStream_t)stream);
+}
+
+lo_status lo_local_energy_host(const lo_factors* fc, int n_w, const void* phi_a_host, const void* phi_b_host, void* E_host, int* status_host,
+                               void* stream) {
+    lo_status st = check_call(fc, n_w, phi_a_host, phi_b_host);
+    if (st != LO_OK) return st;
+    if (!E_host) { set_error("lo_local_energy_host: E_host is NULL"); return LO_EINVAL; }
+    lo_factors* f = const_cast<lo_factors*>(fc);
+    cudaStream_t s = (cudaStream_t)stream;
+    CK(cudaSetDevice(f->device));
+    const void* ph[2] = {phi_a_host, phi_b_host};
+    for (int sp = 0; sp < f->n_spin; ++sp)
+        CK(cudaMemcpyAsync(f->dPhi[sp], ph[sp], (size_t)n_w * f->N * f->n_occ[sp] * 16, cudaMemcpyHostToDevice, s));
+    st = launch_local_energy(f, n_w, f->dPhi[0], f->dPhi[1], nullptr, nullptr, nullptr, nullptr, f->dStatusOut, f->dEout, s);
+    if (st != LO_OK) return st;
+    CK(cudaMemcpyAsync(E_host, f->dEout, (size_t)n_w * 4 * 16, cudaMemcpyDeviceToHost, s));
+    if (status_host) CK(cudaMemcpyAsync(status_host, f->dStatusOut, (size_t)n_w * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    return LO_OK;
+}
+
+lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld) {
+    if (!f || !X_dev || !ld) { set_error("lo_coulomb_x: NULL argument"); return LO_EINVAL; }
+    if (f->device < 0) { set_error("lo_coulomb_x: no device"); return LO_ECUDA; }
+    *X_dev = f->dXpart;
+    *ld = f->Wcap;
+    return LO_OK;
+}
+
+lo_status lo_theta_host(const lo_factors* f, int spin, int n_w, void* theta_host) {
+    if (!f || !theta_host || spin < 0 || spin >= f->n_spin || n_w <= 0 || n_w > f->max_walkers) { set_error("lo_theta_host: invalid argument"); return LO_EINVAL; }
+    if (f->device < 0) { set_error("lo_theta_host: no device"); return LO_ECUDA; }
+    CK(cudaSetDevice(f->device));
+    CK(cudaDeviceSynchronize());
+    const int O = f->n_occ[spin], N = f->N, N_pad = f->N_pad;
+    std::vector<double> panel((size_t)2 * n_w * N_pad);
+    double* out = static_cast<double*>(theta_host);
+    for (int i = 0; i < O; ++i) {
+        CK(cudaMemcpy(panel.data(), f->dThT + (size_t)(f->o_base[spin] + i) * f->ldw * N_pad, panel.size() * 8, cudaMemcpyDeviceToHost));
+        for (int w = 0; w < n_w; ++w)
+            for (int p = 0; p < N; ++p) {
+                out[(((size_t)w * N + p) * O + i) * 2] = panel[(size_t)(2 * w) * N_pad + p];
+                out[(((size_t)w * N + p) * O + i) * 2 + 1] = panel[(size_t)(2 * w + 1) * N_pad + p];
+            }
+    }
+    return LO_OK;
+}
+
+lo_status lo_timing_enable(lo_factors* f, int enable) {
+    if (!f) { set_error("lo_timing_enable: NULL"); return LO_EINVAL; }
+    f->timing = enable != 0;
+    return LO_OK;
+}
+
+lo_status lo_timing_get(lo_factors* f, double ms[LO_K_COUNT], long long launches[LO_K_COUNT]) {
+    if (!f || !ms || !launches) { set_error("lo_timing_get: NULL"); return LO_EINVAL; }
+    if (f->device >= 0) {
+        CK(cudaSetDevice(f->device));
+        for (auto& ev : f->events) {
+            CK(cudaEventSynchronize(ev.e1));
+            float t = 0;
+            CK(cudaEventElapsedTime(&t, ev.e0, ev.e1));
+            f->t_ms[ev.kind] += t;
+            f->t_n[ev.kind] += 1;
+            f->pool.push_back(ev);
+        }
+        f->events.clear();
+    }
+    for (int k = 0; k < LO_K_COUNT; ++k) { ms[k] = f->t_ms[k]; launches[k] = f->t_n[k]; f->t_ms[k] = 0; f->t_n[k] = 0; }
+    return LO_OK;
+}
+
+lo_status lo_flops_per_walker(const lo_factors* f, double fl[LO_K_COUNT]) {
+    if (!f || !fl) { set_error("lo_flops_per_walker: NULL"); return LO_EINVAL; }
+    for (int k = 0; k < LO_K_COUNT; ++k) fl[k] = 0;
+    const double N = f->N;
+    double R = 0;
+    for (int s = 0; s < f->n_spin; ++s) {
+        const double O = f->n_occ[s];
+        fl[LO_K_OVERLAP] += 4.0 * N * O * O;            // real x complex
+        fl[LO_K_INVERSE] += 8.0 * O * O * O;            // Gauss-Jordan, complex
+        fl[LO_K_THETA] += 8.0 * N * O * O;              // complex x complex
+        for (int r : f->rank[s]) R += r;
+    }
+    fl[LO_K_COULOMB] = 4.0 * (f->n_chol + 1.0) * N * f->O_tot;   // real x complex, incl. the hbar row (S2)
+    fl[LO_K_EXCHANGE] = 8.0 * N * R + 8.0 * R;                   // two real x complex GEMMs + weighted complex dot
+    return LO_OK;
+}
+
+lo_status lo_measure_peak(int device, int kind, double* value) {
+    if (!value) { set_error("lo_measure_peak: NULL"); return LO_EINVAL; }
+    return measure_peak(device, kind, value);
+}
+
+void lo_free(lo_factors* f) { free_all(f); }
+
+}  // extern "C"

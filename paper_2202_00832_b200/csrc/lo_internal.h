@@ -1,0 +1,109 @@
+// lo_internal.h -- internal definitions of liblo_afqmc.so (not part of the C ABI).
+// Data layout in HBM:
+//   thT   [O_tot][ldw][N_pad] f64   Theta^T: orbital panel o, column c = 2*w + {0:re,1:im}, basis index p fastest.
+//                                   ldw = 2*Wcap, Wcap = max_walkers rounded up to 64; rows p>=N and walkers >= n_w are 0.
+//   LbarD [Xp][O_tot][N_pad]  f64   rows g<n_chol: Lbar^g_ip; row n_chol: hbar; rest 0.  Xp = ceil128(n_chol+1).
+//   U, W  [rows][N_pad]       f64   packed factor rows of all pairs, pairs sorted by rank (descending), every pair
+//                                   padded to a multiple of 8 rows; 64 slack rows at the end.
+//   wgt   [rows]              f64   -cK * m_ij * sigma_K  (0 on padding rows).
+//   tiles [n_tiles]                 row tiles of the grouped GEMM: {row0, nfrag (valid 8-row fragments, 1..8), pi, pj}.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "../../include/lo_afqmc.h"
+
+namespace lo {
+
+constexpr int KTILE = 16;        // K tile (basis index p) of both GEMMs, in doubles
+constexpr int WALKER_TILE = 64;  // walkers per column block (128 real columns)
+constexpr int EX_BM = 64;        // rows (singular vectors) per exchange tile
+constexpr int CO_BM = 128;       // rows (Cholesky vectors) per Coulomb tile
+constexpr int MAX_SPLIT = 8;     // split-K partial buffers of the Coulomb GEMM
+
+struct ExTile {
+    int row0;   // first packed row of the tile
+    int nfrag;  // valid 8-row fragments in the tile (1..8)
+    int pi;     // Theta panel (global orbital index) contracted with W  (orbital i)
+    int pj;     // Theta panel contracted with U                         (orbital j)
+};
+
+void set_error(const std::string& s);
+std::string& err_buf();
+
+// Device-resident operands shared between a factor set and its re-truncations.
+struct SharedOps {
+    int device = -1;
+    double* dLbar = nullptr;      // [Xp][O_tot][N_pad]
+    double* dPsi[2] = {nullptr, nullptr};  // [N][O_s]
+    std::vector<double> hLbar;    // host copy [n_chol][O_tot][N] (+ hbar as row n_chol), kept for host-only sets / retruncate on host
+    ~SharedOps();
+};
+
+struct TimingEvent {
+    cudaEvent_t e0, e1;
+    int kind;
+};
+
+}  // namespace lo
+
+struct lo_factors {
+    int N = 0, N_pad = 0, n_chol = 0, Xp = 0, n_spin = 0, n_occ[2] = {0, 0}, O_tot = 0, o_base[2] = {0, 0};
+    double threshold = 0;
+    int device = -1, max_walkers = 0, Wcap = 0, ldw = 0, num_sms = 0;
+    int setup_on_gpu = 0;
+    // pair bookkeeping, natural (row-major i<=j) order per spin
+    std::vector<int> rank[2];
+    std::vector<long long> row_off[2];   // first packed row of the pair
+    std::vector<double> sigma_next[2];   // first discarded singular value of the pair (0 if none); for the truncation bound
+    long long rows = 0;                  // packed rows incl. per-pair padding (without slack)
+    long long n_tiles = 0;
+    // host copies of the packed arrays (kept only for host-only sets)
+    std::vector<double> hU, hW, hWgt;
+    std::vector<lo::ExTile> hTiles;
+    // device factor set
+    double *dU = nullptr, *dW = nullptr, *dWgt = nullptr;
+    lo::ExTile* dTiles = nullptr;
+    std::shared_ptr<lo::SharedOps> ops;
+    // workspace
+    double* dThT = nullptr;       // [O_tot][ldw][N_pad]
+    double* dA[2] = {nullptr, nullptr};  // [Wcap][O_s][O_s] complex
+    double* dXpart = nullptr;     // [MAX_SPLIT][Xp][ldw]
+    double* dEJpart = nullptr;    // [Xp/128][Wcap] complex
+    double* dEKpart = nullptr;    // [num_sms][Wcap] complex
+    int* dStatus = nullptr;       // [2][Wcap]
+    double* dEout = nullptr;      // [Wcap][4] complex (host variant)
+    int* dStatusOut = nullptr;    // [Wcap]
+    double* dPhi[2] = {nullptr, nullptr};  // staging for the host variant
+    unsigned long long factor_bytes = 0, lbar_bytes = 0, workspace_bytes = 0;
+    int last_n_w = 0;
+    // timing
+    bool timing = false;
+    std::vector<lo::TimingEvent> events;
+    std::vector<lo::TimingEvent> pool;
+    double t_ms[LO_K_COUNT] = {0};
+    long long t_n[LO_K_COUNT] = {0};
+};
+
+namespace lo {
+
+// hot path (lo_kernels.cu)
+lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J,
+                              void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
+lo_status configure_kernels();   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)
+
+// GPU setup (lo_setup_gpu.cu): pair Gram matrices + one-sided Jacobi SVD for a batch of pairs of one spin.
+// For the n listed pairs: returns sigma (descending, [n][N]) on the host and leaves the sorted U/W rows on the
+// device in tmpU/tmpW ([n][N][N_pad]).  tmpY/tmpV are scratch of the same size.
+lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV,
+                       double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma);
+size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad);
+
+// microbenchmarks (lo_peak.cu)
+lo_status measure_peak(int device, int kind, double* value);
+
+}  // namespace lo

@@ -1,0 +1,678 @@
+// lo_kernels.cu -- the hot path of lo_local_energy (steps S1-S5 of SURVEY.md 8(a)), hand-written for sm_100a.
+//
+//   k_overlap   A_w = Psi^T Phi_w
+//   k_inverse   A_w^-1 by in-place Gauss-Jordan with partial pivoting, in shared memory (global fallback for big O)
+//   k_theta     Theta_w = Phi_w A_w^-1 (Eq. 15), written as Theta^T panels [o][2w+c][p]
+//   k_coulomb   X = [Lbar; hbar] . Theta   real FP64 GEMM on the DMMA pipe, split-K partials  (Eq. 16 Coulomb part)
+//   k_ej        X = sum of partials, E_J partial sums of X^2 (complex square), E1 from the hbar row
+//   k_exchange  grouped variable-rank dual GEMM a = U Theta_j, b = W Theta_i with fused weight * a * b reduction
+//               (Eq. 19/22 exchange part)
+//   k_finalize  E_K = sum of CTA partials, E_L = E1 + E_J + E_K, NaN for singular walkers
+//
+// FP64 on sm_100a has no tcgen05 path; the FP64 tensor instruction is the warp-level DMMA.8x8x4
+// (mma.sync.aligned.m8n8k4.f64), measured at 37.1 TFLOP/s on this B200 (same rate as the DFMA pipe, but one
+// instruction carries 256 FMAs, so fragments can be fed from shared memory at 25% of its bandwidth).
+// Fragment layout (PTX ISA, m8n8k4 f64): lane = 4*g + t;  A: (row g, k t);  B: (k t, col g);  C: (row g, cols 2t, 2t+1).
+// Both operands are K-major in shared memory with a row pitch of 20 doubles (== 4 mod 16), which makes the
+// 64-bit fragment loads of a half-warp hit 16 distinct 8-byte banks.
+#include <cstdio>
+
+#include "lo_internal.h"
+
+namespace lo {
+
+namespace {
+
+constexpr int PITCH = KTILE + 4;  // doubles
+
+__device__ __forceinline__ void mma884(double& c0, double& c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gptr) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gptr));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N));
+}
+
+// ------------------------------------------------------------------------------------------------ S1: overlap
+// One CTA per walker.  Thread micro-tile 4x4 of A; Psi/Phi rows staged through shared memory 8 rows at a time.
+constexpr int OV_PC = 8;
+__global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi, const double2* __restrict__ phi, double2* __restrict__ A,
+                                                 int N, int O) {
+    extern __shared__ __align__(16) double sm[];
+    const int Op = (O + 3) & ~3;
+    double* psi_s = sm;                                       // [OV_PC][Op]
+    double2* phi_s = reinterpret_cast<double2*>(sm + OV_PC * Op);  // [OV_PC][Op]
+    const int w = blockIdx.x, tid = threadIdx.x;
+    const double2* phw = phi + (size_t)w * N * O;
+    const int nt = Op / 4, ntile = nt * nt;
+    for (int base = 0; base < ntile; base += 256) {
+        const int id = base + tid;
+        const bool valid = id < ntile;
+        const int ti = valid ? id / nt : 0, tj = valid ? id % nt : 0;
+        double2 acc[4][4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) acc[a][b] = make_double2(0.0, 0.0);
+        for (int p0 = 0; p0 < N; p0 += OV_PC) {
+            __syncthreads();
+            for (int e = tid; e < OV_PC * Op; e += 256) {
+                int pp = e / Op, c = e % Op, p = p0 + pp;
+                bool in = (p < N) && (c < O);
+                psi_s[e] = in ? psi[(size_t)p * O + c] : 0.0;
+                phi_s[e] = in ? phw[(size_t)p * O + c] : make_double2(0.0, 0.0);
+            }
+            __syncthreads();
+            if (valid) {
+#pragma unroll
+                for (int pp = 0; pp < OV_PC; ++pp) {
+                    double ps[4];
+                    double2 ph[4];
+#pragma unroll
+                    for (int a = 0; a < 4; ++a) ps[a] = psi_s[pp * Op + ti * 4 + a];
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) ph[b] = phi_s[pp * Op + tj * 4 + b];
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+#pragma unroll
+                        for (int b = 0; b < 4; ++b) {
+                            acc[a][b].x = fma(ps[a], ph[b].x, acc[a][b].x);
+                            acc[a][b].y = fma(ps[a], ph[b].y, acc[a][b].y);
+                        }
+                }
+            }
+        }
+        if (valid) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    int i = ti * 4 + a, j = tj * 4 + b;
+                    if (i < O && j < O) A[((size_t)w * O + i) * O + j] = acc[a][b];
+                }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ S1: inverse
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 crecip(double2 a) {
+    // Smith's algorithm
+    if (fabs(a.x) >= fabs(a.y)) {
+        double r = a.y / a.x, d = a.x + a.y * r;
+        return make_double2(1.0 / d, -r / d);
+    } else {
+        double r = a.x / a.y, d = a.x * r + a.y;
+        return make_double2(r / d, -1.0 / d);
+    }
+}
+
+// In-place Gauss-Jordan inversion with partial (row) pivoting.  One CTA per walker; the O x O complex matrix
+// lives in shared memory (IN_SMEM) or is updated in place in the global workspace (L2 resident) when it does
+// not fit.  status[w] = 1 and A^-1 = NaN when a pivot is zero / non-finite.
+template <bool IN_SMEM>
+__global__ void __launch_bounds__(256) k_inverse(double2* __restrict__ Aws, int* __restrict__ status, int O) {
+    extern __shared__ __align__(16) double sm[];
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double2* Ag = Aws + (size_t)w * O * O;
+    double2* colk = reinterpret_cast<double2*>(sm);              // [O]
+    int* perm = reinterpret_cast<int*>(colk + O);                // [O] padded to a multiple of 4
+    double* red_v = reinterpret_cast<double*>(perm + ((O + 3) & ~3));  // [8]
+    int* red_i = reinterpret_cast<int*>(red_v + 8);              // [8] (+ [8] = pivot row broadcast, [9] = singular flag)
+    double2* M = IN_SMEM ? reinterpret_cast<double2*>(red_i + 16) : Ag;
+    const int OO = O * O;
+    if (IN_SMEM) {
+        for (int e = tid; e < OO; e += 256) M[e] = Ag[e];
+    }
+    if (tid == 0) red_i[9] = 0;
+    __syncthreads();
+    for (int k = 0; k < O; ++k) {
+        // pivot search in column k, rows k..O-1
+        double best = -1.0;
+        int bi = k;
+        for (int r = k + tid; r < O; r += 256) {
+            double2 v = M[r * O + k];
+            double m = v.x * v.x + v.y * v.y;
+            if (!(m == m)) m = INFINITY;   // NaN -> treated as non-finite pivot
+            if (m > best) { best = m; bi = r; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            double ob = __shfl_xor_sync(0xffffffffu, best, o);
+            int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+        }
+        if (lane == 0) { red_v[warp] = best; red_i[warp] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            double b = red_v[0];
+            int i = red_i[0];
+            for (int q = 1; q < 8; ++q)
+                if (red_v[q] > b || (red_v[q] == b && red_i[q] < i)) { b = red_v[q]; i = red_i[q]; }
+            red_i[8] = i;
+            perm[k] = i;
+            if (!(b > 1e-300) || isinf(b)) red_i[9] = 1;
+        }
+        __syncthreads();
+        const int piv = red_i[8];
+        if (red_i[9]) break;   // uniform
+        if (piv != k) {
+            for (int c = tid; c < O; c += 256) {
+                double2 a = M[k * O + c], b = M[piv * O + c];
+                M[k * O + c] = b;
+                M[piv * O + c] = a;
+            }
+        }
+        __syncthreads();
+        const double2 inv = crecip(M[k * O + k]);
+        __syncthreads();
+        for (int r = tid; r < O; r += 256) {
+            colk[r] = M[r * O + k];
+            M[r * O + k] = (r == k) ? make_double2(1.0, 0.0) : make_double2(0.0, 0.0);
+        }
+        __syncthreads();
+        for (int c = tid; c < O; c += 256) M[k * O + c] = cmul(M[k * O + c], inv);
+        __syncthreads();
+        for (int e = tid; e < OO; e += 256) {
+            int r = e / O, c = e - r * O;
+            if (r == k) continue;
+            double2 f = colk[r], v = M[k * O + c], m = M[e];
+            m.x = fma(-f.x, v.x, fma(f.y, v.y, m.x));
+            m.y = fma(-f.x, v.y, fma(-f.y, v.x, m.y));
+            M[e] = m;
+        }
+        __syncthreads();
+    }
+    const bool singular = red_i[9] != 0;
+    if (!singular) {
+        // undo the row interchanges: A^-1 = (P A)^-1 P, i.e. swap columns in reverse order
+        for (int k = O - 1; k >= 0; --k) {
+            int piv = perm[k];
+            if (piv != k) {
+                for (int r = tid; r < O; r += 256) {
+                    double2 a = M[r * O + k], b = M[r * O + piv];
+                    M[r * O + k] = b;
+                    M[r * O + piv] = a;
+                }
+                __syncthreads();
+            }
+        }
+    }
+    __syncthreads();
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    if (singular) {
+        for (int e = tid; e < OO; e += 256) Ag[e] = make_double2(nan, nan);
+    } else if (IN_SMEM) {
+        for (int e = tid; e < OO; e += 256) Ag[e] = M[e];
+    }
+    if (tid == 0) status[w] = singular ? 1 : 0;
+}
+
+// ------------------------------------------------------------------------------------------------ S1: Theta
+// Theta[p][i] = sum_j Phi[p][j] Ainv[j][i]; one CTA = 32 basis rows of one walker; lane = p (coalesced stores of
+// the transposed panels), warps stride over 4-orbital groups.  Rows p in [N, N_pad) are written as zeros.
+__global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, const double2* __restrict__ Ainv, double* __restrict__ thT,
+                                               int N, int N_pad, int O, int o_base, int ldw) {
+    extern __shared__ __align__(16) double sm[];
+    double2* phi_s = reinterpret_cast<double2*>(sm);   // [32][PJ]
+    const int PJ = O | 1;
+    const int p0 = blockIdx.x * 32, w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double2* phw = phi + (size_t)w * N * O;
+    for (int e = tid; e < 32 * O; e += 256) {
+        int pp = e / O, j = e - pp * O, p = p0 + pp;
+        phi_s[pp * PJ + j] = (p < N) ? phw[(size_t)p * O + j] : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    const double2* Aw = Ainv + (size_t)w * O * O;
+    const int p = p0 + lane;
+    for (int i0 = warp * 4; i0 < O; i0 += 32) {
+        double2 acc[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) acc[a] = make_double2(0.0, 0.0);
+        int ia[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) ia[a] = min(i0 + a, O - 1);
+        for (int j = 0; j < O; ++j) {
+            double2 f = phi_s[lane * PJ + j];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                double2 m = __ldg(&Aw[j * O + ia[a]]);
+                acc[a].x = fma(f.x, m.x, fma(-f.y, m.y, acc[a].x));
+                acc[a].y = fma(f.x, m.y, fma(f.y, m.x, acc[a].y));
+            }
+        }
+        if (p < N_pad) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+                if (i0 + a < O) {
+                    size_t base = ((size_t)(o_base + i0 + a) * ldw + 2 * w) * N_pad + p;
+                    thT[base] = acc[a].x;
+                    thT[base + N_pad] = acc[a].y;
+                }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ S3: Coulomb GEMM
+// X[g][c] = sum_{o,p} LbarD[g][o][p] thT[o][c][p]; CTA tile 128 x 128, K tile 16, 8 warps of 64 x 32, 4-stage
+// cp.async pipeline that runs across work items.  Work item = (row block, column block, K split); the K range
+// (flattened over (o, p-tile)) is cut into `nsplit` nearly equal parts to fill 148 SMs; partials go to Xpart[split].
+constexpr int CO_STAGES = 4;
+constexpr int CO_STAGE_DOUBLES = (CO_BM + 128) * PITCH;
+constexpr int CO_SMEM = CO_STAGES * CO_STAGE_DOUBLES * 8;
+
+struct CoItem {
+    int rb, nb, sp, ks0, nsteps;
+};
+__device__ __forceinline__ CoItem co_item(long long q, int RB, int NB, int nsplit, int ksteps) {
+    CoItem it;
+    it.nb = (int)(q % NB);
+    long long r = q / NB;
+    it.rb = (int)(r % RB);
+    it.sp = (int)(r / RB);
+    int base = ksteps / nsplit, rem = ksteps % nsplit;
+    it.ks0 = it.sp * base + min(it.sp, rem);
+    it.nsteps = base + (it.sp < rem ? 1 : 0);
+    return it;
+}
+
+__global__ void __launch_bounds__(256, 1) k_coulomb(const double* __restrict__ A, const double* __restrict__ thT, double* __restrict__ Xpart,
+                                                    int Xp, int O_tot, int N_pad, int ldw, int RB, int NB, int nsplit) {
+    extern __shared__ __align__(16) double sm[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3, wm = warp >> 2, wn = warp & 3;
+    const int KT = N_pad / KTILE, ksteps = O_tot * KT;
+    const size_t Ktot = (size_t)O_tot * N_pad;
+    const long long n_items = (long long)RB * NB * nsplit;
+    // producer state
+    long long pq = blockIdx.x;
+    CoItem pit = {0, 0, 0, 0, 0};
+    int pstep = 0, pslot = 0;
+    if (pq < n_items) pit = co_item(pq, RB, NB, nsplit, ksteps);
+    auto issue = [&]() {
+        if (pq < n_items) {
+            int ks = pit.ks0 + pstep;
+            int o = ks / KT, kt = ks - o * KT;
+            double* st = sm + pslot * CO_STAGE_DOUBLES;
+            const int ch = tid & 7, r0 = tid >> 3;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int row = r0 + 32 * u;
+                cp_async16(st + row * PITCH + ch * 2, A + (size_t)(pit.rb * CO_BM + row) * Ktot + (size_t)o * N_pad + kt * KTILE + ch * 2);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int row = r0 + 32 * u;
+                cp_async16(st + (CO_BM + row) * PITCH + ch * 2,
+                           thT + ((size_t)o * ldw + pit.nb * 128 + row) * N_pad + kt * KTILE + ch * 2);
+            }
+            if (++pstep == pit.nsteps) {
+                pstep = 0;
+                pq += gridDim.x;
+                if (pq < n_items) pit = co_item(pq, RB, NB, nsplit, ksteps);
+            }
+            pslot = (pslot + 1 == CO_STAGES) ? 0 : pslot + 1;
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int s = 0; s < CO_STAGES - 1; ++s) issue();
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    int cslot = 0;
+    for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
+        const CoItem it = co_item(q, RB, NB, nsplit, ksteps);
+        for (int s = 0; s < it.nsteps; ++s) {
+            cp_async_wait<CO_STAGES - 2>();
+            __syncthreads();
+            issue();
+            const double* st = sm + cslot * CO_STAGE_DOUBLES;
+            const double* As = st + (wm * 64 + g) * PITCH + t;
+            const double* Bs = st + (CO_BM + wn * 32 + g) * PITCH + t;
+#pragma unroll
+            for (int ks = 0; ks < KTILE / 4; ++ks) {
+                double a[8], b[4];
+#pragma unroll
+                for (int mf = 0; mf < 8; ++mf) a[mf] = As[mf * 8 * PITCH + ks * 4];
+#pragma unroll
+                for (int nf = 0; nf < 4; ++nf) b[nf] = Bs[nf * 8 * PITCH + ks * 4];
+#pragma unroll
+                for (int mf = 0; mf < 8; ++mf)
+#pragma unroll
+                    for (int nf = 0; nf < 4; ++nf) mma884(acc[mf][nf][0], acc[mf][nf][1], a[mf], b[nf]);
+            }
+            cslot = (cslot + 1 == CO_STAGES) ? 0 : cslot + 1;
+        }
+        double* Xs = Xpart + (size_t)it.sp * Xp * ldw;
+#pragma unroll
+        for (int mf = 0; mf < 8; ++mf)
+#pragma unroll
+            for (int nf = 0; nf < 4; ++nf) {
+                int row = it.rb * CO_BM + wm * 64 + mf * 8 + g;
+                int col = it.nb * 128 + wn * 32 + nf * 8 + 2 * t;
+                *reinterpret_cast<double2*>(Xs + (size_t)row * ldw + col) = make_double2(acc[mf][nf][0], acc[mf][nf][1]);
+                acc[mf][nf][0] = acc[mf][nf][1] = 0.0;
+            }
+    }
+    cp_async_wait<0>();
+}
+
+// X = sum over K-split partials (written back to partial 0, the buffer lo_coulomb_x exposes); E_J partial sums per
+// 128-row chunk: sum_g (X^g)^2 (complex square), the hbar row (g == n_chol) gives E1.  Fixed-order
+// reductions.  grid (Wcap/32, Xp/128), block 256: lane = walker, warp = row stride.
+__global__ void __launch_bounds__(256) k_ej(double* __restrict__ Xpart, double2* __restrict__ EJpart, double2* __restrict__ E1raw, int Xp,
+                                            int ldw, int nsplit, int n_chol, int Wcap) {
+    __shared__ double2 red[8][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int w = blockIdx.x * 32 + lane, chunk = blockIdx.y;
+    double2 s = make_double2(0.0, 0.0);
+    for (int rr = warp; rr < 128; rr += 8) {
+        int row = chunk * 128 + rr;
+        double2* x0 = reinterpret_cast<double2*>(Xpart + (size_t)row * ldw) + w;
+        double2 x = *x0;
+        for (int sp = 1; sp < nsplit; ++sp) {
+            double2 y = *(reinterpret_cast<const double2*>(Xpart + ((size_t)sp * Xp + row) * ldw) + w);
+            x.x += y.x;
+            x.y += y.y;
+        }
+        if (nsplit > 1) *x0 = x;
+        if (row < n_chol) {
+            s.x += x.x * x.x - x.y * x.y;
+            s.y += 2.0 * x.x * x.y;
+        } else if (row == n_chol) {
+            E1raw[w] = x;
+        }
+    }
+    red[warp][lane] = s;
+    __syncthreads();
+    if (warp == 0) {
+        double2 a = red[0][lane];
+        for (int q = 1; q < 8; ++q) { a.x += red[q][lane].x; a.y += red[q][lane].y; }
+        EJpart[(size_t)chunk * Wcap + w] = a;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ S4: exchange
+// Work item = (row tile of one pair, block of 64 walkers).  For the tile's rows K (singular vectors of pair (i,j)):
+//   a[K][w] = sum_p U[K][p] Theta_j[p][w],  b[K][w] = sum_p W[K][p] Theta_i[p][w]   (two real FP64 GEMMs, DMMA)
+//   e[w]   += wgt[K] * a[K][w] * b[K][w]  (complex product; wgt = -cK m_ij sigma_K)
+// CTA tile 64 rows x 128 real columns x 2 accumulators, K tile 16; 8 warps of 32 x 32 (x2); 3-stage cp.async
+// pipeline running across items.  The C fragment holds (re, im) of one walker in one lane, for a and b alike, so the
+// complex product is lane-local; the sum over rows stays in registers across items and is shuffle-reduced only when
+// the CTA's column block changes.  Persistent CTAs with a static round-robin schedule -> deterministic sums.
+constexpr int EX_STAGES = 3;
+constexpr int EX_STAGE_DOUBLES = (2 * EX_BM + 2 * 128) * PITCH;
+constexpr int EX_SMEM = EX_STAGES * EX_STAGE_DOUBLES * 8 + 2 * 128 * 8;
+
+__global__ void __launch_bounds__(256, 1) k_exchange(const double* __restrict__ U, const double* __restrict__ W, const double* __restrict__ wgt,
+                                                     const ExTile* __restrict__ tiles, long long n_items, int NB,
+                                                     const double* __restrict__ thT, int N_pad, int ldw, double* __restrict__ ekpart,
+                                                     int Wcap) {
+    extern __shared__ __align__(16) double sm[];
+    double* red = sm + EX_STAGES * EX_STAGE_DOUBLES;   // [2][128]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3, wm = warp >> 2, wn = warp & 3;
+    const int KT = N_pad / KTILE;
+    double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
+    for (int i = tid; i < 2 * Wcap; i += 256) mypart[i] = 0.0;
+
+    // producer state
+    long long pq = blockIdx.x;
+    int pkt = 0, pslot = 0;
+    ExTile ptile = {0, 0, 0, 0};
+    int pnb = 0;
+    if (pq < n_items) { ptile = tiles[pq / NB]; pnb = (int)(pq % NB); }
+    auto issue = [&]() {
+        if (pq < n_items) {
+            double* st = sm + pslot * EX_STAGE_DOUBLES;
+            const int ch = tid & 7, r0 = tid >> 3;
+            const size_t koff = (size_t)pkt * KTILE + ch * 2;
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                int row = r0 + 32 * u;
+                cp_async16(st + row * PITCH + ch * 2, U + (size_t)(ptile.row0 + row) * N_pad + koff);
+                cp_async16(st + (EX_BM + row) * PITCH + ch * 2, W + (size_t)(ptile.row0 + row) * N_pad + koff);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int row = r0 + 32 * u;
+                cp_async16(st + (2 * EX_BM + row) * PITCH + ch * 2, thT + ((size_t)ptile.pj * ldw + pnb * 128 + row) * N_pad + koff);
+                cp_async16(st + (2 * EX_BM + 128 + row) * PITCH + ch * 2, thT + ((size_t)ptile.pi * ldw + pnb * 128 + row) * N_pad + koff);
+            }
+            if (++pkt == KT) {
+                pkt = 0;
+                pq += gridDim.x;
+                if (pq < n_items) { ptile = tiles[pq / NB]; pnb = (int)(pq % NB); }
+            }
+            pslot = (pslot + 1 == EX_STAGES) ? 0 : pslot + 1;
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int s = 0; s < EX_STAGES - 1; ++s) issue();
+
+    double accA[4][4][2], accB[4][4][2], eacc[4][2];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        eacc[a][0] = eacc[a][1] = 0.0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
+    }
+    int cslot = 0;
+    for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
+        const ExTile tile = tiles[q / NB];
+        const int nb = (int)(q % NB);
+        const int nvalid = min(4, max(0, tile.nfrag - wm * 4));
+        for (int kt = 0; kt < KT; ++kt) {
+            cp_async_wait<EX_STAGES - 2>();
+            __syncthreads();
+            issue();
+            const double* st = sm + cslot * EX_STAGE_DOUBLES;
+            const double* Us = st + (wm * 32 + g) * PITCH + t;
+            const double* Ws = Us + EX_BM * PITCH;
+            const double* Tj = st + (2 * EX_BM + wn * 32 + g) * PITCH + t;
+            const double* Ti = Tj + 128 * PITCH;
+#pragma unroll
+            for (int ks = 0; ks < KTILE / 4; ++ks) {
+                double a[4], w[4], bj[4], bi[4];
+#pragma unroll
+                for (int mf = 0; mf < 4; ++mf) { a[mf] = Us[mf * 8 * PITCH + ks * 4]; w[mf] = Ws[mf * 8 * PITCH + ks * 4]; }
+#pragma unroll
+                for (int nf = 0; nf < 4; ++nf) { bj[nf] = Tj[nf * 8 * PITCH + ks * 4]; bi[nf] = Ti[nf * 8 * PITCH + ks * 4]; }
+#pragma unroll
+                for (int mf = 0; mf < 4; ++mf)
+                    if (mf < nvalid) {
+#pragma unroll
+                        for (int nf = 0; nf < 4; ++nf) {
+                            mma884(accA[mf][nf][0], accA[mf][nf][1], a[mf], bj[nf]);
+                            mma884(accB[mf][nf][0], accB[mf][nf][1], w[mf], bi[nf]);
+                        }
+                    }
+            }
+            cslot = (cslot + 1 == EX_STAGES) ? 0 : cslot + 1;
+        }
+        // fused epilogue: weight * a * b, summed over this lane's rows
+#pragma unroll
+        for (int mf = 0; mf < 4; ++mf) {
+            if (mf < nvalid) {
+                const double wv = __ldg(wgt + tile.row0 + wm * 32 + mf * 8 + g);
+#pragma unroll
+                for (int nf = 0; nf < 4; ++nf) {
+                    double ar = accA[mf][nf][0], ai = accA[mf][nf][1], br = accB[mf][nf][0], bi = accB[mf][nf][1];
+                    eacc[nf][0] = fma(wv, ar * br - ai * bi, eacc[nf][0]);
+                    eacc[nf][1] = fma(wv, ar * bi + ai * br, eacc[nf][1]);
+                }
+            }
+#pragma unroll
+            for (int nf = 0; nf < 4; ++nf) accA[mf][nf][0] = accA[mf][nf][1] = accB[mf][nf][0] = accB[mf][nf][1] = 0.0;
+        }
+        const long long qn = q + gridDim.x;
+        const bool flush = (qn >= n_items) || ((int)(qn % NB) != nb);
+        if (flush) {   // uniform over the CTA
+#pragma unroll
+            for (int nf = 0; nf < 4; ++nf)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    double v = eacc[nf][c];
+                    v += __shfl_xor_sync(0xffffffffu, v, 4);
+                    v += __shfl_xor_sync(0xffffffffu, v, 8);
+                    v += __shfl_xor_sync(0xffffffffu, v, 16);
+                    if (g == 0) red[wm * 128 + (wn * 16 + nf * 4 + t) * 2 + c] = v;
+                    eacc[nf][c] = 0.0;
+                }
+            __syncthreads();
+            if (tid < 128) mypart[(size_t)nb * 128 + tid] += red[tid] + red[128 + tid];
+            __syncthreads();
+        }
+    }
+    cp_async_wait<0>();
+}
+
+// ------------------------------------------------------------------------------------------------ S5: combine
+__global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, const double2* __restrict__ E1raw,
+                           const double2* __restrict__ EKpart, int n_ctas, const int* __restrict__ status, int n_spin, int Wcap,
+                           int n_w, double c1, double cJ, double2* __restrict__ E_L, double2* __restrict__ E1, double2* __restrict__ E_J,
+                           double2* __restrict__ E_K, int* __restrict__ st_out, double2* __restrict__ Eout4) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_w) return;
+    double2 ej = make_double2(0.0, 0.0), ek = make_double2(0.0, 0.0);
+    for (int c = 0; c < n_chunks; ++c) { double2 v = EJpart[(size_t)c * Wcap + w]; ej.x += v.x; ej.y += v.y; }
+    for (int b = 0; b < n_ctas; ++b) { double2 v = EKpart[(size_t)b * Wcap + w]; ek.x += v.x; ek.y += v.y; }
+    double2 e1 = E1raw[w];
+    e1.x *= c1; e1.y *= c1;
+    ej.x *= cJ; ej.y *= cJ;
+    int bad = status[w];
+    if (n_spin == 2) bad |= status[Wcap + w];
+    if (bad) {
+        const double nan = __longlong_as_double(0x7ff8000000000000LL);
+        e1 = ej = ek = make_double2(nan, nan);
+    }
+    double2 el = make_double2(e1.x + ej.x + ek.x, e1.y + ej.y + ek.y);
+    if (E_L) E_L[w] = el;
+    if (E1) E1[w] = e1;
+    if (E_J) E_J[w] = ej;
+    if (E_K) E_K[w] = ek;
+    if (st_out) st_out[w] = bad;
+    if (Eout4) { Eout4[4 * w] = el; Eout4[4 * w + 1] = e1; Eout4[4 * w + 2] = ej; Eout4[4 * w + 3] = ek; }
+}
+
+struct Timer {
+    lo_factors* f;
+    cudaStream_t s;
+    int idx = -1;
+    Timer(lo_factors* f_, cudaStream_t s_, int kind) : f(f_), s(s_) {
+        if (!f->timing) return;
+        TimingEvent ev;
+        if (!f->pool.empty()) { ev = f->pool.back(); f->pool.pop_back(); }
+        else { cudaEventCreate(&ev.e0); cudaEventCreate(&ev.e1); }
+        ev.kind = kind;
+        cudaEventRecord(ev.e0, s);
+        f->events.push_back(ev);
+        idx = (int)f->events.size() - 1;
+    }
+    ~Timer() { if (idx >= 0) cudaEventRecord(f->events[idx].e1, s); }
+};
+
+int pick_split(long long base_items, int ksteps, int sms) {
+    int best = 1;
+    double best_eff = -1;
+    for (int s = 1; s <= MAX_SPLIT; ++s) {
+        if (ksteps / s < 8 && s > 1) break;
+        long long items = base_items * s;
+        long long waves = (items + sms - 1) / sms;
+        double eff = (double)items / (double)(waves * sms);
+        if (eff > best_eff + 0.02) { best_eff = eff; best = s; }
+    }
+    return best;
+}
+
+}  // namespace
+
+lo_status configure_kernels() {
+    cudaError_t e;
+    e = cudaFuncSetAttribute(k_coulomb, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_coulomb): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    e = cudaFuncSetAttribute(k_exchange, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_exchange): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    e = cudaFuncSetAttribute(k_theta, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_theta): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    e = cudaFuncSetAttribute(k_overlap, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_overlap): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    return LO_OK;
+}
+
+lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
+                              int* walker_status, void* Eout4, cudaStream_t stream) {
+    const int N = f->N, N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
+    const void* phis[2] = {phi_a, phi_b};
+    // ---- S1
+    for (int s = 0; s < f->n_spin; ++s) {
+        const int O = f->n_occ[s];
+        const int Op = (O + 3) & ~3;
+        {
+            Timer tm(f, stream, LO_K_OVERLAP);
+            k_overlap<<<n_w, 256, (size_t)OV_PC * Op * 24, stream>>>(f->ops->dPsi[s], (const double2*)phis[s], (double2*)f->dA[s], N, O);
+        }
+        {
+            Timer tm(f, stream, LO_K_INVERSE);
+            size_t aux = (size_t)O * 16 + (size_t)((O + 3) & ~3) * 4 + 64 + 64;
+            size_t need = aux + (size_t)O * O * 16;
+            if (need <= 200 * 1024)
+                k_inverse<true><<<n_w, 256, need, stream>>>((double2*)f->dA[s], f->dStatus + (size_t)s * Wcap, O);
+            else
+                k_inverse<false><<<n_w, 256, aux, stream>>>((double2*)f->dA[s], f->dStatus + (size_t)s * Wcap, O);
+        }
+        {
+            Timer tm(f, stream, LO_K_THETA);
+            dim3 grid((N_pad + 31) / 32, n_w);
+            k_theta<<<grid, 256, (size_t)32 * (O | 1) * 16, stream>>>((const double2*)phis[s], (const double2*)f->dA[s], f->dThT, N, N_pad, O,
+                                                                      f->o_base[s], ldw);
+        }
+    }
+    const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
+    // ---- S2 + S3
+    const int RB = f->Xp / CO_BM;
+    const int ksteps = f->O_tot * (N_pad / KTILE);
+    const int nsplit = pick_split((long long)RB * NB, ksteps, f->num_sms);
+    double2* EJpart = (double2*)f->dEJpart;
+    double2* E1raw = EJpart + (size_t)RB * Wcap;
+    {
+        Timer tm(f, stream, LO_K_COULOMB);
+        long long items = (long long)RB * NB * nsplit;
+        int grid = (int)std::min<long long>(items, f->num_sms);
+        k_coulomb<<<grid, 256, CO_SMEM, stream>>>(f->ops->dLbar, f->dThT, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit);
+        dim3 g2(NB * 2, RB);
+        k_ej<<<g2, 256, 0, stream>>>(f->dXpart, EJpart, E1raw, f->Xp, ldw, nsplit, f->n_chol, Wcap);
+    }
+    // ---- S4
+    int ex_grid = 0;
+    {
+        Timer tm(f, stream, LO_K_EXCHANGE);
+        long long items = f->n_tiles * NB;
+        ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
+        k_exchange<<<ex_grid, 256, EX_SMEM, stream>>>(f->dU, f->dW, f->dWgt, f->dTiles, items, NB, f->dThT, N_pad, ldw, f->dEKpart, Wcap);
+    }
+    // ---- S5
+    {
+        Timer tm(f, stream, LO_K_FINAL);
+        const double c1 = f->n_spin == 1 ? 2.0 : 1.0, cJ = f->n_spin == 1 ? 2.0 : 0.5;
+        k_finalize<<<(n_w + 127) / 128, 128, 0, stream>>>(EJpart, RB, E1raw, (const double2*)f->dEKpart, ex_grid, f->dStatus, f->n_spin, Wcap,
+                                                          n_w, c1, cJ, (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K,
+                                                          walker_status, (double2*)Eout4);
+    }
+    f->last_n_w = n_w;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_error(std::string("kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    return LO_OK;
+}
+
+}  // namespace lo
