@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py -- walker local energies/s of the LO-AFQMC hot path (BASELINE.json:metric) on B200.
+
+  python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path (one rank per GPU under torchrun)
+  python bench.py --impl reference --gpus N --steps K ...  # the CPU oracle, as it stands, on the box's host cores
+
+A "step" is one pass of the whole hot path (S1 Theta, S2 one-body, S3 Coulomb, S4 exchange, S5 combine)
+over one batch of N_w synthetic walkers of BASELINE.json:configs[2] (pentacene-sized; the headline config).  Setup
+(lo_setup: half-rotation, pair SVDs, truncation, packing) is outside the timed region, as the paper's is.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "walker local energies/s (complex128 LO-AFQMC E_L)"
+UNIT = "energies/s"
+NOMINAL_FP64_TFLOPS = 40.0     # B200 datasheet FP64 (vector = tensor); context for the ratio-derived peak
+NOMINAL_BF16_TFLOPS = 2250.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_exchange launch at the default workload, from the committed
+# ncu --set full capture (profiles/); None until that capture exists for the workload being run.
+NCU_TRAFFIC_BYTES = {("C2", "element", 1e-5, 512): None}
+
+
+def workload_name(cfg, reading, T, n_w):
+    import gen
+    spec = gen.CONFIGS[cfg]
+    return "configs[%d] %s, %s reading, T_SVD=%g, N_w=%d" % (cfg, spec.name, reading, T, n_w)
+
+
+class ClockSampler:
+    """nvidia-smi sampled every 100 ms while the timed region runs (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.th = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.th = threading.Thread(target=self._read, daemon=True)
+        self.th.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        pw = [float(r[2]) for r in rows if r[2].replace(".", "", 1).isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows),
+                "power_w_max": max(pw) if pw else None}
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+def oracle_inputs_from_library(P, F):
+    """Host copies the oracle needs to evaluate on the LIBRARY's factor set (parity protocol A)."""
+    import oracle
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+    fs = []
+    for s in range(P.n_spin):
+        U, sg, W = F.factor_all(s)
+        pi, pj = oracle.all_pairs(P.n_occ[s])
+        fs.append(oracle.make_factor_set(P.N, P.n_occ[s], pi, pj, F.ranks(s), U, sg, W))
+    return [a for a, _ in hr], [b for _, b in hr], fs
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import gen
+    import paper_2202_00832_b200 as lo
+    from paper_2202_00832_b200.dist import max_over_ranks
+
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg, reading = args.config, args.reading
+    spec = gen.CONFIGS[cfg]
+    T = args.threshold if args.threshold is not None else spec.thresholds[0]
+    n_w = args.walkers or spec.n_w
+
+    t0 = time.time()
+    P = gen.make_problem(cfg, reading=reading)          # same seed on every rank: the factor set is replicated
+    F = lo.Factors.setup(P.h, P.L, P.psi, T, device=local, max_walkers=n_w, gpu_svd=True)
+    info = F.info()
+    setup_s = time.time() - t0
+    # weak scaling: every rank owns a full batch of n_w walkers (its own seed); no data-path collective
+    phis = gen.make_walkers(P, n_w, seed=P.seed + 1000 * rank)
+    dphi = [torch.from_numpy(p).to(dev) for p in phis]
+    fl = F.flops_per_walker()
+    flops_walker = sum(fl.values())
+
+    peak_dmma = lo.measure_peak("dmma", local)
+    peak_dfma = lo.measure_peak("dfma", local)
+    peak_hbm = lo.measure_peak("hbm", local)
+
+    for _ in range(max(args.warmup, 3)):
+        F.local_energy(dphi, parts=True)
+    torch.cuda.synchronize()
+    F.timing_enable(True)
+    F.timing_get()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    tw0 = time.time()
+    ev0.record()
+    for _ in range(args.steps):
+        out = F.local_energy(dphi, parts=True)
+    ev1.record()
+    torch.cuda.synchronize()
+    tw1 = time.time()
+    if world > 1:
+        dist.barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop(tw0, tw1)
+    ms_max = max_over_ranks(ms, dev)
+    tm = F.timing_get()
+    F.timing_enable(False)
+    n_kernels = sum(n for _, n in tm.values()) + tm["coulomb"][1]      # the coulomb bracket holds 2 launches (GEMM + k_ej)
+    value = world * n_w * args.steps / (ms_max * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of Phi and D2H of E inside the timed region
+    pinned = [torch.from_numpy(p).pin_memory() for p in phis]
+    E_host = torch.empty((n_w, 4), dtype=torch.complex128).pin_memory()
+    st_host = torch.empty(n_w, dtype=torch.int32).pin_memory()
+    for _ in range(2):
+        F.local_energy_host(pinned, E_host, st_host)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        F.local_energy_host(pinned, E_host, st_host)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_e2e = max_over_ranks(e0.elapsed_time(e1), dev)
+    h2d = sum(p.numel() * 16 for p in pinned)
+    d2h = n_w * 4 * 16 + n_w * 4
+    e2e_value = world * n_w * args.steps / (ms_e2e * 1e-3)
+    E_dev = torch.stack(out[:4], dim=1).cpu().numpy()
+    assert np.array_equal(E_host.numpy(), E_dev), "host-buffer path and device path disagree"
+
+    # ---- roofline of the dominant kernel (exchange grouped GEMM), timed live with CUDA events on the launch stream
+    ex_ms, ex_n = tm["exchange"]
+    ex_avg = ex_ms / max(ex_n, 1)
+    ex_flops = fl["exchange"] * n_w
+    achieved = ex_flops / (ex_avg * 1e-3) * 1e-12
+    peak = max(peak_dmma, peak_dfma)
+    mp = measured_peaks()
+    wl = ("C%d" % cfg, reading, T, n_w)
+    roofline = {"bound": "tensor", "kernel": "k_exchange (grouped variable-rank dual DGEMM + fused sigma-weighted a.b)",
+                "achieved": round(achieved, 3), "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
+                "traffic": NCU_TRAFFIC_BYTES.get(wl),
+                "peak_source": "in-run register-resident DMMA.8x8x4 / DFMA loops (lo_measure_peak), of measured",
+                "peak_dmma": round(peak_dmma, 3), "peak_dfma": round(peak_dfma, 3),
+                "peak_from_bf16_ratio": round(mp.get("bf16_tflops", 0) * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS, 2) if mp else None,
+                "hbm_gbs_in_run": round(peak_hbm, 1), "hbm_gbs_measured_peaks": mp.get("hbm_gbs"),
+                "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
+                "algorithmic_flops_per_launch": ex_flops,
+                "algorithmic_bytes_per_launch": 16.0 * info.N * sum(info.sum_rank) + 8.0 * sum(info.sum_rank) + 16.0 * info.N * sum(info.n_occ) * n_w}
+    kernels = {k: {"ms": round(m / max(n, 1), 4), "tflops": round(fl[k] * n_w / (m / max(n, 1) * 1e-3) * 1e-12, 3) if m > 0 else 0.0}
+               for k, (m, n) in tm.items()}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and args.cpu_walkers > 0:
+        import oracle
+        Lbars, hbars, fs = oracle_inputs_from_library(P, F)
+        nb = min(args.cpu_walkers, n_w)
+        sel = [p[:nb] for p in phis]
+        t = time.time()
+        Eo, _ = oracle.local_energy_lo(P.psi, Lbars, hbars, fs, sel)
+        dt = time.time() - t
+        err = float((np.abs(E_dev[:nb] - Eo) / np.abs(Eo[:, :1])).max())
+        cpu_baseline = {"value": round(nb / dt, 3), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                        "sample": "first %d of %d walkers of the same batch, library factor set, %.1f s" % (nb, n_w, dt),
+                        "max_rel_err_gpu_vs_oracle": err}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                "ms_per_step": round(ms_max / args.steps, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload_name(cfg, reading, T, n_w), "N": info.N, "N_occ": list(info.n_occ)[:info.n_spin],
+                           "N_chol": info.n_chol, "N_w_per_gpu": n_w, "T_SVD": T, "sum_rank": sum(info.sum_rank),
+                           "compression_pct": round(100 * (1 - sum(info.sum_rank) / (sum(info.n_pairs) * info.N)), 2),
+                           "factor_GB": round(info.factor_bytes / 1e9, 3), "parallelism": "walker-sharded replicas x%d, no collective" % world,
+                           "l2": "inputs larger than L2 (factor set %.1f GB, Theta %.0f MB per step)" % (
+                               info.factor_bytes / 1e9, 16e-6 * info.N_pad * sum(info.n_occ) * n_w),
+                           "setup_s": round(setup_s, 1)},
+                "tflops": round(flops_walker * n_w * world * args.steps / (ms_max * 1e-3) * 1e-12, 3),
+                "flops_per_walker": flops_walker, "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu_baseline,
+                "e2e": {"value": round(e2e_value, 2), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "ms_per_step": round(ms_e2e / args.steps, 4), "api": "lo_local_energy_host (C ABI, pinned host buffers)"},
+                "gpu_launches": int(n_kernels), "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The CPU oracle, as it stands, end to end on its OWN factors.  Its pair SVDs at the pentacene size take ~2 s per
+    pair per core, so the exchange is timed on a seeded, |i-j|-stratified subset of pairs and the exchange time is
+    scaled to the full pair count; Theta, one-body and Coulomb are timed in full.  A reported baseline, not a target."""
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    import gen
+    import oracle
+    cfg, reading = args.config, args.reading
+    spec = gen.CONFIGS[cfg]
+    T = args.threshold if args.threshold is not None else spec.thresholds[0]
+    n_w = args.walkers or spec.n_w
+    P = gen.make_problem(cfg, reading=reading)
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+    Lbars, hbars = [a for a, _ in hr], [b for _, b in hr]
+    rng = np.random.default_rng(P.seed)
+    fs, frac = [], []
+    for s in range(P.n_spin):
+        pi, pj = oracle.all_pairs(P.n_occ[s])
+        n_sub = min(len(pi), args.ref_pairs)
+        order = np.argsort(pj - pi, kind="stable")
+        sub = np.sort(order[np.linspace(0, len(pi) - 1, n_sub).astype(int)]) if n_sub < len(pi) else np.arange(len(pi))
+        Ut, sg, Wt = oracle.full_svd_pairs(Lbars[s], pi[sub], pj[sub])
+        fs.append(oracle.truncate(P.N, P.n_occ[s], pi[sub], pj[sub], Ut, sg, Wt, T))
+        frac.append(len(sub) / len(pi))
+    empty = [oracle.truncate(P.N, P.n_occ[s], np.zeros(0, np.int32), np.zeros(0, np.int32), np.zeros((0, P.N, P.N)),
+                             np.zeros((0, P.N)), np.zeros((0, P.N, P.N)), T) for s in range(P.n_spin)]
+    nb = min(args.ref_walkers, n_w)
+    phis = gen.make_walkers(P, n_w, seed=P.seed)
+    sel = [p[:nb] for p in phis]
+    times = []
+    for it in range(args.warmup + args.steps):
+        t = time.time()
+        oracle.local_energy_lo(P.psi, Lbars, hbars, empty, sel)
+        t_base = time.time() - t
+        t = time.time()
+        oracle.local_energy_lo(P.psi, Lbars, hbars, fs, sel)
+        t_sub = time.time() - t
+        t_full = t_base + max(t_sub - t_base, 0.0) / (sum(frac) / len(frac))
+        if it >= args.warmup:
+            times.append(t_full)
+    dt = float(np.mean(times))
+    value = nb / dt
+    sample = ("%d of %d walkers per step; exchange on %s of the i<=j pairs (stratified by |i-j|, own Jacobi factors), its time scaled to "
+              "all pairs; Theta/one-body/Coulomb in full" % (nb, n_w, "+".join("%d/%d" % (len(f.r), len(oracle.all_pairs(o)[0])) for f, o in zip(fs, P.n_occ))))
+    line = {"impl": "reference", "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, reading, T, n_w)},
+            "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "kind": "oracle", "cores": oracle.num_threads(), "sample": sample},
+            "e2e": {"value": round(value, 3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: pentacene-sized, the headline)")
+    ap.add_argument("--reading", default="element", choices=["element", "vector"])
+    ap.add_argument("--threshold", type=float, default=None)
+    ap.add_argument("--walkers", type=int, default=None)
+    ap.add_argument("--cpu-walkers", type=int, default=192, help="walkers of the batch the oracle is timed on (cpu_baseline)")
+    ap.add_argument("--ref-walkers", type=int, default=32)
+    ap.add_argument("--ref-pairs", type=int, default=128)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

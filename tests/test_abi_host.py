@@ -1,0 +1,125 @@
+"""CPU-only checks of the boundary: the C-ABI library loads and exports every symbol include/lo_afqmc.h declares,
+argument errors are reported (no compute without a GPU), and the host side of lo_setup (half-rotation, pair SVD,
+truncation, rank sort, padding, tiling, re-truncation) agrees with the oracle."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+import paper_2202_00832_b200 as lo
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "lo_afqmc.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(lo_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(lo.EXPORTS), declared ^ set(lo.EXPORTS)
+    L = lo.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert b"sm_100a" in L.lo_version()
+
+
+def test_argument_errors(c0):
+    with pytest.raises(lo.LoError) as e:
+        lo.Factors.setup(c0.h, c0.L, c0.psi, -1.0, device=-1)
+    assert e.value.status == 1
+    with pytest.raises(lo.LoError) as e:
+        lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=-1, gpu_svd=True)
+    assert e.value.status == 1
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=-1, max_walkers=4)
+    # no device: the energy call must fail loudly, never fall back to the CPU
+    out = np.zeros((4, 4), dtype=np.complex128)
+    phi = np.zeros((4, c0.N, 6), dtype=np.complex128)
+    st = lo.lib().lo_local_energy_host(F._h, 4, phi.ctypes.data, None, out.ctypes.data, None, None)
+    assert st == 3 and b"no CPU path" in lo.lib().lo_last_error()
+    st = lo.lib().lo_local_energy(F._h, 4, phi.ctypes.data, None, out.ctypes.data, None, None, None, None, None)
+    assert st == 3
+    with pytest.raises(lo.LoError):
+        F.retruncate(1e-9)          # tighter than the original threshold
+
+
+@pytest.fixture(scope="module")
+def c1_host(c1):
+    return lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=-1, max_walkers=8)
+
+
+def test_host_factors_match_oracle(c1, c1_host):
+    info = c1_host.info()
+    O, N = c1.n_occ[0], c1.N
+    assert (info.N, info.N_pad, info.n_chol, info.n_spin, info.n_pairs[0]) == (N, 128, 570, 1, O * (O + 1) // 2)
+    Lbar, _ = oracle.half_rotate(c1.L, c1.h, c1.psi[0])
+    pi, pj = oracle.all_pairs(O)
+    sel = np.arange(0, len(pi), 9)
+    Ut, s, Wt = oracle.full_svd_pairs(Lbar, pi[sel], pj[sel])
+    ranks = c1_host.ranks()
+    assert info.sum_rank[0] == ranks.sum() and info.max_rank == ranks.max() and info.min_rank == ranks.min()
+    assert info.sum_rank_padded == ((ranks + 7) // 8 * 8).sum()
+    for n, k in enumerate(sel):
+        r_or = int((s[n] > 1e-4).sum())
+        assert ranks[k] == r_or
+        U, sg, W = c1_host.factor_pair(0, int(pi[k]), int(pj[k]))
+        assert np.abs(sg - s[n, :r_or]).max() <= 1e-12 * s[n, 0]
+        Y = oracle.pair_eri(Lbar, pi[k], pj[k])
+        assert np.abs((U.T * sg) @ W - (Ut[n, :r_or].T * s[n, :r_or]) @ Wt[n, :r_or]).max() <= 1e-11 * s[n, 0]
+        assert np.abs((U.T * sg) @ W - Y).max() <= 2 * max(s[n, r_or] if r_or < N else 0, 1e-12 * s[n, 0])
+        assert np.abs(U @ U.T - np.eye(r_or)).max() < 1e-12 and np.abs(W @ W.T - np.eye(r_or)).max() < 1e-12
+
+
+def test_factor_all_order_and_tiles(c1_host, c1):
+    U, s, W = c1_host.factor_all()
+    ranks = c1_host.ranks()
+    off = np.concatenate([[0], np.cumsum(ranks)])
+    O = c1.n_occ[0]
+    k = 3 * O - 3 + 5 - 3                     # pair (3,5)
+    Up, sp, Wp = c1_host.factor_pair(0, 3, 5)
+    assert np.array_equal(U[off[k]:off[k + 1]], Up) and np.array_equal(s[off[k]:off[k + 1]], sp)
+    info = c1_host.info()
+    # every pair is cut into ceil(r_pad/64) row tiles of near-equal size
+    assert info.n_tiles == (((ranks + 7) // 8 + 7) // 8).sum()
+
+
+def test_retruncate_is_prefix(c1_host):
+    T2 = 2.0
+    F2 = c1_host.retruncate(T2)
+    r1, r2 = c1_host.ranks(), F2.ranks()
+    assert (r2 <= r1).all() and r2.sum() < r1.sum()
+    for (i, j) in [(0, 0), (2, 7), (20, 20)]:
+        U1, s1, W1 = c1_host.factor_pair(0, i, j)
+        U2, s2, W2 = F2.factor_pair(0, i, j)
+        r = len(s2)
+        assert r == int((s1 > T2).sum())
+        assert np.array_equal(U2, U1[:r]) and np.array_equal(s2, s1[:r]) and np.array_equal(W2, W1[:r])
+    assert F2.info().threshold == T2
+
+
+def test_unrestricted_and_zero_rank_pairs():
+    xyz, fns = gen.site_geometry(0)
+    P = gen.make_problem_from_geometry(xyz, fns, (5, 3), 30, seed=5, reading="vector")
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-3, device=-1, max_walkers=4)
+    info = F.info()
+    assert info.n_spin == 2 and tuple(info.n_pairs) == (15, 6)
+    ra, rb = F.ranks(0), F.ranks(1)
+    assert ra.max() <= 4 and rb.max() <= 4            # "vector" reading: rank <= number of sites
+    Fbig = F.retruncate(1e6)                           # everything truncated away
+    assert Fbig.info().sum_rank[0] == 0 and Fbig.info().n_tiles == 0
+    hr = oracle.half_rotate(P.L, P.h, P.psi[1])
+    U, s, W = F.factor_pair(1, 0, 2)
+    Y = oracle.pair_eri(hr[0], 0, 2)
+    assert np.abs((U.T * s) @ W - Y).max() < 2e-3
+
+
+def test_walker_shard():
+    from paper_2202_00832_b200.dist import walker_shard
+    for n, world in [(512, 2), (7, 3), (1, 4), (0, 2)]:
+        spans = [walker_shard(n, r, world) for r in range(world)]
+        assert spans[0][0] == 0 and spans[-1][1] == n
+        assert all(a[1] == b[0] for a, b in zip(spans, spans[1:]))
+        sizes = [b - a for a, b in spans]
+        assert max(sizes) - min(sizes) <= 1

@@ -1,0 +1,272 @@
+"""GPU parity tests (run with -m gpu on the B200 box): the CUDA path, called through the C ABI, against the CPU oracle
+on the same seeded inputs and -- protocol (A) of SURVEY.md 8(c) -- on the LIBRARY's factor set.
+Tolerance (BASELINE.json:north_star): |dE|/|E_L| <= 1e-10 per walker, for E_L and for every part."""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+import paper_2202_00832_b200 as lo
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (there is no CPU fallback)")
+    return torch
+
+
+def oracle_factor_sets(P, F):
+    fs = []
+    for s in range(P.n_spin):
+        U, sg, W = F.factor_all(s)
+        pi, pj = oracle.all_pairs(P.n_occ[s])
+        fs.append(oracle.make_factor_set(P.N, P.n_occ[s], pi, pj, F.ranks(s), U, sg, W))
+    return fs
+
+
+def oracle_energy(P, F, phis, idx=None):
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+    sel = [p if idx is None else p[idx] for p in phis]
+    return oracle.local_energy_lo(P.psi, [a for a, _ in hr], [b for _, b in hr], oracle_factor_sets(P, F), sel)
+
+
+def gpu_energy(F, phis):
+    torch = torch_cuda()
+    d = [torch.from_numpy(np.ascontiguousarray(p)).cuda() for p in phis]
+    out = F.local_energy(d)
+    torch.cuda.synchronize()
+    E = np.stack([e.cpu().numpy() for e in out[:4]], axis=1)
+    return E, out[4].cpu().numpy()
+
+
+def assert_parity(Eg, Eo, tol=TOL):
+    scale = np.abs(Eo[:, 0:1])
+    err = np.abs(Eg - Eo) / scale
+    assert err.max() <= tol, "max rel err per part (E_L,E1,E_J,E_K) = %s" % err.max(axis=0)
+    assert np.abs(Eg[:, 0] - Eg[:, 1:].sum(axis=1)).max() <= 1e-12 * np.abs(Eg).max()
+
+
+# ------------------------------------------------------------------------------------------ C0, C1: every walker
+@pytest.mark.parametrize("gpu_svd", [False, True])
+def test_c0_all_walkers(c0, gpu_svd):
+    phis = gen.make_walkers(c0)
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=0, max_walkers=c0.n_w, gpu_svd=gpu_svd)
+    Eg, st = gpu_energy(F, phis)
+    Eo, so = oracle_energy(c0, F, phis)
+    assert (st == 0).all() and (so == 0).all()
+    assert_parity(Eg, Eo)
+    # untruncated in effect (T=1e-8 keeps all 24 values): equals the exact brute-force energy (Eq. 10) as well
+    for w in range(c0.n_w):
+        e = np.array(oracle.local_energy_exact(c0.h, c0.L, c0.psi, [phis[0][w]], "bruteforce"))
+        assert np.abs(Eg[w] - e).max() <= 1e-9 * abs(e[0])
+
+
+@pytest.mark.parametrize("T", [1e-4, 1e-6])
+def test_c1_all_walkers(c1, T):
+    phis = gen.make_walkers(c1)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, T, device=0, max_walkers=c1.n_w, gpu_svd=True)
+    Eg, st = gpu_energy(F, phis)
+    Eo, _ = oracle_energy(c1, F, phis)
+    assert (st == 0).all()
+    assert_parity(Eg, Eo)
+
+
+def test_c1_theta_parity(c1):
+    phis = gen.make_walkers(c1, 40)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1.0, device=0, max_walkers=40)
+    gpu_energy(F, phis)
+    th = F.theta_host(0, 40)
+    for w in range(40):
+        tho, _, _ = oracle.theta(c1.psi[0], phis[0][w])
+        assert np.abs(th[w] - tho).max() <= 1e-12 * np.abs(tho).max()
+        assert np.abs(c1.psi[0].T @ th[w] - np.eye(c1.n_occ[0])).max() < 1e-11      # Psi^T Theta = I
+
+
+# ------------------------------------------------------------------------------------------ small / ragged ranks
+def test_c1_vector_reading_small_ragged_ranks():
+    P = gen.make_problem(1, reading="vector")
+    phis = gen.make_walkers(P, 100)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-4, device=0, max_walkers=128, gpu_svd=True)
+    r = F.ranks()
+    assert r.max() <= 12 and r.min() < r.max()
+    Eg, _ = gpu_energy(F, phis)
+    Eo, _ = oracle_energy(P, F, phis)
+    assert_parity(Eg, Eo)
+    # a looser threshold through lo_retruncate: ragged ranks incl. zeros, still parity on that factor set
+    F2 = F.retruncate(0.05)
+    r2 = F2.ranks()
+    assert r2.sum() < r.sum()
+    Eg2, _ = gpu_energy(F2, phis)
+    Eo2, _ = oracle_energy(P, F2, phis)
+    assert_parity(Eg2, Eo2)
+
+
+@pytest.mark.parametrize("n_w", [1, 5, 64, 65, 130])
+def test_ragged_walker_counts(c1, n_w):
+    phis = gen.make_walkers(c1, n_w, seed=99)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 5.0, device=0, max_walkers=130)
+    Eg, st = gpu_energy(F, phis)
+    Eo, _ = oracle_energy(c1, F, phis)
+    assert Eg.shape == (n_w, 4)
+    assert_parity(Eg, Eo)
+
+
+def test_all_pairs_truncated_away(c0):
+    phis = gen.make_walkers(c0)
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e9, device=0, max_walkers=8)
+    assert F.info().sum_rank[0] == 0
+    Eg, _ = gpu_energy(F, phis)
+    assert (Eg[:, 3] == 0).all()
+    Eo, _ = oracle_energy(c0, F, phis)
+    assert_parity(Eg, Eo)
+
+
+# ------------------------------------------------------------------------------------------ unrestricted (O6)
+def test_unrestricted_small():
+    xyz, fns = gen.site_geometry(1)
+    P = gen.make_problem_from_geometry(xyz, fns, (9, 7), 300, seed=31)
+    phis = gen.make_walkers(P, 70)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-6, device=0, max_walkers=70, gpu_svd=True)
+    Eg, st = gpu_energy(F, phis)
+    Eo, _ = oracle_energy(P, F, phis)
+    assert_parity(Eg, Eo)
+    for w in (0, 33):
+        e = np.array(oracle.local_energy_exact(P.h, P.L, P.psi, [phis[0][w], phis[1][w]], "cholesky"))
+        assert np.abs(Eg[w] - e).max() <= 1e-4 * abs(e[0])      # T=1e-6: close to exact
+    # identical alpha/beta inputs reproduce the closed-shell result (P9)
+    P2 = gen.make_problem_from_geometry(xyz, fns, (9,), 300, seed=31)
+    Fr = lo.Factors.setup(P2.h, P2.L, P2.psi, 1e-6, device=0, max_walkers=70)
+    Fu = lo.Factors.setup(P2.h, P2.L, [P2.psi[0], P2.psi[0]], 1e-6, device=0, max_walkers=70)
+    ph = gen.make_walkers(P2, 70)
+    Er, _ = gpu_energy(Fr, ph)
+    Eu, _ = gpu_energy(Fu, [ph[0], ph[0]])
+    assert np.abs(Er - Eu).max() <= 1e-12 * np.abs(Er).max()
+
+
+# ------------------------------------------------------------------------------------------ degenerate inputs
+def test_singular_walker_is_flagged(c0):
+    phis = gen.make_walkers(c0)
+    phi = phis[0].copy()
+    phi[3, :, 1] = 0.0                          # a zero orbital: exactly singular overlap (zero pivot on both sides)
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=0, max_walkers=8)
+    Eg, st = gpu_energy(F, [phi])
+    Eo, so = oracle_energy(c0, F, [phi])
+    assert st[3] == 1 and so[3] == 1 and st.sum() == 1
+    assert np.isnan(Eg[3]).all() and np.isnan(Eo[3]).all()
+    ok = [w for w in range(8) if w != 3]
+    assert_parity(Eg[ok], Eo[ok])
+
+
+def test_trial_walker_gives_hf_energy(c1):
+    psi = c1.psi[0]
+    D = psi @ psi.T
+    LD = np.einsum("gpq,qr->gpr", c1.L, D)
+    e_hf = 2 * np.trace(c1.h @ D) + 2 * (np.trace(LD, axis1=1, axis2=2) ** 2).sum() - np.einsum("gpr,grp->", LD, LD)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 0.0, device=0, max_walkers=2, gpu_svd=True)
+    Eg, st = gpu_energy(F, [np.stack([psi, psi]).astype(np.complex128)])
+    assert abs(Eg[0, 0].real - e_hf) <= 1e-10 * abs(e_hf) and abs(Eg[0, 0].imag) <= 1e-10 * abs(e_hf)
+
+
+# ------------------------------------------------------------------------------------------ API variants
+def test_host_variant_and_determinism(c1):
+    torch = torch_cuda()
+    phis = gen.make_walkers(c1, 96)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=96, gpu_svd=True)
+    E1, _ = gpu_energy(F, phis)
+    E2, _ = gpu_energy(F, phis)
+    assert np.array_equal(E1, E2)                                  # fixed-order reductions: bitwise repeatable
+    pinned = [torch.from_numpy(p).pin_memory() for p in phis]
+    Eh, sh = F.local_energy_host(pinned)
+    assert np.array_equal(Eh, E1) and (sh == 0).all()
+    Eh2, _ = F.local_energy_host(phis)                              # pageable numpy buffers
+    assert np.array_equal(Eh2, E1)
+    e_only = F.local_energy([torch.from_numpy(p).cuda() for p in phis], parts=False, status=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(e_only[0].cpu().numpy(), E1[:, 0])
+    with pytest.raises(lo.LoError):
+        F.local_energy([torch.from_numpy(gen.make_walkers(c1, 97)[0]).cuda()])      # n_w > max_walkers
+
+
+def test_gpu_svd_matches_host_svd(c1):
+    Fh = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=8, gpu_svd=False)
+    Fg = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=8, gpu_svd=True)
+    assert np.array_equal(Fh.ranks(), Fg.ranks())
+    assert Fg.info().setup_on_gpu == 1 and Fh.info().setup_on_gpu == 0
+    for (i, j) in [(0, 0), (4, 11), (20, 20)]:
+        Uh, sh, Wh = Fh.factor_pair(0, i, j)
+        Ug, sg, Wg = Fg.factor_pair(0, i, j)
+        assert np.abs(sh - sg).max() <= 1e-12 * sh[0]
+        assert np.abs((Uh.T * sh) @ Wh - (Ug.T * sg) @ Wg).max() <= 1e-11 * sh[0]
+        assert np.abs(Ug @ Ug.T - np.eye(len(sg))).max() < 1e-12
+    # protocol (B): oracle on its own factors vs oracle on the library's factors
+    phis = gen.make_walkers(c1, 4)
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, c1.psi[0])
+    own = oracle.own_factors(Lbar, 1e-4)
+    assert np.array_equal(own.r, Fg.ranks())
+    E_own, _ = oracle.local_energy_lo(c1.psi, [Lbar], [hbar], [own], phis)
+    E_lib, _ = oracle_energy(c1, Fg, phis)
+    assert np.abs(E_own - E_lib).max() <= 1e-9 * np.abs(E_own[:, 0]).min()
+
+
+def test_exact_energy_within_truncation_bound():
+    # protocol (C): GPU LO energy vs the exact exchange, inside the bound of SURVEY 8c-D14
+    P = gen.make_problem(1, reading="vector")
+    phis = gen.make_walkers(P, 8)
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, P.psi[0])
+    pi, pj = oracle.all_pairs(P.n_occ[0])
+    m = np.where(pi == pj, 1.0, 2.0)
+    for T in (1e-4, 0.05, 0.5):
+        F = lo.Factors.setup(P.h, P.L, P.psi, T, device=0, max_walkers=8, gpu_svd=True)
+        Eg, _ = gpu_energy(F, phis)
+        for w in range(8):
+            th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+            nrm = np.linalg.norm(th, axis=0)
+            ek = oracle.exchange_cholesky(Lbar, th)
+            assert abs(Eg[w, 3] - ek) <= T * (m * nrm[pi] * nrm[pj]).sum() + 1e-10 * abs(ek)
+
+
+def test_coulomb_x_export(c1):
+    import ctypes
+    torch = torch_cuda()
+    phis = gen.make_walkers(c1, 10)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 5.0, device=0, max_walkers=10)
+    gpu_energy(F, phis)
+    ptr, ld = F.coulomb_x()
+    X = np.empty((c1.n_chol, ld), dtype=np.complex128)
+    cudart = ctypes.CDLL("libcudart.so")
+    assert cudart.cudaMemcpy(ctypes.c_void_p(X.ctypes.data), ctypes.c_void_p(ptr), ctypes.c_size_t(X.nbytes), 2) == 0
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, c1.psi[0])
+    for w in (0, 9):
+        th, _, _ = oracle.theta(c1.psi[0], phis[0][w])
+        _, _, Xo = oracle.onebody_coulomb([Lbar], [hbar], [th], want_X=True)
+        assert np.abs(X[:, w] - Xo).max() <= 1e-12 * np.abs(Xo).max()
+
+
+# ------------------------------------------------------------------------------------------ full size, sampled outputs
+def test_c2_full_size_sampled_walkers():
+    """BASELINE.json:configs[2] (pentacene-sized, headline) in bench.py's launch configuration: all 512 walkers on
+    the GPU; 24 seeded walkers checked one by one by the oracle on the library's factor set; imaginary-part and
+    sum identities on all walkers."""
+    P = gen.make_problem(2)
+    phis = gen.make_walkers(P)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-5, device=0, max_walkers=P.n_w, gpu_svd=True)
+    info = F.info()
+    assert info.n_pairs[0] == 73 * 74 // 2 and info.max_rank <= 378
+    Eg, st = gpu_energy(F, phis)
+    assert (st == 0).all() and np.isfinite(Eg).all()
+    idx = np.random.default_rng(2).choice(P.n_w, 24, replace=False)
+    Eo, _ = oracle_energy(P, F, phis, idx)
+    assert_parity(Eg[idx], Eo)
+    # exact Cholesky-route exchange for two walkers: inside the truncation bound
+    Lbar, _ = oracle.half_rotate(P.L, P.h, P.psi[0])
+    pi, pj = oracle.all_pairs(73)
+    m = np.where(pi == pj, 1.0, 2.0)
+    for w in idx[:2]:
+        th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+        nrm = np.linalg.norm(th, axis=0)
+        ek = oracle.exchange_cholesky(Lbar, th)
+        assert abs(Eg[w, 3] - ek) <= 1e-5 * (m * nrm[pi] * nrm[pj]).sum() + 1e-10 * abs(ek)
