@@ -26,6 +26,35 @@ SharedOps::~SharedOps() {
     }
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                 CUtensorMapFloatOOBfill);
+
+lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner, unsigned long long rows, unsigned box_rows) {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !p) {
+            set_error("cuTensorMapEncodeTiled is not available from the driver");
+            return LO_ECUDA;
+        }
+        fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    cuuint64_t dims[2] = {inner, rows};
+    cuuint64_t strides[1] = {inner * 8};
+    cuuint32_t box[2] = {(cuuint32_t)KTILE, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r));
+        return LO_ECUDA;
+    }
+    return LO_OK;
+}
+
 namespace {
 
 #define CK(call)                                                                                          \
@@ -198,7 +227,9 @@ lo_status alloc_device(lo_factors* f) {
     CK(cudaMemset(f->dW, 0, rows_alloc * f->N_pad * 8));
     CK(cudaMemset(f->dWgt, 0, rows_alloc * 8));
     f->factor_bytes = 2 * rows_alloc * f->N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
-    return LO_OK;
+    lo_status st = make_tmap(&f->tmU, f->dU, f->N_pad, rows_alloc, EX_BM);
+    if (st == LO_OK) st = make_tmap(&f->tmW, f->dW, f->N_pad, rows_alloc, EX_BM);
+    return st;
 }
 
 lo_status alloc_workspace(lo_factors* f) {
@@ -223,6 +254,8 @@ lo_status alloc_workspace(lo_factors* f) {
     CK(al((void**)&f->dEout, Wcap * 4 * 16));
     CK(al((void**)&f->dStatusOut, Wcap * 4));
     f->workspace_bytes = total;
+    lo_status st = make_tmap(&f->tmTheta, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 128);
+    if (st != LO_OK) return st;
     return configure_kernels();
 }
 
@@ -236,7 +269,7 @@ lo_status upload_lbar(lo_factors* f) {
     CK(cudaMemcpy2D(ops.dLbar, (size_t)f->N_pad * 8, ops.hLbar.data(), (size_t)f->N * 8, (size_t)f->N * 8,
                     (size_t)(f->n_chol + 1) * f->O_tot, cudaMemcpyHostToDevice));
     f->lbar_bytes = (size_t)f->Xp * K * 8;
-    return LO_OK;
+    return make_tmap(&ops.tmLbar, ops.dLbar, K, f->Xp, CO_BM);
 }
 
 void free_all(lo_factors* f) {

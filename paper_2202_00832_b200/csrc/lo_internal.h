@@ -8,6 +8,7 @@
 //   wgt   [rows]              f64   -cK * m_ij * sigma_K  (0 on padding rows).
 //   tiles [n_tiles]                 row tiles of the grouped GEMM: {row0, nfrag (valid 8-row fragments, 1..8), pi, pj}.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstdint>
@@ -39,6 +40,7 @@ std::string& err_buf();
 struct SharedOps {
     int device = -1;
     double* dLbar = nullptr;      // [Xp][O_tot][N_pad]
+    CUtensorMap tmLbar;           // 2D [Xp][O_tot*N_pad], box 128 x 16, 128B swizzle
     double* dPsi[2] = {nullptr, nullptr};  // [N][O_s]
     std::vector<double> hLbar;    // host copy [n_chol][O_tot][N] (+ hbar as row n_chol), kept for host-only sets / retruncate on host
     ~SharedOps();
@@ -68,6 +70,7 @@ struct lo_factors {
     // device factor set
     double *dU = nullptr, *dW = nullptr, *dWgt = nullptr;
     lo::ExTile* dTiles = nullptr;
+    CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
     std::shared_ptr<lo::SharedOps> ops;
     // workspace
     double* dThT = nullptr;       // [O_tot][ldw][N_pad]
@@ -94,7 +97,9 @@ namespace lo {
 // hot path (lo_kernels.cu)
 lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J,
                               void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
-lo_status configure_kernels();   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)
+lo_status configure_kernels();
+// 2D fp64 tensor map over a row-major [rows][inner] array, box [box_rows][16], 128-byte swizzle, zero OOB fill.
+lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner, unsigned long long rows, unsigned box_rows);   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)
 
 // GPU setup (lo_setup_gpu.cu): pair Gram matrices + one-sided Jacobi SVD for a batch of pairs of one spin.
 // For the n listed pairs: returns sigma (descending, [n][N]) on the host and leaves the sorted U/W rows on the

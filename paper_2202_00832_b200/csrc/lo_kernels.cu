@@ -13,8 +13,11 @@
 // (mma.sync.aligned.m8n8k4.f64), measured at 37.1 TFLOP/s on this B200 (same rate as the DFMA pipe, but one
 // instruction carries 256 FMAs, so fragments can be fed from shared memory at 25% of its bandwidth).
 // Fragment layout (PTX ISA, m8n8k4 f64): lane = 4*g + t;  A: (row g, k t);  B: (k t, col g);  C: (row g, cols 2t, 2t+1).
-// Both operands are K-major in shared memory with a row pitch of 20 doubles (== 4 mod 16), which makes the
-// 64-bit fragment loads of a half-warp hit 16 distinct 8-byte banks.
+// Both operands are K-major; TMA (cp.async.bulk.tensor, 128-byte swizzle) stages [rows][16 doubles] tiles into shared
+// memory behind mbarriers, and a fixed permutation of k inside the K tile makes the 64-bit fragment loads of a
+// half-warp hit 16 distinct 8-byte banks (see frag_off).
+#include <cuda.h>
+
 #include <cstdio>
 
 #include "lo_internal.h"
@@ -23,19 +26,52 @@ namespace lo {
 
 namespace {
 
-constexpr int PITCH = KTILE + 4;  // doubles
-
 __device__ __forceinline__ void mma884(double& c0, double& c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async16(void* smem, const void* gptr) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gptr));
+
+// ---- TMA + mbarrier plumbing (cp.async.bulk.tensor; SASS: UTMALDG / SYNCS)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;" ::"n"(N));
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// 2D tiled TMA load: box [rows][16 doubles] at (k0 = inner coordinate in doubles, row0) -> 128-byte-swizzled smem tile
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int k0, int row0, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(k0), "r"(row0), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* tm) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
+}
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+
+// Shared-memory operand tiles are [rows][16 doubles] = 128 bytes per row, written by TMA with the 128-byte swizzle:
+// the 16-byte chunk c of row r lands at chunk c ^ (r & 7) (tile base 1024-byte aligned).  MMA k-step s (0..3) of a
+// K tile takes the logical k indices {2s, 2s+1, 2s+8, 2s+9} for t = 0..3 -- the same permutation for A and B, so the
+// contraction is unchanged -- which puts the 16 lanes of a half-warp (4 rows x 4 k) on 16 distinct 8-byte banks.
+// frag_off(g, t, s): byte offset inside a row whose (r & 7) == g.
+__device__ __forceinline__ uint32_t frag_off(int g, int t, int s) {
+    return (uint32_t)((((s + 4 * (t >> 1)) ^ g) << 4) + (t & 1) * 8);
 }
 
 // ------------------------------------------------------------------------------------------------ S1: overlap
@@ -260,11 +296,11 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
 
 // ------------------------------------------------------------------------------------------------ S3: Coulomb GEMM
 // X[g][c] = sum_{o,p} LbarD[g][o][p] thT[o][c][p]; CTA tile 128 x 128, K tile 16, 8 warps of 64 x 32, 4-stage
-// cp.async pipeline that runs across work items.  Work item = (row block, column block, K split); the K range
+// TMA/mbarrier pipeline that runs across work items.  Work item = (row block, column block, K split); the K range
 // (flattened over (o, p-tile)) is cut into `nsplit` nearly equal parts to fill 148 SMs; partials go to Xpart[split].
 constexpr int CO_STAGES = 4;
-constexpr int CO_STAGE_DOUBLES = (CO_BM + 128) * PITCH;
-constexpr int CO_SMEM = CO_STAGES * CO_STAGE_DOUBLES * 8;
+constexpr int CO_STAGE_BYTES = (CO_BM + 128) * 128;
+constexpr int CO_SMEM = CO_STAGES * CO_STAGE_BYTES + 1024 + 64;
 
 struct CoItem {
     int rb, nb, sp, ks0, nsteps;
@@ -281,35 +317,35 @@ __device__ __forceinline__ CoItem co_item(long long q, int RB, int NB, int nspli
     return it;
 }
 
-__global__ void __launch_bounds__(256, 1) k_coulomb(const double* __restrict__ A, const double* __restrict__ thT, double* __restrict__ Xpart,
-                                                    int Xp, int O_tot, int N_pad, int ldw, int RB, int NB, int nsplit) {
-    extern __shared__ __align__(16) double sm[];
+__global__ void __launch_bounds__(256, 1) k_coulomb(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmT,
+                                                    double* __restrict__ Xpart, int Xp, int O_tot, int N_pad, int ldw, int RB, int NB,
+                                                    int nsplit) {
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bars = sbase + CO_STAGES * CO_STAGE_BYTES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3, wm = warp >> 2, wn = warp & 3;
     const int KT = N_pad / KTILE, ksteps = O_tot * KT;
-    const size_t Ktot = (size_t)O_tot * N_pad;
     const long long n_items = (long long)RB * NB * nsplit;
-    // producer state
+    if (tid == 0) {
+        prefetch_tmap(&tmA);
+        prefetch_tmap(&tmT);
+        for (int i = 0; i < CO_STAGES; ++i) mbar_init(bars + 8 * i, 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
+    // producer state (thread 0 only)
     long long pq = blockIdx.x;
     CoItem pit = {0, 0, 0, 0, 0};
     int pstep = 0, pslot = 0;
     if (pq < n_items) pit = co_item(pq, RB, NB, nsplit, ksteps);
     auto issue = [&]() {
         if (pq < n_items) {
-            int ks = pit.ks0 + pstep;
-            int o = ks / KT, kt = ks - o * KT;
-            double* st = sm + pslot * CO_STAGE_DOUBLES;
-            const int ch = tid & 7, r0 = tid >> 3;
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                int row = r0 + 32 * u;
-                cp_async16(st + row * PITCH + ch * 2, A + (size_t)(pit.rb * CO_BM + row) * Ktot + (size_t)o * N_pad + kt * KTILE + ch * 2);
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                int row = r0 + 32 * u;
-                cp_async16(st + (CO_BM + row) * PITCH + ch * 2,
-                           thT + ((size_t)o * ldw + pit.nb * 128 + row) * N_pad + kt * KTILE + ch * 2);
-            }
+            const int ks = pit.ks0 + pstep;
+            const int o = ks / KT, kt = ks - o * KT;
+            const uint32_t st = sbase + pslot * CO_STAGE_BYTES, bar = bars + 8 * pslot;
+            mbar_expect_tx(bar, CO_STAGE_BYTES);
+            tma_load_2d(st, &tmA, o * N_pad + kt * KTILE, pit.rb * CO_BM, bar);
+            tma_load_2d(st + CO_BM * 128, &tmT, kt * KTILE, o * ldw + pit.nb * 128, bar);
             if (++pstep == pit.nsteps) {
                 pstep = 0;
                 pq += gridDim.x;
@@ -317,39 +353,43 @@ __global__ void __launch_bounds__(256, 1) k_coulomb(const double* __restrict__ A
             }
             pslot = (pslot + 1 == CO_STAGES) ? 0 : pslot + 1;
         }
-        cp_async_commit();
     };
+    if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < CO_STAGES - 1; ++s) issue();
+        for (int s = 0; s < CO_STAGES - 1; ++s) issue();
+    }
 
     double acc[8][4][2];
 #pragma unroll
     for (int a = 0; a < 8; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    uint32_t xo[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
+    const uint32_t a_row = (uint32_t)(wm * 64 + g) * 128, b_row = (uint32_t)(CO_BM + wn * 32 + g) * 128;
     int cslot = 0;
+    uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
         const CoItem it = co_item(q, RB, NB, nsplit, ksteps);
         for (int s = 0; s < it.nsteps; ++s) {
-            cp_async_wait<CO_STAGES - 2>();
-            __syncthreads();
-            issue();
-            const double* st = sm + cslot * CO_STAGE_DOUBLES;
-            const double* As = st + (wm * 64 + g) * PITCH + t;
-            const double* Bs = st + (CO_BM + wn * 32 + g) * PITCH + t;
+            mbar_wait(bars + 8 * cslot, cphase);
+            __syncthreads();          // every warp is done with the slot consumed one step ago -> refill it
+            if (tid == 0) issue();
+            const uint32_t st = sbase + cslot * CO_STAGE_BYTES;
 #pragma unroll
             for (int ks = 0; ks < KTILE / 4; ++ks) {
                 double a[8], b[4];
 #pragma unroll
-                for (int mf = 0; mf < 8; ++mf) a[mf] = As[mf * 8 * PITCH + ks * 4];
+                for (int mf = 0; mf < 8; ++mf) a[mf] = lds_f64(st + a_row + mf * 1024 + xo[ks]);
 #pragma unroll
-                for (int nf = 0; nf < 4; ++nf) b[nf] = Bs[nf * 8 * PITCH + ks * 4];
+                for (int nf = 0; nf < 4; ++nf) b[nf] = lds_f64(st + b_row + nf * 1024 + xo[ks]);
 #pragma unroll
                 for (int mf = 0; mf < 8; ++mf)
 #pragma unroll
                     for (int nf = 0; nf < 4; ++nf) mma884(acc[mf][nf][0], acc[mf][nf][1], a[mf], b[nf]);
             }
-            cslot = (cslot + 1 == CO_STAGES) ? 0 : cslot + 1;
+            if (++cslot == CO_STAGES) { cslot = 0; cphase ^= 1; }
         }
         double* Xs = Xpart + (size_t)it.sp * Xp * ldw;
 #pragma unroll
@@ -362,7 +402,6 @@ __global__ void __launch_bounds__(256, 1) k_coulomb(const double* __restrict__ A
                 acc[mf][nf][0] = acc[mf][nf][1] = 0.0;
             }
     }
-    cp_async_wait<0>();
 }
 
 // X = sum over K-split partials (written back to partial 0, the buffer lo_coulomb_x exposes); E_J partial sums per
@@ -408,44 +447,46 @@ __global__ void __launch_bounds__(256) k_ej(double* __restrict__ Xpart, double2*
 // pipeline running across items.  The C fragment holds (re, im) of one walker in one lane, for a and b alike, so the
 // complex product is lane-local; the sum over rows stays in registers across items and is shuffle-reduced only when
 // the CTA's column block changes.  Persistent CTAs with a static round-robin schedule -> deterministic sums.
-constexpr int EX_STAGES = 3;
-constexpr int EX_STAGE_DOUBLES = (2 * EX_BM + 2 * 128) * PITCH;
-constexpr int EX_SMEM = EX_STAGES * EX_STAGE_DOUBLES * 8 + 2 * 128 * 8;
+constexpr int EX_STAGES = 4;
+constexpr int EX_STAGE_BYTES = (2 * EX_BM + 2 * 128) * 128;
+constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 64 + 2 * 128 * 8;
 
-__global__ void __launch_bounds__(256, 1) k_exchange(const double* __restrict__ U, const double* __restrict__ W, const double* __restrict__ wgt,
-                                                     const ExTile* __restrict__ tiles, long long n_items, int NB,
-                                                     const double* __restrict__ thT, int N_pad, int ldw, double* __restrict__ ekpart,
-                                                     int Wcap) {
-    extern __shared__ __align__(16) double sm[];
-    double* red = sm + EX_STAGES * EX_STAGE_DOUBLES;   // [2][128]
+__global__ void __launch_bounds__(256, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
+                                                     const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
+                                                     const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
+                                                     double* __restrict__ ekpart, int Wcap) {
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bars = sbase + EX_STAGES * EX_STAGE_BYTES;
+    double* red = reinterpret_cast<double*>(smem_raw + (sbase - smem_u32(smem_raw)) + EX_STAGES * EX_STAGE_BYTES + 64);   // [2][128]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3, wm = warp >> 2, wn = warp & 3;
     const int KT = N_pad / KTILE;
     double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
     for (int i = tid; i < 2 * Wcap; i += 256) mypart[i] = 0.0;
+    if (tid == 0) {
+        prefetch_tmap(&tmU);
+        prefetch_tmap(&tmW);
+        prefetch_tmap(&tmT);
+        for (int i = 0; i < EX_STAGES; ++i) mbar_init(bars + 8 * i, 1);
+        fence_barrier_init();
+    }
+    __syncthreads();
 
-    // producer state
+    // producer state (thread 0 only)
     long long pq = blockIdx.x;
     int pkt = 0, pslot = 0;
     ExTile ptile = {0, 0, 0, 0};
     int pnb = 0;
-    if (pq < n_items) { ptile = tiles[pq / NB]; pnb = (int)(pq % NB); }
+    if (tid == 0 && pq < n_items) { ptile = tiles[pq / NB]; pnb = (int)(pq % NB); }
     auto issue = [&]() {
         if (pq < n_items) {
-            double* st = sm + pslot * EX_STAGE_DOUBLES;
-            const int ch = tid & 7, r0 = tid >> 3;
-            const size_t koff = (size_t)pkt * KTILE + ch * 2;
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                int row = r0 + 32 * u;
-                cp_async16(st + row * PITCH + ch * 2, U + (size_t)(ptile.row0 + row) * N_pad + koff);
-                cp_async16(st + (EX_BM + row) * PITCH + ch * 2, W + (size_t)(ptile.row0 + row) * N_pad + koff);
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                int row = r0 + 32 * u;
-                cp_async16(st + (2 * EX_BM + row) * PITCH + ch * 2, thT + ((size_t)ptile.pj * ldw + pnb * 128 + row) * N_pad + koff);
-                cp_async16(st + (2 * EX_BM + 128 + row) * PITCH + ch * 2, thT + ((size_t)ptile.pi * ldw + pnb * 128 + row) * N_pad + koff);
-            }
+            const uint32_t st = sbase + pslot * EX_STAGE_BYTES, bar = bars + 8 * pslot;
+            const int k0 = pkt * KTILE;
+            mbar_expect_tx(bar, EX_STAGE_BYTES);
+            tma_load_2d(st, &tmU, k0, ptile.row0, bar);
+            tma_load_2d(st + EX_BM * 128, &tmW, k0, ptile.row0, bar);
+            tma_load_2d(st + 2 * EX_BM * 128, &tmT, k0, ptile.pj * ldw + pnb * 128, bar);
+            tma_load_2d(st + (2 * EX_BM + 128) * 128, &tmT, k0, ptile.pi * ldw + pnb * 128, bar);
             if (++pkt == KT) {
                 pkt = 0;
                 pq += gridDim.x;
@@ -453,10 +494,11 @@ __global__ void __launch_bounds__(256, 1) k_exchange(const double* __restrict__ 
             }
             pslot = (pslot + 1 == EX_STAGES) ? 0 : pslot + 1;
         }
-        cp_async_commit();
     };
+    if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < EX_STAGES - 1; ++s) issue();
+        for (int s = 0; s < EX_STAGES - 1; ++s) issue();
+    }
 
     double accA[4][4][2], accB[4][4][2], eacc[4][2];
 #pragma unroll
@@ -465,27 +507,35 @@ __global__ void __launch_bounds__(256, 1) k_exchange(const double* __restrict__ 
 #pragma unroll
         for (int b = 0; b < 4; ++b) accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
     }
+    uint32_t xo[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
+    const uint32_t u_row = (uint32_t)(wm * 32 + g) * 128, w_row = u_row + EX_BM * 128;
+    const uint32_t tj_row = (uint32_t)(2 * EX_BM + wn * 32 + g) * 128, ti_row = tj_row + 128 * 128;
     int cslot = 0;
+    uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
         const ExTile tile = tiles[q / NB];
         const int nb = (int)(q % NB);
         const int nvalid = min(4, max(0, tile.nfrag - wm * 4));
         for (int kt = 0; kt < KT; ++kt) {
-            cp_async_wait<EX_STAGES - 2>();
-            __syncthreads();
-            issue();
-            const double* st = sm + cslot * EX_STAGE_DOUBLES;
-            const double* Us = st + (wm * 32 + g) * PITCH + t;
-            const double* Ws = Us + EX_BM * PITCH;
-            const double* Tj = st + (2 * EX_BM + wn * 32 + g) * PITCH + t;
-            const double* Ti = Tj + 128 * PITCH;
+            mbar_wait(bars + 8 * cslot, cphase);
+            __syncthreads();          // every warp is done with the slot consumed one step ago -> refill it
+            if (tid == 0) issue();
+            const uint32_t st = sbase + cslot * EX_STAGE_BYTES;
 #pragma unroll
             for (int ks = 0; ks < KTILE / 4; ++ks) {
                 double a[4], w[4], bj[4], bi[4];
 #pragma unroll
-                for (int mf = 0; mf < 4; ++mf) { a[mf] = Us[mf * 8 * PITCH + ks * 4]; w[mf] = Ws[mf * 8 * PITCH + ks * 4]; }
+                for (int mf = 0; mf < 4; ++mf) {
+                    a[mf] = lds_f64(st + u_row + mf * 1024 + xo[ks]);
+                    w[mf] = lds_f64(st + w_row + mf * 1024 + xo[ks]);
+                }
 #pragma unroll
-                for (int nf = 0; nf < 4; ++nf) { bj[nf] = Tj[nf * 8 * PITCH + ks * 4]; bi[nf] = Ti[nf * 8 * PITCH + ks * 4]; }
+                for (int nf = 0; nf < 4; ++nf) {
+                    bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
+                    bi[nf] = lds_f64(st + ti_row + nf * 1024 + xo[ks]);
+                }
 #pragma unroll
                 for (int mf = 0; mf < 4; ++mf)
                     if (mf < nvalid) {
@@ -496,7 +546,7 @@ __global__ void __launch_bounds__(256, 1) k_exchange(const double* __restrict__ 
                         }
                     }
             }
-            cslot = (cslot + 1 == EX_STAGES) ? 0 : cslot + 1;
+            if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
         }
         // fused epilogue: weight * a * b, summed over this lane's rows
 #pragma unroll
@@ -532,7 +582,6 @@ __global__ void __launch_bounds__(256, 1) k_exchange(const double* __restrict__ 
             __syncthreads();
         }
     }
-    cp_async_wait<0>();
 }
 
 // ------------------------------------------------------------------------------------------------ S5: combine
@@ -649,7 +698,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         Timer tm(f, stream, LO_K_COULOMB);
         long long items = (long long)RB * NB * nsplit;
         int grid = (int)std::min<long long>(items, f->num_sms);
-        k_coulomb<<<grid, 256, CO_SMEM, stream>>>(f->ops->dLbar, f->dThT, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit);
+        k_coulomb<<<grid, 256, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit);
         dim3 g2(NB * 2, RB);
         k_ej<<<g2, 256, 0, stream>>>(f->dXpart, EJpart, E1raw, f->Xp, ldw, nsplit, f->n_chol, Wcap);
     }
@@ -659,7 +708,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         Timer tm(f, stream, LO_K_EXCHANGE);
         long long items = f->n_tiles * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        k_exchange<<<ex_grid, 256, EX_SMEM, stream>>>(f->dU, f->dW, f->dWgt, f->dTiles, items, NB, f->dThT, N_pad, ldw, f->dEKpart, Wcap);
+        k_exchange<<<ex_grid, 256, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad, ldw, f->dEKpart, Wcap);
     }
     // ---- S5
     {
