@@ -174,11 +174,21 @@ struct PairRec {
     long long src;   // offset (rows) of this pair's kept rows in the staging arrays
 };
 
-// Sort pairs by rank (descending; ties by spin, i, j), assign padded row offsets, cut row tiles.
+// Order the pairs, assign padded row offsets, cut row tiles.  Order: L2 blocks of BO x BO orbitals (row-major over
+// (spin, i-block, j-block)) so that the Theta panels a block touches (2*BO panels of ldw*N_pad*8 bytes) stay in the
+// 126 MB L2 while the block's factor rows stream through once; inside a block pairs are sorted by rank, descending.
 void plan_layout(lo_factors* f, std::vector<PairRec>& pairs, std::vector<int>& sorted) {
+    const double panel_bytes = (double)f->ldw * f->N_pad * 8.0;
+    const int BO = std::max(1, std::min(16, (int)(48e6 / (2.0 * panel_bytes))));
     sorted.resize(pairs.size());
     std::iota(sorted.begin(), sorted.end(), 0);
-    std::stable_sort(sorted.begin(), sorted.end(), [&](int a, int b) { return pairs[a].r > pairs[b].r; });
+    std::stable_sort(sorted.begin(), sorted.end(), [&](int a, int b) {
+        const PairRec &x = pairs[a], &y = pairs[b];
+        if (x.spin != y.spin) return x.spin < y.spin;
+        if (x.i / BO != y.i / BO) return x.i / BO < y.i / BO;
+        if (x.j / BO != y.j / BO) return x.j / BO < y.j / BO;
+        return x.r > y.r;
+    });
     for (int s = 0; s < f->n_spin; ++s) {
         size_t np = (size_t)f->n_occ[s] * (f->n_occ[s] + 1) / 2;
         f->rank[s].assign(np, 0);

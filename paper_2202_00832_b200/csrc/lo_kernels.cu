@@ -40,6 +40,12 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
+// Warp-specialised register budget (setmaxnreg, per warpgroup): the kernels launch 3 warpgroups at 168 registers per
+// thread; the producer warpgroup shrinks to 40, the two consumer warpgroups grow to 232 (4*32*40 + 8*32*232 = 64512).
+__device__ __forceinline__ void reg_dec_producer() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
+__device__ __forceinline__ void reg_inc_consumer() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
+__device__ __forceinline__ void bar_sync_consumers() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
@@ -300,7 +306,7 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
 // (flattened over (o, p-tile)) is cut into `nsplit` nearly equal parts to fill 148 SMs; partials go to Xpart[split].
 constexpr int CO_STAGES = 4;
 constexpr int CO_STAGE_BYTES = (CO_BM + 128) * 128;
-constexpr int CO_SMEM = CO_STAGES * CO_STAGE_BYTES + 1024 + 64;
+constexpr int CO_SMEM = CO_STAGES * CO_STAGE_BYTES + 1024 + 128;
 
 struct CoItem {
     int rb, nb, sp, ks0, nsteps;
@@ -317,48 +323,47 @@ __device__ __forceinline__ CoItem co_item(long long q, int RB, int NB, int nspli
     return it;
 }
 
-__global__ void __launch_bounds__(256, 1) k_coulomb(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmT,
+__global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmT,
                                                     double* __restrict__ Xpart, int Xp, int O_tot, int N_pad, int ldw, int RB, int NB,
                                                     int nsplit) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bars = sbase + CO_STAGES * CO_STAGE_BYTES;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3, wm = warp >> 2, wn = warp & 3;
+    const uint32_t full = sbase + CO_STAGES * CO_STAGE_BYTES, empty = full + 8 * CO_STAGES;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE, ksteps = O_tot * KT;
     const long long n_items = (long long)RB * NB * nsplit;
     if (tid == 0) {
         prefetch_tmap(&tmA);
         prefetch_tmap(&tmT);
-        for (int i = 0; i < CO_STAGES; ++i) mbar_init(bars + 8 * i, 1);
+        for (int i = 0; i < CO_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
     }
     __syncthreads();
-    // producer state (thread 0 only)
-    long long pq = blockIdx.x;
-    CoItem pit = {0, 0, 0, 0, 0};
-    int pstep = 0, pslot = 0;
-    if (pq < n_items) pit = co_item(pq, RB, NB, nsplit, ksteps);
-    auto issue = [&]() {
-        if (pq < n_items) {
-            const int ks = pit.ks0 + pstep;
-            const int o = ks / KT, kt = ks - o * KT;
-            const uint32_t st = sbase + pslot * CO_STAGE_BYTES, bar = bars + 8 * pslot;
-            mbar_expect_tx(bar, CO_STAGE_BYTES);
-            tma_load_2d(st, &tmA, o * N_pad + kt * KTILE, pit.rb * CO_BM, bar);
-            tma_load_2d(st + CO_BM * 128, &tmT, kt * KTILE, o * ldw + pit.nb * 128, bar);
-            if (++pstep == pit.nsteps) {
-                pstep = 0;
-                pq += gridDim.x;
-                if (pq < n_items) pit = co_item(pq, RB, NB, nsplit, ksteps);
+    if (warp < 4) {
+        // ===== producer warpgroup; one lane drives TMA, running ahead of the consumers by up to CO_STAGES stages
+        reg_dec_producer();
+        if (warp == 0 && lane == 0) {
+            int slot = 0;
+            uint32_t phase = 0;
+            for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
+                const CoItem it = co_item(q, RB, NB, nsplit, ksteps);
+                for (int s = 0; s < it.nsteps; ++s) {
+                    const int ks = it.ks0 + s;
+                    const int o = ks / KT, kt = ks - o * KT;
+                    mbar_wait(empty + 8 * slot, phase ^ 1);
+                    const uint32_t st = sbase + slot * CO_STAGE_BYTES, bar = full + 8 * slot;
+                    mbar_expect_tx(bar, CO_STAGE_BYTES);
+                    tma_load_2d(st, &tmA, o * N_pad + kt * KTILE, it.rb * CO_BM, bar);
+                    tma_load_2d(st + CO_BM * 128, &tmT, kt * KTILE, o * ldw + it.nb * 128, bar);
+                    if (++slot == CO_STAGES) { slot = 0; phase ^= 1; }
+                }
             }
-            pslot = (pslot + 1 == CO_STAGES) ? 0 : pslot + 1;
         }
-    };
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < CO_STAGES - 1; ++s) issue();
+        return;
     }
-
+    // ===== 8 consumer warps (64 x 32 each)
+    reg_inc_consumer();
+    const int cw = warp - 4, g = lane >> 2, t = lane & 3, wm = cw >> 2, wn = cw & 3;
     double acc[8][4][2];
 #pragma unroll
     for (int a = 0; a < 8; ++a)
@@ -373,9 +378,7 @@ __global__ void __launch_bounds__(256, 1) k_coulomb(const __grid_constant__ CUte
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
         const CoItem it = co_item(q, RB, NB, nsplit, ksteps);
         for (int s = 0; s < it.nsteps; ++s) {
-            mbar_wait(bars + 8 * cslot, cphase);
-            __syncthreads();          // every warp is done with the slot consumed one step ago -> refill it
-            if (tid == 0) issue();
+            mbar_wait(full + 8 * cslot, cphase);
             const uint32_t st = sbase + cslot * CO_STAGE_BYTES;
 #pragma unroll
             for (int ks = 0; ks < KTILE / 4; ++ks) {
@@ -389,6 +392,8 @@ __global__ void __launch_bounds__(256, 1) k_coulomb(const __grid_constant__ CUte
 #pragma unroll
                     for (int nf = 0; nf < 4; ++nf) mma884(acc[mf][nf][0], acc[mf][nf][1], a[mf], b[nf]);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + 8 * cslot);
             if (++cslot == CO_STAGES) { cslot = 0; cphase ^= 1; }
         }
         double* Xs = Xpart + (size_t)it.sp * Xp * ldw;
@@ -449,79 +454,82 @@ __global__ void __launch_bounds__(256) k_ej(double* __restrict__ Xpart, double2*
 // the CTA's column block changes.  Persistent CTAs with a static round-robin schedule -> deterministic sums.
 constexpr int EX_STAGES = 4;
 constexpr int EX_STAGE_BYTES = (2 * EX_BM + 2 * 128) * 128;
-constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 64 + 2 * 128 * 8;
+constexpr int EX_RING = 8;      // tile-descriptor ring (producer -> consumers), > EX_STAGES items can never be in flight
+constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 2 * 128 * 8;
 
-__global__ void __launch_bounds__(256, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
+__global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
                                                      const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
                                                      const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
                                                      double* __restrict__ ekpart, int Wcap) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bars = sbase + EX_STAGES * EX_STAGE_BYTES;
-    double* red = reinterpret_cast<double*>(smem_raw + (sbase - smem_u32(smem_raw)) + EX_STAGES * EX_STAGE_BYTES + 64);   // [2][128]
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3, wm = warp >> 2, wn = warp & 3;
+    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
+    const uint32_t full = sbase + EX_STAGES * EX_STAGE_BYTES, empty = full + 8 * EX_STAGES;
+    ExTile* ring = reinterpret_cast<ExTile*>(sgen + EX_STAGES * EX_STAGE_BYTES + 128);            // [EX_RING]
+    double* red = reinterpret_cast<double*>(sgen + EX_STAGES * EX_STAGE_BYTES + 128 + EX_RING * 16);   // [2][128]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
-    for (int i = tid; i < 2 * Wcap; i += 256) mypart[i] = 0.0;
+    for (int i = tid; i < 2 * Wcap; i += 384) mypart[i] = 0.0;
     if (tid == 0) {
         prefetch_tmap(&tmU);
         prefetch_tmap(&tmW);
         prefetch_tmap(&tmT);
-        for (int i = 0; i < EX_STAGES; ++i) mbar_init(bars + 8 * i, 1);
+        for (int i = 0; i < EX_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
     }
     __syncthreads();
-
-    // producer state (thread 0 only)
-    long long pq = blockIdx.x;
-    int pkt = 0, pslot = 0;
-    ExTile ptile = {0, 0, 0, 0};
-    int pnb = 0;
-    if (tid == 0 && pq < n_items) { ptile = tiles[pq / NB]; pnb = (int)(pq % NB); }
-    auto issue = [&]() {
-        if (pq < n_items) {
-            const uint32_t st = sbase + pslot * EX_STAGE_BYTES, bar = bars + 8 * pslot;
-            const int k0 = pkt * KTILE;
-            mbar_expect_tx(bar, EX_STAGE_BYTES);
-            tma_load_2d(st, &tmU, k0, ptile.row0, bar);
-            tma_load_2d(st + EX_BM * 128, &tmW, k0, ptile.row0, bar);
-            tma_load_2d(st + 2 * EX_BM * 128, &tmT, k0, ptile.pj * ldw + pnb * 128, bar);
-            tma_load_2d(st + (2 * EX_BM + 128) * 128, &tmT, k0, ptile.pi * ldw + pnb * 128, bar);
-            if (++pkt == KT) {
-                pkt = 0;
-                pq += gridDim.x;
-                if (pq < n_items) { ptile = tiles[pq / NB]; pnb = (int)(pq % NB); }
+    if (warp < 4) {
+        // ===== producer warpgroup; one lane drives TMA, running ahead of the consumers by up to EX_STAGES stages, across
+        // work items.  The tile descriptor of item n is published in ring[n % EX_RING] before the item's first stage is armed.
+        reg_dec_producer();
+        if (warp == 0 && lane == 0) {
+            int slot = 0, n = 0;
+            uint32_t phase = 0;
+            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
+                const ExTile tile = tiles[q / NB];
+                const int nb = (int)(q % NB);
+                for (int kt = 0; kt < KT; ++kt) {
+                    mbar_wait(empty + 8 * slot, phase ^ 1);
+                    if (kt == 0) ring[n % EX_RING] = tile;      // ordered before the consumers' wait by arrive.expect_tx (release)
+                    const uint32_t st = sbase + slot * EX_STAGE_BYTES, bar = full + 8 * slot;
+                    const int k0 = kt * KTILE;
+                    mbar_expect_tx(bar, EX_STAGE_BYTES);
+                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
+                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
+                    tma_load_2d(st + 2 * EX_BM * 128, &tmT, k0, tile.pj * ldw + nb * 128, bar);
+                    tma_load_2d(st + (2 * EX_BM + 128) * 128, &tmT, k0, tile.pi * ldw + nb * 128, bar);
+                    if (++slot == EX_STAGES) { slot = 0; phase ^= 1; }
+                }
             }
-            pslot = (pslot + 1 == EX_STAGES) ? 0 : pslot + 1;
         }
-    };
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < EX_STAGES - 1; ++s) issue();
+        return;
     }
-
-    double accA[4][4][2], accB[4][4][2], eacc[4][2];
+    // ===== 8 consumer warps (32 rows x 32 columns x 2 accumulators each)
+    reg_inc_consumer();
+    const int ctid = tid - 128, cw = warp - 4, g = lane >> 2, t = lane & 3, wm = cw >> 2, wn = cw & 3;
+    double accA[4][4][2], accB[4][4][2];
 #pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        eacc[a][0] = eacc[a][1] = 0.0;
+    for (int a = 0; a < 4; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
-    }
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
     const uint32_t u_row = (uint32_t)(wm * 32 + g) * 128, w_row = u_row + EX_BM * 128;
     const uint32_t tj_row = (uint32_t)(2 * EX_BM + wn * 32 + g) * 128, ti_row = tj_row + 128 * 128;
-    int cslot = 0;
+    int cslot = 0, n = 0;
     uint32_t cphase = 0;
-    for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
-        const ExTile tile = tiles[q / NB];
+    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
         const int nb = (int)(q % NB);
+        mbar_wait(full + 8 * cslot, cphase);            // first stage of the item: its descriptor is in the ring now
+        const ExTile tile = ring[n % EX_RING];
         const int nvalid = min(4, max(0, tile.nfrag - wm * 4));
+        double wv[4];
+#pragma unroll
+        for (int mf = 0; mf < 4; ++mf) wv[mf] = (mf < nvalid) ? __ldg(wgt + tile.row0 + wm * 32 + mf * 8 + g) : 0.0;
         for (int kt = 0; kt < KT; ++kt) {
-            mbar_wait(bars + 8 * cslot, cphase);
-            __syncthreads();          // every warp is done with the slot consumed one step ago -> refill it
-            if (tid == 0) issue();
+            if (kt) mbar_wait(full + 8 * cslot, cphase);
             const uint32_t st = sbase + cslot * EX_STAGE_BYTES;
 #pragma unroll
             for (int ks = 0; ks < KTILE / 4; ++ks) {
@@ -546,41 +554,38 @@ __global__ void __launch_bounds__(256, 1) k_exchange(const __grid_constant__ CUt
                         }
                     }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + 8 * cslot);
             if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
         }
-        // fused epilogue: weight * a * b, summed over this lane's rows
+        // fused epilogue: e[w] = sum over this lane's rows of weight * a * b (complex), then over the 8 row groups of
+        // the warp (shuffles) and the two row-halves of the tile (shared memory), in a fixed order
+        double e[4][2];
+#pragma unroll
+        for (int nf = 0; nf < 4; ++nf) e[nf][0] = e[nf][1] = 0.0;
 #pragma unroll
         for (int mf = 0; mf < 4; ++mf) {
-            if (mf < nvalid) {
-                const double wv = __ldg(wgt + tile.row0 + wm * 32 + mf * 8 + g);
 #pragma unroll
-                for (int nf = 0; nf < 4; ++nf) {
-                    double ar = accA[mf][nf][0], ai = accA[mf][nf][1], br = accB[mf][nf][0], bi = accB[mf][nf][1];
-                    eacc[nf][0] = fma(wv, ar * br - ai * bi, eacc[nf][0]);
-                    eacc[nf][1] = fma(wv, ar * bi + ai * br, eacc[nf][1]);
-                }
+            for (int nf = 0; nf < 4; ++nf) {
+                double ar = accA[mf][nf][0], ai = accA[mf][nf][1], br = accB[mf][nf][0], bi = accB[mf][nf][1];
+                e[nf][0] = fma(wv[mf], ar * br - ai * bi, e[nf][0]);
+                e[nf][1] = fma(wv[mf], ar * bi + ai * br, e[nf][1]);
+                accA[mf][nf][0] = accA[mf][nf][1] = accB[mf][nf][0] = accB[mf][nf][1] = 0.0;
             }
-#pragma unroll
-            for (int nf = 0; nf < 4; ++nf) accA[mf][nf][0] = accA[mf][nf][1] = accB[mf][nf][0] = accB[mf][nf][1] = 0.0;
         }
-        const long long qn = q + gridDim.x;
-        const bool flush = (qn >= n_items) || ((int)(qn % NB) != nb);
-        if (flush) {   // uniform over the CTA
 #pragma unroll
-            for (int nf = 0; nf < 4; ++nf)
+        for (int nf = 0; nf < 4; ++nf)
 #pragma unroll
-                for (int c = 0; c < 2; ++c) {
-                    double v = eacc[nf][c];
-                    v += __shfl_xor_sync(0xffffffffu, v, 4);
-                    v += __shfl_xor_sync(0xffffffffu, v, 8);
-                    v += __shfl_xor_sync(0xffffffffu, v, 16);
-                    if (g == 0) red[wm * 128 + (wn * 16 + nf * 4 + t) * 2 + c] = v;
-                    eacc[nf][c] = 0.0;
-                }
-            __syncthreads();
-            if (tid < 128) mypart[(size_t)nb * 128 + tid] += red[tid] + red[128 + tid];
-            __syncthreads();
-        }
+            for (int c = 0; c < 2; ++c) {
+                double v = e[nf][c];
+                v += __shfl_xor_sync(0xffffffffu, v, 4);
+                v += __shfl_xor_sync(0xffffffffu, v, 8);
+                v += __shfl_xor_sync(0xffffffffu, v, 16);
+                if (g == 0) red[wm * 128 + (wn * 16 + nf * 4 + t) * 2 + c] = v;
+            }
+        bar_sync_consumers();
+        if (ctid < 128) mypart[(size_t)nb * 128 + ctid] += red[ctid] + red[128 + ctid];
+        bar_sync_consumers();
     }
 }
 
@@ -698,7 +703,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         Timer tm(f, stream, LO_K_COULOMB);
         long long items = (long long)RB * NB * nsplit;
         int grid = (int)std::min<long long>(items, f->num_sms);
-        k_coulomb<<<grid, 256, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit);
+        k_coulomb<<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit);
         dim3 g2(NB * 2, RB);
         k_ej<<<g2, 256, 0, stream>>>(f->dXpart, EJpart, E1raw, f->Xp, ldw, nsplit, f->n_chol, Wcap);
     }
@@ -708,7 +713,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         Timer tm(f, stream, LO_K_EXCHANGE);
         long long items = f->n_tiles * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        k_exchange<<<ex_grid, 256, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad, ldw, f->dEKpart, Wcap);
+        k_exchange<<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad, ldw, f->dEKpart, Wcap);
     }
     // ---- S5
     {
