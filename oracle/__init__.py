@@ -228,6 +228,14 @@ def exchange_lo(fs: FactorSet, th):
     return out[0]
 
 
+def exchange_lo_batch(fs: FactorSet, thetas):
+    """O5 single-spin truncated exchange sums of several walkers (thetas [n_w,N,O]); OpenMP over walkers."""
+    thetas = _c128(thetas)
+    out = np.zeros(thetas.shape[0], dtype=np.complex128)
+    _l().orc_exchange_lo_batch(C.c_int(thetas.shape[0]), *_fs_args(fs), _p(thetas), _p(out))
+    return out
+
+
 def coulomb_lo(fs: FactorSet, th):
     """Paper-literal compressed Coulomb double sum S (closed shell E_J^LO = 2 S), Eq. 19/22."""
     th = _c128(th)
@@ -281,3 +289,40 @@ def local_energy_lo(psis, Lbars, hbars, fsets, phis):
                              _ptr_array([f.U for f in fsets]), _ptr_array([f.sigma for f in fsets]),
                              _ptr_array([f.W for f in fsets]), _ptr_array(phis), _p(out), _p(status))
     return out, status
+
+
+def empty_factor_set(N, O) -> FactorSet:
+    z = np.zeros(0, np.int32)
+    return FactorSet(N, O, z, z, z, np.zeros(0, np.int64), np.zeros((0, N)), np.zeros(0), np.zeros((0, N)))
+
+
+def local_energy_lo_streamed(psis, Lbars, hbars, phis, n_pairs, fetch, chunk=256):
+    """local_energy_lo for factor sets too large to hold on the host: Theta, E1 and E_J as in local_energy_lo, the
+    exchange sum accumulated over chunks of pairs, fetch(spin, k0, k1) -> FactorSet of the pairs [k0, k1) of that spin
+    (natural i<=j order).  Returns (E [n_w,4], status [n_w], seconds spent in the oracle's own arithmetic)."""
+    import time
+    ns = len(psis)
+    t0 = time.time()
+    E, status = local_energy_lo(psis, Lbars, hbars, [empty_factor_set(p.shape[0], p.shape[1]) for p in psis], phis)
+    n_w = phis[0].shape[0]
+    thetas = []
+    for s in range(ns):
+        th = np.zeros(phis[s].shape, dtype=np.complex128)
+        for w in range(n_w):
+            if status[w] == 0:
+                th[w] = theta(psis[s], phis[s][w])[0]
+        thetas.append(th)
+    secs = time.time() - t0
+    ek = np.zeros(n_w, dtype=np.complex128)
+    for s in range(ns):
+        for k0 in range(0, n_pairs[s], chunk):
+            fs = fetch(s, k0, min(n_pairs[s], k0 + chunk))
+            t0 = time.time()
+            ek += exchange_lo_batch(fs, thetas[s])
+            secs += time.time() - t0
+    if ns == 2:
+        ek *= 0.5
+    ok = status == 0
+    E[ok, 3] = ek[ok]
+    E[ok, 0] = E[ok, 1] + E[ok, 2] + E[ok, 3]
+    return E, status, secs

@@ -346,6 +346,15 @@ void orc_exchange_lo(int N, int O, int n_pairs, const int* pi, const int* pj, co
     *out = ek;
 }
 
+// O5 for several walkers at once (the same sum as orc_exchange_lo, one walker per OpenMP task): thetas [n_w][N][O],
+// out [n_w] single-spin sums.  Lets a checker stream a large factor set through in chunks of pairs and add up.
+void orc_exchange_lo_batch(int n_w, int N, int O, int n_pairs, const int* pi, const int* pj, const int* r, const int64_t* off,
+                           const double* U, const double* sigma, const double* W, const cd* thetas, cd* out) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int w = 0; w < n_w; ++w)
+        orc_exchange_lo(N, O, n_pairs, pi, pj, r, off, U, sigma, W, thetas + (size_t)w * N * O, out + w);
+}
+
 // Paper-literal compressed Coulomb term (Eq. 19 / 22, "4 Q̄_{K,L,i} Q̄_{K,R,j}"):
 // closed shell E_J^{LO} = 2 sum_{ij ordered} sum_K sigma_K (U^T Theta_i)_K (W Theta_j)_K, where the (j,i) block of an
 // i<j pair, Y^{ji} = (Y^{ij})^T, contributes the same number as the (i,j) block (weight m_ij).  Returns the single-spin double sum S so that

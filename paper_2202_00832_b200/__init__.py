@@ -144,6 +144,23 @@ class Factors:
         _check(lib().lo_factor_all(self._h, spin, U.ctypes.data, s.ctypes.data, W.ctypes.data))
         return U, s, W
 
+    def factor_range(self, spin, k0, k1):
+        """Factors of the pairs [k0, k1) of one spin (lo_ranks order), rows back to back: (ranks, U, sigma, W).
+        One lo_factor_pair call per pair; for factor sets too large to copy to the host in one piece."""
+        info = self.info()
+        O, N = info.n_occ[spin], info.N
+        r = self.ranks(spin)[k0:k1]
+        off = np.concatenate([[0], np.cumsum(r)]).astype(np.int64)
+        U, s, W = np.zeros((int(off[-1]), N)), np.zeros(int(off[-1])), np.zeros((int(off[-1]), N))
+        ii, jj = np.triu_indices(O)
+        L = lib()
+        for n, k in enumerate(range(k0, k1)):
+            if r[n] == 0:
+                continue
+            a = int(off[n])
+            _check(L.lo_factor_pair(self._h, spin, int(ii[k]), int(jj[k]), U[a:].ctypes.data, s[a:].ctypes.data, W[a:].ctypes.data))
+        return r, U, s, W
+
     def retruncate(self, threshold) -> "Factors":
         out = C.c_void_p()
         _check(lib().lo_retruncate(self._h, float(threshold), C.byref(out)))

@@ -171,75 +171,123 @@ void host_jacobi(int n, double* G, double* V, std::vector<double>& sigma, std::v
 
 struct PairRec {
     int spin, i, j, r;
-    long long src;   // offset (rows) of this pair's kept rows in the staging arrays
+    int x;            // index of the pair inside the batch being packed (source of its rows)
+    long long src;    // lo_retruncate: first packed row of the pair in the source factor set
+    double snext;     // first discarded singular value (0 if none)
 };
 
-// Order the pairs, assign padded row offsets, cut row tiles.  Order: L2 blocks of BO x BO orbitals (row-major over
-// (spin, i-block, j-block)) so that the Theta panels a block touches (2*BO panels of ldw*N_pad*8 bytes) stay in the
-// 126 MB L2 while the block's factor rows stream through once; inside a block pairs are sorted by rank, descending.
-void plan_layout(lo_factors* f, std::vector<PairRec>& pairs, std::vector<int>& sorted) {
+inline size_t pair_index(int O, int i, int j) { return (size_t)i * O - (size_t)i * (i - 1) / 2 + (j - i); }
+
+// Pair order of the packed arrays: L2 blocks of BO x BO orbitals (row-major over (spin, i-block, j-block)) so that
+// the Theta panels a block touches (2*BO panels of ldw*N_pad*8 bytes) stay in the 126 MB L2 while the block's factor
+// rows stream through once; inside a block pairs are sorted by rank, descending (done when the ranks are known).
+// Returns the pairs in that order and the start index of every block (+ end sentinel).
+void enumerate_blocks(const lo_factors* f, std::vector<PairRec>& pairs, std::vector<size_t>& block_start) {
     const double panel_bytes = (double)f->ldw * f->N_pad * 8.0;
     const int BO = std::max(1, std::min(16, (int)(48e6 / (2.0 * panel_bytes))));
-    sorted.resize(pairs.size());
-    std::iota(sorted.begin(), sorted.end(), 0);
-    std::stable_sort(sorted.begin(), sorted.end(), [&](int a, int b) {
-        const PairRec &x = pairs[a], &y = pairs[b];
-        if (x.spin != y.spin) return x.spin < y.spin;
-        if (x.i / BO != y.i / BO) return x.i / BO < y.i / BO;
-        if (x.j / BO != y.j / BO) return x.j / BO < y.j / BO;
-        return x.r > y.r;
-    });
+    pairs.clear();
+    block_start.clear();
     for (int s = 0; s < f->n_spin; ++s) {
-        size_t np = (size_t)f->n_occ[s] * (f->n_occ[s] + 1) / 2;
-        f->rank[s].assign(np, 0);
-        f->row_off[s].assign(np, 0);
-    }
-    long long row = 0;
-    f->hTiles.clear();
-    for (int idx : sorted) {
-        const PairRec& pr = pairs[idx];
-        const int O = f->n_occ[pr.spin];
-        const size_t k = (size_t)pr.i * O - (size_t)pr.i * (pr.i - 1) / 2 + (pr.j - pr.i);
-        f->rank[pr.spin][k] = pr.r;
-        f->row_off[pr.spin][k] = row;
-        const int r_pad = round_up(pr.r, 8);
-        if (r_pad > 0) {
-            const int F = r_pad / 8, nt = (F + 7) / 8;
-            int done = 0;
-            for (int t = 0; t < nt; ++t) {
-                int nf = F / nt + (t < F % nt ? 1 : 0);
-                ExTile T;
-                T.row0 = (int)(row + (long long)done * 8);
-                T.nfrag = nf;
-                T.pi = f->o_base[pr.spin] + pr.i;
-                T.pj = f->o_base[pr.spin] + pr.j;
-                f->hTiles.push_back(T);
-                done += nf;
+        const int O = f->n_occ[s], nb = (O + BO - 1) / BO;
+        for (int ib = 0; ib < nb; ++ib)
+            for (int jb = ib; jb < nb; ++jb) {
+                block_start.push_back(pairs.size());
+                for (int i = ib * BO; i < std::min(O, (ib + 1) * BO); ++i)
+                    for (int j = std::max(i, jb * BO); j < std::min(O, (jb + 1) * BO); ++j) pairs.push_back({s, i, j, 0, 0, 0, 0.0});
             }
-        }
-        row += r_pad;
     }
-    f->rows = row;
-    f->n_tiles = (long long)f->hTiles.size();
+    block_start.push_back(pairs.size());
 }
 
-lo_status alloc_device(lo_factors* f) {
-    CK(cudaSetDevice(f->device));
-    cudaDeviceProp prop;
-    CK(cudaGetDeviceProperties(&prop, f->device));
-    f->num_sms = prop.multiProcessorCount;
+// Appends pairs (ranks known) to the packed layout: sorts [first,last) by rank inside the block, assigns padded row
+// offsets, cuts row tiles, appends the weights  -cK m_ij sigma_K  (sig(pr, K) gives sigma_K) and fills `table` with the
+// row copies to perform (src_row is set by the caller's src_row_of).
+template <class SigmaFn, class SrcFn>
+void layout_block(lo_factors* f, PairRec* first, PairRec* last, SigmaFn sig, SrcFn src_row_of, std::vector<GatherRec>& table) {
+    std::stable_sort(first, last, [](const PairRec& a, const PairRec& b) { return a.r > b.r; });
+    const double cK = f->n_spin == 1 ? 1.0 : 0.5;
+    for (PairRec* pr = first; pr != last; ++pr) {
+        const size_t k = pair_index(f->n_occ[pr->spin], pr->i, pr->j);
+        f->rank[pr->spin][k] = pr->r;
+        f->row_off[pr->spin][k] = f->rows;
+        f->sigma_next[pr->spin][k] = pr->snext;
+        const int r_pad = round_up(pr->r, 8);
+        if (r_pad == 0) continue;
+        const int F = r_pad / 8, nt = (F + 7) / 8;
+        int done = 0;
+        for (int t = 0; t < nt; ++t) {
+            const int nf = F / nt + (t < F % nt ? 1 : 0);
+            ExTile T;
+            T.row0 = (int)(f->rows + (long long)done * 8);
+            T.nfrag = nf;
+            T.pi = f->o_base[pr->spin] + pr->i;
+            T.pj = f->o_base[pr->spin] + pr->j;
+            f->hTiles.push_back(T);
+            done += nf;
+        }
+        const double m = pr->i == pr->j ? 1.0 : 2.0;
+        f->hWgt.resize((size_t)f->rows + r_pad, 0.0);
+        for (int K = 0; K < pr->r; ++K) f->hWgt[(size_t)f->rows + K] = -cK * m * sig(*pr, K);
+        table.push_back({src_row_of(*pr), f->rows, pr->r, 0});
+        f->rows += r_pad;
+    }
+}
+
+lo_status begin_pack(lo_factors* f) {
+    for (int s = 0; s < f->n_spin; ++s) {
+        const size_t np = (size_t)f->n_occ[s] * (f->n_occ[s] + 1) / 2;
+        f->rank[s].assign(np, 0);
+        f->row_off[s].assign(np, 0);
+        f->sigma_next[s].assign(np, 0.0);
+    }
+    f->rows = 0;
+    f->hTiles.clear();
+    f->hWgt.clear();
+    if (f->device >= 0) {
+        CK(cudaSetDevice(f->device));
+        size_t max_rows = EX_BM;
+        for (int s = 0; s < f->n_spin; ++s) max_rows += (size_t)f->n_occ[s] * (f->n_occ[s] + 1) / 2 * round_up(f->N, 8);
+        lo_status st = f->bU.reserve(f->device, max_rows * f->N_pad * 8);
+        if (st == LO_OK) st = f->bW.reserve(f->device, max_rows * f->N_pad * 8);
+        if (st != LO_OK) return st;
+        f->dU = static_cast<double*>(f->bU.base);
+        f->dW = static_cast<double*>(f->bW.base);
+    }
+    return LO_OK;
+}
+
+// make rows [0, rows + EX_BM) of the packed arrays usable (zero-filled where new)
+lo_status grow_pack(lo_factors* f) {
+    const size_t bytes = ((size_t)f->rows + EX_BM) * f->N_pad * 8;
+    if (f->device >= 0) {
+        lo_status st = f->bU.ensure(bytes);
+        if (st == LO_OK) st = f->bW.ensure(bytes);
+        return st;
+    }
+    f->hU.resize(bytes / 8, 0.0);
+    f->hW.resize(bytes / 8, 0.0);
+    return LO_OK;
+}
+
+lo_status alloc_workspace(lo_factors* f);
+
+lo_status finish_pack(lo_factors* f) {
+    lo_status st = grow_pack(f);
+    if (st != LO_OK) return st;
     const size_t rows_alloc = (size_t)f->rows + EX_BM;
-    CK(cudaMalloc(&f->dU, rows_alloc * f->N_pad * 8));
-    CK(cudaMalloc(&f->dW, rows_alloc * f->N_pad * 8));
+    f->hWgt.resize(rows_alloc, 0.0);
+    f->n_tiles = (long long)f->hTiles.size();
+    f->factor_bytes = 2 * rows_alloc * f->N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
+    if (f->device < 0) return LO_OK;
+    CK(cudaSetDevice(f->device));
     CK(cudaMalloc(&f->dWgt, rows_alloc * 8));
     CK(cudaMalloc(&f->dTiles, std::max<size_t>(1, f->hTiles.size()) * sizeof(ExTile)));
-    CK(cudaMemset(f->dU, 0, rows_alloc * f->N_pad * 8));
-    CK(cudaMemset(f->dW, 0, rows_alloc * f->N_pad * 8));
-    CK(cudaMemset(f->dWgt, 0, rows_alloc * 8));
-    f->factor_bytes = 2 * rows_alloc * f->N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
-    lo_status st = make_tmap(&f->tmU, f->dU, f->N_pad, rows_alloc, EX_BM);
+    CK(cudaMemcpy(f->dWgt, f->hWgt.data(), rows_alloc * 8, cudaMemcpyHostToDevice));
+    if (!f->hTiles.empty()) CK(cudaMemcpy(f->dTiles, f->hTiles.data(), f->hTiles.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
+    st = make_tmap(&f->tmU, f->dU, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmW, f->dW, f->N_pad, rows_alloc, EX_BM);
-    return st;
+    if (st != LO_OK) return st;
+    return alloc_workspace(f);
 }
 
 lo_status alloc_workspace(lo_factors* f) {
@@ -288,54 +336,14 @@ void free_all(lo_factors* f) {
         cudaSetDevice(f->device);
         for (auto& ev : f->events) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
         for (auto& ev : f->pool) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
-        void* ptrs[] = {f->dU, f->dW, f->dWgt, f->dTiles, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
+        f->bU.release();
+        f->bW.release();
+        void* ptrs[] = {f->dWgt, f->dTiles, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
                         f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1]};
         for (void* p : ptrs)
             if (p) cudaFree(p);
     }
     delete f;
-}
-
-// common tail of lo_setup / lo_retruncate: staging rows (hUs/hWs/hSig in `pairs[].src` order, row pitch N) -> packed + upload
-lo_status pack_and_upload(lo_factors* f, std::vector<PairRec>& pairs, const std::vector<double>& sU, const std::vector<double>& sW,
-                          const std::vector<double>& sSig) {
-    std::vector<int> sorted;
-    plan_layout(f, pairs, sorted);
-    const size_t rows_alloc = (size_t)f->rows + EX_BM;
-    const double cK = f->n_spin == 1 ? 1.0 : 0.5;
-    const int N = f->N, N_pad = f->N_pad;
-    f->hU.assign(rows_alloc * N_pad, 0.0);
-    f->hW.assign(rows_alloc * N_pad, 0.0);
-    f->hWgt.assign(rows_alloc, 0.0);
-#pragma omp parallel for schedule(dynamic, 16)
-    for (size_t x = 0; x < pairs.size(); ++x) {
-        const PairRec& pr = pairs[x];
-        const int O = f->n_occ[pr.spin];
-        const size_t k = (size_t)pr.i * O - (size_t)pr.i * (pr.i - 1) / 2 + (pr.j - pr.i);
-        const long long row0 = f->row_off[pr.spin][k];
-        const double m = pr.i == pr.j ? 1.0 : 2.0;
-        for (int K = 0; K < pr.r; ++K) {
-            std::memcpy(&f->hU[(size_t)(row0 + K) * N_pad], &sU[(size_t)(pr.src + K) * N], (size_t)N * 8);
-            std::memcpy(&f->hW[(size_t)(row0 + K) * N_pad], &sW[(size_t)(pr.src + K) * N], (size_t)N * 8);
-            f->hWgt[row0 + K] = -cK * m * sSig[pr.src + K];
-        }
-    }
-    if (f->device >= 0) {
-        lo_status st = alloc_device(f);
-        if (st != LO_OK) return st;
-        CK(cudaMemcpy(f->dU, f->hU.data(), rows_alloc * N_pad * 8, cudaMemcpyHostToDevice));
-        CK(cudaMemcpy(f->dW, f->hW.data(), rows_alloc * N_pad * 8, cudaMemcpyHostToDevice));
-        CK(cudaMemcpy(f->dWgt, f->hWgt.data(), rows_alloc * 8, cudaMemcpyHostToDevice));
-        if (!f->hTiles.empty())
-            CK(cudaMemcpy(f->dTiles, f->hTiles.data(), f->hTiles.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
-        std::vector<double>().swap(f->hU);
-        std::vector<double>().swap(f->hW);
-        st = alloc_workspace(f);
-        if (st != LO_OK) return st;
-    } else {
-        f->factor_bytes = 2 * rows_alloc * N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
-    }
-    return LO_OK;
 }
 
 // fetch packed rows [row0,row0+r) of U or W to a host buffer with pitch N
@@ -405,105 +413,110 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             st = upload_lbar(f);
             if (st != LO_OK) { free_all(f); return st; }
         }
-        // ---- per-pair SVD + truncation
+        // ---- per-pair SVD + truncation + packing, batch by batch in layout order (whole L2 blocks per batch)
         std::vector<PairRec> pairs;
-        for (int s = 0; s < n_spin; ++s)
-            for (int i = 0; i < n_occ[s]; ++i)
-                for (int j = i; j < n_occ[s]; ++j) pairs.push_back({s, i, j, 0, 0});
-        const size_t np = pairs.size();
-        std::vector<std::vector<double>> pU(np), pW(np), pS(np);
-        std::vector<double> snext(np, 0.0);
-        if (flags & LO_SETUP_GPU_SVD) {
-            f->setup_on_gpu = 1;
-            // batches of pairs on the device
+        std::vector<size_t> bstart;
+        enumerate_blocks(f, pairs, bstart);
+        st = begin_pack(f);
+        if (st != LO_OK) { free_all(f); return st; }
+        const bool on_gpu = (flags & LO_SETUP_GPU_SVD) != 0;
+        f->setup_on_gpu = on_gpu ? 1 : 0;
+        size_t B = 256;   // pairs per batch
+        double *tY = nullptr, *tV = nullptr, *tU = nullptr, *tW = nullptr, *dSig = nullptr;
+        int* dOrd = nullptr;
+        auto free_tmp = [&]() { cudaFree(tY); cudaFree(tV); cudaFree(tU); cudaFree(tW); cudaFree(dSig); cudaFree(dOrd); };
+        if (on_gpu) {
             const size_t per_pair = gpu_pair_svd_bytes_per_pair(N, f->N_pad);
             size_t free_b = 0, total_b = 0;
             cudaMemGetInfo(&free_b, &total_b);
-            size_t B = std::max<size_t>(1, std::min<size_t>({np, (size_t)(f->num_sms * 4), (free_b / 4) / per_pair}));
-            double *tY = nullptr, *tV = nullptr, *tU = nullptr, *tW = nullptr, *dSig = nullptr;
-            int* dOrd = nullptr;
+            B = std::max<size_t>(1, std::min<size_t>({pairs.size(), (size_t)(f->num_sms * 4), (free_b / 8) / per_pair}));
             const size_t mat = (size_t)N * f->N_pad * 8;
             if (cudaMalloc(&tY, B * mat) != cudaSuccess || cudaMalloc(&tV, B * mat) != cudaSuccess || cudaMalloc(&tU, B * mat) != cudaSuccess ||
                 cudaMalloc(&tW, B * mat) != cudaSuccess || cudaMalloc(&dSig, B * N * 8) != cudaSuccess || cudaMalloc(&dOrd, B * N * 4) != cudaSuccess) {
-                set_error("lo_setup: cannot allocate GPU SVD workspace"); free_all(f); return LO_ENOMEM;
+                set_error("lo_setup: cannot allocate GPU SVD workspace"); free_tmp(); free_all(f); return LO_ENOMEM;
             }
-            std::vector<double> hSig(B * N), hRow((size_t)N * f->N_pad);
-            std::vector<int> bi(B), bj(B);
-            for (size_t k0 = 0; k0 < np && st == LO_OK;) {
-                const int spin = pairs[k0].spin;
-                size_t k1 = k0;
-                while (k1 < np && k1 - k0 < B && pairs[k1].spin == spin) ++k1;
-                const int n = (int)(k1 - k0);
-                for (int x = 0; x < n; ++x) { bi[x] = pairs[k0 + x].i; bj[x] = pairs[k0 + x].j; }
+        }
+        std::vector<double> hSig(B * N);
+        std::vector<std::vector<double>> pU(on_gpu ? 0 : B), pW(on_gpu ? 0 : B);
+        std::vector<int> bi(B), bj(B);
+        std::vector<GatherRec> table;
+        const double* Lbar = f->ops->hLbar.data();
+        for (size_t blk = 0; blk + 1 < bstart.size() && st == LO_OK;) {
+            // batch = consecutive whole blocks of one spin, at most B pairs (a block larger than B is split)
+            const size_t k0 = bstart[blk];
+            const int spin = pairs[k0].spin;
+            size_t k1 = k0, blk1 = blk;
+            while (blk1 + 1 < bstart.size() && pairs[bstart[blk1]].spin == spin && bstart[blk1 + 1] - k0 <= B) k1 = bstart[++blk1];
+            const bool split = (k1 == k0);
+            if (split) k1 = std::min(k0 + B, bstart[blk + 1]);
+            const int n = (int)(k1 - k0);
+            for (int x = 0; x < n; ++x) { pairs[k0 + x].x = x; bi[x] = pairs[k0 + x].i; bj[x] = pairs[k0 + x].j; }
+            if (on_gpu) {
                 st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data());
                 if (st != LO_OK) break;
-                for (int x = 0; x < n; ++x) {
-                    const double* sg = &hSig[(size_t)x * N];
-                    int r = 0;
-                    while (r < N && sg[r] > threshold) ++r;
-                    pairs[k0 + x].r = r;
-                    snext[k0 + x] = r < N ? sg[r] : 0.0;
-                    pS[k0 + x].assign(sg, sg + r);
-                    pU[k0 + x].resize((size_t)r * N);
-                    pW[k0 + x].resize((size_t)r * N);
-                    if (r > 0) {
-                        cudaMemcpy2D(pU[k0 + x].data(), (size_t)N * 8, tU + (size_t)x * N * f->N_pad, (size_t)f->N_pad * 8, (size_t)N * 8, r,
-                                     cudaMemcpyDeviceToHost);
-                        cudaMemcpy2D(pW[k0 + x].data(), (size_t)N * 8, tW + (size_t)x * N * f->N_pad, (size_t)f->N_pad * 8, (size_t)N * 8, r,
-                                     cudaMemcpyDeviceToHost);
-                    }
-                }
-                k0 = k1;
-            }
-            cudaFree(tY); cudaFree(tV); cudaFree(tU); cudaFree(tW); cudaFree(dSig); cudaFree(dOrd);
-            if (st != LO_OK) { free_all(f); return st; }
-        } else {
-            const double* Lbar = f->ops->hLbar.data();
+            } else {
 #pragma omp parallel
-            {
-                std::vector<double> G((size_t)N * N), V((size_t)N * N), sg;
-                std::vector<int> order;
+                {
+                    std::vector<double> G((size_t)N * N), V((size_t)N * N), sg;
+                    std::vector<int> order;
 #pragma omp for schedule(dynamic, 1)
-                for (long long x = 0; x < (long long)np; ++x) {
-                    PairRec& pr = pairs[x];
-                    host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[pr.spin] + pr.i, f->o_base[pr.spin] + pr.j, G.data());
-                    host_jacobi(N, G.data(), V.data(), sg, order);
-                    int r = 0;
-                    while (r < N && sg[r] > threshold) ++r;
-                    pr.r = r;
-                    snext[x] = r < N ? sg[r] : 0.0;
-                    pS[x].assign(sg.begin(), sg.begin() + r);
-                    pU[x].resize((size_t)r * N);
-                    pW[x].resize((size_t)r * N);
-                    for (int K = 0; K < r; ++K) {
-                        const double* g = &G[(size_t)order[K] * N];
-                        const double inv = 1.0 / sg[K];
-                        for (int e = 0; e < N; ++e) pU[x][(size_t)K * N + e] = g[e] * inv;
-                        std::memcpy(&pW[x][(size_t)K * N], &V[(size_t)order[K] * N], (size_t)N * 8);
+                    for (int x = 0; x < n; ++x) {
+                        host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[spin] + bi[x], f->o_base[spin] + bj[x], G.data());
+                        host_jacobi(N, G.data(), V.data(), sg, order);
+                        std::copy(sg.begin(), sg.end(), hSig.begin() + (size_t)x * N);
+                        int r = 0;
+                        while (r < N && sg[r] > threshold) ++r;
+                        pU[x].resize((size_t)r * N);
+                        pW[x].resize((size_t)r * N);
+                        for (int K = 0; K < r; ++K) {
+                            const double* g = &G[(size_t)order[K] * N];
+                            const double inv = 1.0 / sg[K];
+                            for (int e = 0; e < N; ++e) pU[x][(size_t)K * N + e] = g[e] * inv;
+                            std::memcpy(&pW[x][(size_t)K * N], &V[(size_t)order[K] * N], (size_t)N * 8);
+                        }
                     }
                 }
             }
+            for (int x = 0; x < n; ++x) {
+                const double* sg = &hSig[(size_t)x * N];
+                int r = 0;
+                while (r < N && sg[r] > threshold) ++r;
+                pairs[k0 + x].r = r;
+                pairs[k0 + x].snext = r < N ? sg[r] : 0.0;
+            }
+            table.clear();
+            auto sig = [&](const PairRec& pr, int K) { return hSig[(size_t)pr.x * N + K]; };
+            auto src = [&](const PairRec& pr) { return (long long)pr.x * N; };
+            if (split) layout_block(f, &pairs[k0], &pairs[k0] + n, sig, src, table);
+            else
+                for (size_t bb = blk; bb < blk1; ++bb) layout_block(f, &pairs[bstart[bb]], &pairs[bstart[bb + 1]], sig, src, table);
+            st = grow_pack(f);
+            if (st != LO_OK) break;
+            if (on_gpu) {
+                st = gpu_gather_rows(tU, f->dU, table.data(), (int)table.size(), f->N_pad);
+                if (st == LO_OK) st = gpu_gather_rows(tW, f->dW, table.data(), (int)table.size(), f->N_pad);
+            } else {
+                for (const GatherRec& g : table) {
+                    const int x = (int)(g.src_row / N);
+                    if (device >= 0) {
+                        if (cudaMemcpy2D(f->dU + (size_t)g.dst_row * f->N_pad, (size_t)f->N_pad * 8, pU[x].data(), (size_t)N * 8, (size_t)N * 8, g.r, cudaMemcpyHostToDevice) != cudaSuccess ||
+                            cudaMemcpy2D(f->dW + (size_t)g.dst_row * f->N_pad, (size_t)f->N_pad * 8, pW[x].data(), (size_t)N * 8, (size_t)N * 8, g.r, cudaMemcpyHostToDevice) != cudaSuccess) {
+                            set_error("lo_setup: factor upload failed"); st = LO_ECUDA; break;
+                        }
+                    } else {
+                        for (int K = 0; K < g.r; ++K) {
+                            std::memcpy(&f->hU[(size_t)(g.dst_row + K) * f->N_pad], &pU[x][(size_t)K * N], (size_t)N * 8);
+                            std::memcpy(&f->hW[(size_t)(g.dst_row + K) * f->N_pad], &pW[x][(size_t)K * N], (size_t)N * 8);
+                        }
+                    }
+                }
+            }
+            if (split && k1 < bstart[blk + 1]) { bstart[blk] = k1; }   // rest of the oversized block next time
+            else blk = split ? blk + 1 : blk1;
         }
-        // ---- staging in natural order
-        long long src = 0;
-        for (size_t x = 0; x < np; ++x) { pairs[x].src = src; src += pairs[x].r; }
-        std::vector<double> sU((size_t)src * N), sW((size_t)src * N), sS((size_t)src);
-        for (size_t x = 0; x < np; ++x) {
-            if (pairs[x].r == 0) continue;
-            std::memcpy(&sU[(size_t)pairs[x].src * N], pU[x].data(), pU[x].size() * 8);
-            std::memcpy(&sW[(size_t)pairs[x].src * N], pW[x].data(), pW[x].size() * 8);
-            std::memcpy(&sS[(size_t)pairs[x].src], pS[x].data(), pS[x].size() * 8);
-            std::vector<double>().swap(pU[x]);
-            std::vector<double>().swap(pW[x]);
-        }
-        st = pack_and_upload(f, pairs, sU, sW, sS);
+        if (on_gpu) free_tmp();
+        if (st == LO_OK) st = finish_pack(f);
         if (st != LO_OK) { free_all(f); return st; }
-        size_t off = 0;
-        for (int s = 0; s < n_spin; ++s) {
-            size_t cnt = (size_t)n_occ[s] * (n_occ[s] + 1) / 2;
-            f->sigma_next[s].assign(snext.begin() + off, snext.begin() + off + cnt);
-            off += cnt;
-        }
     } catch (const std::bad_alloc&) {
         set_error("lo_setup: out of host memory");
         free_all(f);
@@ -548,15 +561,8 @@ lo_status lo_factor_pair(const lo_factors* f, int spin, int i, int j, double* U,
     if (U && (st = fetch_rows(f, true, row0, r, U)) != LO_OK) return st;
     if (W && (st = fetch_rows(f, false, row0, r, W)) != LO_OK) return st;
     if (sigma && r > 0) {
-        std::vector<double> w(r);
-        if (f->device >= 0) {
-            CK(cudaSetDevice(f->device));
-            CK(cudaMemcpy(w.data(), f->dWgt + row0, (size_t)r * 8, cudaMemcpyDeviceToHost));
-        } else {
-            std::copy(f->hWgt.begin() + row0, f->hWgt.begin() + row0 + r, w.begin());
-        }
         const double scale = -(f->n_spin == 1 ? 1.0 : 0.5) * (i == j ? 1.0 : 2.0);   // power of two: exact
-        for (int K = 0; K < r; ++K) sigma[K] = w[K] / scale;
+        for (int K = 0; K < r; ++K) sigma[K] = f->hWgt[(size_t)row0 + K] / scale;
     }
     return LO_OK;
 }
@@ -585,46 +591,40 @@ lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
     g->num_sms = f->num_sms; g->setup_on_gpu = f->setup_on_gpu; g->ops = f->ops; g->lbar_bytes = f->lbar_bytes;
     try {
         std::vector<PairRec> pairs;
-        std::vector<double> snext;
-        long long src = 0;
-        std::vector<std::vector<double>> sig;
-        for (int s = 0; s < f->n_spin; ++s) {
-            const int O = f->n_occ[s];
-            size_t k = 0;
-            for (int i = 0; i < O; ++i)
-                for (int j = i; j < O; ++j, ++k) {
-                    const int r0 = f->rank[s][k];
-                    std::vector<double> sg(r0);
-                    lo_status st = lo_factor_pair(f, s, i, j, nullptr, sg.data(), nullptr);
-                    if (st != LO_OK) { free_all(g); return st; }
-                    int r = 0;
-                    while (r < r0 && sg[r] > looser) ++r;
-                    pairs.push_back({s, i, j, r, src});
-                    snext.push_back(r < r0 ? sg[r] : f->sigma_next[s][k]);
-                    src += r;
-                    sg.resize(r);
-                    sig.push_back(std::move(sg));
-                }
-        }
-        std::vector<double> sU((size_t)src * f->N), sW((size_t)src * f->N), sS((size_t)src);
-        for (size_t x = 0; x < pairs.size(); ++x) {
-            const PairRec& pr = pairs[x];
-            if (pr.r == 0) continue;
-            const int O = f->n_occ[pr.spin];
-            const size_t k = (size_t)pr.i * O - (size_t)pr.i * (pr.i - 1) / 2 + (pr.j - pr.i);
-            lo_status st = fetch_rows(f, true, f->row_off[pr.spin][k], pr.r, &sU[(size_t)pr.src * f->N]);
-            if (st == LO_OK) st = fetch_rows(f, false, f->row_off[pr.spin][k], pr.r, &sW[(size_t)pr.src * f->N]);
-            if (st != LO_OK) { free_all(g); return st; }
-            std::copy(sig[x].begin(), sig[x].end(), sS.begin() + pr.src);
-        }
-        lo_status st = pack_and_upload(g, pairs, sU, sW, sS);
+        std::vector<size_t> bstart;
+        enumerate_blocks(g, pairs, bstart);
+        lo_status st = begin_pack(g);
         if (st != LO_OK) { free_all(g); return st; }
-        size_t off = 0;
-        for (int s = 0; s < f->n_spin; ++s) {
-            size_t cnt = f->rank[s].size();
-            g->sigma_next[s].assign(snext.begin() + off, snext.begin() + off + cnt);
-            off += cnt;
+        auto sigma_of = [&](const PairRec& pr, int K) {
+            const double scale = -(f->n_spin == 1 ? 1.0 : 0.5) * (pr.i == pr.j ? 1.0 : 2.0);
+            return f->hWgt[(size_t)pr.src + K] / scale;
+        };
+        for (PairRec& pr : pairs) {
+            const size_t k = pair_index(f->n_occ[pr.spin], pr.i, pr.j);
+            const int r0 = f->rank[pr.spin][k];
+            pr.src = f->row_off[pr.spin][k];
+            int r = 0;
+            while (r < r0 && sigma_of(pr, r) > looser) ++r;
+            pr.r = r;
+            pr.snext = r < r0 ? sigma_of(pr, r) : f->sigma_next[pr.spin][k];
         }
+        std::vector<GatherRec> table;
+        auto src = [&](const PairRec& pr) { return pr.src; };
+        for (size_t blk = 0; blk + 1 < bstart.size(); ++blk) layout_block(g, &pairs[bstart[blk]], &pairs[bstart[blk + 1]], sigma_of, src, table);
+        st = grow_pack(g);
+        if (st == LO_OK) {
+            if (g->device >= 0) {
+                st = gpu_gather_rows(f->dU, g->dU, table.data(), (int)table.size(), g->N_pad);
+                if (st == LO_OK) st = gpu_gather_rows(f->dW, g->dW, table.data(), (int)table.size(), g->N_pad);
+            } else {
+                for (const GatherRec& t : table) {
+                    std::memcpy(&g->hU[(size_t)t.dst_row * g->N_pad], &f->hU[(size_t)t.src_row * g->N_pad], (size_t)t.r * g->N_pad * 8);
+                    std::memcpy(&g->hW[(size_t)t.dst_row * g->N_pad], &f->hW[(size_t)t.src_row * g->N_pad], (size_t)t.r * g->N_pad * 8);
+                }
+            }
+        }
+        if (st == LO_OK) st = finish_pack(g);
+        if (st != LO_OK) { free_all(g); return st; }
     } catch (const std::bad_alloc&) {
         set_error("lo_retruncate: out of host memory");
         free_all(g);

@@ -46,6 +46,23 @@ struct SharedOps {
     ~SharedOps();
 };
 
+// Growable device array over one contiguous virtual address range (lo_mem.cu).
+struct GrowBuf {
+    void* base = nullptr;
+    size_t reserved = 0, mapped = 0, chunk = 0;
+    int device = -1;
+    std::vector<unsigned long long> handles;   // CUmemGenericAllocationHandle of every mapped chunk
+    lo_status reserve(int device, size_t max_bytes);
+    lo_status ensure(size_t bytes);            // map (zero-filled) physical memory so that [0, bytes) is usable
+    void release();
+};
+
+// One row-block copy of the packing step: r rows of N_pad doubles from src_row to dst_row.
+struct GatherRec {
+    long long src_row, dst_row;
+    int r, pad_;
+};
+
 struct TimingEvent {
     cudaEvent_t e0, e1;
     int kind;
@@ -64,10 +81,11 @@ struct lo_factors {
     std::vector<double> sigma_next[2];   // first discarded singular value of the pair (0 if none); for the truncation bound
     long long rows = 0;                  // packed rows incl. per-pair padding (without slack)
     long long n_tiles = 0;
-    // host copies of the packed arrays (kept only for host-only sets)
+    // host copies: hU/hW only for host-only sets (device < 0); hWgt (weights incl. sigma) always
     std::vector<double> hU, hW, hWgt;
     std::vector<lo::ExTile> hTiles;
     // device factor set
+    lo::GrowBuf bU, bW;                  // backing store of dU / dW
     double *dU = nullptr, *dW = nullptr, *dWgt = nullptr;
     lo::ExTile* dTiles = nullptr;
     CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
@@ -107,6 +125,8 @@ lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner,
 lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV,
                        double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma);
 size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad);
+// dst[rec.dst_row + K][:] = src[rec.src_row + K][:] for K < rec.r, every rec of the host table (rows of N_pad doubles).
+lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table, int n, int N_pad);
 
 // microbenchmarks (lo_peak.cu)
 lo_status measure_peak(int device, int kind, double* value);

@@ -179,7 +179,32 @@ __global__ void __launch_bounds__(512) k_svd_finish(const double* __restrict__ G
     }
 }
 
+// packing: copy row blocks (whole rows of N_pad doubles, 16-byte vectors) according to a table
+__global__ void __launch_bounds__(256) k_gather_rows(const double2* __restrict__ src, double2* __restrict__ dst, const GatherRec* __restrict__ table,
+                                                     int half_pad) {
+    const GatherRec rec = table[blockIdx.x];
+    const double2* s = src + (size_t)rec.src_row * half_pad;
+    double2* d = dst + (size_t)rec.dst_row * half_pad;
+    const size_t n = (size_t)rec.r * half_pad;
+    for (size_t e = threadIdx.x; e < n; e += 256) d[e] = s[e];
+}
+
 }  // namespace
+
+lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table, int n, int N_pad) {
+    if (n <= 0) return LO_OK;
+    GatherRec* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, (size_t)n * sizeof(GatherRec));
+    if (e == cudaSuccess) e = cudaMemcpy(d, table, (size_t)n * sizeof(GatherRec), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_gather_rows<<<n, 256>>>(reinterpret_cast<const double2*>(src), reinterpret_cast<double2*>(dst), d, N_pad / 2);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (d) cudaFree(d);
+    if (e != cudaSuccess) { set_error(std::string("gpu_gather_rows: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    return LO_OK;
+}
 
 size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad) { return (size_t)4 * N * N_pad * 8 + (size_t)N * 12; }
 

@@ -34,6 +34,21 @@ def oracle_energy(P, F, phis, idx=None):
     return oracle.local_energy_lo(P.psi, [a for a, _ in hr], [b for _, b in hr], oracle_factor_sets(P, F), sel)
 
 
+def oracle_energy_streamed(P, F, phis, idx, chunk=128):
+    """Protocol (A) for factor sets too large to copy to the host in one piece: the oracle's exchange sum is
+    accumulated over chunks of pairs fetched from the library (lo_factor_pair)."""
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+
+    def fetch(spin, k0, k1):
+        r, U, sg, W = F.factor_range(spin, k0, k1)
+        pi, pj = oracle.all_pairs(P.n_occ[spin])
+        return oracle.make_factor_set(P.N, P.n_occ[spin], pi[k0:k1], pj[k0:k1], r, U, sg, W)
+
+    n_pairs = [o * (o + 1) // 2 for o in P.n_occ]
+    E, st, _ = oracle.local_energy_lo_streamed(P.psi, [a for a, _ in hr], [b for _, b in hr], [p[idx] for p in phis], n_pairs, fetch, chunk)
+    return E, st
+
+
 def gpu_energy(F, phis):
     torch = torch_cuda()
     d = [torch.from_numpy(np.ascontiguousarray(p)).cuda() for p in phis]
@@ -270,3 +285,43 @@ def test_c2_full_size_sampled_walkers():
         nrm = np.linalg.norm(th, axis=0)
         ek = oracle.exchange_cholesky(Lbar, th)
         assert abs(Eg[w, 3] - ek) <= 1e-5 * (m * nrm[pi] * nrm[pj]).sum() + 1e-10 * abs(ek)
+
+
+def test_c3_full_size_unrestricted_sampled_walkers():
+    """BASELINE.json:configs[3] (open-shell metallocene-sized, N=500, 65 alpha + 63 beta, N_chol=2500, T=1e-5): all
+    1024 walkers on the GPU, 16 seeded walkers checked one by one by the oracle on the library's factor set (exchange
+    streamed in chunks of pairs: the 2 x 8 GB of factors do not need to sit on the host at once)."""
+    P = gen.make_problem(3)
+    phis = gen.make_walkers(P)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-5, device=0, max_walkers=P.n_w, gpu_svd=True)
+    info = F.info()
+    assert tuple(info.n_pairs) == (65 * 66 // 2, 63 * 64 // 2) and info.n_spin == 2
+    Eg, st = gpu_energy(F, phis)
+    assert (st == 0).all() and np.isfinite(Eg).all()
+    idx = np.sort(np.random.default_rng(3).choice(P.n_w, 16, replace=False))
+    Eo, so = oracle_energy_streamed(P, F, phis, idx)
+    assert (so == 0).all()
+    assert_parity(Eg[idx], Eo)
+
+
+def test_c4_full_size_sampled_walkers_and_retruncation():
+    """BASELINE.json:configs[4] (3D cage, N=700, N_occ=130, N_chol=3500, 2048 walkers): factor set built once at the
+    loosest threshold of the sweep that the test affords in time (T=1e-3 from a 1e-3 build; the full sweep 1e-3..1e-6 is
+    `bench.py --config 4 --sweep`), all 2048 walkers on the GPU, 16 seeded walkers checked by the oracle on the
+    library's factors; then a re-truncated (looser) set is checked the same way on 4 walkers."""
+    P = gen.make_problem(4)
+    phis = gen.make_walkers(P)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-3, device=0, max_walkers=P.n_w, gpu_svd=True)
+    info = F.info()
+    assert info.n_pairs[0] == 130 * 131 // 2 and info.max_rank <= 700
+    Eg, st = gpu_energy(F, phis)
+    assert (st == 0).all() and np.isfinite(Eg).all()
+    idx = np.sort(np.random.default_rng(4).choice(P.n_w, 16, replace=False))
+    Eo, so = oracle_energy_streamed(P, F, phis, idx)
+    assert (so == 0).all()
+    assert_parity(Eg[idx], Eo)
+    F2 = F.retruncate(1e-2)
+    assert F2.info().sum_rank[0] < info.sum_rank[0]
+    Eg2, _ = gpu_energy(F2, phis)
+    Eo2, _ = oracle_energy_streamed(P, F2, phis, idx[:4])
+    assert_parity(Eg2[idx[:4]], Eo2)

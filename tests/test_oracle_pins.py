@@ -301,3 +301,24 @@ def test_golden_c0_regression(c0, c0_walkers):
         e = exact(c0, c0_walkers, w, "cholesky")
         got = np.array([x for z in e for x in (z.real, z.imag)])
         assert np.abs(got - ref[w]).max() <= 1e-11 * np.abs(ref[w]).max()
+
+
+def test_streamed_evaluation_equals_one_piece(c1, c1_walkers):
+    """local_energy_lo_streamed (chunks of pairs, used for the factor sets too large for the host) adds up to
+    local_energy_lo on the same factors."""
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, c1.psi[0])
+    pi, pj = oracle.all_pairs(c1.n_occ[0])
+    sel = np.arange(0, len(pi), 7)
+    Ut, s, Wt = oracle.full_svd_pairs(Lbar, pi[sel], pj[sel])
+    fs = oracle.truncate(c1.N, c1.n_occ[0], pi[sel], pj[sel], Ut, s, Wt, 1e-2)
+    phis = [c1_walkers[0][:5]]
+    E, st = oracle.local_energy_lo(c1.psi, [Lbar], [hbar], [fs], phis)
+
+    def fetch(spin, k0, k1):
+        r = fs.r[k0:k1]
+        a, b = int(fs.off[k0]), int(fs.off[k0] + r.sum())
+        return oracle.make_factor_set(c1.N, c1.n_occ[0], fs.pi[k0:k1], fs.pj[k0:k1], r, fs.U[a:b], fs.sigma[a:b], fs.W[a:b])
+
+    Es, sts, secs = oracle.local_energy_lo_streamed(c1.psi, [Lbar], [hbar], phis, [len(sel)], fetch, chunk=5)
+    assert (st == 0).all() and (sts == 0).all() and secs > 0
+    assert np.abs(Es - E).max() <= 1e-12 * np.abs(E[:, 0]).max()
