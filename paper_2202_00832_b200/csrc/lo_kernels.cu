@@ -27,9 +27,15 @@ namespace lo {
 namespace {
 
 __device__ __forceinline__ void mma884(double& c0, double& c1, double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
-
+// Stage release must not overtake the stage's shared-memory reads.  ptxas is free to sink register-only MMAs below the
+// mbarrier arrive, and then the last ld.shared of a stage can still be in flight when the arrive issues (the arrive goes
+// through the SYNCS unit, not the load pipe) and the producer's TMA refill (async proxy) can land first -- seen as rare
+// wrong rows of X at configs[3].  release_stage() is the documented ordering for generic-proxy reads followed by an
+// async-proxy overwrite: fence.proxy.async (SASS: MEMBAR.ALL.CTA + FENCE.VIEW.ASYNC, waits for the warp's outstanding
+// loads), then the arrive.  It is issued right after the LAST fragment loads of a stage and before their MMAs, so the
+// wait overlaps the MMAs still queued on the tensor pipe.
 // ---- TMA + mbarrier plumbing (cp.async.bulk.tensor; SASS: UTMALDG / SYNCS)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -41,6 +47,11 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
+__device__ __forceinline__ void release_stage(uint32_t empty_bar, int lane) {
+    fence_proxy_async();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty_bar);
+}
 // Warp-specialised register budget (setmaxnreg, per warpgroup): the kernels launch 3 warpgroups at 168 registers per
 // thread; the producer warpgroup shrinks to 40, the two consumer warpgroups grow to 232 (4*32*40 + 8*32*232 = 64512).
 __device__ __forceinline__ void reg_dec_producer() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
@@ -387,13 +398,12 @@ __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUte
                 for (int mf = 0; mf < 8; ++mf) a[mf] = lds_f64(st + a_row + mf * 1024 + xo[ks]);
 #pragma unroll
                 for (int nf = 0; nf < 4; ++nf) b[nf] = lds_f64(st + b_row + nf * 1024 + xo[ks]);
+                if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
 #pragma unroll
                 for (int mf = 0; mf < 8; ++mf)
 #pragma unroll
                     for (int nf = 0; nf < 4; ++nf) mma884(acc[mf][nf][0], acc[mf][nf][1], a[mf], b[nf]);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty + 8 * cslot);
             if (++cslot == CO_STAGES) { cslot = 0; cphase ^= 1; }
         }
         double* Xs = Xpart + (size_t)it.sp * Xp * ldw;
@@ -531,31 +541,35 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
         for (int kt = 0; kt < KT; ++kt) {
             if (kt) mbar_wait(full + 8 * cslot, cphase);
             const uint32_t st = sbase + cslot * EX_STAGE_BYTES;
+            if (nvalid > 0) {           // warp-uniform; a warp whose 32 rows are all padding only releases the stage
 #pragma unroll
-            for (int ks = 0; ks < KTILE / 4; ++ks) {
-                double a[4], w[4], bj[4], bi[4];
+                for (int ks = 0; ks < KTILE / 4; ++ks) {
+                    double a[4], w[4], bj[4], bi[4];
 #pragma unroll
-                for (int mf = 0; mf < 4; ++mf) {
-                    a[mf] = lds_f64(st + u_row + mf * 1024 + xo[ks]);
-                    w[mf] = lds_f64(st + w_row + mf * 1024 + xo[ks]);
-                }
-#pragma unroll
-                for (int nf = 0; nf < 4; ++nf) {
-                    bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
-                    bi[nf] = lds_f64(st + ti_row + nf * 1024 + xo[ks]);
-                }
-#pragma unroll
-                for (int mf = 0; mf < 4; ++mf)
-                    if (mf < nvalid) {
-#pragma unroll
-                        for (int nf = 0; nf < 4; ++nf) {
-                            mma884(accA[mf][nf][0], accA[mf][nf][1], a[mf], bj[nf]);
-                            mma884(accB[mf][nf][0], accB[mf][nf][1], w[mf], bi[nf]);
-                        }
+                    for (int mf = 0; mf < 4; ++mf) {
+                        a[mf] = lds_f64(st + u_row + mf * 1024 + xo[ks]);
+                        w[mf] = lds_f64(st + w_row + mf * 1024 + xo[ks]);
                     }
+#pragma unroll
+                    for (int nf = 0; nf < 4; ++nf) {
+                        bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
+                        bi[nf] = lds_f64(st + ti_row + nf * 1024 + xo[ks]);
+                    }
+                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
+#pragma unroll
+                    for (int mf = 0; mf < 4; ++mf)
+                        if (mf < nvalid) {
+#pragma unroll
+                            for (int nf = 0; nf < 4; ++nf) {
+                                mma884(accA[mf][nf][0], accA[mf][nf][1], a[mf], bj[nf]);
+                                mma884(accB[mf][nf][0], accB[mf][nf][1], w[mf], bi[nf]);
+                            }
+                        }
+                }
+            } else {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + 8 * cslot);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty + 8 * cslot);
             if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
         }
         // fused epilogue: e[w] = sum over this lane's rows of weight * a * b (complex), then over the 8 row groups of

@@ -65,6 +65,26 @@ def assert_parity(Eg, Eo, tol=TOL):
     assert np.abs(Eg[:, 0] - Eg[:, 1:].sum(axis=1)).max() <= 1e-12 * np.abs(Eg).max()
 
 
+def assert_all_walkers(P, F, phis, Eg, stride=1):
+    """Properties that hold at any size, on walkers the sampled oracle check does not visit: (i) repeated calls and
+    the host-buffer variant are bitwise equal on EVERY walker and every part (fixed-order reductions; this is what
+    exposes a pipeline race), (ii) E1 and E_J of every stride-th walker against the oracle (Theta, one-body, Cholesky
+    Coulomb: cheap enough for whole batches), E_L = E1 + E_J + E_K on all."""
+    torch = torch_cuda()
+    for _ in range(2):
+        E2, _ = gpu_energy(F, phis)
+        assert np.array_equal(E2, Eg), "repeated call differs on walkers %s" % np.nonzero((E2 != Eg).any(axis=1))[0][:8]
+    Eh, sh = F.local_energy_host([torch.from_numpy(np.ascontiguousarray(p)).pin_memory() for p in phis])
+    assert np.array_equal(Eh, Eg), "host-buffer variant differs on walkers %s" % np.nonzero((Eh != Eg).any(axis=1))[0][:8]
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+    empty = [oracle.empty_factor_set(P.N, o) for o in P.n_occ]
+    sel = [p[::stride] for p in phis]
+    Eo, _ = oracle.local_energy_lo(P.psi, [a for a, _ in hr], [b for _, b in hr], empty, sel)
+    scale = np.abs(Eg[::stride, 0:1])
+    err = np.abs(Eg[::stride, 1:3] - Eo[:, 1:3]) / scale
+    assert err.max() <= TOL, "E1/E_J of all walkers: max rel err %s at walker %d" % (err.max(axis=0), stride * int(err.max(axis=1).argmax()))
+
+
 # ------------------------------------------------------------------------------------------ C0, C1: every walker
 @pytest.mark.parametrize("gpu_svd", [False, True])
 def test_c0_all_walkers(c0, gpu_svd):
@@ -276,6 +296,7 @@ def test_c2_full_size_sampled_walkers():
     idx = np.random.default_rng(2).choice(P.n_w, 24, replace=False)
     Eo, _ = oracle_energy(P, F, phis, idx)
     assert_parity(Eg[idx], Eo)
+    assert_all_walkers(P, F, phis, Eg)
     # exact Cholesky-route exchange for two walkers: inside the truncation bound
     Lbar, _ = oracle.half_rotate(P.L, P.h, P.psi[0])
     pi, pj = oracle.all_pairs(73)
@@ -302,6 +323,7 @@ def test_c3_full_size_unrestricted_sampled_walkers():
     Eo, so = oracle_energy_streamed(P, F, phis, idx)
     assert (so == 0).all()
     assert_parity(Eg[idx], Eo)
+    assert_all_walkers(P, F, phis, Eg)
 
 
 def test_c4_full_size_sampled_walkers_and_retruncation():
@@ -320,6 +342,7 @@ def test_c4_full_size_sampled_walkers_and_retruncation():
     Eo, so = oracle_energy_streamed(P, F, phis, idx)
     assert (so == 0).all()
     assert_parity(Eg[idx], Eo)
+    assert_all_walkers(P, F, phis, Eg, stride=4)
     F2 = F.retruncate(1e-2)
     assert F2.info().sum_rank[0] < info.sum_rank[0]
     Eg2, _ = gpu_energy(F2, phis)
