@@ -245,6 +245,97 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json:configs[4] threshold sweep: the factor set is built ONCE at the tightest threshold (device SVD) and
+    re-truncated (prefix truncation, lo_retruncate) to each looser one; per threshold one JSON line with sum r_ij,
+    factor bytes, compression, E_K error against the exact full-ERI/Cholesky exchange (oracle, a few walkers), the
+    truncation bound (R5) and throughput.  Not the default bench line; one GPU."""
+    import concurrent.futures as cf
+
+    import torch
+
+    import gen
+    import oracle
+    import paper_2202_00832_b200 as lo
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    cfg, reading = args.config, args.reading
+    spec = gen.CONFIGS[cfg]
+    Ts = sorted(spec.thresholds if args.threshold is None else [args.threshold])
+    n_w = args.walkers or spec.n_w
+    P = gen.make_problem(cfg, reading=reading)
+    phis = gen.make_walkers(P, n_w)
+    dphi = [torch.from_numpy(p).cuda() for p in phis]
+    t0 = time.time()
+    F0 = lo.Factors.setup(P.h, P.L, P.psi, Ts[0], device=0, max_walkers=n_w, gpu_svd=True)
+    setup_s = time.time() - t0
+    peak = max(lo.measure_peak("dmma", 0), lo.measure_peak("dfma", 0))
+    # exact exchange (Eq. 16, oracle O2) and the norms of the R5 bound for a few seeded walkers
+    idx = np.sort(np.random.default_rng(P.seed).choice(n_w, min(args.sweep_exact_walkers, n_w), replace=False))
+    hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
+    cK = 1.0 if P.n_spin == 1 else 0.5
+
+    def exact_one(w):
+        ek, nrm = 0.0, []
+        for s in range(P.n_spin):
+            th, _, _ = oracle.theta(P.psi[s], phis[s][w])
+            ek += cK * oracle.exchange_cholesky(hr[s][0], th)
+            nrm.append(np.linalg.norm(th, axis=0))
+        return ek, nrm
+
+    t0 = time.time()
+    with cf.ThreadPoolExecutor(max_workers=max(1, len(idx))) as ex:
+        exact = list(ex.map(exact_one, idx))
+    exact_s = time.time() - t0
+    rows = []
+    for T in Ts:
+        F = F0 if T == Ts[0] else F0.retruncate(T)
+        info = F.info()
+        fl = F.flops_per_walker()
+        for _ in range(max(args.warmup, 3)):
+            out = F.local_energy(dphi, parts=True)
+        torch.cuda.synchronize()
+        F.timing_enable(True)
+        F.timing_get()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(args.steps):
+            out = F.local_energy(dphi, parts=True)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1) / args.steps
+        tm = F.timing_get()
+        F.timing_enable(False)
+        EK = out[3].cpu().numpy()
+        ex_ms = tm["exchange"][0] / max(tm["exchange"][1], 1)
+        errs, bounds = [], []
+        for (ek, nrm), w in zip(exact, idx):
+            errs.append(abs(EK[w] - ek))
+            b = 0.0
+            for s in range(P.n_spin):
+                pi, pj = oracle.all_pairs(P.n_occ[s])
+                m = np.where(pi == pj, 1.0, 2.0)
+                b += cK * T * float((m * nrm[s][pi] * nrm[s][pj]).sum())
+            bounds.append(b)
+        sum_r = int(sum(info.sum_rank))
+        row = {"sweep": workload_name(cfg, reading, T, n_w), "T_SVD": T, "sum_rank": sum_r, "min_rank": info.min_rank,
+               "max_rank": info.max_rank, "compression_pct": round(100 * (1 - sum_r / (sum(info.n_pairs) * info.N)), 2),
+               "factor_bytes": int(info.factor_bytes), "EK_abs_err_vs_exact_max": float(max(errs)),
+               "EK_abs_err_vs_exact_mean": float(np.mean(errs)), "EK_exact_abs_mean": float(np.mean([abs(e) for e, _ in exact])),
+               "R5_bound_min": float(min(bounds)), "exact_walkers": [int(w) for w in idx],
+               "ms_per_step": round(ms, 3), "energies_per_s": round(n_w / (ms * 1e-3), 2),
+               "tflops": round(sum(fl.values()) * n_w / (ms * 1e-3) * 1e-12, 3), "exchange_ms": round(ex_ms, 3),
+               "exchange_tflops": round(fl["exchange"] * n_w / (ex_ms * 1e-3) * 1e-12, 3) if ex_ms > 0 else 0.0,
+               "exchange_frac_of_peak": round(fl["exchange"] * n_w / (ex_ms * 1e-3) * 1e-12 / peak, 4) if ex_ms > 0 else 0.0,
+               "peak_tflops": round(peak, 3), "setup_s_tightest": round(setup_s, 1), "oracle_exact_s": round(exact_s, 1)}
+        print(json.dumps(row), flush=True)
+        rows.append(row)
+        if F is not F0:
+            F.free()
+    F0.free()
+
+
 def run_reference(args):
     """The CPU oracle, as it stands, end to end on its OWN factors.  Its pair SVDs at the pentacene size take ~2 s per
     pair per core, so the exchange is timed on a seeded, |i-j|-stratified subset of pairs and the exchange time is
@@ -313,8 +404,14 @@ def main():
     ap.add_argument("--cpu-walkers", type=int, default=192, help="walkers of the batch the oracle is timed on (cpu_baseline)")
     ap.add_argument("--ref-walkers", type=int, default=32)
     ap.add_argument("--ref-pairs", type=int, default=128)
+    ap.add_argument("--sweep", action="store_true", help="threshold sweep (BASELINE.json:configs[4]): one JSON line per threshold")
+    ap.add_argument("--sweep-exact-walkers", type=int, default=4, help="walkers whose exact E_K the oracle computes in --sweep")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        if args.config == 2 and "--config" not in " ".join(sys.argv):
+            args.config = 4
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -286,6 +286,8 @@ lo_status finish_pack(lo_factors* f) {
     if (!f->hTiles.empty()) CK(cudaMemcpy(f->dTiles, f->hTiles.data(), f->hTiles.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
     st = make_tmap(&f->tmU, f->dU, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmW, f->dW, f->N_pad, rows_alloc, EX_BM);
+    if (st == LO_OK) st = make_tmap(&f->tmU8, f->dU, f->N_pad, rows_alloc, 8);
+    if (st == LO_OK) st = make_tmap(&f->tmW8, f->dW, f->N_pad, rows_alloc, 8);
     if (st != LO_OK) return st;
     return alloc_workspace(f);
 }

@@ -89,6 +89,7 @@ struct lo_factors {
     double *dU = nullptr, *dW = nullptr, *dWgt = nullptr;
     lo::ExTile* dTiles = nullptr;
     CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
+    CUtensorMap tmU8, tmW8;              // same arrays, boxes 8 x 16 (one row fragment): tiles shorter than 64 rows
     std::shared_ptr<lo::SharedOps> ops;
     // workspace
     double* dThT = nullptr;       // [O_tot][ldw][N_pad]

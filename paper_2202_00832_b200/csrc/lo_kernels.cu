@@ -92,64 +92,65 @@ __device__ __forceinline__ uint32_t frag_off(int g, int t, int s) {
 }
 
 // ------------------------------------------------------------------------------------------------ S1: overlap
-// One CTA per walker.  Thread micro-tile 4x4 of A; Psi/Phi rows staged through shared memory 8 rows at a time.
-constexpr int OV_PC = 8;
+// A_w[i][j] = sum_p Psi[p][i] Phi_w[p][j]  as a real GEMM on the DMMA pipe: M = i (block of 32 per CTA), N = (j, re/im)
+// = the 2*O interleaved doubles of a Phi row, K = p.  grid (ceil(O/32), n_w), 8 warps; warp w owns column fragments
+// w, w+8, ... (NFW of them) and all 4 row fragments.  Psi / Phi rows are staged OV_PC at a time through shared memory;
+// both operands are stored with k (= p) as the slow index, so a fragment load reads 8 consecutive doubles of 4 rows and
+// a leading dimension = 4 (mod 16) doubles keeps the 16 lanes of a half-warp on distinct 8-byte banks.
+constexpr int OV_PC = 32;
+constexpr int OV_LDA = 36;
+constexpr int OV_NFB = 64;   // column fragments per CTA (grid.z blocks of 512 real columns = 256 orbitals)
+__host__ __device__ inline int ov_ldb(int O) { int nf8 = min((2 * O + 7) / 8, OV_NFB) * 8; return nf8 + ((4 - nf8 % 16) + 16) % 16; }
+
+template <int NFW>
 __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi, const double2* __restrict__ phi, double2* __restrict__ A,
                                                  int N, int O) {
     extern __shared__ __align__(16) double sm[];
-    const int Op = (O + 3) & ~3;
-    double* psi_s = sm;                                       // [OV_PC][Op]
-    double2* phi_s = reinterpret_cast<double2*>(sm + OV_PC * Op);  // [OV_PC][Op]
-    const int w = blockIdx.x, tid = threadIdx.x;
-    const double2* phw = phi + (size_t)w * N * O;
-    const int nt = Op / 4, ntile = nt * nt;
-    for (int base = 0; base < ntile; base += 256) {
-        const int id = base + tid;
-        const bool valid = id < ntile;
-        const int ti = valid ? id / nt : 0, tj = valid ? id % nt : 0;
-        double2 acc[4][4];
+    const int LDB = ov_ldb(O), nf0 = blockIdx.z * OV_NFB, NF = min((2 * O + 7) / 8 - nf0, OV_NFB), c0 = nf0 * 8;
+    double* As = sm;                   // [OV_PC][OV_LDA]
+    double* Bs = sm + OV_PC * OV_LDA;  // [OV_PC][LDB]
+    const int i0 = blockIdx.x * 32, w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    const double* phw = reinterpret_cast<const double*>(phi + (size_t)w * N * O);
+    const int O2 = 2 * O, ncb = NF * 8;
+    double acc[4][NFW][2];
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+    for (int a = 0; a < 4; ++a)
 #pragma unroll
-            for (int b = 0; b < 4; ++b) acc[a][b] = make_double2(0.0, 0.0);
-        for (int p0 = 0; p0 < N; p0 += OV_PC) {
-            __syncthreads();
-            for (int e = tid; e < OV_PC * Op; e += 256) {
-                int pp = e / Op, c = e % Op, p = p0 + pp;
-                bool in = (p < N) && (c < O);
-                psi_s[e] = in ? psi[(size_t)p * O + c] : 0.0;
-                phi_s[e] = in ? phw[(size_t)p * O + c] : make_double2(0.0, 0.0);
-            }
-            __syncthreads();
-            if (valid) {
-#pragma unroll
-                for (int pp = 0; pp < OV_PC; ++pp) {
-                    double ps[4];
-                    double2 ph[4];
-#pragma unroll
-                    for (int a = 0; a < 4; ++a) ps[a] = psi_s[pp * Op + ti * 4 + a];
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) ph[b] = phi_s[pp * Op + tj * 4 + b];
-#pragma unroll
-                    for (int a = 0; a < 4; ++a)
-#pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            acc[a][b].x = fma(ps[a], ph[b].x, acc[a][b].x);
-                            acc[a][b].y = fma(ps[a], ph[b].y, acc[a][b].y);
-                        }
-                }
-            }
+        for (int b = 0; b < NFW; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    for (int p0 = 0; p0 < N; p0 += OV_PC) {
+        __syncthreads();
+        for (int e = tid; e < OV_PC * 32; e += 256) {
+            const int pp = e >> 5, c = e & 31, pg = p0 + pp;
+            As[pp * OV_LDA + c] = (pg < N && i0 + c < O) ? psi[(size_t)pg * O + i0 + c] : 0.0;
         }
-        if (valid) {
+        for (int e = tid; e < OV_PC * ncb; e += 256) {
+            const int pp = e / ncb, c = e - pp * ncb, pg = p0 + pp;
+            Bs[pp * LDB + c] = (pg < N && c0 + c < O2) ? phw[(size_t)pg * O2 + c0 + c] : 0.0;
+        }
+        __syncthreads();
 #pragma unroll
-            for (int a = 0; a < 4; ++a)
+        for (int ks = 0; ks < OV_PC / 4; ++ks) {
+            double a[4], b[NFW];
 #pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    int i = ti * 4 + a, j = tj * 4 + b;
-                    if (i < O && j < O) A[((size_t)w * O + i) * O + j] = acc[a][b];
-                }
+            for (int mf = 0; mf < 4; ++mf) a[mf] = As[(ks * 4 + t) * OV_LDA + mf * 8 + g];
+#pragma unroll
+            for (int j = 0; j < NFW; ++j) {
+                const int nf = min(warp + 8 * j, NF - 1);
+                b[j] = Bs[(ks * 4 + t) * LDB + nf * 8 + g];
+            }
+#pragma unroll
+            for (int mf = 0; mf < 4; ++mf)
+#pragma unroll
+                for (int j = 0; j < NFW; ++j) mma884(acc[mf][j][0], acc[mf][j][1], a[mf], b[j]);
         }
     }
+#pragma unroll
+    for (int mf = 0; mf < 4; ++mf)
+#pragma unroll
+        for (int j = 0; j < NFW; ++j) {
+            const int nf = warp + 8 * j, i = i0 + mf * 8 + g, jo = (nf0 + nf) * 4 + t;
+            if (nf < NF && i < O && jo < O) A[((size_t)w * O + i) * O + jo] = make_double2(acc[mf][j][0], acc[mf][j][1]);
+        }
 }
 
 // ------------------------------------------------------------------------------------------------ S1: inverse
@@ -168,80 +169,110 @@ __device__ __forceinline__ double2 crecip(double2 a) {
 // In-place Gauss-Jordan inversion with partial (row) pivoting.  One CTA per walker; the O x O complex matrix
 // lives in shared memory (IN_SMEM) or is updated in place in the global workspace (L2 resident) when it does
 // not fit.  status[w] = 1 and A^-1 = NaN when a pivot is zero / non-finite.
+// Step k (3 barriers): (1) warp 0 finds the pivot of column k among rows k..O-1 (largest |.|^2, lowest row on ties) and
+// publishes the row, the pivot value and the singular flag; (2) rows k and piv are exchanged while the new row k is
+// scaled by 1/pivot (copy kept in rowk), column k is saved in colk -- nobody writes column k in this phase; (3) every
+// other row r gets M[r][c] -= colk[r] * rowk[c], and column k becomes -colk[r]/pivot (1/pivot on the diagonal).
+// Threads form a 16 x 16 grid over (row, column) so that the update reads each rowk / colk entry once per thread.
+constexpr int INV_CT = 9;   // register-cached rowk entries per thread: covers O <= 144
 template <bool IN_SMEM>
 __global__ void __launch_bounds__(256) k_inverse(double2* __restrict__ Aws, int* __restrict__ status, int O) {
     extern __shared__ __align__(16) double sm[];
-    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, tx = tid & 15, ty = tid >> 4;
     double2* Ag = Aws + (size_t)w * O * O;
     double2* colk = reinterpret_cast<double2*>(sm);              // [O]
-    int* perm = reinterpret_cast<int*>(colk + O);                // [O] padded to a multiple of 4
-    double* red_v = reinterpret_cast<double*>(perm + ((O + 3) & ~3));  // [8]
-    int* red_i = reinterpret_cast<int*>(red_v + 8);              // [8] (+ [8] = pivot row broadcast, [9] = singular flag)
-    double2* M = IN_SMEM ? reinterpret_cast<double2*>(red_i + 16) : Ag;
+    double2* rowk = colk + O;                                    // [O]
+    double2* pvs = rowk + O;                                     // [1] pivot value
+    int* perm = reinterpret_cast<int*>(pvs + 1);                 // [O] padded to a multiple of 4
+    int* ctl = perm + ((O + 3) & ~3);                            // [0] pivot row, [1] singular flag (+2 pad)
+    double2* M = IN_SMEM ? reinterpret_cast<double2*>(ctl + 4) : Ag;
     const int OO = O * O;
     if (IN_SMEM) {
         for (int e = tid; e < OO; e += 256) M[e] = Ag[e];
     }
-    if (tid == 0) red_i[9] = 0;
+    if (tid == 0) ctl[1] = 0;
     __syncthreads();
+    const bool cached = O <= 16 * INV_CT;
     for (int k = 0; k < O; ++k) {
-        // pivot search in column k, rows k..O-1
-        double best = -1.0;
-        int bi = k;
-        for (int r = k + tid; r < O; r += 256) {
-            double2 v = M[r * O + k];
-            double m = v.x * v.x + v.y * v.y;
-            if (!(m == m)) m = INFINITY;   // NaN -> treated as non-finite pivot
-            if (m > best) { best = m; bi = r; }
-        }
+        if (warp == 0) {
+            double best = -1.0;
+            int bi = k;
+            for (int r = k + lane; r < O; r += 32) {
+                double2 v = M[r * O + k];
+                double m = v.x * v.x + v.y * v.y;
+                if (!(m == m)) m = INFINITY;   // NaN -> treated as non-finite pivot
+                if (m > best) { best = m; bi = r; }
+            }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            double ob = __shfl_xor_sync(0xffffffffu, best, o);
-            int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
-        }
-        if (lane == 0) { red_v[warp] = best; red_i[warp] = bi; }
-        __syncthreads();
-        if (tid == 0) {
-            double b = red_v[0];
-            int i = red_i[0];
-            for (int q = 1; q < 8; ++q)
-                if (red_v[q] > b || (red_v[q] == b && red_i[q] < i)) { b = red_v[q]; i = red_i[q]; }
-            red_i[8] = i;
-            perm[k] = i;
-            if (!(b > 1e-300) || isinf(b)) red_i[9] = 1;
-        }
-        __syncthreads();
-        const int piv = red_i[8];
-        if (red_i[9]) break;   // uniform
-        if (piv != k) {
-            for (int c = tid; c < O; c += 256) {
-                double2 a = M[k * O + c], b = M[piv * O + c];
-                M[k * O + c] = b;
-                M[piv * O + c] = a;
+            for (int o = 16; o > 0; o >>= 1) {
+                double ob = __shfl_xor_sync(0xffffffffu, best, o);
+                int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+            }
+            if (lane == 0) {
+                ctl[0] = bi;
+                perm[k] = bi;
+                pvs[0] = M[bi * O + k];
+                if (!(best > 1e-300) || isinf(best)) ctl[1] = 1;
             }
         }
         __syncthreads();
-        const double2 inv = crecip(M[k * O + k]);
-        __syncthreads();
-        for (int r = tid; r < O; r += 256) {
-            colk[r] = M[r * O + k];
-            M[r * O + k] = (r == k) ? make_double2(1.0, 0.0) : make_double2(0.0, 0.0);
+        if (ctl[1]) break;   // uniform
+        const int piv = ctl[0];
+        const double2 inv = crecip(pvs[0]);
+        for (int c = tid; c < O; c += 256) {
+            // column k of the exchanged matrix (read only here), then rows k / piv without their column-k entries
+            colk[c] = M[(c == k ? piv : (c == piv ? k : c)) * O + k];
+            if (c != k) {
+                const double2 a = M[piv * O + c], b = M[k * O + c];
+                const double2 ak = cmul(a, inv);
+                rowk[c] = ak;
+                M[k * O + c] = ak;
+                if (piv != k) M[piv * O + c] = b;
+            }
         }
         __syncthreads();
-        for (int c = tid; c < O; c += 256) M[k * O + c] = cmul(M[k * O + c], inv);
-        __syncthreads();
-        for (int e = tid; e < OO; e += 256) {
-            int r = e / O, c = e - r * O;
-            if (r == k) continue;
-            double2 f = colk[r], v = M[k * O + c], m = M[e];
-            m.x = fma(-f.x, v.x, fma(f.y, v.y, m.x));
-            m.y = fma(-f.x, v.y, fma(-f.y, v.x, m.y));
-            M[e] = m;
+        if (cached) {
+            double2 v[INV_CT];
+#pragma unroll
+            for (int b = 0; b < INV_CT; ++b) { const int c = tx + 16 * b; v[b] = (c < O && c != k) ? rowk[c] : make_double2(0.0, 0.0); }
+            for (int r = ty; r < O; r += 16) {
+                if (r == k) continue;
+                const double2 f = colk[r];
+                double2* Mr = M + r * O;
+#pragma unroll
+                for (int b = 0; b < INV_CT; ++b) {
+                    const int c = tx + 16 * b;
+                    if (c < O && c != k) {
+                        double2 m = Mr[c];
+                        m.x = fma(-f.x, v[b].x, fma(f.y, v[b].y, m.x));
+                        m.y = fma(-f.x, v[b].y, fma(-f.y, v[b].x, m.y));
+                        Mr[c] = m;
+                    }
+                }
+            }
+        } else {
+            for (int r = ty; r < O; r += 16) {
+                if (r == k) continue;
+                const double2 f = colk[r];
+                double2* Mr = M + r * O;
+                for (int c = tx; c < O; c += 16) {
+                    if (c == k) continue;
+                    const double2 vv = rowk[c];
+                    double2 m = Mr[c];
+                    m.x = fma(-f.x, vv.x, fma(f.y, vv.y, m.x));
+                    m.y = fma(-f.x, vv.y, fma(-f.y, vv.x, m.y));
+                    Mr[c] = m;
+                }
+            }
+        }
+        for (int r = tid; r < O; r += 256) {
+            const double2 f = colk[r];
+            M[r * O + k] = (r == k) ? inv : make_double2(-(f.x * inv.x - f.y * inv.y), -(f.x * inv.y + f.y * inv.x));
         }
         __syncthreads();
     }
-    const bool singular = red_i[9] != 0;
+    const bool singular = ctl[1] != 0;
     if (!singular) {
         // undo the row interchanges: A^-1 = (P A)^-1 P, i.e. swap columns in reverse order
         for (int k = O - 1; k >= 0; --k) {
@@ -267,46 +298,64 @@ __global__ void __launch_bounds__(256) k_inverse(double2* __restrict__ Aws, int*
 }
 
 // ------------------------------------------------------------------------------------------------ S1: Theta
-// Theta[p][i] = sum_j Phi[p][j] Ainv[j][i]; one CTA = 32 basis rows of one walker; lane = p (coalesced stores of
-// the transposed panels), warps stride over 4-orbital groups.  Rows p in [N, N_pad) are written as zeros.
+// Theta[p][i] = sum_j Phi[p][j] Ainv[j][i] (complex x complex, Eq. 15) as ONE real GEMM on the DMMA pipe, computed
+// transposed so that the output fragments land in the Theta^T panel layout [o][2w+c'][p]:
+//   ThT[(i,c')][p] = sum_{(j,c)} Bt[(i,c')][(j,c)] * Phi[p][(j,c)],   Bt[(i,0)][(j,0)] = Re Ainv[j][i], Bt[(i,0)][(j,1)] = -Im,
+//                                                                     Bt[(i,1)][(j,0)] = Im,            Bt[(i,1)][(j,1)] = Re.
+// M = (i,c') (block of MFB fragments of 8 rows per CTA), N = p (64 per CTA, 8 per warp), K = (j,c) = the 2*O interleaved
+// doubles of a Phi row.  grid (N_pad/64 rounded up, M blocks, n_w).  K is staged TH_KC doubles at a time; both smem
+// operands are K-major with leading dimension TH_KC + 4 (= 4 mod 16: conflict-free fragment loads).  Rows p in
+// [N, N_pad) are written as zeros.
+constexpr int TH_KC = 32;
+constexpr int TH_LD = TH_KC + 4;
+
+template <int MFB>
 __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, const double2* __restrict__ Ainv, double* __restrict__ thT,
-                                               int N, int N_pad, int O, int o_base, int ldw) {
+                                               int N, int N_pad, int O, int o_base, int ldw, int mfb) {
     extern __shared__ __align__(16) double sm[];
-    double2* phi_s = reinterpret_cast<double2*>(sm);   // [32][PJ]
-    const int PJ = O | 1;
-    const int p0 = blockIdx.x * 32, w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const double2* phw = phi + (size_t)w * N * O;
-    for (int e = tid; e < 32 * O; e += 256) {
-        int pp = e / O, j = e - pp * O, p = p0 + pp;
-        phi_s[pp * PJ + j] = (p < N) ? phw[(size_t)p * O + j] : make_double2(0.0, 0.0);
-    }
-    __syncthreads();
+    double* Bt = sm;                       // [MFB*8][TH_LD]
+    double* Ph = sm + MFB * 8 * TH_LD;     // [64][TH_LD]
+    const int p0 = blockIdx.x * 64, m0 = blockIdx.y * mfb * 8, w = blockIdx.z;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    const int O2 = 2 * O, ib0 = m0 / 2, ni = MFB * 4;
+    const double* phw = reinterpret_cast<const double*>(phi + (size_t)w * N * O);
     const double2* Aw = Ainv + (size_t)w * O * O;
-    const int p = p0 + lane;
-    for (int i0 = warp * 4; i0 < O; i0 += 32) {
-        double2 acc[4];
+    double acc[MFB][2];
 #pragma unroll
-        for (int a = 0; a < 4; ++a) acc[a] = make_double2(0.0, 0.0);
-        int ia[4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) ia[a] = min(i0 + a, O - 1);
-        for (int j = 0; j < O; ++j) {
-            double2 f = phi_s[lane * PJ + j];
-#pragma unroll
-            for (int a = 0; a < 4; ++a) {
-                double2 m = __ldg(&Aw[j * O + ia[a]]);
-                acc[a].x = fma(f.x, m.x, fma(-f.y, m.y, acc[a].x));
-                acc[a].y = fma(f.x, m.y, fma(f.y, m.x, acc[a].y));
-            }
+    for (int a = 0; a < MFB; ++a) acc[a][0] = acc[a][1] = 0.0;
+    for (int k0 = 0; k0 < O2; k0 += TH_KC) {
+        __syncthreads();
+        // Bt chunk: rows (i,c') of this M block, columns (j,c) with 2j+c in [k0, k0+TH_KC)
+        for (int e = tid; e < (TH_KC / 2) * ni; e += 256) {
+            const int jj = e / ni, ii = e - jj * ni, i = ib0 + ii, j = k0 / 2 + jj;
+            double2 v = make_double2(0.0, 0.0);
+            if (i < O && j < O) v = Aw[(size_t)j * O + i];
+            double* r0 = Bt + (2 * ii) * TH_LD + 2 * jj;
+            r0[0] = v.x; r0[1] = -v.y;
+            r0[TH_LD] = v.y; r0[TH_LD + 1] = v.x;
         }
-        if (p < N_pad) {
+        for (int e = tid; e < 64 * TH_KC; e += 256) {
+            const int pp = e / TH_KC, k = e - pp * TH_KC, pg = p0 + pp, kk = k0 + k;
+            Ph[pp * TH_LD + k] = (pg < N && kk < O2) ? phw[(size_t)pg * O2 + kk] : 0.0;
+        }
+        __syncthreads();
 #pragma unroll
-            for (int a = 0; a < 4; ++a)
-                if (i0 + a < O) {
-                    size_t base = ((size_t)(o_base + i0 + a) * ldw + 2 * w) * N_pad + p;
-                    thT[base] = acc[a].x;
-                    thT[base + N_pad] = acc[a].y;
-                }
+        for (int ks = 0; ks < TH_KC / 4; ++ks) {
+            const double b = Ph[(warp * 8 + g) * TH_LD + ks * 4 + t];
+            double a[MFB];
+#pragma unroll
+            for (int mf = 0; mf < MFB; ++mf) a[mf] = Bt[(mf * 8 + g) * TH_LD + ks * 4 + t];
+#pragma unroll
+            for (int mf = 0; mf < MFB; ++mf) mma884(acc[mf][0], acc[mf][1], a[mf], b);
+        }
+    }
+    const int p = p0 + warp * 8 + 2 * t;
+    if (p < N_pad) {
+#pragma unroll
+        for (int mf = 0; mf < MFB; ++mf) {
+            const int m = m0 + mf * 8 + g, i = m >> 1, c = m & 1;
+            if (mf < mfb && i < O)
+                *reinterpret_cast<double2*>(thT + ((size_t)(o_base + i) * ldw + 2 * w + c) * N_pad + p) = make_double2(acc[mf][0], acc[mf][1]);
         }
     }
 }
@@ -458,16 +507,55 @@ __global__ void __launch_bounds__(256) k_ej(double* __restrict__ Xpart, double2*
 // Work item = (row tile of one pair, block of 64 walkers).  For the tile's rows K (singular vectors of pair (i,j)):
 //   a[K][w] = sum_p U[K][p] Theta_j[p][w],  b[K][w] = sum_p W[K][p] Theta_i[p][w]   (two real FP64 GEMMs, DMMA)
 //   e[w]   += wgt[K] * a[K][w] * b[K][w]  (complex product; wgt = -cK m_ij sigma_K)
-// CTA tile 64 rows x 128 real columns x 2 accumulators, K tile 16; 8 warps of 32 x 32 (x2); 3-stage cp.async
-// pipeline running across items.  The C fragment holds (re, im) of one walker in one lane, for a and b alike, so the
-// complex product is lane-local; the sum over rows stays in registers across items and is shuffle-reduced only when
-// the CTA's column block changes.  Persistent CTAs with a static round-robin schedule -> deterministic sums.
+// CTA tile <= 64 rows x 128 real columns x 2 accumulators, K tile 16.  Each of the 8 consumer warps owns ALL row
+// fragments of the tile and 16 real columns (8 walkers), so any rank (nfrag = 1..8 fragments of 8 rows) is balanced
+// over the warps and no cross-warp reduction is needed; the K loop is instantiated per nfrag (ex_kloop<NFRAG>) so a
+// short tile issues no DMMA on padding (predicated-off DMMAs still occupy the pipe: seen with ncu on the paper-like
+// small-rank workload).  4-stage TMA/mbarrier pipeline running across items; a short tile loads only its own 8-row
+// fragments of U and W.  The C fragment holds (re, im) of one walker in one lane, for a and b alike, so the complex
+// product is lane-local; rows are reduced by warp shuffles.  Persistent CTAs with a static round-robin schedule and
+// per-CTA partial sums accumulated in a fixed order -> bitwise repeatable.
 constexpr int EX_STAGES = 4;
 constexpr int EX_STAGE_BYTES = (2 * EX_BM + 2 * 128) * 128;
 constexpr int EX_RING = 8;      // tile-descriptor ring (producer -> consumers), > EX_STAGES items can never be in flight
-constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 2 * 128 * 8;
+constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 128 + EX_RING * 16;
+
+template <int NFRAG>
+__device__ __forceinline__ void ex_kloop(int KT, uint32_t sbase, uint32_t full, uint32_t empty, int& cslot, uint32_t& cphase, int lane,
+                                         const uint32_t (&xo)[4], uint32_t u_row, uint32_t tj_row, double (&accA)[8][2][2],
+                                         double (&accB)[8][2][2]) {
+    constexpr uint32_t W_OFF = EX_BM * 128, TI_OFF = 128 * 128;
+    for (int kt = 0; kt < KT; ++kt) {
+        if (kt) mbar_wait(full + 8 * cslot, cphase);     // the item's first stage was awaited by the caller
+        const uint32_t st = sbase + cslot * EX_STAGE_BYTES;
+#pragma unroll
+        for (int ks = 0; ks < KTILE / 4; ++ks) {
+            double a[NFRAG], w[NFRAG], bj[2], bi[2];
+#pragma unroll
+            for (int mf = 0; mf < NFRAG; ++mf) {
+                a[mf] = lds_f64(st + u_row + mf * 1024 + xo[ks]);
+                w[mf] = lds_f64(st + u_row + W_OFF + mf * 1024 + xo[ks]);
+            }
+#pragma unroll
+            for (int nf = 0; nf < 2; ++nf) {
+                bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
+                bi[nf] = lds_f64(st + tj_row + TI_OFF + nf * 1024 + xo[ks]);
+            }
+            if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
+#pragma unroll
+            for (int mf = 0; mf < NFRAG; ++mf)
+#pragma unroll
+                for (int nf = 0; nf < 2; ++nf) {
+                    mma884(accA[mf][nf][0], accA[mf][nf][1], a[mf], bj[nf]);
+                    mma884(accB[mf][nf][0], accB[mf][nf][1], w[mf], bi[nf]);
+                }
+        }
+        if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
+    }
+}
 
 __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
+                                                     const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
                                                      const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
                                                      const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
                                                      double* __restrict__ ekpart, int Wcap) {
@@ -476,7 +564,6 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
     const uint32_t full = sbase + EX_STAGES * EX_STAGE_BYTES, empty = full + 8 * EX_STAGES;
     ExTile* ring = reinterpret_cast<ExTile*>(sgen + EX_STAGES * EX_STAGE_BYTES + 128);            // [EX_RING]
-    double* red = reinterpret_cast<double*>(sgen + EX_STAGES * EX_STAGE_BYTES + 128 + EX_RING * 16);   // [2][128]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
@@ -484,6 +571,8 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
     if (tid == 0) {
         prefetch_tmap(&tmU);
         prefetch_tmap(&tmW);
+        prefetch_tmap(&tmU8);
+        prefetch_tmap(&tmW8);
         prefetch_tmap(&tmT);
         for (int i = 0; i < EX_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
@@ -499,14 +588,22 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
             for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
                 const ExTile tile = tiles[q / NB];
                 const int nb = (int)(q % NB);
+                const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + 2 * 128) * 128;
                 for (int kt = 0; kt < KT; ++kt) {
                     mbar_wait(empty + 8 * slot, phase ^ 1);
                     if (kt == 0) ring[n % EX_RING] = tile;      // ordered before the consumers' wait by arrive.expect_tx (release)
                     const uint32_t st = sbase + slot * EX_STAGE_BYTES, bar = full + 8 * slot;
                     const int k0 = kt * KTILE;
-                    mbar_expect_tx(bar, EX_STAGE_BYTES);
-                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
-                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
+                    mbar_expect_tx(bar, tx);
+                    if (tile.nfrag == EX_BM / 8) {
+                        tma_load_2d(st, &tmU, k0, tile.row0, bar);
+                        tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
+                    } else {
+                        for (int fr = 0; fr < tile.nfrag; ++fr) {
+                            tma_load_2d(st + fr * 1024, &tmU8, k0, tile.row0 + fr * 8, bar);
+                            tma_load_2d(st + EX_BM * 128 + fr * 1024, &tmW8, k0, tile.row0 + fr * 8, bar);
+                        }
+                    }
                     tma_load_2d(st + 2 * EX_BM * 128, &tmT, k0, tile.pj * ldw + nb * 128, bar);
                     tma_load_2d(st + (2 * EX_BM + 128) * 128, &tmT, k0, tile.pi * ldw + nb * 128, bar);
                     if (++slot == EX_STAGES) { slot = 0; phase ^= 1; }
@@ -515,91 +612,70 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
         }
         return;
     }
-    // ===== 8 consumer warps (32 rows x 32 columns x 2 accumulators each)
+    // ===== 8 consumer warps (all row fragments x 16 real columns x 2 accumulators each)
     reg_inc_consumer();
-    const int ctid = tid - 128, cw = warp - 4, g = lane >> 2, t = lane & 3, wm = cw >> 2, wn = cw & 3;
-    double accA[4][4][2], accB[4][4][2];
+    const int cw = warp - 4, g = lane >> 2, t = lane & 3;
+    double accA[8][2][2], accB[8][2][2];
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
+    for (int a = 0; a < 8; ++a)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
+        for (int b = 0; b < 2; ++b) accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
-    const uint32_t u_row = (uint32_t)(wm * 32 + g) * 128, w_row = u_row + EX_BM * 128;
-    const uint32_t tj_row = (uint32_t)(2 * EX_BM + wn * 32 + g) * 128, ti_row = tj_row + 128 * 128;
+    const uint32_t u_row = (uint32_t)g * 128;
+    const uint32_t tj_row = (uint32_t)(2 * EX_BM + cw * 16 + g) * 128;
     int cslot = 0, n = 0;
     uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
         const int nb = (int)(q % NB);
+        // this lane's slice of the CTA partial (lanes with g == 0 own walker cw*8 + nf*4 + t of the block): fetched now,
+        // updated after the K loop (same thread wrote it last, so program order makes the previous update visible)
+        double2* myp = reinterpret_cast<double2*>(mypart + (size_t)nb * 128 + cw * 16 + 2 * t);
+        double2 prev[2];
+        if (g == 0) { prev[0] = myp[0]; prev[1] = myp[4]; }
         mbar_wait(full + 8 * cslot, cphase);            // first stage of the item: its descriptor is in the ring now
         const ExTile tile = ring[n % EX_RING];
-        const int nvalid = min(4, max(0, tile.nfrag - wm * 4));
-        double wv[4];
-#pragma unroll
-        for (int mf = 0; mf < 4; ++mf) wv[mf] = (mf < nvalid) ? __ldg(wgt + tile.row0 + wm * 32 + mf * 8 + g) : 0.0;
-        for (int kt = 0; kt < KT; ++kt) {
-            if (kt) mbar_wait(full + 8 * cslot, cphase);
-            const uint32_t st = sbase + cslot * EX_STAGE_BYTES;
-            if (nvalid > 0) {           // warp-uniform; a warp whose 32 rows are all padding only releases the stage
-#pragma unroll
-                for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    double a[4], w[4], bj[4], bi[4];
-#pragma unroll
-                    for (int mf = 0; mf < 4; ++mf) {
-                        a[mf] = lds_f64(st + u_row + mf * 1024 + xo[ks]);
-                        w[mf] = lds_f64(st + w_row + mf * 1024 + xo[ks]);
-                    }
-#pragma unroll
-                    for (int nf = 0; nf < 4; ++nf) {
-                        bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
-                        bi[nf] = lds_f64(st + ti_row + nf * 1024 + xo[ks]);
-                    }
-                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
-#pragma unroll
-                    for (int mf = 0; mf < 4; ++mf)
-                        if (mf < nvalid) {
-#pragma unroll
-                            for (int nf = 0; nf < 4; ++nf) {
-                                mma884(accA[mf][nf][0], accA[mf][nf][1], a[mf], bj[nf]);
-                                mma884(accB[mf][nf][0], accB[mf][nf][1], w[mf], bi[nf]);
-                            }
-                        }
-                }
-            } else {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty + 8 * cslot);
-            }
-            if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
+        switch (tile.nfrag) {                           // warp- and CTA-uniform
+            case 1: ex_kloop<1>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 2: ex_kloop<2>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 3: ex_kloop<3>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 4: ex_kloop<4>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 5: ex_kloop<5>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 6: ex_kloop<6>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 7: ex_kloop<7>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            default: ex_kloop<8>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
         }
         // fused epilogue: e[w] = sum over this lane's rows of weight * a * b (complex), then over the 8 row groups of
-        // the warp (shuffles) and the two row-halves of the tile (shared memory), in a fixed order
-        double e[4][2];
+        // the warp (shuffles), in a fixed order; fragments beyond nfrag hold zeros
+        double e[2][2];
 #pragma unroll
-        for (int nf = 0; nf < 4; ++nf) e[nf][0] = e[nf][1] = 0.0;
+        for (int nf = 0; nf < 2; ++nf) e[nf][0] = e[nf][1] = 0.0;
 #pragma unroll
-        for (int mf = 0; mf < 4; ++mf) {
+        for (int mf = 0; mf < 8; ++mf) {
+            const double wv = (mf < tile.nfrag) ? __ldg(wgt + tile.row0 + mf * 8 + g) : 0.0;
 #pragma unroll
-            for (int nf = 0; nf < 4; ++nf) {
+            for (int nf = 0; nf < 2; ++nf) {
                 double ar = accA[mf][nf][0], ai = accA[mf][nf][1], br = accB[mf][nf][0], bi = accB[mf][nf][1];
-                e[nf][0] = fma(wv[mf], ar * br - ai * bi, e[nf][0]);
-                e[nf][1] = fma(wv[mf], ar * bi + ai * br, e[nf][1]);
+                e[nf][0] = fma(wv, ar * br - ai * bi, e[nf][0]);
+                e[nf][1] = fma(wv, ar * bi + ai * br, e[nf][1]);
                 accA[mf][nf][0] = accA[mf][nf][1] = accB[mf][nf][0] = accB[mf][nf][1] = 0.0;
             }
         }
 #pragma unroll
-        for (int nf = 0; nf < 4; ++nf)
+        for (int nf = 0; nf < 2; ++nf)
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
                 double v = e[nf][c];
                 v += __shfl_xor_sync(0xffffffffu, v, 4);
                 v += __shfl_xor_sync(0xffffffffu, v, 8);
                 v += __shfl_xor_sync(0xffffffffu, v, 16);
-                if (g == 0) red[wm * 128 + (wn * 16 + nf * 4 + t) * 2 + c] = v;
+                e[nf][c] = v;
             }
-        bar_sync_consumers();
-        if (ctid < 128) mypart[(size_t)nb * 128 + ctid] += red[ctid] + red[128 + ctid];
-        bar_sync_consumers();
+        if (g == 0) {
+            myp[0] = make_double2(prev[0].x + e[0][0], prev[0].y + e[0][1]);
+            myp[4] = make_double2(prev[1].x + e[1][0], prev[1].y + e[1][1]);
+        }
     }
 }
 
@@ -671,10 +747,13 @@ lo_status configure_kernels() {
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_exchange): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
-    e = cudaFuncSetAttribute(k_theta, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_theta): ") + cudaGetErrorString(e)); return LO_ECUDA; }
-    e = cudaFuncSetAttribute(k_overlap, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_overlap): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    const void* s1[] = {(const void*)k_theta<4>, (const void*)k_theta<8>, (const void*)k_theta<12>, (const void*)k_theta<16>,
+                        (const void*)k_overlap<1>, (const void*)k_overlap<2>, (const void*)k_overlap<3>, (const void*)k_overlap<4>,
+                        (const void*)k_overlap<5>, (const void*)k_overlap<6>, (const void*)k_overlap<8>};
+    for (const void* fn : s1) {
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+        if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(S1 kernels): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    }
     return LO_OK;
 }
 
@@ -688,11 +767,25 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         const int Op = (O + 3) & ~3;
         {
             Timer tm(f, stream, LO_K_OVERLAP);
-            k_overlap<<<n_w, 256, (size_t)OV_PC * Op * 24, stream>>>(f->ops->dPsi[s], (const double2*)phis[s], (double2*)f->dA[s], N, O);
+            const int NF = (2 * O + 7) / 8, nfw = (std::min(NF, OV_NFB) + 7) / 8;
+            dim3 grid((O + 31) / 32, n_w, (NF + OV_NFB - 1) / OV_NFB);
+            const size_t smem = (size_t)OV_PC * (OV_LDA + ov_ldb(O)) * 8;
+            const double* psi = f->ops->dPsi[s];
+            const double2* ph = (const double2*)phis[s];
+            double2* Ad = (double2*)f->dA[s];
+            switch (nfw) {
+                case 1: k_overlap<1><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+                case 2: k_overlap<2><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+                case 3: k_overlap<3><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+                case 4: k_overlap<4><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+                case 5: k_overlap<5><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+                case 6: k_overlap<6><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+                default: k_overlap<8><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
+            }
         }
         {
             Timer tm(f, stream, LO_K_INVERSE);
-            size_t aux = (size_t)O * 16 + (size_t)((O + 3) & ~3) * 4 + 64 + 64;
+            size_t aux = (size_t)(2 * O + 1) * 16 + (size_t)((O + 3) & ~3) * 4 + 16;
             size_t need = aux + (size_t)O * O * 16;
             if (need <= 200 * 1024)
                 k_inverse<true><<<n_w, 256, need, stream>>>((double2*)f->dA[s], f->dStatus + (size_t)s * Wcap, O);
@@ -701,9 +794,14 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         }
         {
             Timer tm(f, stream, LO_K_THETA);
-            dim3 grid((N_pad + 31) / 32, n_w);
-            k_theta<<<grid, 256, (size_t)32 * (O | 1) * 16, stream>>>((const double2*)phis[s], (const double2*)f->dA[s], f->dThT, N, N_pad, O,
-                                                                      f->o_base[s], ldw);
+            const int MF = (2 * O + 7) / 8, n_mb = (MF + 15) / 16, mfb = (MF + n_mb - 1) / n_mb;
+            dim3 grid((N_pad + 63) / 64, n_mb, n_w);
+            const double2* ph = (const double2*)phis[s];
+            const double2* Ai = (const double2*)f->dA[s];
+            if (mfb <= 4) k_theta<4><<<grid, 256, (4 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
+            else if (mfb <= 8) k_theta<8><<<grid, 256, (8 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
+            else if (mfb <= 12) k_theta<12><<<grid, 256, (12 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
+            else k_theta<16><<<grid, 256, (16 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
         }
     }
     const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
@@ -727,7 +825,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         Timer tm(f, stream, LO_K_EXCHANGE);
         long long items = f->n_tiles * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        k_exchange<<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad, ldw, f->dEKpart, Wcap);
+        k_exchange<<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad, ldw, f->dEKpart, Wcap);
     }
     // ---- S5
     {
