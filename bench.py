@@ -187,7 +187,9 @@ def run_ours(args):
     d2h = n_w * 4 * 16 + n_w * 4
     e2e_value = world * n_w * args.steps / (ms_e2e * 1e-3)
     E_dev = torch.stack(out[:4], dim=1).cpu().numpy()
-    assert np.array_equal(E_host.numpy(), E_dev), "host-buffer path and device path disagree"
+    # the host variant runs the batch in walker chunks (H2D of chunk c+1 under the kernels of chunk c): same arithmetic,
+    # another fixed summation order of the per-CTA partials
+    assert (np.abs(E_host.numpy() - E_dev).max(axis=1) <= 1e-12 * np.abs(E_dev[:, 0])).all(), "host-buffer path and device path disagree"
 
     # ---- roofline of the dominant kernel (exchange grouped GEMM), timed live with CUDA events on the launch stream
     ex_ms, ex_n = tm["exchange"]
@@ -207,7 +209,8 @@ def run_ours(args):
                 "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
                 "algorithmic_flops_per_launch": ex_flops,
                 "algorithmic_bytes_per_launch": 16.0 * info.N * sum(info.sum_rank) + 8.0 * sum(info.sum_rank) + 16.0 * info.N * sum(info.n_occ) * n_w}
-    kernels = {k: {"ms": round(m / max(n, 1), 4), "tflops": round(fl[k] * n_w / (m / max(n, 1) * 1e-3) * 1e-12, 3) if m > 0 else 0.0}
+    # per STEP (an unrestricted config launches the S1 kernels once per spin; flops_per_walker sums both spins)
+    kernels = {k: {"ms": round(m / args.steps, 4), "tflops": round(fl[k] * n_w / (m / args.steps * 1e-3) * 1e-12, 3) if m > 0 else 0.0}
                for k, (m, n) in tm.items()}
 
     cpu_baseline = None

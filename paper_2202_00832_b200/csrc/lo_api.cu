@@ -314,6 +314,8 @@ lo_status alloc_workspace(lo_factors* f) {
     CK(al((void**)&f->dEout, Wcap * 4 * 16));
     CK(al((void**)&f->dStatusOut, Wcap * 4));
     f->workspace_bytes = total;
+    CK(cudaStreamCreateWithFlags(&f->copyStream, cudaStreamNonBlocking));
+    for (int c = 0; c < LO_HOST_CHUNKS; ++c) CK(cudaEventCreateWithFlags(&f->evCopy[c], cudaEventDisableTiming));
     lo_status st = make_tmap(&f->tmTheta, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 128);
     if (st != LO_OK) return st;
     return configure_kernels();
@@ -340,6 +342,9 @@ void free_all(lo_factors* f) {
         for (auto& ev : f->pool) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
         f->bU.release();
         f->bW.release();
+        if (f->copyStream) cudaStreamDestroy(f->copyStream);
+        for (int c = 0; c < LO_HOST_CHUNKS; ++c)
+            if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
         void* ptrs[] = {f->dWgt, f->dTiles, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
                         f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1]};
         for (void* p : ptrs)
@@ -667,11 +672,28 @@ lo_status lo_local_energy_host(const lo_factors* fc, int n_w, const void* phi_a_
     lo_factors* f = const_cast<lo_factors*>(fc);
     cudaStream_t s = (cudaStream_t)stream;
     CK(cudaSetDevice(f->device));
-    const void* ph[2] = {phi_a_host, phi_b_host};
-    for (int sp = 0; sp < f->n_spin; ++sp)
-        CK(cudaMemcpyAsync(f->dPhi[sp], ph[sp], (size_t)n_w * f->N * f->n_occ[sp] * 16, cudaMemcpyHostToDevice, s));
-    st = launch_local_energy(f, n_w, f->dPhi[0], f->dPhi[1], nullptr, nullptr, nullptr, nullptr, f->dStatusOut, f->dEout, s);
-    if (st != LO_OK) return st;
+    // Walker chunks (multiples of 64, at least 128 walkers each, at most LO_HOST_CHUNKS): the H2D copy of chunk c+1 runs on
+    // a private copy stream while the kernels of chunk c run on `s`; walkers are independent, so a chunk is a complete
+    // pass of the hot path over its walkers (the factor rows are streamed once per chunk).
+    const char* ph[2] = {static_cast<const char*>(phi_a_host), static_cast<const char*>(phi_b_host)};
+    const int n_chunks = std::max(1, std::min(LO_HOST_CHUNKS, n_w / 128));
+    const int per = ((n_w + n_chunks - 1) / n_chunks + WALKER_TILE - 1) / WALKER_TILE * WALKER_TILE;
+    for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
+        const int nc = std::min(per, n_w - w0);
+        for (int sp = 0; sp < f->n_spin; ++sp) {
+            const size_t per_w = (size_t)f->N * f->n_occ[sp] * 16;
+            CK(cudaMemcpyAsync(reinterpret_cast<char*>(f->dPhi[sp]) + w0 * per_w, ph[sp] + w0 * per_w, nc * per_w, cudaMemcpyHostToDevice, f->copyStream));
+        }
+        CK(cudaEventRecord(f->evCopy[c], f->copyStream));
+    }
+    for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
+        const int nc = std::min(per, n_w - w0);
+        CK(cudaStreamWaitEvent(s, f->evCopy[c], 0));
+        const char* pa = reinterpret_cast<const char*>(f->dPhi[0]) + (size_t)w0 * f->N * f->n_occ[0] * 16;
+        const char* pb = f->n_spin == 2 ? reinterpret_cast<const char*>(f->dPhi[1]) + (size_t)w0 * f->N * f->n_occ[1] * 16 : nullptr;
+        st = launch_local_energy(f, nc, pa, pb, nullptr, nullptr, nullptr, nullptr, f->dStatusOut + w0, f->dEout + (size_t)w0 * 8, s);
+        if (st != LO_OK) return st;
+    }
     CK(cudaMemcpyAsync(E_host, f->dEout, (size_t)n_w * 4 * 16, cudaMemcpyDeviceToHost, s));
     if (status_host) CK(cudaMemcpyAsync(status_host, f->dStatusOut, (size_t)n_w * 4, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));

@@ -25,6 +25,7 @@ constexpr int WALKER_TILE = 64;  // walkers per column block (128 real columns)
 constexpr int EX_BM = 64;        // rows (singular vectors) per exchange tile
 constexpr int CO_BM = 128;       // rows (Cholesky vectors) per Coulomb tile
 constexpr int MAX_SPLIT = 8;     // split-K partial buffers of the Coulomb GEMM
+#define LO_HOST_CHUNKS 4         // walker chunks of lo_local_energy_host (copy/compute overlap)
 
 struct ExTile {
     int row0;   // first packed row of the tile
@@ -101,6 +102,8 @@ struct lo_factors {
     double* dEout = nullptr;      // [Wcap][4] complex (host variant)
     int* dStatusOut = nullptr;    // [Wcap]
     double* dPhi[2] = {nullptr, nullptr};  // staging for the host variant
+    cudaStream_t copyStream = nullptr;     // host variant: H2D of walker chunk c+1 overlaps the kernels of chunk c
+    cudaEvent_t evCopy[LO_HOST_CHUNKS] = {nullptr, nullptr, nullptr, nullptr};
     unsigned long long factor_bytes = 0, lbar_bytes = 0, workspace_bytes = 0;
     int last_n_w = 0;
     // timing

@@ -93,34 +93,34 @@ __device__ __forceinline__ uint32_t frag_off(int g, int t, int s) {
 
 // ------------------------------------------------------------------------------------------------ S1: overlap
 // A_w[i][j] = sum_p Psi[p][i] Phi_w[p][j]  as a real GEMM on the DMMA pipe: M = i (block of 32 per CTA), N = (j, re/im)
-// = the 2*O interleaved doubles of a Phi row, K = p.  grid (ceil(O/32), n_w), 8 warps; warp w owns column fragments
-// w, w+8, ... (NFW of them) and all 4 row fragments.  Psi / Phi rows are staged OV_PC at a time through shared memory;
+// = the 2*O interleaved doubles of a Phi row, K = p.  grid (row blocks of MFB fragments, n_w, column blocks), 8 warps;
+// warp w owns column fragments w, w+8, ... (NFW of them) and all MFB row fragments.  Psi / Phi rows are staged OV_PC at a time through shared memory;
 // both operands are stored with k (= p) as the slow index, so a fragment load reads 8 consecutive doubles of 4 rows and
 // a leading dimension = 4 (mod 16) doubles keeps the 16 lanes of a half-warp on distinct 8-byte banks.
 constexpr int OV_PC = 32;
-constexpr int OV_LDA = 36;
+constexpr int OV_LDA = 52;   // >= 5 row fragments (40 columns), = 4 (mod 16)
 constexpr int OV_NFB = 64;   // column fragments per CTA (grid.z blocks of 512 real columns = 256 orbitals)
 __host__ __device__ inline int ov_ldb(int O) { int nf8 = min((2 * O + 7) / 8, OV_NFB) * 8; return nf8 + ((4 - nf8 % 16) + 16) % 16; }
 
-template <int NFW>
+template <int MFB, int NFW>
 __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi, const double2* __restrict__ phi, double2* __restrict__ A,
                                                  int N, int O) {
     extern __shared__ __align__(16) double sm[];
     const int LDB = ov_ldb(O), nf0 = blockIdx.z * OV_NFB, NF = min((2 * O + 7) / 8 - nf0, OV_NFB), c0 = nf0 * 8;
     double* As = sm;                   // [OV_PC][OV_LDA]
     double* Bs = sm + OV_PC * OV_LDA;  // [OV_PC][LDB]
-    const int i0 = blockIdx.x * 32, w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    const int i0 = blockIdx.x * (MFB * 8), w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     const double* phw = reinterpret_cast<const double*>(phi + (size_t)w * N * O);
     const int O2 = 2 * O, ncb = NF * 8;
-    double acc[4][NFW][2];
+    double acc[MFB][NFW][2];
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
+    for (int a = 0; a < MFB; ++a)
 #pragma unroll
         for (int b = 0; b < NFW; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
     for (int p0 = 0; p0 < N; p0 += OV_PC) {
         __syncthreads();
-        for (int e = tid; e < OV_PC * 32; e += 256) {
-            const int pp = e >> 5, c = e & 31, pg = p0 + pp;
+        for (int e = tid; e < OV_PC * (MFB * 8); e += 256) {
+            const int pp = e / (MFB * 8), c = e - pp * (MFB * 8), pg = p0 + pp;
             As[pp * OV_LDA + c] = (pg < N && i0 + c < O) ? psi[(size_t)pg * O + i0 + c] : 0.0;
         }
         for (int e = tid; e < OV_PC * ncb; e += 256) {
@@ -130,22 +130,22 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
         __syncthreads();
 #pragma unroll
         for (int ks = 0; ks < OV_PC / 4; ++ks) {
-            double a[4], b[NFW];
+            double a[MFB], b[NFW];
 #pragma unroll
-            for (int mf = 0; mf < 4; ++mf) a[mf] = As[(ks * 4 + t) * OV_LDA + mf * 8 + g];
+            for (int mf = 0; mf < MFB; ++mf) a[mf] = As[(ks * 4 + t) * OV_LDA + mf * 8 + g];
 #pragma unroll
             for (int j = 0; j < NFW; ++j) {
                 const int nf = min(warp + 8 * j, NF - 1);
                 b[j] = Bs[(ks * 4 + t) * LDB + nf * 8 + g];
             }
 #pragma unroll
-            for (int mf = 0; mf < 4; ++mf)
+            for (int mf = 0; mf < MFB; ++mf)
 #pragma unroll
                 for (int j = 0; j < NFW; ++j) mma884(acc[mf][j][0], acc[mf][j][1], a[mf], b[j]);
         }
     }
 #pragma unroll
-    for (int mf = 0; mf < 4; ++mf)
+    for (int mf = 0; mf < MFB; ++mf)
 #pragma unroll
         for (int j = 0; j < NFW; ++j) {
             const int nf = warp + 8 * j, i = i0 + mf * 8 + g, jo = (nf0 + nf) * 4 + t;
@@ -311,11 +311,11 @@ constexpr int TH_LD = TH_KC + 4;
 
 template <int MFB>
 __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, const double2* __restrict__ Ainv, double* __restrict__ thT,
-                                               int N, int N_pad, int O, int o_base, int ldw, int mfb) {
+                                               int N, int N_pad, int O, int o_base, int ldw) {
     extern __shared__ __align__(16) double sm[];
     double* Bt = sm;                       // [MFB*8][TH_LD]
     double* Ph = sm + MFB * 8 * TH_LD;     // [64][TH_LD]
-    const int p0 = blockIdx.x * 64, m0 = blockIdx.y * mfb * 8, w = blockIdx.z;
+    const int p0 = blockIdx.x * 64, m0 = blockIdx.y * MFB * 8, w = blockIdx.z;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     const int O2 = 2 * O, ib0 = m0 / 2, ni = MFB * 4;
     const double* phw = reinterpret_cast<const double*>(phi + (size_t)w * N * O);
@@ -339,8 +339,10 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
             Ph[pp * TH_LD + k] = (pg < N && kk < O2) ? phw[(size_t)pg * O2 + kk] : 0.0;
         }
         __syncthreads();
+        const int nks = min(TH_KC / 4, (O2 - k0 + 3) / 4);      // K tail: whole k-steps of zeros are skipped (uniform)
 #pragma unroll
         for (int ks = 0; ks < TH_KC / 4; ++ks) {
+            if (ks >= nks) break;
             const double b = Ph[(warp * 8 + g) * TH_LD + ks * 4 + t];
             double a[MFB];
 #pragma unroll
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
 #pragma unroll
         for (int mf = 0; mf < MFB; ++mf) {
             const int m = m0 + mf * 8 + g, i = m >> 1, c = m & 1;
-            if (mf < mfb && i < O)
+            if (i < O)
                 *reinterpret_cast<double2*>(thT + ((size_t)(o_base + i) * ldw + 2 * w + c) * N_pad + p) = make_double2(acc[mf][0], acc[mf][1]);
         }
     }
@@ -737,6 +739,38 @@ int pick_split(long long base_items, int ksteps, int sms) {
     return best;
 }
 
+typedef void (*OvFn)(const double*, const double2*, double2*, int, int);
+template <int M>
+OvFn ov_fn_n(int nfw) {
+    switch (nfw) {
+        case 1: return k_overlap<M, 1>;
+        case 2: return k_overlap<M, 2>;
+        case 3: return k_overlap<M, 3>;
+        case 4: return k_overlap<M, 4>;
+        case 5: return k_overlap<M, 5>;
+        case 6: return k_overlap<M, 6>;
+        case 7: return k_overlap<M, 7>;
+        default: return k_overlap<M, 8>;
+    }
+}
+OvFn ov_fn(int mfb, int nfw) {
+    switch (mfb) {
+        case 1: return ov_fn_n<1>(nfw);
+        case 2: return ov_fn_n<2>(nfw);
+        case 3: return ov_fn_n<3>(nfw);
+        case 4: return ov_fn_n<4>(nfw);
+        default: return ov_fn_n<5>(nfw);
+    }
+}
+typedef void (*ThFn)(const double2*, const double2*, double*, int, int, int, int, int);
+template <int M>
+ThFn th_fn_t() { return k_theta<M>; }
+ThFn th_fn(int mfb) {
+    static const ThFn tab[16] = {th_fn_t<1>(), th_fn_t<2>(), th_fn_t<3>(), th_fn_t<4>(), th_fn_t<5>(), th_fn_t<6>(), th_fn_t<7>(), th_fn_t<8>(),
+                                 th_fn_t<9>(), th_fn_t<10>(), th_fn_t<11>(), th_fn_t<12>(), th_fn_t<13>(), th_fn_t<14>(), th_fn_t<15>(), th_fn_t<16>()};
+    return tab[mfb - 1];
+}
+
 }  // namespace
 
 lo_status configure_kernels() {
@@ -747,13 +781,19 @@ lo_status configure_kernels() {
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_exchange): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
-    const void* s1[] = {(const void*)k_theta<4>, (const void*)k_theta<8>, (const void*)k_theta<12>, (const void*)k_theta<16>,
-                        (const void*)k_overlap<1>, (const void*)k_overlap<2>, (const void*)k_overlap<3>, (const void*)k_overlap<4>,
-                        (const void*)k_overlap<5>, (const void*)k_overlap<6>, (const void*)k_overlap<8>};
-    for (const void* fn : s1) {
-        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-        if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(S1 kernels): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    for (int m = 1; m <= 16; ++m) {
+        e = cudaFuncSetAttribute((const void*)th_fn(m), cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)th_fn(m), cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_theta): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     }
+    for (int m = 1; m <= 5; ++m)
+        for (int n = 1; n <= 8; ++n) {
+            e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+            if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_overlap): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+        }
+    e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
 }
 
@@ -768,20 +808,10 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         {
             Timer tm(f, stream, LO_K_OVERLAP);
             const int NF = (2 * O + 7) / 8, nfw = (std::min(NF, OV_NFB) + 7) / 8;
-            dim3 grid((O + 31) / 32, n_w, (NF + OV_NFB - 1) / OV_NFB);
+            const int MF = (O + 7) / 8, n_mb = (MF + 4) / 5, mfb = (MF + n_mb - 1) / n_mb;     // row blocks of <= 5 fragments
+            dim3 grid(n_mb, n_w, (NF + OV_NFB - 1) / OV_NFB);
             const size_t smem = (size_t)OV_PC * (OV_LDA + ov_ldb(O)) * 8;
-            const double* psi = f->ops->dPsi[s];
-            const double2* ph = (const double2*)phis[s];
-            double2* Ad = (double2*)f->dA[s];
-            switch (nfw) {
-                case 1: k_overlap<1><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-                case 2: k_overlap<2><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-                case 3: k_overlap<3><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-                case 4: k_overlap<4><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-                case 5: k_overlap<5><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-                case 6: k_overlap<6><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-                default: k_overlap<8><<<grid, 256, smem, stream>>>(psi, ph, Ad, N, O); break;
-            }
+            ov_fn(mfb, nfw)<<<grid, 256, smem, stream>>>(f->ops->dPsi[s], (const double2*)phis[s], (double2*)f->dA[s], N, O);
         }
         {
             Timer tm(f, stream, LO_K_INVERSE);
@@ -798,10 +828,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
             dim3 grid((N_pad + 63) / 64, n_mb, n_w);
             const double2* ph = (const double2*)phis[s];
             const double2* Ai = (const double2*)f->dA[s];
-            if (mfb <= 4) k_theta<4><<<grid, 256, (4 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
-            else if (mfb <= 8) k_theta<8><<<grid, 256, (8 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
-            else if (mfb <= 12) k_theta<12><<<grid, 256, (12 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
-            else k_theta<16><<<grid, 256, (16 * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw, mfb);
+            th_fn(mfb)<<<grid, 256, (size_t)(mfb * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw);
         }
     }
     const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;

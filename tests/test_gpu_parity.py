@@ -65,6 +65,13 @@ def assert_parity(Eg, Eo, tol=TOL):
     assert np.abs(Eg[:, 0] - Eg[:, 1:].sum(axis=1)).max() <= 1e-12 * np.abs(Eg).max()
 
 
+def assert_close(Ea, Eb, what, tol=1e-12):
+    """Two launch configurations of the same arithmetic (different fixed summation orders): 1e-12 of |E_L| per walker."""
+    err = np.abs(Ea - Eb).max(axis=1) / np.abs(Eb[:, 0])
+    assert err.max() <= tol, "%s differs: max rel %.2e on walker %d" % (what, err.max(), int(err.argmax()))
+    return True
+
+
 def assert_all_walkers(P, F, phis, Eg, stride=1):
     """Properties that hold at any size, on walkers the sampled oracle check does not visit: (i) repeated calls and
     the host-buffer variant are bitwise equal on EVERY walker and every part (fixed-order reductions; this is what
@@ -75,7 +82,9 @@ def assert_all_walkers(P, F, phis, Eg, stride=1):
         E2, _ = gpu_energy(F, phis)
         assert np.array_equal(E2, Eg), "repeated call differs on walkers %s" % np.nonzero((E2 != Eg).any(axis=1))[0][:8]
     Eh, sh = F.local_energy_host([torch.from_numpy(np.ascontiguousarray(p)).pin_memory() for p in phis])
-    assert np.array_equal(Eh, Eg), "host-buffer variant differs on walkers %s" % np.nonzero((Eh != Eg).any(axis=1))[0][:8]
+    # the host variant runs the batch in walker chunks (copy/compute overlap): same arithmetic per walker, but the
+    # fixed summation order of the split-K / per-CTA partials depends on the number of walker blocks in a launch
+    assert_close(Eh, Eg, "host-buffer variant")
     hr = [oracle.half_rotate(P.L, P.h, psi) for psi in P.psi]
     empty = [oracle.empty_factor_set(P.N, o) for o in P.n_occ]
     sel = [p[::stride] for p in phis]
@@ -209,21 +218,22 @@ def test_trial_walker_gives_hf_energy(c1):
 # ------------------------------------------------------------------------------------------ API variants
 def test_host_variant_and_determinism(c1):
     torch = torch_cuda()
-    phis = gen.make_walkers(c1, 96)
-    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=96, gpu_svd=True)
+    phis = gen.make_walkers(c1, 300)    # host variant: 2 walker chunks (192 + a ragged 108)
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=300, gpu_svd=True)
     E1, _ = gpu_energy(F, phis)
     E2, _ = gpu_energy(F, phis)
     assert np.array_equal(E1, E2)                                  # fixed-order reductions: bitwise repeatable
     pinned = [torch.from_numpy(p).pin_memory() for p in phis]
     Eh, sh = F.local_energy_host(pinned)
-    assert np.array_equal(Eh, E1) and (sh == 0).all()
+    assert_close(Eh, E1, "host-buffer variant") and (sh == 0).all()
     Eh2, _ = F.local_energy_host(phis)                              # pageable numpy buffers
-    assert np.array_equal(Eh2, E1)
+    assert np.array_equal(Eh2, Eh)                                  # the host variant is bitwise repeatable too
+    assert_close(Eh2, E1, "host-buffer variant (pageable)")
     e_only = F.local_energy([torch.from_numpy(p).cuda() for p in phis], parts=False, status=False)
     torch.cuda.synchronize()
     assert np.array_equal(e_only[0].cpu().numpy(), E1[:, 0])
     with pytest.raises(lo.LoError):
-        F.local_energy([torch.from_numpy(gen.make_walkers(c1, 97)[0]).cuda()])      # n_w > max_walkers
+        F.local_energy([torch.from_numpy(gen.make_walkers(c1, 301)[0]).cuda()])     # n_w > max_walkers
 
 
 def test_gpu_svd_matches_host_svd(c1):
