@@ -125,14 +125,14 @@ def run_ours(args):
 
     t0 = time.time()
     P = gen.make_problem(cfg, reading=reading)          # same seed on every rank: the factor set is replicated
-    F = lo.Factors.setup(P.h, P.L, P.psi, T, device=local, max_walkers=n_w, gpu_svd=True)
+    F = lo.Factors.setup(P.h, P.L, P.psi, T, device=local, max_walkers=n_w, gpu_svd=True, propagator=args.propagator)
     info = F.info()
     setup_s = time.time() - t0
     # weak scaling: every rank owns a full batch of n_w walkers (its own seed); no data-path collective
     phis = gen.make_walkers(P, n_w, seed=P.seed + 1000 * rank)
     dphi = [torch.from_numpy(p).to(dev) for p in phis]
     fl = F.flops_per_walker()
-    flops_walker = sum(fl.values())
+    flops_walker = sum(v for k, v in fl.items() if k != "propagator")     # the steps of lo_local_energy (S1-S5)
 
     peak_dmma = lo.measure_peak("dmma", local)
     peak_dfma = lo.measure_peak("dfma", local)
@@ -213,6 +213,28 @@ def run_ours(args):
     kernels = {k: {"ms": round(m / args.steps, 4), "tflops": round(fl[k] * n_w / (m / args.steps * 1e-3) * 1e-12, 3) if m > 0 else 0.0}
                for k, (m, n) in tm.items()}
 
+    # ---- SURVEY 8(f) NEXT-1 (outside the timed step and outside `value`): propagator formation B_w = sum_g x^g_w L^g
+    nxt = None
+    if args.propagator:
+        gx = torch.Generator(device=dev).manual_seed(P.seed + rank)
+        x = torch.randn((n_w, info.n_chol, 2), dtype=torch.float64, device=dev, generator=gx)
+        x = torch.view_as_complex(x).contiguous()
+        for _ in range(3):
+            F.propagator(x)
+        torch.cuda.synchronize()
+        F.timing_enable(True)
+        F.timing_get()
+        for _ in range(args.steps):
+            F.propagator(x)
+        torch.cuda.synchronize()
+        pm, pn = F.timing_get()["propagator"]
+        F.timing_enable(False)
+        p_ms = pm / max(pn, 1)
+        p_tf = fl["propagator"] * n_w / (p_ms * 1e-3) * 1e-12
+        nxt = {"propagator": {"what": "B_w = sum_g x^g_w L^g for all walkers, upper triangle (PAPER.md:310), k_pack_x + DMMA GEMM",
+                              "ms": round(p_ms, 4), "tflops": round(p_tf, 3), "frac_of_peak": round(p_tf / peak, 4),
+                              "flops_per_walker": fl["propagator"]}}
+
     cpu_baseline = None
     if rank == 0 and world == 1 and args.cpu_walkers > 0:
         import oracle
@@ -242,7 +264,7 @@ def run_ours(args):
                 "flops_per_walker": flops_walker, "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu_baseline,
                 "e2e": {"value": round(e2e_value, 2), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "ms_per_step": round(ms_e2e / args.steps, 4), "api": "lo_local_energy_host (C ABI, pinned host buffers)"},
-                "gpu_launches": int(n_kernels), "clocks": clocks}
+                "gpu_launches": int(n_kernels), "clocks": clocks, "next": nxt}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -328,7 +350,7 @@ def run_sweep(args):
                "EK_abs_err_vs_exact_mean": float(np.mean(errs)), "EK_exact_abs_mean": float(np.mean([abs(e) for e, _ in exact])),
                "R5_bound_min": float(min(bounds)), "exact_walkers": [int(w) for w in idx],
                "ms_per_step": round(ms, 3), "energies_per_s": round(n_w / (ms * 1e-3), 2),
-               "tflops": round(sum(fl.values()) * n_w / (ms * 1e-3) * 1e-12, 3), "exchange_ms": round(ex_ms, 3),
+               "tflops": round(sum(v for k, v in fl.items() if k != "propagator") * n_w / (ms * 1e-3) * 1e-12, 3), "exchange_ms": round(ex_ms, 3),
                "exchange_tflops": round(fl["exchange"] * n_w / (ex_ms * 1e-3) * 1e-12, 3) if ex_ms > 0 else 0.0,
                "exchange_frac_of_peak": round(fl["exchange"] * n_w / (ex_ms * 1e-3) * 1e-12 / peak, 4) if ex_ms > 0 else 0.0,
                "peak_tflops": round(peak, 3), "setup_s_tightest": round(setup_s, 1), "oracle_exact_s": round(exact_s, 1)}
@@ -407,6 +429,8 @@ def main():
     ap.add_argument("--cpu-walkers", type=int, default=192, help="walkers of the batch the oracle is timed on (cpu_baseline)")
     ap.add_argument("--ref-walkers", type=int, default=32)
     ap.add_argument("--ref-pairs", type=int, default=128)
+    ap.add_argument("--no-propagator", dest="propagator", action="store_false",
+                    help="skip the NEXT-1 propagator-formation measurement (reported under \"next\", never part of `value`)")
     ap.add_argument("--sweep", action="store_true", help="threshold sweep (BASELINE.json:configs[4]): one JSON line per threshold")
     ap.add_argument("--sweep-exact-walkers", type=int, default=4, help="walkers whose exact E_K the oracle computes in --sweep")
     args = ap.parse_args()

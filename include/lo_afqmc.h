@@ -56,7 +56,7 @@ typedef struct {
 } lo_info;
 
 /* Kernel indices for lo_timing_get */
-enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_K_EXCHANGE = 4, LO_K_FINAL = 5, LO_K_COUNT = 6 };
+enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_K_EXCHANGE = 4, LO_K_FINAL = 5, LO_K_PROPAGATOR = 6, LO_K_COUNT = 7 };
 
 /* S0 setup (untimed, deterministic): half-rotation, per-pair Y^{ij}, SVD,
  * truncation sigma_K > threshold (strict, absolute; Eq. 18), sorting pairs by rank, padding
@@ -70,6 +70,9 @@ enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_
  *          (needs device >= 0); otherwise they run on the host with OpenMP.
  * On success *out owns everything; release with lo_free. */
 #define LO_SETUP_GPU_SVD 1
+/* flags bit 1 (LO_SETUP_PROPAGATOR, needs device >= 0): also keep the Cholesky vectors L on the device, packed for
+ * lo_propagator (upper triangle p<=q, K-major: [N(N+1)/2][n_chol]), and reserve its output buffer. */
+#define LO_SETUP_PROPAGATOR 2
 lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const double* h, const double* L,
                    const double* psi_a, const double* psi_b, double threshold, int device, int max_walkers,
                    unsigned flags, lo_factors** out);
@@ -109,6 +112,20 @@ lo_status lo_local_energy_host(const lo_factors* f, int n_w, const void* phi_a_h
  * PAPER.md:34): device complex128 [n_chol][ld] with ld returned in *ld (walker index fastest).
  * Valid until the next call on this factor set. */
 lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld);
+
+/* SURVEY 8(f) NEXT-1, propagator formation: B_w = sum_g x^g_w L^g ("forming the propagation matrix
+ * (B = sum_alpha x_alpha L_alpha), scaling as X M^2"), for n_w walkers at once as one real x
+ * complex FP64 GEMM on the DMMA pipe ([N(N+1)/2 x n_chol] x [n_chol x 2 n_w]).  Every L^g is symmetric, so B_w is
+ * (complex) symmetric and only the upper triangle is formed.
+ *   x_dev  device complex128 [n_w][n_chol] (walker-major): the shifted auxiliary fields of each walker.
+ * The result stays in a library-owned device buffer (lo_propagator_buffer): complex128 [n_rows][ld], row
+ * r(p,q) = p*N - p*(p-1)/2 + (q-p) for p<=q, walker index fastest; valid until the next lo_propagator call.
+ * Needs a factor set built with LO_SETUP_PROPAGATOR (else LO_EINVAL).  Asynchronous on `stream`; allocates nothing. */
+lo_status lo_propagator(const lo_factors* f, int n_w, const void* x_dev, void* stream);
+lo_status lo_propagator_buffer(const lo_factors* f, const void** B_dev, int* ld, long long* n_rows);
+/* B_w of the last lo_propagator call for one walker, unpacked to the full symmetric matrix, for tests:
+ * host complex128 [N][N].  Synchronises the device. */
+lo_status lo_propagator_host(const lo_factors* f, int w, void* B_host);
 
 /* Theta of the last call, for tests: host complex128 [n_w][N][n_occ[spin]] (walker-major, same layout as phi). */
 lo_status lo_theta_host(const lo_factors* f, int spin, int n_w, void* theta_host);

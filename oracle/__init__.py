@@ -112,6 +112,15 @@ def onebody_coulomb(Lbars, hbars, thetas, want_X=False):
     return (out[0], out[1], Xg) if want_X else (out[0], out[1])
 
 
+def propagator(L, x):
+    """B[p,q] = sum_g x[g] L[g,p,q] (the propagation matrix of one walker)."""
+    L, x = _f64(L), _c128(x)
+    X, N, _ = L.shape
+    B = np.zeros((N, N), dtype=np.complex128)
+    _l().orc_propagator(C.c_int(N), C.c_int(X), _p(L), _p(x), _p(B))
+    return B
+
+
 def exchange_cholesky(Lbar, th):
     """O2 single-spin exchange sum, Eq. 16."""
     Lbar, th = _f64(Lbar), _c128(th)

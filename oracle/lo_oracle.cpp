@@ -421,4 +421,15 @@ void orc_local_energy_lo(int n_w, int N, int X, int n_spin, const int* O, const 
     }
 }
 
+// NEXT-1 -- propagator formation ("forming the propagation matrix (B = sum_alpha x_alpha L_alpha),
+// scaling as X M^2"): B[p][q] = sum_g x[g] L[g][p][q], x complex (shifted auxiliary fields), L real.
+void orc_propagator(int N, int X, const double* L, const cd* x, cd* B) {
+    for (int p = 0; p < N; ++p)
+        for (int q = 0; q < N; ++q) {
+            cd s = 0;
+            for (int g = 0; g < X; ++g) s += x[g] * L[((size_t)g * N + p) * N + q];
+            B[(size_t)p * N + q] = s;
+        }
+}
+
 }  // extern "C"

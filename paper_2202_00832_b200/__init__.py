@@ -14,10 +14,11 @@ import numpy as np
 from . import build as _build
 
 LO_SETUP_GPU_SVD = 1
-K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize")
+LO_SETUP_PROPAGATOR = 2
+K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 4: "LO_ESINGULAR", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_local_energy",
-           "lo_local_energy_host", "lo_coulomb_x", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
+           "lo_local_energy_host", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
            "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
 
 
@@ -55,6 +56,9 @@ def lib():
         L.lo_local_energy_host.argtypes = [vp, ci, vp, vp, vp, vp, vp]
         L.lo_coulomb_x.argtypes = [vp, C.POINTER(vp), C.POINTER(ci)]
         L.lo_theta_host.argtypes = [vp, ci, ci, vp]
+        L.lo_propagator.argtypes = [vp, ci, vp, vp]
+        L.lo_propagator_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(ci), C.POINTER(C.c_longlong)]
+        L.lo_propagator_host.argtypes = [vp, ci, vp]
         L.lo_timing_enable.argtypes = [vp, ci]
         L.lo_timing_get.argtypes = [vp, C.POINTER(cd), C.POINTER(C.c_longlong)]
         L.lo_flops_per_walker.argtypes = [vp, C.POINTER(cd)]
@@ -94,7 +98,7 @@ class Factors:
         self._h = C.c_void_p(handle)
 
     @classmethod
-    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False):
+    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False, propagator=False):
         """lo_setup: h [N,N], L [n_chol,N,N], psis = [psi] (closed shell) or [psi_a, psi_b]; host numpy arrays."""
         h, L = _np(h, np.float64), _np(L, np.float64)
         psis = [_np(p, np.float64) for p in psis]
@@ -103,7 +107,7 @@ class Factors:
         out = C.c_void_p()
         st = lib().lo_setup(N, n_chol, len(psis), n_occ, h.ctypes.data, L.ctypes.data, psis[0].ctypes.data,
                             psis[1].ctypes.data if len(psis) == 2 else None, float(threshold), int(device), int(max_walkers),
-                            LO_SETUP_GPU_SVD if gpu_svd else 0, C.byref(out))
+                            (LO_SETUP_GPU_SVD if gpu_svd else 0) | (LO_SETUP_PROPAGATOR if propagator else 0), C.byref(out))
         _check(st)
         return cls(out.value)
 
@@ -210,6 +214,29 @@ class Factors:
         p, ld = C.c_void_p(), C.c_int()
         _check(lib().lo_coulomb_x(self._h, C.byref(p), C.byref(ld)))
         return p.value, ld.value
+
+    def propagator(self, x, stream=None):
+        """lo_propagator: x = torch CUDA complex128 [n_w, n_chol] (shifted auxiliary fields); forms
+        B_w = sum_g x[w,g] L^g into the library's buffer (see propagator_buffer / propagator_host).  Asynchronous."""
+        import torch
+        if x.dtype != torch.complex128 or not x.is_cuda:
+            raise LoError(1, "x must be a CUDA complex128 tensor")
+        x = x if x.is_contiguous() else x.contiguous()
+        s = torch.cuda.current_stream(x.device) if stream is None else stream
+        _check(lib().lo_propagator(self._h, int(x.shape[0]), C.c_void_p(x.data_ptr()), C.c_void_p(s.cuda_stream)))
+        return x
+
+    def propagator_buffer(self):
+        """(device pointer, ld, n_rows) of the packed upper-triangle result, complex128 [n_rows][ld], walker fastest."""
+        p, ld, n = C.c_void_p(), C.c_int(), C.c_longlong()
+        _check(lib().lo_propagator_buffer(self._h, C.byref(p), C.byref(ld), C.byref(n)))
+        return p.value, ld.value, n.value
+
+    def propagator_host(self, w) -> np.ndarray:
+        N = self.info().N
+        B = np.empty((N, N), dtype=np.complex128)
+        _check(lib().lo_propagator_host(self._h, int(w), B.ctypes.data))
+        return B
 
     def timing_enable(self, on=True):
         _check(lib().lo_timing_enable(self._h, 1 if on else 0))

@@ -21,6 +21,7 @@ SharedOps::~SharedOps() {
     if (device >= 0) {
         cudaSetDevice(device);
         if (dLbar) cudaFree(dLbar);
+        if (dLt) cudaFree(dLt);
         for (int s = 0; s < 2; ++s)
             if (dPsi[s]) cudaFree(dPsi[s]);
     }
@@ -313,10 +314,15 @@ lo_status alloc_workspace(lo_factors* f) {
     CK(al((void**)&f->dStatus, 2 * Wcap * 4));
     CK(al((void**)&f->dEout, Wcap * 4 * 16));
     CK(al((void**)&f->dStatusOut, Wcap * 4));
+    if (f->ops->dLt) {
+        CK(al((void**)&f->dXT, ldw * (size_t)f->ops->Xk_pad * 8));
+        CK(al((void**)&f->dB, (size_t)f->ops->tri_pad * ldw * 8));
+    }
     f->workspace_bytes = total;
     CK(cudaStreamCreateWithFlags(&f->copyStream, cudaStreamNonBlocking));
     for (int c = 0; c < LO_HOST_CHUNKS; ++c) CK(cudaEventCreateWithFlags(&f->evCopy[c], cudaEventDisableTiming));
     lo_status st = make_tmap(&f->tmTheta, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 128);
+    if (st == LO_OK && f->dXT) st = make_tmap(&f->tmXT, f->dXT, (unsigned long long)f->ops->Xk_pad, ldw, 128);
     if (st != LO_OK) return st;
     return configure_kernels();
 }
@@ -334,6 +340,39 @@ lo_status upload_lbar(lo_factors* f) {
     return make_tmap(&ops.tmLbar, ops.dLbar, K, f->Xp, CO_BM);
 }
 
+// Propagator operand: Lt[r(p,q)][g] = L^g_pq, p<=q, K-major with g fastest; built on the host in
+// row blocks (OpenMP over rows) and uploaded block by block.
+lo_status upload_lt(lo_factors* f, const double* L) {
+    SharedOps& ops = *f->ops;
+    CK(cudaSetDevice(f->device));
+    const long long N = f->N;
+    ops.tri = N * (N + 1) / 2;
+    ops.tri_pad = (ops.tri + CO_BM - 1) / CO_BM * CO_BM;
+    ops.Xk_pad = round_up(f->n_chol, KTILE);
+    const size_t ld = (size_t)ops.Xk_pad;
+    CK(cudaMalloc(&ops.dLt, (size_t)ops.tri_pad * ld * 8));
+    CK(cudaMemset(ops.dLt, 0, (size_t)ops.tri_pad * ld * 8));
+    const long long RBLK = 8192;
+    std::vector<double> buf((size_t)RBLK * ld, 0.0);
+    std::vector<int> rp((size_t)ops.tri), rq((size_t)ops.tri);
+    {
+        long long r = 0;
+        for (int p = 0; p < N; ++p)
+            for (int q = p; q < N; ++q, ++r) { rp[r] = p; rq[r] = q; }
+    }
+    for (long long r0 = 0; r0 < ops.tri; r0 += RBLK) {
+        const long long nr = std::min(RBLK, ops.tri - r0);
+#pragma omp parallel for schedule(static)
+        for (long long rr = 0; rr < nr; ++rr) {
+            const size_t off = (size_t)rp[r0 + rr] * N + rq[r0 + rr];
+            double* dst = buf.data() + (size_t)rr * ld;
+            for (int g = 0; g < f->n_chol; ++g) dst[g] = L[(size_t)g * N * N + off];
+        }
+        CK(cudaMemcpy(ops.dLt + (size_t)r0 * ld, buf.data(), (size_t)nr * ld * 8, cudaMemcpyHostToDevice));
+    }
+    return make_tmap(&ops.tmLt, ops.dLt, ld, (unsigned long long)ops.tri_pad, CO_BM);
+}
+
 void free_all(lo_factors* f) {
     if (!f) return;
     if (f->device >= 0) {
@@ -346,7 +385,7 @@ void free_all(lo_factors* f) {
         for (int c = 0; c < LO_HOST_CHUNKS; ++c)
             if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
         void* ptrs[] = {f->dWgt, f->dTiles, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
-                        f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1]};
+                        f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1], f->dXT, f->dB};
         for (void* p : ptrs)
             if (p) cudaFree(p);
     }
@@ -388,7 +427,10 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
     }
     for (int s = 0; s < n_spin; ++s)
         if (n_occ[s] <= 0 || n_occ[s] > N) { set_error("lo_setup: n_occ out of range"); return LO_EINVAL; }
-    if ((flags & LO_SETUP_GPU_SVD) && device < 0) { set_error("lo_setup: LO_SETUP_GPU_SVD needs device >= 0"); return LO_EINVAL; }
+    if ((flags & (LO_SETUP_GPU_SVD | LO_SETUP_PROPAGATOR)) && device < 0) {
+        set_error("lo_setup: LO_SETUP_GPU_SVD / LO_SETUP_PROPAGATOR need device >= 0");
+        return LO_EINVAL;
+    }
 
     lo_factors* f = new (std::nothrow) lo_factors();
     if (!f) { set_error("lo_setup: out of host memory"); return LO_ENOMEM; }
@@ -418,6 +460,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
         host_half_rotate(N, n_chol, n_spin, f->n_occ, f->o_base, f->O_tot, h, L, psi, f->ops->hLbar);
         if (device >= 0) {
             st = upload_lbar(f);
+            if (st == LO_OK && (flags & LO_SETUP_PROPAGATOR)) st = upload_lt(f, L);
             if (st != LO_OK) { free_all(f); return st; }
         }
         // ---- per-pair SVD + truncation + packing, batch by batch in layout order (whole L2 blocks per batch)
@@ -708,6 +751,46 @@ lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld) {
     return LO_OK;
 }
 
+lo_status lo_propagator(const lo_factors* fc, int n_w, const void* x_dev, void* stream) {
+    if (!fc || !x_dev) { set_error("lo_propagator: NULL argument"); return LO_EINVAL; }
+    if (fc->device < 0) { set_error("lo_propagator: no device"); return LO_ECUDA; }
+    if (!fc->ops->dLt || !fc->dB) { set_error("lo_propagator: the factor set was built without LO_SETUP_PROPAGATOR"); return LO_EINVAL; }
+    if (n_w <= 0 || n_w > fc->max_walkers) { set_error("lo_propagator: n_w out of range (1..max_walkers)"); return LO_EINVAL; }
+    if ((uintptr_t)x_dev & 15) { set_error("lo_propagator: x must be 16-byte aligned"); return LO_EINVAL; }
+    lo_factors* f = const_cast<lo_factors*>(fc);
+    CK(cudaSetDevice(f->device));
+    return launch_propagator(f, n_w, x_dev, (cudaStream_t)stream);
+}
+
+lo_status lo_propagator_buffer(const lo_factors* f, const void** B_dev, int* ld, long long* n_rows) {
+    if (!f || !B_dev || !ld || !n_rows) { set_error("lo_propagator_buffer: NULL argument"); return LO_EINVAL; }
+    if (f->device < 0 || !f->dB) { set_error("lo_propagator_buffer: the factor set was built without LO_SETUP_PROPAGATOR"); return LO_EINVAL; }
+    *B_dev = f->dB;
+    *ld = f->Wcap;
+    *n_rows = f->ops->tri;
+    return LO_OK;
+}
+
+lo_status lo_propagator_host(const lo_factors* f, int w, void* B_host) {
+    if (!f || !B_host || w < 0 || w >= f->max_walkers) { set_error("lo_propagator_host: invalid argument"); return LO_EINVAL; }
+    if (f->device < 0 || !f->dB) { set_error("lo_propagator_host: the factor set was built without LO_SETUP_PROPAGATOR"); return LO_EINVAL; }
+    CK(cudaSetDevice(f->device));
+    CK(cudaDeviceSynchronize());
+    const long long tri = f->ops->tri;
+    std::vector<double> col((size_t)tri * 2);
+    // column w of complex [tri][Wcap]: 16 bytes per row, pitch ldw*8
+    CK(cudaMemcpy2D(col.data(), 16, f->dB + (size_t)2 * w, (size_t)f->ldw * 8, 16, (size_t)tri, cudaMemcpyDeviceToHost));
+    double* out = static_cast<double*>(B_host);
+    const int N = f->N;
+    long long r = 0;
+    for (int p = 0; p < N; ++p)
+        for (int q = p; q < N; ++q, ++r) {
+            out[((size_t)p * N + q) * 2] = out[((size_t)q * N + p) * 2] = col[2 * r];
+            out[((size_t)p * N + q) * 2 + 1] = out[((size_t)q * N + p) * 2 + 1] = col[2 * r + 1];
+        }
+    return LO_OK;
+}
+
 lo_status lo_theta_host(const lo_factors* f, int spin, int n_w, void* theta_host) {
     if (!f || !theta_host || spin < 0 || spin >= f->n_spin || n_w <= 0 || n_w > f->max_walkers) { set_error("lo_theta_host: invalid argument"); return LO_EINVAL; }
     if (f->device < 0) { set_error("lo_theta_host: no device"); return LO_ECUDA; }
@@ -765,6 +848,7 @@ lo_status lo_flops_per_walker(const lo_factors* f, double fl[LO_K_COUNT]) {
     }
     fl[LO_K_COULOMB] = 4.0 * (f->n_chol + 1.0) * N * f->O_tot;   // real x complex, incl. the hbar row (S2)
     fl[LO_K_EXCHANGE] = 8.0 * N * R + 8.0 * R;                   // two real x complex GEMMs + weighted complex dot
+    fl[LO_K_PROPAGATOR] = 4.0 * f->n_chol * (N * (N + 1.0) / 2.0);  // lo_propagator (not part of lo_local_energy): real x complex
     return LO_OK;
 }
 

@@ -43,6 +43,11 @@ struct SharedOps {
     double* dLbar = nullptr;      // [Xp][O_tot][N_pad]
     CUtensorMap tmLbar;           // 2D [Xp][O_tot*N_pad], box 128 x 16, 128B swizzle
     double* dPsi[2] = {nullptr, nullptr};  // [N][O_s]
+    // propagator operand (LO_SETUP_PROPAGATOR): Lt[r(p,q)][g] = L^g_pq for p<=q, [tri_pad][Xk_pad] f64, zero padded
+    double* dLt = nullptr;
+    CUtensorMap tmLt;             // 2D [tri_pad][Xk_pad], box 128 x 16, 128B swizzle
+    long long tri = 0, tri_pad = 0;
+    int Xk_pad = 0;
     std::vector<double> hLbar;    // host copy [n_chol][O_tot][N] (+ hbar as row n_chol), kept for host-only sets / retruncate on host
     ~SharedOps();
 };
@@ -102,6 +107,9 @@ struct lo_factors {
     double* dEout = nullptr;      // [Wcap][4] complex (host variant)
     int* dStatusOut = nullptr;    // [Wcap]
     double* dPhi[2] = {nullptr, nullptr};  // staging for the host variant
+    double* dXT = nullptr;        // propagator: fields as a K-major real operand [ldw][Xk_pad] (row 2w+c = re/im of walker w)
+    double* dB = nullptr;         // propagator output [tri_pad][ldw] (= complex [tri_pad][Wcap])
+    CUtensorMap tmXT;
     cudaStream_t copyStream = nullptr;     // host variant: H2D of walker chunk c+1 overlaps the kernels of chunk c
     cudaEvent_t evCopy[LO_HOST_CHUNKS] = {nullptr, nullptr, nullptr, nullptr};
     unsigned long long factor_bytes = 0, lbar_bytes = 0, workspace_bytes = 0;
@@ -120,6 +128,7 @@ namespace lo {
 lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J,
                               void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 lo_status configure_kernels();
+lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStream_t stream);
 // 2D fp64 tensor map over a row-major [rows][inner] array, box [box_rows][16], 128-byte swizzle, zero OOB fill.
 lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner, unsigned long long rows, unsigned box_rows);   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)
 

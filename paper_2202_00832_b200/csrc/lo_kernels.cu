@@ -681,6 +681,17 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
     }
 }
 
+// ------------------------------------------------------------------------------------------------ NEXT-1: propagator
+// x[w][g] (complex128, walker-major) -> XT[2w + c][g] (K-major real operand of the propagator GEMM); the K padding
+// columns g >= n_chol stay zero from allocation.  grid (ceil(n_chol/128), n_w), block 128.
+__global__ void __launch_bounds__(128) k_pack_x(const double2* __restrict__ x, double* __restrict__ XT, int n_chol, int Xk_pad) {
+    const int g = blockIdx.x * 128 + threadIdx.x, w = blockIdx.y;
+    if (g >= n_chol) return;
+    const double2 v = x[(size_t)w * n_chol + g];
+    XT[(size_t)(2 * w) * Xk_pad + g] = v.x;
+    XT[(size_t)(2 * w + 1) * Xk_pad + g] = v.y;
+}
+
 // ------------------------------------------------------------------------------------------------ S5: combine
 __global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, const double2* __restrict__ E1raw,
                            const double2* __restrict__ EKpart, int n_ctas, const int* __restrict__ status, int n_spin, int Wcap,
@@ -865,6 +876,25 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
     f->last_n_w = n_w;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    return LO_OK;
+}
+
+// B[r(p,q)][w] = sum_g L^g_pq x^g_w: the Coulomb GEMM kernel with A = Lt (K = g), one "orbital panel",
+// no split-K (N(N+1)/2 / 128 row blocks fill the machine), output straight into dB.
+lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStream_t stream) {
+    SharedOps& ops = *f->ops;
+    const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
+    const int RB = (int)(ops.tri_pad / CO_BM);
+    {
+        Timer tm(f, stream, LO_K_PROPAGATOR);
+        dim3 g1((f->n_chol + 127) / 128, n_w);
+        k_pack_x<<<g1, 128, 0, stream>>>((const double2*)x_dev, f->dXT, f->n_chol, ops.Xk_pad);
+        const long long items = (long long)RB * NB;
+        const int grid = (int)std::min<long long>(items, f->num_sms);
+        k_coulomb<<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_error(std::string("lo_propagator: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
 }
 

@@ -358,3 +358,34 @@ def test_c4_full_size_sampled_walkers_and_retruncation():
     Eg2, _ = gpu_energy(F2, phis)
     Eo2, _ = oracle_energy_streamed(P, F2, phis, idx[:4])
     assert_parity(Eg2[idx[:4]], Eo2)
+
+
+# ------------------------------------------------------------------------------------------ NEXT-1: propagator
+@pytest.mark.parametrize("n_w", [5, 130])
+def test_propagator_matches_oracle(c1, n_w):
+    """lo_propagator: B_w = sum_g x^g_w L^g for every walker of a ragged batch, element by element
+    against the oracle's plain triple loop; 1e-13 of max|B_w| (a length-570 fp64 dot product in another order)."""
+    torch = torch_cuda()
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=n_w, gpu_svd=True, propagator=True)
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal((n_w, c1.n_chol)) + 1j * rng.standard_normal((n_w, c1.n_chol))
+    F.propagator(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    ptr, ld, n_rows = F.propagator_buffer()
+    assert n_rows == c1.N * (c1.N + 1) // 2 and ld >= n_w and ptr
+    for w in ([0, 3, 4] if n_w == 5 else [0, 63, 64, 129]):
+        Bo = oracle.propagator(c1.L, x[w])
+        Bg = F.propagator_host(w)
+        assert np.abs(Bg - Bo).max() <= 1e-13 * np.abs(Bo).max()
+    # the energy path is untouched by the propagator call and its workspace
+    phis = gen.make_walkers(c1, n_w)
+    Eg, st = gpu_energy(F, phis)
+    Eo, _ = oracle_energy(c1, F, phis)
+    assert_parity(Eg, Eo)
+
+
+def test_propagator_needs_flag(c0):
+    torch = torch_cuda()
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=0, max_walkers=4, gpu_svd=True)
+    with pytest.raises(lo.LoError):
+        F.propagator(torch.zeros((4, c0.n_chol), dtype=torch.complex128, device="cuda"))

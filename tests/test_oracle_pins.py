@@ -322,3 +322,32 @@ def test_streamed_evaluation_equals_one_piece(c1, c1_walkers):
     Es, sts, secs = oracle.local_energy_lo_streamed(c1.psi, [Lbar], [hbar], phis, [len(sel)], fetch, chunk=5)
     assert (st == 0).all() and (sts == 0).all() and secs > 0
     assert np.abs(Es - E).max() <= 1e-12 * np.abs(E[:, 0]).max()
+
+
+# ------------------------------------------------------------------------------------------ NEXT-1: propagator
+def test_propagator_pins(c0, c0_walkers):
+    """B = sum_g x_g L^g (PAPER.md:310).  Pins: a unit field returns that Cholesky matrix exactly; B is symmetric;
+    tr B = sum_g x_g tr L^g; and contracting B with the walker's Green's function gives sum_g x_g X^g with the X^g of
+    the (already pinned) Coulomb route: sum_pq B_pq G_pq = sum_g x_g sum_ip Lbar^g_ip Theta_pi (Eq. 14, 16)."""
+    L, N, X = c0.L, c0.N, c0.n_chol
+    for g in (0, 17, X - 1):
+        e = np.zeros(X, dtype=np.complex128)
+        e[g] = 1.0
+        assert np.array_equal(oracle.propagator(L, e), L[g].astype(np.complex128))
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal(X) + 1j * rng.standard_normal(X)
+    B = oracle.propagator(L, x)
+    assert np.abs(B - B.T).max() <= 1e-14 * np.abs(B).max()
+    tr = sum(x[g] * np.trace(L[g]) for g in range(X))
+    assert abs(np.trace(B) - tr) <= 1e-12 * abs(tr)
+    psi = c0.psi[0]
+    th, _, _ = oracle.theta(psi, c0_walkers[0][0])
+    G = oracle.green(psi, th)
+    Lbar, hbar = oracle.half_rotate(L, c0.h, psi)
+    _, _, Xg = oracle.onebody_coulomb([Lbar], [hbar], [th], want_X=True)
+    lhs = (B * G).sum()
+    rhs = (x * Xg).sum()
+    assert abs(lhs - rhs) <= 1e-12 * abs(rhs)
+    # linearity in the fields
+    y = rng.standard_normal(X) + 1j * rng.standard_normal(X)
+    assert np.abs(oracle.propagator(L, 2.0 * x - 1j * y) - (2.0 * B - 1j * oracle.propagator(L, y))).max() <= 1e-12 * np.abs(B).max()
