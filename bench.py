@@ -235,6 +235,32 @@ def run_ours(args):
                               "ms": round(p_ms, 4), "tflops": round(p_tf, 3), "frac_of_peak": round(p_tf / peak, 4),
                               "flops_per_walker": fl["propagator"]}}
 
+    # ---- SURVEY 8(f) NEXT-3 (outside `value`): the paper-literal energy, Coulomb term from the compressed factors too
+    if info.n_spin == 1:
+        F.set_coulomb_mode(True)
+        flc = F.flops_per_walker()
+        for _ in range(3):
+            F.local_energy(dphi, parts=True)
+        torch.cuda.synchronize()
+        F.timing_enable(True)
+        F.timing_get()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for _ in range(args.steps):
+            F.local_energy(dphi, parts=True)
+        c1.record()
+        torch.cuda.synchronize()
+        cm, cn = F.timing_get()["exchange"]
+        F.timing_enable(False)
+        F.set_coulomb_mode(False)
+        c_ms = cm / max(cn, 1)
+        c_tf = flc["exchange"] * n_w / (c_ms * 1e-3) * 1e-12
+        nxt = dict(nxt or {})
+        nxt["compressed_coulomb"] = {"what": "lo_set_coulomb_mode(COMPRESSED): E_J and E_K both from the pair factors (Eq. 19/22), 4 projections per pair",
+                                     "ms_per_step": round(c0.elapsed_time(c1) / args.steps, 4),
+                                     "energies_per_s": round(n_w * args.steps / (c0.elapsed_time(c1) * 1e-3), 2),
+                                     "exchange_ms": round(c_ms, 4), "exchange_tflops": round(c_tf, 3), "exchange_frac_of_peak": round(c_tf / peak, 4)}
+
     cpu_baseline = None
     if rank == 0 and world == 1 and args.cpu_walkers > 0:
         import oracle

@@ -113,6 +113,17 @@ lo_status lo_local_energy_host(const lo_factors* f, int n_w, const void* phi_a_h
  * Valid until the next call on this factor set. */
 lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld);
 
+/* SURVEY 8(f) NEXT-3, the paper-literal energy expression: with LO_COULOMB_COMPRESSED the Coulomb term of every later
+ * lo_local_energy* call is evaluated from the SVD-compressed pair factors as well,
+ *   E_J^LO = 2 sum_{i<=j} m_ij sum_{K<=r_ij} sigma_K (U^{ij T} Theta_i)_K (W^{ij} Theta_j)_K     (closed shell)
+ * (Eq. 19/22 first term "4 Q_{K,L,i} Q_{K,R,j}"; the four projections per pair of PAPER.md:181
+ * come from the same staged tiles as the exchange), so E_J carries the truncation error too.  The default
+ * LO_COULOMB_CHOLESKY evaluates E_J = cJ sum_g (X^g)^2 exactly (Eq. 16).  X^g (lo_coulomb_x) and E1 are formed in both
+ * modes.  Closed shell only: an unrestricted factor set holds same-spin pairs only (LO_EINVAL). */
+#define LO_COULOMB_CHOLESKY 0
+#define LO_COULOMB_COMPRESSED 1
+lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
+
 /* SURVEY 8(f) NEXT-1, propagator formation: B_w = sum_g x^g_w L^g ("forming the propagation matrix
  * (B = sum_alpha x_alpha L_alpha), scaling as X M^2"), for n_w walkers at once as one real x
  * complex FP64 GEMM on the DMMA pipe ([N(N+1)/2 x n_chol] x [n_chol x 2 n_w]).  Every L^g is symmetric, so B_w is

@@ -18,7 +18,7 @@ LO_SETUP_PROPAGATOR = 2
 K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 4: "LO_ESINGULAR", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_local_energy",
-           "lo_local_energy_host", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
+           "lo_local_energy_host", "lo_set_coulomb_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
            "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
 
 
@@ -56,6 +56,7 @@ def lib():
         L.lo_local_energy_host.argtypes = [vp, ci, vp, vp, vp, vp, vp]
         L.lo_coulomb_x.argtypes = [vp, C.POINTER(vp), C.POINTER(ci)]
         L.lo_theta_host.argtypes = [vp, ci, ci, vp]
+        L.lo_set_coulomb_mode.argtypes = [vp, ci]
         L.lo_propagator.argtypes = [vp, ci, vp, vp]
         L.lo_propagator_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(ci), C.POINTER(C.c_longlong)]
         L.lo_propagator_host.argtypes = [vp, ci, vp]
@@ -214,6 +215,10 @@ class Factors:
         p, ld = C.c_void_p(), C.c_int()
         _check(lib().lo_coulomb_x(self._h, C.byref(p), C.byref(ld)))
         return p.value, ld.value
+
+    def set_coulomb_mode(self, compressed: bool):
+        """lo_set_coulomb_mode: E_J from the compressed pair factors (Eq. 19/22, paper-literal) or the Cholesky route."""
+        _check(lib().lo_set_coulomb_mode(self._h, 1 if compressed else 0))
 
     def propagator(self, x, stream=None):
         """lo_propagator: x = torch CUDA complex128 [n_w, n_chol] (shifted auxiliary fields); forms

@@ -226,6 +226,16 @@ void layout_block(lo_factors* f, PairRec* first, PairRec* last, SigmaFn sig, Src
             f->hTiles.push_back(T);
             done += nf;
         }
+        for (int d4 = 0, nt4 = (F + 3) / 4, t = 0; t < nt4; ++t) {      // NEXT-3 cut: <= 4 fragments per tile
+            const int nf = F / nt4 + (t < F % nt4 ? 1 : 0);
+            ExTile T;
+            T.row0 = (int)(f->rows + (long long)d4 * 8);
+            T.nfrag = nf;
+            T.pi = f->o_base[pr->spin] + pr->i;
+            T.pj = f->o_base[pr->spin] + pr->j;
+            f->hTiles4.push_back(T);
+            d4 += nf;
+        }
         const double m = pr->i == pr->j ? 1.0 : 2.0;
         f->hWgt.resize((size_t)f->rows + r_pad, 0.0);
         for (int K = 0; K < pr->r; ++K) f->hWgt[(size_t)f->rows + K] = -cK * m * sig(*pr, K);
@@ -243,6 +253,7 @@ lo_status begin_pack(lo_factors* f) {
     }
     f->rows = 0;
     f->hTiles.clear();
+    f->hTiles4.clear();
     f->hWgt.clear();
     if (f->device >= 0) {
         CK(cudaSetDevice(f->device));
@@ -278,6 +289,7 @@ lo_status finish_pack(lo_factors* f) {
     const size_t rows_alloc = (size_t)f->rows + EX_BM;
     f->hWgt.resize(rows_alloc, 0.0);
     f->n_tiles = (long long)f->hTiles.size();
+    f->n_tiles4 = (long long)f->hTiles4.size();
     f->factor_bytes = 2 * rows_alloc * f->N_pad * 8 + rows_alloc * 8 + f->hTiles.size() * sizeof(ExTile);
     if (f->device < 0) return LO_OK;
     CK(cudaSetDevice(f->device));
@@ -285,6 +297,8 @@ lo_status finish_pack(lo_factors* f) {
     CK(cudaMalloc(&f->dTiles, std::max<size_t>(1, f->hTiles.size()) * sizeof(ExTile)));
     CK(cudaMemcpy(f->dWgt, f->hWgt.data(), rows_alloc * 8, cudaMemcpyHostToDevice));
     if (!f->hTiles.empty()) CK(cudaMemcpy(f->dTiles, f->hTiles.data(), f->hTiles.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
+    CK(cudaMalloc(&f->dTiles4, std::max<size_t>(1, f->hTiles4.size()) * sizeof(ExTile)));
+    if (!f->hTiles4.empty()) CK(cudaMemcpy(f->dTiles4, f->hTiles4.data(), f->hTiles4.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
     st = make_tmap(&f->tmU, f->dU, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmW, f->dW, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmU8, f->dU, f->N_pad, rows_alloc, 8);
@@ -311,6 +325,7 @@ lo_status alloc_workspace(lo_factors* f) {
     CK(al((void**)&f->dXpart, (size_t)MAX_SPLIT * f->Xp * ldw * 8));
     CK(al((void**)&f->dEJpart, (size_t)(f->Xp / CO_BM + 1) * Wcap * 16));
     CK(al((void**)&f->dEKpart, (size_t)f->num_sms * Wcap * 16));
+    CK(al((void**)&f->dEJLpart, (size_t)f->num_sms * Wcap * 16));
     CK(al((void**)&f->dStatus, 2 * Wcap * 4));
     CK(al((void**)&f->dEout, Wcap * 4 * 16));
     CK(al((void**)&f->dStatusOut, Wcap * 4));
@@ -384,7 +399,7 @@ void free_all(lo_factors* f) {
         if (f->copyStream) cudaStreamDestroy(f->copyStream);
         for (int c = 0; c < LO_HOST_CHUNKS; ++c)
             if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
-        void* ptrs[] = {f->dWgt, f->dTiles, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
+        void* ptrs[] = {f->dWgt, f->dTiles, f->dTiles4, f->dEJLpart, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
                         f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1], f->dXT, f->dB};
         for (void* p : ptrs)
             if (p) cudaFree(p);
@@ -751,6 +766,16 @@ lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld) {
     return LO_OK;
 }
 
+lo_status lo_set_coulomb_mode(lo_factors* f, int mode) {
+    if (!f || (mode != LO_COULOMB_CHOLESKY && mode != LO_COULOMB_COMPRESSED)) { set_error("lo_set_coulomb_mode: invalid argument"); return LO_EINVAL; }
+    if (mode == LO_COULOMB_COMPRESSED && f->n_spin != 1) {
+        set_error("lo_set_coulomb_mode: the compressed Coulomb term needs opposite-spin pair blocks, which an unrestricted factor set does not hold");
+        return LO_EINVAL;
+    }
+    f->coulomb_lo = mode == LO_COULOMB_COMPRESSED ? 1 : 0;
+    return LO_OK;
+}
+
 lo_status lo_propagator(const lo_factors* fc, int n_w, const void* x_dev, void* stream) {
     if (!fc || !x_dev) { set_error("lo_propagator: NULL argument"); return LO_EINVAL; }
     if (fc->device < 0) { set_error("lo_propagator: no device"); return LO_ECUDA; }
@@ -847,7 +872,7 @@ lo_status lo_flops_per_walker(const lo_factors* f, double fl[LO_K_COUNT]) {
         for (int r : f->rank[s]) R += r;
     }
     fl[LO_K_COULOMB] = 4.0 * (f->n_chol + 1.0) * N * f->O_tot;   // real x complex, incl. the hbar row (S2)
-    fl[LO_K_EXCHANGE] = 8.0 * N * R + 8.0 * R;                   // two real x complex GEMMs + weighted complex dot
+    fl[LO_K_EXCHANGE] = (f->coulomb_lo ? 2.0 : 1.0) * (8.0 * N * R + 8.0 * R);   // two (compressed-Coulomb mode: four) real x complex GEMMs + weighted complex dots
     fl[LO_K_PROPAGATOR] = 4.0 * f->n_chol * (N * (N + 1.0) / 2.0);  // lo_propagator (not part of lo_local_energy): real x complex
     return LO_OK;
 }

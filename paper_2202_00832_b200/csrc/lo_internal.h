@@ -90,10 +90,14 @@ struct lo_factors {
     // host copies: hU/hW only for host-only sets (device < 0); hWgt (weights incl. sigma) always
     std::vector<double> hU, hW, hWgt;
     std::vector<lo::ExTile> hTiles;
+    std::vector<lo::ExTile> hTiles4;     // same rows cut at <= 4 fragments (compressed-Coulomb mode, NEXT-3)
+    long long n_tiles4 = 0;
+    int coulomb_lo = 0;                  // 1: E_J from the compressed factors (Eq. 19/22) instead of the Cholesky route
     // device factor set
     lo::GrowBuf bU, bW;                  // backing store of dU / dW
     double *dU = nullptr, *dW = nullptr, *dWgt = nullptr;
     lo::ExTile* dTiles = nullptr;
+    lo::ExTile* dTiles4 = nullptr;
     CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
     CUtensorMap tmU8, tmW8;              // same arrays, boxes 8 x 16 (one row fragment): tiles shorter than 64 rows
     std::shared_ptr<lo::SharedOps> ops;
@@ -103,6 +107,7 @@ struct lo_factors {
     double* dXpart = nullptr;     // [MAX_SPLIT][Xp][ldw]
     double* dEJpart = nullptr;    // [Xp/128][Wcap] complex
     double* dEKpart = nullptr;    // [num_sms][Wcap] complex
+    double* dEJLpart = nullptr;   // [num_sms][Wcap] complex (compressed-Coulomb partials)
     int* dStatus = nullptr;       // [2][Wcap]
     double* dEout = nullptr;      // [Wcap][4] complex (host variant)
     int* dStatusOut = nullptr;    // [Wcap]

@@ -522,10 +522,14 @@ constexpr int EX_STAGE_BYTES = (2 * EX_BM + 2 * 128) * 128;
 constexpr int EX_RING = 8;      // tile-descriptor ring (producer -> consumers), > EX_STAGES items can never be in flight
 constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 128 + EX_RING * 16;
 
-template <int NFRAG>
+// COUL: also accumulate the two projections of the paper-literal compressed Coulomb term,
+// aJ = U Theta_i and bJ = W Theta_j (Eq. 19/22 first term, "forming the projected vectors must occur four times",
+// PAPER.md:181), from the same staged tiles; tiles are then cut at 4 fragments so the four accumulator sets fit.
+template <int NFRAG, bool COUL, int MFMAX>
 __device__ __forceinline__ void ex_kloop(int KT, uint32_t sbase, uint32_t full, uint32_t empty, int& cslot, uint32_t& cphase, int lane,
-                                         const uint32_t (&xo)[4], uint32_t u_row, uint32_t tj_row, double (&accA)[8][2][2],
-                                         double (&accB)[8][2][2]) {
+                                         const uint32_t (&xo)[4], uint32_t u_row, uint32_t tj_row, double (&accA)[MFMAX][2][2],
+                                         double (&accB)[MFMAX][2][2], double (&accC)[COUL ? MFMAX : 1][2][2],
+                                         double (&accD)[COUL ? MFMAX : 1][2][2]) {
     constexpr uint32_t W_OFF = EX_BM * 128, TI_OFF = 128 * 128;
     for (int kt = 0; kt < KT; ++kt) {
         if (kt) mbar_wait(full + 8 * cslot, cphase);     // the item's first stage was awaited by the caller
@@ -550,17 +554,22 @@ __device__ __forceinline__ void ex_kloop(int KT, uint32_t sbase, uint32_t full, 
                 for (int nf = 0; nf < 2; ++nf) {
                     mma884(accA[mf][nf][0], accA[mf][nf][1], a[mf], bj[nf]);
                     mma884(accB[mf][nf][0], accB[mf][nf][1], w[mf], bi[nf]);
+                    if constexpr (COUL) {
+                        mma884(accC[mf][nf][0], accC[mf][nf][1], a[mf], bi[nf]);
+                        mma884(accD[mf][nf][0], accD[mf][nf][1], w[mf], bj[nf]);
+                    }
                 }
         }
         if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
     }
 }
 
+template <bool COUL>
 __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
                                                      const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
                                                      const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
                                                      const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
-                                                     double* __restrict__ ekpart, int Wcap) {
+                                                     double* __restrict__ ekpart, double* __restrict__ ejpart, int Wcap) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
@@ -569,7 +578,11 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
-    for (int i = tid; i < 2 * Wcap; i += 384) mypart[i] = 0.0;
+    double* mypartJ = COUL ? ejpart + (size_t)blockIdx.x * 2 * Wcap : nullptr;
+    for (int i = tid; i < 2 * Wcap; i += 384) {
+        mypart[i] = 0.0;
+        if constexpr (COUL) mypartJ[i] = 0.0;
+    }
     if (tid == 0) {
         prefetch_tmap(&tmU);
         prefetch_tmap(&tmW);
@@ -617,11 +630,15 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
     // ===== 8 consumer warps (all row fragments x 16 real columns x 2 accumulators each)
     reg_inc_consumer();
     const int cw = warp - 4, g = lane >> 2, t = lane & 3;
-    double accA[8][2][2], accB[8][2][2];
+    constexpr int MFMAX = COUL ? 4 : 8;
+    double accA[MFMAX][2][2], accB[MFMAX][2][2], accC[COUL ? MFMAX : 1][2][2], accD[COUL ? MFMAX : 1][2][2];
 #pragma unroll
-    for (int a = 0; a < 8; ++a)
+    for (int a = 0; a < MFMAX; ++a)
 #pragma unroll
-        for (int b = 0; b < 2; ++b) accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
+        for (int b = 0; b < 2; ++b) {
+            accA[a][b][0] = accA[a][b][1] = accB[a][b][0] = accB[a][b][1] = 0.0;
+            if constexpr (COUL) accC[a][b][0] = accC[a][b][1] = accD[a][b][0] = accD[a][b][1] = 0.0;
+        }
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
@@ -634,27 +651,42 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
         // this lane's slice of the CTA partial (lanes with g == 0 own walker cw*8 + nf*4 + t of the block): fetched now,
         // updated after the K loop (same thread wrote it last, so program order makes the previous update visible)
         double2* myp = reinterpret_cast<double2*>(mypart + (size_t)nb * 128 + cw * 16 + 2 * t);
-        double2 prev[2];
-        if (g == 0) { prev[0] = myp[0]; prev[1] = myp[4]; }
+        double2* mypJ = reinterpret_cast<double2*>(mypartJ + (size_t)nb * 128 + cw * 16 + 2 * t);
+        double2 prev[2], prevJ[2];
+        if (g == 0) {
+            prev[0] = myp[0]; prev[1] = myp[4];
+            if constexpr (COUL) { prevJ[0] = mypJ[0]; prevJ[1] = mypJ[4]; }
+        }
         mbar_wait(full + 8 * cslot, cphase);            // first stage of the item: its descriptor is in the ring now
         const ExTile tile = ring[n % EX_RING];
-        switch (tile.nfrag) {                           // warp- and CTA-uniform
-            case 1: ex_kloop<1>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            case 2: ex_kloop<2>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            case 3: ex_kloop<3>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            case 4: ex_kloop<4>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            case 5: ex_kloop<5>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            case 6: ex_kloop<6>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            case 7: ex_kloop<7>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
-            default: ex_kloop<8>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+#define LO_EX_CASE(NF_) ex_kloop<NF_, COUL, MFMAX>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB, accC, accD)
+        if constexpr (COUL) {
+            switch (tile.nfrag) {                       // warp- and CTA-uniform; COUL tiles have at most 4 fragments
+                case 1: LO_EX_CASE(1); break;
+                case 2: LO_EX_CASE(2); break;
+                case 3: LO_EX_CASE(3); break;
+                default: LO_EX_CASE(4); break;
+            }
+        } else {
+            switch (tile.nfrag) {
+                case 1: LO_EX_CASE(1); break;
+                case 2: LO_EX_CASE(2); break;
+                case 3: LO_EX_CASE(3); break;
+                case 4: LO_EX_CASE(4); break;
+                case 5: LO_EX_CASE(COUL ? 4 : 5); break;
+                case 6: LO_EX_CASE(COUL ? 4 : 6); break;
+                case 7: LO_EX_CASE(COUL ? 4 : 7); break;
+                default: LO_EX_CASE(COUL ? 4 : 8); break;
+            }
         }
+#undef LO_EX_CASE
         // fused epilogue: e[w] = sum over this lane's rows of weight * a * b (complex), then over the 8 row groups of
         // the warp (shuffles), in a fixed order; fragments beyond nfrag hold zeros
-        double e[2][2];
+        double e[2][2], eJ[2][2];
 #pragma unroll
-        for (int nf = 0; nf < 2; ++nf) e[nf][0] = e[nf][1] = 0.0;
+        for (int nf = 0; nf < 2; ++nf) e[nf][0] = e[nf][1] = eJ[nf][0] = eJ[nf][1] = 0.0;
 #pragma unroll
-        for (int mf = 0; mf < 8; ++mf) {
+        for (int mf = 0; mf < MFMAX; ++mf) {
             const double wv = (mf < tile.nfrag) ? __ldg(wgt + tile.row0 + mf * 8 + g) : 0.0;
 #pragma unroll
             for (int nf = 0; nf < 2; ++nf) {
@@ -662,6 +694,12 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
                 e[nf][0] = fma(wv, ar * br - ai * bi, e[nf][0]);
                 e[nf][1] = fma(wv, ar * bi + ai * br, e[nf][1]);
                 accA[mf][nf][0] = accA[mf][nf][1] = accB[mf][nf][0] = accB[mf][nf][1] = 0.0;
+                if constexpr (COUL) {
+                    ar = accC[mf][nf][0]; ai = accC[mf][nf][1]; br = accD[mf][nf][0]; bi = accD[mf][nf][1];
+                    eJ[nf][0] = fma(wv, ar * br - ai * bi, eJ[nf][0]);
+                    eJ[nf][1] = fma(wv, ar * bi + ai * br, eJ[nf][1]);
+                    accC[mf][nf][0] = accC[mf][nf][1] = accD[mf][nf][0] = accD[mf][nf][1] = 0.0;
+                }
             }
         }
 #pragma unroll
@@ -673,10 +711,21 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
                 v += __shfl_xor_sync(0xffffffffu, v, 8);
                 v += __shfl_xor_sync(0xffffffffu, v, 16);
                 e[nf][c] = v;
+                if constexpr (COUL) {
+                    v = eJ[nf][c];
+                    v += __shfl_xor_sync(0xffffffffu, v, 4);
+                    v += __shfl_xor_sync(0xffffffffu, v, 8);
+                    v += __shfl_xor_sync(0xffffffffu, v, 16);
+                    eJ[nf][c] = v;
+                }
             }
         if (g == 0) {
             myp[0] = make_double2(prev[0].x + e[0][0], prev[0].y + e[0][1]);
             myp[4] = make_double2(prev[1].x + e[1][0], prev[1].y + e[1][1]);
+            if constexpr (COUL) {
+                mypJ[0] = make_double2(prevJ[0].x + eJ[0][0], prevJ[0].y + eJ[0][1]);
+                mypJ[4] = make_double2(prevJ[1].x + eJ[1][0], prevJ[1].y + eJ[1][1]);
+            }
         }
     }
 }
@@ -696,7 +745,8 @@ __global__ void __launch_bounds__(128) k_pack_x(const double2* __restrict__ x, d
 __global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, const double2* __restrict__ E1raw,
                            const double2* __restrict__ EKpart, int n_ctas, const int* __restrict__ status, int n_spin, int Wcap,
                            int n_w, double c1, double cJ, double2* __restrict__ E_L, double2* __restrict__ E1, double2* __restrict__ E_J,
-                           double2* __restrict__ E_K, int* __restrict__ st_out, double2* __restrict__ Eout4) {
+                           double2* __restrict__ E_K, int* __restrict__ st_out, double2* __restrict__ Eout4,
+                           const double2* __restrict__ EJLpart) {
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= n_w) return;
     double2 ej = make_double2(0.0, 0.0), ek = make_double2(0.0, 0.0);
@@ -705,6 +755,12 @@ __global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, con
     double2 e1 = E1raw[w];
     e1.x *= c1; e1.y *= c1;
     ej.x *= cJ; ej.y *= cJ;
+    if (EJLpart) {
+        // paper-literal compressed Coulomb term (Eq. 19/22): E_J^LO = 2 sum_{i<=j} m_ij sum_K sigma_K aJ_K bJ_K = -2 sum(wgt aJ bJ)
+        ej = make_double2(0.0, 0.0);
+        for (int b = 0; b < n_ctas; ++b) { double2 v = EJLpart[(size_t)b * Wcap + w]; ej.x += v.x; ej.y += v.y; }
+        ej.x *= -2.0; ej.y *= -2.0;
+    }
     int bad = status[w];
     if (n_spin == 2) bad |= status[Wcap + w];
     if (bad) {
@@ -788,7 +844,8 @@ lo_status configure_kernels() {
     cudaError_t e;
     e = cudaFuncSetAttribute(k_coulomb, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_coulomb): ") + cudaGetErrorString(e)); return LO_ECUDA; }
-    e = cudaFuncSetAttribute(k_exchange, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    e = cudaFuncSetAttribute(k_exchange<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_exchange): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
@@ -861,9 +918,15 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
     int ex_grid = 0;
     {
         Timer tm(f, stream, LO_K_EXCHANGE);
-        long long items = f->n_tiles * NB;
+        const bool coul = f->coulomb_lo != 0;
+        long long items = (coul ? f->n_tiles4 : f->n_tiles) * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        k_exchange<<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad, ldw, f->dEKpart, Wcap);
+        if (coul)
+            k_exchange<true><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, f->dTiles4, items, NB, N_pad,
+                                                                ldw, f->dEKpart, f->dEJLpart, Wcap);
+        else
+            k_exchange<false><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad,
+                                                                 ldw, f->dEKpart, nullptr, Wcap);
     }
     // ---- S5
     {
@@ -871,7 +934,8 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
         const double c1 = f->n_spin == 1 ? 2.0 : 1.0, cJ = f->n_spin == 1 ? 2.0 : 0.5;
         k_finalize<<<(n_w + 127) / 128, 128, 0, stream>>>(EJpart, RB, E1raw, (const double2*)f->dEKpart, ex_grid, f->dStatus, f->n_spin, Wcap,
                                                           n_w, c1, cJ, (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K,
-                                                          walker_status, (double2*)Eout4);
+                                                          walker_status, (double2*)Eout4,
+                                                          f->coulomb_lo ? (const double2*)f->dEJLpart : nullptr);
     }
     f->last_n_w = n_w;
     cudaError_t e = cudaGetLastError();

@@ -389,3 +389,49 @@ def test_propagator_needs_flag(c0):
     F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=0, max_walkers=4, gpu_svd=True)
     with pytest.raises(lo.LoError):
         F.propagator(torch.zeros((4, c0.n_chol), dtype=torch.complex128, device="cuda"))
+
+
+# ------------------------------------------------------------------------------------------ NEXT-3: compressed Coulomb
+@pytest.mark.parametrize("T,reading", [(1e-4, "element"), (1e-2, "element"), (1e-6, "vector")])
+def test_compressed_coulomb_mode(T, reading):
+    """lo_set_coulomb_mode(COMPRESSED): E_J = 2 sum_{i<=j} m_ij sum_K sigma_K (U^T Theta_i)_K (W Theta_j)_K (Eq. 19/22
+    first term) from the same tiles as the exchange, against the oracle's paper-literal sum on
+    the library's factor set; E1 and E_K are those of the default mode bit for bit up to the tile cut (1e-10), and
+    E_L = E1 + E_J^LO + E_K.  Ragged ranks (T=1e-2 truncates; the vector reading has ranks 11-12) and a ragged batch."""
+    P = gen.make_problem(1, reading=reading)
+    n_w = 70
+    phis = gen.make_walkers(P, n_w)
+    F = lo.Factors.setup(P.h, P.L, P.psi, T, device=0, max_walkers=n_w, gpu_svd=True)
+    E_ch, _ = gpu_energy(F, phis)
+    F.set_coulomb_mode(True)
+    E_lo, st = gpu_energy(F, phis)
+    assert (st == 0).all()
+    fs = oracle_factor_sets(P, F)[0]
+    scale = np.abs(E_ch[:, 0])
+    for w in range(n_w):
+        th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+        ej = 2.0 * oracle.coulomb_lo(fs, th)
+        assert abs(E_lo[w, 2] - ej) <= TOL * scale[w]
+    assert (np.abs(E_lo[:, 1] - E_ch[:, 1]) <= TOL * scale).all() and (np.abs(E_lo[:, 3] - E_ch[:, 3]) <= TOL * scale).all()
+    assert (np.abs(E_lo[:, 0] - (E_lo[:, 1] + E_lo[:, 2] + E_lo[:, 3])) <= TOL * scale).all()
+    # the compressed Coulomb term carries a truncation error of the same order as the exchange's
+    if T >= 1e-2:
+        assert np.abs(E_lo[:, 2] - E_ch[:, 2]).max() > 1e-9 * scale.max()
+    F.set_coulomb_mode(False)
+    E_back, _ = gpu_energy(F, phis)
+    assert np.array_equal(E_back, E_ch)
+
+
+def test_compressed_coulomb_exact_at_zero_threshold(c0, c0_walkers):
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 0.0, device=0, max_walkers=c0.n_w, gpu_svd=True)
+    E_ch, _ = gpu_energy(F, c0_walkers)
+    F.set_coulomb_mode(True)
+    E_lo, _ = gpu_energy(F, c0_walkers)
+    assert (np.abs(E_lo - E_ch).max(axis=1) <= 1e-10 * np.abs(E_ch[:, 0])).all()
+
+
+def test_compressed_coulomb_rejects_unrestricted():
+    P = gen.make_problem_from_geometry(*gen.site_geometry(0), n_occ=(3, 2), n_chol=24, seed=7)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-8, device=0, max_walkers=2, gpu_svd=True)
+    with pytest.raises(lo.LoError):
+        F.set_coulomb_mode(True)
