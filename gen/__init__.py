@@ -4,6 +4,6 @@ This package produces *data only* (geometry, h, L, Psi, Phi).  It holds none of 
 LO-AFQMC arithmetic, and is the one module both the CPU oracle's tests and the CUDA
 path's tests/bench share.  See DESIGN.md "Input recipe".
 """
-from .configs import (CONFIGS, Problem, make_problem, make_problem_from_geometry, make_walkers,  # noqa: F401
+from .configs import (CONFIGS, CasTrial, Problem, make_cas_trial, make_problem, make_problem_from_geometry, make_walkers,  # noqa: F401
                       site_geometry,
                       random_orthogonal)

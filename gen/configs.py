@@ -245,3 +245,65 @@ def random_orthogonal(n: int, seed: int) -> np.ndarray:
     """Haar-ish random orthogonal matrix (QR of a normal draw, sign-fixed); used by rotation pins."""
     q, r = np.linalg.qr(_rng(seed, _TAG_ROT).standard_normal((n, n)))
     return q * np.sign(np.diag(r))
+
+
+_TAG_CAS = 7
+
+
+@dataclass
+class CasTrial:
+    """A seeded multi-determinant (CAS-type) trial sum_d c_d |d> of closed-shell determinants (the same excitation in
+    both spins), every |d> at most `max_exc` excitations away from the reference: data only."""
+    C: np.ndarray        # [N, n_ref + n_virt] orthonormal orbitals: reference occupied first, then active virtuals
+    n_ref: int
+    holes: np.ndarray    # [n_det, max_exc] int32: replaced column positions of the reference (< n_ref), -1 = unused
+    parts: np.ndarray    # [n_det, max_exc] int32: orbital (column of C, >= n_ref) put in that position, -1 = unused
+    coef: np.ndarray     # [n_det] fp64 CI coefficients c_d
+
+    @property
+    def n_det(self):
+        return len(self.coef)
+
+    def columns(self, d):
+        """Columns of C occupied in determinant d, in the reference's column positions."""
+        cols = np.arange(self.n_ref)
+        for hpos, part in zip(self.holes[d], self.parts[d]):
+            if hpos >= 0:
+                cols[hpos] = part
+        return cols
+
+
+def make_cas_trial(problem: Problem, n_virt: int, n_act_occ: int, n_det: int, max_exc: int, seed: int | None = None) -> CasTrial:
+    """Reference = problem.psi[0]; `n_virt` active virtuals = Gaussian columns damped like the occupied ones, projected
+    onto the complement of the reference and Loewdin-orthonormalised; determinant 0 is the reference (c=1), the others
+    replace e in 1..max_exc of the last `n_act_occ` reference columns by distinct virtuals (no duplicates), with
+    c_d = 0.3 N(0,1) 2^-e."""
+    seed = problem.seed if seed is None else seed
+    rng = _rng(seed, _TAG_CAS)
+    psi = problem.psi[0]
+    N, O = psi.shape
+    Rp = problem.site_xyz[problem.site_of_fn]
+    centers = problem.site_xyz[np.arange(n_virt) % len(problem.site_xyz)]
+    damp = np.exp(-np.linalg.norm(Rp[:, None, :] - centers[None, :, :], axis=2))
+    v = rng.standard_normal((N, n_virt)) * damp
+    v = v - psi @ (psi.T @ v)
+    v = _lowdin(v)
+    v = v - psi @ (psi.T @ v)          # re-project: keeps C^T C = 1 to rounding
+    C = np.ascontiguousarray(np.concatenate([psi, _lowdin(v)], axis=1))
+    holes = -np.ones((n_det, max_exc), dtype=np.int32)
+    parts = -np.ones((n_det, max_exc), dtype=np.int32)
+    coef = np.ones(n_det)
+    seen = {()}
+    d = 1
+    while d < n_det:
+        e = int(rng.integers(1, min(max_exc, n_act_occ, n_virt) + 1))
+        hs = np.sort(rng.choice(np.arange(O - n_act_occ, O), e, replace=False))
+        ps = np.sort(rng.choice(np.arange(O, O + n_virt), e, replace=False))
+        key = tuple(hs) + tuple(ps)
+        if key in seen:
+            continue
+        seen.add(key)
+        holes[d, :e], parts[d, :e] = hs, ps
+        coef[d] = 0.3 * rng.standard_normal() * 0.5 ** e
+        d += 1
+    return CasTrial(C=C, n_ref=O, holes=holes, parts=parts, coef=coef)

@@ -335,3 +335,48 @@ def local_energy_lo_streamed(psis, Lbars, hbars, phis, n_pairs, fetch, chunk=256
     E[ok, 3] = ek[ok]
     E[ok, 0] = E[ok, 1] + E[ok, 2] + E[ok, 3]
     return E, status, secs
+
+
+# ------------------------------------------------------------------ NEXT-2: multi-determinant trial (Eq. 12, 13)
+def sub_factor_set(fs: FactorSet, cols) -> FactorSet:
+    """Factors of the pairs among the orbitals `cols` (ascending) of a factor set over more orbitals, re-indexed to
+    0..len(cols)-1: the integrals of a determinant that occupies exactly those orbitals."""
+    cols = np.asarray(cols)
+    assert (np.diff(cols) > 0).all()
+    pos = -np.ones(fs.O, dtype=np.int64)
+    pos[cols] = np.arange(len(cols))
+    keep = [k for k in range(len(fs.r)) if pos[fs.pi[k]] >= 0 and pos[fs.pj[k]] >= 0]
+    rows = np.concatenate([np.arange(fs.off[k], fs.off[k] + fs.r[k]) for k in keep]) if keep else np.zeros(0, np.int64)
+    return make_factor_set(fs.N, len(cols), pos[fs.pi[keep]], pos[fs.pj[keep]], fs.r[keep], fs.U[rows], fs.sigma[rows], fs.W[rows])
+
+
+def local_energy_cas(Cmo, columns, coef, Lbar, hbar, fs, phi, exact=False):
+    """Local energy of ONE closed-shell walker phi [N,O] with the multi-determinant trial sum_d c_d |d>, every |d> a
+    closed-shell determinant occupying the orbitals columns[d] (columns of Cmo, in the reference's column positions),
+    straight from the definition (Eq. 12 with Eq. 13, applied to every energy term):
+        E = sum_d w_d E^d / sum_d w_d,   w_d = c_d <d|phi> = c_d det(Psi_d^T phi)^2   (alpha and beta strings equal),
+    E^d = the single-determinant local energy with trial Psi_d = Cmo[:, columns[d]] (Theta^d by its own LU, Eq. 15).
+    Lbar [X,n_orb,N], hbar [n_orb,N]: half-rotated integrals for ALL orbitals of Cmo; fs: factor set over all their
+    pairs (exchange by O5 on the sub-set of pairs the determinant occupies); exact=True uses the Cholesky route (O2)
+    for the exchange instead.  Returns (E_L, E1, E_J, E_K, sum_d w_d / det(Psi_0^T phi)^2)."""
+    Cmo, phi = _f64(Cmo), _c128(phi)
+    num = np.zeros(3, dtype=np.complex128)
+    den = 0.0 + 0.0j
+    w0 = None
+    for d, cols in enumerate(columns):
+        cols = np.asarray(cols)
+        th, det, st = theta(Cmo[:, cols], phi)
+        if w0 is None:
+            w0 = det * det                    # determinant 0 is the reference
+        if st != 0:
+            continue                          # <d|phi> = 0: no contribution
+        order = np.argsort(cols)
+        sc = cols[order]
+        ths = np.ascontiguousarray(th[:, order])
+        e1, ej = onebody_coulomb([np.ascontiguousarray(Lbar[:, sc, :])], [np.ascontiguousarray(hbar[sc])], [ths])
+        ek = exchange_cholesky(np.ascontiguousarray(Lbar[:, sc, :]), ths) if exact else exchange_lo(sub_factor_set(fs, sc), ths)
+        w = coef[d] * det * det
+        num += w * np.array([e1, ej, ek])
+        den += w
+    E = num / den
+    return E.sum(), E[0], E[1], E[2], den / w0

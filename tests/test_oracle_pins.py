@@ -351,3 +351,57 @@ def test_propagator_pins(c0, c0_walkers):
     # linearity in the fields
     y = rng.standard_normal(X) + 1j * rng.standard_normal(X)
     assert np.abs(oracle.propagator(L, 2.0 * x - 1j * y) - (2.0 * B - 1j * oracle.propagator(L, y))).max() <= 1e-12 * np.abs(B).max()
+
+
+# ------------------------------------------------------------------------------------------ NEXT-2: multi-determinant trial
+def test_cas_exact_eigenstate_two_orbitals():
+    """Textbook pin (two electrons in two orbitals of different symmetry): with h diagonal and every Cholesky matrix
+    either diagonal or purely off-diagonal, the closed-shell determinants |1 1bar>, |2 2bar> decouple from the singly
+    excited ones, H restricted to them is [[2h1+(11|11), (12|12)], [(12|12), 2h2+(22|22)]] (Slater-Condon), and its
+    eigenvectors are eigenstates of the full H.  The mixed estimator <Psi_T|H|phi>/<Psi_T|phi> of an eigenstate is its
+    eigenvalue for ANY walker: pins the weights c_d det^2, the per-determinant Green's functions and all three terms."""
+    h = np.diag([-1.3, 0.4])
+    L = np.zeros((3, 2, 2))
+    L[0] = np.diag([0.9, 0.5])
+    L[1] = np.diag([-0.3, 0.7])
+    L[2] = np.array([[0.0, 0.6], [0.6, 0.0]])
+    J11, J22, K12 = (L[:2, 0, 0] ** 2).sum(), (L[:2, 1, 1] ** 2).sum(), L[2, 0, 1] ** 2
+    H = np.array([[2 * h[0, 0] + J11, K12], [K12, 2 * h[1, 1] + J22]])
+    ev, vec = np.linalg.eigh(H)
+    Cmo = np.eye(2)
+    Lbar, hbar = oracle.half_rotate(L, h, Cmo)
+    fs = oracle.own_factors(Lbar, 0.0)
+    rng = np.random.default_rng(3)
+    for k in range(2):
+        for _ in range(3):
+            phi = (rng.standard_normal((2, 1)) + 1j * rng.standard_normal((2, 1)))
+            for exact in (True, False):
+                E = oracle.local_energy_cas(Cmo, [[0], [1]], vec[:, k], Lbar, hbar, fs, phi, exact=exact)
+                assert abs(E[0] - ev[k]) <= 1e-12 * max(1.0, abs(ev[k]))
+
+
+def test_cas_single_determinant_and_bruteforce(c0, c0_walkers):
+    """N_det = 1 is the single-determinant energy; a duplicated determinant changes nothing; and for a real expansion
+    the weighted sum of per-determinant brute-force energies (Eq. 10 with the G^d of Eq. 13, N^4 sums) agrees."""
+    T = gen.make_cas_trial(c0, n_virt=3, n_act_occ=3, n_det=6, max_exc=2)
+    Lbar, hbar = oracle.half_rotate(c0.L, c0.h, T.C)
+    fs = oracle.own_factors(Lbar, 0.0)
+    cols = [T.columns(d) for d in range(T.n_det)]
+    phi = c0_walkers[0][1]
+    single = oracle.local_energy_exact(c0.h, c0.L, c0.psi, [phi], "cholesky")
+    one = oracle.local_energy_cas(T.C, cols[:1], T.coef[:1], Lbar, hbar, fs, phi)
+    assert abs(one[0] - single[0]) <= 1e-11 * abs(single[0]) and abs(one[4] - 1.0) <= 1e-13
+    dup = oracle.local_energy_cas(T.C, [cols[0], cols[0]], [0.3, 0.9], Lbar, hbar, fs, phi)
+    assert abs(dup[0] - single[0]) <= 1e-11 * abs(single[0])
+    E = oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi)
+    Ex = oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi, exact=True)
+    num, den = 0.0, 0.0
+    for d in range(T.n_det):
+        psi_d = np.ascontiguousarray(T.C[:, cols[d]])
+        th, det, st = oracle.theta(psi_d, phi)
+        G = oracle.green(psi_d, th)
+        e = oracle.energy_bruteforce(c0.h, c0.L, G)
+        num += T.coef[d] * det * det * e.sum()
+        den += T.coef[d] * det * det
+    assert abs(E[0] - num / den) <= 1e-10 * abs(E[0]) and abs(Ex[0] - num / den) <= 1e-10 * abs(E[0])
+    assert abs(E[0] - single[0]) > 1e-6 * abs(E[0])          # the expansion does change the energy
