@@ -124,6 +124,28 @@ lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld);
 #define LO_COULOMB_COMPRESSED 1
 lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
 
+/* SURVEY 8(f) NEXT-2, multi-determinant (CAS-type) trial |Psi_T> = sum_d c_d |d> of closed-shell determinants (the
+ * same excitation string in both spins), each at most max_exc (<= 8) excitations from the reference:
+ *   E = sum_d w_d E^d / sum_d w_d,  w_d = c_d <d|Phi>   (Eq. 12 with Eq. 13, applied to every energy term)
+ * evaluated by direct summation over determinants ("direct summation"); the determinants' overlaps and
+ * half-rotated Green's functions come from Sherman-Morrison-Woodbury updates of the reference (Eq. 20),
+ * and every (walker, determinant) runs through the Coulomb / exchange kernels as one virtual walker.  The factor set
+ * must have been built (n_spin = 1) with psi = [reference occupied orbitals | active virtual orbitals], i.e.
+ * n_occ[0] = n_ref + n_virt orthonormal columns, and max_walkers >= max_real_walkers * n_det.
+ *   holes  host int32 [n_det][max_exc]: replaced column positions of the reference (< n_ref), -1 padding at the end
+ *   parts  host int32 [n_det][max_exc]: the orbital (column of psi, in [n_ref, n_occ[0])) put in that position
+ *   coef   host [n_det]: c_d.   Determinant 0 is normally the reference (no excitation).
+ * lo_set_cas_trial copies the lists and reserves the workspace; it may be called again to replace the trial.
+ * lo_local_energy_cas: phi device complex128 [n_w][N][n_ref]; E_L (required), E1, E_J, E_K, ovlp device complex128
+ * [n_w] (ovlp = sum_d w_d / <reference|Phi>, the trial overlap in units of the reference overlap); walker_status as in
+ * lo_local_energy.  A determinant with a singular overlap contributes nothing.  Asynchronous; allocates nothing.
+ * The rearranged SMW energy of Eq. 23 (cost independent of N_det in the leading term) is not built: cost here is n_det x
+ * the single-determinant evaluation. */
+lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts,
+                           const double* coef, int max_real_walkers);
+lo_status lo_local_energy_cas(const lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K,
+                              void* ovlp, int* walker_status, void* stream);
+
 /* SURVEY 8(f) NEXT-1, propagator formation: B_w = sum_g x^g_w L^g ("forming the propagation matrix
  * (B = sum_alpha x_alpha L_alpha), scaling as X M^2"), for n_w walkers at once as one real x
  * complex FP64 GEMM on the DMMA pipe ([N(N+1)/2 x n_chol] x [n_chol x 2 n_w]).  Every L^g is symmetric, so B_w is

@@ -396,6 +396,14 @@ void free_all(lo_factors* f) {
         for (auto& ev : f->pool) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
         f->bU.release();
         f->bW.release();
+        if (f->cas) {
+            void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd,
+                          f->cas->dEv, f->cas->dSt0};
+            for (void* q : cp)
+                if (q) cudaFree(q);
+            delete f->cas;
+            f->cas = nullptr;
+        }
         if (f->copyStream) cudaStreamDestroy(f->copyStream);
         for (int c = 0; c < LO_HOST_CHUNKS; ++c)
             if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
@@ -774,6 +782,77 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode) {
     }
     f->coulomb_lo = mode == LO_COULOMB_COMPRESSED ? 1 : 0;
     return LO_OK;
+}
+
+lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts, const double* coef,
+                           int max_real_walkers) {
+    if (!f || !holes || !parts || !coef) { set_error("lo_set_cas_trial: NULL argument"); return LO_EINVAL; }
+    if (f->device < 0) { set_error("lo_set_cas_trial: no device"); return LO_ECUDA; }
+    if (f->n_spin != 1) { set_error("lo_set_cas_trial: closed-shell factor sets only (n_spin == 1)"); return LO_EINVAL; }
+    const int n_orb = f->n_occ[0];
+    if (n_ref <= 0 || n_ref > n_orb || n_det <= 0 || max_exc <= 0 || max_exc > CAS_MAX_EXC || max_real_walkers <= 0 ||
+        (long long)max_real_walkers * n_det > f->max_walkers) {
+        set_error("lo_set_cas_trial: invalid sizes (need 0 < n_ref <= n_occ, 1 <= max_exc <= 8, max_real_walkers * n_det <= max_walkers)");
+        return LO_EINVAL;
+    }
+    for (int d = 0; d < n_det; ++d) {
+        bool ended = false;
+        for (int k = 0; k < max_exc; ++k) {
+            const int h = holes[(size_t)d * max_exc + k], p = parts[(size_t)d * max_exc + k];
+            if (h < 0 || p < 0) { if (h >= 0 || p >= 0) { set_error("lo_set_cas_trial: hole/particle lists of different length"); return LO_EINVAL; } ended = true; continue; }
+            if (ended || h >= n_ref || p < n_ref || p >= n_orb) { set_error("lo_set_cas_trial: hole must be < n_ref, particle in [n_ref, n_occ), -1 padding at the end"); return LO_EINVAL; }
+            for (int l = 0; l < k; ++l)
+                if (holes[(size_t)d * max_exc + l] == h || parts[(size_t)d * max_exc + l] == p) { set_error("lo_set_cas_trial: repeated hole or particle in one determinant"); return LO_EINVAL; }
+        }
+    }
+    CK(cudaSetDevice(f->device));
+    if (f->cas) {
+        void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd, f->cas->dEv, f->cas->dSt0};
+        for (void* q : cp)
+            if (q) cudaFree(q);
+        delete f->cas;
+        f->cas = nullptr;
+    }
+    CasPlan* c = new (std::nothrow) CasPlan();
+    if (!c) { set_error("lo_set_cas_trial: out of host memory"); return LO_ENOMEM; }
+    f->cas = c;
+    c->n_ref = n_ref; c->n_det = n_det; c->max_exc = max_exc; c->n_virt = n_orb - n_ref; c->max_real = max_real_walkers;
+    c->W0cap = round_up(max_real_walkers, WALKER_TILE);
+    const size_t nv = (size_t)max_real_walkers * n_det, ne = (size_t)n_det * max_exc;
+    auto al = [&](void** p, size_t bytes) -> cudaError_t {
+        cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16));
+        if (e == cudaSuccess) e = cudaMemset(*p, 0, std::max<size_t>(bytes, 16));
+        return e;
+    };
+    CK(al((void**)&c->dHoles, ne * 4));
+    CK(al((void**)&c->dParts, ne * 4));
+    CK(al((void**)&c->dCoef, (size_t)n_det * 8));
+    CK(al((void**)&c->dTh0, (size_t)n_ref * 2 * c->W0cap * f->N_pad * 8));
+    CK(al((void**)&c->dA0, (size_t)c->W0cap * n_ref * n_ref * 16));
+    CK(al((void**)&c->dT, (size_t)c->W0cap * std::max(c->n_virt, 1) * n_ref * 16));
+    CK(al((void**)&c->dG, nv * max_exc * n_orb * 16));
+    CK(al((void**)&c->dWd, nv * 16));
+    CK(al((void**)&c->dEv, nv * 4 * 16));
+    CK(al((void**)&c->dSt0, (size_t)c->W0cap * 4));
+    CK(cudaMemcpy(c->dHoles, holes, ne * 4, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->dParts, parts, ne * 4, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->dCoef, coef, (size_t)n_det * 8, cudaMemcpyHostToDevice));
+    return LO_OK;
+}
+
+lo_status lo_local_energy_cas(const lo_factors* fc, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
+                              int* walker_status, void* stream) {
+    if (!fc || !phi || !E_L) { set_error("lo_local_energy_cas: NULL argument"); return LO_EINVAL; }
+    if (fc->device < 0) { set_error("lo_local_energy_cas: no device; there is no CPU path"); return LO_ECUDA; }
+    if (!fc->cas) { set_error("lo_local_energy_cas: call lo_set_cas_trial first"); return LO_EINVAL; }
+    if (n_w <= 0 || n_w > fc->cas->max_real) { set_error("lo_local_energy_cas: n_w out of range (1..max_real_walkers)"); return LO_EINVAL; }
+    if (((uintptr_t)phi & 15) || ((uintptr_t)E_L & 15) || ((uintptr_t)E1 & 15) || ((uintptr_t)E_J & 15) || ((uintptr_t)E_K & 15) || ((uintptr_t)ovlp & 15)) {
+        set_error("lo_local_energy_cas: pointers must be 16-byte aligned");
+        return LO_EINVAL;
+    }
+    lo_factors* f = const_cast<lo_factors*>(fc);
+    CK(cudaSetDevice(f->device));
+    return launch_local_energy_cas(f, n_w, phi, E_L, E1, E_J, E_K, ovlp, walker_status, (cudaStream_t)stream);
 }
 
 lo_status lo_propagator(const lo_factors* fc, int n_w, const void* x_dev, void* stream) {

@@ -69,6 +69,23 @@ struct GatherRec {
     int r, pad_;
 };
 
+// Multi-determinant trial (lo_set_cas_trial): determinants as excitation lists of the reference
+// (= the first n_ref orbitals of the factor set's Psi), workspace for max_real real walkers; the n_det determinants of a
+// real walker are laid out as n_det consecutive VIRTUAL walkers of the ordinary S3-S5 path.
+constexpr int CAS_MAX_EXC = 8;
+struct CasPlan {
+    int n_ref = 0, n_det = 0, max_exc = 0, n_virt = 0, max_real = 0, W0cap = 0;
+    int *dHoles = nullptr, *dParts = nullptr;   // [n_det][max_exc]
+    double* dCoef = nullptr;                    // [n_det]
+    double* dTh0 = nullptr;                     // Theta0^T panels [n_ref][2*W0cap][N_pad]
+    double* dA0 = nullptr;                      // [W0cap][n_ref][n_ref] complex
+    double* dT = nullptr;                       // T = C_virt^T Theta0: [W0cap][n_virt][n_ref] complex
+    double* dG = nullptr;                       // SMW coefficients [max_real*n_det][max_exc][n_orb] complex
+    double* dWd = nullptr;                      // weights c_d det(T_d)^2: [max_real*n_det] complex
+    double* dEv = nullptr;                      // per virtual walker {E_L,E1,E_J,E_K}: [max_real*n_det][4] complex
+    int* dSt0 = nullptr;                        // [W0cap] status of the reference overlap
+};
+
 struct TimingEvent {
     cudaEvent_t e0, e1;
     int kind;
@@ -119,6 +136,7 @@ struct lo_factors {
     cudaEvent_t evCopy[LO_HOST_CHUNKS] = {nullptr, nullptr, nullptr, nullptr};
     unsigned long long factor_bytes = 0, lbar_bytes = 0, workspace_bytes = 0;
     int last_n_w = 0;
+    lo::CasPlan* cas = nullptr;
     // timing
     bool timing = false;
     std::vector<lo::TimingEvent> events;
@@ -134,6 +152,8 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
                               void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 lo_status configure_kernels();
 lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStream_t stream);
+lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
+                                  int* walker_status, cudaStream_t stream);
 // 2D fp64 tensor map over a row-major [rows][inner] array, box [box_rows][16], 128-byte swizzle, zero OOB fill.
 lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner, unsigned long long rows, unsigned box_rows);   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)
 

@@ -104,7 +104,7 @@ __host__ __device__ inline int ov_ldb(int O) { int nf8 = min((2 * O + 7) / 8, OV
 
 template <int MFB, int NFW>
 __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi, const double2* __restrict__ phi, double2* __restrict__ A,
-                                                 int N, int O) {
+                                                 int N, int O, int ldpsi) {
     extern __shared__ __align__(16) double sm[];
     const int LDB = ov_ldb(O), nf0 = blockIdx.z * OV_NFB, NF = min((2 * O + 7) / 8 - nf0, OV_NFB), c0 = nf0 * 8;
     double* As = sm;                   // [OV_PC][OV_LDA]
@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
         __syncthreads();
         for (int e = tid; e < OV_PC * (MFB * 8); e += 256) {
             const int pp = e / (MFB * 8), c = e - pp * (MFB * 8), pg = p0 + pp;
-            As[pp * OV_LDA + c] = (pg < N && i0 + c < O) ? psi[(size_t)pg * O + i0 + c] : 0.0;
+            As[pp * OV_LDA + c] = (pg < N && i0 + c < O) ? psi[(size_t)pg * ldpsi + i0 + c] : 0.0;
         }
         for (int e = tid; e < OV_PC * ncb; e += 256) {
             const int pp = e / ncb, c = e - pp * ncb, pg = p0 + pp;
@@ -741,6 +741,177 @@ __global__ void __launch_bounds__(128) k_pack_x(const double2* __restrict__ x, d
     XT[(size_t)(2 * w + 1) * Xk_pad + g] = v.y;
 }
 
+// ------------------------------------------------------------------------------------------------ NEXT-2: multi-determinant trial
+// Sherman-Morrison-Woodbury update of the reference (Eq. 20): determinant d replaces the reference columns
+// h_1..h_e by the orbitals p_1..p_e, A_d = A + U V^T.  With T = C_virt^T Theta0 (Theta0 = Phi A^-1) and T_d = T[p_k, h_l]:
+//   det A_d / det A = det T_d,      Theta^d = Theta0 (I - E_h T_d^-1 (T[p,:] - I[h,:])),
+// so in orbital-indexed panels (x = orbital of the factor set, zero when d does not occupy x)
+//   Theta^d_x = [x reference, not a hole] Theta0_x + sum_k G_d[k][x] Theta0_{h_k},
+//   G_d[k][x] = -sum_l (T_d^-1)_kl T[p_l][x]  (x reference, not a hole),  (T_d^-1)_km  (x = p_m),  0 otherwise.
+// k_cas_T: T[w][v][a] = sum_p C[p][n_ref+v] Theta0[a][w][p]; grid n_w, one warp per (v,a), lanes over p.
+__global__ void __launch_bounds__(256) k_cas_T(const double* __restrict__ C, int ldc, const double* __restrict__ th0, double2* __restrict__ T,
+                                               int N, int N_pad, int n_ref, int n_virt, int ldw0) {
+    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int e = warp; e < n_virt * n_ref; e += 8) {
+        const int v = e / n_ref, a = e - v * n_ref;
+        const double* re = th0 + ((size_t)a * ldw0 + 2 * w) * N_pad;
+        const double* im = re + N_pad;
+        double sr = 0.0, si = 0.0;
+        for (int p = lane; p < N; p += 32) {
+            const double c = C[(size_t)p * ldc + n_ref + v];
+            sr = fma(c, re[p], sr);
+            si = fma(c, im[p], si);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
+        if (lane == 0) T[((size_t)w * n_virt + v) * n_ref + a] = make_double2(sr, si);
+    }
+}
+
+// One warp per virtual walker v = w*n_det + d: lane 0 inverts T_d (<= 8 x 8, Gauss-Jordan with partial pivoting) and
+// takes its determinant; all lanes then fill G_d.  weight = c_d det(T_d)^2 (closed shell: the same string in both spins);
+// status 1 when the reference overlap or T_d is singular (that determinant is then left out of the sums).
+__global__ void __launch_bounds__(128) k_cas_coef(const double2* __restrict__ T, const int* __restrict__ holes, const int* __restrict__ parts,
+                                                  const double* __restrict__ coef, const int* __restrict__ st0, double2* __restrict__ G,
+                                                  double2* __restrict__ wd, int* __restrict__ stv, int n_v, int n_det, int max_exc, int n_ref,
+                                                  int n_virt, int n_orb) {
+    __shared__ double2 inv_s[4][CAS_MAX_EXC][CAS_MAX_EXC];
+    __shared__ int ok_s[4];
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5, v = blockIdx.x * 4 + wi;
+    if (v >= n_v) return;
+    const int w = v / n_det, d = v - w * n_det;
+    const int* hs = holes + (size_t)d * max_exc;
+    const int* ps = parts + (size_t)d * max_exc;
+    int e = 0;
+    while (e < max_exc && hs[e] >= 0) ++e;
+    const double2* Tw = T + (size_t)w * n_virt * n_ref;
+    if (lane == 0) {
+        double2 M[CAS_MAX_EXC][CAS_MAX_EXC], I[CAS_MAX_EXC][CAS_MAX_EXC];
+        for (int k = 0; k < e; ++k)
+            for (int l = 0; l < e; ++l) {
+                M[k][l] = Tw[(size_t)(ps[k] - n_ref) * n_ref + hs[l]];
+                I[k][l] = make_double2(k == l ? 1.0 : 0.0, 0.0);
+            }
+        double2 det = make_double2(1.0, 0.0);
+        bool ok = st0[w] == 0;
+        for (int k = 0; k < e && ok; ++k) {
+            int piv = k;
+            double best = -1.0;
+            for (int r = k; r < e; ++r) {
+                double m = M[r][k].x * M[r][k].x + M[r][k].y * M[r][k].y;
+                if (!(m == m)) m = INFINITY;
+                if (m > best) { best = m; piv = r; }
+            }
+            if (!(best > 1e-300) || isinf(best)) { ok = false; break; }
+            if (piv != k) {
+                for (int c = 0; c < e; ++c) { double2 t1 = M[k][c]; M[k][c] = M[piv][c]; M[piv][c] = t1; t1 = I[k][c]; I[k][c] = I[piv][c]; I[piv][c] = t1; }
+                det = make_double2(-det.x, -det.y);
+            }
+            det = cmul(det, M[k][k]);
+            const double2 ip = crecip(M[k][k]);
+            for (int c = 0; c < e; ++c) { M[k][c] = cmul(M[k][c], ip); I[k][c] = cmul(I[k][c], ip); }
+            for (int r = 0; r < e; ++r) {
+                if (r == k) continue;
+                const double2 fct = M[r][k];
+                for (int c = 0; c < e; ++c) {
+                    double2 t1 = cmul(fct, M[k][c]), t2 = cmul(fct, I[k][c]);
+                    M[r][c] = make_double2(M[r][c].x - t1.x, M[r][c].y - t1.y);
+                    I[r][c] = make_double2(I[r][c].x - t2.x, I[r][c].y - t2.y);
+                }
+            }
+        }
+        for (int k = 0; k < e; ++k)
+            for (int l = 0; l < e; ++l) inv_s[wi][k][l] = I[k][l];
+        ok_s[wi] = ok ? 1 : 0;
+        const double2 d2 = cmul(det, det);
+        wd[v] = ok ? make_double2(coef[d] * d2.x, coef[d] * d2.y) : make_double2(0.0, 0.0);
+        stv[v] = ok ? 0 : 1;
+    }
+    __syncwarp();
+    const bool ok = ok_s[wi] != 0;
+    double2* Gv = G + (size_t)v * max_exc * n_orb;
+    for (int x = lane; x < n_orb; x += 32) {
+        int kind = x < n_ref ? 0 : -1;     // 0: reference non-hole, 1+m: particle p_m, -1: zero
+        for (int m = 0; m < e; ++m) {
+            if (hs[m] == x) kind = -1;
+            if (ps[m] == x) kind = 1 + m;
+        }
+        for (int k = 0; k < e; ++k) {
+            double2 gk = make_double2(0.0, 0.0);
+            if (ok && kind == 0) {
+                for (int l = 0; l < e; ++l) {
+                    const double2 t1 = cmul(inv_s[wi][k][l], Tw[(size_t)(ps[l] - n_ref) * n_ref + x]);
+                    gk.x -= t1.x; gk.y -= t1.y;
+                }
+            } else if (ok && kind > 0) {
+                gk = inv_s[wi][k][kind - 1];
+            }
+            Gv[(size_t)k * n_orb + x] = gk;
+        }
+    }
+}
+
+// Theta^d panels of every virtual walker: grid (n_v, n_orb, ceil(N_pad/128)), thread = basis index p.
+__global__ void __launch_bounds__(128) k_cas_theta(const double* __restrict__ th0, const double2* __restrict__ G, const int* __restrict__ holes,
+                                                   double* __restrict__ thT, int N_pad, int n_ref, int n_orb, int n_det, int max_exc, int ldw0,
+                                                   int ldw) {
+    const int p = blockIdx.z * 128 + threadIdx.x, x = blockIdx.y, v = blockIdx.x;
+    if (p >= N_pad) return;
+    const int w = v / n_det, d = v - w * n_det;
+    const int* hs = holes + (size_t)d * max_exc;
+    double re = 0.0, im = 0.0;
+    bool is_hole = false;
+    int e = 0;
+    for (; e < max_exc && hs[e] >= 0; ++e) is_hole |= hs[e] == x;
+    if (x < n_ref && !is_hole) {
+        re = th0[((size_t)x * ldw0 + 2 * w) * N_pad + p];
+        im = th0[((size_t)x * ldw0 + 2 * w + 1) * N_pad + p];
+    }
+    const double2* Gv = G + (size_t)v * max_exc * n_orb + x;
+    for (int k = 0; k < e; ++k) {
+        const double2 g = Gv[(size_t)k * n_orb];
+        const double tr = th0[((size_t)hs[k] * ldw0 + 2 * w) * N_pad + p], ti = th0[((size_t)hs[k] * ldw0 + 2 * w + 1) * N_pad + p];
+        re = fma(g.x, tr, fma(-g.y, ti, re));
+        im = fma(g.x, ti, fma(g.y, tr, im));
+    }
+    thT[((size_t)x * ldw + 2 * v) * N_pad + p] = re;
+    thT[((size_t)x * ldw + 2 * v + 1) * N_pad + p] = im;
+}
+
+// E = sum_d w_d E^d / sum_d w_d per real walker and energy term (Eq. 12), determinants in index order (fixed order).
+__global__ void k_cas_combine(const double2* __restrict__ Ev, const double2* __restrict__ wd, const int* __restrict__ stv,
+                              const int* __restrict__ st0, int n_w, int n_det, double2* __restrict__ E_L, double2* __restrict__ E1,
+                              double2* __restrict__ E_J, double2* __restrict__ E_K, double2* __restrict__ ovlp, int* __restrict__ st_out) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_w) return;
+    double2 num[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)}, den = make_double2(0.0, 0.0);
+    for (int d = 0; d < n_det; ++d) {
+        const size_t v = (size_t)w * n_det + d;
+        if (stv[v]) continue;
+        const double2 wv = wd[v];
+        for (int c = 0; c < 3; ++c) {
+            const double2 t1 = cmul(wv, Ev[4 * v + 1 + c]);
+            num[c].x += t1.x; num[c].y += t1.y;
+        }
+        den.x += wv.x; den.y += wv.y;
+    }
+    const double m2 = den.x * den.x + den.y * den.y;
+    const bool bad = st0[w] != 0 || !(m2 > 0.0) || isinf(m2);
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    double2 e[3], el = make_double2(0.0, 0.0);
+    const double2 id = bad ? make_double2(nan, nan) : crecip(den);
+    for (int c = 0; c < 3; ++c) {
+        e[c] = bad ? make_double2(nan, nan) : cmul(num[c], id);
+        el.x += e[c].x; el.y += e[c].y;
+    }
+    if (E_L) E_L[w] = el;
+    if (E1) E1[w] = e[0];
+    if (E_J) E_J[w] = e[1];
+    if (E_K) E_K[w] = e[2];
+    if (ovlp) ovlp[w] = bad ? make_double2(nan, nan) : den;
+    if (st_out) st_out[w] = bad ? 1 : 0;
+}
+
 // ------------------------------------------------------------------------------------------------ S5: combine
 __global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, const double2* __restrict__ E1raw,
                            const double2* __restrict__ EKpart, int n_ctas, const int* __restrict__ status, int n_spin, int Wcap,
@@ -806,7 +977,7 @@ int pick_split(long long base_items, int ksteps, int sms) {
     return best;
 }
 
-typedef void (*OvFn)(const double*, const double2*, double2*, int, int);
+typedef void (*OvFn)(const double*, const double2*, double2*, int, int, int);
 template <int M>
 OvFn ov_fn_n(int nfw) {
     switch (nfw) {
@@ -865,40 +1036,50 @@ lo_status configure_kernels() {
     return LO_OK;
 }
 
+// S1 of one spin block: A = Psi^T Phi (Psi = the first O columns of a [N][ldpsi] orbital matrix), A^-1 with per-walker
+// status, Theta^T panels written to `thT` (panel stride ldw_t) starting at panel o_base.
+void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, const void* phi, double* dA, int* status, double* thT,
+               int o_base, int ldw_t, cudaStream_t stream) {
+    const int N = f->N, N_pad = f->N_pad;
+    {
+        Timer tm(f, stream, LO_K_OVERLAP);
+        const int NF = (2 * O + 7) / 8, nfw = (std::min(NF, OV_NFB) + 7) / 8;
+        const int MF = (O + 7) / 8, n_mb = (MF + 4) / 5, mfb = (MF + n_mb - 1) / n_mb;     // row blocks of <= 5 fragments
+        dim3 grid(n_mb, n_w, (NF + OV_NFB - 1) / OV_NFB);
+        const size_t smem = (size_t)OV_PC * (OV_LDA + ov_ldb(O)) * 8;
+        ov_fn(mfb, nfw)<<<grid, 256, smem, stream>>>(psi, (const double2*)phi, (double2*)dA, N, O, ldpsi);
+    }
+    {
+        Timer tm(f, stream, LO_K_INVERSE);
+        size_t aux = (size_t)(2 * O + 1) * 16 + (size_t)((O + 3) & ~3) * 4 + 16;
+        size_t need = aux + (size_t)O * O * 16;
+        if (need <= 200 * 1024)
+            k_inverse<true><<<n_w, 256, need, stream>>>((double2*)dA, status, O);
+        else
+            k_inverse<false><<<n_w, 256, aux, stream>>>((double2*)dA, status, O);
+    }
+    {
+        Timer tm(f, stream, LO_K_THETA);
+        const int MF = (2 * O + 7) / 8, n_mb = (MF + 15) / 16, mfb = (MF + n_mb - 1) / n_mb;
+        dim3 grid((N_pad + 63) / 64, n_mb, n_w);
+        th_fn(mfb)<<<grid, 256, (size_t)(mfb * 8 + 64) * TH_LD * 8, stream>>>((const double2*)phi, (const double2*)dA, thT, N, N_pad, O, o_base, ldw_t);
+    }
+}
+
+lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
+
 lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
                               int* walker_status, void* Eout4, cudaStream_t stream) {
-    const int N = f->N, N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
     const void* phis[2] = {phi_a, phi_b};
-    // ---- S1
-    for (int s = 0; s < f->n_spin; ++s) {
-        const int O = f->n_occ[s];
-        const int Op = (O + 3) & ~3;
-        {
-            Timer tm(f, stream, LO_K_OVERLAP);
-            const int NF = (2 * O + 7) / 8, nfw = (std::min(NF, OV_NFB) + 7) / 8;
-            const int MF = (O + 7) / 8, n_mb = (MF + 4) / 5, mfb = (MF + n_mb - 1) / n_mb;     // row blocks of <= 5 fragments
-            dim3 grid(n_mb, n_w, (NF + OV_NFB - 1) / OV_NFB);
-            const size_t smem = (size_t)OV_PC * (OV_LDA + ov_ldb(O)) * 8;
-            ov_fn(mfb, nfw)<<<grid, 256, smem, stream>>>(f->ops->dPsi[s], (const double2*)phis[s], (double2*)f->dA[s], N, O);
-        }
-        {
-            Timer tm(f, stream, LO_K_INVERSE);
-            size_t aux = (size_t)(2 * O + 1) * 16 + (size_t)((O + 3) & ~3) * 4 + 16;
-            size_t need = aux + (size_t)O * O * 16;
-            if (need <= 200 * 1024)
-                k_inverse<true><<<n_w, 256, need, stream>>>((double2*)f->dA[s], f->dStatus + (size_t)s * Wcap, O);
-            else
-                k_inverse<false><<<n_w, 256, aux, stream>>>((double2*)f->dA[s], f->dStatus + (size_t)s * Wcap, O);
-        }
-        {
-            Timer tm(f, stream, LO_K_THETA);
-            const int MF = (2 * O + 7) / 8, n_mb = (MF + 15) / 16, mfb = (MF + n_mb - 1) / n_mb;
-            dim3 grid((N_pad + 63) / 64, n_mb, n_w);
-            const double2* ph = (const double2*)phis[s];
-            const double2* Ai = (const double2*)f->dA[s];
-            th_fn(mfb)<<<grid, 256, (size_t)(mfb * 8 + 64) * TH_LD * 8, stream>>>(ph, Ai, f->dThT, N, N_pad, O, f->o_base[s], ldw);
-        }
-    }
+    for (int s = 0; s < f->n_spin; ++s)
+        launch_s1(f, n_w, f->ops->dPsi[s], f->n_occ[s], f->n_occ[s], phis[s], f->dA[s], f->dStatus + (size_t)s * f->Wcap, f->dThT, f->o_base[s],
+                  f->ldw, stream);
+    return launch_s3_s5(f, n_w, E_L, E1, E_J, E_K, walker_status, Eout4, stream);
+}
+
+// S2-S5 on the Theta^T panels of n_w (possibly virtual, see lo_local_energy_cas) walkers.
+lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream) {
+    const int N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
     const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
     // ---- S2 + S3
     const int RB = f->Xp / CO_BM;
@@ -959,6 +1140,28 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_propagator: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    return LO_OK;
+}
+
+// local energy with a multi-determinant trial by direct summation over determinants (Eq. 12), the
+// determinants' overlaps and Green's functions by SMW updates of the reference (Eq. 20); each (walker, determinant) is a
+// virtual walker of the ordinary Coulomb / exchange kernels (orbital-indexed Theta^d panels, zero where unoccupied).
+lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
+                                  int* walker_status, cudaStream_t stream) {
+    CasPlan& c = *f->cas;
+    const int n_orb = f->n_occ[0], n_v = n_w * c.n_det, ldw0 = 2 * c.W0cap;
+    launch_s1(f, n_w, f->ops->dPsi[0], n_orb, c.n_ref, phi, c.dA0, c.dSt0, c.dTh0, 0, ldw0, stream);
+    k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[0], n_orb, c.dTh0, (double2*)c.dT, f->N, f->N_pad, c.n_ref, c.n_virt, ldw0);
+    k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dT, c.dHoles, c.dParts, c.dCoef, c.dSt0, (double2*)c.dG, (double2*)c.dWd,
+                                                  f->dStatus, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb);
+    dim3 g3(n_v, n_orb, (f->N_pad + 127) / 128);
+    k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw);
+    lo_status st = launch_s3_s5(f, n_v, nullptr, nullptr, nullptr, nullptr, nullptr, c.dEv, stream);
+    if (st != LO_OK) return st;
+    k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, f->dStatus, c.dSt0, n_w, c.n_det,
+                                                         (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K, (double2*)ovlp, walker_status);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_error(std::string("lo_local_energy_cas: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
 }
 

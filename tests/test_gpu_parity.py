@@ -435,3 +435,54 @@ def test_compressed_coulomb_rejects_unrestricted():
     F = lo.Factors.setup(P.h, P.L, P.psi, 1e-8, device=0, max_walkers=2, gpu_svd=True)
     with pytest.raises(lo.LoError):
         F.set_coulomb_mode(True)
+
+
+# ------------------------------------------------------------------------------------------ NEXT-2: multi-determinant trial
+def _cas_case(P, n_virt, n_act_occ, n_det, max_exc, n_w, T_svd):
+    torch = torch_cuda()
+    T = gen.make_cas_trial(P, n_virt=n_virt, n_act_occ=n_act_occ, n_det=n_det, max_exc=max_exc)
+    F = lo.Factors.setup(P.h, P.L, [T.C], T_svd, device=0, max_walkers=n_w * n_det, gpu_svd=True)
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w)
+    phi = gen.make_walkers(P, n_w)[0]
+    E, st = F.local_energy_cas(torch.from_numpy(phi).cuda())
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, T.C)
+    n_orb = T.C.shape[1]
+    U, sg, W = F.factor_all(0)
+    pi, pj = oracle.all_pairs(n_orb)
+    fs = oracle.make_factor_set(P.N, n_orb, pi, pj, F.ranks(0), U, sg, W)
+    cols = [T.columns(d) for d in range(T.n_det)]
+    return T, F, phi, E, st, Lbar, hbar, fs, cols
+
+
+def test_cas_trial_matches_oracle(c1):
+    """lo_local_energy_cas (SMW overlaps / Green's functions, virtual walkers) against the oracle's definition
+    (Eq. 12/13: every determinant's own LU, Theta^d and energy) on the library's factor set: all five outputs of every
+    walker, 1e-10 relative; 10 determinants (singles and doubles out of the last 3 occupied into 4 virtuals), 7 walkers."""
+    T, F, phi, E, st, Lbar, hbar, fs, cols = _cas_case(c1, 4, 3, 10, 2, 7, 1e-4)
+    assert (st == 0).all()
+    for w in range(phi.shape[0]):
+        Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w]))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+    # one determinant = the single-determinant path on the reference columns
+    F.set_cas_trial(T.n_ref, T.holes[:1], T.parts[:1], T.coef[:1], 7)
+    torch = torch_cuda()
+    E1d, _ = F.local_energy_cas(torch.from_numpy(phi).cuda())
+    F0 = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=7, gpu_svd=True)
+    Es, _ = gpu_energy(F0, [phi])
+    assert np.abs(E1d.cpu().numpy().T[:, :4] - Es).max() <= 1e-9 * np.abs(Es[:, 0]).max()
+
+
+def test_cas_trial_triples_and_argument_errors(c0):
+    T, F, phi, E, st, Lbar, hbar, fs, cols = _cas_case(c0, 3, 3, 12, 3, 5, 1e-8)
+    for w in range(phi.shape[0]):
+        Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w]))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0])
+    with pytest.raises(lo.LoError):
+        F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, 6)            # 6 * 12 virtual walkers > max_walkers
+    bad = T.parts.copy()
+    bad[1, 0] = 2                                                        # particle inside the reference
+    with pytest.raises(lo.LoError):
+        F.set_cas_trial(T.n_ref, T.holes, bad, T.coef, 5)
