@@ -262,6 +262,30 @@ def run_ours(args):
                                      "energies_per_s": round(n_w * args.steps / (c0.elapsed_time(c1) * 1e-3), 2),
                                      "exchange_ms": round(c_ms, 4), "exchange_tflops": round(c_tf, 3), "exchange_frac_of_peak": round(c_tf / peak, 4)}
 
+    # ---- SURVEY 8(f) NEXT-2 (opt-in, outside `value`): multi-determinant trial by direct summation, own factor set
+    if args.cas > 0 and info.n_spin == 1:
+        n_virt, n_real = 6, max(1, n_w // args.cas)
+        Tr = gen.make_cas_trial(P, n_virt=n_virt, n_act_occ=6, n_det=args.cas, max_exc=4)
+        Fc = lo.Factors.setup(P.h, P.L, [Tr.C], T, device=local, max_walkers=n_real * args.cas, gpu_svd=True)
+        Fc.set_cas_trial(Tr.n_ref, Tr.holes, Tr.parts, Tr.coef, n_real)
+        phic = dphi[0][:n_real].contiguous()
+        for _ in range(3):
+            Fc.local_energy_cas(phic)
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for _ in range(args.steps):
+            Fc.local_energy_cas(phic)
+        c1.record()
+        torch.cuda.synchronize()
+        cas_ms = c0.elapsed_time(c1) / args.steps
+        nxt = dict(nxt or {})
+        nxt["cas_trial"] = {"what": "lo_local_energy_cas: %d determinants (<= 4 excitations, 6 active occupied x %d virtuals), %d real walkers = %d "
+                                    "virtual walkers, direct summation with SMW Green's functions" % (args.cas, n_virt, n_real, n_real * args.cas),
+                            "ms_per_step": round(cas_ms, 4), "energies_per_s": round(n_real / (cas_ms * 1e-3), 2),
+                            "determinant_energies_per_s": round(n_real * args.cas / (cas_ms * 1e-3), 2)}
+        Fc.free()
+
     cpu_baseline = None
     if rank == 0 and world == 1 and args.cpu_walkers > 0:
         import oracle
@@ -458,6 +482,8 @@ def main():
     ap.add_argument("--ref-pairs", type=int, default=128)
     ap.add_argument("--no-propagator", dest="propagator", action="store_false",
                     help="skip the NEXT-1 propagator-formation measurement (reported under \"next\", never part of `value`)")
+    ap.add_argument("--cas", type=int, default=0, help="also time the NEXT-2 multi-determinant path with this many determinants "
+                    "(N_w / cas real walkers; reported under \"next\", never part of `value`)")
     ap.add_argument("--sweep", action="store_true", help="threshold sweep (BASELINE.json:configs[4]): one JSON line per threshold")
     ap.add_argument("--sweep-exact-walkers", type=int, default=4, help="walkers whose exact E_K the oracle computes in --sweep")
     args = ap.parse_args()
