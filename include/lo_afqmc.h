@@ -139,10 +139,18 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
  * lo_local_energy_cas: phi device complex128 [n_w][N][n_ref]; E_L (required), E1, E_J, E_K, ovlp device complex128
  * [n_w] (ovlp = sum_d w_d / <reference|Phi>, the trial overlap in units of the reference overlap); walker_status as in
  * lo_local_energy.  A determinant with a singular overlap contributes nothing.  Asynchronous; allocates nothing.
- * The rearranged SMW energy of Eq. 23 (cost independent of N_det in the leading term) is not built: cost here is n_det x
- * the single-determinant evaluation. */
+ * mode LO_CAS_DIRECT: cost = n_det x the single-determinant evaluation; needs max_walkers >= max_real_walkers * n_det.
+ * mode LO_CAS_SMW_ENERGY: the rearranged sums of Eq. 21-23: every Theta^d column is the reference
+ *   column plus a combination of the active (hole) columns of Theta0 = Phi A^-1, so for each pair (x<=y) the projections
+ *   of U^{xy}, W^{xy} onto the panel set {x, y} u active ("Q_L^int") are formed ONCE per walker, contracted
+ *   over the singular index into S^{xy}[c][c'] = sum_K sigma_K (U_K.Theta0_c)(W_K.Theta0_c'), and each determinant's
+ *   exchange AND Coulomb pair energies (Eq. 22: both terms from the compressed factors, as LO_COULOMB_COMPRESSED) are
+ *   small bilinear forms in S; E1 likewise from hbar.Theta0 intermediates.  Leading cost (2 + n_active)/2 x the
+ *   4-projection single-determinant evaluation, independent of n_det; at most 6 distinct hole columns. */
+#define LO_CAS_DIRECT 0
+#define LO_CAS_SMW_ENERGY 1
 lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts,
-                           const double* coef, int max_real_walkers);
+                           const double* coef, int max_real_walkers, int mode);
 lo_status lo_local_energy_cas(const lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K,
                               void* ovlp, int* walker_status, void* stream);
 

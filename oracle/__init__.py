@@ -350,7 +350,7 @@ def sub_factor_set(fs: FactorSet, cols) -> FactorSet:
     return make_factor_set(fs.N, len(cols), pos[fs.pi[keep]], pos[fs.pj[keep]], fs.r[keep], fs.U[rows], fs.sigma[rows], fs.W[rows])
 
 
-def local_energy_cas(Cmo, columns, coef, Lbar, hbar, fs, phi, exact=False):
+def local_energy_cas(Cmo, columns, coef, Lbar, hbar, fs, phi, exact=False, compressed_coulomb=False):
     """Local energy of ONE closed-shell walker phi [N,O] with the multi-determinant trial sum_d c_d |d>, every |d> a
     closed-shell determinant occupying the orbitals columns[d] (columns of Cmo, in the reference's column positions),
     straight from the definition (Eq. 12 with Eq. 13, applied to every energy term):
@@ -358,7 +358,8 @@ def local_energy_cas(Cmo, columns, coef, Lbar, hbar, fs, phi, exact=False):
     E^d = the single-determinant local energy with trial Psi_d = Cmo[:, columns[d]] (Theta^d by its own LU, Eq. 15).
     Lbar [X,n_orb,N], hbar [n_orb,N]: half-rotated integrals for ALL orbitals of Cmo; fs: factor set over all their
     pairs (exchange by O5 on the sub-set of pairs the determinant occupies); exact=True uses the Cholesky route (O2)
-    for the exchange instead.  Returns (E_L, E1, E_J, E_K, sum_d w_d / det(Psi_0^T phi)^2)."""
+    for the exchange instead; compressed_coulomb=True takes E_J from the factors too (Eq. 19/22 first term, the paper's
+    own multi-determinant expression Eq. 22).  Returns (E_L, E1, E_J, E_K, sum_d w_d / det(Psi_0^T phi)^2)."""
     Cmo, phi = _f64(Cmo), _c128(phi)
     num = np.zeros(3, dtype=np.complex128)
     den = 0.0 + 0.0j
@@ -375,6 +376,8 @@ def local_energy_cas(Cmo, columns, coef, Lbar, hbar, fs, phi, exact=False):
         ths = np.ascontiguousarray(th[:, order])
         e1, ej = onebody_coulomb([np.ascontiguousarray(Lbar[:, sc, :])], [np.ascontiguousarray(hbar[sc])], [ths])
         ek = exchange_cholesky(np.ascontiguousarray(Lbar[:, sc, :]), ths) if exact else exchange_lo(sub_factor_set(fs, sc), ths)
+        if compressed_coulomb:
+            ej = 2.0 * coulomb_lo(sub_factor_set(fs, sc), ths)
         w = coef[d] * det * det
         num += w * np.array([e1, ej, ek])
         den += w

@@ -57,7 +57,7 @@ def lib():
         L.lo_coulomb_x.argtypes = [vp, C.POINTER(vp), C.POINTER(ci)]
         L.lo_theta_host.argtypes = [vp, ci, ci, vp]
         L.lo_set_coulomb_mode.argtypes = [vp, ci]
-        L.lo_set_cas_trial.argtypes = [vp, ci, ci, ci, vp, vp, vp, ci]
+        L.lo_set_cas_trial.argtypes = [vp, ci, ci, ci, vp, vp, vp, ci, ci]
         L.lo_local_energy_cas.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp]
         L.lo_propagator.argtypes = [vp, ci, vp, vp]
         L.lo_propagator_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(ci), C.POINTER(C.c_longlong)]
@@ -218,12 +218,13 @@ class Factors:
         _check(lib().lo_coulomb_x(self._h, C.byref(p), C.byref(ld)))
         return p.value, ld.value
 
-    def set_cas_trial(self, n_ref, holes, parts, coef, max_real_walkers):
-        """lo_set_cas_trial: holes/parts int32 [n_det, max_exc] (-1 padded), coef [n_det]."""
+    def set_cas_trial(self, n_ref, holes, parts, coef, max_real_walkers, smw_energy=False):
+        """lo_set_cas_trial: holes/parts int32 [n_det, max_exc] (-1 padded), coef [n_det]; smw_energy selects the
+        rearranged sums of Eq. 21-23 (LO_CAS_SMW_ENERGY) instead of direct summation over determinants."""
         holes, parts, coef = _np(holes, np.int32), _np(parts, np.int32), _np(coef, np.float64)
         n_det, max_exc = holes.shape
         _check(lib().lo_set_cas_trial(self._h, int(n_ref), n_det, max_exc, holes.ctypes.data, parts.ctypes.data, coef.ctypes.data,
-                                      int(max_real_walkers)))
+                                      int(max_real_walkers), 1 if smw_energy else 0))
 
     def local_energy_cas(self, phi, stream=None):
         """lo_local_energy_cas on a torch CUDA complex128 tensor [n_w, N, n_ref]; returns (E [5, n_w] = E_L, E1, E_J,

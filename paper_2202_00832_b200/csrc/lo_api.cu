@@ -398,7 +398,7 @@ void free_all(lo_factors* f) {
         f->bW.release();
         if (f->cas) {
             void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd,
-                          f->cas->dEv, f->cas->dSt0};
+                          f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS, f->cas->dH, f->cas->dPart, f->cas->dStV};
             for (void* q : cp)
                 if (q) cudaFree(q);
             delete f->cas;
@@ -785,14 +785,16 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode) {
 }
 
 lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts, const double* coef,
-                           int max_real_walkers) {
+                           int max_real_walkers, int mode) {
     if (!f || !holes || !parts || !coef) { set_error("lo_set_cas_trial: NULL argument"); return LO_EINVAL; }
     if (f->device < 0) { set_error("lo_set_cas_trial: no device"); return LO_ECUDA; }
     if (f->n_spin != 1) { set_error("lo_set_cas_trial: closed-shell factor sets only (n_spin == 1)"); return LO_EINVAL; }
     const int n_orb = f->n_occ[0];
+    if (mode != LO_CAS_DIRECT && mode != LO_CAS_SMW_ENERGY) { set_error("lo_set_cas_trial: mode must be LO_CAS_DIRECT or LO_CAS_SMW_ENERGY"); return LO_EINVAL; }
     if (n_ref <= 0 || n_ref > n_orb || n_det <= 0 || max_exc <= 0 || max_exc > CAS_MAX_EXC || max_real_walkers <= 0 ||
-        (long long)max_real_walkers * n_det > f->max_walkers) {
-        set_error("lo_set_cas_trial: invalid sizes (need 0 < n_ref <= n_occ, 1 <= max_exc <= 8, max_real_walkers * n_det <= max_walkers)");
+        (mode == LO_CAS_DIRECT && (long long)max_real_walkers * n_det > f->max_walkers) || max_real_walkers > f->max_walkers) {
+        set_error("lo_set_cas_trial: invalid sizes (need 0 < n_ref <= n_occ, 1 <= max_exc <= 8, max_real_walkers * n_det <= max_walkers "
+                  "in LO_CAS_DIRECT mode, max_real_walkers <= max_walkers)");
         return LO_EINVAL;
     }
     for (int d = 0; d < n_det; ++d) {
@@ -805,9 +807,19 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
                 if (holes[(size_t)d * max_exc + l] == h || parts[(size_t)d * max_exc + l] == p) { set_error("lo_set_cas_trial: repeated hole or particle in one determinant"); return LO_EINVAL; }
         }
     }
+    // active set = the reference columns that are a hole in some determinant (the columns of A^-1 the SMW corrections touch)
+    std::vector<int> act;
+    for (size_t k = 0; k < (size_t)n_det * max_exc; ++k)
+        if (holes[k] >= 0 && std::find(act.begin(), act.end(), holes[k]) == act.end()) act.push_back(holes[k]);
+    std::sort(act.begin(), act.end());
+    if (mode == LO_CAS_SMW_ENERGY && act.size() > 6) {
+        set_error("lo_set_cas_trial: LO_CAS_SMW_ENERGY supports at most 6 distinct hole columns (active occupied orbitals); use LO_CAS_DIRECT");
+        return LO_EINVAL;
+    }
     CK(cudaSetDevice(f->device));
     if (f->cas) {
-        void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd, f->cas->dEv, f->cas->dSt0};
+        void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd, f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS,
+                      f->cas->dH, f->cas->dPart, f->cas->dStV};
         for (void* q : cp)
             if (q) cudaFree(q);
         delete f->cas;
@@ -827,7 +839,7 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     CK(al((void**)&c->dHoles, ne * 4));
     CK(al((void**)&c->dParts, ne * 4));
     CK(al((void**)&c->dCoef, (size_t)n_det * 8));
-    CK(al((void**)&c->dTh0, (size_t)n_ref * 2 * c->W0cap * f->N_pad * 8));
+    CK(al((void**)&c->dTh0, (size_t)n_orb * 2 * c->W0cap * f->N_pad * 8));      // virtual panels stay zero
     CK(al((void**)&c->dA0, (size_t)c->W0cap * n_ref * n_ref * 16));
     CK(al((void**)&c->dT, (size_t)c->W0cap * std::max(c->n_virt, 1) * n_ref * 16));
     CK(al((void**)&c->dG, nv * max_exc * n_orb * 16));
@@ -837,6 +849,37 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     CK(cudaMemcpy(c->dHoles, holes, ne * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->dParts, parts, ne * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->dCoef, coef, (size_t)n_det * 8, cudaMemcpyHostToDevice));
+    c->mode = mode;
+    c->n_act = (int)act.size();
+    if (mode == LO_CAS_SMW_ENERGY) {
+        const int na_pad = c->n_act <= 2 ? 2 : (c->n_act <= 4 ? 4 : 6);
+        c->NP = 2 + na_pad;
+        std::vector<int> hidx(ne + 8, -1);
+        for (size_t k = 0; k < ne; ++k)
+            if (holes[k] >= 0) hidx[k] = (int)(std::find(act.begin(), act.end(), holes[k]) - act.begin());
+        for (int a = 0; a < 8; ++a) hidx[ne + a] = a < c->n_act ? act[a] : 0;          // A_set (padded with column 0) behind the indices
+        std::vector<signed char> kind((size_t)n_det * n_orb);
+        for (int d = 0; d < n_det; ++d)
+            for (int x = 0; x < n_orb; ++x) {
+                signed char kd = x < n_ref ? 0 : -1;
+                for (int k = 0; k < max_exc; ++k) {
+                    if (holes[(size_t)d * max_exc + k] == x) kd = -1;
+                    if (parts[(size_t)d * max_exc + k] == x) kd = (signed char)(1 + k);
+                }
+                kind[(size_t)d * n_orb + x] = kd;
+            }
+        c->n_chunks = (int)((f->n_tiles + 15) / 16);
+        CK(al((void**)&c->dHoleIdx, hidx.size() * 4));
+        CK(al((void**)&c->dKind, kind.size()));
+        CK(al((void**)&c->dStV, nv * 4));
+        CK(al((void**)&c->dS, (size_t)std::max<long long>(f->n_tiles, 1) * max_real_walkers * c->NP * c->NP * 16));
+        CK(al((void**)&c->dH, (size_t)c->W0cap * n_orb * 9 * 16));
+        CK(al((void**)&c->dPart, (size_t)std::max(c->n_chunks, 1) * nv * 2 * 16));
+        CK(cudaMemcpy(c->dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(c->dKind, kind.data(), kind.size(), cudaMemcpyHostToDevice));
+        lo_status st = make_tmap(&c->tmTh0, c->dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 8);
+        if (st != LO_OK) return st;
+    }
     return LO_OK;
 }
 

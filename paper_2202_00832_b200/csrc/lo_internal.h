@@ -84,6 +84,18 @@ struct CasPlan {
     double* dWd = nullptr;                      // weights c_d det(T_d)^2: [max_real*n_det] complex
     double* dEv = nullptr;                      // per virtual walker {E_L,E1,E_J,E_K}: [max_real*n_det][4] complex
     int* dSt0 = nullptr;                        // [W0cap] status of the reference overlap
+    int* dStV = nullptr;                        // [max_real*n_det] status per (walker, determinant), SMW-energy mode
+    // ---- rearranged SMW energy (Eq. 23), mode 1
+    int mode = 0;                               // 0: direct summation over virtual walkers, 1: SMW energy
+    int n_act = 0, NP = 0;                      // active (hole) columns A_set, panel-set size NP = 2 + padded n_act (4, 6 or 8)
+    int hAct[8] = {0, 0, 0, 0, 0, 0, 0, 0};     // A_set (orbital = reference column), padded with 0
+    int* dHoleIdx = nullptr;                    // [n_det][max_exc]: index of hole k in A_set
+    signed char* dKind = nullptr;               // [n_det][n_orb]: -1 unoccupied, 0 reference non-hole, 1+m particle m
+    double* dS = nullptr;                       // S[tile][w][NP][NP] complex (Eq. 23 intermediates contracted over K)
+    double* dH = nullptr;                       // one-body intermediates [W0cap][n_orb][1 + 8] complex (self, A_set)
+    double* dPart = nullptr;                    // [n_chunks][max_real*n_det][2] complex partial (E_K, E_J) sums
+    int n_chunks = 0;
+    CUtensorMap tmTh0;                          // Theta0^T panels [n_orb*2*W0cap][N_pad], box 16 x 16
 };
 
 struct TimingEvent {

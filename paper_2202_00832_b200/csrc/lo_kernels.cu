@@ -768,6 +768,280 @@ __global__ void __launch_bounds__(256) k_cas_T(const double* __restrict__ C, int
     }
 }
 
+// ---- NEXT-2, rearranged SMW energy (Eq. 21-23).  Every Theta^d column is a combination of the
+// reference column and the active (hole) columns of Theta0, so for pair (x <= y) the projections of U^{xy}, W^{xy} onto the
+// panel set P = [x, y, A_1..A_na] of Theta0 ("Q_L^int = U Phi A_act^-1") serve ALL determinants.  They are
+// contracted over the singular index K at once,
+//     S_t[c][c'] = sum_{K in tile t} wgt_K (U_K . Theta0_c)(W_K . Theta0_c'),     c, c' in P,
+// and a determinant's pair energies are small bilinear forms in S (k_cas_energy).  Work item = (row tile, block of 8
+// walkers); consumer warp m owns row fragment m and all NP panels x 16 real columns; same TMA/mbarrier pipeline.
+constexpr int CP_STAGES = 4;
+template <int NP>
+struct CpCfg {
+    static constexpr int STAGE_BYTES = 2 * EX_BM * 128 + NP * 16 * 128;
+    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * NP * NP * 16;
+};
+
+template <int NP>
+__global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
+                                                      const __grid_constant__ CUtensorMap tmT0, const double* __restrict__ wgt,
+                                                      const ExTile* __restrict__ tiles, long long n_items, int WB, int N_pad, int ldw0,
+                                                      const int* __restrict__ act /* [NP-2] */, double2* __restrict__ S, int n_w) {
+    constexpr int STAGE = CpCfg<NP>::STAGE_BYTES;
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
+    const uint32_t full = sbase + CP_STAGES * STAGE, empty = full + 8 * CP_STAGES;
+    ExTile* ring = reinterpret_cast<ExTile*>(sgen + CP_STAGES * STAGE + 128);
+    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 walkers][NP*NP]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int KT = N_pad / KTILE;
+    if (tid == 0) {
+        prefetch_tmap(&tmU8);
+        prefetch_tmap(&tmW8);
+        prefetch_tmap(&tmT0);
+        for (int i = 0; i < CP_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
+        fence_barrier_init();
+    }
+    __syncthreads();
+    if (warp < 4) {
+        reg_dec_producer();
+        if (warp == 0 && lane == 0) {
+            int pan[NP];
+#pragma unroll
+            for (int c = 2; c < NP; ++c) pan[c] = act[c - 2];
+            int slot = 0, n = 0;
+            uint32_t phase = 0;
+            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
+                const ExTile tile = tiles[q / WB];
+                const int wb = (int)(q % WB);
+                pan[0] = tile.pi;
+                pan[1] = tile.pj;
+                const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + NP * 16) * 128;
+                for (int kt = 0; kt < KT; ++kt) {
+                    mbar_wait(empty + 8 * slot, phase ^ 1);
+                    if (kt == 0) ring[n % EX_RING] = tile;
+                    const uint32_t st = sbase + slot * STAGE, bar = full + 8 * slot;
+                    const int k0 = kt * KTILE;
+                    mbar_expect_tx(bar, tx);
+                    for (int fr = 0; fr < tile.nfrag; ++fr) {
+                        tma_load_2d(st + fr * 1024, &tmU8, k0, tile.row0 + fr * 8, bar);
+                        tma_load_2d(st + EX_BM * 128 + fr * 1024, &tmW8, k0, tile.row0 + fr * 8, bar);
+                    }
+#pragma unroll
+                    for (int c = 0; c < NP; ++c) {      // 16 real rows of panel c = 2 boxes of 8 rows
+                        tma_load_2d(st + 2 * EX_BM * 128 + c * 2048, &tmT0, k0, pan[c] * ldw0 + wb * 16, bar);
+                        tma_load_2d(st + 2 * EX_BM * 128 + c * 2048 + 1024, &tmT0, k0, pan[c] * ldw0 + wb * 16 + 8, bar);
+                    }
+                    if (++slot == CP_STAGES) { slot = 0; phase ^= 1; }
+                }
+            }
+        }
+        return;
+    }
+    reg_inc_consumer();
+    const int cw = warp - 4, g = lane >> 2, t = lane & 3, ctid = tid - 128;
+    double accU[NP][2][2], accW[NP][2][2];
+#pragma unroll
+    for (int c = 0; c < NP; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) accU[c][b][0] = accU[c][b][1] = accW[c][b][0] = accW[c][b][1] = 0.0;
+    uint32_t xo[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
+    const uint32_t u_row = (uint32_t)(cw * 8 + g) * 128, p_row = (uint32_t)(2 * EX_BM * 128) + (uint32_t)g * 128;
+    int cslot = 0, n = 0;
+    uint32_t cphase = 0;
+    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
+        const int wb = (int)(q % WB);
+        const long long tix = q / WB;
+        mbar_wait(full + 8 * cslot, cphase);
+        const ExTile tile = ring[n % EX_RING];
+        const bool active = cw < tile.nfrag;            // warp-uniform
+        for (int kt = 0; kt < KT; ++kt) {
+            if (kt) mbar_wait(full + 8 * cslot, cphase);
+            const uint32_t st = sbase + cslot * STAGE;
+            if (active) {
+#pragma unroll
+                for (int ks = 0; ks < KTILE / 4; ++ks) {
+                    const double a = lds_f64(st + u_row + xo[ks]), w = lds_f64(st + u_row + EX_BM * 128 + xo[ks]);
+#pragma unroll
+                    for (int c = 0; c < NP; ++c) {
+                        const double b0 = lds_f64(st + p_row + c * 2048 + xo[ks]), b1 = lds_f64(st + p_row + c * 2048 + 1024 + xo[ks]);
+                        if (ks == KTILE / 4 - 1 && c == NP - 1) release_stage(empty + 8 * cslot, lane);
+                        mma884(accU[c][0][0], accU[c][0][1], a, b0);
+                        mma884(accW[c][0][0], accW[c][0][1], w, b0);
+                        mma884(accU[c][1][0], accU[c][1][1], a, b1);
+                        mma884(accW[c][1][0], accW[c][1][1], w, b1);
+                    }
+                }
+            } else {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + 8 * cslot);
+            }
+            if (++cslot == CP_STAGES) { cslot = 0; cphase ^= 1; }
+        }
+        // epilogue: S[c][c'] of the 8 walkers of the block, rows of the tile summed in a fixed order (lane rows by
+        // shuffles, then the fragments one warp after the other through shared memory)
+        const double wv = active ? __ldg(wgt + tile.row0 + cw * 8 + g) : 0.0;
+        for (int i = ctid; i < 8 * NP * NP; i += 256) Sacc[i] = make_double2(0.0, 0.0);
+        bar_sync_consumers();
+        for (int turn = 0; turn < 8; ++turn) {
+            if (turn == cw && active) {
+#pragma unroll
+                for (int c = 0; c < NP; ++c) {
+#pragma unroll
+                    for (int nf = 0; nf < 2; ++nf) {
+                        const double ur = wv * accU[c][nf][0], ui = wv * accU[c][nf][1];
+#pragma unroll
+                        for (int c2 = 0; c2 < NP; ++c2) {
+                            double vr = ur * accW[c2][nf][0] - ui * accW[c2][nf][1];
+                            double vi = ur * accW[c2][nf][1] + ui * accW[c2][nf][0];
+                            vr += __shfl_xor_sync(0xffffffffu, vr, 4);
+                            vi += __shfl_xor_sync(0xffffffffu, vi, 4);
+                            vr += __shfl_xor_sync(0xffffffffu, vr, 8);
+                            vi += __shfl_xor_sync(0xffffffffu, vi, 8);
+                            vr += __shfl_xor_sync(0xffffffffu, vr, 16);
+                            vi += __shfl_xor_sync(0xffffffffu, vi, 16);
+                            if (g == 0) {
+                                double2* dst = Sacc + (nf * 4 + t) * NP * NP + c * NP + c2;
+                                double2 o = *dst;
+                                *dst = make_double2(o.x + vr, o.y + vi);
+                            }
+                        }
+                    }
+                }
+            }
+            bar_sync_consumers();
+        }
+#pragma unroll
+        for (int c = 0; c < NP; ++c)
+#pragma unroll
+            for (int b = 0; b < 2; ++b) accU[c][b][0] = accU[c][b][1] = accW[c][b][0] = accW[c][b][1] = 0.0;
+        for (int i = ctid; i < 8 * NP * NP; i += 256) {
+            const int wl = i / (NP * NP), wg = wb * 8 + wl;
+            if (wg < n_w) S[((size_t)tix * n_w + wg) * NP * NP + (i - wl * NP * NP)] = Sacc[i];
+        }
+        bar_sync_consumers();
+    }
+}
+
+// One-body intermediates of the SMW energy: H[w][x][0] = hbar_x . Theta0_x (reference x), H[w][x][1+a] = hbar_x . Theta0_{A_a}.
+// grid n_w, one warp per (x, slot), lanes over p.  hbar = row n_chol of the [Lbar; hbar] operand.
+__global__ void __launch_bounds__(256) k_cas_H(const double* __restrict__ hbar, const double* __restrict__ th0, const int* __restrict__ act,
+                                               int n_act, double2* __restrict__ H, int N, int N_pad, int n_ref, int n_orb, int ldw0) {
+    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int e = warp; e < n_orb * (1 + n_act); e += 8) {
+        const int x = e / (1 + n_act), sl = e - x * (1 + n_act);
+        const int c = sl == 0 ? x : act[sl - 1];
+        double sr = 0.0, si = 0.0;
+        if (c < n_ref) {
+            const double* hx = hbar + (size_t)x * N_pad;
+            const double* re = th0 + ((size_t)c * ldw0 + 2 * w) * N_pad;
+            const double* im = re + N_pad;
+            for (int p = lane; p < N; p += 32) {
+                sr = fma(hx[p], re[p], sr);
+                si = fma(hx[p], im[p], si);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
+        }
+        if (lane == 0) H[((size_t)w * n_orb + x) * 9 + sl] = make_double2(sr, si);
+    }
+}
+
+// Pair energies of every determinant from the S intermediates (Eq. 22 with Eq. 23 inserted): with
+// Theta^d_x = s_x Theta0_x + sum_k G_d[k][x] Theta0_{h_k}  (s_x = 1 for a reference non-hole, else 0),
+//   exchange  e = sum_{c in y-list} sum_{c' in x-list} coef_y[c] coef_x[c'] S[c][c'],
+//   Coulomb   j = sum_{c in x-list} sum_{c' in y-list} coef_x[c] coef_y[c'] S[c][c'],
+// lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of CE_CH tiles sits in shared memory, threads
+// run over determinants; partial (E_K, E_J) sums per chunk are added in chunk order by k_cas_e1sum.
+constexpr int CE_CH = 16;
+__global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const ExTile* __restrict__ tiles, long long n_tiles,
+                                                    const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
+                                                    const double2* __restrict__ G, double2* __restrict__ part, int n_w, int n_det, int max_exc,
+                                                    int n_orb, int NP, int n_vtot) {
+    extern __shared__ __align__(16) double2 Ss[];      // [CE_CH][NP*NP]
+    __shared__ int tx_s[CE_CH], ty_s[CE_CH];
+    const int chunk = blockIdx.x, w = blockIdx.y, tid = threadIdx.x;
+    const long long t0 = (long long)chunk * CE_CH;
+    const int nt = (int)min((long long)CE_CH, n_tiles - t0), NP2 = NP * NP;
+    for (int i = tid; i < nt * NP2; i += 128) {
+        const int tl = i / NP2;
+        Ss[i] = S[((size_t)(t0 + tl) * n_w + w) * NP2 + (i - tl * NP2)];
+    }
+    if (tid < nt) { tx_s[tid] = tiles[t0 + tid].pi; ty_s[tid] = tiles[t0 + tid].pj; }
+    __syncthreads();
+    for (int d = tid; d < n_det; d += 128) {
+        const size_t v = (size_t)w * n_det + d;
+        const signed char* kd = kind + (size_t)d * n_orb;
+        const int* hi = holeIdx + (size_t)d * max_exc;
+        int e = 0;
+        while (e < max_exc && hi[e] >= 0) ++e;
+        const double2* Gv = G + v * max_exc * n_orb;
+        double2 ek = make_double2(0.0, 0.0), ej = make_double2(0.0, 0.0);
+        for (int tl = 0; tl < nt; ++tl) {
+            const int x = tx_s[tl], y = ty_s[tl];
+            const int kx = kd[x], ky = kd[y];
+            if (kx < 0 || ky < 0) continue;
+            const double2* St = Ss + tl * NP2;
+            // coefficient lists: entry 0 = self (index 0 for the x role, 1 for the y role), entries 1..e = the holes
+            double2 cx[CAS_MAX_EXC + 1], cy[CAS_MAX_EXC + 1];
+            int ix[CAS_MAX_EXC + 1], iy[CAS_MAX_EXC + 1];
+            cx[0] = make_double2(kx == 0 ? 1.0 : 0.0, 0.0); ix[0] = 0;
+            cy[0] = make_double2(ky == 0 ? 1.0 : 0.0, 0.0); iy[0] = 1;
+            for (int k = 0; k < e; ++k) {
+                cx[1 + k] = Gv[(size_t)k * n_orb + x]; ix[1 + k] = 2 + hi[k];
+                cy[1 + k] = Gv[(size_t)k * n_orb + y]; iy[1 + k] = 2 + hi[k];
+            }
+            for (int a = 0; a <= e; ++a)
+                for (int b = 0; b <= e; ++b) {
+                    const double2 cc = cmul(cy[a], cx[b]);
+                    const double2 se = St[iy[a] * NP + ix[b]], sj = St[ix[b] * NP + iy[a]];
+                    const double2 t1 = cmul(cc, se), t2 = cmul(cc, sj);
+                    ek.x += t1.x; ek.y += t1.y;
+                    ej.x += t2.x; ej.y += t2.y;
+                }
+        }
+        part[((size_t)chunk * n_vtot + v) * 2] = ek;
+        part[((size_t)chunk * n_vtot + v) * 2 + 1] = make_double2(-2.0 * ej.x, -2.0 * ej.y);
+    }
+}
+
+// Per virtual walker: E_K^d, E_J^d = chunk partials in chunk order; E1^d = 2 [sum_{x ref non-hole} H[x][self] +
+// sum_k sum_x G_d[k][x] H[x][hole k]]; writes Ev[v] = {E_L, E1, E_J, E_K} for k_cas_combine.
+__global__ void __launch_bounds__(128) k_cas_e1sum(const double2* __restrict__ part, int n_chunks, const double2* __restrict__ H,
+                                                   const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
+                                                   const double2* __restrict__ G, double2* __restrict__ Ev, int n_v, int n_det, int max_exc,
+                                                   int n_orb, int n_vtot) {
+    const int v = blockIdx.x * 128 + threadIdx.x;
+    if (v >= n_v) return;
+    const int w = v / n_det, d = v - w * n_det;
+    double2 ek = make_double2(0.0, 0.0), ej = make_double2(0.0, 0.0), e1 = make_double2(0.0, 0.0);
+    for (int c = 0; c < n_chunks; ++c) {
+        const double2 a = part[((size_t)c * n_vtot + v) * 2], b = part[((size_t)c * n_vtot + v) * 2 + 1];
+        ek.x += a.x; ek.y += a.y;
+        ej.x += b.x; ej.y += b.y;
+    }
+    const signed char* kd = kind + (size_t)d * n_orb;
+    const int* hi = holeIdx + (size_t)d * max_exc;
+    const double2* Hw = H + (size_t)w * n_orb * 9;
+    const double2* Gv = G + (size_t)v * max_exc * n_orb;
+    for (int x = 0; x < n_orb; ++x) {
+        if (kd[x] < 0) continue;
+        if (kd[x] == 0) { e1.x += Hw[x * 9].x; e1.y += Hw[x * 9].y; }
+        for (int k = 0; k < max_exc && hi[k] >= 0; ++k) {
+            const double2 t1 = cmul(Gv[(size_t)k * n_orb + x], Hw[x * 9 + 1 + hi[k]]);
+            e1.x += t1.x; e1.y += t1.y;
+        }
+    }
+    e1.x *= 2.0; e1.y *= 2.0;
+    Ev[4 * (size_t)v] = make_double2(e1.x + ej.x + ek.x, e1.y + ej.y + ek.y);
+    Ev[4 * (size_t)v + 1] = e1;
+    Ev[4 * (size_t)v + 2] = ej;
+    Ev[4 * (size_t)v + 3] = ek;
+}
+
 // One warp per virtual walker v = w*n_det + d: lane 0 inverts T_d (<= 8 x 8, Gauss-Jordan with partial pivoting) and
 // takes its determinant; all lanes then fill G_d.  weight = c_d det(T_d)^2 (closed shell: the same string in both spins);
 // status 1 when the reference overlap or T_d is singular (that determinant is then left out of the sums).
@@ -1031,6 +1305,11 @@ lo_status configure_kernels() {
             if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributePreferredSharedMemoryCarveout, 100);
             if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_overlap): ") + cudaGetErrorString(e)); return LO_ECUDA; }
         }
+    e = cudaFuncSetAttribute(k_cas_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<4>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<6>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<8>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_energy, cudaFuncAttributeMaxDynamicSharedMemorySize, CE_CH * 64 * 16);
+    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_cas_*): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
@@ -1152,13 +1431,40 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void*
     const int n_orb = f->n_occ[0], n_v = n_w * c.n_det, ldw0 = 2 * c.W0cap;
     launch_s1(f, n_w, f->ops->dPsi[0], n_orb, c.n_ref, phi, c.dA0, c.dSt0, c.dTh0, 0, ldw0, stream);
     k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[0], n_orb, c.dTh0, (double2*)c.dT, f->N, f->N_pad, c.n_ref, c.n_virt, ldw0);
+    int* stv = c.mode == 0 ? f->dStatus : c.dStV;
     k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dT, c.dHoles, c.dParts, c.dCoef, c.dSt0, (double2*)c.dG, (double2*)c.dWd,
-                                                  f->dStatus, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb);
-    dim3 g3(n_v, n_orb, (f->N_pad + 127) / 128);
-    k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw);
-    lo_status st = launch_s3_s5(f, n_v, nullptr, nullptr, nullptr, nullptr, nullptr, c.dEv, stream);
-    if (st != LO_OK) return st;
-    k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, f->dStatus, c.dSt0, n_w, c.n_det,
+                                                  stv, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb);
+    if (c.mode == 0) {
+        dim3 g3(n_v, n_orb, (f->N_pad + 127) / 128);
+        k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw);
+        lo_status st = launch_s3_s5(f, n_v, nullptr, nullptr, nullptr, nullptr, nullptr, c.dEv, stream);
+        if (st != LO_OK) return st;
+    } else {
+        // rearranged SMW energy (Eq. 23): S intermediates once per (tile, walker), then small per-determinant forms
+        const int WB = (n_w + 7) / 8;
+        const long long items = f->n_tiles * WB;
+        const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
+        const int* actd = c.dHoleIdx + (size_t)c.n_det * c.max_exc;      // A_set stored behind the hole indices
+        if (c.NP == 4)
+            k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU8, f->tmW8, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
+        else if (c.NP == 6)
+            k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU8, f->tmW8, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
+        else
+            k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU8, f->tmW8, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
+        const double* hbar = f->ops->dLbar + (size_t)f->n_chol * f->O_tot * f->N_pad;
+        k_cas_H<<<n_w, 256, 0, stream>>>(hbar, c.dTh0, actd, c.n_act, (double2*)c.dH, f->N, f->N_pad, c.n_ref, n_orb, ldw0);
+        const int n_chunks = (int)((f->n_tiles + CE_CH - 1) / CE_CH);
+        const int n_vtot = c.max_real * c.n_det;
+        if (n_chunks > 0) {
+            dim3 g4(n_chunks, n_w);
+            k_cas_energy<<<g4, 128, (size_t)CE_CH * c.NP * c.NP * 16, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx,
+                                                                              (const double2*)c.dG, (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb,
+                                                                              c.NP, n_vtot);
+        }
+        k_cas_e1sum<<<(n_v + 127) / 128, 128, 0, stream>>>((const double2*)c.dPart, n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx,
+                                                           (const double2*)c.dG, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_orb, n_vtot);
+    }
+    k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, stv, c.dSt0, n_w, c.n_det,
                                                          (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K, (double2*)ovlp, walker_status);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_local_energy_cas: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }

@@ -486,3 +486,37 @@ def test_cas_trial_triples_and_argument_errors(c0):
     bad[1, 0] = 2                                                        # particle inside the reference
     with pytest.raises(lo.LoError):
         F.set_cas_trial(T.n_ref, T.holes, bad, T.coef, 5)
+
+
+@pytest.mark.parametrize("cfg,n_virt,n_act,n_det,max_exc,n_w,T_svd", [(1, 4, 3, 10, 2, 7, 1e-4), (0, 3, 3, 12, 3, 5, 1e-8),
+                                                                      (1, 5, 6, 40, 4, 19, 1e-3)])
+def test_cas_smw_energy_matches_oracle(cfg, n_virt, n_act, n_det, max_exc, n_w, T_svd):
+    """LO_CAS_SMW_ENERGY (the rearranged sums of Eq. 21-23: S intermediates once per pair and walker, per-determinant
+    bilinear forms) against the oracle's definition with both two-body terms from the factors (Eq. 22), every output of
+    every walker, 1e-10 relative; also against the direct-summation mode in compressed-Coulomb mode."""
+    torch = torch_cuda()
+    P = gen.make_problem(cfg)
+    T = gen.make_cas_trial(P, n_virt=n_virt, n_act_occ=n_act, n_det=n_det, max_exc=max_exc)
+    F = lo.Factors.setup(P.h, P.L, [T.C], T_svd, device=0, max_walkers=n_w * n_det, gpu_svd=True)
+    phi = gen.make_walkers(P, n_w)[0]
+    dphi = torch.from_numpy(phi).cuda()
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w, smw_energy=True)
+    E, st = F.local_energy_cas(dphi)
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    assert (st == 0).all()
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, T.C)
+    n_orb = T.C.shape[1]
+    U, sg, W = F.factor_all(0)
+    pi, pj = oracle.all_pairs(n_orb)
+    fs = oracle.make_factor_set(P.N, n_orb, pi, pj, F.ranks(0), U, sg, W)
+    cols = [T.columns(d) for d in range(T.n_det)]
+    for w in range(0, n_w, 3):
+        Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w], compressed_coulomb=True))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+    F.set_coulomb_mode(True)
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w, smw_energy=False)
+    Ed, _ = F.local_energy_cas(dphi)
+    Ed = Ed.cpu().numpy().T
+    assert (np.abs(E - Ed).max(axis=1) <= 1e-9 * np.abs(Ed[:, 0])).all()
