@@ -877,7 +877,7 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
         CK(al((void**)&c->dPart, (size_t)std::max(c->n_chunks, 1) * nv * 2 * 16));
         CK(cudaMemcpy(c->dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
         CK(cudaMemcpy(c->dKind, kind.data(), kind.size(), cudaMemcpyHostToDevice));
-        lo_status st = make_tmap(&c->tmTh0, c->dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 8);
+        lo_status st = make_tmap(&c->tmTh0, c->dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 16);
         if (st != LO_OK) return st;
     }
     return LO_OK;

@@ -779,11 +779,11 @@ constexpr int CP_STAGES = 4;
 template <int NP>
 struct CpCfg {
     static constexpr int STAGE_BYTES = 2 * EX_BM * 128 + NP * 16 * 128;
-    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * NP * NP * 16;
+    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * 8 * NP * NP * 16;
 };
 
 template <int NP>
-__global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
+__global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
                                                       const __grid_constant__ CUtensorMap tmT0, const double* __restrict__ wgt,
                                                       const ExTile* __restrict__ tiles, long long n_items, int WB, int N_pad, int ldw0,
                                                       const int* __restrict__ act /* [NP-2] */, double2* __restrict__ S, int n_w) {
@@ -793,12 +793,12 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
     const uint32_t full = sbase + CP_STAGES * STAGE, empty = full + 8 * CP_STAGES;
     ExTile* ring = reinterpret_cast<ExTile*>(sgen + CP_STAGES * STAGE + 128);
-    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 walkers][NP*NP]
+    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 row groups g][8 walkers][NP*NP]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     if (tid == 0) {
-        prefetch_tmap(&tmU8);
-        prefetch_tmap(&tmW8);
+        prefetch_tmap(&tmU);
+        prefetch_tmap(&tmW);
         prefetch_tmap(&tmT0);
         for (int i = 0; i < CP_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
@@ -817,22 +817,19 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
                 const int wb = (int)(q % WB);
                 pan[0] = tile.pi;
                 pan[1] = tile.pj;
-                const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + NP * 16) * 128;
+                // whole 64-row boxes of U and W whatever the tile's length (rows past the tile are never read): one TMA each
+                const uint32_t tx = (uint32_t)(2 * EX_BM + NP * 16) * 128;
                 for (int kt = 0; kt < KT; ++kt) {
                     mbar_wait(empty + 8 * slot, phase ^ 1);
                     if (kt == 0) ring[n % EX_RING] = tile;
                     const uint32_t st = sbase + slot * STAGE, bar = full + 8 * slot;
                     const int k0 = kt * KTILE;
                     mbar_expect_tx(bar, tx);
-                    for (int fr = 0; fr < tile.nfrag; ++fr) {
-                        tma_load_2d(st + fr * 1024, &tmU8, k0, tile.row0 + fr * 8, bar);
-                        tma_load_2d(st + EX_BM * 128 + fr * 1024, &tmW8, k0, tile.row0 + fr * 8, bar);
-                    }
+                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
+                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
 #pragma unroll
-                    for (int c = 0; c < NP; ++c) {      // 16 real rows of panel c = 2 boxes of 8 rows
+                    for (int c = 0; c < NP; ++c)        // 16 real rows (8 walkers) of panel c
                         tma_load_2d(st + 2 * EX_BM * 128 + c * 2048, &tmT0, k0, pan[c] * ldw0 + wb * 16, bar);
-                        tma_load_2d(st + 2 * EX_BM * 128 + c * 2048 + 1024, &tmT0, k0, pan[c] * ldw0 + wb * 16 + 8, bar);
-                    }
                     if (++slot == CP_STAGES) { slot = 0; phase ^= 1; }
                 }
             }
@@ -881,33 +878,26 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
             }
             if (++cslot == CP_STAGES) { cslot = 0; cphase ^= 1; }
         }
-        // epilogue: S[c][c'] of the 8 walkers of the block, rows of the tile summed in a fixed order (lane rows by
-        // shuffles, then the fragments one warp after the other through shared memory)
+        // epilogue: S[c][c'] of the 8 walkers of the block.  Each lane adds the products of its own row into the slice of
+        // its row group g (no cross-lane traffic); the fragments take turns in a fixed order; the 8 row groups are summed
+        // in order when the block is written out.
         const double wv = active ? __ldg(wgt + tile.row0 + cw * 8 + g) : 0.0;
-        for (int i = ctid; i < 8 * NP * NP; i += 256) Sacc[i] = make_double2(0.0, 0.0);
+        for (int i = ctid; i < 8 * 8 * NP * NP; i += 256) Sacc[i] = make_double2(0.0, 0.0);
         bar_sync_consumers();
         for (int turn = 0; turn < 8; ++turn) {
             if (turn == cw && active) {
 #pragma unroll
-                for (int c = 0; c < NP; ++c) {
+                for (int nf = 0; nf < 2; ++nf) {
+                    double2* dst = Sacc + ((g * 8) + nf * 4 + t) * NP * NP;
 #pragma unroll
-                    for (int nf = 0; nf < 2; ++nf) {
+                    for (int c = 0; c < NP; ++c) {
                         const double ur = wv * accU[c][nf][0], ui = wv * accU[c][nf][1];
 #pragma unroll
                         for (int c2 = 0; c2 < NP; ++c2) {
-                            double vr = ur * accW[c2][nf][0] - ui * accW[c2][nf][1];
-                            double vi = ur * accW[c2][nf][1] + ui * accW[c2][nf][0];
-                            vr += __shfl_xor_sync(0xffffffffu, vr, 4);
-                            vi += __shfl_xor_sync(0xffffffffu, vi, 4);
-                            vr += __shfl_xor_sync(0xffffffffu, vr, 8);
-                            vi += __shfl_xor_sync(0xffffffffu, vi, 8);
-                            vr += __shfl_xor_sync(0xffffffffu, vr, 16);
-                            vi += __shfl_xor_sync(0xffffffffu, vi, 16);
-                            if (g == 0) {
-                                double2* dst = Sacc + (nf * 4 + t) * NP * NP + c * NP + c2;
-                                double2 o = *dst;
-                                *dst = make_double2(o.x + vr, o.y + vi);
-                            }
+                            double2 o = dst[c * NP + c2];
+                            o.x += ur * accW[c2][nf][0] - ui * accW[c2][nf][1];
+                            o.y += ur * accW[c2][nf][1] + ui * accW[c2][nf][0];
+                            dst[c * NP + c2] = o;
                         }
                     }
                 }
@@ -920,7 +910,10 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
             for (int b = 0; b < 2; ++b) accU[c][b][0] = accU[c][b][1] = accW[c][b][0] = accW[c][b][1] = 0.0;
         for (int i = ctid; i < 8 * NP * NP; i += 256) {
             const int wl = i / (NP * NP), wg = wb * 8 + wl;
-            if (wg < n_w) S[((size_t)tix * n_w + wg) * NP * NP + (i - wl * NP * NP)] = Sacc[i];
+            double2 sum = Sacc[i];
+#pragma unroll
+            for (int gg = 1; gg < 8; ++gg) { const double2 v = Sacc[gg * 8 * NP * NP + i]; sum.x += v.x; sum.y += v.y; }
+            if (wg < n_w) S[((size_t)tix * n_w + wg) * NP * NP + (i - wl * NP * NP)] = sum;
         }
         bar_sync_consumers();
     }
@@ -1446,11 +1439,11 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void*
         const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
         const int* actd = c.dHoleIdx + (size_t)c.n_det * c.max_exc;      // A_set stored behind the hole indices
         if (c.NP == 4)
-            k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU8, f->tmW8, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
+            k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
         else if (c.NP == 6)
-            k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU8, f->tmW8, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
+            k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
         else
-            k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU8, f->tmW8, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
+            k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
         const double* hbar = f->ops->dLbar + (size_t)f->n_chol * f->O_tot * f->N_pad;
         k_cas_H<<<n_w, 256, 0, stream>>>(hbar, c.dTh0, actd, c.n_act, (double2*)c.dH, f->N, f->N_pad, c.n_ref, n_orb, ldw0);
         const int n_chunks = (int)((f->n_tiles + CE_CH - 1) / CE_CH);
