@@ -779,7 +779,9 @@ constexpr int CP_STAGES = 4;
 template <int NP>
 struct CpCfg {
     static constexpr int STAGE_BYTES = 2 * EX_BM * 128 + NP * 16 * 128;
-    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * 8 * NP * NP * 16;
+    static constexpr int SL = NP * NP + 1;      // slice stride (double2) of one (row group, walker): odd, so the 8 lanes of a
+                                                // 128-bit shared access land on distinct 16-byte bank groups
+    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * 8 * SL * 16;
 };
 
 template <int NP>
@@ -793,7 +795,7 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
     const uint32_t full = sbase + CP_STAGES * STAGE, empty = full + 8 * CP_STAGES;
     ExTile* ring = reinterpret_cast<ExTile*>(sgen + CP_STAGES * STAGE + 128);
-    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 row groups g][8 walkers][NP*NP]
+    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 fragments (warps)][8 walkers][SL]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     if (tid == 0) {
@@ -837,16 +839,23 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
         return;
     }
     reg_inc_consumer();
+    // Work units of an item = (row fragment, column half nf) = 2 * nfrag; consumer warp cw owns units cw and cw + 8, i.e.
+    // fragments cw/2 and 4 + cw/2 of the SAME column half nf = cw & 1 (they share the panel fragments).  The two warps
+    // of a scheduler (cw, cw + 4) then hold at most ceil(nfrag / 2) + ... units: 5 fragments load the four schedulers
+    // 3/3/2/2 instead of 2/1/1/1 whole fragments.
     const int cw = warp - 4, g = lane >> 2, t = lane & 3, ctid = tid - 128;
-    double accU[NP][2][2], accW[NP][2][2];
+    const int nf = cw & 1, fr0 = cw >> 1, fr1 = 4 + (cw >> 1);
+    double accU[2][NP][2], accW[2][NP][2];
 #pragma unroll
-    for (int c = 0; c < NP; ++c)
+    for (int j = 0; j < 2; ++j)
 #pragma unroll
-        for (int b = 0; b < 2; ++b) accU[c][b][0] = accU[c][b][1] = accW[c][b][0] = accW[c][b][1] = 0.0;
+        for (int c = 0; c < NP; ++c) accU[j][c][0] = accU[j][c][1] = accW[j][c][0] = accW[j][c][1] = 0.0;
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
-    const uint32_t u_row = (uint32_t)(cw * 8 + g) * 128, p_row = (uint32_t)(2 * EX_BM * 128) + (uint32_t)g * 128;
+    const uint32_t u_row0 = (uint32_t)(fr0 * 8 + g) * 128, u_row1 = (uint32_t)(fr1 * 8 + g) * 128;
+    const uint32_t p_row = (uint32_t)(2 * EX_BM * 128) + (uint32_t)(nf * 8 + g) * 128;
+    constexpr int SL = CpCfg<NP>::SL;
     int cslot = 0, n = 0;
     uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
@@ -854,22 +863,39 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
         const long long tix = q / WB;
         mbar_wait(full + 8 * cslot, cphase);
         const ExTile tile = ring[n % EX_RING];
-        const bool active = cw < tile.nfrag;            // warp-uniform
+        const int nu = (fr0 < tile.nfrag ? 1 : 0) + (fr1 < tile.nfrag ? 1 : 0);     // warp-uniform: 0, 1 or 2 units
         for (int kt = 0; kt < KT; ++kt) {
             if (kt) mbar_wait(full + 8 * cslot, cphase);
             const uint32_t st = sbase + cslot * STAGE;
-            if (active) {
+            if (nu == 2) {
 #pragma unroll
                 for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    const double a = lds_f64(st + u_row + xo[ks]), w = lds_f64(st + u_row + EX_BM * 128 + xo[ks]);
+                    const double a0 = lds_f64(st + u_row0 + xo[ks]), w0 = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
+                    const double a1 = lds_f64(st + u_row1 + xo[ks]), w1 = lds_f64(st + u_row1 + EX_BM * 128 + xo[ks]);
+                    double bb[NP];
+#pragma unroll
+                    for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 2048 + xo[ks]);
+                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
 #pragma unroll
                     for (int c = 0; c < NP; ++c) {
-                        const double b0 = lds_f64(st + p_row + c * 2048 + xo[ks]), b1 = lds_f64(st + p_row + c * 2048 + 1024 + xo[ks]);
-                        if (ks == KTILE / 4 - 1 && c == NP - 1) release_stage(empty + 8 * cslot, lane);
-                        mma884(accU[c][0][0], accU[c][0][1], a, b0);
-                        mma884(accW[c][0][0], accW[c][0][1], w, b0);
-                        mma884(accU[c][1][0], accU[c][1][1], a, b1);
-                        mma884(accW[c][1][0], accW[c][1][1], w, b1);
+                        mma884(accU[0][c][0], accU[0][c][1], a0, bb[c]);
+                        mma884(accW[0][c][0], accW[0][c][1], w0, bb[c]);
+                        mma884(accU[1][c][0], accU[1][c][1], a1, bb[c]);
+                        mma884(accW[1][c][0], accW[1][c][1], w1, bb[c]);
+                    }
+                }
+            } else if (nu == 1) {
+#pragma unroll
+                for (int ks = 0; ks < KTILE / 4; ++ks) {
+                    const double a0 = lds_f64(st + u_row0 + xo[ks]), w0 = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
+                    double bb[NP];
+#pragma unroll
+                    for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 2048 + xo[ks]);
+                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
+#pragma unroll
+                    for (int c = 0; c < NP; ++c) {
+                        mma884(accU[0][c][0], accU[0][c][1], a0, bb[c]);
+                        mma884(accW[0][c][0], accW[0][c][1], w0, bb[c]);
                     }
                 }
             } else {
@@ -878,41 +904,56 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
             }
             if (++cslot == CP_STAGES) { cslot = 0; cphase ^= 1; }
         }
-        // epilogue: S[c][c'] of the 8 walkers of the block.  Each lane adds the products of its own row into the slice of
-        // its row group g (no cross-lane traffic); the fragments take turns in a fixed order; the 8 row groups are summed
-        // in order when the block is written out.
-        const double wv = active ? __ldg(wgt + tile.row0 + cw * 8 + g) : 0.0;
-        for (int i = ctid; i < 8 * 8 * NP * NP; i += 256) Sacc[i] = make_double2(0.0, 0.0);
-        bar_sync_consumers();
-        for (int turn = 0; turn < 8; ++turn) {
-            if (turn == cw && active) {
+        // epilogue: S[c][c'] of the 4 walkers of this warp's column half, per unit.  For every panel c the lane holds the 8
+        // complex products of its own row g (c' = 0..7, zero beyond NP); a transposing butterfly over the 8 row groups
+        // (each round sends half of the values and keeps the other half: 8+4+2 exchanges instead of 3 per value) leaves
+        // the row sum of column c' = 4 b0 + 2 b1 + b2 (bits of g) in lane g.  Every fragment's S goes to its own slice;
+        // the slices are added in fragment order when the block is written out (fixed order).
+        {
+            const bool b0 = g & 1, b1 = g & 2, b2 = g & 4;
+            const int c2own = (b0 ? 4 : 0) + (b1 ? 2 : 0) + (b2 ? 1 : 0);
 #pragma unroll
-                for (int nf = 0; nf < 2; ++nf) {
-                    double2* dst = Sacc + ((g * 8) + nf * 4 + t) * NP * NP;
+            for (int j = 0; j < 2; ++j) {
+                if (j >= nu) break;                     // warp-uniform
+                const int fr = j == 0 ? fr0 : fr1;
+                const double wv = __ldg(wgt + tile.row0 + fr * 8 + g);
+                double2* dst = Sacc + ((fr * 8) + nf * 4 + t) * SL;
 #pragma unroll
-                    for (int c = 0; c < NP; ++c) {
-                        const double ur = wv * accU[c][nf][0], ui = wv * accU[c][nf][1];
+                for (int c = 0; c < NP; ++c) {
+                    const double ur = wv * accU[j][c][0], ui = wv * accU[j][c][1];
+                    double v[16];
 #pragma unroll
-                        for (int c2 = 0; c2 < NP; ++c2) {
-                            double2 o = dst[c * NP + c2];
-                            o.x += ur * accW[c2][nf][0] - ui * accW[c2][nf][1];
-                            o.y += ur * accW[c2][nf][1] + ui * accW[c2][nf][0];
-                            dst[c * NP + c2] = o;
-                        }
+                    for (int c2 = 0; c2 < 8; ++c2) {
+                        v[2 * c2] = c2 < NP ? ur * accW[j][c2 < NP ? c2 : 0][0] - ui * accW[j][c2 < NP ? c2 : 0][1] : 0.0;
+                        v[2 * c2 + 1] = c2 < NP ? ur * accW[j][c2 < NP ? c2 : 0][1] + ui * accW[j][c2 < NP ? c2 : 0][0] : 0.0;
                     }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {       // round 1: lanes g^1, halves of 8
+                        const double snd = b0 ? v[i] : v[i + 8], kp = b0 ? v[i + 8] : v[i];
+                        v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 4);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {       // round 2: lanes g^2, halves of 4
+                        const double snd = b1 ? v[i] : v[i + 4], kp = b1 ? v[i + 4] : v[i];
+                        v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 8);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {       // round 3: lanes g^4, halves of 2
+                        const double snd = b2 ? v[i] : v[i + 2], kp = b2 ? v[i + 2] : v[i];
+                        v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 16);
+                    }
+                    if (c2own < NP) dst[c * NP + c2own] = make_double2(v[0], v[1]);
                 }
+#pragma unroll
+                for (int c = 0; c < NP; ++c) accU[j][c][0] = accU[j][c][1] = accW[j][c][0] = accW[j][c][1] = 0.0;
             }
-            bar_sync_consumers();
         }
-#pragma unroll
-        for (int c = 0; c < NP; ++c)
-#pragma unroll
-            for (int b = 0; b < 2; ++b) accU[c][b][0] = accU[c][b][1] = accW[c][b][0] = accW[c][b][1] = 0.0;
+        bar_sync_consumers();
         for (int i = ctid; i < 8 * NP * NP; i += 256) {
             const int wl = i / (NP * NP), wg = wb * 8 + wl;
-            double2 sum = Sacc[i];
-#pragma unroll
-            for (int gg = 1; gg < 8; ++gg) { const double2 v = Sacc[gg * 8 * NP * NP + i]; sum.x += v.x; sum.y += v.y; }
+            const int is = wl * SL + (i - wl * NP * NP);
+            double2 sum = Sacc[is];
+            for (int fr = 1; fr < tile.nfrag; ++fr) { const double2 v = Sacc[fr * 8 * SL + is]; sum.x += v.x; sum.y += v.y; }
             if (wg < n_w) S[((size_t)tix * n_w + wg) * NP * NP + (i - wl * NP * NP)] = sum;
         }
         bar_sync_consumers();
