@@ -520,3 +520,35 @@ def test_cas_smw_energy_matches_oracle(cfg, n_virt, n_act, n_det, max_exc, n_w, 
     Ed, _ = F.local_energy_cas(dphi)
     Ed = Ed.cpu().numpy().T
     assert (np.abs(E - Ed).max(axis=1) <= 1e-9 * np.abs(Ed[:, 0])).all()
+
+
+def test_local_energy_is_cuda_graph_capturable(c1):
+    """lo_local_energy allocates nothing, does not synchronise and launches only on the caller's stream, so a whole
+    step can be captured in a CUDA graph and replayed on new walker data (launch-bound small configs)."""
+    torch = torch_cuda()
+    n_w = 64
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=n_w, gpu_svd=True)
+    phis = gen.make_walkers(c1, n_w)
+    E_ref, _ = gpu_energy(F, phis)
+    buf = torch.zeros((n_w, c1.N, c1.n_occ[0]), dtype=torch.complex128, device="cuda")
+    E = torch.empty((4, n_w), dtype=torch.complex128, device="cuda")
+    st = torch.empty(n_w, dtype=torch.int32, device="cuda")
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    import ctypes as C
+    with torch.cuda.graph(g, stream=s):
+        rc = lo.lib().lo_local_energy(F._h, n_w, C.c_void_p(buf.data_ptr()), None, C.c_void_p(E[0].data_ptr()), C.c_void_p(E[1].data_ptr()),
+                                      C.c_void_p(E[2].data_ptr()), C.c_void_p(E[3].data_ptr()), C.c_void_p(st.data_ptr()),
+                                      C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert rc == 0
+    buf.copy_(torch.from_numpy(phis[0]))
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(E.cpu().numpy().T, E_ref)
+    phis2 = gen.make_walkers(c1, n_w, seed=99)
+    E2_ref, _ = gpu_energy(F, phis2)
+    buf.copy_(torch.from_numpy(phis2[0]))
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(E.cpu().numpy().T, E2_ref)
