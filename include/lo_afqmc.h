@@ -20,6 +20,10 @@
  * "host" / "device" is stated for every pointer.  No call throws; every call returns a lo_status and
  * lo_last_error() gives a thread-local message for the last failure.  The library never frees or keeps
  * caller memory.  There is no CPU fallback: lo_local_energy* need a factor set built with device >= 0.
+ * A lo_factors handle owns ONE workspace (Theta panels, partial sums): calls on the same handle must be serialised by
+ * the caller (stream order on one stream is enough); different handles, e.g. lo_retruncate copies, are independent.
+ * lo_local_energy / lo_local_energy_cas / lo_propagator only enqueue work on the given stream, so a step can be captured
+ * in a CUDA graph (with timing disabled).
  */
 #ifndef LO_AFQMC_H
 #define LO_AFQMC_H
