@@ -156,13 +156,14 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
 // ------------------------------------------------------------------------------------------------ S1: inverse
 __device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ double2 crecip(double2 a) {
-    // Smith's algorithm
+    // Smith's algorithm with correctly rounded reciprocals (MUFU.RCP64H + Newton) instead of the two divisions: the
+    // reciprocal sits on the serial chain of every Gauss-Jordan step
     if (fabs(a.x) >= fabs(a.y)) {
-        double r = a.y / a.x, d = a.x + a.y * r;
-        return make_double2(1.0 / d, -r / d);
+        const double r = a.y * __drcp_rn(a.x), id = __drcp_rn(a.x + a.y * r);
+        return make_double2(id, -r * id);
     } else {
-        double r = a.x / a.y, d = a.x * r + a.y;
-        return make_double2(r / d, -1.0 / d);
+        const double r = a.x * __drcp_rn(a.y), id = __drcp_rn(a.x * r + a.y);
+        return make_double2(r * id, -id);
     }
 }
 
@@ -294,6 +295,127 @@ __global__ void __launch_bounds__(256) k_inverse(double2* __restrict__ Aws, int*
     } else if (IN_SMEM) {
         for (int e = tid; e < OO; e += 256) Ag[e] = M[e];
     }
+    if (tid == 0) status[w] = singular ? 1 : 0;
+}
+
+// Register-resident variant for O <= 16*RT <= 48: the 16 x 16 thread grid keeps the matrix in registers (thread (tx,ty) owns
+// rows ty + 16a, columns tx + 16b); only the pivot column and the two exchanged rows go through (double-buffered) shared
+// memory, so a step costs 3 barriers and no shared-memory traffic for the rank-1 update.  Same pivoting rule and the
+// same column un-permutation as k_inverse.
+template <int RT>
+__global__ void __launch_bounds__(256) k_inverse_reg(double2* __restrict__ Aws, int* __restrict__ status, int O) {
+    __shared__ double2 colbuf[2][RT * 16], rowk[2][RT * 16], rowp[2][RT * 16], pvs;
+    __shared__ int perm[RT * 16], dest[RT * 16], ctl[2];
+    const int w = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, tx = tid & 15, ty = tid >> 4;
+    double2* Ag = Aws + (size_t)w * O * O;
+    double2 M[RT][RT];
+#pragma unroll
+    for (int a = 0; a < RT; ++a)
+#pragma unroll
+        for (int b = 0; b < RT; ++b) {
+            const int r = ty + 16 * a, c = tx + 16 * b;
+            M[a][b] = (r < O && c < O) ? Ag[(size_t)r * O + c] : make_double2(0.0, 0.0);
+        }
+    if (tid == 0) ctl[1] = 0;
+    __syncthreads();
+    for (int k = 0; k < O; ++k) {
+        const int kb = k >> 4, kx = k & 15, ka = kb, ky = kx, buf = k & 1;
+        if (tx == kx) {
+#pragma unroll
+            for (int a = 0; a < RT; ++a)
+#pragma unroll
+                for (int b = 0; b < RT; ++b)
+                    if (b == kb) colbuf[buf][ty + 16 * a] = M[a][b];
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double best = -1.0;
+            int bi = k;
+            for (int r = k + lane; r < O; r += 32) {
+                const double2 v = colbuf[buf][r];
+                double m = v.x * v.x + v.y * v.y;
+                if (!(m == m)) m = INFINITY;
+                if (m > best) { best = m; bi = r; }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+            }
+            if (lane == 0) {
+                ctl[0] = bi;
+                perm[k] = bi;
+                pvs = colbuf[buf][bi];
+                if (!(best > 1e-300) || isinf(best)) ctl[1] = 1;
+            }
+        }
+        __syncthreads();
+        if (ctl[1]) break;   // uniform
+        const int piv = ctl[0], pa = piv >> 4, py = piv & 15;
+        const double2 inv = crecip(pvs);
+#pragma unroll
+        for (int a = 0; a < RT; ++a) {
+            if (ty == ky && a == ka) {
+#pragma unroll
+                for (int b = 0; b < RT; ++b) rowk[buf][tx + 16 * b] = M[a][b];
+            }
+            if (ty == py && a == pa) {
+#pragma unroll
+                for (int b = 0; b < RT; ++b) rowp[buf][tx + 16 * b] = M[a][b];
+            }
+        }
+        __syncthreads();
+        double2 v[RT];
+#pragma unroll
+        for (int b = 0; b < RT; ++b) v[b] = cmul(rowp[buf][tx + 16 * b], inv);
+#pragma unroll
+        for (int a = 0; a < RT; ++a) {
+            const int r = ty + 16 * a;
+            const bool is_k = r == k, is_p = r == piv && piv != k;
+            const double2 f = is_p ? colbuf[buf][k] : colbuf[buf][r];
+#pragma unroll
+            for (int b = 0; b < RT; ++b) {
+                const int c = tx + 16 * b;
+                if (is_k) {
+                    M[a][b] = c == k ? inv : v[b];
+                } else {
+                    const double2 base = is_p ? rowk[buf][c] : M[a][b];
+                    double2 m;
+                    if (c == k) {
+                        m = make_double2(-(f.x * inv.x - f.y * inv.y), -(f.x * inv.y + f.y * inv.x));
+                    } else {
+                        m.x = fma(-f.x, v[b].x, fma(f.y, v[b].y, base.x));
+                        m.y = fma(-f.x, v[b].y, fma(-f.y, v[b].x, base.y));
+                    }
+                    M[a][b] = m;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    const bool singular = ctl[1] != 0;
+    if (tid == 0 && !singular) {
+        // column un-permutation A^-1 = (P A)^-1 P: the swaps of k_inverse applied to an index list, then inverted
+        for (int c = 0; c < O; ++c) dest[c] = c;            // dest used as position -> content first
+        for (int k = O - 1; k >= 0; --k) {
+            const int p2 = perm[k];
+            const int t1 = dest[k]; dest[k] = dest[p2]; dest[p2] = t1;
+        }
+        for (int j = 0; j < O; ++j) perm[dest[j]] = j;      // perm reused as content -> position
+    }
+    __syncthreads();
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+#pragma unroll
+    for (int a = 0; a < RT; ++a)
+#pragma unroll
+        for (int b = 0; b < RT; ++b) {
+            const int r = ty + 16 * a, c = tx + 16 * b;
+            if (r < O && c < O) {
+                if (singular) Ag[(size_t)r * O + c] = make_double2(nan, nan);
+                else Ag[(size_t)r * O + perm[c]] = M[a][b];
+            }
+        }
     if (tid == 0) status[w] = singular ? 1 : 0;
 }
 
@@ -1366,10 +1488,17 @@ void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, cons
         Timer tm(f, stream, LO_K_INVERSE);
         size_t aux = (size_t)(2 * O + 1) * 16 + (size_t)((O + 3) & ~3) * 4 + 16;
         size_t need = aux + (size_t)O * O * 16;
-        if (need <= 200 * 1024)
-            k_inverse<true><<<n_w, 256, need, stream>>>((double2*)dA, status, O);
+        const int rt = (O + 15) / 16;
+        double2* Ad = (double2*)dA;
+        // register-resident variant while >= 2 CTAs per SM fit (<= 96 registers: O <= 48); beyond that its serial chain
+        // (pivot search, reciprocal, 3 barriers) is no longer hidden by a second CTA and the shared-memory kernel wins
+        if (rt == 1) k_inverse_reg<1><<<n_w, 256, 0, stream>>>(Ad, status, O);
+        else if (rt == 2) k_inverse_reg<2><<<n_w, 256, 0, stream>>>(Ad, status, O);
+        else if (rt == 3) k_inverse_reg<3><<<n_w, 256, 0, stream>>>(Ad, status, O);
+        else if (need <= 200 * 1024)
+            k_inverse<true><<<n_w, 256, need, stream>>>(Ad, status, O);
         else
-            k_inverse<false><<<n_w, 256, aux, stream>>>((double2*)dA, status, O);
+            k_inverse<false><<<n_w, 256, aux, stream>>>(Ad, status, O);
     }
     {
         Timer tm(f, stream, LO_K_THETA);
