@@ -552,3 +552,54 @@ def test_local_energy_is_cuda_graph_capturable(c1):
     g.replay()
     torch.cuda.synchronize()
     assert np.array_equal(E.cpu().numpy().T, E2_ref)
+
+
+def test_cas_smw_full_size_sampled_walkers():
+    """NEXT-2 at the bench's size: configs[2] in the paper-like (vector) reading, 79 orbitals (73 reference + 6 active
+    virtuals), 24 determinants with up to 4 excitations out of 6 active occupied columns, 64 walkers through
+    LO_CAS_SMW_ENERGY; two seeded walkers checked against the oracle's definition on the library's factor set."""
+    torch = torch_cuda()
+    P = gen.make_problem(2, reading="vector")
+    T = gen.make_cas_trial(P, n_virt=6, n_act_occ=6, n_det=24, max_exc=4)
+    n_w = 64
+    F = lo.Factors.setup(P.h, P.L, [T.C], 1e-5, device=0, max_walkers=n_w, gpu_svd=True)
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w, smw_energy=True)
+    phi = gen.make_walkers(P, n_w)[0]
+    E, st = F.local_energy_cas(torch.from_numpy(phi).cuda())
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    assert (st == 0).all() and np.isfinite(E).all()
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, T.C)
+    n_orb = T.C.shape[1]
+    U, sg, W = F.factor_all(0)
+    pi, pj = oracle.all_pairs(n_orb)
+    fs = oracle.make_factor_set(P.N, n_orb, pi, pj, F.ranks(0), U, sg, W)
+    cols = [T.columns(d) for d in range(T.n_det)]
+    for w in np.random.default_rng(22).choice(n_w, 2, replace=False):
+        Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w], compressed_coulomb=True))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+
+
+def test_cas_smw_edge_cases(c0):
+    """One determinant (no excitation) through the SMW-energy mode = the single-determinant energy with the
+    compressed Coulomb term; more than 6 distinct hole columns are refused in that mode (and accepted in direct mode)."""
+    torch = torch_cuda()
+    T = gen.make_cas_trial(c0, n_virt=3, n_act_occ=3, n_det=4, max_exc=2)
+    F = lo.Factors.setup(c0.h, c0.L, [T.C], 1e-8, device=0, max_walkers=64, gpu_svd=True)
+    phi = gen.make_walkers(c0, 8)[0]
+    dphi = torch.from_numpy(phi).cuda()
+    F.set_cas_trial(T.n_ref, T.holes[:1], T.parts[:1], T.coef[:1], 8, smw_energy=True)
+    E1d, st = F.local_energy_cas(dphi)
+    F0 = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=0, max_walkers=8, gpu_svd=True)
+    F0.set_coulomb_mode(True)
+    Es, _ = gpu_energy(F0, [phi])
+    assert np.abs(E1d.cpu().numpy().T[:, :4] - Es).max() <= 1e-9 * np.abs(Es[:, 0]).max()
+    # 7 distinct hole columns (c0 has 6 reference columns -> use a wider reference)
+    P = gen.make_problem(1)
+    Tw = gen.make_cas_trial(P, n_virt=4, n_act_occ=9, n_det=40, max_exc=2)
+    assert len(set(Tw.holes[Tw.holes >= 0].tolist())) > 6
+    Fw = lo.Factors.setup(P.h, P.L, [Tw.C], 1e-2, device=0, max_walkers=80, gpu_svd=True)
+    with pytest.raises(lo.LoError):
+        Fw.set_cas_trial(Tw.n_ref, Tw.holes, Tw.parts, Tw.coef, 2, smw_energy=True)
+    Fw.set_cas_trial(Tw.n_ref, Tw.holes, Tw.parts, Tw.coef, 2, smw_energy=False)
