@@ -1113,6 +1113,7 @@ __global__ void __launch_bounds__(256) k_cas_H(const double* __restrict__ hbar, 
 // lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of CE_CH tiles sits in shared memory, threads
 // run over determinants; partial (E_K, E_J) sums per chunk are added in chunk order by k_cas_e1sum.
 constexpr int CE_CH = 16;
+template <int MAXE>     // compile-time bound of the excitation rank: the coefficient lists stay in registers
 __global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const ExTile* __restrict__ tiles, long long n_tiles,
                                                     const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
                                                     const double2* __restrict__ G, double2* __restrict__ part, int n_w, int n_det, int max_exc,
@@ -1142,22 +1143,29 @@ __global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ 
             if (kx < 0 || ky < 0) continue;
             const double2* St = Ss + tl * NP2;
             // coefficient lists: entry 0 = self (index 0 for the x role, 1 for the y role), entries 1..e = the holes
-            double2 cx[CAS_MAX_EXC + 1], cy[CAS_MAX_EXC + 1];
-            int ix[CAS_MAX_EXC + 1], iy[CAS_MAX_EXC + 1];
+            double2 cx[MAXE + 1], cy[MAXE + 1];
+            int ix[MAXE + 1], iy[MAXE + 1];
             cx[0] = make_double2(kx == 0 ? 1.0 : 0.0, 0.0); ix[0] = 0;
             cy[0] = make_double2(ky == 0 ? 1.0 : 0.0, 0.0); iy[0] = 1;
-            for (int k = 0; k < e; ++k) {
-                cx[1 + k] = Gv[(size_t)k * n_orb + x]; ix[1 + k] = 2 + hi[k];
-                cy[1 + k] = Gv[(size_t)k * n_orb + y]; iy[1 + k] = 2 + hi[k];
+#pragma unroll
+            for (int k = 0; k < MAXE; ++k) {
+                const bool on = k < e;
+                cx[1 + k] = on ? Gv[(size_t)k * n_orb + x] : make_double2(0.0, 0.0); ix[1 + k] = on ? 2 + hi[k] : 0;
+                cy[1 + k] = on ? Gv[(size_t)k * n_orb + y] : make_double2(0.0, 0.0); iy[1 + k] = on ? 2 + hi[k] : 0;
             }
-            for (int a = 0; a <= e; ++a)
-                for (int b = 0; b <= e; ++b) {
+#pragma unroll
+            for (int a = 0; a <= MAXE; ++a) {
+                if (a > e) break;
+#pragma unroll
+                for (int b = 0; b <= MAXE; ++b) {
+                    if (b > e) break;
                     const double2 cc = cmul(cy[a], cx[b]);
                     const double2 se = St[iy[a] * NP + ix[b]], sj = St[ix[b] * NP + iy[a]];
                     const double2 t1 = cmul(cc, se), t2 = cmul(cc, sj);
                     ek.x += t1.x; ek.y += t1.y;
                     ej.x += t2.x; ej.y += t2.y;
                 }
+            }
         }
         part[((size_t)chunk * n_vtot + v) * 2] = ek;
         part[((size_t)chunk * n_vtot + v) * 2 + 1] = make_double2(-2.0 * ej.x, -2.0 * ej.y);
@@ -1464,7 +1472,6 @@ lo_status configure_kernels() {
     e = cudaFuncSetAttribute(k_cas_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<4>::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<6>::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<8>::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_energy, cudaFuncAttributeMaxDynamicSharedMemorySize, CE_CH * 64 * 16);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_cas_*): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
@@ -1620,9 +1627,16 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void*
         const int n_vtot = c.max_real * c.n_det;
         if (n_chunks > 0) {
             dim3 g4(n_chunks, n_w);
-            k_cas_energy<<<g4, 128, (size_t)CE_CH * c.NP * c.NP * 16, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx,
-                                                                              (const double2*)c.dG, (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb,
-                                                                              c.NP, n_vtot);
+            const size_t sm4 = (size_t)CE_CH * c.NP * c.NP * 16;
+            if (c.max_exc <= 2)
+                k_cas_energy<2><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
+                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
+            else if (c.max_exc <= 4)
+                k_cas_energy<4><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
+                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
+            else
+                k_cas_energy<8><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
+                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
         }
         k_cas_e1sum<<<(n_v + 127) / 128, 128, 0, stream>>>((const double2*)c.dPart, n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx,
                                                            (const double2*)c.dG, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_orb, n_vtot);
