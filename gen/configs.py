@@ -273,14 +273,16 @@ class CasTrial:
         return cols
 
 
-def make_cas_trial(problem: Problem, n_virt: int, n_act_occ: int, n_det: int, max_exc: int, seed: int | None = None) -> CasTrial:
+def make_cas_trial(problem: Problem, n_virt: int, n_act_occ: int, n_det: int, max_exc: int, seed: int | None = None,
+                   spin: int = 0) -> CasTrial:
     """Reference = problem.psi[0]; `n_virt` active virtuals = Gaussian columns damped like the occupied ones, projected
     onto the complement of the reference and Loewdin-orthonormalised; determinant 0 is the reference (c=1), the others
     replace e in 1..max_exc of the last `n_act_occ` reference columns by distinct virtuals (no duplicates), with
-    c_d = 0.3 N(0,1) 2^-e."""
+    c_d = 0.3 N(0,1) 2^-e.  `spin` picks problem.psi[spin] (its own random stream): an unrestricted trial is one call per
+    spin with the same n_det / max_exc, the alpha call's coefficients being the c_d."""
     seed = problem.seed if seed is None else seed
-    rng = _rng(seed, _TAG_CAS)
-    psi = problem.psi[0]
+    rng = _rng(seed, _TAG_CAS, spin)
+    psi = problem.psi[spin]
     N, O = psi.shape
     Rp = problem.site_xyz[problem.site_of_fn]
     centers = problem.site_xyz[np.arange(n_virt) % len(problem.site_xyz)]

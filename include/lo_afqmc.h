@@ -143,6 +143,7 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
  * lo_local_energy_cas: phi device complex128 [n_w][N][n_ref]; E_L (required), E1, E_J, E_K, ovlp device complex128
  * [n_w] (ovlp = sum_d w_d / <reference|Phi>, the trial overlap in units of the reference overlap); walker_status as in
  * lo_local_energy.  A determinant with a singular overlap contributes nothing.  Asynchronous; allocates nothing.
+ * Closed-shell factor sets (n_spin = 1) use the same string for both spins (w_d = c_d det^2).
  * mode LO_CAS_DIRECT: cost = n_det x the single-determinant evaluation; needs max_walkers >= max_real_walkers * n_det.
  * mode LO_CAS_SMW_ENERGY: the rearranged sums of Eq. 21-23: every Theta^d column is the reference
  *   column plus a combination of the active (hole) columns of Theta0 = Phi A^-1, so for each pair (x<=y) the projections
@@ -155,8 +156,14 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
 #define LO_CAS_SMW_ENERGY 1
 lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts,
                            const double* coef, int max_real_walkers, int mode);
-lo_status lo_local_energy_cas(const lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K,
-                              void* ovlp, int* walker_status, void* stream);
+/* Unrestricted trial (factor set with n_spin = 2, LO_CAS_DIRECT only): determinant d = |alpha string d> |beta string d>.
+ * lo_set_cas_trial gives the alpha strings (reference = the first n_ref columns of psi_a), lo_set_cas_trial_beta the
+ * beta strings of the same n_det / max_exc (reference = the first n_ref_b columns of psi_b); w_d = c_d det_a det_b, and
+ * every (walker, determinant) is one virtual walker of the unrestricted path (Eq. 10 with explicit spin sums). */
+lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, const int* parts_b);
+/* phi_b: device complex128 [n_w][N][n_ref_b] for an unrestricted trial, NULL otherwise. */
+lo_status lo_local_energy_cas(const lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1,
+                              void* E_J, void* E_K, void* ovlp, int* walker_status, void* stream);
 
 /* SURVEY 8(f) NEXT-1, propagator formation: B_w = sum_g x^g_w L^g ("forming the propagation matrix
  * (B = sum_alpha x_alpha L_alpha), scaling as X M^2"), for n_w walkers at once as one real x

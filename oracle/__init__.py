@@ -383,3 +383,38 @@ def local_energy_cas(Cmo, columns, coef, Lbar, hbar, fs, phi, exact=False, compr
         den += w
     E = num / den
     return E.sum(), E[0], E[1], E[2], den / w0
+
+
+def local_energy_cas_u(Cmo, columns, coef, Lbar, hbar, fs, phi):
+    """Unrestricted version of local_energy_cas: per-spin lists Cmo[s], columns[s][d], Lbar[s], hbar[s], fs[s], phi[s];
+    determinant d = |alpha string d>|beta string d>, w_d = c_d det(Psi_d^a^T phi_a) det(Psi_d^b^T phi_b), and E^d by the
+    unrestricted formulas (E1 summed over spins, E_J = 1/2 sum_g (X_a+X_b)^2, E_K = 1/2 sum over same-spin
+    pairs).  Returns (E_L, E1, E_J, E_K, sum_d w_d / w_reference)."""
+    num = np.zeros(3, dtype=np.complex128)
+    den = 0.0 + 0.0j
+    w0 = None
+    for d in range(len(coef)):
+        ths, Ls, hs, dets, ek, bad = [], [], [], [], 0.0 + 0.0j, False
+        for s in range(2):
+            cols = np.asarray(columns[s][d])
+            th, det, st = theta(_f64(Cmo[s])[:, cols], _c128(phi[s]))
+            bad |= st != 0
+            order = np.argsort(cols)
+            sc = cols[order]
+            t = np.ascontiguousarray(th[:, order])
+            ths.append(t)
+            Ls.append(np.ascontiguousarray(Lbar[s][:, sc, :]))
+            hs.append(np.ascontiguousarray(hbar[s][sc]))
+            dets.append(det)
+            if not bad:
+                ek += 0.5 * exchange_lo(sub_factor_set(fs[s], sc), t)
+        if w0 is None:
+            w0 = dets[0] * dets[1]
+        if bad:
+            continue
+        e1, ej = onebody_coulomb(Ls, hs, ths)
+        w = coef[d] * dets[0] * dets[1]
+        num += w * np.array([e1, ej, ek])
+        den += w
+    E = num / den
+    return E.sum(), E[0], E[1], E[2], den / w0

@@ -18,7 +18,7 @@ LO_SETUP_PROPAGATOR = 2
 K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 4: "LO_ESINGULAR", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_local_energy",
-           "lo_local_energy_host", "lo_set_cas_trial", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
+           "lo_local_energy_host", "lo_set_cas_trial", "lo_set_cas_trial_beta", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
            "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
 
 
@@ -58,7 +58,8 @@ def lib():
         L.lo_theta_host.argtypes = [vp, ci, ci, vp]
         L.lo_set_coulomb_mode.argtypes = [vp, ci]
         L.lo_set_cas_trial.argtypes = [vp, ci, ci, ci, vp, vp, vp, ci, ci]
-        L.lo_local_energy_cas.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.lo_set_cas_trial_beta.argtypes = [vp, ci, vp, vp]
+        L.lo_local_energy_cas.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.lo_propagator.argtypes = [vp, ci, vp, vp]
         L.lo_propagator_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(ci), C.POINTER(C.c_longlong)]
         L.lo_propagator_host.argtypes = [vp, ci, vp]
@@ -226,7 +227,12 @@ class Factors:
         _check(lib().lo_set_cas_trial(self._h, int(n_ref), n_det, max_exc, holes.ctypes.data, parts.ctypes.data, coef.ctypes.data,
                                       int(max_real_walkers), 1 if smw_energy else 0))
 
-    def local_energy_cas(self, phi, stream=None):
+    def set_cas_trial_beta(self, n_ref_b, holes_b, parts_b):
+        """lo_set_cas_trial_beta: beta strings of an unrestricted trial (after set_cas_trial with the alpha strings)."""
+        holes_b, parts_b = _np(holes_b, np.int32), _np(parts_b, np.int32)
+        _check(lib().lo_set_cas_trial_beta(self._h, int(n_ref_b), holes_b.ctypes.data, parts_b.ctypes.data))
+
+    def local_energy_cas(self, phi, phi_b=None, stream=None):
         """lo_local_energy_cas on a torch CUDA complex128 tensor [n_w, N, n_ref]; returns (E [5, n_w] = E_L, E1, E_J,
         E_K, overlap ratio; status [n_w]) torch tensors.  Asynchronous on the current (or given) stream."""
         import torch
@@ -238,7 +244,9 @@ class Factors:
         E = torch.empty((5, n_w), dtype=torch.complex128, device=dev)
         st_t = torch.empty(n_w, dtype=torch.int32, device=dev)
         ptr = lambda t: C.c_void_p(t.data_ptr())
-        _check(lib().lo_local_energy_cas(self._h, n_w, ptr(phi), ptr(E[0]), ptr(E[1]), ptr(E[2]), ptr(E[3]), ptr(E[4]), ptr(st_t),
+        if phi_b is not None:
+            phi_b = phi_b if phi_b.is_contiguous() else phi_b.contiguous()
+        _check(lib().lo_local_energy_cas(self._h, n_w, ptr(phi), ptr(phi_b) if phi_b is not None else None, ptr(E[0]), ptr(E[1]), ptr(E[2]), ptr(E[3]), ptr(E[4]), ptr(st_t),
                                          C.c_void_p(s.cuda_stream)))
         return E, st_t
 

@@ -398,7 +398,8 @@ void free_all(lo_factors* f) {
         f->bW.release();
         if (f->cas) {
             void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd,
-                          f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS, f->cas->dH, f->cas->dPart, f->cas->dStV};
+                          f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS, f->cas->dH, f->cas->dPart, f->cas->dStV, f->cas->dHolesB, f->cas->dPartsB,
+                          f->cas->dTh0B, f->cas->dA0B, f->cas->dTB, f->cas->dGB, f->cas->dWdB, f->cas->dSt0B};
             for (void* q : cp)
                 if (q) cudaFree(q);
             delete f->cas;
@@ -788,7 +789,10 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
                            int max_real_walkers, int mode) {
     if (!f || !holes || !parts || !coef) { set_error("lo_set_cas_trial: NULL argument"); return LO_EINVAL; }
     if (f->device < 0) { set_error("lo_set_cas_trial: no device"); return LO_ECUDA; }
-    if (f->n_spin != 1) { set_error("lo_set_cas_trial: closed-shell factor sets only (n_spin == 1)"); return LO_EINVAL; }
+    if (f->n_spin != 1 && mode != LO_CAS_DIRECT) {
+        set_error("lo_set_cas_trial: an unrestricted factor set (n_spin == 2) supports LO_CAS_DIRECT only");
+        return LO_EINVAL;
+    }
     const int n_orb = f->n_occ[0];
     if (mode != LO_CAS_DIRECT && mode != LO_CAS_SMW_ENERGY) { set_error("lo_set_cas_trial: mode must be LO_CAS_DIRECT or LO_CAS_SMW_ENERGY"); return LO_EINVAL; }
     if (n_ref <= 0 || n_ref > n_orb || n_det <= 0 || max_exc <= 0 || max_exc > CAS_MAX_EXC || max_real_walkers <= 0 ||
@@ -819,7 +823,8 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     CK(cudaSetDevice(f->device));
     if (f->cas) {
         void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd, f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS,
-                      f->cas->dH, f->cas->dPart, f->cas->dStV};
+                      f->cas->dH, f->cas->dPart, f->cas->dStV, f->cas->dHolesB, f->cas->dPartsB, f->cas->dTh0B, f->cas->dA0B, f->cas->dTB,
+                      f->cas->dGB, f->cas->dWdB, f->cas->dSt0B};
         for (void* q : cp)
             if (q) cudaFree(q);
         delete f->cas;
@@ -883,9 +888,66 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     return LO_OK;
 }
 
-lo_status lo_local_energy_cas(const lo_factors* fc, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
-                              int* walker_status, void* stream) {
+// validates one spin's excitation lists (shared by lo_set_cas_trial and lo_set_cas_trial_beta)
+static lo_status check_strings(int n_det, int max_exc, int n_ref, int n_orb, const int* holes, const int* parts) {
+    for (int d = 0; d < n_det; ++d) {
+        bool ended = false;
+        for (int k = 0; k < max_exc; ++k) {
+            const int h = holes[(size_t)d * max_exc + k], p = parts[(size_t)d * max_exc + k];
+            if (h < 0 || p < 0) { if (h >= 0 || p >= 0) { set_error("lo_set_cas_trial: hole/particle lists of different length"); return LO_EINVAL; } ended = true; continue; }
+            if (ended || h >= n_ref || p < n_ref || p >= n_orb) { set_error("lo_set_cas_trial: hole must be < n_ref, particle in [n_ref, n_occ), -1 padding at the end"); return LO_EINVAL; }
+            for (int l = 0; l < k; ++l)
+                if (holes[(size_t)d * max_exc + l] == h || parts[(size_t)d * max_exc + l] == p) { set_error("lo_set_cas_trial: repeated hole or particle in one determinant"); return LO_EINVAL; }
+        }
+    }
+    return LO_OK;
+}
+
+lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, const int* parts_b) {
+    if (!f || !holes_b || !parts_b) { set_error("lo_set_cas_trial_beta: NULL argument"); return LO_EINVAL; }
+    if (!f->cas || f->n_spin != 2 || f->cas->mode != LO_CAS_DIRECT) {
+        set_error("lo_set_cas_trial_beta: needs an unrestricted factor set and a preceding lo_set_cas_trial(..., LO_CAS_DIRECT) with the alpha strings");
+        return LO_EINVAL;
+    }
+    CasPlan* c = f->cas;
+    const int n_orb_b = f->n_occ[1];
+    if (n_ref_b <= 0 || n_ref_b > n_orb_b) { set_error("lo_set_cas_trial_beta: n_ref_b out of range"); return LO_EINVAL; }
+    lo_status st = check_strings(c->n_det, c->max_exc, n_ref_b, n_orb_b, holes_b, parts_b);
+    if (st != LO_OK) return st;
+    CK(cudaSetDevice(f->device));
+    void* old[] = {c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B};
+    for (void* q : old)
+        if (q) cudaFree(q);
+    c->dHolesB = c->dPartsB = nullptr; c->dTh0B = c->dA0B = c->dTB = c->dGB = c->dWdB = nullptr; c->dSt0B = nullptr;
+    c->has_beta = false;
+    c->n_ref_b = n_ref_b; c->n_virt_b = n_orb_b - n_ref_b;
+    const size_t nv = (size_t)c->max_real * c->n_det, ne = (size_t)c->n_det * c->max_exc;
+    auto al = [&](void** p, size_t bytes) -> cudaError_t {
+        cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16));
+        if (e == cudaSuccess) e = cudaMemset(*p, 0, std::max<size_t>(bytes, 16));
+        return e;
+    };
+    CK(al((void**)&c->dHolesB, ne * 4));
+    CK(al((void**)&c->dPartsB, ne * 4));
+    CK(al((void**)&c->dTh0B, (size_t)n_orb_b * 2 * c->W0cap * f->N_pad * 8));
+    CK(al((void**)&c->dA0B, (size_t)c->W0cap * n_ref_b * n_ref_b * 16));
+    CK(al((void**)&c->dTB, (size_t)c->W0cap * std::max(c->n_virt_b, 1) * n_ref_b * 16));
+    CK(al((void**)&c->dGB, nv * c->max_exc * n_orb_b * 16));
+    CK(al((void**)&c->dWdB, nv * 16));
+    CK(al((void**)&c->dSt0B, (size_t)c->W0cap * 4));
+    CK(cudaMemcpy(c->dHolesB, holes_b, ne * 4, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->dPartsB, parts_b, ne * 4, cudaMemcpyHostToDevice));
+    c->has_beta = true;
+    return LO_OK;
+}
+
+lo_status lo_local_energy_cas(const lo_factors* fc, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
+                              void* ovlp, int* walker_status, void* stream) {
     if (!fc || !phi || !E_L) { set_error("lo_local_energy_cas: NULL argument"); return LO_EINVAL; }
+    if (fc->cas && fc->n_spin == 2 && (!fc->cas->has_beta || !phi_b || ((uintptr_t)phi_b & 15))) {
+        set_error("lo_local_energy_cas: an unrestricted trial needs lo_set_cas_trial_beta and a 16-byte aligned phi_b");
+        return LO_EINVAL;
+    }
     if (fc->device < 0) { set_error("lo_local_energy_cas: no device; there is no CPU path"); return LO_ECUDA; }
     if (!fc->cas) { set_error("lo_local_energy_cas: call lo_set_cas_trial first"); return LO_EINVAL; }
     if (n_w <= 0 || n_w > fc->cas->max_real) { set_error("lo_local_energy_cas: n_w out of range (1..max_real_walkers)"); return LO_EINVAL; }
@@ -895,7 +957,7 @@ lo_status lo_local_energy_cas(const lo_factors* fc, int n_w, const void* phi, vo
     }
     lo_factors* f = const_cast<lo_factors*>(fc);
     CK(cudaSetDevice(f->device));
-    return launch_local_energy_cas(f, n_w, phi, E_L, E1, E_J, E_K, ovlp, walker_status, (cudaStream_t)stream);
+    return launch_local_energy_cas(f, n_w, phi, f->n_spin == 2 ? phi_b : nullptr, E_L, E1, E_J, E_K, ovlp, walker_status, (cudaStream_t)stream);
 }
 
 lo_status lo_propagator(const lo_factors* fc, int n_w, const void* x_dev, void* stream) {

@@ -85,6 +85,12 @@ struct CasPlan {
     double* dEv = nullptr;                      // per virtual walker {E_L,E1,E_J,E_K}: [max_real*n_det][4] complex
     int* dSt0 = nullptr;                        // [W0cap] status of the reference overlap
     int* dStV = nullptr;                        // [max_real*n_det] status per (walker, determinant), SMW-energy mode
+    // ---- beta strings of an unrestricted trial (lo_set_cas_trial_beta; direct mode only); alpha uses the fields above
+    bool has_beta = false;
+    int n_ref_b = 0, n_virt_b = 0;
+    int *dHolesB = nullptr, *dPartsB = nullptr;
+    double *dTh0B = nullptr, *dA0B = nullptr, *dTB = nullptr, *dGB = nullptr, *dWdB = nullptr;
+    int* dSt0B = nullptr;
     // ---- rearranged SMW energy (Eq. 23), mode 1
     int mode = 0;                               // 0: direct summation over virtual walkers, 1: SMW energy
     int n_act = 0, NP = 0;                      // active (hole) columns A_set, panel-set size NP = 2 + padded n_act (4, 6 or 8)
@@ -164,7 +170,7 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
                               void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 lo_status configure_kernels();
 lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStream_t stream);
-lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
+lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
                                   int* walker_status, cudaStream_t stream);
 // 2D fp64 tensor map over a row-major [rows][inner] array, box [box_rows][16], 128-byte swizzle, zero OOB fill.
 lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner, unsigned long long rows, unsigned box_rows);   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)

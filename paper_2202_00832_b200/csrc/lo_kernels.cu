@@ -1207,12 +1207,13 @@ __global__ void __launch_bounds__(128) k_cas_e1sum(const double2* __restrict__ p
 }
 
 // One warp per virtual walker v = w*n_det + d: lane 0 inverts T_d (<= 8 x 8, Gauss-Jordan with partial pivoting) and
-// takes its determinant; all lanes then fill G_d.  weight = c_d det(T_d)^2 (closed shell: the same string in both spins);
+// takes its determinant; all lanes then fill G_d.  weight = c_d det(T_d)^2 (closed shell: the same string in both spins;
+// unrestricted: c_d det(T_d^alpha) from the alpha call times det(T_d^beta) from the beta call, multiplied in k_cas_combine);
 // status 1 when the reference overlap or T_d is singular (that determinant is then left out of the sums).
 __global__ void __launch_bounds__(128) k_cas_coef(const double2* __restrict__ T, const int* __restrict__ holes, const int* __restrict__ parts,
                                                   const double* __restrict__ coef, const int* __restrict__ st0, double2* __restrict__ G,
                                                   double2* __restrict__ wd, int* __restrict__ stv, int n_v, int n_det, int max_exc, int n_ref,
-                                                  int n_virt, int n_orb) {
+                                                  int n_virt, int n_orb, int wmode /* 0: c det^2, 1: c det (alpha), 2: det (beta) */) {
     __shared__ double2 inv_s[4][CAS_MAX_EXC][CAS_MAX_EXC];
     __shared__ int ok_s[4];
     const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5, v = blockIdx.x * 4 + wi;
@@ -1261,8 +1262,9 @@ __global__ void __launch_bounds__(128) k_cas_coef(const double2* __restrict__ T,
         for (int k = 0; k < e; ++k)
             for (int l = 0; l < e; ++l) inv_s[wi][k][l] = I[k][l];
         ok_s[wi] = ok ? 1 : 0;
-        const double2 d2 = cmul(det, det);
-        wd[v] = ok ? make_double2(coef[d] * d2.x, coef[d] * d2.y) : make_double2(0.0, 0.0);
+        const double2 d2 = wmode == 0 ? cmul(det, det) : det;
+        const double cf = wmode == 2 ? 1.0 : coef[d];
+        wd[v] = ok ? make_double2(cf * d2.x, cf * d2.y) : make_double2(0.0, 0.0);
         stv[v] = ok ? 0 : 1;
     }
     __syncwarp();
@@ -1292,7 +1294,7 @@ __global__ void __launch_bounds__(128) k_cas_coef(const double2* __restrict__ T,
 // Theta^d panels of every virtual walker: grid (n_v, n_orb, ceil(N_pad/128)), thread = basis index p.
 __global__ void __launch_bounds__(128) k_cas_theta(const double* __restrict__ th0, const double2* __restrict__ G, const int* __restrict__ holes,
                                                    double* __restrict__ thT, int N_pad, int n_ref, int n_orb, int n_det, int max_exc, int ldw0,
-                                                   int ldw) {
+                                                   int ldw, int o_base) {
     const int p = blockIdx.z * 128 + threadIdx.x, x = blockIdx.y, v = blockIdx.x;
     if (p >= N_pad) return;
     const int w = v / n_det, d = v - w * n_det;
@@ -1312,21 +1314,22 @@ __global__ void __launch_bounds__(128) k_cas_theta(const double* __restrict__ th
         re = fma(g.x, tr, fma(-g.y, ti, re));
         im = fma(g.x, ti, fma(g.y, tr, im));
     }
-    thT[((size_t)x * ldw + 2 * v) * N_pad + p] = re;
-    thT[((size_t)x * ldw + 2 * v + 1) * N_pad + p] = im;
+    thT[((size_t)(o_base + x) * ldw + 2 * v) * N_pad + p] = re;
+    thT[((size_t)(o_base + x) * ldw + 2 * v + 1) * N_pad + p] = im;
 }
 
 // E = sum_d w_d E^d / sum_d w_d per real walker and energy term (Eq. 12), determinants in index order (fixed order).
 __global__ void k_cas_combine(const double2* __restrict__ Ev, const double2* __restrict__ wd, const int* __restrict__ stv,
-                              const int* __restrict__ st0, int n_w, int n_det, double2* __restrict__ E_L, double2* __restrict__ E1,
+                              const int* __restrict__ st0, const double2* __restrict__ wdB, const int* __restrict__ stvB,
+                              const int* __restrict__ st0B, int n_w, int n_det, double2* __restrict__ E_L, double2* __restrict__ E1,
                               double2* __restrict__ E_J, double2* __restrict__ E_K, double2* __restrict__ ovlp, int* __restrict__ st_out) {
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= n_w) return;
     double2 num[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)}, den = make_double2(0.0, 0.0);
     for (int d = 0; d < n_det; ++d) {
         const size_t v = (size_t)w * n_det + d;
-        if (stv[v]) continue;
-        const double2 wv = wd[v];
+        if (stv[v] || (stvB && stvB[v])) continue;
+        const double2 wv = wdB ? cmul(wd[v], wdB[v]) : wd[v];
         for (int c = 0; c < 3; ++c) {
             const double2 t1 = cmul(wv, Ev[4 * v + 1 + c]);
             num[c].x += t1.x; num[c].y += t1.y;
@@ -1334,7 +1337,7 @@ __global__ void k_cas_combine(const double2* __restrict__ Ev, const double2* __r
         den.x += wv.x; den.y += wv.y;
     }
     const double m2 = den.x * den.x + den.y * den.y;
-    const bool bad = st0[w] != 0 || !(m2 > 0.0) || isinf(m2);
+    const bool bad = st0[w] != 0 || (st0B && st0B[w] != 0) || !(m2 > 0.0) || isinf(m2);
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     double2 e[3], el = make_double2(0.0, 0.0);
     const double2 id = bad ? make_double2(nan, nan) : crecip(den);
@@ -1595,18 +1598,30 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
 // local energy with a multi-determinant trial by direct summation over determinants (Eq. 12), the
 // determinants' overlaps and Green's functions by SMW updates of the reference (Eq. 20); each (walker, determinant) is a
 // virtual walker of the ordinary Coulomb / exchange kernels (orbital-indexed Theta^d panels, zero where unoccupied).
-lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
-                                  int* walker_status, cudaStream_t stream) {
+lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
+                                  void* ovlp, int* walker_status, cudaStream_t stream) {
     CasPlan& c = *f->cas;
     const int n_orb = f->n_occ[0], n_v = n_w * c.n_det, ldw0 = 2 * c.W0cap;
     launch_s1(f, n_w, f->ops->dPsi[0], n_orb, c.n_ref, phi, c.dA0, c.dSt0, c.dTh0, 0, ldw0, stream);
     k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[0], n_orb, c.dTh0, (double2*)c.dT, f->N, f->N_pad, c.n_ref, c.n_virt, ldw0);
     int* stv = c.mode == 0 ? f->dStatus : c.dStV;
     k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dT, c.dHoles, c.dParts, c.dCoef, c.dSt0, (double2*)c.dG, (double2*)c.dWd,
-                                                  stv, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb);
+                                                  stv, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb, c.has_beta ? 1 : 0);
+    if (c.has_beta) {
+        // unrestricted trial: the beta strings get their own SMW data; their Theta^d panels follow the alpha panels
+        const int n_orb_b = f->n_occ[1];
+        launch_s1(f, n_w, f->ops->dPsi[1], n_orb_b, c.n_ref_b, phi_b, c.dA0B, c.dSt0B, c.dTh0B, 0, ldw0, stream);
+        k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[1], n_orb_b, c.dTh0B, (double2*)c.dTB, f->N, f->N_pad, c.n_ref_b, c.n_virt_b, ldw0);
+        k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dTB, c.dHolesB, c.dPartsB, c.dCoef, c.dSt0B, (double2*)c.dGB,
+                                                      (double2*)c.dWdB, f->dStatus + f->Wcap, n_v, c.n_det, c.max_exc, c.n_ref_b, c.n_virt_b,
+                                                      n_orb_b, 2);
+        dim3 g3b(n_v, n_orb_b, (f->N_pad + 127) / 128);
+        k_cas_theta<<<g3b, 128, 0, stream>>>(c.dTh0B, (const double2*)c.dGB, c.dHolesB, f->dThT, f->N_pad, c.n_ref_b, n_orb_b, c.n_det, c.max_exc,
+                                             ldw0, f->ldw, f->o_base[1]);
+    }
     if (c.mode == 0) {
         dim3 g3(n_v, n_orb, (f->N_pad + 127) / 128);
-        k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw);
+        k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw, 0);
         lo_status st = launch_s3_s5(f, n_v, nullptr, nullptr, nullptr, nullptr, nullptr, c.dEv, stream);
         if (st != LO_OK) return st;
     } else {
@@ -1641,7 +1656,9 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, void*
         k_cas_e1sum<<<(n_v + 127) / 128, 128, 0, stream>>>((const double2*)c.dPart, n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx,
                                                            (const double2*)c.dG, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_orb, n_vtot);
     }
-    k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, stv, c.dSt0, n_w, c.n_det,
+    k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, stv, c.dSt0,
+                                                         c.has_beta ? (const double2*)c.dWdB : nullptr, c.has_beta ? f->dStatus + f->Wcap : nullptr,
+                                                         c.has_beta ? c.dSt0B : nullptr, n_w, c.n_det,
                                                          (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K, (double2*)ovlp, walker_status);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_local_energy_cas: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }

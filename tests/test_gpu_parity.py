@@ -603,3 +603,39 @@ def test_cas_smw_edge_cases(c0):
     with pytest.raises(lo.LoError):
         Fw.set_cas_trial(Tw.n_ref, Tw.holes, Tw.parts, Tw.coef, 2, smw_energy=True)
     Fw.set_cas_trial(Tw.n_ref, Tw.holes, Tw.parts, Tw.coef, 2, smw_energy=False)
+
+
+def test_cas_unrestricted_matches_oracle():
+    """Unrestricted multi-determinant trial (different alpha / beta strings, LO_CAS_DIRECT on an n_spin = 2 factor set)
+    against the oracle's definition on the library's factor sets: every output of every walker, 1e-10 relative."""
+    torch = torch_cuda()
+    xyz, fns = gen.site_geometry(1)
+    P = gen.make_problem_from_geometry(xyz, fns, (9, 7), 300, seed=31)
+    n_det, n_w = 8, 5
+    Ta = gen.make_cas_trial(P, n_virt=3, n_act_occ=3, n_det=n_det, max_exc=2, spin=0)
+    Tb = gen.make_cas_trial(P, n_virt=4, n_act_occ=2, n_det=n_det, max_exc=2, spin=1)
+    F = lo.Factors.setup(P.h, P.L, [Ta.C, Tb.C], 1e-6, device=0, max_walkers=n_w * n_det, gpu_svd=True)
+    F.set_cas_trial(Ta.n_ref, Ta.holes, Ta.parts, Ta.coef, n_w)
+    phis = gen.make_walkers(P, n_w)
+    with pytest.raises(lo.LoError):
+        F.local_energy_cas(torch.from_numpy(phis[0]).cuda())                 # beta strings missing
+    F.set_cas_trial_beta(Tb.n_ref, Tb.holes, Tb.parts)
+    E, st = F.local_energy_cas(torch.from_numpy(phis[0]).cuda(), torch.from_numpy(phis[1]).cuda())
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    assert (st == 0).all()
+    hr = [oracle.half_rotate(P.L, P.h, t.C) for t in (Ta, Tb)]
+    fss = []
+    for s, t in enumerate((Ta, Tb)):
+        n_orb = t.C.shape[1]
+        U, sg, W = F.factor_all(s)
+        pi, pj = oracle.all_pairs(n_orb)
+        fss.append(oracle.make_factor_set(P.N, n_orb, pi, pj, F.ranks(s), U, sg, W))
+    cols = [[t.columns(d) for d in range(n_det)] for t in (Ta, Tb)]
+    for w in range(n_w):
+        Eo = np.array(oracle.local_energy_cas_u([Ta.C, Tb.C], cols, Ta.coef, [a for a, _ in hr], [b for _, b in hr], fss,
+                                                [phis[0][w], phis[1][w]]))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+    with pytest.raises(lo.LoError):
+        F.set_cas_trial(Ta.n_ref, Ta.holes, Ta.parts, Ta.coef, n_w, smw_energy=True)      # SMW-energy mode is closed-shell only

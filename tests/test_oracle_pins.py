@@ -405,3 +405,30 @@ def test_cas_single_determinant_and_bruteforce(c0, c0_walkers):
         den += T.coef[d] * det * det
     assert abs(E[0] - num / den) <= 1e-10 * abs(E[0]) and abs(Ex[0] - num / den) <= 1e-10 * abs(E[0])
     assert abs(E[0] - single[0]) > 1e-6 * abs(E[0])          # the expansion does change the energy
+
+
+def test_cas_unrestricted_pins(c0, c0_walkers):
+    """Unrestricted multi-determinant oracle: identical alpha/beta orbitals, strings and walkers reproduce the
+    closed-shell multi-determinant energy; one determinant reproduces the unrestricted single-determinant energy."""
+    T = gen.make_cas_trial(c0, n_virt=3, n_act_occ=3, n_det=6, max_exc=2)
+    Lbar, hbar = oracle.half_rotate(c0.L, c0.h, T.C)
+    fs = oracle.own_factors(Lbar, 0.0)
+    cols = [T.columns(d) for d in range(T.n_det)]
+    phi = c0_walkers[0][2]
+    Ec = oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi)
+    Eu = oracle.local_energy_cas_u([T.C, T.C], [cols, cols], T.coef, [Lbar, Lbar], [hbar, hbar], [fs, fs], [phi, phi])
+    assert np.abs(np.array(Eu) - np.array(Ec)).max() <= 1e-11 * abs(Ec[0])
+    # different strings and walkers per spin, one determinant: the unrestricted single-determinant energy
+    xyz, fns = gen.site_geometry(0)
+    P = gen.make_problem_from_geometry(xyz, fns, (4, 3), 48, seed=5)
+    phis = gen.make_walkers(P, 2)
+    Ta, Tb = gen.make_cas_trial(P, 2, 2, 4, 2, spin=0), gen.make_cas_trial(P, 2, 2, 4, 2, spin=1)
+    hr = [oracle.half_rotate(P.L, P.h, t.C) for t in (Ta, Tb)]
+    fss = [oracle.own_factors(a, 0.0) for a, _ in hr]
+    colsu = [[Ta.columns(d) for d in range(4)], [Tb.columns(d) for d in range(4)]]
+    E1 = oracle.local_energy_cas_u([Ta.C, Tb.C], [colsu[0][:1], colsu[1][:1]], Ta.coef[:1], [a for a, _ in hr], [b for _, b in hr], fss,
+                                   [phis[0][1], phis[1][1]])
+    Es = oracle.local_energy_exact(P.h, P.L, P.psi, [phis[0][1], phis[1][1]], "cholesky")
+    assert np.abs(np.array(E1[:4]) - np.array(Es)).max() <= 1e-10 * abs(Es[0])
+    Eall = oracle.local_energy_cas_u([Ta.C, Tb.C], colsu, Ta.coef, [a for a, _ in hr], [b for _, b in hr], fss, [phis[0][1], phis[1][1]])
+    assert abs(Eall[0] - Es[0]) > 1e-6 * abs(Es[0])
