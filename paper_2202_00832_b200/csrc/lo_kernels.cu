@@ -1,13 +1,18 @@
 // lo_kernels.cu -- the hot path of lo_local_energy (steps S1-S5 of SURVEY.md 8(a)), hand-written for sm_100a.
 //
-//   k_overlap   A_w = Psi^T Phi_w
-//   k_inverse   A_w^-1 by in-place Gauss-Jordan with partial pivoting, in shared memory (global fallback for big O)
-//   k_theta     Theta_w = Phi_w A_w^-1 (Eq. 15), written as Theta^T panels [o][2w+c][p]
-//   k_coulomb   X = [Lbar; hbar] . Theta   real FP64 GEMM on the DMMA pipe, split-K partials  (Eq. 16 Coulomb part)
+//   k_overlap   A_w = Psi^T Phi_w   real x complex GEMM on the DMMA pipe
+//   k_inverse   A_w^-1 by in-place Gauss-Jordan with partial pivoting, in shared memory (global fallback for big O);
+//               k_inverse_reg: register-resident variant for O <= 48
+//   k_theta     Theta_w = Phi_w A_w^-1 (Eq. 15) as one real GEMM on the DMMA pipe, written as Theta^T panels
+//               [o][2w+c][p]
+//   k_coulomb   X = [Lbar; hbar] . Theta   real FP64 GEMM on the DMMA pipe, split-K partials  (Eq. 16 Coulomb part);
+//               also the propagator GEMM B = Lt . x (NEXT-1, with k_pack_x)
 //   k_ej        X = sum of partials, E_J partial sums of X^2 (complex square), E1 from the hbar row
 //   k_exchange  grouped variable-rank dual GEMM a = U Theta_j, b = W Theta_i with fused weight * a * b reduction
-//               (Eq. 19/22 exchange part)
+//               (Eq. 19/22 exchange part); <true>: also the compressed Coulomb projections (NEXT-3)
 //   k_finalize  E_K = sum of CTA partials, E_L = E1 + E_J + E_K, NaN for singular walkers
+//   k_cas_*     multi-determinant trial (NEXT-2): SMW overlaps / Green's functions (k_cas_T, k_cas_coef, k_cas_theta),
+//               rearranged SMW energy (k_cas_pairs, k_cas_H, k_cas_energy, k_cas_e1sum), k_cas_combine
 //
 // FP64 on sm_100a has no tcgen05 path; the FP64 tensor instruction is the warp-level DMMA.8x8x4
 // (mma.sync.aligned.m8n8k4.f64), measured at 37.1 TFLOP/s on this B200 (same rate as the DFMA pipe, but one
