@@ -81,6 +81,16 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* tm) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
 }
+// Ampere-style asynchronous copies (LDGSTS) for the S1 staging; src_size 0 zero-fills the destination
+__device__ __forceinline__ void cp_async8(void* dst, const void* src, bool valid) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 8 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* dst, const void* src, bool valid) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 16 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 __device__ __forceinline__ double lds_f64(uint32_t addr) {
     double v;
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
@@ -112,8 +122,7 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
                                                  int N, int O, int ldpsi) {
     extern __shared__ __align__(16) double sm[];
     const int LDB = ov_ldb(O), nf0 = blockIdx.z * OV_NFB, NF = min((2 * O + 7) / 8 - nf0, OV_NFB), c0 = nf0 * 8;
-    double* As = sm;                   // [OV_PC][OV_LDA]
-    double* Bs = sm + OV_PC * OV_LDA;  // [OV_PC][LDB]
+    const int buf_doubles = OV_PC * (OV_LDA + LDB);     // two buffers: [OV_PC][OV_LDA] Psi rows, [OV_PC][LDB] Phi rows
     const int i0 = blockIdx.x * (MFB * 8), w = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     const double* phw = reinterpret_cast<const double*>(phi + (size_t)w * N * O);
     const int O2 = 2 * O, ncb = NF * 8;
@@ -122,15 +131,31 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
     for (int a = 0; a < MFB; ++a)
 #pragma unroll
         for (int b = 0; b < NFW; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
-    for (int p0 = 0; p0 < N; p0 += OV_PC) {
-        __syncthreads();
+    // asynchronous staging (cp.async, zero fill outside the matrix): chunk k+1 is in flight while chunk k feeds the MMAs
+    auto issue = [&](int p0, double* As, double* Bs) {
         for (int e = tid; e < OV_PC * (MFB * 8); e += 256) {
             const int pp = e / (MFB * 8), c = e - pp * (MFB * 8), pg = p0 + pp;
-            As[pp * OV_LDA + c] = (pg < N && i0 + c < O) ? psi[(size_t)pg * ldpsi + i0 + c] : 0.0;
+            const bool ok = pg < N && i0 + c < O;
+            cp_async8(As + pp * OV_LDA + c, ok ? psi + (size_t)pg * ldpsi + i0 + c : psi, ok);
         }
-        for (int e = tid; e < OV_PC * ncb; e += 256) {
-            const int pp = e / ncb, c = e - pp * ncb, pg = p0 + pp;
-            Bs[pp * LDB + c] = (pg < N && c0 + c < O2) ? phw[(size_t)pg * O2 + c0 + c] : 0.0;
+        for (int e = tid; e < OV_PC * (ncb / 2); e += 256) {
+            const int pp = e / (ncb / 2), c = 2 * (e - pp * (ncb / 2)), pg = p0 + pp;
+            const bool ok = pg < N && c0 + c < O2;
+            cp_async16(Bs + pp * LDB + c, ok ? phw + (size_t)pg * O2 + c0 + c : phw, ok);
+        }
+        cp_async_commit();
+    };
+    issue(0, sm, sm + OV_PC * OV_LDA);
+    int kbuf = 0;
+    for (int p0 = 0; p0 < N; p0 += OV_PC, kbuf ^= 1) {
+        const double* As = sm + kbuf * buf_doubles;
+        const double* Bs = As + OV_PC * OV_LDA;
+        if (p0 + OV_PC < N) {
+            double* nb = sm + (kbuf ^ 1) * buf_doubles;
+            issue(p0 + OV_PC, nb, nb + OV_PC * OV_LDA);
+            cp_async_wait<1>();
+        } else {
+            cp_async_wait<0>();
         }
         __syncthreads();
 #pragma unroll
@@ -148,6 +173,7 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
 #pragma unroll
                 for (int j = 0; j < NFW; ++j) mma884(acc[mf][j][0], acc[mf][j][1], a[mf], b[j]);
         }
+        __syncthreads();      // the buffer is refilled by the issue of the next iteration
     }
 #pragma unroll
     for (int mf = 0; mf < MFB; ++mf)
@@ -440,8 +466,8 @@ template <int MFB>
 __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, const double2* __restrict__ Ainv, double* __restrict__ thT,
                                                int N, int N_pad, int O, int o_base, int ldw) {
     extern __shared__ __align__(16) double sm[];
-    double* Bt = sm;                       // [MFB*8][TH_LD]
-    double* Ph = sm + MFB * 8 * TH_LD;     // [64][TH_LD]
+    constexpr int BUF = (MFB * 8 + 64) * TH_LD;      // per buffer: Bt [MFB*8][TH_LD] then Ph [64][TH_LD]; two buffers
+    constexpr int NREG = (MFB * 4 * (TH_KC / 2) + 255) / 256;
     const int p0 = blockIdx.x * 64, m0 = blockIdx.y * MFB * 8, w = blockIdx.z;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     const int O2 = 2 * O, ib0 = m0 / 2, ni = MFB * 4;
@@ -450,22 +476,50 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
     double acc[MFB][2];
 #pragma unroll
     for (int a = 0; a < MFB; ++a) acc[a][0] = acc[a][1] = 0.0;
-    for (int k0 = 0; k0 < O2; k0 += TH_KC) {
-        __syncthreads();
-        // Bt chunk: rows (i,c') of this M block, columns (j,c) with 2j+c in [k0, k0+TH_KC)
-        for (int e = tid; e < (TH_KC / 2) * ni; e += 256) {
-            const int jj = e / ni, ii = e - jj * ni, i = ib0 + ii, j = k0 / 2 + jj;
-            double2 v = make_double2(0.0, 0.0);
-            if (i < O && j < O) v = Aw[(size_t)j * O + i];
-            double* r0 = Bt + (2 * ii) * TH_LD + 2 * jj;
-            r0[0] = v.x; r0[1] = -v.y;
-            r0[TH_LD] = v.y; r0[TH_LD + 1] = v.x;
+    // Pipeline over the K chunks: the Phi rows of chunk k+1 arrive by cp.async and the A^-1 entries of chunk k+1 sit in
+    // registers (loads in flight) while the MMAs of chunk k run; they are expanded into the 2x2 real blocks of Bt afterwards.
+    auto issue_phi = [&](int k0, double* Ph) {
+        for (int e = tid; e < 64 * (TH_KC / 2); e += 256) {
+            const int pp = e / (TH_KC / 2), k = 2 * (e - pp * (TH_KC / 2)), pg = p0 + pp, kk = k0 + k;
+            const bool ok = pg < N && kk < O2;
+            cp_async16(Ph + pp * TH_LD + k, ok ? phw + (size_t)pg * O2 + kk : phw, ok);
         }
-        for (int e = tid; e < 64 * TH_KC; e += 256) {
-            const int pp = e / TH_KC, k = e - pp * TH_KC, pg = p0 + pp, kk = k0 + k;
-            Ph[pp * TH_LD + k] = (pg < N && kk < O2) ? phw[(size_t)pg * O2 + kk] : 0.0;
+        cp_async_commit();
+    };
+    auto load_ainv = [&](int k0, double2 (&v)[NREG]) {
+#pragma unroll
+        for (int r = 0; r < NREG; ++r) {
+            const int e = tid + 256 * r, jj = e / ni, ii = e - jj * ni, i = ib0 + ii, j = k0 / 2 + jj;
+            v[r] = (e < (TH_KC / 2) * ni && i < O && j < O) ? Aw[(size_t)j * O + i] : make_double2(0.0, 0.0);
         }
-        __syncthreads();
+    };
+    auto store_bt = [&](double* Bt, const double2 (&v)[NREG]) {
+#pragma unroll
+        for (int r = 0; r < NREG; ++r) {
+            const int e = tid + 256 * r, jj = e / ni, ii = e - jj * ni;
+            if (e < (TH_KC / 2) * ni) {
+                double* r0 = Bt + (2 * ii) * TH_LD + 2 * jj;
+                r0[0] = v[r].x; r0[1] = -v[r].y;
+                r0[TH_LD] = v[r].y; r0[TH_LD + 1] = v[r].x;
+            }
+        }
+    };
+    double2 av[NREG];
+    issue_phi(0, sm + MFB * 8 * TH_LD);
+    load_ainv(0, av);
+    store_bt(sm, av);
+    cp_async_wait<0>();
+    __syncthreads();
+    int kbuf = 0;
+    for (int k0 = 0; k0 < O2; k0 += TH_KC, kbuf ^= 1) {
+        const double* Bt = sm + kbuf * BUF;
+        const double* Ph = Bt + MFB * 8 * TH_LD;
+        double* nBt = sm + (kbuf ^ 1) * BUF;
+        const bool more = k0 + TH_KC < O2;
+        if (more) {
+            issue_phi(k0 + TH_KC, nBt + MFB * 8 * TH_LD);
+            load_ainv(k0 + TH_KC, av);
+        }
         const int nks = min(TH_KC / 4, (O2 - k0 + 3) / 4);      // K tail: whole k-steps of zeros are skipped (uniform)
 #pragma unroll
         for (int ks = 0; ks < TH_KC / 4; ++ks) {
@@ -477,6 +531,11 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
 #pragma unroll
             for (int mf = 0; mf < MFB; ++mf) mma884(acc[mf][0], acc[mf][1], a[mf], b);
         }
+        if (more) {
+            store_bt(nBt, av);
+            cp_async_wait<0>();
+        }
+        __syncthreads();
     }
     const int p = p0 + warp * 8 + 2 * t;
     if (p < N_pad) {
@@ -1467,13 +1526,13 @@ lo_status configure_kernels() {
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     for (int m = 1; m <= 16; ++m) {
-        e = cudaFuncSetAttribute((const void*)th_fn(m), cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        e = cudaFuncSetAttribute((const void*)th_fn(m), cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
         if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)th_fn(m), cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_theta): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     }
     for (int m = 1; m <= 5; ++m)
         for (int n = 1; n <= 8; ++n) {
-            e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
             if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributePreferredSharedMemoryCarveout, 100);
             if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_overlap): ") + cudaGetErrorString(e)); return LO_ECUDA; }
         }
@@ -1496,7 +1555,7 @@ void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, cons
         const int NF = (2 * O + 7) / 8, nfw = (std::min(NF, OV_NFB) + 7) / 8;
         const int MF = (O + 7) / 8, n_mb = (MF + 4) / 5, mfb = (MF + n_mb - 1) / n_mb;     // row blocks of <= 5 fragments
         dim3 grid(n_mb, n_w, (NF + OV_NFB - 1) / OV_NFB);
-        const size_t smem = (size_t)OV_PC * (OV_LDA + ov_ldb(O)) * 8;
+        const size_t smem = (size_t)2 * OV_PC * (OV_LDA + ov_ldb(O)) * 8;      // two staging buffers
         ov_fn(mfb, nfw)<<<grid, 256, smem, stream>>>(psi, (const double2*)phi, (double2*)dA, N, O, ldpsi);
     }
     {
@@ -1519,7 +1578,7 @@ void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, cons
         Timer tm(f, stream, LO_K_THETA);
         const int MF = (2 * O + 7) / 8, n_mb = (MF + 15) / 16, mfb = (MF + n_mb - 1) / n_mb;
         dim3 grid((N_pad + 63) / 64, n_mb, n_w);
-        th_fn(mfb)<<<grid, 256, (size_t)(mfb * 8 + 64) * TH_LD * 8, stream>>>((const double2*)phi, (const double2*)dA, thT, N, N_pad, O, o_base, ldw_t);
+        th_fn(mfb)<<<grid, 256, (size_t)2 * (mfb * 8 + 64) * TH_LD * 8, stream>>>((const double2*)phi, (const double2*)dA, thT, N, N_pad, O, o_base, ldw_t);
     }
 }
 
