@@ -114,7 +114,7 @@ __device__ __forceinline__ uint32_t frag_off(int g, int t, int s) {
 // a leading dimension = 4 (mod 16) doubles keeps the 16 lanes of a half-warp on distinct 8-byte banks.
 constexpr int OV_PC = 32;
 constexpr int OV_LDA = 52;   // >= 5 row fragments (40 columns), = 4 (mod 16)
-constexpr int OV_NFB = 64;   // column fragments per CTA (grid.z blocks of 512 real columns = 256 orbitals)
+constexpr int OV_NFB = 40;   // column fragments per CTA (grid.z blocks of 320 real columns = 160 orbitals): two staging buffers stay < 200 KB
 __host__ __device__ inline int ov_ldb(int O) { int nf8 = min((2 * O + 7) / 8, OV_NFB) * 8; return nf8 + ((4 - nf8 % 16) + 16) % 16; }
 
 template <int MFB, int NFW>

@@ -639,3 +639,26 @@ def test_cas_unrestricted_matches_oracle():
         assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
     with pytest.raises(lo.LoError):
         F.set_cas_trial(Ta.n_ref, Ta.holes, Ta.parts, Ta.coef, n_w, smw_energy=True)      # SMW-energy mode is closed-shell only
+
+
+def test_large_occupation_s1_path():
+    """More occupied orbitals than one column block of the overlap kernel holds (O = 200 > 160) and than the
+    shared-memory Gauss-Jordan holds (global-workspace variant): Theta against the oracle's LU, E1 / E_J against the
+    oracle's Cholesky route.  The threshold truncates every pair away (the pair SVDs still run: 20 100 pairs)."""
+    torch = torch_cuda()
+    xyz, fns = gen.site_geometry(0)
+    P = gen.make_problem_from_geometry(xyz, [52] * 4, (200,), 8, seed=77)
+    n_w = 3
+    phis = gen.make_walkers(P, n_w)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e9, device=0, max_walkers=n_w, gpu_svd=True)
+    assert F.info().sum_rank[0] == 0
+    Eg, st = gpu_energy(F, phis)
+    assert (st == 0).all()
+    th_g = F.theta_host(0, n_w)
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, P.psi[0])
+    for w in range(n_w):
+        th, _, s = oracle.theta(P.psi[0], phis[0][w])
+        assert s == 0 and np.abs(th_g[w] - th).max() <= 1e-10 * np.abs(th).max()
+        e1, ej = oracle.onebody_coulomb([Lbar], [hbar], [th])
+        scale = abs(e1 + ej)
+        assert abs(Eg[w, 1] - e1) <= TOL * scale and abs(Eg[w, 2] - ej) <= TOL * scale and Eg[w, 3] == 0
