@@ -712,6 +712,7 @@ static lo_status check_call(const lo_factors* f, int n_w, const void* phi_a, con
     if (!f) { set_error("lo_local_energy: factors is NULL"); return LO_EINVAL; }
     if (f->device < 0) { set_error("lo_local_energy: factor set was built without a device (device < 0); there is no CPU path"); return LO_ECUDA; }
     if (n_w <= 0 || n_w > f->max_walkers) { set_error("lo_local_energy: n_w out of range (1..max_walkers)"); return LO_EINVAL; }
+    if (n_w > 65535) { set_error("lo_local_energy: at most 65535 walkers per call (grid dimension of the S1 kernels); split the batch"); return LO_EINVAL; }
     if (!phi_a || (f->n_spin == 2 && !phi_b)) { set_error("lo_local_energy: phi is NULL"); return LO_EINVAL; }
     if (((uintptr_t)phi_a & 15) || ((uintptr_t)phi_b & 15)) { set_error("lo_local_energy: phi must be 16-byte aligned"); return LO_EINVAL; }
     return LO_OK;
@@ -950,7 +951,7 @@ lo_status lo_local_energy_cas(const lo_factors* fc, int n_w, const void* phi, co
     }
     if (fc->device < 0) { set_error("lo_local_energy_cas: no device; there is no CPU path"); return LO_ECUDA; }
     if (!fc->cas) { set_error("lo_local_energy_cas: call lo_set_cas_trial first"); return LO_EINVAL; }
-    if (n_w <= 0 || n_w > fc->cas->max_real) { set_error("lo_local_energy_cas: n_w out of range (1..max_real_walkers)"); return LO_EINVAL; }
+    if (n_w <= 0 || n_w > fc->cas->max_real || n_w > 65535) { set_error("lo_local_energy_cas: n_w out of range (1..min(max_real_walkers, 65535))"); return LO_EINVAL; }
     if (((uintptr_t)phi & 15) || ((uintptr_t)E_L & 15) || ((uintptr_t)E1 & 15) || ((uintptr_t)E_J & 15) || ((uintptr_t)E_K & 15) || ((uintptr_t)ovlp & 15)) {
         set_error("lo_local_energy_cas: pointers must be 16-byte aligned");
         return LO_EINVAL;
