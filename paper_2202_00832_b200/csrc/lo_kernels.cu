@@ -489,18 +489,19 @@ __global__ void __launch_bounds__(256) k_theta(const double2* __restrict__ phi, 
     auto load_ainv = [&](int k0, double2 (&v)[NREG]) {
 #pragma unroll
         for (int r = 0; r < NREG; ++r) {
-            const int e = tid + 256 * r, jj = e / ni, ii = e - jj * ni, i = ib0 + ii, j = k0 / 2 + jj;
+            // consecutive threads take consecutive j of one i: their 128-bit stores below fill one Bt row contiguously
+            const int e = tid + 256 * r, ii = e / (TH_KC / 2), jj = e - ii * (TH_KC / 2), i = ib0 + ii, j = k0 / 2 + jj;
             v[r] = (e < (TH_KC / 2) * ni && i < O && j < O) ? Aw[(size_t)j * O + i] : make_double2(0.0, 0.0);
         }
     };
     auto store_bt = [&](double* Bt, const double2 (&v)[NREG]) {
 #pragma unroll
         for (int r = 0; r < NREG; ++r) {
-            const int e = tid + 256 * r, jj = e / ni, ii = e - jj * ni;
+            const int e = tid + 256 * r, ii = e / (TH_KC / 2), jj = e - ii * (TH_KC / 2);
             if (e < (TH_KC / 2) * ni) {
                 double* r0 = Bt + (2 * ii) * TH_LD + 2 * jj;
-                r0[0] = v[r].x; r0[1] = -v[r].y;
-                r0[TH_LD] = v[r].y; r0[TH_LD + 1] = v[r].x;
+                *reinterpret_cast<double2*>(r0) = make_double2(v[r].x, -v[r].y);
+                *reinterpret_cast<double2*>(r0 + TH_LD) = make_double2(v[r].y, v[r].x);
             }
         }
     };
