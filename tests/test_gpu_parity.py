@@ -662,3 +662,22 @@ def test_large_occupation_s1_path():
         e1, ej = oracle.onebody_coulomb([Lbar], [hbar], [th])
         scale = abs(e1 + ej)
         assert abs(Eg[w, 1] - e1) <= TOL * scale and abs(Eg[w, 2] - ej) <= TOL * scale and Eg[w, 3] == 0
+
+
+@pytest.mark.parametrize("smw", [False, True])
+def test_cas_singular_reference_overlap_is_flagged(c0, smw):
+    """A walker with a zero orbital has a singular reference overlap: status 1 and NaN energies for that walker only,
+    in both multi-determinant modes; the other walkers are unaffected."""
+    torch = torch_cuda()
+    T = gen.make_cas_trial(c0, n_virt=3, n_act_occ=3, n_det=6, max_exc=2)
+    F = lo.Factors.setup(c0.h, c0.L, [T.C], 1e-8, device=0, max_walkers=24, gpu_svd=True)
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, 4, smw_energy=smw)
+    phi = gen.make_walkers(c0, 4)[0].copy()
+    E_ok, st_ok = F.local_energy_cas(torch.from_numpy(phi).cuda())
+    phi[2, :, 1] = 0.0
+    E, st = F.local_energy_cas(torch.from_numpy(phi).cuda())
+    torch.cuda.synchronize()
+    E, st, E_ok = E.cpu().numpy().T, st.cpu().numpy(), E_ok.cpu().numpy().T
+    assert st.tolist() == [0, 0, 1, 0] and np.isnan(E[2]).all()
+    ok = [0, 1, 3]
+    assert np.array_equal(E[ok], E_ok[ok])
