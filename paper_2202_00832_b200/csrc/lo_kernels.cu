@@ -751,12 +751,12 @@ __device__ __forceinline__ void ex_kloop(int KT, uint32_t sbase, uint32_t full, 
     }
 }
 
-template <bool COUL>
+template <bool COUL, bool RAGGED>   // RAGGED: the batch is not a multiple of 64 walkers (warps without walkers skip their MMAs)
 __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
                                                      const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
                                                      const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
                                                      const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
-                                                     double* __restrict__ ekpart, double* __restrict__ ejpart, int Wcap) {
+                                                     double* __restrict__ ekpart, double* __restrict__ ejpart, int Wcap, int n_w) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
@@ -846,6 +846,17 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
         }
         mbar_wait(full + 8 * cslot, cphase);            // first stage of the item: its descriptor is in the ring now
         const ExTile tile = ring[n % EX_RING];
+        if (RAGGED && nb * WALKER_TILE + cw * 8 >= n_w) {
+            // none of this warp's 8 walkers exists (ragged last block, batches below 64 walkers): no MMAs, only hand the
+            // stages back; the warps that do have walkers then get the tensor pipe of their scheduler to themselves
+            for (int kt = 0; kt < KT; ++kt) {
+                if (kt) mbar_wait(full + 8 * cslot, cphase);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + 8 * cslot);
+                if (++cslot == EX_STAGES) { cslot = 0; cphase ^= 1; }
+            }
+            continue;
+        }
 #define LO_EX_CASE(NF_) ex_kloop<NF_, COUL, MFMAX>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB, accC, accD)
         if constexpr (COUL) {
             switch (tile.nfrag) {                       // warp- and CTA-uniform; COUL tiles have at most 4 fragments
@@ -1521,8 +1532,10 @@ lo_status configure_kernels() {
     cudaError_t e;
     e = cudaFuncSetAttribute(k_coulomb, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_coulomb): ") + cudaGetErrorString(e)); return LO_ECUDA; }
-    e = cudaFuncSetAttribute(k_exchange<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    e = cudaFuncSetAttribute(k_exchange<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_exchange): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
@@ -1619,12 +1632,15 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         const bool coul = f->coulomb_lo != 0;
         long long items = (coul ? f->n_tiles4 : f->n_tiles) * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        if (coul)
-            k_exchange<true><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, f->dTiles4, items, NB, N_pad,
-                                                                ldw, f->dEKpart, f->dEJLpart, Wcap);
-        else
-            k_exchange<false><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, f->dTiles, items, NB, N_pad,
-                                                                 ldw, f->dEKpart, nullptr, Wcap);
+        const bool ragged = n_w % WALKER_TILE != 0;
+#define LO_EX_LAUNCH(C_, R_, TILES_, EJ_)                                                                                              \
+    k_exchange<C_, R_><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, TILES_, items, NB, N_pad, ldw, \
+                                                          f->dEKpart, EJ_, Wcap, n_w)
+        if (coul && ragged) LO_EX_LAUNCH(true, true, f->dTiles4, f->dEJLpart);
+        else if (coul) LO_EX_LAUNCH(true, false, f->dTiles4, f->dEJLpart);
+        else if (ragged) LO_EX_LAUNCH(false, true, f->dTiles, nullptr);
+        else LO_EX_LAUNCH(false, false, f->dTiles, nullptr);
+#undef LO_EX_LAUNCH
     }
     // ---- S5
     {
