@@ -337,6 +337,7 @@ lo_status alloc_workspace(lo_factors* f) {
     CK(cudaStreamCreateWithFlags(&f->copyStream, cudaStreamNonBlocking));
     for (int c = 0; c < LO_HOST_CHUNKS; ++c) CK(cudaEventCreateWithFlags(&f->evCopy[c], cudaEventDisableTiming));
     lo_status st = make_tmap(&f->tmTheta, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 128);
+    if (st == LO_OK) st = make_tmap(&f->tmTheta32, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 32);
     if (st == LO_OK && f->dXT) st = make_tmap(&f->tmXT, f->dXT, (unsigned long long)f->ops->Xk_pad, ldw, 128);
     if (st != LO_OK) return st;
     return configure_kernels();

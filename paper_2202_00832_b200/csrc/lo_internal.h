@@ -135,6 +135,7 @@ struct lo_factors {
     lo::ExTile* dTiles4 = nullptr;
     CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
     CUtensorMap tmU8, tmW8;              // same arrays, boxes 8 x 16 (one row fragment): tiles shorter than 64 rows
+    CUtensorMap tmTheta32;               // Theta^T panels with a 32 x 16 box (16 walkers): narrow-batch exchange
     std::shared_ptr<lo::SharedOps> ops;
     // workspace
     double* dThT = nullptr;       // [O_tot][ldw][N_pad]

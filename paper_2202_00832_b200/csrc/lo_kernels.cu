@@ -928,6 +928,160 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
     }
 }
 
+// ---- narrow-batch exchange (n_w <= 32, e.g. the paper's 16 walkers per GPU): a 64-walker column block
+// would leave 6 of the 8 consumer warps without walkers, so here a work item is (row tile, block of 16 walkers = 32 real
+// columns) and the warps split the ROW fragments instead: warp cw owns column half cw & 1 (8 walkers) and fragments
+// cw >> 1 and 4 + (cw >> 1).  Same TMA/mbarrier pipeline (6 stages of 24 KB); the four fragment groups of a column half
+// are added in a fixed order through shared memory.
+constexpr int EN_STAGES = 6;
+constexpr int EN_STAGE_BYTES = (2 * EX_BM + 2 * 32) * 128;
+constexpr int EN_SMEM = EN_STAGES * EN_STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 4 * 32 * 8;
+
+__global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
+                                                            const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
+                                                            const __grid_constant__ CUtensorMap tmT32, const double* __restrict__ wgt,
+                                                            const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
+                                                            double* __restrict__ ekpart, int Wcap) {
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
+    const uint32_t full = sbase + EN_STAGES * EN_STAGE_BYTES, empty = full + 8 * EN_STAGES;
+    ExTile* ring = reinterpret_cast<ExTile*>(sgen + EN_STAGES * EN_STAGE_BYTES + 128);
+    double* red = reinterpret_cast<double*>(sgen + EN_STAGES * EN_STAGE_BYTES + 128 + EX_RING * 16);      // [4 fragment groups][32 columns]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int KT = N_pad / KTILE;
+    double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
+    for (int i = tid; i < 2 * Wcap; i += 384) mypart[i] = 0.0;
+    if (tid == 0) {
+        prefetch_tmap(&tmU);
+        prefetch_tmap(&tmW);
+        prefetch_tmap(&tmU8);
+        prefetch_tmap(&tmW8);
+        prefetch_tmap(&tmT32);
+        for (int i = 0; i < EN_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
+        fence_barrier_init();
+    }
+    __syncthreads();
+    if (warp < 4) {
+        reg_dec_producer();
+        if (warp == 0 && lane == 0) {
+            int slot = 0, n = 0;
+            uint32_t phase = 0;
+            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
+                const ExTile tile = tiles[q / NB];
+                const int nb = (int)(q % NB);
+                const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + 2 * 32) * 128;
+                for (int kt = 0; kt < KT; ++kt) {
+                    mbar_wait(empty + 8 * slot, phase ^ 1);
+                    if (kt == 0) ring[n % EX_RING] = tile;
+                    const uint32_t st = sbase + slot * EN_STAGE_BYTES, bar = full + 8 * slot;
+                    const int k0 = kt * KTILE;
+                    mbar_expect_tx(bar, tx);
+                    if (tile.nfrag == EX_BM / 8) {
+                        tma_load_2d(st, &tmU, k0, tile.row0, bar);
+                        tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
+                    } else {
+                        for (int fr = 0; fr < tile.nfrag; ++fr) {
+                            tma_load_2d(st + fr * 1024, &tmU8, k0, tile.row0 + fr * 8, bar);
+                            tma_load_2d(st + EX_BM * 128 + fr * 1024, &tmW8, k0, tile.row0 + fr * 8, bar);
+                        }
+                    }
+                    tma_load_2d(st + 2 * EX_BM * 128, &tmT32, k0, tile.pj * ldw + nb * 32, bar);
+                    tma_load_2d(st + 2 * EX_BM * 128 + 32 * 128, &tmT32, k0, tile.pi * ldw + nb * 32, bar);
+                    if (++slot == EN_STAGES) { slot = 0; phase ^= 1; }
+                }
+            }
+        }
+        return;
+    }
+    reg_inc_consumer();
+    const int cw = warp - 4, g = lane >> 2, t = lane & 3, ctid = tid - 128;
+    const int cg = cw & 1, fr0 = cw >> 1, fr1 = 4 + (cw >> 1);
+    double accA[2][2][2], accB[2][2][2];
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) accA[j][b][0] = accA[j][b][1] = accB[j][b][0] = accB[j][b][1] = 0.0;
+    uint32_t xo[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
+    const uint32_t u_row0 = (uint32_t)(fr0 * 8 + g) * 128, u_row1 = (uint32_t)(fr1 * 8 + g) * 128;
+    const uint32_t tj_row = (uint32_t)(2 * EX_BM + cg * 16 + g) * 128, ti_row = tj_row + 32 * 128;
+    int cslot = 0, n = 0;
+    uint32_t cphase = 0;
+    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
+        const int nb = (int)(q % NB);
+        mbar_wait(full + 8 * cslot, cphase);
+        const ExTile tile = ring[n % EX_RING];
+        const int nu = (fr0 < tile.nfrag ? 1 : 0) + (fr1 < tile.nfrag ? 1 : 0);     // warp-uniform
+        for (int kt = 0; kt < KT; ++kt) {
+            if (kt) mbar_wait(full + 8 * cslot, cphase);
+            const uint32_t st = sbase + cslot * EN_STAGE_BYTES;
+            if (nu > 0) {
+#pragma unroll
+                for (int ks = 0; ks < KTILE / 4; ++ks) {
+                    double a[2], w[2], bj[2], bi[2];
+                    a[0] = lds_f64(st + u_row0 + xo[ks]);
+                    w[0] = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
+                    if (nu == 2) {
+                        a[1] = lds_f64(st + u_row1 + xo[ks]);
+                        w[1] = lds_f64(st + u_row1 + EX_BM * 128 + xo[ks]);
+                    }
+#pragma unroll
+                    for (int nf = 0; nf < 2; ++nf) {
+                        bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
+                        bi[nf] = lds_f64(st + ti_row + nf * 1024 + xo[ks]);
+                    }
+                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
+#pragma unroll
+                    for (int nf = 0; nf < 2; ++nf) {
+                        mma884(accA[0][nf][0], accA[0][nf][1], a[0], bj[nf]);
+                        mma884(accB[0][nf][0], accB[0][nf][1], w[0], bi[nf]);
+                    }
+                    if (nu == 2) {
+#pragma unroll
+                        for (int nf = 0; nf < 2; ++nf) {
+                            mma884(accA[1][nf][0], accA[1][nf][1], a[1], bj[nf]);
+                            mma884(accB[1][nf][0], accB[1][nf][1], w[1], bi[nf]);
+                        }
+                    }
+                }
+            } else {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + 8 * cslot);
+            }
+            if (++cslot == EN_STAGES) { cslot = 0; cphase ^= 1; }
+        }
+        double e[2][2];
+#pragma unroll
+        for (int nf = 0; nf < 2; ++nf) e[nf][0] = e[nf][1] = 0.0;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const double wv = j < nu ? __ldg(wgt + tile.row0 + (j == 0 ? fr0 : fr1) * 8 + g) : 0.0;
+#pragma unroll
+            for (int nf = 0; nf < 2; ++nf) {
+                const double ar = accA[j][nf][0], ai = accA[j][nf][1], br = accB[j][nf][0], bi = accB[j][nf][1];
+                e[nf][0] = fma(wv, ar * br - ai * bi, e[nf][0]);
+                e[nf][1] = fma(wv, ar * bi + ai * br, e[nf][1]);
+                accA[j][nf][0] = accA[j][nf][1] = accB[j][nf][0] = accB[j][nf][1] = 0.0;
+            }
+        }
+#pragma unroll
+        for (int nf = 0; nf < 2; ++nf)
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                double v = e[nf][c];
+                v += __shfl_xor_sync(0xffffffffu, v, 4);
+                v += __shfl_xor_sync(0xffffffffu, v, 8);
+                v += __shfl_xor_sync(0xffffffffu, v, 16);
+                if (g == 0) red[(cw >> 1) * 32 + cg * 16 + nf * 8 + 2 * t + c] = v;
+            }
+        bar_sync_consumers();
+        if (ctid < 32) mypart[(size_t)nb * 32 + ctid] += (red[ctid] + red[32 + ctid]) + (red[64 + ctid] + red[96 + ctid]);
+        bar_sync_consumers();
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ NEXT-1: propagator
 // x[w][g] (complex128, walker-major) -> XT[2w + c][g] (K-major real operand of the propagator GEMM); the K padding
 // columns g >= n_chol stay zero from allocation.  grid (ceil(n_chol/128), n_w), block 128.
@@ -1536,6 +1690,7 @@ lo_status configure_kernels() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, EN_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_exchange): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
@@ -1633,6 +1788,14 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         long long items = (coul ? f->n_tiles4 : f->n_tiles) * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
         const bool ragged = n_w % WALKER_TILE != 0;
+        if (!coul && n_w <= 32) {
+            // narrow batch: 16-walker column blocks, row fragments split over the warps
+            const int NB16 = (n_w + 15) / 16;
+            items = f->n_tiles * NB16;
+            ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
+            k_exchange_narrow<<<ex_grid, 384, EN_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta32, f->dWgt, f->dTiles, items, NB16,
+                                                                 N_pad, ldw, f->dEKpart, Wcap);
+        } else
 #define LO_EX_LAUNCH(C_, R_, TILES_, EJ_)                                                                                              \
     k_exchange<C_, R_><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, TILES_, items, NB, N_pad, ldw, \
                                                           f->dEKpart, EJ_, Wcap, n_w)

@@ -149,7 +149,7 @@ def test_c1_vector_reading_small_ragged_ranks():
     assert_parity(Eg2, Eo2)
 
 
-@pytest.mark.parametrize("n_w", [1, 5, 64, 65, 130])
+@pytest.mark.parametrize("n_w", [1, 5, 17, 33, 48, 49, 64, 65, 130])
 def test_ragged_walker_counts(c1, n_w):
     phis = gen.make_walkers(c1, n_w, seed=99)
     F = lo.Factors.setup(c1.h, c1.L, c1.psi, 5.0, device=0, max_walkers=130)
