@@ -970,22 +970,17 @@ __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constan
             for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
                 const ExTile tile = tiles[q / NB];
                 const int nb = (int)(q % NB);
-                const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + 2 * 32) * 128;
+                // whole 64-row boxes of U and W whatever the tile's length (rows past the tile are never read): 4 TMA
+                // issues per 24 KB stage -- a narrow item has too little MMA work per stage to hide more
+                const uint32_t tx = (uint32_t)(2 * EX_BM + 2 * 32) * 128;
                 for (int kt = 0; kt < KT; ++kt) {
                     mbar_wait(empty + 8 * slot, phase ^ 1);
                     if (kt == 0) ring[n % EX_RING] = tile;
                     const uint32_t st = sbase + slot * EN_STAGE_BYTES, bar = full + 8 * slot;
                     const int k0 = kt * KTILE;
                     mbar_expect_tx(bar, tx);
-                    if (tile.nfrag == EX_BM / 8) {
-                        tma_load_2d(st, &tmU, k0, tile.row0, bar);
-                        tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
-                    } else {
-                        for (int fr = 0; fr < tile.nfrag; ++fr) {
-                            tma_load_2d(st + fr * 1024, &tmU8, k0, tile.row0 + fr * 8, bar);
-                            tma_load_2d(st + EX_BM * 128 + fr * 1024, &tmW8, k0, tile.row0 + fr * 8, bar);
-                        }
-                    }
+                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
+                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
                     tma_load_2d(st + 2 * EX_BM * 128, &tmT32, k0, tile.pj * ldw + nb * 32, bar);
                     tma_load_2d(st + 2 * EX_BM * 128 + 32 * 128, &tmT32, k0, tile.pi * ldw + nb * 32, bar);
                     if (++slot == EN_STAGES) { slot = 0; phase ^= 1; }
