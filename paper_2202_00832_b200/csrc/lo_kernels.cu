@@ -572,9 +572,12 @@ __device__ __forceinline__ CoItem co_item(long long q, int RB, int NB, int nspli
     return it;
 }
 
+// RAGGED (the batch is not a multiple of 64 walkers): the warps are numbered column-slice first (the two warps of a
+// 32-column slice sit on different schedulers) and a warp whose slice holds no walker issues no MMAs.
+template <bool RAGGED>
 __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmT,
                                                     double* __restrict__ Xpart, int Xp, int O_tot, int N_pad, int ldw, int RB, int NB,
-                                                    int nsplit) {
+                                                    int nsplit, int n_cols) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t full = sbase + CO_STAGES * CO_STAGE_BYTES, empty = full + 8 * CO_STAGES;
@@ -612,7 +615,7 @@ __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUte
     }
     // ===== 8 consumer warps (64 x 32 each)
     reg_inc_consumer();
-    const int cw = warp - 4, g = lane >> 2, t = lane & 3, wm = cw >> 2, wn = cw & 3;
+    const int cw = warp - 4, g = lane >> 2, t = lane & 3, wm = RAGGED ? (cw & 1) : (cw >> 2), wn = RAGGED ? (cw >> 1) : (cw & 3);
     double acc[8][4][2];
 #pragma unroll
     for (int a = 0; a < 8; ++a)
@@ -626,6 +629,15 @@ __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUte
     uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
         const CoItem it = co_item(q, RB, NB, nsplit, ksteps);
+        if (RAGGED && it.nb * 128 + wn * 32 >= n_cols) {          // warp-uniform: no walker in this warp's 32 columns
+            for (int s = 0; s < it.nsteps; ++s) {
+                mbar_wait(full + 8 * cslot, cphase);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + 8 * cslot);
+                if (++cslot == CO_STAGES) { cslot = 0; cphase ^= 1; }
+            }
+            continue;
+        }
         for (int s = 0; s < it.nsteps; ++s) {
             mbar_wait(full + 8 * cslot, cphase);
             const uint32_t st = sbase + cslot * CO_STAGE_BYTES;
@@ -1679,7 +1691,8 @@ ThFn th_fn(int mfb) {
 
 lo_status configure_kernels() {
     cudaError_t e;
-    e = cudaFuncSetAttribute(k_coulomb, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    e = cudaFuncSetAttribute(k_coulomb<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coulomb<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_coulomb): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_exchange<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
@@ -1771,7 +1784,10 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         Timer tm(f, stream, LO_K_COULOMB);
         long long items = (long long)RB * NB * nsplit;
         int grid = (int)std::min<long long>(items, f->num_sms);
-        k_coulomb<<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit);
+        if (n_w % WALKER_TILE)
+            k_coulomb<true><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
+        else
+            k_coulomb<false><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
         dim3 g2(NB * 2, RB);
         k_ej<<<g2, 256, 0, stream>>>(f->dXpart, EJpart, E1raw, f->Xp, ldw, nsplit, f->n_chol, Wcap);
     }
@@ -1827,7 +1843,10 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
         k_pack_x<<<g1, 128, 0, stream>>>((const double2*)x_dev, f->dXT, f->n_chol, ops.Xk_pad);
         const long long items = (long long)RB * NB;
         const int grid = (int)std::min<long long>(items, f->num_sms);
-        k_coulomb<<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1);
+        if (n_w % WALKER_TILE)
+            k_coulomb<true><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
+        else
+            k_coulomb<false><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_propagator: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
