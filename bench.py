@@ -31,8 +31,8 @@ NOMINAL_FP64_TFLOPS = 40.0     # B200 datasheet FP64 (vector = tensor); context 
 NOMINAL_BF16_TFLOPS = 2250.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_exchange launch at the default workload, from the committed
 # ncu --set full capture (profiles/); None until that capture exists for the workload being run.
-NCU_TRAFFIC_BYTES = {("C2", "element", 1e-5, 512): 8.953645e9 + 12.967680e6,     # profiles/r01_ncu_full_c2.md
-                     ("C2", "vector", 1e-5, 512): 2.091726e9 + 10.547456e6}
+NCU_TRAFFIC_BYTES = {("C2", "element", 1e-5, 512): 8.969740e9 + 12.259840e6,     # profiles/r01_ncu_full_c2.md
+                     ("C2", "vector", 1e-5, 512): 2.090478e9 + 10.211584e6}
 
 
 def workload_name(cfg, reading, T, n_w):
