@@ -170,6 +170,11 @@ namespace lo {
 lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J,
                               void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 lo_status configure_kernels();
+lo_status configure_cas_kernels();     // lo_cas.cu
+// pieces of the hot path reused by the multi-determinant driver (lo_cas.cu)
+void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, const void* phi, double* dA, int* status, double* thT,
+               int o_base, int ldw_t, cudaStream_t stream);
+lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStream_t stream);
 lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
                                   int* walker_status, cudaStream_t stream);

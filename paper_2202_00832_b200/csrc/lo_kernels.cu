@@ -11,8 +11,7 @@
 //   k_exchange  grouped variable-rank dual GEMM a = U Theta_j, b = W Theta_i with fused weight * a * b reduction
 //               (Eq. 19/22 exchange part); <true>: also the compressed Coulomb projections (NEXT-3)
 //   k_finalize  E_K = sum of CTA partials, E_L = E1 + E_J + E_K, NaN for singular walkers
-//   k_cas_*     multi-determinant trial (NEXT-2): SMW overlaps / Green's functions (k_cas_T, k_cas_coef, k_cas_theta),
-//               rearranged SMW energy (k_cas_pairs, k_cas_H, k_cas_energy, k_cas_e1sum), k_cas_combine
+//   (the multi-determinant kernels k_cas_* are in lo_cas.cu; the shared device helpers in lo_device.cuh)
 //
 // FP64 on sm_100a has no tcgen05 path; the FP64 tensor instruction is the warp-level DMMA.8x8x4
 // (mma.sync.aligned.m8n8k4.f64), measured at 37.1 TFLOP/s on this B200 (same rate as the DFMA pipe, but one
@@ -27,84 +26,11 @@
 
 #include "lo_internal.h"
 
+#include "lo_device.cuh"
+
 namespace lo {
 
 namespace {
-
-__device__ __forceinline__ void mma884(double& c0, double& c1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-// Stage release must not overtake the stage's shared-memory reads.  ptxas is free to sink register-only MMAs below the
-// mbarrier arrive, and then the last ld.shared of a stage can still be in flight when the arrive issues (the arrive goes
-// through the SYNCS unit, not the load pipe) and the producer's TMA refill (async proxy) can land first -- seen as rare
-// wrong rows of X at configs[3].  release_stage() is the documented ordering for generic-proxy reads followed by an
-// async-proxy overwrite: fence.proxy.async (SASS: MEMBAR.ALL.CTA + FENCE.VIEW.ASYNC, waits for the warp's outstanding
-// loads), then the arrive.  It is issued right after the LAST fragment loads of a stage and before their MMAs, so the
-// wait overlaps the MMAs still queued on the tensor pipe.
-// ---- TMA + mbarrier plumbing (cp.async.bulk.tensor; SASS: UTMALDG / SYNCS)
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
-__device__ __forceinline__ void release_stage(uint32_t empty_bar, int lane) {
-    fence_proxy_async();
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty_bar);
-}
-// Warp-specialised register budget (setmaxnreg, per warpgroup): the kernels launch 3 warpgroups at 168 registers per
-// thread; the producer warpgroup shrinks to 40, the two consumer warpgroups grow to 232 (4*32*40 + 8*32*232 = 64512).
-__device__ __forceinline__ void reg_dec_producer() { asm volatile("setmaxnreg.dec.sync.aligned.u32 40;"); }
-__device__ __forceinline__ void reg_inc_consumer() { asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); }
-__device__ __forceinline__ void bar_sync_consumers() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}" ::"r"(bar), "r"(parity) : "memory");
-}
-// 2D tiled TMA load: box [rows][16 doubles] at (k0 = inner coordinate in doubles, row0) -> 128-byte-swizzled smem tile
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, int k0, int row0, uint32_t bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(k0), "r"(row0), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* tm) {
-    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
-}
-// Ampere-style asynchronous copies (LDGSTS) for the S1 staging; src_size 0 zero-fills the destination
-__device__ __forceinline__ void cp_async8(void* dst, const void* src, bool valid) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 8 : 0) : "memory");
-}
-__device__ __forceinline__ void cp_async16(void* dst, const void* src, bool valid) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 16 : 0) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N_>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
-__device__ __forceinline__ double lds_f64(uint32_t addr) {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-    return v;
-}
-
-// Shared-memory operand tiles are [rows][16 doubles] = 128 bytes per row, written by TMA with the 128-byte swizzle:
-// the 16-byte chunk c of row r lands at chunk c ^ (r & 7) (tile base 1024-byte aligned).  MMA k-step s (0..3) of a
-// K tile takes the logical k indices {2s, 2s+1, 2s+8, 2s+9} for t = 0..3 -- the same permutation for A and B, so the
-// contraction is unchanged -- which puts the 16 lanes of a half-warp (4 rows x 4 k) on 16 distinct 8-byte banks.
-// frag_off(g, t, s): byte offset inside a row whose (r & 7) == g.
-__device__ __forceinline__ uint32_t frag_off(int g, int t, int s) {
-    return (uint32_t)((((s + 4 * (t >> 1)) ^ g) << 4) + (t & 1) * 8);
-}
 
 // ------------------------------------------------------------------------------------------------ S1: overlap
 // A_w[i][j] = sum_p Psi[p][i] Phi_w[p][j]  as a real GEMM on the DMMA pipe: M = i (block of 32 per CTA), N = (j, re/im)
@@ -185,19 +111,6 @@ __global__ void __launch_bounds__(256) k_overlap(const double* __restrict__ psi,
 }
 
 // ------------------------------------------------------------------------------------------------ S1: inverse
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ double2 crecip(double2 a) {
-    // Smith's algorithm with correctly rounded reciprocals (MUFU.RCP64H + Newton) instead of the two divisions: the
-    // reciprocal sits on the serial chain of every Gauss-Jordan step
-    if (fabs(a.x) >= fabs(a.y)) {
-        const double r = a.y * __drcp_rn(a.x), id = __drcp_rn(a.x + a.y * r);
-        return make_double2(id, -r * id);
-    } else {
-        const double r = a.x * __drcp_rn(a.y), id = __drcp_rn(a.x * r + a.y);
-        return make_double2(r * id, -id);
-    }
-}
-
 // In-place Gauss-Jordan inversion with partial (row) pivoting.  One CTA per walker; the O x O complex matrix
 // lives in shared memory (IN_SMEM) or is updated in place in the global workspace (L2 resident) when it does
 // not fit.  status[w] = 1 and A^-1 = NaN when a pivot is zero / non-finite.
@@ -718,7 +631,6 @@ __global__ void __launch_bounds__(256) k_ej(double* __restrict__ Xpart, double2*
 // per-CTA partial sums accumulated in a fixed order -> bitwise repeatable.
 constexpr int EX_STAGES = 4;
 constexpr int EX_STAGE_BYTES = (2 * EX_BM + 2 * 128) * 128;
-constexpr int EX_RING = 8;      // tile-descriptor ring (producer -> consumers), > EX_STAGES items can never be in flight
 constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 128 + EX_RING * 16;
 
 // COUL: also accumulate the two projections of the paper-literal compressed Coulomb term,
@@ -1100,496 +1012,6 @@ __global__ void __launch_bounds__(128) k_pack_x(const double2* __restrict__ x, d
     XT[(size_t)(2 * w + 1) * Xk_pad + g] = v.y;
 }
 
-// ------------------------------------------------------------------------------------------------ NEXT-2: multi-determinant trial
-// Sherman-Morrison-Woodbury update of the reference (Eq. 20): determinant d replaces the reference columns
-// h_1..h_e by the orbitals p_1..p_e, A_d = A + U V^T.  With T = C_virt^T Theta0 (Theta0 = Phi A^-1) and T_d = T[p_k, h_l]:
-//   det A_d / det A = det T_d,      Theta^d = Theta0 (I - E_h T_d^-1 (T[p,:] - I[h,:])),
-// so in orbital-indexed panels (x = orbital of the factor set, zero when d does not occupy x)
-//   Theta^d_x = [x reference, not a hole] Theta0_x + sum_k G_d[k][x] Theta0_{h_k},
-//   G_d[k][x] = -sum_l (T_d^-1)_kl T[p_l][x]  (x reference, not a hole),  (T_d^-1)_km  (x = p_m),  0 otherwise.
-// k_cas_T: T[w][v][a] = sum_p C[p][n_ref+v] Theta0[a][w][p]; grid n_w, one warp per (v,a), lanes over p.
-__global__ void __launch_bounds__(256) k_cas_T(const double* __restrict__ C, int ldc, const double* __restrict__ th0, double2* __restrict__ T,
-                                               int N, int N_pad, int n_ref, int n_virt, int ldw0) {
-    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int e = warp; e < n_virt * n_ref; e += 8) {
-        const int v = e / n_ref, a = e - v * n_ref;
-        const double* re = th0 + ((size_t)a * ldw0 + 2 * w) * N_pad;
-        const double* im = re + N_pad;
-        double sr = 0.0, si = 0.0;
-        for (int p = lane; p < N; p += 32) {
-            const double c = C[(size_t)p * ldc + n_ref + v];
-            sr = fma(c, re[p], sr);
-            si = fma(c, im[p], si);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
-        if (lane == 0) T[((size_t)w * n_virt + v) * n_ref + a] = make_double2(sr, si);
-    }
-}
-
-// ---- NEXT-2, rearranged SMW energy (Eq. 21-23).  Every Theta^d column is a combination of the
-// reference column and the active (hole) columns of Theta0, so for pair (x <= y) the projections of U^{xy}, W^{xy} onto the
-// panel set P = [x, y, A_1..A_na] of Theta0 ("Q_L^int = U Phi A_act^-1") serve ALL determinants.  They are
-// contracted over the singular index K at once,
-//     S_t[c][c'] = sum_{K in tile t} wgt_K (U_K . Theta0_c)(W_K . Theta0_c'),     c, c' in P,
-// and a determinant's pair energies are small bilinear forms in S (k_cas_energy).  Work item = (row tile, block of 8
-// walkers); consumer warp m owns row fragment m and all NP panels x 16 real columns; same TMA/mbarrier pipeline.
-constexpr int CP_STAGES = 4;
-template <int NP>
-struct CpCfg {
-    static constexpr int STAGE_BYTES = 2 * EX_BM * 128 + NP * 16 * 128;
-    static constexpr int SL = NP * NP + 1;      // slice stride (double2) of one (row group, walker): odd, so the 8 lanes of a
-                                                // 128-bit shared access land on distinct 16-byte bank groups
-    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * 8 * SL * 16;
-};
-
-template <int NP>
-__global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
-                                                      const __grid_constant__ CUtensorMap tmT0, const double* __restrict__ wgt,
-                                                      const ExTile* __restrict__ tiles, long long n_items, int WB, int N_pad, int ldw0,
-                                                      const int* __restrict__ act /* [NP-2] */, double2* __restrict__ S, int n_w) {
-    constexpr int STAGE = CpCfg<NP>::STAGE_BYTES;
-    extern __shared__ unsigned char smem_raw[];
-    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
-    const uint32_t full = sbase + CP_STAGES * STAGE, empty = full + 8 * CP_STAGES;
-    ExTile* ring = reinterpret_cast<ExTile*>(sgen + CP_STAGES * STAGE + 128);
-    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 fragments (warps)][8 walkers][SL]
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int KT = N_pad / KTILE;
-    if (tid == 0) {
-        prefetch_tmap(&tmU);
-        prefetch_tmap(&tmW);
-        prefetch_tmap(&tmT0);
-        for (int i = 0; i < CP_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
-        fence_barrier_init();
-    }
-    __syncthreads();
-    if (warp < 4) {
-        reg_dec_producer();
-        if (warp == 0 && lane == 0) {
-            int pan[NP];
-#pragma unroll
-            for (int c = 2; c < NP; ++c) pan[c] = act[c - 2];
-            int slot = 0, n = 0;
-            uint32_t phase = 0;
-            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-                const ExTile tile = tiles[q / WB];
-                const int wb = (int)(q % WB);
-                pan[0] = tile.pi;
-                pan[1] = tile.pj;
-                // whole 64-row boxes of U and W whatever the tile's length (rows past the tile are never read): one TMA each
-                const uint32_t tx = (uint32_t)(2 * EX_BM + NP * 16) * 128;
-                for (int kt = 0; kt < KT; ++kt) {
-                    mbar_wait(empty + 8 * slot, phase ^ 1);
-                    if (kt == 0) ring[n % EX_RING] = tile;
-                    const uint32_t st = sbase + slot * STAGE, bar = full + 8 * slot;
-                    const int k0 = kt * KTILE;
-                    mbar_expect_tx(bar, tx);
-                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
-                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
-#pragma unroll
-                    for (int c = 0; c < NP; ++c)        // 16 real rows (8 walkers) of panel c
-                        tma_load_2d(st + 2 * EX_BM * 128 + c * 2048, &tmT0, k0, pan[c] * ldw0 + wb * 16, bar);
-                    if (++slot == CP_STAGES) { slot = 0; phase ^= 1; }
-                }
-            }
-        }
-        return;
-    }
-    reg_inc_consumer();
-    // Work units of an item = (row fragment, column half nf) = 2 * nfrag; consumer warp cw owns units cw and cw + 8, i.e.
-    // fragments cw/2 and 4 + cw/2 of the SAME column half nf = cw & 1 (they share the panel fragments).  The two warps
-    // of a scheduler (cw, cw + 4) then hold at most ceil(nfrag / 2) + ... units: 5 fragments load the four schedulers
-    // 3/3/2/2 instead of 2/1/1/1 whole fragments.
-    const int cw = warp - 4, g = lane >> 2, t = lane & 3, ctid = tid - 128;
-    const int nf = cw & 1, fr0 = cw >> 1, fr1 = 4 + (cw >> 1);
-    double accU[2][NP][2], accW[2][NP][2];
-#pragma unroll
-    for (int j = 0; j < 2; ++j)
-#pragma unroll
-        for (int c = 0; c < NP; ++c) accU[j][c][0] = accU[j][c][1] = accW[j][c][0] = accW[j][c][1] = 0.0;
-    uint32_t xo[4];
-#pragma unroll
-    for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
-    const uint32_t u_row0 = (uint32_t)(fr0 * 8 + g) * 128, u_row1 = (uint32_t)(fr1 * 8 + g) * 128;
-    const uint32_t p_row = (uint32_t)(2 * EX_BM * 128) + (uint32_t)(nf * 8 + g) * 128;
-    constexpr int SL = CpCfg<NP>::SL;
-    int cslot = 0, n = 0;
-    uint32_t cphase = 0;
-    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-        const int wb = (int)(q % WB);
-        const long long tix = q / WB;
-        mbar_wait(full + 8 * cslot, cphase);
-        const ExTile tile = ring[n % EX_RING];
-        const int nu = (fr0 < tile.nfrag ? 1 : 0) + (fr1 < tile.nfrag ? 1 : 0);     // warp-uniform: 0, 1 or 2 units
-        for (int kt = 0; kt < KT; ++kt) {
-            if (kt) mbar_wait(full + 8 * cslot, cphase);
-            const uint32_t st = sbase + cslot * STAGE;
-            if (nu == 2) {
-#pragma unroll
-                for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    const double a0 = lds_f64(st + u_row0 + xo[ks]), w0 = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
-                    const double a1 = lds_f64(st + u_row1 + xo[ks]), w1 = lds_f64(st + u_row1 + EX_BM * 128 + xo[ks]);
-                    double bb[NP];
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 2048 + xo[ks]);
-                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) {
-                        mma884(accU[0][c][0], accU[0][c][1], a0, bb[c]);
-                        mma884(accW[0][c][0], accW[0][c][1], w0, bb[c]);
-                        mma884(accU[1][c][0], accU[1][c][1], a1, bb[c]);
-                        mma884(accW[1][c][0], accW[1][c][1], w1, bb[c]);
-                    }
-                }
-            } else if (nu == 1) {
-#pragma unroll
-                for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    const double a0 = lds_f64(st + u_row0 + xo[ks]), w0 = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
-                    double bb[NP];
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 2048 + xo[ks]);
-                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) {
-                        mma884(accU[0][c][0], accU[0][c][1], a0, bb[c]);
-                        mma884(accW[0][c][0], accW[0][c][1], w0, bb[c]);
-                    }
-                }
-            } else {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty + 8 * cslot);
-            }
-            if (++cslot == CP_STAGES) { cslot = 0; cphase ^= 1; }
-        }
-        // epilogue: S[c][c'] of the 4 walkers of this warp's column half, per unit.  For every panel c the lane holds the 8
-        // complex products of its own row g (c' = 0..7, zero beyond NP); a transposing butterfly over the 8 row groups
-        // (each round sends half of the values and keeps the other half: 8+4+2 exchanges instead of 3 per value) leaves
-        // the row sum of column c' = 4 b0 + 2 b1 + b2 (bits of g) in lane g.  Every fragment's S goes to its own slice;
-        // the slices are added in fragment order when the block is written out (fixed order).
-        {
-            const bool b0 = g & 1, b1 = g & 2, b2 = g & 4;
-            const int c2own = (b0 ? 4 : 0) + (b1 ? 2 : 0) + (b2 ? 1 : 0);
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                if (j >= nu) break;                     // warp-uniform
-                const int fr = j == 0 ? fr0 : fr1;
-                const double wv = __ldg(wgt + tile.row0 + fr * 8 + g);
-                double2* dst = Sacc + ((fr * 8) + nf * 4 + t) * SL;
-#pragma unroll
-                for (int c = 0; c < NP; ++c) {
-                    const double ur = wv * accU[j][c][0], ui = wv * accU[j][c][1];
-                    double v[16];
-#pragma unroll
-                    for (int c2 = 0; c2 < 8; ++c2) {
-                        v[2 * c2] = c2 < NP ? ur * accW[j][c2 < NP ? c2 : 0][0] - ui * accW[j][c2 < NP ? c2 : 0][1] : 0.0;
-                        v[2 * c2 + 1] = c2 < NP ? ur * accW[j][c2 < NP ? c2 : 0][1] + ui * accW[j][c2 < NP ? c2 : 0][0] : 0.0;
-                    }
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {       // round 1: lanes g^1, halves of 8
-                        const double snd = b0 ? v[i] : v[i + 8], kp = b0 ? v[i + 8] : v[i];
-                        v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 4);
-                    }
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {       // round 2: lanes g^2, halves of 4
-                        const double snd = b1 ? v[i] : v[i + 4], kp = b1 ? v[i + 4] : v[i];
-                        v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 8);
-                    }
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {       // round 3: lanes g^4, halves of 2
-                        const double snd = b2 ? v[i] : v[i + 2], kp = b2 ? v[i + 2] : v[i];
-                        v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 16);
-                    }
-                    if (c2own < NP) dst[c * NP + c2own] = make_double2(v[0], v[1]);
-                }
-#pragma unroll
-                for (int c = 0; c < NP; ++c) accU[j][c][0] = accU[j][c][1] = accW[j][c][0] = accW[j][c][1] = 0.0;
-            }
-        }
-        bar_sync_consumers();
-        for (int i = ctid; i < 8 * NP * NP; i += 256) {
-            const int wl = i / (NP * NP), wg = wb * 8 + wl;
-            const int is = wl * SL + (i - wl * NP * NP);
-            double2 sum = Sacc[is];
-            for (int fr = 1; fr < tile.nfrag; ++fr) { const double2 v = Sacc[fr * 8 * SL + is]; sum.x += v.x; sum.y += v.y; }
-            if (wg < n_w) S[((size_t)tix * n_w + wg) * NP * NP + (i - wl * NP * NP)] = sum;
-        }
-        bar_sync_consumers();
-    }
-}
-
-// One-body intermediates of the SMW energy: H[w][x][0] = hbar_x . Theta0_x (reference x), H[w][x][1+a] = hbar_x . Theta0_{A_a}.
-// grid n_w, one warp per (x, slot), lanes over p.  hbar = row n_chol of the [Lbar; hbar] operand.
-__global__ void __launch_bounds__(256) k_cas_H(const double* __restrict__ hbar, const double* __restrict__ th0, const int* __restrict__ act,
-                                               int n_act, double2* __restrict__ H, int N, int N_pad, int n_ref, int n_orb, int ldw0) {
-    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int e = warp; e < n_orb * (1 + n_act); e += 8) {
-        const int x = e / (1 + n_act), sl = e - x * (1 + n_act);
-        const int c = sl == 0 ? x : act[sl - 1];
-        double sr = 0.0, si = 0.0;
-        if (c < n_ref) {
-            const double* hx = hbar + (size_t)x * N_pad;
-            const double* re = th0 + ((size_t)c * ldw0 + 2 * w) * N_pad;
-            const double* im = re + N_pad;
-            for (int p = lane; p < N; p += 32) {
-                sr = fma(hx[p], re[p], sr);
-                si = fma(hx[p], im[p], si);
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
-        }
-        if (lane == 0) H[((size_t)w * n_orb + x) * 9 + sl] = make_double2(sr, si);
-    }
-}
-
-// Pair energies of every determinant from the S intermediates (Eq. 22 with Eq. 23 inserted): with
-// Theta^d_x = s_x Theta0_x + sum_k G_d[k][x] Theta0_{h_k}  (s_x = 1 for a reference non-hole, else 0),
-//   exchange  e = sum_{c in y-list} sum_{c' in x-list} coef_y[c] coef_x[c'] S[c][c'],
-//   Coulomb   j = sum_{c in x-list} sum_{c' in y-list} coef_x[c] coef_y[c'] S[c][c'],
-// lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of CE_CH tiles sits in shared memory, threads
-// run over determinants; partial (E_K, E_J) sums per chunk are added in chunk order by k_cas_e1sum.
-constexpr int CE_CH = 16;
-template <int MAXE>     // compile-time bound of the excitation rank: the coefficient lists stay in registers
-__global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const ExTile* __restrict__ tiles, long long n_tiles,
-                                                    const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
-                                                    const double2* __restrict__ G, double2* __restrict__ part, int n_w, int n_det, int max_exc,
-                                                    int n_orb, int NP, int n_vtot) {
-    extern __shared__ __align__(16) double2 Ss[];      // [CE_CH][NP*NP]
-    __shared__ int tx_s[CE_CH], ty_s[CE_CH];
-    const int chunk = blockIdx.x, w = blockIdx.y, tid = threadIdx.x;
-    const long long t0 = (long long)chunk * CE_CH;
-    const int nt = (int)min((long long)CE_CH, n_tiles - t0), NP2 = NP * NP;
-    for (int i = tid; i < nt * NP2; i += 128) {
-        const int tl = i / NP2;
-        Ss[i] = S[((size_t)(t0 + tl) * n_w + w) * NP2 + (i - tl * NP2)];
-    }
-    if (tid < nt) { tx_s[tid] = tiles[t0 + tid].pi; ty_s[tid] = tiles[t0 + tid].pj; }
-    __syncthreads();
-    for (int d = tid; d < n_det; d += 128) {
-        const size_t v = (size_t)w * n_det + d;
-        const signed char* kd = kind + (size_t)d * n_orb;
-        const int* hi = holeIdx + (size_t)d * max_exc;
-        int e = 0;
-        while (e < max_exc && hi[e] >= 0) ++e;
-        const double2* Gv = G + v * max_exc * n_orb;
-        double2 ek = make_double2(0.0, 0.0), ej = make_double2(0.0, 0.0);
-        for (int tl = 0; tl < nt; ++tl) {
-            const int x = tx_s[tl], y = ty_s[tl];
-            const int kx = kd[x], ky = kd[y];
-            if (kx < 0 || ky < 0) continue;
-            const double2* St = Ss + tl * NP2;
-            // coefficient lists: entry 0 = self (index 0 for the x role, 1 for the y role), entries 1..e = the holes
-            double2 cx[MAXE + 1], cy[MAXE + 1];
-            int ix[MAXE + 1], iy[MAXE + 1];
-            cx[0] = make_double2(kx == 0 ? 1.0 : 0.0, 0.0); ix[0] = 0;
-            cy[0] = make_double2(ky == 0 ? 1.0 : 0.0, 0.0); iy[0] = 1;
-#pragma unroll
-            for (int k = 0; k < MAXE; ++k) {
-                const bool on = k < e;
-                cx[1 + k] = on ? Gv[(size_t)k * n_orb + x] : make_double2(0.0, 0.0); ix[1 + k] = on ? 2 + hi[k] : 0;
-                cy[1 + k] = on ? Gv[(size_t)k * n_orb + y] : make_double2(0.0, 0.0); iy[1 + k] = on ? 2 + hi[k] : 0;
-            }
-#pragma unroll
-            for (int a = 0; a <= MAXE; ++a) {
-                if (a > e) break;
-#pragma unroll
-                for (int b = 0; b <= MAXE; ++b) {
-                    if (b > e) break;
-                    const double2 cc = cmul(cy[a], cx[b]);
-                    const double2 se = St[iy[a] * NP + ix[b]], sj = St[ix[b] * NP + iy[a]];
-                    const double2 t1 = cmul(cc, se), t2 = cmul(cc, sj);
-                    ek.x += t1.x; ek.y += t1.y;
-                    ej.x += t2.x; ej.y += t2.y;
-                }
-            }
-        }
-        part[((size_t)chunk * n_vtot + v) * 2] = ek;
-        part[((size_t)chunk * n_vtot + v) * 2 + 1] = make_double2(-2.0 * ej.x, -2.0 * ej.y);
-    }
-}
-
-// Per virtual walker: E_K^d, E_J^d = chunk partials in chunk order; E1^d = 2 [sum_{x ref non-hole} H[x][self] +
-// sum_k sum_x G_d[k][x] H[x][hole k]]; writes Ev[v] = {E_L, E1, E_J, E_K} for k_cas_combine.
-__global__ void __launch_bounds__(128) k_cas_e1sum(const double2* __restrict__ part, int n_chunks, const double2* __restrict__ H,
-                                                   const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
-                                                   const double2* __restrict__ G, double2* __restrict__ Ev, int n_v, int n_det, int max_exc,
-                                                   int n_orb, int n_vtot) {
-    const int v = blockIdx.x * 128 + threadIdx.x;
-    if (v >= n_v) return;
-    const int w = v / n_det, d = v - w * n_det;
-    double2 ek = make_double2(0.0, 0.0), ej = make_double2(0.0, 0.0), e1 = make_double2(0.0, 0.0);
-    for (int c = 0; c < n_chunks; ++c) {
-        const double2 a = part[((size_t)c * n_vtot + v) * 2], b = part[((size_t)c * n_vtot + v) * 2 + 1];
-        ek.x += a.x; ek.y += a.y;
-        ej.x += b.x; ej.y += b.y;
-    }
-    const signed char* kd = kind + (size_t)d * n_orb;
-    const int* hi = holeIdx + (size_t)d * max_exc;
-    const double2* Hw = H + (size_t)w * n_orb * 9;
-    const double2* Gv = G + (size_t)v * max_exc * n_orb;
-    for (int x = 0; x < n_orb; ++x) {
-        if (kd[x] < 0) continue;
-        if (kd[x] == 0) { e1.x += Hw[x * 9].x; e1.y += Hw[x * 9].y; }
-        for (int k = 0; k < max_exc && hi[k] >= 0; ++k) {
-            const double2 t1 = cmul(Gv[(size_t)k * n_orb + x], Hw[x * 9 + 1 + hi[k]]);
-            e1.x += t1.x; e1.y += t1.y;
-        }
-    }
-    e1.x *= 2.0; e1.y *= 2.0;
-    Ev[4 * (size_t)v] = make_double2(e1.x + ej.x + ek.x, e1.y + ej.y + ek.y);
-    Ev[4 * (size_t)v + 1] = e1;
-    Ev[4 * (size_t)v + 2] = ej;
-    Ev[4 * (size_t)v + 3] = ek;
-}
-
-// One warp per virtual walker v = w*n_det + d: lane 0 inverts T_d (<= 8 x 8, Gauss-Jordan with partial pivoting) and
-// takes its determinant; all lanes then fill G_d.  weight = c_d det(T_d)^2 (closed shell: the same string in both spins;
-// unrestricted: c_d det(T_d^alpha) from the alpha call times det(T_d^beta) from the beta call, multiplied in k_cas_combine);
-// status 1 when the reference overlap or T_d is singular (that determinant is then left out of the sums).
-__global__ void __launch_bounds__(128) k_cas_coef(const double2* __restrict__ T, const int* __restrict__ holes, const int* __restrict__ parts,
-                                                  const double* __restrict__ coef, const int* __restrict__ st0, double2* __restrict__ G,
-                                                  double2* __restrict__ wd, int* __restrict__ stv, int n_v, int n_det, int max_exc, int n_ref,
-                                                  int n_virt, int n_orb, int wmode /* 0: c det^2, 1: c det (alpha), 2: det (beta) */) {
-    __shared__ double2 inv_s[4][CAS_MAX_EXC][CAS_MAX_EXC];
-    __shared__ int ok_s[4];
-    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5, v = blockIdx.x * 4 + wi;
-    if (v >= n_v) return;
-    const int w = v / n_det, d = v - w * n_det;
-    const int* hs = holes + (size_t)d * max_exc;
-    const int* ps = parts + (size_t)d * max_exc;
-    int e = 0;
-    while (e < max_exc && hs[e] >= 0) ++e;
-    const double2* Tw = T + (size_t)w * n_virt * n_ref;
-    if (lane == 0) {
-        double2 M[CAS_MAX_EXC][CAS_MAX_EXC], I[CAS_MAX_EXC][CAS_MAX_EXC];
-        for (int k = 0; k < e; ++k)
-            for (int l = 0; l < e; ++l) {
-                M[k][l] = Tw[(size_t)(ps[k] - n_ref) * n_ref + hs[l]];
-                I[k][l] = make_double2(k == l ? 1.0 : 0.0, 0.0);
-            }
-        double2 det = make_double2(1.0, 0.0);
-        bool ok = st0[w] == 0;
-        for (int k = 0; k < e && ok; ++k) {
-            int piv = k;
-            double best = -1.0;
-            for (int r = k; r < e; ++r) {
-                double m = M[r][k].x * M[r][k].x + M[r][k].y * M[r][k].y;
-                if (!(m == m)) m = INFINITY;
-                if (m > best) { best = m; piv = r; }
-            }
-            if (!(best > 1e-300) || isinf(best)) { ok = false; break; }
-            if (piv != k) {
-                for (int c = 0; c < e; ++c) { double2 t1 = M[k][c]; M[k][c] = M[piv][c]; M[piv][c] = t1; t1 = I[k][c]; I[k][c] = I[piv][c]; I[piv][c] = t1; }
-                det = make_double2(-det.x, -det.y);
-            }
-            det = cmul(det, M[k][k]);
-            const double2 ip = crecip(M[k][k]);
-            for (int c = 0; c < e; ++c) { M[k][c] = cmul(M[k][c], ip); I[k][c] = cmul(I[k][c], ip); }
-            for (int r = 0; r < e; ++r) {
-                if (r == k) continue;
-                const double2 fct = M[r][k];
-                for (int c = 0; c < e; ++c) {
-                    double2 t1 = cmul(fct, M[k][c]), t2 = cmul(fct, I[k][c]);
-                    M[r][c] = make_double2(M[r][c].x - t1.x, M[r][c].y - t1.y);
-                    I[r][c] = make_double2(I[r][c].x - t2.x, I[r][c].y - t2.y);
-                }
-            }
-        }
-        for (int k = 0; k < e; ++k)
-            for (int l = 0; l < e; ++l) inv_s[wi][k][l] = I[k][l];
-        ok_s[wi] = ok ? 1 : 0;
-        const double2 d2 = wmode == 0 ? cmul(det, det) : det;
-        const double cf = wmode == 2 ? 1.0 : coef[d];
-        wd[v] = ok ? make_double2(cf * d2.x, cf * d2.y) : make_double2(0.0, 0.0);
-        stv[v] = ok ? 0 : 1;
-    }
-    __syncwarp();
-    const bool ok = ok_s[wi] != 0;
-    double2* Gv = G + (size_t)v * max_exc * n_orb;
-    for (int x = lane; x < n_orb; x += 32) {
-        int kind = x < n_ref ? 0 : -1;     // 0: reference non-hole, 1+m: particle p_m, -1: zero
-        for (int m = 0; m < e; ++m) {
-            if (hs[m] == x) kind = -1;
-            if (ps[m] == x) kind = 1 + m;
-        }
-        for (int k = 0; k < e; ++k) {
-            double2 gk = make_double2(0.0, 0.0);
-            if (ok && kind == 0) {
-                for (int l = 0; l < e; ++l) {
-                    const double2 t1 = cmul(inv_s[wi][k][l], Tw[(size_t)(ps[l] - n_ref) * n_ref + x]);
-                    gk.x -= t1.x; gk.y -= t1.y;
-                }
-            } else if (ok && kind > 0) {
-                gk = inv_s[wi][k][kind - 1];
-            }
-            Gv[(size_t)k * n_orb + x] = gk;
-        }
-    }
-}
-
-// Theta^d panels of every virtual walker: grid (n_v, n_orb, ceil(N_pad/128)), thread = basis index p.
-__global__ void __launch_bounds__(128) k_cas_theta(const double* __restrict__ th0, const double2* __restrict__ G, const int* __restrict__ holes,
-                                                   double* __restrict__ thT, int N_pad, int n_ref, int n_orb, int n_det, int max_exc, int ldw0,
-                                                   int ldw, int o_base) {
-    const int p = blockIdx.z * 128 + threadIdx.x, x = blockIdx.y, v = blockIdx.x;
-    if (p >= N_pad) return;
-    const int w = v / n_det, d = v - w * n_det;
-    const int* hs = holes + (size_t)d * max_exc;
-    double re = 0.0, im = 0.0;
-    bool is_hole = false;
-    int e = 0;
-    for (; e < max_exc && hs[e] >= 0; ++e) is_hole |= hs[e] == x;
-    if (x < n_ref && !is_hole) {
-        re = th0[((size_t)x * ldw0 + 2 * w) * N_pad + p];
-        im = th0[((size_t)x * ldw0 + 2 * w + 1) * N_pad + p];
-    }
-    const double2* Gv = G + (size_t)v * max_exc * n_orb + x;
-    for (int k = 0; k < e; ++k) {
-        const double2 g = Gv[(size_t)k * n_orb];
-        const double tr = th0[((size_t)hs[k] * ldw0 + 2 * w) * N_pad + p], ti = th0[((size_t)hs[k] * ldw0 + 2 * w + 1) * N_pad + p];
-        re = fma(g.x, tr, fma(-g.y, ti, re));
-        im = fma(g.x, ti, fma(g.y, tr, im));
-    }
-    thT[((size_t)(o_base + x) * ldw + 2 * v) * N_pad + p] = re;
-    thT[((size_t)(o_base + x) * ldw + 2 * v + 1) * N_pad + p] = im;
-}
-
-// E = sum_d w_d E^d / sum_d w_d per real walker and energy term (Eq. 12), determinants in index order (fixed order).
-__global__ void k_cas_combine(const double2* __restrict__ Ev, const double2* __restrict__ wd, const int* __restrict__ stv,
-                              const int* __restrict__ st0, const double2* __restrict__ wdB, const int* __restrict__ stvB,
-                              const int* __restrict__ st0B, int n_w, int n_det, double2* __restrict__ E_L, double2* __restrict__ E1,
-                              double2* __restrict__ E_J, double2* __restrict__ E_K, double2* __restrict__ ovlp, int* __restrict__ st_out) {
-    const int w = blockIdx.x * blockDim.x + threadIdx.x;
-    if (w >= n_w) return;
-    double2 num[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)}, den = make_double2(0.0, 0.0);
-    for (int d = 0; d < n_det; ++d) {
-        const size_t v = (size_t)w * n_det + d;
-        if (stv[v] || (stvB && stvB[v])) continue;
-        const double2 wv = wdB ? cmul(wd[v], wdB[v]) : wd[v];
-        for (int c = 0; c < 3; ++c) {
-            const double2 t1 = cmul(wv, Ev[4 * v + 1 + c]);
-            num[c].x += t1.x; num[c].y += t1.y;
-        }
-        den.x += wv.x; den.y += wv.y;
-    }
-    const double m2 = den.x * den.x + den.y * den.y;
-    const bool bad = st0[w] != 0 || (st0B && st0B[w] != 0) || !(m2 > 0.0) || isinf(m2);
-    const double nan = __longlong_as_double(0x7ff8000000000000LL);
-    double2 e[3], el = make_double2(0.0, 0.0);
-    const double2 id = bad ? make_double2(nan, nan) : crecip(den);
-    for (int c = 0; c < 3; ++c) {
-        e[c] = bad ? make_double2(nan, nan) : cmul(num[c], id);
-        el.x += e[c].x; el.y += e[c].y;
-    }
-    if (E_L) E_L[w] = el;
-    if (E1) E1[w] = e[0];
-    if (E_J) E_J[w] = e[1];
-    if (E_K) E_K[w] = e[2];
-    if (ovlp) ovlp[w] = bad ? make_double2(nan, nan) : den;
-    if (st_out) st_out[w] = bad ? 1 : 0;
-}
-
 // ------------------------------------------------------------------------------------------------ S5: combine
 __global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, const double2* __restrict__ E1raw,
                            const double2* __restrict__ EKpart, int n_ctas, const int* __restrict__ status, int n_spin, int Wcap,
@@ -1624,23 +1046,6 @@ __global__ void k_finalize(const double2* __restrict__ EJpart, int n_chunks, con
     if (st_out) st_out[w] = bad;
     if (Eout4) { Eout4[4 * w] = el; Eout4[4 * w + 1] = e1; Eout4[4 * w + 2] = ej; Eout4[4 * w + 3] = ek; }
 }
-
-struct Timer {
-    lo_factors* f;
-    cudaStream_t s;
-    int idx = -1;
-    Timer(lo_factors* f_, cudaStream_t s_, int kind) : f(f_), s(s_) {
-        if (!f->timing) return;
-        TimingEvent ev;
-        if (!f->pool.empty()) { ev = f->pool.back(); f->pool.pop_back(); }
-        else { cudaEventCreate(&ev.e0); cudaEventCreate(&ev.e1); }
-        ev.kind = kind;
-        cudaEventRecord(ev.e0, s);
-        f->events.push_back(ev);
-        idx = (int)f->events.size() - 1;
-    }
-    ~Timer() { if (idx >= 0) cudaEventRecord(f->events[idx].e1, s); }
-};
 
 int pick_split(long long base_items, int ksteps, int sms) {
     int best = 1;
@@ -1713,10 +1118,7 @@ lo_status configure_kernels() {
             if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)ov_fn(m, n), cudaFuncAttributePreferredSharedMemoryCarveout, 100);
             if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_overlap): ") + cudaGetErrorString(e)); return LO_ECUDA; }
         }
-    e = cudaFuncSetAttribute(k_cas_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<4>::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<6>::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<8>::SMEM);
-    if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_cas_*): ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    if (configure_cas_kernels() != LO_OK) return LO_ECUDA;
     e = cudaFuncSetAttribute(k_inverse<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_inverse): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
@@ -1758,8 +1160,6 @@ void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, cons
         th_fn(mfb)<<<grid, 256, (size_t)2 * (mfb * 8 + 64) * TH_LD * 8, stream>>>((const double2*)phi, (const double2*)dA, thT, N, N_pad, O, o_base, ldw_t);
     }
 }
-
-lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 
 lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
                               int* walker_status, void* Eout4, cudaStream_t stream) {
@@ -1850,76 +1250,6 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_propagator: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
-    return LO_OK;
-}
-
-// local energy with a multi-determinant trial by direct summation over determinants (Eq. 12), the
-// determinants' overlaps and Green's functions by SMW updates of the reference (Eq. 20); each (walker, determinant) is a
-// virtual walker of the ordinary Coulomb / exchange kernels (orbital-indexed Theta^d panels, zero where unoccupied).
-lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K,
-                                  void* ovlp, int* walker_status, cudaStream_t stream) {
-    CasPlan& c = *f->cas;
-    const int n_orb = f->n_occ[0], n_v = n_w * c.n_det, ldw0 = 2 * c.W0cap;
-    launch_s1(f, n_w, f->ops->dPsi[0], n_orb, c.n_ref, phi, c.dA0, c.dSt0, c.dTh0, 0, ldw0, stream);
-    k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[0], n_orb, c.dTh0, (double2*)c.dT, f->N, f->N_pad, c.n_ref, c.n_virt, ldw0);
-    int* stv = c.mode == 0 ? f->dStatus : c.dStV;
-    k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dT, c.dHoles, c.dParts, c.dCoef, c.dSt0, (double2*)c.dG, (double2*)c.dWd,
-                                                  stv, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb, c.has_beta ? 1 : 0);
-    if (c.has_beta) {
-        // unrestricted trial: the beta strings get their own SMW data; their Theta^d panels follow the alpha panels
-        const int n_orb_b = f->n_occ[1];
-        launch_s1(f, n_w, f->ops->dPsi[1], n_orb_b, c.n_ref_b, phi_b, c.dA0B, c.dSt0B, c.dTh0B, 0, ldw0, stream);
-        k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[1], n_orb_b, c.dTh0B, (double2*)c.dTB, f->N, f->N_pad, c.n_ref_b, c.n_virt_b, ldw0);
-        k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dTB, c.dHolesB, c.dPartsB, c.dCoef, c.dSt0B, (double2*)c.dGB,
-                                                      (double2*)c.dWdB, f->dStatus + f->Wcap, n_v, c.n_det, c.max_exc, c.n_ref_b, c.n_virt_b,
-                                                      n_orb_b, 2);
-        dim3 g3b(n_v, n_orb_b, (f->N_pad + 127) / 128);
-        k_cas_theta<<<g3b, 128, 0, stream>>>(c.dTh0B, (const double2*)c.dGB, c.dHolesB, f->dThT, f->N_pad, c.n_ref_b, n_orb_b, c.n_det, c.max_exc,
-                                             ldw0, f->ldw, f->o_base[1]);
-    }
-    if (c.mode == 0) {
-        dim3 g3(n_v, n_orb, (f->N_pad + 127) / 128);
-        k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw, 0);
-        lo_status st = launch_s3_s5(f, n_v, nullptr, nullptr, nullptr, nullptr, nullptr, c.dEv, stream);
-        if (st != LO_OK) return st;
-    } else {
-        // rearranged SMW energy (Eq. 23): S intermediates once per (tile, walker), then small per-determinant forms
-        const int WB = (n_w + 7) / 8;
-        const long long items = f->n_tiles * WB;
-        const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        const int* actd = c.dHoleIdx + (size_t)c.n_det * c.max_exc;      // A_set stored behind the hole indices
-        if (c.NP == 4)
-            k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
-        else if (c.NP == 6)
-            k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
-        else
-            k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
-        const double* hbar = f->ops->dLbar + (size_t)f->n_chol * f->O_tot * f->N_pad;
-        k_cas_H<<<n_w, 256, 0, stream>>>(hbar, c.dTh0, actd, c.n_act, (double2*)c.dH, f->N, f->N_pad, c.n_ref, n_orb, ldw0);
-        const int n_chunks = (int)((f->n_tiles + CE_CH - 1) / CE_CH);
-        const int n_vtot = c.max_real * c.n_det;
-        if (n_chunks > 0) {
-            dim3 g4(n_chunks, n_w);
-            const size_t sm4 = (size_t)CE_CH * c.NP * c.NP * 16;
-            if (c.max_exc <= 2)
-                k_cas_energy<2><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
-                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
-            else if (c.max_exc <= 4)
-                k_cas_energy<4><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
-                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
-            else
-                k_cas_energy<8><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
-                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
-        }
-        k_cas_e1sum<<<(n_v + 127) / 128, 128, 0, stream>>>((const double2*)c.dPart, n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx,
-                                                           (const double2*)c.dG, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_orb, n_vtot);
-    }
-    k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, stv, c.dSt0,
-                                                         c.has_beta ? (const double2*)c.dWdB : nullptr, c.has_beta ? f->dStatus + f->Wcap : nullptr,
-                                                         c.has_beta ? c.dSt0B : nullptr, n_w, c.n_det,
-                                                         (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K, (double2*)ovlp, walker_status);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) { set_error(std::string("lo_local_energy_cas: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
 }
 
