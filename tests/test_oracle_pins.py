@@ -432,3 +432,38 @@ def test_cas_unrestricted_pins(c0, c0_walkers):
     assert np.abs(np.array(E1[:4]) - np.array(Es)).max() <= 1e-10 * abs(Es[0])
     Eall = oracle.local_energy_cas_u([Ta.C, Tb.C], colsu, Ta.coef, [a for a, _ in hr], [b for _, b in hr], fss, [phis[0][1], phis[1][1]])
     assert abs(Eall[0] - Es[0]) > 1e-6 * abs(Es[0])
+
+
+def test_cas_unrestricted_open_shell_singlet_and_triplet():
+    """Pin of oracle.local_energy_cas_u for determinants whose alpha and beta strings DIFFER (Eq. 12/13, PAPER.md:108-114;
+    Slater-Condon rules).  One alpha and one beta electron in two orbitals of different symmetry (h diagonal, every
+    Cholesky matrix either diagonal or purely off-diagonal): |1a 2b> and |2a 1b> decouple from the closed-shell
+    determinants (<1a1b|H|1a2b> = h_12 + (11|12) = 0) and couple to each other through (12|21) = K12, so
+        singlet (|1a2b> + |2a1b>)/sqrt2 :  E = h1 + h2 + J12 + K12,
+        triplet (|1a2b> - |2a1b>)/sqrt2 :  E = h1 + h2 + J12 - K12,      J12 = sum_g L^g_11 L^g_22,  K12 = sum_g (L^g_12)^2
+    are exact eigenstates, and the mixed estimator returns the eigenvalue for ANY pair of alpha/beta walkers.  This
+    fixes the weight w_d = c_d det_a det_b (det_a^2 would give another number: det_a != det_b here) and the relative
+    sign of determinants with different strings (a flipped coefficient turns the singlet into the triplet, 2 K12 away)."""
+    h = np.diag([-0.8, 0.35])
+    L = np.zeros((4, 2, 2))
+    L[0] = np.diag([0.7, 0.4])
+    L[1] = np.diag([-0.2, 0.9])
+    L[2] = np.array([[0.0, 0.55], [0.55, 0.0]])
+    L[3] = np.array([[0.0, -0.3], [-0.3, 0.0]])
+    J12 = (L[:, 0, 0] * L[:, 1, 1]).sum()
+    K12 = (L[:, 0, 1] ** 2).sum()
+    assert K12 > 0.1
+    Cmo = np.eye(2)
+    Lbar, hbar = oracle.half_rotate(L, h, Cmo)
+    fs = oracle.own_factors(Lbar, 0.0)
+    cols = [[[0], [1]], [[1], [0]]]          # alpha strings of the two determinants, beta strings of the two determinants
+    rng = np.random.default_rng(11)
+    for sign, name in ((+1.0, "singlet"), (-1.0, "triplet")):
+        E_exact = h[0, 0] + h[1, 1] + J12 + sign * K12
+        coef = np.array([1.0, sign]) / np.sqrt(2.0)
+        for _ in range(4):
+            pa = rng.standard_normal((2, 1)) + 1j * rng.standard_normal((2, 1))
+            pb = rng.standard_normal((2, 1)) + 1j * rng.standard_normal((2, 1))
+            E = oracle.local_energy_cas_u([Cmo, Cmo], cols, coef, [Lbar, Lbar], [hbar, hbar], [fs, fs], [pa, pb])
+            assert abs(E[0] - E_exact) <= 1e-12 * max(1.0, abs(E_exact)), (name, E[0], E_exact)
+            assert abs(E[1] + E[2] + E[3] - E[0]) <= 1e-13
