@@ -29,10 +29,41 @@ METRIC = "walker local energies/s (complex128 LO-AFQMC E_L)"
 UNIT = "energies/s"
 NOMINAL_FP64_TFLOPS = 40.0     # B200 datasheet FP64 (vector = tensor); context for the ratio-derived peak
 NOMINAL_BF16_TFLOPS = 2250.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_exchange launch at the default workload, from the committed
-# ncu --set full capture (profiles/); None until that capture exists for the workload being run.
-NCU_TRAFFIC_BYTES = {("C2", "element", 1e-5, 512): 8.969740e9 + 12.259840e6,     # profiles/r01_ncu_full_c2.md
-                     ("C2", "vector", 1e-5, 512): 2.090478e9 + 10.211584e6}
+# roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, read from the
+# sidecar of the committed `ncu --set full` capture (one row per workload: the two counters, the commit and the SHA-256 of
+# the kernel sources the capture was taken at).  A row whose hash is not that of the kernel sources being run is stale:
+# traffic is then null and `traffic_note` says why.
+TRAFFIC_SIDECAR = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+KERNEL_SOURCES = ("lo_kernels.cu", "lo_device.cuh")
+
+
+def kernel_sources_sha256():
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2202_00832_b200", "csrc", name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def ncu_traffic(workload):
+    """(bytes per launch or None, note) for `workload` from profiles/ncu_traffic.csv."""
+    import csv
+    try:
+        with open(TRAFFIC_SIDECAR, newline="") as fh:
+            rows = [r for r in csv.DictReader(fh) if r["workload"] == workload]
+    except OSError:
+        return None, "no sidecar %s" % os.path.relpath(TRAFFIC_SIDECAR, ROOT)
+    if not rows:
+        return None, "no ncu --set full capture of this workload in %s" % os.path.relpath(TRAFFIC_SIDECAR, ROOT)
+    sha = kernel_sources_sha256()
+    fresh = [r for r in rows if r["kernel_sources_sha256"] == sha]
+    if not fresh:
+        return None, "capture of commit %s is stale: %s changed since (sha256 %s.. != %s..)" % (
+            rows[-1]["commit"], "+".join(KERNEL_SOURCES), rows[-1]["kernel_sources_sha256"][:12], sha[:12])
+    r = fresh[-1]
+    return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), "%s of %s at commit %s (%s)" % (
+        r["kernel"], r["capture"], r["commit"], "dram__bytes_read.sum + dram__bytes_write.sum")
 
 
 def workload_name(cfg, reading, T, n_w):
@@ -199,10 +230,10 @@ def run_ours(args):
     achieved = ex_flops / (ex_avg * 1e-3) * 1e-12
     peak = max(peak_dmma, peak_dfma)
     mp = measured_peaks()
-    wl = ("C%d" % cfg, reading, T, n_w)
+    traffic, traffic_note = ncu_traffic(workload_name(cfg, reading, T, n_w))
     roofline = {"bound": "tensor", "kernel": "k_exchange (grouped variable-rank dual DGEMM + fused sigma-weighted a.b)",
                 "achieved": round(achieved, 3), "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
-                "traffic": NCU_TRAFFIC_BYTES.get(wl),
+                "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": "in-run register-resident DMMA.8x8x4 / DFMA loops (lo_measure_peak), of measured",
                 "peak_dmma": round(peak_dmma, 3), "peak_dfma": round(peak_dfma, 3),
                 "peak_from_bf16_ratio": round(mp.get("bf16_tflops", 0) * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS, 2) if mp else None,
@@ -460,7 +491,7 @@ def run_reference(args):
     nb = min(args.ref_walkers, n_w)
     phis = gen.make_walkers(P, n_w, seed=P.seed)
     sel = [p[:nb] for p in phis]
-    times = []
+    walls, fulls = [], []
     for it in range(args.warmup + args.steps):
         t = time.time()
         oracle.local_energy_lo(P.psi, Lbars, hbars, empty, sel)
@@ -468,20 +499,100 @@ def run_reference(args):
         t = time.time()
         oracle.local_energy_lo(P.psi, Lbars, hbars, fs, sel)
         t_sub = time.time() - t
-        t_full = t_base + max(t_sub - t_base, 0.0) / (sum(frac) / len(frac))
         if it >= args.warmup:
-            times.append(t_full)
-    dt = float(np.mean(times))
+            walls.append(t_base + t_sub)                                                   # what this iteration really took
+            fulls.append(t_base + max(t_sub - t_base, 0.0) / (sum(frac) / len(frac)))      # exchange scaled to all pairs
+    wall, dt = float(np.mean(walls)), float(np.mean(fulls))
     value = nb / dt
     sample = ("%d of %d walkers per step; exchange on %s of the i<=j pairs (stratified by |i-j|, own Jacobi factors), its time scaled to "
               "all pairs; Theta/one-body/Coulomb in full" % (nb, n_w, "+".join("%d/%d" % (len(f.r), len(oracle.all_pairs(o)[0])) for f, o in zip(fs, P.n_occ))))
+    # ms_per_step is the wall time MEASURED per iteration (two oracle calls on the sample); `value` is an estimate for the
+    # full pair list (the oracle's own SVD of every pair would take hours), hence "extrapolated": true.
     line = {"impl": "reference", "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "warmup": args.warmup, "ms_per_step": round(wall * 1e3, 2), "extrapolated": True,
+            "ms_per_step_all_pairs_estimate": round(dt * 1e3, 2),
+            "extrapolation": "value = sample walkers / (t_noexchange + (t_sample - t_noexchange) * all pairs / sampled pairs)",
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(cfg, reading, T, n_w)},
+            "config": {"workload": workload_name(cfg, reading, T, n_w), "N": P.N, "N_occ": list(P.n_occ)[:P.n_spin], "N_chol": int(P.L.shape[0]),
+                       "N_w_per_gpu": n_w, "T_SVD": T},
             "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "kind": "oracle", "cores": oracle.num_threads(), "sample": sample},
             "e2e": {"value": round(value, 3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+def run_cas_step(args):
+    """--cas-step N_DET: multi-determinant local-energy steps alone, for ncu captures of the k_cas_*
+    kernels: --walkers real walkers (default 400) of --config/--reading, 6 active virtuals, --cas-holes active occupied
+    columns, excitation rank <= --cas-exc, mode --cas-mode; one JSON line."""
+    import torch
+
+    import gen
+    import paper_2202_00832_b200 as lo
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    n_det, n_w, smw = args.cas_step, args.walkers or 400, args.cas_mode == "smw"
+    P = gen.make_problem(args.config, reading=args.reading)
+    T = args.threshold if args.threshold is not None else gen.CONFIGS[args.config].thresholds[0]
+    Tr = gen.make_cas_trial(P, n_virt=6, n_act_occ=args.cas_holes, n_det=n_det, max_exc=args.cas_exc)
+    F = lo.Factors.setup(P.h, P.L, [Tr.C], T, device=0, max_walkers=n_w if smw else n_w * n_det, gpu_svd=True)
+    F.set_cas_trial(Tr.n_ref, Tr.holes, Tr.parts, Tr.coef, n_w, smw_energy=smw)
+    phi = torch.from_numpy(gen.make_walkers(P, n_w)[0]).cuda()
+    for _ in range(max(args.warmup, 1)):
+        E, st = F.local_energy_cas(phi)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        E, st = F.local_energy_cas(phi)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    info = F.info()
+    print(json.dumps({"cas_step": workload_name(args.config, args.reading, T, n_w), "mode": args.cas_mode, "n_det": n_det,
+                      "max_exc": args.cas_exc, "active_occupied": args.cas_holes, "tiles": info.n_tiles, "sum_rank": sum(info.sum_rank),
+                      "ms_per_step": round(ms, 4), "energies_per_s": round(n_w / (ms * 1e-3), 2),
+                      "determinant_energies_per_s": round(n_w * n_det / (ms * 1e-3), 2), "status_ok": bool((st == 0).all()),
+                      "E_L0": [E[0, 0].real.item(), E[0, 0].imag.item()]}), flush=True)
+
+
+def self_launch(n):
+    """Re-run this command line under torch.distributed.run with n ranks on this node (rendezvous on 127.0.0.1, a free
+    port); NCCL's INFO log stays on (stderr) so the rank count can be read off the run.  Returns the exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("OMP_NUM_THREADS", str(max(1, (os.cpu_count() or n) // n)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
+def run_launch_check(args):
+    """Bring up the ranks exactly as run_ours does (NCCL with one GPU per rank; gloo when the box has no GPU), take the
+    max over ranks of a per-rank number and the sum of the ranks' walker counts, print one line on rank 0."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2202_00832_b200.dist import max_over_ranks, sum_over_ranks
+    rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
+    cuda = torch.cuda.is_available()
+    dev = torch.device("cuda", local) if cuda else None
+    if cuda:
+        torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl" if cuda else "gloo", **({"device_id": dev} if cuda else {}))
+        dist.barrier()
+    ms = max_over_ranks(10.0 + rank, dev)
+    total = sum_over_ranks(float(args.walkers or 1), dev)
+    if rank == 0:
+        print(json.dumps({"launch_check": True, "n_gpus": world, "backend": ("nccl" if cuda else "gloo") if world > 1 else None,
+                          "max_ms": ms, "walkers_total": total}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def main():
@@ -503,8 +614,27 @@ def main():
                     "(N_w / cas real walkers; reported under \"next\", never part of `value`)")
     ap.add_argument("--sweep", action="store_true", help="threshold sweep (BASELINE.json:configs[4]): one JSON line per threshold")
     ap.add_argument("--sweep-exact-walkers", type=int, default=4, help="walkers whose exact E_K the oracle computes in --sweep")
+    ap.add_argument("--cas-step", type=int, default=0, help="run only multi-determinant steps with this many determinants (ncu target)")
+    ap.add_argument("--cas-mode", default="smw", choices=["smw", "direct"])
+    ap.add_argument("--cas-exc", type=int, default=4, help="maximum excitation rank of the synthetic CI expansion")
+    ap.add_argument("--cas-holes", type=int, default=6, help="active occupied (hole) columns of the synthetic CI expansion")
+    ap.add_argument("--launch-check", action="store_true", help="only bring up the N ranks (NCCL on GPUs, gloo without), reduce a dummy "
+                    "timing over them and print {\"n_gpus\": N, ...}; exercises the --gpus N launcher without the workload")
     args = ap.parse_args()
-    if args.sweep:
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    env_world = os.environ.get("WORLD_SIZE")
+    if env_world is not None and int(env_world) != args.gpus and args.impl == "ours":
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%s; launch one rank per GPU (torchrun --nproc-per-node %d) or drop --gpus"
+                         % (args.gpus, env_world, args.gpus))
+    if env_world is None and args.gpus > 1 and args.impl == "ours" and not args.sweep:
+        # `python bench.py --gpus N` without torchrun: start the N ranks here (one per GPU) and hand over
+        sys.exit(self_launch(args.gpus))
+    if args.launch_check:
+        run_launch_check(args)
+    elif args.cas_step > 0:
+        run_cas_step(args)
+    elif args.sweep:
         if args.config == 2 and "--config" not in " ".join(sys.argv):
             args.config = 4
         run_sweep(args)

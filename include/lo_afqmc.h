@@ -39,8 +39,7 @@ typedef enum {
     LO_EINVAL = 1,    /* bad shape / NULL / misaligned pointer / n_w > max_walkers: nothing was launched */
     LO_ENOMEM = 2,    /* host or device allocation failed */
     LO_ECUDA = 3,     /* a CUDA call failed, or the factor set has no device (built with device < 0) */
-    LO_ESINGULAR = 4, /* reserved (singular overlaps are per-walker data, see walker_status) */
-    LO_EINTERNAL = 5
+    LO_EINTERNAL = 5  /* the setup SVD did not converge (see lo_last_error) */
 } lo_status;
 
 typedef struct {
@@ -57,6 +56,8 @@ typedef struct {
     int device, max_walkers;
     int setup_on_gpu;                /* 1 when pair Gram + SVD ran on the device */
     long long n_tiles;               /* row tiles of the exchange grouped GEMM */
+    int svd_sweeps_max;              /* pair-block SVD: most sweeps any block took (incl. the final checking sweep) */
+    double svd_offdiag_max;          /* and the largest normalised off-diagonal |g_p.g_q|/(|g_p||g_q|) left at the end */
 } lo_info;
 
 /* Kernel indices for lo_timing_get */
@@ -108,7 +109,11 @@ lo_status lo_local_energy(const lo_factors* f, int n_w, const void* phi_a, const
 
 /* Same computation with HOST buffers: copies phi to the device, runs lo_local_energy, copies
  * E[n_w][4] = {E_L, E1, E_J, E_K} (complex128) and status back, and synchronises.  Pinned host memory makes the
- * copies asynchronous with respect to each other; pageable memory works too. */
+ * copies asynchronous with respect to each other; pageable memory works too.
+ * The batch runs in up to 4 walker chunks: the host-to-device copies go on a private stream that first waits for
+ * everything already queued on `stream`, the kernels of chunk c run on `stream` under the copy of chunk c+1.  Both streams
+ * are synchronised before the call returns, also when it fails.  Calls on one handle must be serialised by the caller
+ * (one workspace).  After this call lo_coulomb_x holds the X of the LAST chunk only (columns 0.. of that chunk). */
 lo_status lo_local_energy_host(const lo_factors* f, int n_w, const void* phi_a_host, const void* phi_b_host,
                                void* E_host, int* status_host, void* stream);
 

@@ -16,7 +16,7 @@ from . import build as _build
 LO_SETUP_GPU_SVD = 1
 LO_SETUP_PROPAGATOR = 2
 K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
-_STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 4: "LO_ESINGULAR", 5: "LO_EINTERNAL"}
+_STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_local_energy",
            "lo_local_energy_host", "lo_set_cas_trial", "lo_set_cas_trial_beta", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
            "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
@@ -33,7 +33,7 @@ class LoInfo(C.Structure):
                 ("n_pairs", C.c_longlong * 2), ("sum_rank", C.c_longlong * 2), ("sum_rank_padded", C.c_longlong),
                 ("max_rank", C.c_int), ("min_rank", C.c_int), ("factor_bytes", C.c_ulonglong), ("lbar_bytes", C.c_ulonglong),
                 ("workspace_bytes", C.c_ulonglong), ("threshold", C.c_double), ("device", C.c_int), ("max_walkers", C.c_int),
-                ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong)]
+                ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong), ("svd_sweeps_max", C.c_int), ("svd_offdiag_max", C.c_double)]
 
 
 _lib = None
@@ -174,18 +174,43 @@ class Factors:
         _check(lib().lo_retruncate(self._h, float(threshold), C.byref(out)))
         return Factors(out.value)
 
+    def _check_phis(self, phis, n_cols, what):
+        """Argument checks the C ABI cannot make on raw pointers: dtype, device, shape [n_w, N, n_cols[s]] per spin and one
+        n_w for all spins.  Returns (contiguous tensors, n_w, device)."""
+        import torch
+        info = self.info()
+        if len(phis) != len(n_cols):
+            raise LoError(1, "%s: %d walker tensor(s) given, the factor set needs %d" % (what, len(phis), len(n_cols)))
+        out = []
+        for s, p in enumerate(phis):
+            if not isinstance(p, torch.Tensor) or p.dtype != torch.complex128 or not p.is_cuda:
+                raise LoError(1, "%s: phi must be a CUDA complex128 tensor" % what)
+            if p.device.index != info.device:
+                raise LoError(1, "%s: phi is on cuda:%s, the factor set on cuda:%d" % (what, p.device.index, info.device))
+            if p.dim() != 3 or p.shape[1] != info.N or p.shape[2] != n_cols[s] or p.shape[0] != phis[0].shape[0]:
+                raise LoError(1, "%s: phi[%d] has shape %s, expected [n_w=%d, N=%d, %d]" % (what, s, tuple(p.shape), phis[0].shape[0], info.N, n_cols[s]))
+            out.append(p if p.is_contiguous() else p.contiguous())
+        return out, int(phis[0].shape[0]), phis[0].device
+
+    @staticmethod
+    def _on_stream(stream, dev, *tensors):
+        """Tensors allocated by the caching allocator on the current stream but used on `stream`: tell the allocator."""
+        import torch
+        if stream is not None and stream != torch.cuda.current_stream(dev):
+            for t in tensors:
+                if t is not None:
+                    t.record_stream(stream)
+
     def local_energy(self, phis, parts=True, status=True, stream=None):
         """lo_local_energy on torch CUDA tensors phis = [phi_a(, phi_b)], complex128 [n_w,N,O].  Asynchronous on the
         current (or given) torch stream.  Returns (E_L, E1, E_J, E_K, status) torch tensors (None where not requested)."""
         import torch
-        phis = [p if p.is_contiguous() else p.contiguous() for p in phis]
-        for p in phis:
-            if p.dtype != torch.complex128 or not p.is_cuda:
-                raise LoError(1, "phi must be a CUDA complex128 tensor")
-        n_w, dev = phis[0].shape[0], phis[0].device
+        info = self.info()
+        phis, n_w, dev = self._check_phis(list(phis), list(info.n_occ)[:info.n_spin], "local_energy")
         s = torch.cuda.current_stream(dev) if stream is None else stream
         E = torch.empty((4 if parts else 1, n_w), dtype=torch.complex128, device=dev)
         st_t = torch.empty(n_w, dtype=torch.int32, device=dev) if status else None
+        self._on_stream(stream, dev, E, st_t, *phis)
         ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
         _check(lib().lo_local_energy(self._h, n_w, ptr(phis[0]), ptr(phis[1]) if len(phis) == 2 else None, ptr(E[0]),
                                      ptr(E[1]) if parts else None, ptr(E[2]) if parts else None, ptr(E[3]) if parts else None,
@@ -196,7 +221,16 @@ class Factors:
         """lo_local_energy_host: numpy (or pinned torch CPU) complex128 inputs [n_w,N,O]; copies in, runs, copies
         E [n_w,4] = (E_L,E1,E_J,E_K) and status back, synchronises."""
         import torch
+        info = self.info()
         n_w = phis_host[0].shape[0]
+        if len(phis_host) != info.n_spin:
+            raise LoError(1, "local_energy_host: %d walker array(s) given, the factor set needs %d" % (len(phis_host), info.n_spin))
+        for sp, a in enumerate(phis_host):
+            if tuple(a.shape) != (n_w, info.N, info.n_occ[sp]) or str(a.dtype).split(".")[-1] != "complex128":
+                raise LoError(1, "local_energy_host: phi[%d] must be complex128 [n_w=%d, N=%d, %d], got %s %s" % (
+                    sp, n_w, info.N, info.n_occ[sp], a.dtype, tuple(a.shape)))
+            if not (a.is_contiguous() if hasattr(a, "is_contiguous") else a.flags["C_CONTIGUOUS"]):
+                raise LoError(1, "local_energy_host: phi[%d] must be contiguous" % sp)
         if E_host is None:
             E_host = np.empty((n_w, 4), dtype=np.complex128)
         if status_host is None:
@@ -226,26 +260,27 @@ class Factors:
         n_det, max_exc = holes.shape
         _check(lib().lo_set_cas_trial(self._h, int(n_ref), n_det, max_exc, holes.ctypes.data, parts.ctypes.data, coef.ctypes.data,
                                       int(max_real_walkers), 1 if smw_energy else 0))
+        self._cas_n_ref = [int(n_ref)]
 
     def set_cas_trial_beta(self, n_ref_b, holes_b, parts_b):
         """lo_set_cas_trial_beta: beta strings of an unrestricted trial (after set_cas_trial with the alpha strings)."""
         holes_b, parts_b = _np(holes_b, np.int32), _np(parts_b, np.int32)
         _check(lib().lo_set_cas_trial_beta(self._h, int(n_ref_b), holes_b.ctypes.data, parts_b.ctypes.data))
+        self._cas_n_ref = [self._cas_n_ref[0], int(n_ref_b)]
 
     def local_energy_cas(self, phi, phi_b=None, stream=None):
         """lo_local_energy_cas on a torch CUDA complex128 tensor [n_w, N, n_ref]; returns (E [5, n_w] = E_L, E1, E_J,
         E_K, overlap ratio; status [n_w]) torch tensors.  Asynchronous on the current (or given) stream."""
         import torch
-        phi = phi if phi.is_contiguous() else phi.contiguous()
-        if phi.dtype != torch.complex128 or not phi.is_cuda:
-            raise LoError(1, "phi must be a CUDA complex128 tensor")
-        n_w, dev = phi.shape[0], phi.device
+        if getattr(self, "_cas_n_ref", None) is None:
+            raise LoError(1, "local_energy_cas: call set_cas_trial first")
+        phis, n_w, dev = self._check_phis([phi] if phi_b is None else [phi, phi_b], self._cas_n_ref, "local_energy_cas")
+        phi, phi_b = phis[0], (phis[1] if phi_b is not None else None)
         s = torch.cuda.current_stream(dev) if stream is None else stream
         E = torch.empty((5, n_w), dtype=torch.complex128, device=dev)
         st_t = torch.empty(n_w, dtype=torch.int32, device=dev)
+        self._on_stream(stream, dev, E, st_t, *phis)
         ptr = lambda t: C.c_void_p(t.data_ptr())
-        if phi_b is not None:
-            phi_b = phi_b if phi_b.is_contiguous() else phi_b.contiguous()
         _check(lib().lo_local_energy_cas(self._h, n_w, ptr(phi), ptr(phi_b) if phi_b is not None else None, ptr(E[0]), ptr(E[1]), ptr(E[2]), ptr(E[3]), ptr(E[4]), ptr(st_t),
                                          C.c_void_p(s.cuda_stream)))
         return E, st_t
@@ -258,10 +293,14 @@ class Factors:
         """lo_propagator: x = torch CUDA complex128 [n_w, n_chol] (shifted auxiliary fields); forms
         B_w = sum_g x[w,g] L^g into the library's buffer (see propagator_buffer / propagator_host).  Asynchronous."""
         import torch
-        if x.dtype != torch.complex128 or not x.is_cuda:
-            raise LoError(1, "x must be a CUDA complex128 tensor")
+        info = self.info()
+        if x.dtype != torch.complex128 or not x.is_cuda or x.device.index != info.device:
+            raise LoError(1, "propagator: x must be a complex128 tensor on cuda:%d" % info.device)
+        if x.dim() != 2 or x.shape[1] != info.n_chol:
+            raise LoError(1, "propagator: x has shape %s, expected [n_w, n_chol=%d]" % (tuple(x.shape), info.n_chol))
         x = x if x.is_contiguous() else x.contiguous()
         s = torch.cuda.current_stream(x.device) if stream is None else stream
+        self._on_stream(stream, x.device, x)
         _check(lib().lo_propagator(self._h, int(x.shape[0]), C.c_void_p(x.data_ptr()), C.c_void_p(s.cuda_stream)))
         return x
 

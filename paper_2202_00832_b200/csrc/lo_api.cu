@@ -111,65 +111,6 @@ void host_pair_gram_t(int N, int n_chol, int O_tot, const double* Lbar, int oi, 
     }
 }
 
-// ---- host one-sided Jacobi SVD (Hestenes) with round-robin (tournament) ordering.
-// In: G[q][:] = column q of Y (n vectors of length n).  Rotations orthogonalise the vectors; V accumulates them.
-// Out: order[] sorts the vectors by norm (descending); sigma[K] = |G[order[K]]|; U row K = G[order[K]]/sigma;
-//      W row K = V[order[K]]  (Y v_K = sigma_K u_K).
-void host_jacobi(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order) {
-    std::fill(V, V + (size_t)n * n, 0.0);
-    for (int c = 0; c < n; ++c) V[(size_t)c * n + c] = 1.0;
-    double fro2 = 0;
-    for (size_t k = 0; k < (size_t)n * n; ++k) fro2 += G[k] * G[k];
-    const double tiny2 = fro2 * 1e-30, tol = 1e-15;
-    const int m = n + (n & 1);   // players (one dummy if n is odd)
-    for (int sweep = 0; sweep < 60; ++sweep) {
-        int rotations = 0;
-        for (int round = 0; round < m - 1; ++round) {
-            for (int k = 0; k < m / 2; ++k) {
-                int p, q;
-                if (k == 0) { p = m - 1; q = round; }
-                else { p = (round + k) % (m - 1); q = (round - k + (m - 1)) % (m - 1); }
-                if (p >= n || q >= n) continue;
-                if (p > q) std::swap(p, q);
-                double* gp = G + (size_t)p * n;
-                double* gq = G + (size_t)q * n;
-                double a = 0, b = 0, c = 0;
-                for (int e = 0; e < n; ++e) { a += gp[e] * gp[e]; b += gq[e] * gq[e]; c += gp[e] * gq[e]; }
-                if (a <= tiny2 || b <= tiny2) continue;
-                if (std::fabs(c) <= tol * std::sqrt(a * b)) continue;
-                ++rotations;
-                const double zeta = (b - a) / (2.0 * c);
-                const double t = (zeta >= 0 ? 1.0 : -1.0) / (std::fabs(zeta) + std::sqrt(1.0 + zeta * zeta));
-                const double cs = 1.0 / std::sqrt(1.0 + t * t), sn = cs * t;
-                for (int e = 0; e < n; ++e) {
-                    const double x = gp[e], y = gq[e];
-                    gp[e] = cs * x - sn * y;
-                    gq[e] = sn * x + cs * y;
-                }
-                double* vp = V + (size_t)p * n;
-                double* vq = V + (size_t)q * n;
-                for (int e = 0; e < n; ++e) {
-                    const double x = vp[e], y = vq[e];
-                    vp[e] = cs * x - sn * y;
-                    vq[e] = sn * x + cs * y;
-                }
-            }
-        }
-        if (rotations == 0) break;
-    }
-    std::vector<double> nrm(n);
-    for (int c = 0; c < n; ++c) {
-        double a = 0;
-        for (int e = 0; e < n; ++e) a += G[(size_t)c * n + e] * G[(size_t)c * n + e];
-        nrm[c] = std::sqrt(a);
-    }
-    order.resize(n);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return nrm[x] > nrm[y]; });
-    sigma.resize(n);
-    for (int K = 0; K < n; ++K) sigma[K] = nrm[order[K]];
-}
-
 struct PairRec {
     int spin, i, j, r;
     int x;            // index of the pair inside the batch being packed (source of its rows)
@@ -336,6 +277,7 @@ lo_status alloc_workspace(lo_factors* f) {
     f->workspace_bytes = total;
     CK(cudaStreamCreateWithFlags(&f->copyStream, cudaStreamNonBlocking));
     for (int c = 0; c < LO_HOST_CHUNKS; ++c) CK(cudaEventCreateWithFlags(&f->evCopy[c], cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&f->evEnter, cudaEventDisableTiming));
     lo_status st = make_tmap(&f->tmTheta, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 128);
     if (st == LO_OK) st = make_tmap(&f->tmTheta32, f->dThT, f->N_pad, (unsigned long long)f->O_tot * ldw, 32);
     if (st == LO_OK && f->dXT) st = make_tmap(&f->tmXT, f->dXT, (unsigned long long)f->ops->Xk_pad, ldw, 128);
@@ -389,6 +331,16 @@ lo_status upload_lt(lo_factors* f, const double* L) {
     return make_tmap(&ops.tmLt, ops.dLt, ld, (unsigned long long)ops.tri_pad, CO_BM);
 }
 
+// frees every device array of a multi-determinant plan and the plan itself
+void free_cas_plan(CasPlan* c) {
+    if (!c) return;
+    void* cp[] = {c->dHoles, c->dParts, c->dCoef, c->dTh0, c->dA0, c->dT, c->dG, c->dWd, c->dEv, c->dSt0, c->dHoleIdx, c->dKind, c->dS, c->dH, c->dPart,
+                  c->dStV, c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B};
+    for (void* q : cp)
+        if (q) cudaFree(q);
+    delete c;
+}
+
 void free_all(lo_factors* f) {
     if (!f) return;
     if (f->device >= 0) {
@@ -397,18 +349,12 @@ void free_all(lo_factors* f) {
         for (auto& ev : f->pool) { cudaEventDestroy(ev.e0); cudaEventDestroy(ev.e1); }
         f->bU.release();
         f->bW.release();
-        if (f->cas) {
-            void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd,
-                          f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS, f->cas->dH, f->cas->dPart, f->cas->dStV, f->cas->dHolesB, f->cas->dPartsB,
-                          f->cas->dTh0B, f->cas->dA0B, f->cas->dTB, f->cas->dGB, f->cas->dWdB, f->cas->dSt0B};
-            for (void* q : cp)
-                if (q) cudaFree(q);
-            delete f->cas;
-            f->cas = nullptr;
-        }
+        free_cas_plan(f->cas);
+        f->cas = nullptr;
         if (f->copyStream) cudaStreamDestroy(f->copyStream);
         for (int c = 0; c < LO_HOST_CHUNKS; ++c)
             if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
+        if (f->evEnter) cudaEventDestroy(f->evEnter);
         void* ptrs[] = {f->dWgt, f->dTiles, f->dTiles4, f->dEJLpart, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
                         f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1], f->dXT, f->dB};
         for (void* p : ptrs)
@@ -526,10 +472,13 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             if (split) k1 = std::min(k0 + B, bstart[blk + 1]);
             const int n = (int)(k1 - k0);
             for (int x = 0; x < n; ++x) { pairs[k0 + x].x = x; bi[x] = pairs[k0 + x].i; bj[x] = pairs[k0 + x].j; }
+            std::vector<SvdStat> stats_of_batch;
             if (on_gpu) {
-                st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data());
+                st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data(), &f->svd_stat);
                 if (st != LO_OK) break;
             } else {
+                stats_of_batch.assign(n, SvdStat());
+                std::vector<SvdStat>& stats = stats_of_batch;
 #pragma omp parallel
                 {
                     std::vector<double> G((size_t)N * N), V((size_t)N * N), sg;
@@ -537,7 +486,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
 #pragma omp for schedule(dynamic, 1)
                     for (int x = 0; x < n; ++x) {
                         host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[spin] + bi[x], f->o_base[spin] + bj[x], G.data());
-                        host_jacobi(N, G.data(), V.data(), sg, order);
+                        host_block_svd(N, G.data(), V.data(), sg, order, &stats[x]);
                         std::copy(sg.begin(), sg.end(), hSig.begin() + (size_t)x * N);
                         int r = 0;
                         while (r < N && sg[r] > threshold) ++r;
@@ -551,6 +500,18 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
                         }
                     }
                 }
+            }
+            if (!on_gpu)
+                for (const SvdStat& t : stats_of_batch) {
+                    f->svd_stat.sweeps = std::max(f->svd_stat.sweeps, t.sweeps);
+                    f->svd_stat.offdiag = std::max(f->svd_stat.offdiag, t.offdiag);
+                    if (!t.converged) f->svd_stat.converged = false;
+                }
+            if (!f->svd_stat.converged) {
+                set_error("lo_setup: the pair-block SVD did not converge within " + std::to_string(SVD_MAX_SWEEPS) + " sweeps (largest remaining "
+                          "normalised off-diagonal " + std::to_string(f->svd_stat.offdiag) + ")");
+                st = LO_EINTERNAL;
+                break;
             }
             for (int x = 0; x < n; ++x) {
                 const double* sg = &hSig[(size_t)x * N];
@@ -617,6 +578,7 @@ lo_status lo_info_get(const lo_factors* f, lo_info* info) {
     info->factor_bytes = f->factor_bytes; info->lbar_bytes = f->lbar_bytes; info->workspace_bytes = f->workspace_bytes;
     info->threshold = f->threshold; info->device = f->device; info->max_walkers = f->max_walkers;
     info->setup_on_gpu = f->setup_on_gpu; info->n_tiles = f->n_tiles;
+    info->svd_sweeps_max = f->svd_stat.sweeps; info->svd_offdiag_max = f->svd_stat.offdiag;
     return LO_OK;
 }
 
@@ -663,7 +625,7 @@ lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
     g->N = f->N; g->N_pad = f->N_pad; g->n_chol = f->n_chol; g->Xp = f->Xp; g->n_spin = f->n_spin; g->O_tot = f->O_tot;
     for (int s = 0; s < 2; ++s) { g->n_occ[s] = f->n_occ[s]; g->o_base[s] = f->o_base[s]; }
     g->threshold = looser; g->device = f->device; g->max_walkers = f->max_walkers; g->Wcap = f->Wcap; g->ldw = f->ldw;
-    g->num_sms = f->num_sms; g->setup_on_gpu = f->setup_on_gpu; g->ops = f->ops; g->lbar_bytes = f->lbar_bytes;
+    g->num_sms = f->num_sms; g->setup_on_gpu = f->setup_on_gpu; g->svd_stat = f->svd_stat; g->ops = f->ops; g->lbar_bytes = f->lbar_bytes;
     try {
         std::vector<PairRec> pairs;
         std::vector<size_t> bstart;
@@ -747,26 +709,39 @@ lo_status lo_local_energy_host(const lo_factors* fc, int n_w, const void* phi_a_
     const char* ph[2] = {static_cast<const char*>(phi_a_host), static_cast<const char*>(phi_b_host)};
     const int n_chunks = std::max(1, std::min(LO_HOST_CHUNKS, n_w / 128));
     const int per = ((n_w + n_chunks - 1) / n_chunks + WALKER_TILE - 1) / WALKER_TILE * WALKER_TILE;
-    for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
-        const int nc = std::min(per, n_w - w0);
-        for (int sp = 0; sp < f->n_spin; ++sp) {
-            const size_t per_w = (size_t)f->N * f->n_occ[sp] * 16;
-            CK(cudaMemcpyAsync(reinterpret_cast<char*>(f->dPhi[sp]) + w0 * per_w, ph[sp] + w0 * per_w, nc * per_w, cudaMemcpyHostToDevice, f->copyStream));
+    // The copies are ordered after everything already queued on the caller's stream (a stream-ordered producer of the
+    // pinned Phi buffer, or an earlier call on this handle that still reads the staging area).
+    CK(cudaEventRecord(f->evEnter, s));
+    CK(cudaStreamWaitEvent(f->copyStream, f->evEnter, 0));
+    auto body = [&]() -> lo_status {
+        for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
+            const int nc = std::min(per, n_w - w0);
+            for (int sp = 0; sp < f->n_spin; ++sp) {
+                const size_t per_w = (size_t)f->N * f->n_occ[sp] * 16;
+                CK(cudaMemcpyAsync(reinterpret_cast<char*>(f->dPhi[sp]) + w0 * per_w, ph[sp] + w0 * per_w, nc * per_w, cudaMemcpyHostToDevice, f->copyStream));
+            }
+            CK(cudaEventRecord(f->evCopy[c], f->copyStream));
         }
-        CK(cudaEventRecord(f->evCopy[c], f->copyStream));
+        for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
+            const int nc = std::min(per, n_w - w0);
+            CK(cudaStreamWaitEvent(s, f->evCopy[c], 0));
+            const char* pa = reinterpret_cast<const char*>(f->dPhi[0]) + (size_t)w0 * f->N * f->n_occ[0] * 16;
+            const char* pb = f->n_spin == 2 ? reinterpret_cast<const char*>(f->dPhi[1]) + (size_t)w0 * f->N * f->n_occ[1] * 16 : nullptr;
+            lo_status st2 = launch_local_energy(f, nc, pa, pb, nullptr, nullptr, nullptr, nullptr, f->dStatusOut + w0, f->dEout + (size_t)w0 * 8, s);
+            if (st2 != LO_OK) return st2;
+        }
+        CK(cudaMemcpyAsync(E_host, f->dEout, (size_t)n_w * 4 * 16, cudaMemcpyDeviceToHost, s));
+        if (status_host) CK(cudaMemcpyAsync(status_host, f->dStatusOut, (size_t)n_w * 4, cudaMemcpyDeviceToHost, s));
+        return LO_OK;
+    };
+    st = body();
+    // success or not, nothing of this call is left in flight when it returns (the host buffers are the caller's)
+    const cudaError_t e1 = cudaStreamSynchronize(f->copyStream), e2 = cudaStreamSynchronize(s);
+    if (st == LO_OK && (e1 != cudaSuccess || e2 != cudaSuccess)) {
+        set_error(std::string("lo_local_energy_host: ") + cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+        st = LO_ECUDA;
     }
-    for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
-        const int nc = std::min(per, n_w - w0);
-        CK(cudaStreamWaitEvent(s, f->evCopy[c], 0));
-        const char* pa = reinterpret_cast<const char*>(f->dPhi[0]) + (size_t)w0 * f->N * f->n_occ[0] * 16;
-        const char* pb = f->n_spin == 2 ? reinterpret_cast<const char*>(f->dPhi[1]) + (size_t)w0 * f->N * f->n_occ[1] * 16 : nullptr;
-        st = launch_local_energy(f, nc, pa, pb, nullptr, nullptr, nullptr, nullptr, f->dStatusOut + w0, f->dEout + (size_t)w0 * 8, s);
-        if (st != LO_OK) return st;
-    }
-    CK(cudaMemcpyAsync(E_host, f->dEout, (size_t)n_w * 4 * 16, cudaMemcpyDeviceToHost, s));
-    if (status_host) CK(cudaMemcpyAsync(status_host, f->dStatusOut, (size_t)n_w * 4, cudaMemcpyDeviceToHost, s));
-    CK(cudaStreamSynchronize(s));
-    return LO_OK;
+    return st;
 }
 
 lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld) {
@@ -787,22 +762,8 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode) {
     return LO_OK;
 }
 
-lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts, const double* coef,
-                           int max_real_walkers, int mode) {
-    if (!f || !holes || !parts || !coef) { set_error("lo_set_cas_trial: NULL argument"); return LO_EINVAL; }
-    if (f->device < 0) { set_error("lo_set_cas_trial: no device"); return LO_ECUDA; }
-    if (f->n_spin != 1 && mode != LO_CAS_DIRECT) {
-        set_error("lo_set_cas_trial: an unrestricted factor set (n_spin == 2) supports LO_CAS_DIRECT only");
-        return LO_EINVAL;
-    }
-    const int n_orb = f->n_occ[0];
-    if (mode != LO_CAS_DIRECT && mode != LO_CAS_SMW_ENERGY) { set_error("lo_set_cas_trial: mode must be LO_CAS_DIRECT or LO_CAS_SMW_ENERGY"); return LO_EINVAL; }
-    if (n_ref <= 0 || n_ref > n_orb || n_det <= 0 || max_exc <= 0 || max_exc > CAS_MAX_EXC || max_real_walkers <= 0 ||
-        (mode == LO_CAS_DIRECT && (long long)max_real_walkers * n_det > f->max_walkers) || max_real_walkers > f->max_walkers) {
-        set_error("lo_set_cas_trial: invalid sizes (need 0 < n_ref <= n_occ, 1 <= max_exc <= 8, max_real_walkers * n_det <= max_walkers "
-                  "in LO_CAS_DIRECT mode, max_real_walkers <= max_walkers)");
-        return LO_EINVAL;
-    }
+// validates one spin's excitation lists (shared by lo_set_cas_trial and lo_set_cas_trial_beta)
+static lo_status check_strings(int n_det, int max_exc, int n_ref, int n_orb, const int* holes, const int* parts) {
     for (int d = 0; d < n_det; ++d) {
         bool ended = false;
         for (int k = 0; k < max_exc; ++k) {
@@ -813,31 +774,13 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
                 if (holes[(size_t)d * max_exc + l] == h || parts[(size_t)d * max_exc + l] == p) { set_error("lo_set_cas_trial: repeated hole or particle in one determinant"); return LO_EINVAL; }
         }
     }
-    // active set = the reference columns that are a hole in some determinant (the columns of A^-1 the SMW corrections touch)
-    std::vector<int> act;
-    for (size_t k = 0; k < (size_t)n_det * max_exc; ++k)
-        if (holes[k] >= 0 && std::find(act.begin(), act.end(), holes[k]) == act.end()) act.push_back(holes[k]);
-    std::sort(act.begin(), act.end());
-    if (mode == LO_CAS_SMW_ENERGY && act.size() > 6) {
-        set_error("lo_set_cas_trial: LO_CAS_SMW_ENERGY supports at most 6 distinct hole columns (active occupied orbitals); use LO_CAS_DIRECT");
-        return LO_EINVAL;
-    }
-    CK(cudaSetDevice(f->device));
-    if (f->cas) {
-        void* cp[] = {f->cas->dHoles, f->cas->dParts, f->cas->dCoef, f->cas->dTh0, f->cas->dA0, f->cas->dT, f->cas->dG, f->cas->dWd, f->cas->dEv, f->cas->dSt0, f->cas->dHoleIdx, f->cas->dKind, f->cas->dS,
-                      f->cas->dH, f->cas->dPart, f->cas->dStV, f->cas->dHolesB, f->cas->dPartsB, f->cas->dTh0B, f->cas->dA0B, f->cas->dTB,
-                      f->cas->dGB, f->cas->dWdB, f->cas->dSt0B};
-        for (void* q : cp)
-            if (q) cudaFree(q);
-        delete f->cas;
-        f->cas = nullptr;
-    }
-    CasPlan* c = new (std::nothrow) CasPlan();
-    if (!c) { set_error("lo_set_cas_trial: out of host memory"); return LO_ENOMEM; }
-    f->cas = c;
-    c->n_ref = n_ref; c->n_det = n_det; c->max_exc = max_exc; c->n_virt = n_orb - n_ref; c->max_real = max_real_walkers;
-    c->W0cap = round_up(max_real_walkers, WALKER_TILE);
-    const size_t nv = (size_t)max_real_walkers * n_det, ne = (size_t)n_det * max_exc;
+    return LO_OK;
+}
+
+// allocates and fills plan `c` (already sized); any failure leaves the partial allocations in `c` for the caller to free
+static lo_status fill_cas_plan(lo_factors* f, CasPlan* c, const int* holes, const int* parts, const double* coef, const std::vector<int>& act) {
+    const int n_orb = f->n_occ[0], n_ref = c->n_ref, n_det = c->n_det, max_exc = c->max_exc;
+    const size_t nv = (size_t)c->max_real * n_det, ne = (size_t)n_det * max_exc;
     auto al = [&](void** p, size_t bytes) -> cudaError_t {
         cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16));
         if (e == cudaSuccess) e = cudaMemset(*p, 0, std::max<size_t>(bytes, 16));
@@ -856,9 +799,7 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     CK(cudaMemcpy(c->dHoles, holes, ne * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->dParts, parts, ne * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->dCoef, coef, (size_t)n_det * 8, cudaMemcpyHostToDevice));
-    c->mode = mode;
-    c->n_act = (int)act.size();
-    if (mode == LO_CAS_SMW_ENERGY) {
+    if (c->mode == LO_CAS_SMW_ENERGY) {
         const int na_pad = c->n_act <= 2 ? 2 : (c->n_act <= 4 ? 4 : 6);
         c->NP = 2 + na_pad;
         std::vector<int> hidx(ne + 8, -1);
@@ -879,7 +820,7 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
         CK(al((void**)&c->dHoleIdx, hidx.size() * 4));
         CK(al((void**)&c->dKind, kind.size()));
         CK(al((void**)&c->dStV, nv * 4));
-        CK(al((void**)&c->dS, (size_t)std::max<long long>(f->n_tiles, 1) * max_real_walkers * c->NP * c->NP * 16));
+        CK(al((void**)&c->dS, (size_t)std::max<long long>(f->n_tiles, 1) * c->max_real * c->NP * c->NP * 16));
         CK(al((void**)&c->dH, (size_t)c->W0cap * n_orb * 9 * 16));
         CK(al((void**)&c->dPart, (size_t)std::max(c->n_chunks, 1) * nv * 2 * 16));
         CK(cudaMemcpy(c->dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
@@ -890,18 +831,50 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     return LO_OK;
 }
 
-// validates one spin's excitation lists (shared by lo_set_cas_trial and lo_set_cas_trial_beta)
-static lo_status check_strings(int n_det, int max_exc, int n_ref, int n_orb, const int* holes, const int* parts) {
-    for (int d = 0; d < n_det; ++d) {
-        bool ended = false;
-        for (int k = 0; k < max_exc; ++k) {
-            const int h = holes[(size_t)d * max_exc + k], p = parts[(size_t)d * max_exc + k];
-            if (h < 0 || p < 0) { if (h >= 0 || p >= 0) { set_error("lo_set_cas_trial: hole/particle lists of different length"); return LO_EINVAL; } ended = true; continue; }
-            if (ended || h >= n_ref || p < n_ref || p >= n_orb) { set_error("lo_set_cas_trial: hole must be < n_ref, particle in [n_ref, n_occ), -1 padding at the end"); return LO_EINVAL; }
-            for (int l = 0; l < k; ++l)
-                if (holes[(size_t)d * max_exc + l] == h || parts[(size_t)d * max_exc + l] == p) { set_error("lo_set_cas_trial: repeated hole or particle in one determinant"); return LO_EINVAL; }
-        }
+lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts, const double* coef,
+                           int max_real_walkers, int mode) {
+    if (!f || !holes || !parts || !coef) { set_error("lo_set_cas_trial: NULL argument"); return LO_EINVAL; }
+    if (f->device < 0) { set_error("lo_set_cas_trial: no device"); return LO_ECUDA; }
+    if (f->n_spin != 1 && mode != LO_CAS_DIRECT) {
+        set_error("lo_set_cas_trial: an unrestricted factor set (n_spin == 2) supports LO_CAS_DIRECT only");
+        return LO_EINVAL;
     }
+    const int n_orb = f->n_occ[0];
+    if (mode != LO_CAS_DIRECT && mode != LO_CAS_SMW_ENERGY) { set_error("lo_set_cas_trial: mode must be LO_CAS_DIRECT or LO_CAS_SMW_ENERGY"); return LO_EINVAL; }
+    if (n_ref <= 0 || n_ref > n_orb || n_det <= 0 || max_exc <= 0 || max_exc > CAS_MAX_EXC || max_real_walkers <= 0 ||
+        (mode == LO_CAS_DIRECT && (long long)max_real_walkers * n_det > f->max_walkers) || max_real_walkers > f->max_walkers) {
+        set_error("lo_set_cas_trial: invalid sizes (need 0 < n_ref <= n_occ, 1 <= max_exc <= 8, max_real_walkers * n_det <= max_walkers "
+                  "in LO_CAS_DIRECT mode, max_real_walkers <= max_walkers)");
+        return LO_EINVAL;
+    }
+    lo_status st = check_strings(n_det, max_exc, n_ref, n_orb, holes, parts);
+    if (st != LO_OK) return st;
+    // active set = the reference columns that are a hole in some determinant (the columns of A^-1 the SMW corrections touch)
+    std::vector<int> act;
+    for (size_t k = 0; k < (size_t)n_det * max_exc; ++k)
+        if (holes[k] >= 0 && std::find(act.begin(), act.end(), holes[k]) == act.end()) act.push_back(holes[k]);
+    std::sort(act.begin(), act.end());
+    if (mode == LO_CAS_SMW_ENERGY && act.size() > 6) {
+        set_error("lo_set_cas_trial: LO_CAS_SMW_ENERGY supports at most 6 distinct hole columns (active occupied orbitals); use LO_CAS_DIRECT");
+        return LO_EINVAL;
+    }
+    CK(cudaSetDevice(f->device));
+    // The new plan is built aside and installed only when every allocation and upload has succeeded; on failure the
+    // partial plan is freed and the previous trial (if any) stays in place.
+    CasPlan* c = new (std::nothrow) CasPlan();
+    if (!c) { set_error("lo_set_cas_trial: out of host memory"); return LO_ENOMEM; }
+    c->n_ref = n_ref; c->n_det = n_det; c->max_exc = max_exc; c->n_virt = n_orb - n_ref; c->max_real = max_real_walkers;
+    c->W0cap = round_up(max_real_walkers, WALKER_TILE);
+    c->mode = mode;
+    c->n_act = (int)act.size();
+    st = fill_cas_plan(f, c, holes, parts, coef, act);
+    if (st != LO_OK) {
+        free_cas_plan(c);
+        cudaGetLastError();      // an allocation failure is not sticky; clear it
+        return st;
+    }
+    free_cas_plan(f->cas);
+    f->cas = c;
     return LO_OK;
 }
 
@@ -966,7 +939,7 @@ lo_status lo_propagator(const lo_factors* fc, int n_w, const void* x_dev, void* 
     if (!fc || !x_dev) { set_error("lo_propagator: NULL argument"); return LO_EINVAL; }
     if (fc->device < 0) { set_error("lo_propagator: no device"); return LO_ECUDA; }
     if (!fc->ops->dLt || !fc->dB) { set_error("lo_propagator: the factor set was built without LO_SETUP_PROPAGATOR"); return LO_EINVAL; }
-    if (n_w <= 0 || n_w > fc->max_walkers) { set_error("lo_propagator: n_w out of range (1..max_walkers)"); return LO_EINVAL; }
+    if (n_w <= 0 || n_w > fc->max_walkers || n_w > 65535) { set_error("lo_propagator: n_w out of range (1..min(max_walkers, 65535): grid dimension of the field-packing kernel)"); return LO_EINVAL; }
     if ((uintptr_t)x_dev & 15) { set_error("lo_propagator: x must be 16-byte aligned"); return LO_EINVAL; }
     lo_factors* f = const_cast<lo_factors*>(fc);
     CK(cudaSetDevice(f->device));

@@ -104,6 +104,15 @@ struct CasPlan {
     CUtensorMap tmTh0;                          // Theta0^T panels [n_orb*2*W0cap][N_pad], box 16 x 16
 };
 
+// Pair-block SVD (lo_svd.cu)
+constexpr int SVD_B = 16;            // rows per block (a subproblem = 2 blocks = 32 rows)
+constexpr int SVD_MAX_SWEEPS = 40;
+struct SvdStat {
+    int sweeps = 0;          // sweeps performed (the last one only checks)
+    double offdiag = 0;      // largest |g_p.g_q| / (|g_p||g_q|) over the non-null rows seen in the last sweep
+    bool converged = true;
+};
+
 struct TimingEvent {
     cudaEvent_t e0, e1;
     int kind;
@@ -116,6 +125,7 @@ struct lo_factors {
     double threshold = 0;
     int device = -1, max_walkers = 0, Wcap = 0, ldw = 0, num_sms = 0;
     int setup_on_gpu = 0;
+    lo::SvdStat svd_stat;                // worst case over all pair blocks of lo_setup
     // pair bookkeeping, natural (row-major i<=j) order per spin
     std::vector<int> rank[2];
     std::vector<long long> row_off[2];   // first packed row of the pair
@@ -153,6 +163,7 @@ struct lo_factors {
     CUtensorMap tmXT;
     cudaStream_t copyStream = nullptr;     // host variant: H2D of walker chunk c+1 overlaps the kernels of chunk c
     cudaEvent_t evCopy[LO_HOST_CHUNKS] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t evEnter = nullptr;         // host variant: the copy stream waits for what the caller's stream already holds
     unsigned long long factor_bytes = 0, lbar_bytes = 0, workspace_bytes = 0;
     int last_n_w = 0;
     lo::CasPlan* cas = nullptr;
@@ -181,11 +192,16 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const
 // 2D fp64 tensor map over a row-major [rows][inner] array, box [box_rows][16], 128-byte swizzle, zero OOB fill.
 lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner, unsigned long long rows, unsigned box_rows);   // cudaFuncSetAttribute for the big-smem kernels (once per process/device)
 
-// GPU setup (lo_setup_gpu.cu): pair Gram matrices + one-sided Jacobi SVD for a batch of pairs of one spin.
+// Pair-block SVD (lo_svd.cu): block one-sided Jacobi with Gram subproblems, host and device versions.
+std::vector<int> svd_schedule(int n_blocks);
+void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, SvdStat* stat);
+cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, int* dSweeps, double* dOff, cudaStream_t stream);
+
+// GPU setup (lo_setup_gpu.cu): pair Gram matrices + block-Jacobi SVD (lo_svd.cu) for a batch of pairs of one spin.
 // For the n listed pairs: returns sigma (descending, [n][N]) on the host and leaves the sorted U/W rows on the
 // device in tmpU/tmpW ([n][N][N_pad]).  tmpY/tmpV are scratch of the same size.
 lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV,
-                       double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma);
+                       double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma, SvdStat* stat);
 size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad);
 // dst[rec.dst_row + K][:] = src[rec.src_row + K][:] for K < rec.r, every rec of the host table (rows of N_pad doubles).
 lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table, int n, int N_pad);

@@ -1,7 +1,7 @@
-// lo_setup_gpu.cu -- device side of lo_setup (flag LO_SETUP_GPU_SVD): pair blocks Y^{ij} and their
-// SVDs (Eq. 18) by a batched one-sided (Hestenes) Jacobi method, one CTA per pair block.
-// Setup is untimed; these kernels are written for robustness and a bounded run time at the
-// pentacene-sized config (2701 SVDs of 378 x 378), not for roofline.
+// lo_setup_gpu.cu -- device side of lo_setup (flag LO_SETUP_GPU_SVD): pair blocks Y^{ij}, the epilogue of
+// their SVDs (Eq. 18; the iteration itself is the block Jacobi method of lo_svd.cu) and the packing copies.
+// Setup is untimed.
+#include <algorithm>
 #include <cmath>
 
 #include "lo_internal.h"
@@ -61,83 +61,6 @@ __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
-}
-
-// One CTA (512 threads = 16 warps) per matrix.  Vectors g_c = G[c][0..N) are orthogonalised by plane rotations in
-// round-robin (tournament) order, N/2 disjoint pairs per round spread over the warps; V accumulates the rotations.
-__global__ void __launch_bounds__(512) k_jacobi(double* __restrict__ Gall, double* __restrict__ Vall, int N, int N_pad, int max_sweeps,
-                                                int* __restrict__ sweeps_out) {
-    __shared__ int s_rot;
-    __shared__ double s_red[16];
-    __shared__ double s_tiny2;
-    const int x = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    double* G = Gall + (size_t)x * N * N_pad;
-    double* V = Vall + (size_t)x * N * N_pad;
-    // V = I, Frobenius norm
-    double fro = 0;
-    for (size_t e = tid; e < (size_t)N * N_pad; e += 512) {
-        int r = (int)(e / N_pad), c = (int)(e % N_pad);
-        V[e] = (r == c) ? 1.0 : 0.0;
-        double g = G[e];
-        fro += g * g;
-    }
-    fro = warp_sum(fro);
-    if (lane == 0) s_red[warp] = fro;
-    __syncthreads();
-    if (tid == 0) {
-        double t = 0;
-        for (int q = 0; q < 16; ++q) t += s_red[q];
-        s_tiny2 = t * 1e-30;
-    }
-    __syncthreads();
-    const double tiny2 = s_tiny2, tol = 1e-15;
-    const int m = N + (N & 1);
-    int sweep = 0;
-    for (; sweep < max_sweeps; ++sweep) {
-        if (tid == 0) s_rot = 0;
-        __syncthreads();
-        int myrot = 0;
-        for (int round = 0; round < m - 1; ++round) {
-            for (int k = warp; k < m / 2; k += 16) {
-                int p, q;
-                if (k == 0) { p = m - 1; q = round; }
-                else { p = (round + k) % (m - 1); q = (round - k + (m - 1)) % (m - 1); }
-                if (p >= N || q >= N) continue;
-                if (p > q) { int t = p; p = q; q = t; }
-                double* gp = G + (size_t)p * N_pad;
-                double* gq = G + (size_t)q * N_pad;
-                double a = 0, b = 0, c = 0;
-                for (int e = lane; e < N; e += 32) {
-                    double xx = gp[e], yy = gq[e];
-                    a = fma(xx, xx, a); b = fma(yy, yy, b); c = fma(xx, yy, c);
-                }
-                a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
-                if (a <= tiny2 || b <= tiny2) continue;
-                if (fabs(c) <= tol * sqrt(a * b)) continue;
-                ++myrot;
-                const double zeta = (b - a) / (2.0 * c);
-                const double t = (zeta >= 0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-                const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
-                double* vp = V + (size_t)p * N_pad;
-                double* vq = V + (size_t)q * N_pad;
-                for (int e = lane; e < N; e += 32) {
-                    double xx = gp[e], yy = gq[e];
-                    gp[e] = cs * xx - sn * yy;
-                    gq[e] = sn * xx + cs * yy;
-                    double vx = vp[e], vy = vq[e];
-                    vp[e] = cs * vx - sn * vy;
-                    vq[e] = sn * vx + cs * vy;
-                }
-            }
-            __syncthreads();
-        }
-        if (lane == 0 && myrot) atomicAdd(&s_rot, myrot);
-        __syncthreads();
-        const int rot = s_rot;
-        __syncthreads();
-        if (rot == 0) break;
-    }
-    if (tid == 0 && sweeps_out) sweeps_out[x] = sweep;
 }
 
 // sigma_K = |g_{order[K]}| descending;  U row K = g/sigma;  W row K = v.
@@ -206,33 +129,46 @@ lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table
     return LO_OK;
 }
 
-size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad) { return (size_t)4 * N * N_pad * 8 + (size_t)N * 12; }
+size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad) { return (size_t)4 * N * N_pad * 8 + (size_t)N * 12 + 16; }
 
 lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV, double* tmpU,
-                       double* tmpW, double* dSigma, int* dOrder, double* hSigma) {
-#define GK(call)                                                                                      \
-    do {                                                                                              \
-        cudaError_t e_ = (call);                                                                      \
-        if (e_ != cudaSuccess) { set_error(std::string(#call) + ": " + cudaGetErrorString(e_)); return LO_ECUDA; } \
-    } while (0)
+                       double* tmpW, double* dSigma, int* dOrder, double* hSigma, SvdStat* stat) {
     const int N = f->N, N_pad = f->N_pad;
-    int *dpi = nullptr, *dpj = nullptr;
-    GK(cudaMalloc(&dpi, (size_t)n * 4));
-    GK(cudaMalloc(&dpj, (size_t)n * 4));
-    GK(cudaMemcpy(dpi, pi, (size_t)n * 4, cudaMemcpyHostToDevice));
-    GK(cudaMemcpy(dpj, pj, (size_t)n * 4, cudaMemcpyHostToDevice));
-    dim3 grid((N_pad + 63) / 64, (N + 63) / 64, n);
-    k_pair_gram<<<grid, 256>>>(f->ops->dLbar, f->n_chol, f->O_tot, N, N_pad, f->o_base[spin], dpi, dpj, tmpY);
-    GK(cudaGetLastError());
-    k_jacobi<<<n, 512>>>(tmpY, tmpV, N, N_pad, 60, nullptr);
-    GK(cudaGetLastError());
-    k_svd_finish<<<n, 512, (size_t)N * 8>>>(tmpY, tmpV, N, N_pad, dSigma, dOrder, tmpU, tmpW);
-    GK(cudaGetLastError());
-    GK(cudaMemcpy(hSigma, dSigma, (size_t)n * N * 8, cudaMemcpyDeviceToHost));
-    cudaFree(dpi);
-    cudaFree(dpj);
+    int *dpi = nullptr, *dpj = nullptr, *dSched = nullptr, *dSweeps = nullptr;
+    double* dOff = nullptr;
+    const std::vector<int> sched = svd_schedule((N + SVD_B - 1) / SVD_B);
+    std::vector<int> hSweeps(n);
+    std::vector<double> hOff(n);
+    cudaError_t e = cudaSuccess;
+    const char* where = "";
+    auto step = [&](cudaError_t r, const char* w) { if (e == cudaSuccess && r != cudaSuccess) { e = r; where = w; } return e == cudaSuccess; };
+    step(cudaMalloc(&dpi, (size_t)n * 4), "cudaMalloc") && step(cudaMalloc(&dpj, (size_t)n * 4), "cudaMalloc") &&
+        step(cudaMalloc(&dSched, sched.size() * 4), "cudaMalloc") && step(cudaMalloc(&dSweeps, (size_t)n * 4), "cudaMalloc") &&
+        step(cudaMalloc(&dOff, (size_t)n * 8), "cudaMalloc") &&
+        step(cudaMemcpy(dpi, pi, (size_t)n * 4, cudaMemcpyHostToDevice), "cudaMemcpy") &&
+        step(cudaMemcpy(dpj, pj, (size_t)n * 4, cudaMemcpyHostToDevice), "cudaMemcpy") &&
+        step(cudaMemcpy(dSched, sched.data(), sched.size() * 4, cudaMemcpyHostToDevice), "cudaMemcpy");
+    if (e == cudaSuccess) {
+        dim3 grid((N_pad + 63) / 64, (N + 63) / 64, n);
+        k_pair_gram<<<grid, 256>>>(f->ops->dLbar, f->n_chol, f->O_tot, N, N_pad, f->o_base[spin], dpi, dpj, tmpY);
+        step(cudaGetLastError(), "k_pair_gram");
+    }
+    if (e == cudaSuccess) step(launch_block_jacobi(tmpY, tmpV, n, N, N_pad, dSched, dSweeps, dOff, nullptr), "k_block_jacobi");
+    if (e == cudaSuccess) {
+        k_svd_finish<<<n, 512, (size_t)N * 8>>>(tmpY, tmpV, N, N_pad, dSigma, dOrder, tmpU, tmpW);
+        step(cudaGetLastError(), "k_svd_finish");
+    }
+    step(cudaMemcpy(hSigma, dSigma, (size_t)n * N * 8, cudaMemcpyDeviceToHost), "cudaMemcpy(sigma)") &&
+        step(cudaMemcpy(hSweeps.data(), dSweeps, (size_t)n * 4, cudaMemcpyDeviceToHost), "cudaMemcpy") &&
+        step(cudaMemcpy(hOff.data(), dOff, (size_t)n * 8, cudaMemcpyDeviceToHost), "cudaMemcpy");
+    cudaFree(dpi); cudaFree(dpj); cudaFree(dSched); cudaFree(dSweeps); cudaFree(dOff);      // on every path
+    if (e != cudaSuccess) { set_error(std::string("gpu_pair_svd: ") + where + ": " + cudaGetErrorString(e)); return LO_ECUDA; }
+    for (int x = 0; x < n; ++x) {
+        stat->sweeps = std::max(stat->sweeps, hSweeps[x]);
+        stat->offdiag = std::max(stat->offdiag, hOff[x]);
+        if (hSweeps[x] >= SVD_MAX_SWEEPS) stat->converged = false;
+    }
     return LO_OK;
-#undef GK
 }
 
 }  // namespace lo

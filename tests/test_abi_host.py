@@ -72,6 +72,56 @@ def test_host_factors_match_oracle(c1, c1_host):
         assert np.abs(U @ U.T - np.eye(r_or)).max() < 1e-12 and np.abs(W @ W.T - np.eye(r_or)).max() < 1e-12
 
 
+def lapack_pin(F, spin, Lbar, pairs, T, N):
+    """Pins the LIBRARY's factors of the listed pairs to LAPACK (numpy.linalg.svd of Y^{ij} = Lbar_i^T Lbar_j formed by
+    numpy; none of the repo's SVD routines, oracle or product, takes part): singular values to 1e-12 sigma_1, rank =
+    #(sigma > T) except where |sigma - T| <= 1e-10 sigma_max (DESIGN R13), truncated reconstruction U^T sigma W to
+    1e-11 sigma_1, orthonormal rows.  Returns the number of pairs whose rank sat inside the ambiguity band."""
+    ranks = F.ranks(spin)
+    O = int(round((np.sqrt(8 * len(ranks) + 1) - 1) / 2))
+    band = 0
+    for (i, j) in pairs:
+        k = i * O - i * (i - 1) // 2 + (j - i)
+        Y = Lbar[:, i, :].T @ Lbar[:, j, :]                      # Y^{ij}_pq = sum_g Lbar^g_ip Lbar^g_jq  (PAPER.md:133)
+        Ul, sl, Wl = np.linalg.svd(Y)
+        r_l = int((sl > T).sum())
+        r = int(ranks[k])
+        if r != r_l:
+            lo_, hi = min(r, r_l), max(r, r_l)
+            assert (np.abs(sl[lo_:hi] - T) <= 1e-10 * sl[0]).all(), (i, j, r, r_l)
+            band += 1
+        U, sg, W = F.factor_pair(spin, i, j)
+        assert sg.shape == (r,) and (np.diff(sg) <= 0).all()
+        assert np.abs(sg - sl[:r]).max(initial=0.0) <= 1e-12 * sl[0], (i, j)
+        rec_lib = (U.T * sg) @ W
+        rec_lap = (Ul[:, :r] * sl[:r]) @ Wl[:r]
+        assert np.abs(rec_lib - rec_lap).max(initial=0.0) <= 1e-11 * sl[0], (i, j)
+        if r:
+            assert np.abs(U @ U.T - np.eye(r)).max() < 1e-12 and np.abs(W @ W.T - np.eye(r)).max() < 1e-12, (i, j)
+    return band
+
+
+def test_host_factors_pinned_to_lapack(c1, c1_host):
+    """All 231 pair blocks of configs[1] (T = 1e-4), host setup path, against LAPACK."""
+    O = c1.n_occ[0]
+    Lbar = np.einsum("gpq,qi->gip", c1.L, c1.psi[0])             # PAPER.md:127, typed with numpy
+    band = lapack_pin(c1_host, 0, Lbar, [(i, j) for i in range(O) for j in range(i, O)], 1e-4, c1.N)
+    assert band <= 2
+
+
+def test_host_factors_low_rank_pinned_to_lapack():
+    """Rank-deficient blocks ("vector" reading: rank <= number of sites, the rest of the spectrum is rounding noise) and an
+    unrestricted set: the null space must neither be kept nor disturb the kept vectors."""
+    xyz, fns = gen.site_geometry(1)
+    P = gen.make_problem_from_geometry(xyz, fns, (9, 7), 200, seed=11, reading="vector")
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-6, device=-1, max_walkers=4)
+    for s in range(2):
+        O = P.n_occ[s]
+        Lbar = np.einsum("gpq,qi->gip", P.L, P.psi[s])
+        assert F.ranks(s).max() <= len(xyz)
+        lapack_pin(F, s, Lbar, [(i, j) for i in range(O) for j in range(i, O)], 1e-6, P.N)
+
+
 def test_factor_all_order_and_tiles(c1_host, c1):
     U, s, W = c1_host.factor_all()
     ranks = c1_host.ranks()

@@ -60,3 +60,24 @@ def test_two_rank_walker_sharding():
     got = [x for r in res for x in r[3]]
     assert np.array_equal(np.array(got), np.array(ref))          # shards tile the batch, same numbers
     assert all(r[4] == 11.0 for r in res) and all(r[5] == P.n_w for r in res)
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment must start 2 ranks itself (the flag
+    used to be ignored).  --launch-check runs the launcher and the rank bring-up without the workload (gloo here)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--launch-check", "--walkers", "7"],
+                         capture_output=True, text=True, env=env, timeout=300)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, res.stdout                        # rank 0 alone prints
+    assert lines[0]["n_gpus"] == 2 and lines[0]["max_ms"] == 11.0 and lines[0]["walkers_total"] == 14.0
+    # a world size that contradicts --gpus is refused, not silently run
+    env2 = dict(env, WORLD_SIZE="3", RANK="0", LOCAL_RANK="0")
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--launch-check"], capture_output=True, text=True,
+                         env=env2, timeout=120)
+    assert res.returncode != 0 and "WORLD_SIZE" in res.stderr
