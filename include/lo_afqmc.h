@@ -58,6 +58,8 @@ typedef struct {
     long long n_tiles;               /* row tiles of the exchange grouped GEMM */
     int svd_sweeps_max;              /* pair-block SVD: most sweeps any block took (incl. the final checking sweep) */
     double svd_offdiag_max;          /* and the largest normalised off-diagonal |g_p.g_q|/(|g_p||g_q|) left at the end */
+    double setup_seconds;            /* wall time of lo_setup, and of its pair Gram + SVD part */
+    double setup_svd_seconds;
 } lo_info;
 
 /* Kernel indices for lo_timing_get */

@@ -33,7 +33,8 @@ class LoInfo(C.Structure):
                 ("n_pairs", C.c_longlong * 2), ("sum_rank", C.c_longlong * 2), ("sum_rank_padded", C.c_longlong),
                 ("max_rank", C.c_int), ("min_rank", C.c_int), ("factor_bytes", C.c_ulonglong), ("lbar_bytes", C.c_ulonglong),
                 ("workspace_bytes", C.c_ulonglong), ("threshold", C.c_double), ("device", C.c_int), ("max_walkers", C.c_int),
-                ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong), ("svd_sweeps_max", C.c_int), ("svd_offdiag_max", C.c_double)]
+                ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong), ("svd_sweeps_max", C.c_int), ("svd_offdiag_max", C.c_double),
+                ("setup_seconds", C.c_double), ("setup_svd_seconds", C.c_double)]
 
 
 _lib = None

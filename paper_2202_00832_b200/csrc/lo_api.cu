@@ -403,6 +403,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
         return LO_EINVAL;
     }
 
+    const double t_enter = omp_get_wtime();
     lo_factors* f = new (std::nothrow) lo_factors();
     if (!f) { set_error("lo_setup: out of host memory"); return LO_ENOMEM; }
     f->N = N; f->N_pad = round_up(N, KTILE); f->n_chol = n_chol; f->Xp = round_up(n_chol + 1, CO_BM);
@@ -473,6 +474,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             const int n = (int)(k1 - k0);
             for (int x = 0; x < n; ++x) { pairs[k0 + x].x = x; bi[x] = pairs[k0 + x].i; bj[x] = pairs[k0 + x].j; }
             std::vector<SvdStat> stats_of_batch;
+            const double t_svd = omp_get_wtime();
             if (on_gpu) {
                 st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data(), &f->svd_stat);
                 if (st != LO_OK) break;
@@ -501,6 +503,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
                     }
                 }
             }
+            f->setup_svd_seconds += omp_get_wtime() - t_svd;
             if (!on_gpu)
                 for (const SvdStat& t : stats_of_batch) {
                     f->svd_stat.sweeps = std::max(f->svd_stat.sweeps, t.sweeps);
@@ -558,6 +561,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
         free_all(f);
         return LO_ENOMEM;
     }
+    f->setup_seconds = omp_get_wtime() - t_enter;
     *out = f;
     return LO_OK;
 }
@@ -579,6 +583,7 @@ lo_status lo_info_get(const lo_factors* f, lo_info* info) {
     info->threshold = f->threshold; info->device = f->device; info->max_walkers = f->max_walkers;
     info->setup_on_gpu = f->setup_on_gpu; info->n_tiles = f->n_tiles;
     info->svd_sweeps_max = f->svd_stat.sweeps; info->svd_offdiag_max = f->svd_stat.offdiag;
+    info->setup_seconds = f->setup_seconds; info->setup_svd_seconds = f->setup_svd_seconds;
     return LO_OK;
 }
 

@@ -126,6 +126,7 @@ struct lo_factors {
     int device = -1, max_walkers = 0, Wcap = 0, ldw = 0, num_sms = 0;
     int setup_on_gpu = 0;
     lo::SvdStat svd_stat;                // worst case over all pair blocks of lo_setup
+    double setup_seconds = 0, setup_svd_seconds = 0;
     // pair bookkeeping, natural (row-major i<=j) order per spin
     std::vector<int> rank[2];
     std::vector<long long> row_off[2];   // first packed row of the pair
