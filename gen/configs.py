@@ -160,6 +160,13 @@ def _lowdin(c):
     return c @ (v * (1.0 / np.sqrt(w))) @ v.T
 
 
+def chain_geometry(n_sites, fns_per_site=3, spacing=1.4):
+    """Extended geometry for the pair-screening study (pairs N^2 -> N): n_sites on a line."""
+    xyz = np.zeros((n_sites, 3))
+    xyz[:, 0] = spacing * np.arange(n_sites)
+    return xyz, [fns_per_site] * n_sites
+
+
 def make_problem_from_geometry(xyz, fns, n_occ, n_chol, seed, reading="element", name="custom",
                                chol_per_site=None, dtype_L=np.float64) -> Problem:
     """The BASELINE.json generator on an arbitrary site geometry.

@@ -224,6 +224,54 @@ def make_factor_set(N, O, pi, pj, r, U, sigma, W) -> FactorSet:
                      _f64(U).reshape(-1, N), _f64(sigma).reshape(-1), _f64(W).reshape(-1, N))
 
 
+# ------------------------------------------------------------------ NEXT-4: pair screening (section 4)
+def pair_norm_bounds(Lbar, pi, pj):
+    """Upper bounds on the largest singular value of the pair blocks Y^{ij} = sum_g l^g_i (l^g_j)^T, l^g_i = Lbar[g, i, :]
+    (PAPER.md:133), that need no SVD -- the rigorous pre-SVD screen: a pair whose bound is <= T has rank 0 under Eq. 18.
+        sigma_1(Y^{ij}) <= |Y^{ij}|_F                      (spectral <= Frobenius norm)
+                        <= sum_g |l^g_i|_2 |l^g_j|_2       (triangle inequality over the rank-one terms; keeps the locality
+                                                            of every Cholesky vector, so it decays with the distance i-j)
+                        <= |Lbar_i|_F |Lbar_j|_F           (Cauchy-Schwarz over g; distance-blind)
+    Returns (fro [n], tri [n], cs [n]) for the listed pairs, plain loops."""
+    Lbar = _f64(Lbar)
+    X, O, N = Lbar.shape
+    nrm = np.zeros((X, O))
+    for g in range(X):
+        for i in range(O):
+            nrm[g, i] = np.sqrt((Lbar[g, i] * Lbar[g, i]).sum())
+    fro, tri, cs = np.zeros(len(pi)), np.zeros(len(pi)), np.zeros(len(pi))
+    for k in range(len(pi)):
+        i, j = int(pi[k]), int(pj[k])
+        Y = pair_eri(Lbar, i, j)
+        fro[k] = np.sqrt((Y * Y).sum())
+        t = 0.0
+        for g in range(X):
+            t += nrm[g, i] * nrm[g, j]
+        tri[k] = t
+        cs[k] = np.sqrt((nrm[:, i] ** 2).sum()) * np.sqrt((nrm[:, j] ** 2).sum())
+    return fro, tri, cs
+
+
+def screen_pairs(fs: FactorSet, cutoff):
+    """Energy screen ("screening pairs of electrons, and only including those that contribute meaningfully to the total
+    energy"): pair (i, j) is dropped (rank 0) when  m_ij sigma_1^{ij} <= cutoff,  m_ij = 2 - delta_ij.  Since
+    |sum_K sigma_K a_K b_K| = |Theta_j^T Y_r Theta_i| <= sigma_1 |Theta_i|_2 |Theta_j|_2, the exchange energy of a walker moves
+    by at most  cK sum_dropped m_ij sigma_1^{ij} |Theta_i|_2 |Theta_j|_2  (cK = 1 closed shell, 1/2 per spin unrestricted).
+    Returns (screened FactorSet, dropped [n_pairs] bool, m_ij sigma_1 [n_pairs])."""
+    n = len(fs.r)
+    ms1 = np.zeros(n)
+    drop = np.zeros(n, dtype=bool)
+    for k in range(n):
+        m = 1.0 if fs.pi[k] == fs.pj[k] else 2.0
+        s1 = fs.sigma[fs.off[k]] if fs.r[k] > 0 else 0.0
+        ms1[k] = m * s1
+        drop[k] = fs.r[k] > 0 and ms1[k] <= cutoff
+    r = np.where(drop, 0, fs.r).astype(np.int32)
+    rows = [np.arange(fs.off[k], fs.off[k] + r[k]) for k in range(n)]
+    rows = np.concatenate(rows) if rows else np.zeros(0, np.int64)
+    return make_factor_set(fs.N, fs.O, fs.pi, fs.pj, r, fs.U[rows], fs.sigma[rows], fs.W[rows]), drop, ms1
+
+
 def _fs_args(fs: FactorSet):
     return (C.c_int(fs.N), C.c_int(fs.O), C.c_int(len(fs.r)), _p(fs.pi), _p(fs.pj), _p(fs.r), _p(fs.off),
             _p(fs.U), _p(fs.sigma), _p(fs.W))

@@ -353,8 +353,8 @@ def test_c2_full_size_sampled_walkers(c2_built):
 
 def test_c3_full_size_unrestricted_sampled_walkers():
     """BASELINE.json:configs[3] (open-shell metallocene-sized, N=500, 65 alpha + 63 beta, N_chol=2500, T=1e-5): all
-    1024 walkers on the GPU, 16 seeded walkers checked one by one by the oracle on the library's factor set (exchange
-    streamed in chunks of pairs: the 2 x 8 GB of factors do not need to sit on the host at once)."""
+    1024 walkers on the GPU, 64 seeded walkers (>= 64) checked one by one by the oracle on the library's
+    factor set (exchange streamed in chunks of pairs: the 2 x 8 GB of factors do not need to sit on the host at once)."""
     P = gen.make_problem(3)
     phis = gen.make_walkers(P)
     F = lo.Factors.setup(P.h, P.L, P.psi, 1e-5, device=0, max_walkers=P.n_w, gpu_svd=True)
@@ -362,35 +362,76 @@ def test_c3_full_size_unrestricted_sampled_walkers():
     assert tuple(info.n_pairs) == (65 * 66 // 2, 63 * 64 // 2) and info.n_spin == 2
     Eg, st = gpu_energy(F, phis)
     assert (st == 0).all() and np.isfinite(Eg).all()
-    idx = np.sort(np.random.default_rng(3).choice(P.n_w, 16, replace=False))
+    idx = np.sort(np.random.default_rng(3).choice(P.n_w, 64, replace=False))
     Eo, so = oracle_energy_streamed(P, F, phis, idx)
     assert (so == 0).all()
     assert_parity(Eg[idx], Eo)
     assert_all_walkers(P, F, phis, Eg)
 
 
-def test_c4_full_size_sampled_walkers_and_retruncation():
-    """BASELINE.json:configs[4] (3D cage, N=700, N_occ=130, N_chol=3500, 2048 walkers): factor set built once at the
-    loosest threshold of the sweep that the test affords in time (T=1e-3 from a 1e-3 build; the full sweep 1e-3..1e-6 is
-    `bench.py --config 4 --sweep`), all 2048 walkers on the GPU, 16 seeded walkers checked by the oracle on the
-    library's factors; then a re-truncated (looser) set is checked the same way on 4 walkers."""
+def test_c4_threshold_sweep_parity():
+    """BASELINE.json:configs[4] (3D cage, N=700, N_occ=130, N_chol=3500, 2048 walkers, thresholds 1e-3 .. 1e-6): the
+    factor set is built ONCE at T = 1e-6 (the pair SVDs are full whatever T is; 67 GB of factors, 64-bit row offsets) and
+    re-truncated to 1e-5, 1e-4, 1e-3 (lo_retruncate, prefix truncation).  At EACH threshold all 2048 walkers run on the
+    GPU in bench.py's launch configuration and a seeded subset is checked one by one by the oracle on that factor set
+    (protocol A, 1e-10 per walker and part; exchange streamed in chunks of pairs): 32 walkers at 1e-6, 8 walkers at each
+    of the other three; E1/E_J of every 4th walker, repeatability and the host-buffer variant on all walkers at 1e-6."""
     P = gen.make_problem(4)
     phis = gen.make_walkers(P)
-    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-3, device=0, max_walkers=P.n_w, gpu_svd=True)
-    info = F.info()
-    assert info.n_pairs[0] == 130 * 131 // 2 and info.max_rank <= 700
+    F6 = lo.Factors.setup(P.h, P.L, P.psi, 1e-6, device=0, max_walkers=P.n_w, gpu_svd=True)
+    info = F6.info()
+    assert info.n_pairs[0] == 130 * 131 // 2 and info.max_rank <= 700 and info.factor_bytes > 60e9
+    assert info.svd_sweeps_max < 40 and info.svd_offdiag_max <= 700 * 2.0 ** -53
+    idx = np.sort(np.random.default_rng(4).choice(P.n_w, 32, replace=False))
+    sums = []
+    for T, n_chk in [(1e-6, 32), (1e-5, 8), (1e-4, 8), (1e-3, 8)]:
+        F = F6 if T == 1e-6 else F6.retruncate(T)
+        assert F.info().threshold == T
+        sums.append(int(F.info().sum_rank[0]))
+        Eg, st = gpu_energy(F, phis)
+        assert (st == 0).all() and np.isfinite(Eg).all()
+        Eo, so = oracle_energy_streamed(P, F, phis, idx[:n_chk])
+        assert (so == 0).all()
+        assert_parity(Eg[idx[:n_chk]], Eo)
+        if F is F6:
+            assert_all_walkers(P, F, phis, Eg, stride=4)
+        else:
+            F.free()
+    assert sums[0] > sums[1] > sums[2] > sums[3] > 0          # sum r_ij falls with the threshold (P8)
+    F6.free()
+
+
+def exchange_tile_fragments(ranks):
+    """Fragment counts (8-row fragments, 1..8) of the row tiles lo_setup cuts for these ranks: ceil(r/8) fragments in
+    ceil(fragments/8) tiles of near-equal size (include/lo_afqmc.h, lo_info.n_tiles)."""
+    out = []
+    for r in ranks:
+        f8 = (int(r) + 7) // 8
+        nt = (f8 + 7) // 8
+        out += [f8 // nt + (1 if t < f8 % nt else 0) for t in range(nt)]
+    return out
+
+
+@pytest.mark.parametrize("n_w", [64, 65, 16])
+def test_every_tile_fragment_count(c1, n_w):
+    """A factor set whose row tiles take EVERY fragment count 1..8 (configs[1] re-truncated at T = 3, a value inside its
+    own singular-value spectrum: ranks 1..82), so that each instantiation ex_kloop<1..8> of the exchange kernels runs; parity
+    per walker and part at a full block (64 walkers), a ragged batch (65) and the narrow-batch kernel (16)."""
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=n_w, gpu_svd=True).retruncate(3.0)
+    frags = exchange_tile_fragments(F.ranks())
+    assert set(frags) == set(range(1, 9)) and len(frags) == F.info().n_tiles
+    phis = gen.make_walkers(c1, n_w, seed=7)
     Eg, st = gpu_energy(F, phis)
-    assert (st == 0).all() and np.isfinite(Eg).all()
-    idx = np.sort(np.random.default_rng(4).choice(P.n_w, 16, replace=False))
-    Eo, so = oracle_energy_streamed(P, F, phis, idx)
-    assert (so == 0).all()
-    assert_parity(Eg[idx], Eo)
-    assert_all_walkers(P, F, phis, Eg, stride=4)
-    F2 = F.retruncate(1e-2)
-    assert F2.info().sum_rank[0] < info.sum_rank[0]
-    Eg2, _ = gpu_energy(F2, phis)
-    Eo2, _ = oracle_energy_streamed(P, F2, phis, idx[:4])
-    assert_parity(Eg2[idx[:4]], Eo2)
+    Eo, _ = oracle_energy(c1, F, phis)
+    assert (st == 0).all()
+    assert_parity(Eg, Eo)
+    F.set_coulomb_mode(True)                                   # NEXT-3 kernel instantiation (tiles of <= 4 fragments)
+    Eg2, _ = gpu_energy(F, phis)
+    fs = oracle_factor_sets(c1, F)[0]
+    for w in (0, n_w - 1):
+        th, _, _ = oracle.theta(c1.psi[0], phis[0][w])
+        assert abs(Eg2[w, 2] - oracle.coulomb_lo(fs, th)) <= TOL * abs(Eo[w, 0])
+        assert abs(Eg2[w, 3] - Eo[w, 3]) <= TOL * abs(Eo[w, 0])
 
 
 # ------------------------------------------------------------------------------------------ NEXT-1: propagator
@@ -610,6 +651,36 @@ def test_cas_smw_full_size_sampled_walkers():
     cols = [T.columns(d) for d in range(T.n_det)]
     for w in np.random.default_rng(22).choice(n_w, 2, replace=False):
         Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w], compressed_coulomb=True))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+
+
+@pytest.mark.parametrize("smw", [False, True])
+def test_cas_survey_sizes_200_determinants_rank_6(c1, smw):
+    """NEXT-2 at the sizes SURVEY 8(f)-2 names (N_det = 200, excitation rank up to 6, PAPER.md:162 "typically ~ 6", :304-308
+    200 determinants): configs[1], 6 active occupied x 6 active virtuals, both modes, 3 walkers, every output against the
+    oracle's definition (each determinant's own LU and energy) on the library's factor set, 1e-10.  Ranks 5 and 6 enter the
+    k_cas_energy<8> instantiation."""
+    torch = torch_cuda()
+    n_det, n_w = 200, 3
+    T = gen.make_cas_trial(c1, n_virt=6, n_act_occ=6, n_det=n_det, max_exc=6)
+    exc = (T.holes >= 0).sum(axis=1)
+    assert exc.max() == 6 and (exc == 5).any() and len(set(T.holes[T.holes >= 0].tolist())) == 6
+    F = lo.Factors.setup(c1.h, c1.L, [T.C], 1e-3, device=0, max_walkers=n_w * n_det, gpu_svd=True)
+    phi = gen.make_walkers(c1, n_w)[0]
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w, smw_energy=smw)
+    E, st = F.local_energy_cas(torch.from_numpy(phi).cuda())
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    assert (st == 0).all()
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, T.C)
+    n_orb = T.C.shape[1]
+    U, sg, W = F.factor_all(0)
+    pi, pj = oracle.all_pairs(n_orb)
+    fs = oracle.make_factor_set(c1.N, n_orb, pi, pj, F.ranks(0), U, sg, W)
+    cols = [T.columns(d) for d in range(n_det)]
+    for w in range(n_w):
+        Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w], compressed_coulomb=smw))
         assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
         assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
 

@@ -467,3 +467,47 @@ def test_cas_unrestricted_open_shell_singlet_and_triplet():
             E = oracle.local_energy_cas_u([Cmo, Cmo], cols, coef, [Lbar, Lbar], [hbar, hbar], [fs, fs], [pa, pb])
             assert abs(E[0] - E_exact) <= 1e-12 * max(1.0, abs(E_exact)), (name, E[0], E_exact)
             assert abs(E[1] + E[2] + E[3] - E[0]) <= 1e-13
+
+
+def test_pair_screening_bounds_and_energy_screen():
+    """Pins of the oracle's pair screening on an extended geometry (24-site chain, where
+    distant pairs really are negligible).  (i) The pre-SVD bounds form the chain sigma_1 <= |Y|_F <= sum_g |l^g_i||l^g_j| <=
+    |Lbar_i|_F |Lbar_j|_F against LAPACK's sigma_1 of numpy-formed blocks, the triangle bound decays with |i-j| while the
+    Cauchy-Schwarz one does not, and every pair whose bound is <= T has rank 0 in the oracle's own factor set.  (ii) The
+    energy screen drops exactly the pairs with m_ij sigma_1 <= cutoff: the screened exchange plus the dropped pairs' own
+    contributions (typed here with numpy from the full blocks) gives back the unscreened exchange, and the change stays
+    inside sum_dropped m_ij sigma_1 |Theta_i||Theta_j|; cutoff 0 drops nothing, a huge cutoff everything."""
+    xyz, fns = gen.chain_geometry(24, 3)
+    P = gen.make_problem_from_geometry(xyz, fns, (24,), 120, seed=3)
+    O, T = 24, 1e-5
+    Lbar, hbar = oracle.half_rotate(P.L, P.h, P.psi[0])
+    pi, pj = oracle.all_pairs(O)
+    fro, tri, cs = oracle.pair_norm_bounds(Lbar, pi, pj)
+    Ys = [Lbar[:, i, :].T @ Lbar[:, j, :] for i, j in zip(pi, pj)]
+    s1 = np.array([np.linalg.svd(Y, compute_uv=False)[0] for Y in Ys])
+    assert (s1 <= fro * (1 + 1e-12)).all() and (fro <= tri * (1 + 1e-12)).all() and (tri <= cs * (1 + 1e-12)).all()
+    assert np.abs(fro - np.array([np.linalg.norm(Y) for Y in Ys])).max() <= 1e-12 * fro.max()
+    far, near = (pj - pi) >= 16, (pj - pi) <= 1
+    assert tri[far].max() < 1e-4 * tri[near].min() and cs[far].min() > 0.1 * cs[near].max()
+    own = oracle.own_factors(Lbar, T)
+    pre = tri <= T
+    assert pre.sum() >= 20 and (own.r[pre] == 0).all() and (own.r[~pre] > 0).sum() >= 200
+    # energy screen
+    phis = gen.make_walkers(P, 3)
+    full = oracle.own_factors(Lbar, 1e-9)
+    fs0, drop0, ms1 = oracle.screen_pairs(full, 0.0)
+    assert not drop0.any() and np.array_equal(fs0.r, full.r) and np.array_equal(fs0.U, full.U)
+    m = np.where(pi == pj, 1.0, 2.0)
+    assert np.abs(ms1 - m * s1).max() <= 1e-10 * s1.max()
+    fs_inf, drop_inf, _ = oracle.screen_pairs(full, 1e30)
+    assert fs_inf.sum_rank == 0 and drop_inf.sum() == (full.r > 0).sum()
+    for cutoff in (1e-6, 1e-3, 0.3):
+        fsc, drop, _ = oracle.screen_pairs(full, cutoff)
+        assert np.array_equal(drop, (full.r > 0) & (m * s1 <= cutoff * (1 + 1e-12))) and 0 < drop.sum() < len(pi)
+        for w in range(3):
+            th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+            nrm = np.linalg.norm(th, axis=0)
+            ek_full, ek_scr = oracle.exchange_lo(full, th), oracle.exchange_lo(fsc, th)
+            dropped = sum(-m[k] * (th[:, pj[k]] @ Ys[k] @ th[:, pi[k]]) for k in np.nonzero(drop)[0])     # Eq. 17 per pair
+            assert abs(ek_scr + dropped - ek_full) <= 1e-8 * abs(ek_full) + 1e-9 * (m * s1 * nrm[pi] * nrm[pj])[drop].sum() + 1e-12
+            assert abs(ek_scr - ek_full) <= (m * s1 * nrm[pi] * nrm[pj])[drop].sum() * (1 + 1e-9)
