@@ -358,7 +358,8 @@ def run_ours(args):
                            "factor_GB": round(info.factor_bytes / 1e9, 3), "parallelism": "walker-sharded replicas x%d, no collective" % world,
                            "l2": "inputs larger than L2 (factor set %.1f GB, Theta %.0f MB per step)" % (
                                info.factor_bytes / 1e9, 16e-6 * info.N_pad * sum(info.n_occ) * n_w),
-                           "setup_s": round(setup_s, 1)},
+                           "setup_s": round(setup_s, 1), "lo_setup_s": round(info.setup_seconds, 2), "setup_svd_s": round(info.setup_svd_seconds, 2),
+                           "svd_sweeps_max": info.svd_sweeps_max, "pairs_prescreened": int(info.n_pairs_prescreened)},
                 "tflops": round(flops_walker * n_w * world * args.steps / (ms_max * 1e-3) * 1e-12, 3),
                 "flops_per_walker": flops_walker, "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu_baseline,
                 "e2e": {"value": round(e2e_value, 2), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -458,6 +459,65 @@ def run_sweep(args):
         if F is not F0:
             F.free()
     F0.free()
+
+
+def run_screen(args):
+    """--screen: the pair-screening study ("reduce the number of pairs to N from N^2") on
+    chains of growing length (3 functions and one occupied orbital per site, N_chol = 5N, T_SVD = 1e-5, spacing 1.4): per
+    chain the pairs removed by the rigorous pre-SVD screen, and per energy-screen cutoff the kept pairs, sum r_ij, the
+    largest |dE_K| over the batch against the unscreened GPU result with its bound, the error against the exact
+    (Cholesky-route, oracle) exchange of two walkers, and the throughput.  One JSON line per (chain, cutoff); one GPU."""
+    import torch
+
+    import gen
+    import oracle
+    import paper_2202_00832_b200 as lo
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    n_w, T = args.walkers or 256, args.threshold if args.threshold is not None else 1e-5
+    for n_sites in args.screen_sites:
+        xyz, fns = gen.chain_geometry(n_sites, 3)
+        P = gen.make_problem_from_geometry(xyz, fns, (n_sites,), 15 * n_sites, seed=3, name="chain%d" % n_sites)
+        F0 = lo.Factors.setup(P.h, P.L, P.psi, T, device=0, max_walkers=n_w, gpu_svd=True)
+        i0 = F0.info()
+        phis = gen.make_walkers(P, n_w)
+        dphi = [torch.from_numpy(p).cuda() for p in phis]
+        E0 = torch.stack(F0.local_energy(dphi)[:4], dim=1).cpu().numpy()
+        Lbar, _ = oracle.half_rotate(P.L, P.h, P.psi[0])
+        exact = {}
+        for w in (0, n_w // 2):
+            th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+            exact[w] = (oracle.exchange_cholesky(Lbar, th), float(np.linalg.norm(th, axis=0).max()))
+        for cutoff in args.screen_cutoffs:
+            F = F0 if cutoff == 0 else F0.screen_pairs(cutoff)
+            info = F.info()
+            for _ in range(max(args.warmup, 3)):
+                out = F.local_energy(dphi)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                out = F.local_energy(dphi)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            EK = out[3].cpu().numpy()
+            r = F.ranks()
+            print(json.dumps({"screen": "chain of %d sites, N=%d, N_occ=%d, N_chol=%d, T_SVD=%g, N_w=%d" % (n_sites, P.N, n_sites, 15 * n_sites, T, n_w),
+                              "pairs": int(i0.n_pairs[0]), "pairs_prescreened_no_svd": int(i0.n_pairs_prescreened),
+                              "pair_cutoff": cutoff, "pairs_energy_screened": int(info.n_pairs_energy_screened), "pairs_kept": int((r > 0).sum()),
+                              "pairs_kept_per_orbital": round(float((r > 0).sum()) / n_sites, 2), "sum_rank": int(r.sum()),
+                              "dEK_vs_unscreened_max": float(np.abs(EK - E0[:, 3]).max()),
+                              "dEK_bound_sum_m_sigma1": float(info.energy_screen_bound),
+                              "EK_err_vs_exact": [float(abs(EK[w] - ek)) for w, (ek, _) in exact.items()],
+                              "EK_exact_abs": [float(abs(ek)) for ek, _ in exact.values()],
+                              "theta_norm_max": [nm for _, nm in exact.values()],
+                              "ms_per_step": round(ms, 4), "energies_per_s": round(n_w / (ms * 1e-3), 1),
+                              "setup_s": round(i0.setup_seconds, 2), "setup_svd_s": round(i0.setup_svd_seconds, 2)}), flush=True)
+            if F is not F0:
+                F.free()
+        F0.free()
 
 
 def run_reference(args):
@@ -614,6 +674,9 @@ def main():
                     "(N_w / cas real walkers; reported under \"next\", never part of `value`)")
     ap.add_argument("--sweep", action="store_true", help="threshold sweep (BASELINE.json:configs[4]): one JSON line per threshold")
     ap.add_argument("--sweep-exact-walkers", type=int, default=4, help="walkers whose exact E_K the oracle computes in --sweep")
+    ap.add_argument("--screen", action="store_true", help="pair-screening study on chains (NEXT-4): one JSON line per (chain length, cutoff)")
+    ap.add_argument("--screen-sites", type=int, nargs="+", default=[20, 40, 80, 160])
+    ap.add_argument("--screen-cutoffs", type=float, nargs="+", default=[0.0, 1e-6, 1e-4, 1e-2])
     ap.add_argument("--cas-step", type=int, default=0, help="run only multi-determinant steps with this many determinants (ncu target)")
     ap.add_argument("--cas-mode", default="smw", choices=["smw", "direct"])
     ap.add_argument("--cas-exc", type=int, default=4, help="maximum excitation rank of the synthetic CI expansion")
@@ -634,6 +697,8 @@ def main():
         run_launch_check(args)
     elif args.cas_step > 0:
         run_cas_step(args)
+    elif args.screen:
+        run_screen(args)
     elif args.sweep:
         if args.config == 2 and "--config" not in " ".join(sys.argv):
             args.config = 4

@@ -60,6 +60,10 @@ typedef struct {
     double svd_offdiag_max;          /* and the largest normalised off-diagonal |g_p.g_q|/(|g_p||g_q|) left at the end */
     double setup_seconds;            /* wall time of lo_setup, and of its pair Gram + SVD part */
     double setup_svd_seconds;
+    long long n_pairs_prescreened;   /* pairs given rank 0 by the rigorous pre-SVD norm bounds (no SVD was run for them) */
+    long long n_pairs_energy_screened; /* pairs dropped by lo_screen_pairs (m_ij sigma_1 <= energy_screen_cutoff) */
+    double energy_screen_cutoff;     /* 0 when no energy screen was applied */
+    double energy_screen_bound;      /* cK sum over the dropped pairs of m_ij sigma_1: |dE_K| <= this x max_i |Theta_i|^2 */
 } lo_info;
 
 /* Kernel indices for lo_timing_get */
@@ -80,6 +84,13 @@ enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_
 /* flags bit 1 (LO_SETUP_PROPAGATOR, needs device >= 0): also keep the Cholesky vectors L on the device, packed for
  * lo_propagator (upper triangle p<=q, K-major: [N(N+1)/2][n_chol]), and reserve its output buffer. */
 #define LO_SETUP_PROPAGATOR 2
+/* flags bit 2 (LO_SETUP_NO_PRESCREEN): switch the rigorous pre-SVD pair screen off.  By default a pair (i,j) with
+ *     sigma_1(Y^{ij}) <= |Y^{ij}|_F <= sum_g |Lbar^g_i|_2 |Lbar^g_j|_2 <= threshold
+ * ("screening pairs of electrons") is given rank 0 without forming its block (second bound) or without
+ * running its SVD (first bound); the factor rows, weights, ranks and tiles are the same with and without the screen
+ * (Eq. 18 would discard every singular value of such a pair); only the recorded first discarded singular value of a
+ * screened pair is its bound instead of sigma_1.  lo_info.n_pairs_prescreened counts them. */
+#define LO_SETUP_NO_PRESCREEN 4
 lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const double* h, const double* L,
                    const double* psi_a, const double* psi_b, double threshold, int device, int max_walkers,
                    unsigned flags, lo_factors** out);
@@ -99,6 +110,15 @@ lo_status lo_factor_all(const lo_factors* f, int spin, double* U, double* sigma,
 /* New factor set with a looser threshold (>= the one f was built with): prefix truncation of every pair,
  * re-sorted and re-packed; Lbar/hbar are shared by reference counting.  Used for threshold sweeps. */
 lo_status lo_retruncate(const lo_factors* f, double looser_threshold, lo_factors** out);
+
+/* Energy screen of pairs ("screening pairs of electrons, and only including those
+ * that contribute meaningfully to the total energy"): new factor set, same threshold, in which every pair with
+ *     m_ij sigma_1^{ij} <= pair_cutoff        (m_ij = 2 - delta_ij, sigma_1 = largest kept singular value)
+ * has rank 0.  An approximation with an explicit knob (pair_cutoff = 0 changes nothing): since
+ * |sum_K sigma_K a_K b_K| <= sigma_1 |Theta_i|_2 |Theta_j|_2, a walker's E_K moves by at most
+ * cK sum_dropped m_ij sigma_1 |Theta_i|_2 |Theta_j|_2 <= lo_info.energy_screen_bound x max_i |Theta_i|_2^2.
+ * lo_info.n_pairs_energy_screened counts the dropped pairs.  Lbar/hbar are shared with f. */
+lo_status lo_screen_pairs(const lo_factors* f, double pair_cutoff, lo_factors** out);
 
 /* S1-S5: local energies of n_w walkers.  Asynchronous on `stream`; allocates nothing; no host sync.
  *   phi_a  device complex128 [n_w][N][n_occ[0]] (walker-major; columns = orbitals), 16-byte aligned.

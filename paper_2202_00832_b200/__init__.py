@@ -15,9 +15,10 @@ from . import build as _build
 
 LO_SETUP_GPU_SVD = 1
 LO_SETUP_PROPAGATOR = 2
+LO_SETUP_NO_PRESCREEN = 4
 K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 5: "LO_EINTERNAL"}
-EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_local_energy",
+EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_screen_pairs", "lo_local_energy",
            "lo_local_energy_host", "lo_set_cas_trial", "lo_set_cas_trial_beta", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
            "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
 
@@ -34,7 +35,8 @@ class LoInfo(C.Structure):
                 ("max_rank", C.c_int), ("min_rank", C.c_int), ("factor_bytes", C.c_ulonglong), ("lbar_bytes", C.c_ulonglong),
                 ("workspace_bytes", C.c_ulonglong), ("threshold", C.c_double), ("device", C.c_int), ("max_walkers", C.c_int),
                 ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong), ("svd_sweeps_max", C.c_int), ("svd_offdiag_max", C.c_double),
-                ("setup_seconds", C.c_double), ("setup_svd_seconds", C.c_double)]
+                ("setup_seconds", C.c_double), ("setup_svd_seconds", C.c_double), ("n_pairs_prescreened", C.c_longlong),
+                ("n_pairs_energy_screened", C.c_longlong), ("energy_screen_cutoff", C.c_double), ("energy_screen_bound", C.c_double)]
 
 
 _lib = None
@@ -53,6 +55,7 @@ def lib():
         L.lo_factor_pair.argtypes = [vp, ci, ci, ci, vp, vp, vp]
         L.lo_factor_all.argtypes = [vp, ci, vp, vp, vp]
         L.lo_retruncate.argtypes = [vp, cd, C.POINTER(vp)]
+        L.lo_screen_pairs.argtypes = [vp, cd, C.POINTER(vp)]
         L.lo_local_energy.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp]
         L.lo_local_energy_host.argtypes = [vp, ci, vp, vp, vp, vp, vp]
         L.lo_coulomb_x.argtypes = [vp, C.POINTER(vp), C.POINTER(ci)]
@@ -103,7 +106,7 @@ class Factors:
         self._h = C.c_void_p(handle)
 
     @classmethod
-    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False, propagator=False):
+    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False, propagator=False, prescreen=True):
         """lo_setup: h [N,N], L [n_chol,N,N], psis = [psi] (closed shell) or [psi_a, psi_b]; host numpy arrays."""
         h, L = _np(h, np.float64), _np(L, np.float64)
         psis = [_np(p, np.float64) for p in psis]
@@ -112,7 +115,8 @@ class Factors:
         out = C.c_void_p()
         st = lib().lo_setup(N, n_chol, len(psis), n_occ, h.ctypes.data, L.ctypes.data, psis[0].ctypes.data,
                             psis[1].ctypes.data if len(psis) == 2 else None, float(threshold), int(device), int(max_walkers),
-                            (LO_SETUP_GPU_SVD if gpu_svd else 0) | (LO_SETUP_PROPAGATOR if propagator else 0), C.byref(out))
+                            (LO_SETUP_GPU_SVD if gpu_svd else 0) | (LO_SETUP_PROPAGATOR if propagator else 0) |
+                            (0 if prescreen else LO_SETUP_NO_PRESCREEN), C.byref(out))
         _check(st)
         return cls(out.value)
 
@@ -201,6 +205,12 @@ class Factors:
             for t in tensors:
                 if t is not None:
                     t.record_stream(stream)
+
+    def screen_pairs(self, pair_cutoff) -> "Factors":
+        """lo_screen_pairs: drop every pair with m_ij sigma_1 <= pair_cutoff."""
+        out = C.c_void_p()
+        _check(lib().lo_screen_pairs(self._h, float(pair_cutoff), C.byref(out)))
+        return Factors(out.value)
 
     def local_energy(self, phis, parts=True, status=True, stream=None):
         """lo_local_energy on torch CUDA tensors phis = [phi_a(, phi_b)], complex128 [n_w,N,O].  Asynchronous on the

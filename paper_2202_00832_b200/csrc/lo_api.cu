@@ -435,6 +435,27 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             if (st == LO_OK && (flags & LO_SETUP_PROPAGATOR)) st = upload_lt(f, L);
             if (st != LO_OK) { free_all(f); return st; }
         }
+        // ---- rigorous pre-SVD pair screen: Y^{ij} = sum_g l^g_i (l^g_j)^T with l^g_i = Lbar[g][i][:],
+        // so sigma_1(Y^{ij}) <= |Y^{ij}|_F <= sum_g |l^g_i|_2 |l^g_j|_2.  A pair whose bound is <= threshold has rank 0 under
+        // Eq. 18 whatever its SVD says: neither its block nor its SVD is formed.  (The bound keeps the locality of every
+        // Cholesky vector, so it decays with the distance between the two orbitals.)
+        const bool prescreen = !(flags & LO_SETUP_NO_PRESCREEN);
+        std::vector<double> lnorm((size_t)n_chol * f->O_tot);
+        {
+            const double* Lb = f->ops->hLbar.data();
+#pragma omp parallel for schedule(static)
+            for (long long go = 0; go < (long long)n_chol * f->O_tot; ++go) {
+                const double* v = Lb + (size_t)go * N;
+                double a = 0;
+                for (int p = 0; p < N; ++p) a += v[p] * v[p];
+                lnorm[go] = std::sqrt(a);
+            }
+        }
+        auto pair_bound = [&](int oi, int oj) {
+            double b = 0;
+            for (int g = 0; g < n_chol; ++g) b += lnorm[(size_t)g * f->O_tot + oi] * lnorm[(size_t)g * f->O_tot + oj];
+            return b * (1.0 + 1e-12);       // rounding of the sum itself
+        };
         // ---- per-pair SVD + truncation + packing, batch by batch in layout order (whole L2 blocks per batch)
         std::vector<PairRec> pairs;
         std::vector<size_t> bstart;
@@ -471,12 +492,20 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             while (blk1 + 1 < bstart.size() && pairs[bstart[blk1]].spin == spin && bstart[blk1 + 1] - k0 <= B) k1 = bstart[++blk1];
             const bool split = (k1 == k0);
             if (split) k1 = std::min(k0 + B, bstart[blk + 1]);
-            const int n = (int)(k1 - k0);
-            for (int x = 0; x < n; ++x) { pairs[k0 + x].x = x; bi[x] = pairs[k0 + x].i; bj[x] = pairs[k0 + x].j; }
+            const int n_all = (int)(k1 - k0);
+            int n = 0;                       // pairs of the batch that survive the pre-SVD screen: slots 0..n-1 of the SVD batch
+            for (int y = 0; y < n_all; ++y) {
+                PairRec& pr = pairs[k0 + y];
+                const double bound = prescreen ? pair_bound(f->o_base[spin] + pr.i, f->o_base[spin] + pr.j) : 0.0;
+                if (prescreen && bound <= threshold) { pr.x = -1; pr.r = 0; pr.snext = bound; ++f->n_prescreened; continue; }
+                pr.x = n; bi[n] = pr.i; bj[n] = pr.j; ++n;
+            }
             std::vector<SvdStat> stats_of_batch;
             const double t_svd = omp_get_wtime();
-            if (on_gpu) {
-                st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data(), &f->svd_stat);
+            const double skip_below = prescreen ? threshold : -1.0;     // second screen: |Y|_F <= threshold, known once Y is formed
+            if (n == 0) {
+            } else if (on_gpu) {
+                st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data(), skip_below, &f->svd_stat);
                 if (st != LO_OK) break;
             } else {
                 stats_of_batch.assign(n, SvdStat());
@@ -488,7 +517,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
 #pragma omp for schedule(dynamic, 1)
                     for (int x = 0; x < n; ++x) {
                         host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[spin] + bi[x], f->o_base[spin] + bj[x], G.data());
-                        host_block_svd(N, G.data(), V.data(), sg, order, &stats[x]);
+                        host_block_svd(N, G.data(), V.data(), sg, order, skip_below, &stats[x]);
                         std::copy(sg.begin(), sg.end(), hSig.begin() + (size_t)x * N);
                         int r = 0;
                         while (r < N && sg[r] > threshold) ++r;
@@ -509,6 +538,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
                     f->svd_stat.sweeps = std::max(f->svd_stat.sweeps, t.sweeps);
                     f->svd_stat.offdiag = std::max(f->svd_stat.offdiag, t.offdiag);
                     if (!t.converged) f->svd_stat.converged = false;
+                    f->svd_stat.screened += t.screened;
                 }
             if (!f->svd_stat.converged) {
                 set_error("lo_setup: the pair-block SVD did not converge within " + std::to_string(SVD_MAX_SWEEPS) + " sweeps (largest remaining "
@@ -516,17 +546,19 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
                 st = LO_EINTERNAL;
                 break;
             }
-            for (int x = 0; x < n; ++x) {
-                const double* sg = &hSig[(size_t)x * N];
+            for (int y = 0; y < n_all; ++y) {
+                PairRec& pr = pairs[k0 + y];
+                if (pr.x < 0) continue;
+                const double* sg = &hSig[(size_t)pr.x * N];
                 int r = 0;
                 while (r < N && sg[r] > threshold) ++r;
-                pairs[k0 + x].r = r;
-                pairs[k0 + x].snext = r < N ? sg[r] : 0.0;
+                pr.r = r;
+                pr.snext = r < N ? sg[r] : 0.0;
             }
             table.clear();
             auto sig = [&](const PairRec& pr, int K) { return hSig[(size_t)pr.x * N + K]; };
             auto src = [&](const PairRec& pr) { return (long long)pr.x * N; };
-            if (split) layout_block(f, &pairs[k0], &pairs[k0] + n, sig, src, table);
+            if (split) layout_block(f, &pairs[k0], &pairs[k0] + n_all, sig, src, table);
             else
                 for (size_t bb = blk; bb < blk1; ++bb) layout_block(f, &pairs[bstart[bb]], &pairs[bstart[bb + 1]], sig, src, table);
             st = grow_pack(f);
@@ -584,6 +616,9 @@ lo_status lo_info_get(const lo_factors* f, lo_info* info) {
     info->setup_on_gpu = f->setup_on_gpu; info->n_tiles = f->n_tiles;
     info->svd_sweeps_max = f->svd_stat.sweeps; info->svd_offdiag_max = f->svd_stat.offdiag;
     info->setup_seconds = f->setup_seconds; info->setup_svd_seconds = f->setup_svd_seconds;
+    info->n_pairs_prescreened = f->n_prescreened + f->svd_stat.screened;
+    info->n_pairs_energy_screened = f->n_energy_screened; info->energy_screen_cutoff = f->energy_cutoff;
+    info->energy_screen_bound = f->energy_bound;
     return LO_OK;
 }
 
@@ -622,15 +657,18 @@ lo_status lo_factor_all(const lo_factors* f, int spin, double* U, double* sigma,
     return LO_OK;
 }
 
-lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
-    if (!f || !out || !(looser >= f->threshold)) { set_error("lo_retruncate: invalid argument (threshold must be >= the original)"); return LO_EINVAL; }
+// New factor set from the rows of `f`: every pair keeps the prefix sigma_K > looser of its rows (lo_retruncate), and a
+// pair with m_ij sigma_1 <= pair_cutoff keeps none (lo_screen_pairs).
+static lo_status rebuild_from(const lo_factors* f, double looser, double pair_cutoff, lo_factors** out) {
     *out = nullptr;
     lo_factors* g = new (std::nothrow) lo_factors();
-    if (!g) { set_error("lo_retruncate: out of host memory"); return LO_ENOMEM; }
+    if (!g) { set_error("lo_retruncate / lo_screen_pairs: out of host memory"); return LO_ENOMEM; }
     g->N = f->N; g->N_pad = f->N_pad; g->n_chol = f->n_chol; g->Xp = f->Xp; g->n_spin = f->n_spin; g->O_tot = f->O_tot;
     for (int s = 0; s < 2; ++s) { g->n_occ[s] = f->n_occ[s]; g->o_base[s] = f->o_base[s]; }
     g->threshold = looser; g->device = f->device; g->max_walkers = f->max_walkers; g->Wcap = f->Wcap; g->ldw = f->ldw;
     g->num_sms = f->num_sms; g->setup_on_gpu = f->setup_on_gpu; g->svd_stat = f->svd_stat; g->ops = f->ops; g->lbar_bytes = f->lbar_bytes;
+    g->n_prescreened = f->n_prescreened; g->setup_seconds = f->setup_seconds; g->setup_svd_seconds = f->setup_svd_seconds;
+    g->n_energy_screened = f->n_energy_screened; g->energy_cutoff = std::max(f->energy_cutoff, pair_cutoff); g->energy_bound = f->energy_bound;
     try {
         std::vector<PairRec> pairs;
         std::vector<size_t> bstart;
@@ -647,6 +685,15 @@ lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
             pr.src = f->row_off[pr.spin][k];
             int r = 0;
             while (r < r0 && sigma_of(pr, r) > looser) ++r;
+            if (r > 0 && pair_cutoff > 0.0) {
+                // energy screen: |m_ij sum_K sigma_K a_K b_K| <= m_ij sigma_1 |Theta_i||Theta_j|
+                const double ms1 = (pr.i == pr.j ? 1.0 : 2.0) * sigma_of(pr, 0);
+                if (ms1 <= pair_cutoff) {
+                    r = 0;
+                    ++g->n_energy_screened;
+                    g->energy_bound += (f->n_spin == 1 ? 1.0 : 0.5) * ms1;
+                }
+            }
             pr.r = r;
             pr.snext = r < r0 ? sigma_of(pr, r) : f->sigma_next[pr.spin][k];
         }
@@ -668,12 +715,22 @@ lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
         if (st == LO_OK) st = finish_pack(g);
         if (st != LO_OK) { free_all(g); return st; }
     } catch (const std::bad_alloc&) {
-        set_error("lo_retruncate: out of host memory");
+        set_error("lo_retruncate / lo_screen_pairs: out of host memory");
         free_all(g);
         return LO_ENOMEM;
     }
     *out = g;
     return LO_OK;
+}
+
+lo_status lo_retruncate(const lo_factors* f, double looser, lo_factors** out) {
+    if (!f || !out || !(looser >= f->threshold)) { set_error("lo_retruncate: invalid argument (threshold must be >= the original)"); return LO_EINVAL; }
+    return rebuild_from(f, looser, 0.0, out);
+}
+
+lo_status lo_screen_pairs(const lo_factors* f, double pair_cutoff, lo_factors** out) {
+    if (!f || !out || !(pair_cutoff >= 0.0)) { set_error("lo_screen_pairs: invalid argument (cutoff must be >= 0)"); return LO_EINVAL; }
+    return rebuild_from(f, f->threshold, pair_cutoff, out);
 }
 
 static lo_status check_call(const lo_factors* f, int n_w, const void* phi_a, const void* phi_b) {

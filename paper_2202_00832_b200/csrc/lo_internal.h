@@ -111,6 +111,7 @@ struct SvdStat {
     int sweeps = 0;          // sweeps performed (the last one only checks)
     double offdiag = 0;      // largest |g_p.g_q| / (|g_p||g_q|) over the non-null rows seen in the last sweep
     bool converged = true;
+    long long screened = 0;  // blocks whose |Y|_F was <= the threshold: no iteration, rank 0
 };
 
 struct TimingEvent {
@@ -127,6 +128,9 @@ struct lo_factors {
     int setup_on_gpu = 0;
     lo::SvdStat svd_stat;                // worst case over all pair blocks of lo_setup
     double setup_seconds = 0, setup_svd_seconds = 0;
+    long long n_prescreened = 0;         // pairs the norm bound removed before their block was formed
+    long long n_energy_screened = 0;     // pairs lo_screen_pairs dropped (m_ij sigma_1 <= energy_cutoff)
+    double energy_cutoff = 0, energy_bound = 0;   // and cK * sum over them of m_ij sigma_1
     // pair bookkeeping, natural (row-major i<=j) order per spin
     std::vector<int> rank[2];
     std::vector<long long> row_off[2];   // first packed row of the pair
@@ -195,14 +199,15 @@ lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner,
 
 // Pair-block SVD (lo_svd.cu): block one-sided Jacobi with Gram subproblems, host and device versions.
 std::vector<int> svd_schedule(int n_blocks);
-void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, SvdStat* stat);
-cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, int* dSweeps, double* dOff, cudaStream_t stream);
+void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, double skip_below, SvdStat* stat);
+cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, double skip_below, int* dSweeps, double* dOff,
+                                cudaStream_t stream);
 
 // GPU setup (lo_setup_gpu.cu): pair Gram matrices + block-Jacobi SVD (lo_svd.cu) for a batch of pairs of one spin.
 // For the n listed pairs: returns sigma (descending, [n][N]) on the host and leaves the sorted U/W rows on the
 // device in tmpU/tmpW ([n][N][N_pad]).  tmpY/tmpV are scratch of the same size.
 lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV,
-                       double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma, SvdStat* stat);
+                       double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma, double skip_below, SvdStat* stat);
 size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad);
 // dst[rec.dst_row + K][:] = src[rec.src_row + K][:] for K < rec.r, every rec of the host table (rows of N_pad doubles).
 lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table, int n, int N_pad);

@@ -132,7 +132,7 @@ lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table
 size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad) { return (size_t)4 * N * N_pad * 8 + (size_t)N * 12 + 16; }
 
 lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV, double* tmpU,
-                       double* tmpW, double* dSigma, int* dOrder, double* hSigma, SvdStat* stat) {
+                       double* tmpW, double* dSigma, int* dOrder, double* hSigma, double skip_below, SvdStat* stat) {
     const int N = f->N, N_pad = f->N_pad;
     int *dpi = nullptr, *dpj = nullptr, *dSched = nullptr, *dSweeps = nullptr;
     double* dOff = nullptr;
@@ -153,7 +153,7 @@ lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* 
         k_pair_gram<<<grid, 256>>>(f->ops->dLbar, f->n_chol, f->O_tot, N, N_pad, f->o_base[spin], dpi, dpj, tmpY);
         step(cudaGetLastError(), "k_pair_gram");
     }
-    if (e == cudaSuccess) step(launch_block_jacobi(tmpY, tmpV, n, N, N_pad, dSched, dSweeps, dOff, nullptr), "k_block_jacobi");
+    if (e == cudaSuccess) step(launch_block_jacobi(tmpY, tmpV, n, N, N_pad, dSched, skip_below, dSweeps, dOff, nullptr), "k_block_jacobi");
     if (e == cudaSuccess) {
         k_svd_finish<<<n, 512, (size_t)N * 8>>>(tmpY, tmpV, N, N_pad, dSigma, dOrder, tmpU, tmpW);
         step(cudaGetLastError(), "k_svd_finish");
@@ -164,6 +164,12 @@ lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* 
     cudaFree(dpi); cudaFree(dpj); cudaFree(dSched); cudaFree(dSweeps); cudaFree(dOff);      // on every path
     if (e != cudaSuccess) { set_error(std::string("gpu_pair_svd: ") + where + ": " + cudaGetErrorString(e)); return LO_ECUDA; }
     for (int x = 0; x < n; ++x) {
+        if (hSweeps[x] < 0) {           // screened by |Y|_F <= threshold: sigma_1 reported as that bound, everything else 0
+            std::fill(hSigma + (size_t)x * N, hSigma + (size_t)(x + 1) * N, 0.0);
+            hSigma[(size_t)x * N] = hOff[x];
+            ++stat->screened;
+            continue;
+        }
         stat->sweeps = std::max(stat->sweeps, hSweeps[x]);
         stat->offdiag = std::max(stat->offdiag, hOff[x]);
         if (hSweeps[x] >= SVD_MAX_SWEEPS) stat->converged = false;

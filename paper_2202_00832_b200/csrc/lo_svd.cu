@@ -98,12 +98,22 @@ void sym_jacobi_host(int m, double* S, double* Q, int ld, const bool* live, doub
 
 // Host version.  G: n rows of length n (row c = column c of Y), overwritten; V (n x n) receives the accumulated
 // transformation.  sigma: descending; order[K] = row of G / V that holds singular triplet K.
-void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, SvdStat* stat) {
+void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, double skip_below, SvdStat* stat) {
     const int B = SVD_B, nb = (n + B - 1) / B, M = 2 * B;
     std::fill(V, V + (size_t)n * n, 0.0);
     for (int c = 0; c < n; ++c) V[(size_t)c * n + c] = 1.0;
     double fro2 = 0;
     for (size_t k = 0; k < (size_t)n * n; ++k) fro2 += G[k] * G[k];
+    if (std::sqrt(fro2) * (1.0 + 1e-12) <= skip_below) {
+        // sigma_1 <= |Y|_F <= threshold: rank 0 whatever the vectors are (second level of the pair screen); sigma_1 is
+        // reported as its bound |Y|_F
+        sigma.assign(n, 0.0);
+        sigma[0] = std::sqrt(fro2) * (1.0 + 1e-12);
+        order.resize(n);
+        std::iota(order.begin(), order.end(), 0);
+        if (stat) { stat->sweeps = 0; stat->offdiag = 0; stat->converged = true; stat->screened = 1; }
+        return;
+    }
     const double tau = n * SVD_U, null2 = tau * tau * fro2 / n;
     const std::vector<int> sched = svd_schedule(nb);
     const int half = std::max(2, nb + (nb & 1)) / 2, rounds = 2 * half - 1;
@@ -269,7 +279,7 @@ __device__ void sym_jacobi_warp(double* S, double* Q, double* cs, int* pq, doubl
 }
 
 __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restrict__ Gall, double* __restrict__ Vall, int n, int ld,
-                                                                 const int* __restrict__ sched, int half, int max_sweeps,
+                                                                 const int* __restrict__ sched, int half, int max_sweeps, double skip_below,
                                                                  int* __restrict__ sweeps_out, double* __restrict__ off_out) {
     extern __shared__ double sm[];
     __shared__ int s_touched;
@@ -297,6 +307,10 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
     __syncthreads();
     fro = 0;
     for (int w = 0; w < SVD_WARPS; ++w) fro += s_red[w];
+    if (sqrt(fro) * (1.0 + 1e-12) <= skip_below) {       // |Y|_F <= threshold: rank 0, no iteration (sweeps = -1, off = the bound)
+        if (tid == 0) { sweeps_out[x] = -1; off_out[x] = sqrt(fro) * (1.0 + 1e-12); }
+        return;
+    }
     const double tau = n * SVD_U, null2 = tau * tau * fro / n;
     const int rounds = 2 * half - 1, nb = (n + SVD_B - 1) / SVD_B;
     int sweep = 0;
@@ -432,7 +446,7 @@ size_t svd_kernel_smem() { return (size_t)SVD_WARPS * (2 * SVD_M * SVD_LDS + 2 *
 
 // Batched device SVD driver step: orthogonalise the rows of the n_mat matrices in G (V <- accumulated transformation).
 // dSched: device copy of svd_schedule(ceil(n/16)); dSweeps [n_mat] int, dOff [n_mat] double receive the statistics.
-cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, int* dSweeps, double* dOff,
+cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, double skip_below, int* dSweeps, double* dOff,
                                 cudaStream_t stream) {
     static bool configured = false;
     if (!configured) {
@@ -441,7 +455,7 @@ cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, 
         configured = true;
     }
     const int nb = (n + SVD_B - 1) / SVD_B, half = std::max(2, nb + (nb & 1)) / 2;
-    k_block_jacobi<<<n_mat, SVD_WARPS * 32, svd_kernel_smem(), stream>>>(G, V, n, ld, dSched, half, SVD_MAX_SWEEPS, dSweeps, dOff);
+    k_block_jacobi<<<n_mat, SVD_WARPS * 32, svd_kernel_smem(), stream>>>(G, V, n, ld, dSched, half, SVD_MAX_SWEEPS, skip_below, dSweeps, dOff);
     return cudaGetLastError();
 }
 

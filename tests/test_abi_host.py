@@ -173,3 +173,60 @@ def test_walker_shard():
         assert all(a[1] == b[0] for a, b in zip(spans, spans[1:]))
         sizes = [b - a for a, b in spans]
         assert max(sizes) - min(sizes) <= 1
+
+
+def _chain_problem():
+    xyz, fns = gen.chain_geometry(24, 3)
+    return gen.make_problem_from_geometry(xyz, fns, (24,), 120, seed=3)
+
+
+def test_prescreen_is_bit_identical_and_counts_pairs():
+    """The rigorous pre-SVD pair screen (LO_SETUP flag off/on) on a 24-site chain, host setup path: identical ranks, factor
+    rows, singular values and tile count; lo_info counts the pairs that were never decomposed; every screened pair has a
+    LAPACK sigma_1 <= T (so Eq. 18 gives it rank 0 anyway) and the oracle's bound says the same."""
+    P = _chain_problem()
+    T = 1e-5
+    Fs = lo.Factors.setup(P.h, P.L, P.psi, T, device=-1, max_walkers=4)
+    Fn = lo.Factors.setup(P.h, P.L, P.psi, T, device=-1, max_walkers=4, prescreen=False)
+    i_s, i_n = Fs.info(), Fn.info()
+    assert i_n.n_pairs_prescreened == 0 and i_s.n_pairs_prescreened >= 20
+    assert np.array_equal(Fs.ranks(), Fn.ranks()) and i_s.n_tiles == i_n.n_tiles and i_s.sum_rank_padded == i_n.sum_rank_padded
+    for a, b in zip(Fs.factor_all(), Fn.factor_all()):
+        assert np.array_equal(a, b)
+    Lbar, _ = oracle.half_rotate(P.L, P.h, P.psi[0])
+    pi, pj = oracle.all_pairs(24)
+    fro, tri, _ = oracle.pair_norm_bounds(Lbar, pi, pj)
+    assert i_s.n_pairs_prescreened == int((fro <= T).sum()) and int((tri <= T).sum()) <= i_s.n_pairs_prescreened
+    s1 = np.array([np.linalg.svd(Lbar[:, i, :].T @ Lbar[:, j, :], compute_uv=False)[0] for i, j in zip(pi, pj)])
+    assert (Fs.ranks()[fro <= T] == 0).all() and (s1[fro <= T] <= T).all()
+    # the number of kept pairs grows like the chain length, not its square (PAPER.md:318)
+    kept = []
+    for n_sites in (12, 24):
+        xyz, fns = gen.chain_geometry(n_sites, 3)
+        Pc = gen.make_problem_from_geometry(xyz, fns, (n_sites,), 5 * n_sites, seed=3)
+        Fc = lo.Factors.setup(Pc.h, Pc.L, Pc.psi, 1e-3, device=-1, max_walkers=4)
+        kept.append(int((Fc.ranks() > 0).sum()))
+    assert kept[1] < 3.0 * kept[0] and kept[1] / 300.0 < kept[0] / 78.0        # doubling the chain: pairs x3.85, kept pairs < x3
+
+
+def test_energy_screen_matches_oracle_rule():
+    """lo_screen_pairs against the oracle's plain-loop rule on the library's own factors: the same pairs are dropped, the
+    kept rows are untouched, the recorded bound is cK sum_dropped m_ij sigma_1; cutoff 0 is the identity."""
+    P = _chain_problem()
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-7, device=-1, max_walkers=4)
+    pi, pj = oracle.all_pairs(24)
+    U, sg, W = F.factor_all()
+    fs = oracle.make_factor_set(P.N, 24, pi, pj, F.ranks(), U, sg, W)
+    F0 = F.screen_pairs(0.0)
+    assert np.array_equal(F0.ranks(), F.ranks()) and F0.info().n_pairs_energy_screened == 0
+    for cutoff in (1e-5, 1e-2, 1.0):
+        Fc = F.screen_pairs(cutoff)
+        fso, drop, ms1 = oracle.screen_pairs(fs, cutoff)
+        assert np.array_equal(Fc.ranks(), fso.r) and 0 < drop.sum() < len(pi)
+        Uc, sc, Wc = Fc.factor_all()
+        assert np.array_equal(Uc, fso.U) and np.array_equal(sc, fso.sigma) and np.array_equal(Wc, fso.W)
+        ic = Fc.info()
+        assert ic.n_pairs_energy_screened == int(drop.sum()) and ic.energy_screen_cutoff == cutoff
+        assert abs(ic.energy_screen_bound - ms1[drop].sum()) <= 1e-12 * ms1[drop].sum()
+    with pytest.raises(lo.LoError):
+        F.screen_pairs(-1.0)

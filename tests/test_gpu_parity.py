@@ -430,8 +430,51 @@ def test_every_tile_fragment_count(c1, n_w):
     fs = oracle_factor_sets(c1, F)[0]
     for w in (0, n_w - 1):
         th, _, _ = oracle.theta(c1.psi[0], phis[0][w])
-        assert abs(Eg2[w, 2] - oracle.coulomb_lo(fs, th)) <= TOL * abs(Eo[w, 0])
+        assert abs(Eg2[w, 2] - 2.0 * oracle.coulomb_lo(fs, th)) <= TOL * abs(Eo[w, 0])      # closed shell: E_J^LO = 2 S
         assert abs(Eg2[w, 3] - Eo[w, 3]) <= TOL * abs(Eo[w, 0])
+
+
+# ------------------------------------------------------------------------------------------ NEXT-4: pair screening
+def test_pair_screening_on_a_chain():
+    """SURVEY 8(f) NEXT-4 / PAPER.md:318 on an extended geometry (40-site chain, N = 120, 820 pairs), device setup path.
+    (i) Rigorous pre-SVD screen: with and without it the factor set is bit-identical (ranks, rows, singular values, tiles),
+    lo_info counts the pairs that were never decomposed.  (ii) Energy screen (lo_screen_pairs): GPU parity with the oracle
+    on the screened factor set (1e-10), the same pairs dropped as by the oracle's plain-loop rule, and the change of E_K of
+    every walker inside  sum_dropped m_ij sigma_1 |Theta_i||Theta_j|."""
+    xyz, fns = gen.chain_geometry(40, 3)
+    P = gen.make_problem_from_geometry(xyz, fns, (40,), 600, seed=3)
+    T, n_w = 1e-6, 70
+    Fs = lo.Factors.setup(P.h, P.L, P.psi, T, device=0, max_walkers=n_w, gpu_svd=True)
+    Fn = lo.Factors.setup(P.h, P.L, P.psi, T, device=0, max_walkers=n_w, gpu_svd=True, prescreen=False)
+    i_s, i_n = Fs.info(), Fn.info()
+    assert i_n.n_pairs_prescreened == 0 and i_s.n_pairs_prescreened > 100
+    assert np.array_equal(Fs.ranks(), Fn.ranks()) and i_s.n_tiles == i_n.n_tiles
+    for a, b in zip(Fs.factor_all(), Fn.factor_all()):
+        assert np.array_equal(a, b)
+    assert (Fs.ranks() == 0).sum() >= i_s.n_pairs_prescreened
+    phis = gen.make_walkers(P, n_w)
+    E0, _ = gpu_energy(Fs, phis)
+    assert np.array_equal(E0, gpu_energy(Fn, phis)[0])
+    assert_parity(E0, oracle_energy(P, Fs, phis)[0])
+    pi, pj = oracle.all_pairs(40)
+    fs = oracle_factor_sets(P, Fs)[0]
+    m = np.where(pi == pj, 1.0, 2.0)
+    kept = []
+    for cutoff in (1e-4, 1e-2):
+        Fc = Fs.screen_pairs(cutoff)
+        fso, drop, ms1 = oracle.screen_pairs(fs, cutoff)
+        assert np.array_equal(Fc.ranks(), fso.r) and Fc.info().n_pairs_energy_screened == int(drop.sum()) > 0
+        Ec, st = gpu_energy(Fc, phis)
+        Eo, _ = oracle_energy(P, Fc, phis)
+        assert (st == 0).all()
+        assert_parity(Ec, Eo)
+        for w in range(0, n_w, 7):
+            th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+            nrm = np.linalg.norm(th, axis=0)
+            assert abs(Ec[w, 3] - E0[w, 3]) <= (ms1 * nrm[pi] * nrm[pj])[drop].sum() * (1 + 1e-9)
+            assert abs(Ec[w, 3] - E0[w, 3]) <= Fc.info().energy_screen_bound * nrm.max() ** 2 * (1 + 1e-9)
+        kept.append(int((Fc.ranks() > 0).sum()))
+    assert kept[1] < kept[0] < (Fs.ranks() > 0).sum() <= 820
 
 
 # ------------------------------------------------------------------------------------------ NEXT-1: propagator
