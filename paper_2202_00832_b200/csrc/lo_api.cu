@@ -244,6 +244,10 @@ lo_status finish_pack(lo_factors* f) {
     if (st == LO_OK) st = make_tmap(&f->tmW, f->dW, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmU8, f->dU, f->N_pad, rows_alloc, 8);
     if (st == LO_OK) st = make_tmap(&f->tmW8, f->dW, f->N_pad, rows_alloc, 8);
+    for (int k = 0; k < 8 && st == LO_OK; ++k) {
+        st = make_tmap(&f->tmUf.m[k], f->dU, f->N_pad, rows_alloc, 8 * (k + 1));
+        if (st == LO_OK) st = make_tmap(&f->tmWf.m[k], f->dW, f->N_pad, rows_alloc, 8 * (k + 1));
+    }
     if (st != LO_OK) return st;
     return alloc_workspace(f);
 }
@@ -765,27 +769,35 @@ lo_status lo_local_energy_host(const lo_factors* fc, int n_w, const void* phi_a_
     lo_factors* f = const_cast<lo_factors*>(fc);
     cudaStream_t s = (cudaStream_t)stream;
     CK(cudaSetDevice(f->device));
-    // Walker chunks (multiples of 64, at least 128 walkers each, at most LO_HOST_CHUNKS): the H2D copy of chunk c+1 runs on
+    // Walker chunks (starting at multiples of 64, at most LO_HOST_CHUNKS): the H2D copy of chunk c+1 runs on
     // a private copy stream while the kernels of chunk c run on `s`; walkers are independent, so a chunk is a complete
     // pass of the hot path over its walkers (the factor rows are streamed once per chunk).
     const char* ph[2] = {static_cast<const char*>(phi_a_host), static_cast<const char*>(phi_b_host)};
-    const int n_chunks = std::max(1, std::min(LO_HOST_CHUNKS, n_w / 128));
-    const int per = ((n_w + n_chunks - 1) / n_chunks + WALKER_TILE - 1) / WALKER_TILE * WALKER_TILE;
+    // Chunk sizes grow geometrically (64, 128, 256, rest): the first copy -- the only one nothing can hide -- is short, and
+    // every later chunk's copy is no longer than the kernels of the chunk before it even in the small-rank regime (a walker
+    // costs about twice as long to process as to copy there), while most walkers still run in one large, efficient launch.
+    int chunk[LO_HOST_CHUNKS], n_chunks = 0;
+    {
+        int rem = n_w, c = WALKER_TILE;
+        if (n_w >= 4 * WALKER_TILE)
+            while (n_chunks < LO_HOST_CHUNKS - 1 && rem > 3 * c) { chunk[n_chunks++] = c; rem -= c; c *= 2; }
+        chunk[n_chunks++] = rem;
+    }
     // The copies are ordered after everything already queued on the caller's stream (a stream-ordered producer of the
     // pinned Phi buffer, or an earlier call on this handle that still reads the staging area).
     CK(cudaEventRecord(f->evEnter, s));
     CK(cudaStreamWaitEvent(f->copyStream, f->evEnter, 0));
     auto body = [&]() -> lo_status {
-        for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
-            const int nc = std::min(per, n_w - w0);
+        for (int c = 0, w0 = 0; c < n_chunks; w0 += chunk[c], ++c) {
+            const int nc = chunk[c];
             for (int sp = 0; sp < f->n_spin; ++sp) {
                 const size_t per_w = (size_t)f->N * f->n_occ[sp] * 16;
                 CK(cudaMemcpyAsync(reinterpret_cast<char*>(f->dPhi[sp]) + w0 * per_w, ph[sp] + w0 * per_w, nc * per_w, cudaMemcpyHostToDevice, f->copyStream));
             }
             CK(cudaEventRecord(f->evCopy[c], f->copyStream));
         }
-        for (int c = 0, w0 = 0; w0 < n_w; ++c, w0 += per) {
-            const int nc = std::min(per, n_w - w0);
+        for (int c = 0, w0 = 0; c < n_chunks; w0 += chunk[c], ++c) {
+            const int nc = chunk[c];
             CK(cudaStreamWaitEvent(s, f->evCopy[c], 0));
             const char* pa = reinterpret_cast<const char*>(f->dPhi[0]) + (size_t)w0 * f->N * f->n_occ[0] * 16;
             const char* pb = f->n_spin == 2 ? reinterpret_cast<const char*>(f->dPhi[1]) + (size_t)w0 * f->N * f->n_occ[1] * 16 : nullptr;

@@ -27,6 +27,11 @@ constexpr int CO_BM = 128;       // rows (Cholesky vectors) per Coulomb tile
 constexpr int MAX_SPLIT = 8;     // split-K partial buffers of the Coulomb GEMM
 #define LO_HOST_CHUNKS 4         // walker chunks of lo_local_energy_host (copy/compute overlap)
 
+// Tensor maps of one array for every box height 8, 16, .., 64 rows (passed to kernels as one __grid_constant__ parameter).
+struct TmSet {
+    CUtensorMap m[8];
+};
+
 struct ExTile {
     int row0;   // first packed row of the tile
     int nfrag;  // valid 8-row fragments in the tile (1..8)
@@ -150,6 +155,7 @@ struct lo_factors {
     lo::ExTile* dTiles4 = nullptr;
     CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
     CUtensorMap tmU8, tmW8;              // same arrays, boxes 8 x 16 (one row fragment): tiles shorter than 64 rows
+    lo::TmSet tmUf, tmWf;                // same arrays, boxes (8 k) x 16 for k = 1..8: one TMA issue per operand for a tile of k fragments
     CUtensorMap tmTheta32;               // Theta^T panels with a 32 x 16 box (16 walkers): narrow-batch exchange
     std::shared_ptr<lo::SharedOps> ops;
     // workspace

@@ -625,8 +625,8 @@ __global__ void __launch_bounds__(256) k_ej(double* __restrict__ Xpart, double2*
 // fragments of the tile and 16 real columns (8 walkers), so any rank (nfrag = 1..8 fragments of 8 rows) is balanced
 // over the warps and no cross-warp reduction is needed; the K loop is instantiated per nfrag (ex_kloop<NFRAG>) so a
 // short tile issues no DMMA on padding (predicated-off DMMAs still occupy the pipe: seen with ncu on the paper-like
-// small-rank workload).  4-stage TMA/mbarrier pipeline running across items; a short tile loads only its own 8-row
-// fragments of U and W.  The C fragment holds (re, im) of one walker in one lane, for a and b alike, so the complex
+// small-rank workload).  4-stage TMA/mbarrier pipeline running across items; a tile of k fragments loads U and W as one
+// box of 8 k rows each (a tensor map per box height).  The C fragment holds (re, im) of one walker in one lane, for a and b alike, so the complex
 // product is lane-local; rows are reduced by warp shuffles.  Persistent CTAs with a static round-robin schedule and
 // per-CTA partial sums accumulated in a fixed order -> bitwise repeatable.
 constexpr int EX_STAGES = 4;
@@ -676,8 +676,7 @@ __device__ __forceinline__ void ex_kloop(int KT, uint32_t sbase, uint32_t full, 
 }
 
 template <bool COUL, bool RAGGED>   // RAGGED: the batch is not a multiple of 64 walkers (warps without walkers skip their MMAs)
-__global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
-                                                     const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
+__global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ TmSet tmUs, const __grid_constant__ TmSet tmWs,
                                                      const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
                                                      const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
                                                      double* __restrict__ ekpart, double* __restrict__ ejpart, int Wcap, int n_w) {
@@ -695,10 +694,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
         if constexpr (COUL) mypartJ[i] = 0.0;
     }
     if (tid == 0) {
-        prefetch_tmap(&tmU);
-        prefetch_tmap(&tmW);
-        prefetch_tmap(&tmU8);
-        prefetch_tmap(&tmW8);
+        for (int k = 0; k < 8; ++k) { prefetch_tmap(&tmUs.m[k]); prefetch_tmap(&tmWs.m[k]); }
         prefetch_tmap(&tmT);
         for (int i = 0; i < EX_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
@@ -721,15 +717,9 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
                     const uint32_t st = sbase + slot * EX_STAGE_BYTES, bar = full + 8 * slot;
                     const int k0 = kt * KTILE;
                     mbar_expect_tx(bar, tx);
-                    if (tile.nfrag == EX_BM / 8) {
-                        tma_load_2d(st, &tmU, k0, tile.row0, bar);
-                        tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
-                    } else {
-                        for (int fr = 0; fr < tile.nfrag; ++fr) {
-                            tma_load_2d(st + fr * 1024, &tmU8, k0, tile.row0 + fr * 8, bar);
-                            tma_load_2d(st + EX_BM * 128 + fr * 1024, &tmW8, k0, tile.row0 + fr * 8, bar);
-                        }
-                    }
+                    // one box of exactly the tile's rows per operand (tensor maps per box height 8 .. 64)
+                    tma_load_2d(st, &tmUs.m[tile.nfrag - 1], k0, tile.row0, bar);
+                    tma_load_2d(st + EX_BM * 128, &tmWs.m[tile.nfrag - 1], k0, tile.row0, bar);
                     tma_load_2d(st + 2 * EX_BM * 128, &tmT, k0, tile.pj * ldw + nb * 128, bar);
                     tma_load_2d(st + (2 * EX_BM + 128) * 128, &tmT, k0, tile.pi * ldw + nb * 128, bar);
                     if (++slot == EX_STAGES) { slot = 0; phase ^= 1; }
@@ -854,15 +844,52 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ CUt
 
 // ---- narrow-batch exchange (n_w <= 32, e.g. the paper's 16 walkers per GPU): a 64-walker column block
 // would leave 6 of the 8 consumer warps without walkers, so here a work item is (row tile, block of 16 walkers = 32 real
-// columns) and the warps split the ROW fragments instead: warp cw owns column half cw & 1 (8 walkers) and fragments
-// cw >> 1 and 4 + (cw >> 1).  Same TMA/mbarrier pipeline (6 stages of 24 KB); the four fragment groups of a column half
-// are added in a fixed order through shared memory.
+// columns = 4 column tiles of the m8n8k4 MMA) and the work units are (row fragment, column tile): consumer warp cw owns
+// column tile cw & 3 (4 walkers) and the fragments (cw >> 2), (cw >> 2) + 2, ... of the tile.  The two warps of a
+// scheduler (cw, cw + 4) then hold nfrag units between them whatever nfrag is, so the four tensor pipes carry equal
+// loads (the first version split fragments cw >> 1 and 4 + (cw >> 1): 3 units on two schedulers, 2 on the others at
+// nfrag = 5).  The K loop is instantiated per fragment count of the warp (no padding MMAs).  The weighted complex dots
+// are accumulated IN REGISTERS across all items of the CTA (an item only adds lane-local terms: no shuffle, no barrier,
+// no shared memory per item); one shuffle reduction over the row groups and one fixed-order addition of the two
+// fragment groups at the end of the kernel.  Same TMA/mbarrier pipeline; U and W arrive as ONE box of exactly the
+// tile's rows each (tensor maps per box height).
 constexpr int EN_STAGES = 6;
 constexpr int EN_STAGE_BYTES = (2 * EX_BM + 2 * 32) * 128;
-constexpr int EN_SMEM = EN_STAGES * EN_STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 4 * 32 * 8;
+constexpr int EN_SMEM = EN_STAGES * EN_STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 2 * 64 * 8;
 
-__global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
-                                                            const __grid_constant__ CUtensorMap tmU8, const __grid_constant__ CUtensorMap tmW8,
+template <int NFW>   // fragments of this warp in the current tile (0..4)
+__device__ __forceinline__ void en_kloop(int KT, uint32_t sbase, uint32_t full, uint32_t empty, int& cslot, uint32_t& cphase, int lane,
+                                         const uint32_t (&xo)[4], uint32_t u_row, uint32_t tj_row, double (&accA)[4][2], double (&accB)[4][2]) {
+    constexpr uint32_t W_OFF = EX_BM * 128, TI_OFF = 32 * 128;
+    for (int kt = 0; kt < KT; ++kt) {
+        if (kt) mbar_wait(full + 8 * cslot, cphase);     // the item's first stage was awaited by the caller
+        if constexpr (NFW == 0) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + 8 * cslot);
+        } else {
+            const uint32_t st = sbase + cslot * EN_STAGE_BYTES;
+#pragma unroll
+            for (int ks = 0; ks < KTILE / 4; ++ks) {
+                double a[NFW], w[NFW];
+#pragma unroll
+                for (int j = 0; j < NFW; ++j) {
+                    a[j] = lds_f64(st + u_row + j * 2048 + xo[ks]);            // fragments two apart: 16 rows = 2048 bytes
+                    w[j] = lds_f64(st + u_row + W_OFF + j * 2048 + xo[ks]);
+                }
+                const double bj = lds_f64(st + tj_row + xo[ks]), bi = lds_f64(st + tj_row + TI_OFF + xo[ks]);
+                if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
+#pragma unroll
+                for (int j = 0; j < NFW; ++j) {
+                    mma884(accA[j][0], accA[j][1], a[j], bj);
+                    mma884(accB[j][0], accB[j][1], w[j], bi);
+                }
+            }
+        }
+        if (++cslot == EN_STAGES) { cslot = 0; cphase ^= 1; }
+    }
+}
+
+__global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constant__ TmSet tmUs, const __grid_constant__ TmSet tmWs,
                                                             const __grid_constant__ CUtensorMap tmT32, const double* __restrict__ wgt,
                                                             const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
                                                             double* __restrict__ ekpart, int Wcap) {
@@ -871,16 +898,13 @@ __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constan
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
     const uint32_t full = sbase + EN_STAGES * EN_STAGE_BYTES, empty = full + 8 * EN_STAGES;
     ExTile* ring = reinterpret_cast<ExTile*>(sgen + EN_STAGES * EN_STAGE_BYTES + 128);
-    double* red = reinterpret_cast<double*>(sgen + EN_STAGES * EN_STAGE_BYTES + 128 + EX_RING * 16);      // [4 fragment groups][32 columns]
+    double* red = reinterpret_cast<double*>(sgen + EN_STAGES * EN_STAGE_BYTES + 128 + EX_RING * 16);      // [2 fragment groups][2 blocks x 32 columns]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     double* mypart = ekpart + (size_t)blockIdx.x * 2 * Wcap;
     for (int i = tid; i < 2 * Wcap; i += 384) mypart[i] = 0.0;
     if (tid == 0) {
-        prefetch_tmap(&tmU);
-        prefetch_tmap(&tmW);
-        prefetch_tmap(&tmU8);
-        prefetch_tmap(&tmW8);
+        for (int k = 0; k < 8; ++k) { prefetch_tmap(&tmUs.m[k]); prefetch_tmap(&tmWs.m[k]); }
         prefetch_tmap(&tmT32);
         for (int i = 0; i < EN_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
@@ -894,17 +918,17 @@ __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constan
             for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
                 const ExTile tile = tiles[q / NB];
                 const int nb = (int)(q % NB);
-                // whole 64-row boxes of U and W whatever the tile's length (rows past the tile are never read): 4 TMA
-                // issues per 24 KB stage -- a narrow item has too little MMA work per stage to hide more
-                const uint32_t tx = (uint32_t)(2 * EX_BM + 2 * 32) * 128;
+                const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + 2 * 32) * 128;
+                const CUtensorMap* mu = &tmUs.m[tile.nfrag - 1];
+                const CUtensorMap* mw = &tmWs.m[tile.nfrag - 1];
                 for (int kt = 0; kt < KT; ++kt) {
                     mbar_wait(empty + 8 * slot, phase ^ 1);
                     if (kt == 0) ring[n % EX_RING] = tile;
                     const uint32_t st = sbase + slot * EN_STAGE_BYTES, bar = full + 8 * slot;
                     const int k0 = kt * KTILE;
                     mbar_expect_tx(bar, tx);
-                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
-                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
+                    tma_load_2d(st, mu, k0, tile.row0, bar);
+                    tma_load_2d(st + EX_BM * 128, mw, k0, tile.row0, bar);
                     tma_load_2d(st + 2 * EX_BM * 128, &tmT32, k0, tile.pj * ldw + nb * 32, bar);
                     tma_load_2d(st + 2 * EX_BM * 128 + 32 * 128, &tmT32, k0, tile.pi * ldw + nb * 32, bar);
                     if (++slot == EN_STAGES) { slot = 0; phase ^= 1; }
@@ -915,90 +939,56 @@ __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constan
     }
     reg_inc_consumer();
     const int cw = warp - 4, g = lane >> 2, t = lane & 3, ctid = tid - 128;
-    const int cg = cw & 1, fr0 = cw >> 1, fr1 = 4 + (cw >> 1);
-    double accA[2][2][2], accB[2][2][2];
+    const int nt = cw & 3, fg = cw >> 2;           // column tile (walkers 4 nt .. 4 nt + 3 of the block), fragment group
+    double accA[4][2], accB[4][2];
 #pragma unroll
-    for (int j = 0; j < 2; ++j)
-#pragma unroll
-        for (int b = 0; b < 2; ++b) accA[j][b][0] = accA[j][b][1] = accB[j][b][0] = accB[j][b][1] = 0.0;
+    for (int j = 0; j < 4; ++j) accA[j][0] = accA[j][1] = accB[j][0] = accB[j][1] = 0.0;
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
-    const uint32_t u_row0 = (uint32_t)(fr0 * 8 + g) * 128, u_row1 = (uint32_t)(fr1 * 8 + g) * 128;
-    const uint32_t tj_row = (uint32_t)(2 * EX_BM + cg * 16 + g) * 128, ti_row = tj_row + 32 * 128;
+    const uint32_t u_row = (uint32_t)(fg * 8 + g) * 128;
+    const uint32_t tj_row = (uint32_t)(2 * EX_BM + nt * 8 + g) * 128;
+    double e0r = 0.0, e0i = 0.0, e1r = 0.0, e1i = 0.0;      // this lane's running sums for walker block 0 / 1
     int cslot = 0, n = 0;
     uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
         const int nb = (int)(q % NB);
         mbar_wait(full + 8 * cslot, cphase);
         const ExTile tile = ring[n % EX_RING];
-        const int nu = (fr0 < tile.nfrag ? 1 : 0) + (fr1 < tile.nfrag ? 1 : 0);     // warp-uniform
-        for (int kt = 0; kt < KT; ++kt) {
-            if (kt) mbar_wait(full + 8 * cslot, cphase);
-            const uint32_t st = sbase + cslot * EN_STAGE_BYTES;
-            if (nu > 0) {
-#pragma unroll
-                for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    double a[2], w[2], bj[2], bi[2];
-                    a[0] = lds_f64(st + u_row0 + xo[ks]);
-                    w[0] = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
-                    if (nu == 2) {
-                        a[1] = lds_f64(st + u_row1 + xo[ks]);
-                        w[1] = lds_f64(st + u_row1 + EX_BM * 128 + xo[ks]);
-                    }
-#pragma unroll
-                    for (int nf = 0; nf < 2; ++nf) {
-                        bj[nf] = lds_f64(st + tj_row + nf * 1024 + xo[ks]);
-                        bi[nf] = lds_f64(st + ti_row + nf * 1024 + xo[ks]);
-                    }
-                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
-#pragma unroll
-                    for (int nf = 0; nf < 2; ++nf) {
-                        mma884(accA[0][nf][0], accA[0][nf][1], a[0], bj[nf]);
-                        mma884(accB[0][nf][0], accB[0][nf][1], w[0], bi[nf]);
-                    }
-                    if (nu == 2) {
-#pragma unroll
-                        for (int nf = 0; nf < 2; ++nf) {
-                            mma884(accA[1][nf][0], accA[1][nf][1], a[1], bj[nf]);
-                            mma884(accB[1][nf][0], accB[1][nf][1], w[1], bi[nf]);
-                        }
-                    }
-                }
-            } else {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty + 8 * cslot);
-            }
-            if (++cslot == EN_STAGES) { cslot = 0; cphase ^= 1; }
+        const int nfw = tile.nfrag > fg ? (tile.nfrag - fg + 1) >> 1 : 0;     // warp-uniform
+        switch (nfw) {
+            case 0: en_kloop<0>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 1: en_kloop<1>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 2: en_kloop<2>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            case 3: en_kloop<3>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
+            default: en_kloop<4>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, tj_row, accA, accB); break;
         }
-        double e[2][2];
+        double er = 0.0, ei = 0.0;
 #pragma unroll
-        for (int nf = 0; nf < 2; ++nf) e[nf][0] = e[nf][1] = 0.0;
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const double wv = j < nu ? __ldg(wgt + tile.row0 + (j == 0 ? fr0 : fr1) * 8 + g) : 0.0;
-#pragma unroll
-            for (int nf = 0; nf < 2; ++nf) {
-                const double ar = accA[j][nf][0], ai = accA[j][nf][1], br = accB[j][nf][0], bi = accB[j][nf][1];
-                e[nf][0] = fma(wv, ar * br - ai * bi, e[nf][0]);
-                e[nf][1] = fma(wv, ar * bi + ai * br, e[nf][1]);
-                accA[j][nf][0] = accA[j][nf][1] = accB[j][nf][0] = accB[j][nf][1] = 0.0;
-            }
+        for (int j = 0; j < 4; ++j) {
+            const double wv = j < nfw ? __ldg(wgt + tile.row0 + (fg + 2 * j) * 8 + g) : 0.0;
+            const double ar = accA[j][0], ai = accA[j][1], br = accB[j][0], bi = accB[j][1];
+            er = fma(wv, ar * br - ai * bi, er);
+            ei = fma(wv, ar * bi + ai * br, ei);
+            accA[j][0] = accA[j][1] = accB[j][0] = accB[j][1] = 0.0;
         }
-#pragma unroll
-        for (int nf = 0; nf < 2; ++nf)
-#pragma unroll
-            for (int c = 0; c < 2; ++c) {
-                double v = e[nf][c];
-                v += __shfl_xor_sync(0xffffffffu, v, 4);
-                v += __shfl_xor_sync(0xffffffffu, v, 8);
-                v += __shfl_xor_sync(0xffffffffu, v, 16);
-                if (g == 0) red[(cw >> 1) * 32 + cg * 16 + nf * 8 + 2 * t + c] = v;
-            }
-        bar_sync_consumers();
-        if (ctid < 32) mypart[(size_t)nb * 32 + ctid] += (red[ctid] + red[32 + ctid]) + (red[64 + ctid] + red[96 + ctid]);
-        bar_sync_consumers();
+        if (nb == 0) { e0r += er; e0i += ei; }
+        else { e1r += er; e1i += ei; }
     }
+    // ---- once per kernel: rows (shuffles over g), then the two fragment groups in a fixed order
+    double v[4] = {e0r, e0i, e1r, e1i};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        v[c] += __shfl_xor_sync(0xffffffffu, v[c], 4);
+        v[c] += __shfl_xor_sync(0xffffffffu, v[c], 8);
+        v[c] += __shfl_xor_sync(0xffffffffu, v[c], 16);
+    }
+    if (g == 0) {
+        double* r = red + fg * 64 + nt * 8 + 2 * t;
+        r[0] = v[0]; r[1] = v[1]; r[32] = v[2]; r[33] = v[3];
+    }
+    bar_sync_consumers();
+    if (ctid < 32 * NB) mypart[ctid] = red[ctid] + red[64 + ctid];
 }
 
 // ------------------------------------------------------------------------------------------------ NEXT-1: propagator
@@ -1204,11 +1194,11 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
             const int NB16 = (n_w + 15) / 16;
             items = f->n_tiles * NB16;
             ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-            k_exchange_narrow<<<ex_grid, 384, EN_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta32, f->dWgt, f->dTiles, items, NB16,
+            k_exchange_narrow<<<ex_grid, 384, EN_SMEM, stream>>>(f->tmUf, f->tmWf, f->tmTheta32, f->dWgt, f->dTiles, items, NB16,
                                                                  N_pad, ldw, f->dEKpart, Wcap);
         } else
 #define LO_EX_LAUNCH(C_, R_, TILES_, EJ_)                                                                                              \
-    k_exchange<C_, R_><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmU, f->tmW, f->tmU8, f->tmW8, f->tmTheta, f->dWgt, TILES_, items, NB, N_pad, ldw, \
+    k_exchange<C_, R_><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmUf, f->tmWf, f->tmTheta, f->dWgt, TILES_, items, NB, N_pad, ldw, \
                                                           f->dEKpart, EJ_, Wcap, n_w)
         if (coul && ragged) LO_EX_LAUNCH(true, true, f->dTiles4, f->dEJLpart);
         else if (coul) LO_EX_LAUNCH(true, false, f->dTiles4, f->dEJLpart);

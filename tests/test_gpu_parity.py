@@ -219,7 +219,7 @@ def test_trial_walker_gives_hf_energy(c1):
 # ------------------------------------------------------------------------------------------ API variants
 def test_host_variant_and_determinism(c1):
     torch = torch_cuda()
-    phis = gen.make_walkers(c1, 300)    # host variant: 2 walker chunks (192 + a ragged 108)
+    phis = gen.make_walkers(c1, 300)    # host variant: 2 walker chunks (64 + a ragged 236)
     F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=300, gpu_svd=True)
     E1, _ = gpu_energy(F, phis)
     E2, _ = gpu_energy(F, phis)
