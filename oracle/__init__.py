@@ -272,6 +272,29 @@ def screen_pairs(fs: FactorSet, cutoff):
     return make_factor_set(fs.N, fs.O, fs.pi, fs.pj, r, fs.U[rows], fs.sigma[rows], fs.W[rows]), drop, ms1
 
 
+def randomized_svd(Y, Omega):
+    """Approximate SVD of one pair block by a randomised range finder ("approximate versions of the singular value
+    decomposition, which would reduce the scaling of this step significantly"; Halko, Martinsson & Tropp
+    2011, Alg. 4.1 + 5.1), written out step by step with library primitives as steps:
+        Z = Y^T Omega                     sketch of the row space of Y            (Omega: n x k Gaussian test matrix, an INPUT)
+        P = orth(Z)                       numpy.linalg.qr
+        B = P^T Y^T                       k x n
+        B = Ub diag(s) Vb^T               numpy.linalg.svd of the small matrix
+        Y ~= Vb diag(s) (P Ub)^T          => left vectors Vb^T rows, right vectors (P Ub)^T rows
+        resid = |Y - U^T diag(s) W|_F     a-posteriori error: every singular value of Y is within resid of the returned ones
+                                          (Weyl), so the result is exact to working accuracy iff rank(Y) <= k numerically.
+    Returns (Ut [k,n], s [k] descending, Wt [k,n], resid)."""
+    Y, Omega = _f64(Y), _f64(Omega)
+    Z = Y.T @ Omega
+    P, _ = np.linalg.qr(Z)
+    B = P.T @ Y.T
+    Ub, s, Vbt = np.linalg.svd(B, full_matrices=False)
+    Ut = Vbt
+    Wt = (P @ Ub).T
+    resid = float(np.sqrt(((Y - (Ut.T * s) @ Wt) ** 2).sum()))
+    return Ut, s, Wt, resid
+
+
 def _fs_args(fs: FactorSet):
     return (C.c_int(fs.N), C.c_int(fs.O), C.c_int(len(fs.r)), _p(fs.pi), _p(fs.pj), _p(fs.r), _p(fs.off),
             _p(fs.U), _p(fs.sigma), _p(fs.W))

@@ -511,3 +511,36 @@ def test_pair_screening_bounds_and_energy_screen():
             dropped = sum(-m[k] * (th[:, pj[k]] @ Ys[k] @ th[:, pi[k]]) for k in np.nonzero(drop)[0])     # Eq. 17 per pair
             assert abs(ek_scr + dropped - ek_full) <= 1e-8 * abs(ek_full) + 1e-9 * (m * s1 * nrm[pi] * nrm[pj])[drop].sum() + 1e-12
             assert abs(ek_scr - ek_full) <= (m * s1 * nrm[pi] * nrm[pj])[drop].sum() * (1 + 1e-9)
+
+
+def test_randomized_svd_pins():
+    """Pins of oracle.randomized_svd (NEXT-4).  (i) A matrix of exact rank 9 built from known singular values
+    and orthonormal factors: the sketch (k = 16) returns those singular values to 1e-12, a residual at rounding level and
+    the same truncated matrix as LAPACK.  (ii) A full-rank block: the reported residual is the true error of the rank-k
+    approximation, never below the optimum sqrt(sum_{K>k} sigma_K^2) (Eckart-Young) -- what lets a caller reject the
+    sketch -- and every returned singular value is within resid of LAPACK's (Weyl).  (iii) A rank-deficient pair block
+    of the "vector" reading of the generator."""
+    rng = np.random.default_rng(5)
+    n, r, k = 40, 9, 16
+    A, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    Bm, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    sig = np.array([7.0, 3.0, 2.5, 1.0, 0.3, 0.1, 1e-2, 1e-4, 1e-6])
+    Y = (A[:, :r] * sig) @ Bm[:, :r].T
+    Ut, s, Wt, resid = oracle.randomized_svd(Y, rng.standard_normal((n, k)))
+    assert np.abs(s[:r] - sig).max() <= 1e-12 * sig[0] and s[r:].max() <= 1e-13 * sig[0] and resid <= 1e-13 * sig[0]
+    assert np.abs((Ut[:r].T * s[:r]) @ Wt[:r] - Y).max() <= 1e-13 * sig[0]
+    assert np.abs(np.abs(np.sum(Ut[:r] * A[:, :r].T, axis=1)) - 1).max() <= 1e-9        # same vectors up to sign
+    assert np.abs(Ut @ Ut.T - np.eye(k)).max() <= 1e-12 and np.abs(Wt @ Wt.T - np.eye(k)).max() <= 1e-12
+    Yf = rng.standard_normal((n, n)) * np.exp(-0.2 * np.arange(n))[None, :]
+    sl = np.linalg.svd(Yf, compute_uv=False)
+    Ut, s, Wt, resid = oracle.randomized_svd(Yf, rng.standard_normal((n, k)))
+    assert resid >= np.sqrt((sl[k:] ** 2).sum()) * (1 - 1e-12) and resid <= 20 * np.sqrt((sl[k:] ** 2).sum())
+    assert np.abs(np.linalg.norm(Yf - (Ut.T * s) @ Wt) - resid) <= 1e-12 * sl[0]
+    assert (np.abs(s - sl[:k]) <= resid * (1 + 1e-12)).all()
+    P = gen.make_problem(0, reading="vector")
+    Lbar, _ = oracle.half_rotate(P.L, P.h, P.psi[0])
+    Yv = oracle.pair_eri(Lbar, 1, 4)
+    slv = np.linalg.svd(Yv, compute_uv=False)
+    assert (slv > 1e-10 * slv[0]).sum() <= 4                                       # rank <= number of sites
+    Ut, s, Wt, resid = oracle.randomized_svd(Yv, rng.standard_normal((P.N, 8)))
+    assert resid <= 1e-13 * slv[0] and np.abs(s[:4] - slv[:4]).max() <= 1e-12 * slv[0]
