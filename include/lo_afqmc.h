@@ -60,6 +60,8 @@ typedef struct {
     double svd_offdiag_max;          /* and the largest normalised off-diagonal |g_p.g_q|/(|g_p||g_q|) left at the end */
     double setup_seconds;            /* wall time of lo_setup, and of its pair Gram + SVD part */
     double setup_svd_seconds;
+    int rsvd_sketch;                 /* sketch rows of LO_SETUP_RANDOMIZED_SVD (0: full SVDs only) */
+    long long n_pairs_rsvd;          /* pair blocks whose randomised sketch was accepted */
     long long n_pairs_prescreened;   /* pairs given rank 0 by the rigorous pre-SVD norm bounds (no SVD was run for them) */
     long long n_pairs_energy_screened; /* pairs dropped by lo_screen_pairs (m_ij sigma_1 <= energy_screen_cutoff) */
     double energy_screen_cutoff;     /* 0 when no energy screen was applied */
@@ -91,6 +93,16 @@ enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_
  * (Eq. 18 would discard every singular value of such a pair); only the recorded first discarded singular value of a
  * screened pair is its bound instead of sigma_1.  lo_info.n_pairs_prescreened counts them. */
 #define LO_SETUP_NO_PRESCREEN 4
+/* flags bit 3 (LO_SETUP_RANDOMIZED_SVD, "approximate versions of the singular value decomposition,
+ * which would reduce the scaling of this step significantly"): every pair block is first decomposed through
+ * a randomised sketch of k rows (Gaussian test matrix from a fixed counter-based generator; range finder, projected
+ * block, small SVD; k = 16 x (bits 8..15 of flags), default 64, at most 128 and N/4) whose a-posteriori error
+ * |Y - U^T sigma W|_F is formed explicitly; a block is accepted only when that error is <= 16 N 2^-53 |Y|_F, i.e. when its
+ * numerical rank is below k and the sketch IS its SVD to working accuracy (every singular value of Y is within the error of
+ * a returned one).  All other blocks are decomposed by the full method.  The factor set is therefore the same to rounding
+ * (tests pin it to LAPACK either way); what changes is the setup time of low-rank problems.  lo_info.n_pairs_rsvd counts
+ * the accepted blocks. */
+#define LO_SETUP_RANDOMIZED_SVD 8
 lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const double* h, const double* L,
                    const double* psi_a, const double* psi_b, double threshold, int device, int max_walkers,
                    unsigned flags, lo_factors** out);

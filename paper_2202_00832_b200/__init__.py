@@ -16,6 +16,7 @@ from . import build as _build
 LO_SETUP_GPU_SVD = 1
 LO_SETUP_PROPAGATOR = 2
 LO_SETUP_NO_PRESCREEN = 4
+LO_SETUP_RANDOMIZED_SVD = 8
 K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_screen_pairs", "lo_local_energy",
@@ -35,7 +36,8 @@ class LoInfo(C.Structure):
                 ("max_rank", C.c_int), ("min_rank", C.c_int), ("factor_bytes", C.c_ulonglong), ("lbar_bytes", C.c_ulonglong),
                 ("workspace_bytes", C.c_ulonglong), ("threshold", C.c_double), ("device", C.c_int), ("max_walkers", C.c_int),
                 ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong), ("svd_sweeps_max", C.c_int), ("svd_offdiag_max", C.c_double),
-                ("setup_seconds", C.c_double), ("setup_svd_seconds", C.c_double), ("n_pairs_prescreened", C.c_longlong),
+                ("setup_seconds", C.c_double), ("setup_svd_seconds", C.c_double), ("rsvd_sketch", C.c_int),
+                ("n_pairs_rsvd", C.c_longlong), ("n_pairs_prescreened", C.c_longlong),
                 ("n_pairs_energy_screened", C.c_longlong), ("energy_screen_cutoff", C.c_double), ("energy_screen_bound", C.c_double)]
 
 
@@ -106,8 +108,9 @@ class Factors:
         self._h = C.c_void_p(handle)
 
     @classmethod
-    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False, propagator=False, prescreen=True):
-        """lo_setup: h [N,N], L [n_chol,N,N], psis = [psi] (closed shell) or [psi_a, psi_b]; host numpy arrays."""
+    def setup(cls, h, L, psis, threshold, device=0, max_walkers=1, gpu_svd=False, propagator=False, prescreen=True, rsvd=0):
+        """lo_setup: h [N,N], L [n_chol,N,N], psis = [psi] (closed shell) or [psi_a, psi_b]; host numpy arrays.
+        rsvd = k > 0: LO_SETUP_RANDOMIZED_SVD with a sketch of k rows (a multiple of 16)."""
         h, L = _np(h, np.float64), _np(L, np.float64)
         psis = [_np(p, np.float64) for p in psis]
         N, n_chol = h.shape[0], L.shape[0]
@@ -116,7 +119,8 @@ class Factors:
         st = lib().lo_setup(N, n_chol, len(psis), n_occ, h.ctypes.data, L.ctypes.data, psis[0].ctypes.data,
                             psis[1].ctypes.data if len(psis) == 2 else None, float(threshold), int(device), int(max_walkers),
                             (LO_SETUP_GPU_SVD if gpu_svd else 0) | (LO_SETUP_PROPAGATOR if propagator else 0) |
-                            (0 if prescreen else LO_SETUP_NO_PRESCREEN), C.byref(out))
+                            (0 if prescreen else LO_SETUP_NO_PRESCREEN) |
+                            ((LO_SETUP_RANDOMIZED_SVD | ((int(rsvd) // 16) << 8)) if rsvd else 0), C.byref(out))
         _check(st)
         return cls(out.value)
 

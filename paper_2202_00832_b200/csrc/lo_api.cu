@@ -402,6 +402,13 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
     }
     for (int s = 0; s < n_spin; ++s)
         if (n_occ[s] <= 0 || n_occ[s] > N) { set_error("lo_setup: n_occ out of range"); return LO_EINVAL; }
+    int rsvd_k = 0;
+    if (flags & LO_SETUP_RANDOMIZED_SVD) {
+        // sketch size: bits 8..15 of flags in units of 16 rows, default 64; the sketches live in the V scratch of a block
+        rsvd_k = (int)((flags >> 8) & 0xffu) * 16;
+        if (rsvd_k == 0) rsvd_k = 64;
+        if (rsvd_k > 128 || 4 * rsvd_k > N) rsvd_k = 0;       // block too small for a sketch to pay: full method only
+    }
     if ((flags & (LO_SETUP_GPU_SVD | LO_SETUP_PROPAGATOR)) && device < 0) {
         set_error("lo_setup: LO_SETUP_GPU_SVD / LO_SETUP_PROPAGATOR need device >= 0");
         return LO_EINVAL;
@@ -468,6 +475,7 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
         if (st != LO_OK) { free_all(f); return st; }
         const bool on_gpu = (flags & LO_SETUP_GPU_SVD) != 0;
         f->setup_on_gpu = on_gpu ? 1 : 0;
+        f->rsvd_k = rsvd_k;
         size_t B = 256;   // pairs per batch
         double *tY = nullptr, *tV = nullptr, *tU = nullptr, *tW = nullptr, *dSig = nullptr;
         int* dOrd = nullptr;
@@ -509,19 +517,33 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             const double skip_below = prescreen ? threshold : -1.0;     // second screen: |Y|_F <= threshold, known once Y is formed
             if (n == 0) {
             } else if (on_gpu) {
-                st = gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data(), skip_below, &f->svd_stat);
+                st = rsvd_k ? gpu_pair_rsvd(f, spin, bi.data(), bj.data(), n, rsvd_k, tY, tV, tU, tW, dSig, dOrd, hSig.data(), skip_below, &f->svd_stat,
+                                            &f->n_rsvd_accepted)
+                            : gpu_pair_svd(f, spin, bi.data(), bj.data(), n, tY, tV, tU, tW, dSig, dOrd, hSig.data(), skip_below, &f->svd_stat);
                 if (st != LO_OK) break;
             } else {
                 stats_of_batch.assign(n, SvdStat());
                 std::vector<SvdStat>& stats = stats_of_batch;
 #pragma omp parallel
                 {
-                    std::vector<double> G((size_t)N * N), V((size_t)N * N), sg;
+                    std::vector<double> G((size_t)N * N), V((size_t)N * N), sg, rU, rW;
                     std::vector<int> order;
 #pragma omp for schedule(dynamic, 1)
                     for (int x = 0; x < n; ++x) {
                         host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[spin] + bi[x], f->o_base[spin] + bj[x], G.data());
-                        host_block_svd(N, G.data(), V.data(), sg, order, skip_below, &stats[x]);
+                        if (rsvd_k && host_pair_rsvd(N, rsvd_k, G.data(), sg, rU, rW, &stats[x])) {
+                            // the sketch captured the block: its factors are the SVD to working accuracy
+                            sg.resize(N, 0.0);
+                            std::copy(sg.begin(), sg.end(), hSig.begin() + (size_t)x * N);
+                            int r = 0;
+                            while (r < rsvd_k && sg[r] > threshold) ++r;
+                            pU[x].assign(rU.begin(), rU.begin() + (size_t)r * N);
+                            pW[x].assign(rW.begin(), rW.begin() + (size_t)r * N);
+#pragma omp atomic
+                            ++f->n_rsvd_accepted;
+                            continue;
+                        }
+                        host_block_svd(N, N, G.data(), V.data(), sg, order, skip_below, &stats[x]);
                         std::copy(sg.begin(), sg.end(), hSig.begin() + (size_t)x * N);
                         int r = 0;
                         while (r < N && sg[r] > threshold) ++r;
@@ -620,6 +642,7 @@ lo_status lo_info_get(const lo_factors* f, lo_info* info) {
     info->setup_on_gpu = f->setup_on_gpu; info->n_tiles = f->n_tiles;
     info->svd_sweeps_max = f->svd_stat.sweeps; info->svd_offdiag_max = f->svd_stat.offdiag;
     info->setup_seconds = f->setup_seconds; info->setup_svd_seconds = f->setup_svd_seconds;
+    info->rsvd_sketch = f->rsvd_k; info->n_pairs_rsvd = f->n_rsvd_accepted;
     info->n_pairs_prescreened = f->n_prescreened + f->svd_stat.screened;
     info->n_pairs_energy_screened = f->n_energy_screened; info->energy_screen_cutoff = f->energy_cutoff;
     info->energy_screen_bound = f->energy_bound;
@@ -671,6 +694,7 @@ static lo_status rebuild_from(const lo_factors* f, double looser, double pair_cu
     for (int s = 0; s < 2; ++s) { g->n_occ[s] = f->n_occ[s]; g->o_base[s] = f->o_base[s]; }
     g->threshold = looser; g->device = f->device; g->max_walkers = f->max_walkers; g->Wcap = f->Wcap; g->ldw = f->ldw;
     g->num_sms = f->num_sms; g->setup_on_gpu = f->setup_on_gpu; g->svd_stat = f->svd_stat; g->ops = f->ops; g->lbar_bytes = f->lbar_bytes;
+    g->rsvd_k = f->rsvd_k; g->n_rsvd_accepted = f->n_rsvd_accepted;
     g->n_prescreened = f->n_prescreened; g->setup_seconds = f->setup_seconds; g->setup_svd_seconds = f->setup_svd_seconds;
     g->n_energy_screened = f->n_energy_screened; g->energy_cutoff = std::max(f->energy_cutoff, pair_cutoff); g->energy_bound = f->energy_bound;
     try {

@@ -11,6 +11,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdint>
 #include <memory>
 #include <string>
@@ -133,6 +134,8 @@ struct lo_factors {
     int setup_on_gpu = 0;
     lo::SvdStat svd_stat;                // worst case over all pair blocks of lo_setup
     double setup_seconds = 0, setup_svd_seconds = 0;
+    long long n_rsvd_accepted = 0;       // pair blocks whose randomised sketch was accepted (LO_SETUP_RANDOMIZED_SVD)
+    int rsvd_k = 0;                      // sketch size, 0 = full SVD only
     long long n_prescreened = 0;         // pairs the norm bound removed before their block was formed
     long long n_energy_screened = 0;     // pairs lo_screen_pairs dropped (m_ij sigma_1 <= energy_cutoff)
     double energy_cutoff = 0, energy_bound = 0;   // and cK * sum over them of m_ij sigma_1
@@ -205,9 +208,29 @@ lo_status make_tmap(CUtensorMap* tm, const void* base, unsigned long long inner,
 
 // Pair-block SVD (lo_svd.cu): block one-sided Jacobi with Gram subproblems, host and device versions.
 std::vector<int> svd_schedule(int n_blocks);
-void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, double skip_below, SvdStat* stat);
-cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, double skip_below, int* dSweeps, double* dOff,
-                                cudaStream_t stream);
+void host_block_svd(int R, int len, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, double skip_below, SvdStat* stat);
+cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int len, int ld, int ldv, const int* dSched, double skip_below, int* dSweeps,
+                                double* dOff, const int* dIdx, size_t stride, cudaStream_t stream);
+
+// Counter-based standard normal numbers for the test matrix of the randomised SVD: SplitMix64 of (seed + index) gives two
+// uniforms, Box-Muller one Gaussian.  Host and device versions are the same function.
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+inline double gauss_at(unsigned long long seed, unsigned long long index) {
+    unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (2 * index + 1);
+    unsigned long long u[2];
+    for (int r = 0; r < 2; ++r) {
+        z += 0x9E3779B97F4A7C15ull;
+        unsigned long long y = z;
+        y = (y ^ (y >> 30)) * 0xBF58476D1CE4E5B9ull;
+        y = (y ^ (y >> 27)) * 0x94D049BB133111EBull;
+        u[r] = y ^ (y >> 31);
+    }
+    const double a = ((double)(u[0] >> 11) + 0.5) * (1.0 / 9007199254740992.0);      // (0, 1)
+    const double b = ((double)(u[1] >> 11)) * (1.0 / 9007199254740992.0);            // [0, 1)
+    return sqrt(-2.0 * log(a)) * cos(6.283185307179586 * b);
+}
 
 // GPU setup (lo_setup_gpu.cu): pair Gram matrices + block-Jacobi SVD (lo_svd.cu) for a batch of pairs of one spin.
 // For the n listed pairs: returns sigma (descending, [n][N]) on the host and leaves the sorted U/W rows on the
@@ -215,6 +238,13 @@ cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, 
 lo_status gpu_pair_svd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, double* tmpY, double* tmpV,
                        double* tmpU, double* tmpW, double* dSigma, int* dOrder, double* hSigma, double skip_below, SvdStat* stat);
 size_t gpu_pair_svd_bytes_per_pair(int N, int N_pad);
+// Randomised variant (LO_SETUP_RANDOMIZED_SVD): sketch of k rows, a-posteriori residual check, full method for the blocks
+// the sketch does not capture; *n_accepted counts the blocks whose sketch was accepted.
+lo_status gpu_pair_rsvd(const lo_factors* f, int spin, const int* pi, const int* pj, int n, int k, double* tmpY, double* tmpV, double* tmpU,
+                        double* tmpW, double* dSigma, int* dOrder, double* hSigma, double skip_below, SvdStat* stat, long long* n_accepted);
+// Host version for one pair block G (N x N, rows = columns of Y): returns true and the factors (sigma [k], U rows, W rows,
+// k x N each) when the sketch is accepted.
+bool host_pair_rsvd(int N, int k, const double* G, std::vector<double>& sigma, std::vector<double>& U, std::vector<double>& W, SvdStat* stat);
 // dst[rec.dst_row + K][:] = src[rec.src_row + K][:] for K < rec.r, every rec of the host table (rows of N_pad doubles).
 lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table, int n, int N_pad);
 

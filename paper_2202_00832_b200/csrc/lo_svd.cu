@@ -96,28 +96,31 @@ void sym_jacobi_host(int m, double* S, double* Q, int ld, const bool* live, doub
 
 }  // namespace
 
-// Host version.  G: n rows of length n (row c = column c of Y), overwritten; V (n x n) receives the accumulated
-// transformation.  sigma: descending; order[K] = row of G / V that holds singular triplet K.
-void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, double skip_below, SvdStat* stat) {
-    const int B = SVD_B, nb = (n + B - 1) / B, M = 2 * B;
-    std::fill(V, V + (size_t)n * n, 0.0);
-    for (int c = 0; c < n; ++c) V[(size_t)c * n + c] = 1.0;
+// Host version.  G: R rows of length len (for a pair block: R = len = N, row c = column c of Y), overwritten by the
+// orthogonalised rows; V (R x R, may be NULL) receives the accumulated transformation.  sigma: the row lengths,
+// descending; order[K] = row of G / V that holds singular triplet K.
+void host_block_svd(int R, int len, double* G, double* V, std::vector<double>& sigma, std::vector<int>& order, double skip_below, SvdStat* stat) {
+    const int B = SVD_B, nb = (R + B - 1) / B, M = 2 * B, dim = std::max(R, len);
+    if (V) {
+        std::fill(V, V + (size_t)R * R, 0.0);
+        for (int c = 0; c < R; ++c) V[(size_t)c * R + c] = 1.0;
+    }
     double fro2 = 0;
-    for (size_t k = 0; k < (size_t)n * n; ++k) fro2 += G[k] * G[k];
+    for (size_t k = 0; k < (size_t)R * len; ++k) fro2 += G[k] * G[k];
     if (std::sqrt(fro2) * (1.0 + 1e-12) <= skip_below) {
         // sigma_1 <= |Y|_F <= threshold: rank 0 whatever the vectors are (second level of the pair screen); sigma_1 is
         // reported as its bound |Y|_F
-        sigma.assign(n, 0.0);
+        sigma.assign(R, 0.0);
         sigma[0] = std::sqrt(fro2) * (1.0 + 1e-12);
-        order.resize(n);
+        order.resize(R);
         std::iota(order.begin(), order.end(), 0);
         if (stat) { stat->sweeps = 0; stat->offdiag = 0; stat->converged = true; stat->screened = 1; }
         return;
     }
-    const double tau = n * SVD_U, null2 = tau * tau * fro2 / n;
+    const double tau = dim * SVD_U, null2 = tau * tau * fro2 / dim;
     const std::vector<int> sched = svd_schedule(nb);
     const int half = std::max(2, nb + (nb & 1)) / 2, rounds = 2 * half - 1;
-    std::vector<double> S((size_t)M * M), Q((size_t)M * M), Qs, tmp((size_t)M * n);
+    std::vector<double> S((size_t)M * M), Q((size_t)M * M), Qs, tmp((size_t)M * std::max(len, R));
     int rows[2 * SVD_B];
     bool live[2 * SVD_B];
     int sweep = 0;
@@ -130,14 +133,14 @@ void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std
                 const int bI = sched[((size_t)round * half + k) * 2], bJ = sched[((size_t)round * half + k) * 2 + 1];
                 int m = 0;
                 for (int blk : {bI, bJ})
-                    for (int c = blk * B; c < std::min(n, (blk + 1) * B); ++c)
+                    for (int c = blk * B; c < std::min(R, (blk + 1) * B); ++c)
                         if (blk < nb) rows[m++] = c;
                 if (m < 2) continue;
                 for (int a = 0; a < m; ++a)
                     for (int b = a; b < m; ++b) {
-                        const double *x = G + (size_t)rows[a] * n, *y = G + (size_t)rows[b] * n;
+                        const double *x = G + (size_t)rows[a] * len, *y = G + (size_t)rows[b] * len;
                         double acc = 0;
-                        for (int e = 0; e < n; ++e) acc += x[e] * y[e];
+                        for (int e = 0; e < len; ++e) acc += x[e] * y[e];
                         S[a * M + b] = S[b * M + a] = acc;
                     }
                 double off = 0;
@@ -158,40 +161,101 @@ void host_block_svd(int n, double* G, double* V, std::vector<double>& sigma, std
                     for (int t = 0; t < nl; ++t)
                         for (int b = 0; b < m; ++b) Q[b * M + place[t]] = Qs[b * M + from[t]];
                 }
-                for (double* X : {G, V}) {          // rows <- Q^T rows
+                for (int pass = 0; pass < (V ? 2 : 1); ++pass) {          // rows <- Q^T rows
+                    double* X = pass == 0 ? G : V;
+                    const int w = pass == 0 ? len : R;
                     for (int a = 0; a < m; ++a) {
-                        double* t = tmp.data() + (size_t)a * n;
-                        std::fill(t, t + n, 0.0);
+                        double* t = tmp.data() + (size_t)a * w;
+                        std::fill(t, t + w, 0.0);
                         for (int b = 0; b < m; ++b) {
-                            const double w = Q[b * M + a];
-                            if (w == 0.0) continue;
-                            const double* x = X + (size_t)rows[b] * n;
-                            for (int e = 0; e < n; ++e) t[e] += w * x[e];
+                            const double q = Q[b * M + a];
+                            if (q == 0.0) continue;
+                            const double* x = X + (size_t)rows[b] * w;
+                            for (int e = 0; e < w; ++e) t[e] += q * x[e];
                         }
                     }
-                    for (int a = 0; a < m; ++a) std::memcpy(X + (size_t)rows[a] * n, tmp.data() + (size_t)a * n, (size_t)n * 8);
+                    for (int a = 0; a < m; ++a) std::memcpy(X + (size_t)rows[a] * w, tmp.data() + (size_t)a * w, (size_t)w * 8);
                 }
             }
         if (!touched) break;
     }
     if (stat) { stat->sweeps = sweep; stat->offdiag = worst; stat->converged = sweep < SVD_MAX_SWEEPS; }
-    std::vector<double> len(n);
-    for (int c = 0; c < n; ++c) {
+    std::vector<double> rl(R);
+    for (int c = 0; c < R; ++c) {
         double a = 0;
-        for (int e = 0; e < n; ++e) a += G[(size_t)c * n + e] * G[(size_t)c * n + e];
-        len[c] = std::sqrt(a);
+        for (int e = 0; e < len; ++e) a += G[(size_t)c * len + e] * G[(size_t)c * len + e];
+        rl[c] = std::sqrt(a);
     }
-    order.resize(n);
+    order.resize(R);
     std::iota(order.begin(), order.end(), 0);
-    std::sort(order.begin(), order.end(), [&](int x, int y) { return len[x] != len[y] ? len[x] > len[y] : x < y; });
-    sigma.resize(n);
-    for (int K = 0; K < n; ++K) sigma[K] = len[order[K]];
+    std::sort(order.begin(), order.end(), [&](int x, int y) { return rl[x] != rl[y] ? rl[x] > rl[y] : x < y; });
+    sigma.resize(R);
+    for (int K = 0; K < R; ++K) sigma[K] = rl[order[K]];
+}
+
+// Host version of the randomised SVD of one pair block (steps as in gpu_pair_rsvd, lo_setup_gpu.cu): G = Y^T, N x N.
+bool host_pair_rsvd(int N, int k, const double* G, std::vector<double>& sigma, std::vector<double>& U, std::vector<double>& W, SvdStat* stat) {
+    std::vector<double> Zt((size_t)k * N, 0.0), Bp((size_t)k * N, 0.0), Vr((size_t)k * k), sg;
+    std::vector<int> order;
+    const unsigned long long seed = 0x2202008320000000ull + (unsigned long long)k;
+    for (int q = 0; q < N; ++q)                                   // Zt[kk][q] = sum_p Om[p][kk] G[q][p]
+        for (int p = 0; p < N; ++p) {
+            const double g = G[(size_t)q * N + p];
+            for (int kk = 0; kk < k; ++kk) Zt[(size_t)kk * N + q] += gauss_at(seed, (unsigned long long)p * k + kk) * g;
+        }
+    SvdStat st1, st2;
+    host_block_svd(k, N, Zt.data(), nullptr, sg, order, -1.0, &st1);
+    for (int kk = 0; kk < k; ++kk) {                              // orthonormal rows; a null row (sketch wider than the rank) -> 0
+        double a = 0;
+        for (int q = 0; q < N; ++q) a += Zt[(size_t)kk * N + q] * Zt[(size_t)kk * N + q];
+        const double tau = N * SVD_U, inv = a > tau * tau * sg[0] * sg[0] ? 1.0 / std::sqrt(a) : 0.0;
+        for (int q = 0; q < N; ++q) Zt[(size_t)kk * N + q] *= inv;
+    }
+    for (int kk = 0; kk < k; ++kk)                                // Bp = Pt G
+        for (int q = 0; q < N; ++q) {
+            const double pz = Zt[(size_t)kk * N + q];
+            if (pz == 0.0) continue;
+            for (int c = 0; c < N; ++c) Bp[(size_t)kk * N + c] += pz * G[(size_t)q * N + c];
+        }
+    host_block_svd(k, N, Bp.data(), Vr.data(), sg, order, -1.0, &st2);
+    std::vector<double> Wf((size_t)k * N, 0.0);                   // Wf = Vr Pt
+    for (int K = 0; K < k; ++K)
+        for (int kk = 0; kk < k; ++kk) {
+            const double v = Vr[(size_t)K * k + kk];
+            if (v == 0.0) continue;
+            for (int q = 0; q < N; ++q) Wf[(size_t)K * N + q] += v * Zt[(size_t)kk * N + q];
+        }
+    double r2 = 0, s2 = 0;                                        // |G - Wf^T Bp|_F^2 and |Bp|_F^2
+    for (int q = 0; q < N; ++q)
+        for (int c = 0; c < N; ++c) {
+            double acc = 0;
+            for (int K = 0; K < k; ++K) acc += Wf[(size_t)K * N + q] * Bp[(size_t)K * N + c];
+            const double d = G[(size_t)q * N + c] - acc;
+            r2 += d * d;
+        }
+    for (double v : sg) s2 += v * v;
+    if (stat) { stat->sweeps = std::max(st1.sweeps, st2.sweeps); stat->offdiag = std::max(st1.offdiag, st2.offdiag); stat->converged = true; }
+    if (!st1.converged || !st2.converged || !(std::sqrt(r2) <= 16.0 * N * SVD_U * std::sqrt(s2 + r2))) return false;
+    sigma = sg;
+    U.assign((size_t)k * N, 0.0);
+    W.assign((size_t)k * N, 0.0);
+    for (int K = 0; K < k; ++K) {
+        const int c = order[K];
+        const double inv = sg[K] > 0 ? 1.0 / sg[K] : 0.0;
+        for (int e = 0; e < N; ++e) {
+            U[(size_t)K * N + e] = Bp[(size_t)c * N + e] * inv;
+            W[(size_t)K * N + e] = Wf[(size_t)c * N + e];
+        }
+    }
+    return true;
 }
 
 // =====================================================================================================================
 // Device version: one CTA of SVD_WARPS warps per matrix; every warp owns whole block-pair subproblems of the current
 // round (Gram by DMMA from global memory, eigen-iteration in its own shared-memory slice, Q^T application by DMMA in
-// place); __syncthreads() separates the rounds.  G, V: [rows = n][ld] row-major, ld a multiple of 8, columns >= n zero.
+// place); __syncthreads() separates the rounds.  G: [n rows][ld] row-major, V: [n][ldv] (or NULL: no accumulation), ld and
+// ldv multiples of 8, padding columns zero.  For a pair block n = N and ld = ldv = N_pad; the randomised path also runs it
+// on k x N_pad sketches (n = k rows).
 // =====================================================================================================================
 namespace {
 
@@ -278,17 +342,18 @@ __device__ void sym_jacobi_warp(double* S, double* Q, double* cs, int* pq, doubl
     __syncwarp();
 }
 
-__global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restrict__ Gall, double* __restrict__ Vall, int n, int ld,
+__global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restrict__ Gall, double* __restrict__ Vall, int n, int len, int ld, int ldv,
                                                                  const int* __restrict__ sched, int half, int max_sweeps, double skip_below,
-                                                                 int* __restrict__ sweeps_out, double* __restrict__ off_out) {
+                                                                 int* __restrict__ sweeps_out, double* __restrict__ off_out,
+                                                                 const int* __restrict__ idx, size_t stride) {
     extern __shared__ double sm[];
     __shared__ int s_touched;
     __shared__ double s_red[SVD_WARPS];
     __shared__ double s_off[SVD_WARPS];
-    const int x = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int x = idx ? idx[blockIdx.x] : blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
-    double* G = Gall + (size_t)x * n * ld;
-    double* V = Vall + (size_t)x * n * ld;
+    double* G = Gall + (size_t)x * stride;                        // matrix x (statistics go to slot x as well)
+    double* V = Vall ? Vall + (size_t)x * stride : nullptr;       // n rows of ldv >= n columns (a multiple of 8), or no accumulation
     double* S = sm + (size_t)warp * (2 * SVD_M * SVD_LDS + 2 * SVD_M);
     double* Q = S + SVD_M * SVD_LDS;
     double* cs = Q + SVD_M * SVD_LDS;
@@ -296,11 +361,11 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
     // V = I, |Y|_F^2
     double fro = 0;
     for (size_t e = tid; e < (size_t)n * ld; e += SVD_WARPS * 32) {
-        const int r = (int)(e / ld), c = (int)(e % ld);
-        V[e] = (r == c) ? 1.0 : 0.0;
         const double v = G[e];
         fro = fma(v, v, fro);
     }
+    if (V)
+        for (size_t e = tid; e < (size_t)n * ldv; e += SVD_WARPS * 32) V[e] = (e / ldv == e % ldv) ? 1.0 : 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) fro += __shfl_xor_sync(0xffffffffu, fro, o);
     if (lane == 0) s_red[warp] = fro;
@@ -311,7 +376,8 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
         if (tid == 0) { sweeps_out[x] = -1; off_out[x] = sqrt(fro) * (1.0 + 1e-12); }
         return;
     }
-    const double tau = n * SVD_U, null2 = tau * tau * fro / n;
+    const int dim = max(n, len);           // len = true row length (<= ld)
+    const double tau = dim * SVD_U, null2 = tau * tau * fro / dim;
     const int rounds = 2 * half - 1, nb = (n + SVD_B - 1) / SVD_B;
     int sweep = 0;
     double worst_cta = 0;
@@ -401,16 +467,17 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks) { rowk[ks] = grow(ks * 4 + t); okk[ks] = rowk[ks] < n && (ks < 4 || bJ < nb); }
 #pragma unroll 1
-                for (int pass = 0; pass < 2; ++pass) {
+                for (int pass = 0; pass < (V ? 2 : 1); ++pass) {
                     double* X = pass == 0 ? G : V;
+                    const int ldx = pass == 0 ? ld : ldv;
                     double bf[8];
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) bf[ks] = okk[ks] ? X[(size_t)rowk[ks] * ld + g] : 0.0;
-                    for (int c0 = 0; c0 < ld; c0 += 8) {
+                    for (int ks = 0; ks < 8; ++ks) bf[ks] = okk[ks] ? X[(size_t)rowk[ks] * ldx + g] : 0.0;
+                    for (int c0 = 0; c0 < ldx; c0 += 8) {
                         double nx[8];
                         const int c1 = c0 + 8;
 #pragma unroll
-                        for (int ks = 0; ks < 8; ++ks) nx[ks] = (c1 < ld && okk[ks]) ? X[(size_t)rowk[ks] * ld + c1 + g] : 0.0;
+                        for (int ks = 0; ks < 8; ++ks) nx[ks] = (c1 < ldx && okk[ks]) ? X[(size_t)rowk[ks] * ldx + c1 + g] : 0.0;
                         double d[4][2];
 #pragma unroll
                         for (int mt = 0; mt < 4; ++mt) d[mt][0] = d[mt][1] = 0.0;
@@ -421,7 +488,7 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
                         __syncwarp();                // every lane's loads of this column chunk are done before any store
 #pragma unroll
                         for (int mt = 0; mt < 4; ++mt)
-                            if (okt[mt]) *reinterpret_cast<double2*>(&X[(size_t)rowt[mt] * ld + c0 + 2 * t]) = make_double2(d[mt][0], d[mt][1]);
+                            if (okt[mt]) *reinterpret_cast<double2*>(&X[(size_t)rowt[mt] * ldx + c0 + 2 * t]) = make_double2(d[mt][0], d[mt][1]);
 #pragma unroll
                         for (int ks = 0; ks < 8; ++ks) bf[ks] = nx[ks];
                     }
@@ -444,10 +511,11 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
 
 size_t svd_kernel_smem() { return (size_t)SVD_WARPS * (2 * SVD_M * SVD_LDS + 2 * SVD_M) * 8; }
 
-// Batched device SVD driver step: orthogonalise the rows of the n_mat matrices in G (V <- accumulated transformation).
-// dSched: device copy of svd_schedule(ceil(n/16)); dSweeps [n_mat] int, dOff [n_mat] double receive the statistics.
-cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, const int* dSched, double skip_below, int* dSweeps, double* dOff,
-                                cudaStream_t stream) {
+// Batched device SVD driver step: orthogonalise the rows of n_mat matrices in G (V <- accumulated transformation); matrix
+// m of the launch is slot x = dIdx[m] (or m) at G + x * stride, V + x * stride.  dSched: device copy of
+// svd_schedule(ceil(n/16)); dSweeps[x], dOff[x] receive the statistics.
+cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int len, int ld, int ldv, const int* dSched, double skip_below, int* dSweeps,
+                                double* dOff, const int* dIdx, size_t stride, cudaStream_t stream) {
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_block_jacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)svd_kernel_smem());
@@ -455,7 +523,7 @@ cudaError_t launch_block_jacobi(double* G, double* V, int n_mat, int n, int ld, 
         configured = true;
     }
     const int nb = (n + SVD_B - 1) / SVD_B, half = std::max(2, nb + (nb & 1)) / 2;
-    k_block_jacobi<<<n_mat, SVD_WARPS * 32, svd_kernel_smem(), stream>>>(G, V, n, ld, dSched, half, SVD_MAX_SWEEPS, skip_below, dSweeps, dOff);
+    k_block_jacobi<<<n_mat, SVD_WARPS * 32, svd_kernel_smem(), stream>>>(G, V, n, len, ld, ldv, dSched, half, SVD_MAX_SWEEPS, skip_below, dSweeps, dOff, dIdx, stride);
     return cudaGetLastError();
 }
 

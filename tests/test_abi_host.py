@@ -230,3 +230,26 @@ def test_energy_screen_matches_oracle_rule():
         assert abs(ic.energy_screen_bound - ms1[drop].sum()) <= 1e-12 * ms1[drop].sum()
     with pytest.raises(lo.LoError):
         F.screen_pairs(-1.0)
+
+
+def test_randomized_svd_setup_host_path():
+    """LO_SETUP_RANDOMIZED_SVD on the host path.  Rank-deficient blocks ("vector"
+    reading: rank <= 12 sites, sketch of 16 rows): every non-screened block is accepted, and the factors pass the same
+    LAPACK pin as the full method's (singular values 1e-12 sigma_1, ranks, truncated reconstructions, orthonormal rows).
+    Full-rank blocks ("element" reading): the a-posteriori check rejects every sketch and the full method's factor set
+    comes out bit for bit."""
+    xyz, fns = gen.site_geometry(1)
+    P = gen.make_problem_from_geometry(xyz, fns, (9,), 200, seed=11, reading="vector")
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-6, device=-1, max_walkers=4, rsvd=16)
+    info = F.info()
+    assert info.rsvd_sketch == 16 and info.n_pairs_rsvd + info.n_pairs_prescreened == info.n_pairs[0] == 45
+    Lbar = np.einsum("gpq,qi->gip", P.L, P.psi[0])
+    lapack_pin(F, 0, Lbar, [(i, j) for i in range(9) for j in range(i, 9)], 1e-6, P.N)
+    Ff = lo.Factors.setup(P.h, P.L, P.psi, 1e-6, device=-1, max_walkers=4)
+    assert np.array_equal(F.ranks(), Ff.ranks())
+    Pe = gen.make_problem_from_geometry(xyz, fns, (5,), 200, seed=11)
+    Fe = lo.Factors.setup(Pe.h, Pe.L, Pe.psi, 1e-6, device=-1, max_walkers=4, rsvd=16)
+    Fe0 = lo.Factors.setup(Pe.h, Pe.L, Pe.psi, 1e-6, device=-1, max_walkers=4)
+    assert Fe.info().n_pairs_rsvd == 0
+    for a, b in zip(Fe.factor_all(), Fe0.factor_all()):
+        assert np.array_equal(a, b)

@@ -282,6 +282,37 @@ def test_gpu_factors_pinned_to_lapack(c1, c2_built):
     assert 2 <= i2.svd_sweeps_max < 40 and i2.svd_offdiag_max <= P.N * 2.0 ** -53
 
 
+def test_randomized_svd_setup_device_path(c1):
+    """LO_SETUP_RANDOMIZED_SVD on the device.  configs[2] in the rank-deficient "vector"
+    reading (ranks 23..36, sketch of 64 rows): every pair block is accepted by the a-posteriori check, the factors pass the
+    LAPACK pin (32 |i-j|-stratified pairs) and give the same ranks as the full method, and the energies of 8 walkers match
+    the oracle on that factor set (1e-10).  configs[1] in the full-rank reading: every sketch is rejected and the factor set is
+    the full method's bit for bit."""
+    from test_abi_host import lapack_pin
+    P = gen.make_problem(2, reading="vector")
+    Fr = lo.Factors.setup(P.h, P.L, P.psi, 1e-5, device=0, max_walkers=8, gpu_svd=True, rsvd=64)
+    Ff = lo.Factors.setup(P.h, P.L, P.psi, 1e-5, device=0, max_walkers=8, gpu_svd=True)
+    ir, iff = Fr.info(), Ff.info()
+    assert ir.rsvd_sketch == 64 and ir.n_pairs_rsvd == ir.n_pairs[0] and iff.n_pairs_rsvd == 0
+    assert np.array_equal(Fr.ranks(), Ff.ranks()) and Fr.ranks().max() <= 36
+    print("setup seconds (SVD part): randomised %.2f (%.2f), full %.2f (%.2f)" % (ir.setup_seconds, ir.setup_svd_seconds, iff.setup_seconds, iff.setup_svd_seconds))
+    Lbar = np.einsum("gpq,qi->gip", P.L, P.psi[0])
+    pi, pj = np.triu_indices(P.n_occ[0])
+    order = np.argsort(pj - pi, kind="stable")
+    sel = order[np.linspace(0, len(pi) - 1, 32).astype(int)]
+    lapack_pin(Fr, 0, Lbar, [(int(pi[k]), int(pj[k])) for k in sel], 1e-5, P.N)
+    phis = gen.make_walkers(P, 8)
+    Eg, st = gpu_energy(Fr, phis)
+    Eo, _ = oracle_energy(P, Fr, phis)
+    assert (st == 0).all()
+    assert_parity(Eg, Eo)
+    Fe = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=8, gpu_svd=True, rsvd=16)
+    Fe0 = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=8, gpu_svd=True)
+    assert Fe.info().n_pairs_rsvd == 0
+    for a, b in zip(Fe.factor_all(), Fe0.factor_all()):
+        assert np.array_equal(a, b)
+
+
 def test_exact_energy_within_truncation_bound():
     # protocol (C): GPU LO energy vs the exact exchange, inside the bound of SURVEY 8c-D14
     P = gen.make_problem(1, reading="vector")
