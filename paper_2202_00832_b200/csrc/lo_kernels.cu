@@ -487,10 +487,15 @@ __device__ __forceinline__ CoItem co_item(long long q, int RB, int NB, int nspli
 
 // RAGGED (the batch is not a multiple of 64 walkers): the warps are numbered column-slice first (the two warps of a
 // 32-column slice sit on different schedulers) and a warp whose slice holds no walker issues no MMAs.
-template <bool RAGGED>
+// NWN = column slices of 32 real columns (16 walkers) the 8 consumer warps are spread over: 4 for whole 64-walker blocks
+// (warp tile 64 x 32), 2 / 1 for batches of <= 32 / <= 16 walkers (warp tiles 32 x 32 / 16 x 32: all warps keep working and
+// only the Theta rows that exist are staged, through the 32-row tensor map tmT32) -- the paper's batch of 16 walkers per
+// GPU ran on 2 of 8 warps before.
+template <bool RAGGED, int NWN>
 __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmT,
-                                                    double* __restrict__ Xpart, int Xp, int O_tot, int N_pad, int ldw, int RB, int NB,
-                                                    int nsplit, int n_cols) {
+                                                    const __grid_constant__ CUtensorMap tmT32, double* __restrict__ Xpart, int Xp, int O_tot,
+                                                    int N_pad, int ldw, int RB, int NB, int nsplit, int n_cols) {
+    constexpr int MF = 2 * NWN;                       // row fragments per warp
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t full = sbase + CO_STAGES * CO_STAGE_BYTES, empty = full + 8 * CO_STAGES;
@@ -517,32 +522,35 @@ __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUte
                     const int o = ks / KT, kt = ks - o * KT;
                     mbar_wait(empty + 8 * slot, phase ^ 1);
                     const uint32_t st = sbase + slot * CO_STAGE_BYTES, bar = full + 8 * slot;
-                    mbar_expect_tx(bar, CO_STAGE_BYTES);
+                    mbar_expect_tx(bar, NWN == 4 ? CO_STAGE_BYTES : (CO_BM + 32 * NWN) * 128);
                     tma_load_2d(st, &tmA, o * N_pad + kt * KTILE, it.rb * CO_BM, bar);
-                    tma_load_2d(st + CO_BM * 128, &tmT, kt * KTILE, o * ldw + it.nb * 128, bar);
+                    if constexpr (NWN == 4) tma_load_2d(st + CO_BM * 128, &tmT, kt * KTILE, o * ldw + it.nb * 128, bar);
+                    else
+                        for (int j = 0; j < NWN; ++j) tma_load_2d(st + (CO_BM + 32 * j) * 128, &tmT32, kt * KTILE, o * ldw + it.nb * 128 + 32 * j, bar);
                     if (++slot == CO_STAGES) { slot = 0; phase ^= 1; }
                 }
             }
         }
         return;
     }
-    // ===== 8 consumer warps (64 x 32 each)
+    // ===== 8 consumer warps (8 MF x 32 each)
     reg_inc_consumer();
-    const int cw = warp - 4, g = lane >> 2, t = lane & 3, wm = RAGGED ? (cw & 1) : (cw >> 2), wn = RAGGED ? (cw >> 1) : (cw & 3);
-    double acc[8][4][2];
+    const int cw = warp - 4, g = lane >> 2, t = lane & 3;
+    const int wm = NWN == 4 ? (RAGGED ? (cw & 1) : (cw >> 2)) : cw / NWN, wn = NWN == 4 ? (RAGGED ? (cw >> 1) : (cw & 3)) : cw % NWN;
+    double acc[MF][4][2];
 #pragma unroll
-    for (int a = 0; a < 8; ++a)
+    for (int a = 0; a < MF; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
-    const uint32_t a_row = (uint32_t)(wm * 64 + g) * 128, b_row = (uint32_t)(CO_BM + wn * 32 + g) * 128;
+    const uint32_t a_row = (uint32_t)(wm * MF * 8 + g) * 128, b_row = (uint32_t)(CO_BM + wn * 32 + g) * 128;
     int cslot = 0;
     uint32_t cphase = 0;
     for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
         const CoItem it = co_item(q, RB, NB, nsplit, ksteps);
-        if (RAGGED && it.nb * 128 + wn * 32 >= n_cols) {          // warp-uniform: no walker in this warp's 32 columns
+        if (RAGGED && NWN == 4 && it.nb * 128 + wn * 32 >= n_cols) {          // warp-uniform: no walker in this warp's 32 columns
             for (int s = 0; s < it.nsteps; ++s) {
                 mbar_wait(full + 8 * cslot, cphase);
                 __syncwarp();
@@ -556,14 +564,14 @@ __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUte
             const uint32_t st = sbase + cslot * CO_STAGE_BYTES;
 #pragma unroll
             for (int ks = 0; ks < KTILE / 4; ++ks) {
-                double a[8], b[4];
+                double a[MF], b[4];
 #pragma unroll
-                for (int mf = 0; mf < 8; ++mf) a[mf] = lds_f64(st + a_row + mf * 1024 + xo[ks]);
+                for (int mf = 0; mf < MF; ++mf) a[mf] = lds_f64(st + a_row + mf * 1024 + xo[ks]);
 #pragma unroll
                 for (int nf = 0; nf < 4; ++nf) b[nf] = lds_f64(st + b_row + nf * 1024 + xo[ks]);
                 if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
 #pragma unroll
-                for (int mf = 0; mf < 8; ++mf)
+                for (int mf = 0; mf < MF; ++mf)
 #pragma unroll
                     for (int nf = 0; nf < 4; ++nf) mma884(acc[mf][nf][0], acc[mf][nf][1], a[mf], b[nf]);
             }
@@ -571,10 +579,10 @@ __global__ void __launch_bounds__(384, 1) k_coulomb(const __grid_constant__ CUte
         }
         double* Xs = Xpart + (size_t)it.sp * Xp * ldw;
 #pragma unroll
-        for (int mf = 0; mf < 8; ++mf)
+        for (int mf = 0; mf < MF; ++mf)
 #pragma unroll
             for (int nf = 0; nf < 4; ++nf) {
-                int row = it.rb * CO_BM + wm * 64 + mf * 8 + g;
+                int row = it.rb * CO_BM + wm * MF * 8 + mf * 8 + g;
                 int col = it.nb * 128 + wn * 32 + nf * 8 + 2 * t;
                 *reinterpret_cast<double2*>(Xs + (size_t)row * ldw + col) = make_double2(acc[mf][nf][0], acc[mf][nf][1]);
                 acc[mf][nf][0] = acc[mf][nf][1] = 0.0;
@@ -1086,8 +1094,10 @@ ThFn th_fn(int mfb) {
 
 lo_status configure_kernels() {
     cudaError_t e;
-    e = cudaFuncSetAttribute(k_coulomb<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coulomb<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    e = cudaFuncSetAttribute(k_coulomb<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coulomb<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coulomb<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coulomb<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, CO_SMEM);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_coulomb): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     e = cudaFuncSetAttribute(k_exchange<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_exchange<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_SMEM);
@@ -1174,10 +1184,14 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         Timer tm(f, stream, LO_K_COULOMB);
         long long items = (long long)RB * NB * nsplit;
         int grid = (int)std::min<long long>(items, f->num_sms);
-        if (n_w % WALKER_TILE)
-            k_coulomb<true><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
+        if (n_w <= 16)
+            k_coulomb<true, 1><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->tmTheta32, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
+        else if (n_w <= 32)
+            k_coulomb<true, 2><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->tmTheta32, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
+        else if (n_w % WALKER_TILE)
+            k_coulomb<true, 4><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->tmTheta32, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
         else
-            k_coulomb<false><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
+            k_coulomb<false, 4><<<grid, 384, CO_SMEM, stream>>>(f->ops->tmLbar, f->tmTheta, f->tmTheta32, f->dXpart, f->Xp, f->O_tot, N_pad, ldw, RB, NB, nsplit, 2 * n_w);
         dim3 g2(NB * 2, RB);
         k_ej<<<g2, 256, 0, stream>>>(f->dXpart, EJpart, E1raw, f->Xp, ldw, nsplit, f->n_chol, Wcap);
     }
@@ -1234,9 +1248,9 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
         const long long items = (long long)RB * NB;
         const int grid = (int)std::min<long long>(items, f->num_sms);
         if (n_w % WALKER_TILE)
-            k_coulomb<true><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
+            k_coulomb<true, 4><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
         else
-            k_coulomb<false><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
+            k_coulomb<false, 4><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_propagator: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
