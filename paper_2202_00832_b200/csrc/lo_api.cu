@@ -339,7 +339,8 @@ lo_status upload_lt(lo_factors* f, const double* L) {
 void free_cas_plan(CasPlan* c) {
     if (!c) return;
     void* cp[] = {c->dHoles, c->dParts, c->dCoef, c->dTh0, c->dA0, c->dT, c->dG, c->dWd, c->dEv, c->dSt0, c->dHoleIdx, c->dKind, c->dS, c->dH, c->dPart,
-                  c->dStV, c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B};
+                  c->dStV, c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B, c->dHoleIdxB, c->dKindB, c->dSB, c->dHB,
+                  c->dPartB, c->dStVB, c->dThAct[0], c->dThAct[1], c->dZ[0], c->dZ[1], c->dEJu};
     for (void* q : cp)
         if (q) cudaFree(q);
     delete c;
@@ -875,6 +876,79 @@ static lo_status check_strings(int n_det, int max_exc, int n_ref, int n_orb, con
     return LO_OK;
 }
 
+// SMW-energy data of one spin (0: alpha / closed shell -> the plain fields of the plan, 1: beta -> the *B fields): hole
+// indices into the active set, per-determinant orbital kinds, the S / H intermediates, partial sums, the Theta0 tensor map.
+static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* holes, const int* parts, const std::vector<int>& act) {
+    const int n_orb = f->n_occ[spin], n_ref = spin == 0 ? c->n_ref : c->n_ref_b, n_det = c->n_det, max_exc = c->max_exc;
+    const size_t nv = (size_t)c->max_real * n_det, ne = (size_t)n_det * max_exc;
+    auto al = [&](void** p, size_t bytes) -> cudaError_t {
+        cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16));
+        if (e == cudaSuccess) e = cudaMemset(*p, 0, std::max<size_t>(bytes, 16));
+        return e;
+    };
+    const int n_act = (int)act.size();
+    const int na_pad = n_act <= 2 ? 2 : (n_act <= 4 ? 4 : 6);
+    const int NP = 2 + na_pad;
+    // tiles of this spin: the tile list holds spin 0's tiles first (enumerate_blocks)
+    long long t0 = 0, nt = 0;
+    for (const ExTile& t : f->hTiles) {
+        const bool mine = f->n_spin == 1 || (spin == 0 ? t.pi < f->o_base[1] : t.pi >= f->o_base[1]);
+        if (mine) ++nt;
+        else if (spin == 1 && nt == 0) ++t0;
+    }
+    c->tile0[spin] = spin == 0 ? 0 : t0;
+    c->ntile[spin] = nt;
+    std::vector<int> hidx(ne + 8, -1);
+    for (size_t k = 0; k < ne; ++k)
+        if (holes[k] >= 0) hidx[k] = (int)(std::find(act.begin(), act.end(), holes[k]) - act.begin());
+    for (int a = 0; a < 8; ++a) {
+        hidx[ne + a] = a < n_act ? act[a] : 0;          // A_set (padded with column 0) behind the indices
+        (spin == 0 ? c->hAct : c->hActB)[a] = hidx[ne + a];
+    }
+    std::vector<signed char> kind((size_t)n_det * n_orb);
+    for (int d = 0; d < n_det; ++d)
+        for (int x = 0; x < n_orb; ++x) {
+            signed char kd = x < n_ref ? 0 : -1;
+            for (int k = 0; k < max_exc; ++k) {
+                if (holes[(size_t)d * max_exc + k] == x) kd = -1;
+                if (parts[(size_t)d * max_exc + k] == x) kd = (signed char)(1 + k);
+            }
+            kind[(size_t)d * n_orb + x] = kd;
+        }
+    const int n_chunks = (int)((nt + 15) / 16);
+    int*& dHoleIdx = spin == 0 ? c->dHoleIdx : c->dHoleIdxB;
+    signed char*& dKind = spin == 0 ? c->dKind : c->dKindB;
+    int*& dStV = spin == 0 ? c->dStV : c->dStVB;
+    double*& dS = spin == 0 ? c->dS : c->dSB;
+    double*& dH = spin == 0 ? c->dH : c->dHB;
+    double*& dPart = spin == 0 ? c->dPart : c->dPartB;
+    double* dTh0 = spin == 0 ? c->dTh0 : c->dTh0B;
+    (spin == 0 ? c->n_act : c->n_actB) = n_act;
+    (spin == 0 ? c->NP : c->NPB) = NP;
+    (spin == 0 ? c->n_chunks : c->n_chunksB) = n_chunks;
+    CK(al((void**)&dHoleIdx, hidx.size() * 4));
+    CK(al((void**)&dKind, kind.size()));
+    CK(al((void**)&dStV, nv * 4));
+    CK(al((void**)&dS, (size_t)std::max<long long>(nt, 1) * c->max_real * NP * NP * 16));
+    CK(al((void**)&dH, (size_t)c->W0cap * n_orb * 9 * 16));
+    CK(al((void**)&dPart, (size_t)std::max(n_chunks, 1) * nv * 2 * 16));
+    CK(cudaMemcpy(dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(dKind, kind.data(), kind.size(), cudaMemcpyHostToDevice));
+    lo_status st = make_tmap(spin == 0 ? &c->tmTh0 : &c->tmTh0B, dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 16);
+    if (st != LO_OK) return st;
+    if (f->n_spin == 2) {
+        // Cholesky-route Coulomb term of the unrestricted SMW energy: gathered active panels and the Z intermediates
+        const size_t ldw0 = 2 * (size_t)c->W0cap, zcols = (size_t)f->Xp * f->O_tot;
+        CK(al((void**)&c->dThAct[spin], (size_t)na_pad * ldw0 * f->N_pad * 8));
+        CK(al((void**)&c->dZ[spin], (size_t)na_pad * ldw0 * zcols * 8));
+        st = make_tmap(&c->tmThAct[spin], c->dThAct[spin], f->N_pad, (unsigned long long)na_pad * ldw0, 128);
+        if (st == LO_OK && spin == 0) st = make_tmap(&c->tmLbarRows, f->ops->dLbar, f->N_pad, (unsigned long long)zcols, 128);
+        if (st != LO_OK) return st;
+        if (!c->dEJu) CK(al((void**)&c->dEJu, nv * 16));
+    }
+    return LO_OK;
+}
+
 // allocates and fills plan `c` (already sized); any failure leaves the partial allocations in `c` for the caller to free
 static lo_status fill_cas_plan(lo_factors* f, CasPlan* c, const int* holes, const int* parts, const double* coef, const std::vector<int>& act) {
     const int n_orb = f->n_occ[0], n_ref = c->n_ref, n_det = c->n_det, max_exc = c->max_exc;
@@ -898,32 +972,7 @@ static lo_status fill_cas_plan(lo_factors* f, CasPlan* c, const int* holes, cons
     CK(cudaMemcpy(c->dParts, parts, ne * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->dCoef, coef, (size_t)n_det * 8, cudaMemcpyHostToDevice));
     if (c->mode == LO_CAS_SMW_ENERGY) {
-        const int na_pad = c->n_act <= 2 ? 2 : (c->n_act <= 4 ? 4 : 6);
-        c->NP = 2 + na_pad;
-        std::vector<int> hidx(ne + 8, -1);
-        for (size_t k = 0; k < ne; ++k)
-            if (holes[k] >= 0) hidx[k] = (int)(std::find(act.begin(), act.end(), holes[k]) - act.begin());
-        for (int a = 0; a < 8; ++a) hidx[ne + a] = a < c->n_act ? act[a] : 0;          // A_set (padded with column 0) behind the indices
-        std::vector<signed char> kind((size_t)n_det * n_orb);
-        for (int d = 0; d < n_det; ++d)
-            for (int x = 0; x < n_orb; ++x) {
-                signed char kd = x < n_ref ? 0 : -1;
-                for (int k = 0; k < max_exc; ++k) {
-                    if (holes[(size_t)d * max_exc + k] == x) kd = -1;
-                    if (parts[(size_t)d * max_exc + k] == x) kd = (signed char)(1 + k);
-                }
-                kind[(size_t)d * n_orb + x] = kd;
-            }
-        c->n_chunks = (int)((f->n_tiles + 15) / 16);
-        CK(al((void**)&c->dHoleIdx, hidx.size() * 4));
-        CK(al((void**)&c->dKind, kind.size()));
-        CK(al((void**)&c->dStV, nv * 4));
-        CK(al((void**)&c->dS, (size_t)std::max<long long>(f->n_tiles, 1) * c->max_real * c->NP * c->NP * 16));
-        CK(al((void**)&c->dH, (size_t)c->W0cap * n_orb * 9 * 16));
-        CK(al((void**)&c->dPart, (size_t)std::max(c->n_chunks, 1) * nv * 2 * 16));
-        CK(cudaMemcpy(c->dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
-        CK(cudaMemcpy(c->dKind, kind.data(), kind.size(), cudaMemcpyHostToDevice));
-        lo_status st = make_tmap(&c->tmTh0, c->dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 16);
+        lo_status st = alloc_smw_spin(f, c, 0, holes, parts, act);
         if (st != LO_OK) return st;
     }
     return LO_OK;
@@ -933,10 +982,6 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
                            int max_real_walkers, int mode) {
     if (!f || !holes || !parts || !coef) { set_error("lo_set_cas_trial: NULL argument"); return LO_EINVAL; }
     if (f->device < 0) { set_error("lo_set_cas_trial: no device"); return LO_ECUDA; }
-    if (f->n_spin != 1 && mode != LO_CAS_DIRECT) {
-        set_error("lo_set_cas_trial: an unrestricted factor set (n_spin == 2) supports LO_CAS_DIRECT only");
-        return LO_EINVAL;
-    }
     const int n_orb = f->n_occ[0];
     if (mode != LO_CAS_DIRECT && mode != LO_CAS_SMW_ENERGY) { set_error("lo_set_cas_trial: mode must be LO_CAS_DIRECT or LO_CAS_SMW_ENERGY"); return LO_EINVAL; }
     if (n_ref <= 0 || n_ref > n_orb || n_det <= 0 || max_exc <= 0 || max_exc > CAS_MAX_EXC || max_real_walkers <= 0 ||
@@ -978,8 +1023,8 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
 
 lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, const int* parts_b) {
     if (!f || !holes_b || !parts_b) { set_error("lo_set_cas_trial_beta: NULL argument"); return LO_EINVAL; }
-    if (!f->cas || f->n_spin != 2 || f->cas->mode != LO_CAS_DIRECT) {
-        set_error("lo_set_cas_trial_beta: needs an unrestricted factor set and a preceding lo_set_cas_trial(..., LO_CAS_DIRECT) with the alpha strings");
+    if (!f->cas || f->n_spin != 2) {
+        set_error("lo_set_cas_trial_beta: needs an unrestricted factor set and a preceding lo_set_cas_trial with the alpha strings");
         return LO_EINVAL;
     }
     CasPlan* c = f->cas;
@@ -988,10 +1033,20 @@ lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, 
     lo_status st = check_strings(c->n_det, c->max_exc, n_ref_b, n_orb_b, holes_b, parts_b);
     if (st != LO_OK) return st;
     CK(cudaSetDevice(f->device));
-    void* old[] = {c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B};
+    std::vector<int> act;
+    for (size_t k = 0; k < (size_t)c->n_det * c->max_exc; ++k)
+        if (holes_b[k] >= 0 && std::find(act.begin(), act.end(), holes_b[k]) == act.end()) act.push_back(holes_b[k]);
+    std::sort(act.begin(), act.end());
+    if (c->mode == LO_CAS_SMW_ENERGY && act.size() > 6) {
+        set_error("lo_set_cas_trial_beta: LO_CAS_SMW_ENERGY supports at most 6 distinct hole columns per spin; use LO_CAS_DIRECT");
+        return LO_EINVAL;
+    }
+    void* old[] = {c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B, c->dHoleIdxB, c->dKindB, c->dSB, c->dHB, c->dPartB,
+                   c->dStVB, c->dThAct[1], c->dZ[1]};
     for (void* q : old)
         if (q) cudaFree(q);
     c->dHolesB = c->dPartsB = nullptr; c->dTh0B = c->dA0B = c->dTB = c->dGB = c->dWdB = nullptr; c->dSt0B = nullptr;
+    c->dHoleIdxB = nullptr; c->dKindB = nullptr; c->dSB = c->dHB = c->dPartB = nullptr; c->dStVB = nullptr; c->dThAct[1] = c->dZ[1] = nullptr;
     c->has_beta = false;
     c->n_ref_b = n_ref_b; c->n_virt_b = n_orb_b - n_ref_b;
     const size_t nv = (size_t)c->max_real * c->n_det, ne = (size_t)c->n_det * c->max_exc;
@@ -1010,6 +1065,10 @@ lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, 
     CK(al((void**)&c->dSt0B, (size_t)c->W0cap * 4));
     CK(cudaMemcpy(c->dHolesB, holes_b, ne * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(c->dPartsB, parts_b, ne * 4, cudaMemcpyHostToDevice));
+    if (c->mode == LO_CAS_SMW_ENERGY) {
+        st = alloc_smw_spin(f, c, 1, holes_b, parts_b, act);
+        if (st != LO_OK) return st;      // has_beta stays false: lo_local_energy_cas refuses to run
+    }
     c->has_beta = true;
     return LO_OK;
 }

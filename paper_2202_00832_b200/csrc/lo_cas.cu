@@ -54,7 +54,8 @@ template <int NP>
 __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
                                                       const __grid_constant__ CUtensorMap tmT0, const double* __restrict__ wgt,
                                                       const ExTile* __restrict__ tiles, long long n_items, int WB, int N_pad, int ldw0,
-                                                      const int* __restrict__ act /* [NP-2] */, double2* __restrict__ S, int n_w) {
+                                                      const int* __restrict__ act /* [NP-2] */, double2* __restrict__ S, int n_w,
+                                                      int pan_base /* first orbital of this spin in the factor set's numbering */) {
     constexpr int STAGE = CpCfg<NP>::STAGE_BYTES;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -83,8 +84,8 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
             for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
                 const ExTile tile = tiles[q / WB];
                 const int wb = (int)(q % WB);
-                pan[0] = tile.pi;
-                pan[1] = tile.pj;
+                pan[0] = tile.pi - pan_base;
+                pan[1] = tile.pj - pan_base;
                 // whole 64-row boxes of U and W whatever the tile's length (rows past the tile are never read): one TMA each
                 const uint32_t tx = (uint32_t)(2 * EX_BM + NP * 16) * 128;
                 for (int kt = 0; kt < KT; ++kt) {
@@ -261,7 +262,7 @@ template <int MAXE>     // compile-time bound of the excitation rank: the coeffi
 __global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const ExTile* __restrict__ tiles, long long n_tiles,
                                                     const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
                                                     const double2* __restrict__ G, double2* __restrict__ part, int n_w, int n_det, int max_exc,
-                                                    int n_orb, int NP, int n_vtot) {
+                                                    int n_orb, int NP, int n_vtot, int pan_base) {
     extern __shared__ __align__(16) double2 Ss[];      // [CE_CH][NP*NP]
     __shared__ int tx_s[CE_CH], ty_s[CE_CH];
     const int chunk = blockIdx.x, w = blockIdx.y, tid = threadIdx.x;
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ 
         const int tl = i / NP2;
         Ss[i] = S[((size_t)(t0 + tl) * n_w + w) * NP2 + (i - tl * NP2)];
     }
-    if (tid < nt) { tx_s[tid] = tiles[t0 + tid].pi; ty_s[tid] = tiles[t0 + tid].pj; }
+    if (tid < nt) { tx_s[tid] = tiles[t0 + tid].pi - pan_base; ty_s[tid] = tiles[t0 + tid].pj - pan_base; }
     __syncthreads();
     for (int d = tid; d < n_det; d += 128) {
         const size_t v = (size_t)w * n_det + d;
@@ -497,12 +498,124 @@ __global__ void k_cas_combine(const double2* __restrict__ Ev, const double2* __r
     if (st_out) st_out[w] = bad ? 1 : 0;
 }
 
+// ---- unrestricted SMW energy, Coulomb term by the Cholesky route (R9): for determinant d and spin s
+//   X^{g,d}_s = sum_x Lbar^g_x . Theta^d_x = X0^g_s + sum_k sum_x G'_s[k][x] Z_s[A-index of hole k][g][x],
+//   G'[k][x] = G_d[k][x] - [x == hole k],   Z_s[a][g][x] = Lbar^g_x . Theta0_{s, A_a}   (one DMMA GEMM per spin and call),
+// and E_J^d = 1/2 sum_g (X^{g,d}_alpha + X^{g,d}_beta)^2  (R6; no opposite-spin pair blocks needed).  X0 = X0_alpha + X0_beta
+// comes from the ordinary Coulomb kernel on the reference panels.  grid (ceil(n_det / 16), n_w), block 128 = 16
+// determinants x 8 Cholesky vectors; the Z rows of 8 Cholesky vectors sit in shared memory while the chunk's
+// determinants use them; sums over g in a fixed order.
+struct XjSpin {
+    const double* Z;          // [(a * ldw0 + 2w + c)][zcols]
+    const double2* G;         // [n_v][max_exc][n_orb]
+    const int* holes;         // [n_det][max_exc]
+    const int* holeIdx;       // [n_det][max_exc]
+    int n_orb, o_base, n_act;
+};
+__global__ void __launch_bounds__(128) k_cas_xj(XjSpin sa, XjSpin sb, const double* __restrict__ X0, int ldx0, int n_chol, int O_tot,
+                                                long long zcols, int ldw0, int n_det, int max_exc, double2* __restrict__ EJ) {
+    extern __shared__ __align__(16) double2 Zs[];      // [spin][a][x][8]
+    const int w = blockIdx.y, tid = threadIdx.x, dl = tid >> 3, gl = tid & 7;
+    const int d = blockIdx.x * 16 + dl;
+    const bool live = d < n_det;
+    const size_t v = (size_t)w * n_det + (live ? d : 0);
+    const XjSpin sp[2] = {sa, sb};
+    const int offB = sa.n_act * sa.n_orb * 8;
+    double sr = 0.0, si = 0.0;
+    for (int g0 = 0; g0 < n_chol; g0 += 8) {
+        __syncthreads();
+        for (int s = 0; s < 2; ++s) {
+            const XjSpin& S = sp[s];
+            double2* dst = Zs + (s ? offB : 0);
+            const int per = S.n_orb * 8, total = S.n_act * per;
+            for (int e = tid; e < total; e += 128) {
+                const int a = e / per, r = e - a * per, gg = r / S.n_orb, x = r - gg * S.n_orb;
+                double2 z = make_double2(0.0, 0.0);
+                if (g0 + gg < n_chol) {
+                    const size_t col = (size_t)(g0 + gg) * O_tot + S.o_base + x;
+                    z.x = S.Z[((size_t)a * ldw0 + 2 * w) * zcols + col];
+                    z.y = S.Z[((size_t)a * ldw0 + 2 * w + 1) * zcols + col];
+                }
+                dst[(a * S.n_orb + x) * 8 + gg] = z;
+            }
+        }
+        __syncthreads();
+        if (live && g0 + gl < n_chol) {
+            double xr = X0[(size_t)(g0 + gl) * ldx0 + 2 * w], xi = X0[(size_t)(g0 + gl) * ldx0 + 2 * w + 1];
+            for (int s = 0; s < 2; ++s) {
+                const XjSpin& S = sp[s];
+                const double2* zs = Zs + (s ? offB : 0);
+                const double2* Gv = S.G + v * max_exc * S.n_orb;
+                for (int k = 0; k < max_exc; ++k) {
+                    const int h = S.holes[(size_t)d * max_exc + k];
+                    if (h < 0) break;
+                    const double2* za = zs + (size_t)S.holeIdx[(size_t)d * max_exc + k] * S.n_orb * 8 + gl;
+                    const double2* gk = Gv + (size_t)k * S.n_orb;
+                    for (int x = 0; x < S.n_orb; ++x) {
+                        double2 c = gk[x];
+                        if (x == h) c.x -= 1.0;
+                        const double2 z = za[x * 8];
+                        xr = fma(c.x, z.x, fma(-c.y, z.y, xr));
+                        xi = fma(c.x, z.y, fma(c.y, z.x, xi));
+                    }
+                }
+            }
+            sr += xr * xr - xi * xi;
+            si += 2.0 * xr * xi;
+        }
+    }
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
+    if (live && gl == 0) EJ[v] = make_double2(0.5 * sr, 0.5 * si);
+}
+
+// Per virtual walker of an unrestricted trial: E_K^d = alpha + beta chunk partials (the factor weights carry the 1/2 per
+// spin), E1^d = sum over spins of [sum_{x ref non-hole} H[x][self] + sum_k sum_x G_d[k][x] H[x][hole k]] (R6: no factor 2),
+// E_J^d from k_cas_xj.
+struct EsSpin {
+    const double2* part; int n_chunks;
+    const double2* H; const signed char* kind; const int* holeIdx; const double2* G; int n_orb;
+};
+__global__ void __launch_bounds__(128) k_cas_esum_u(EsSpin sa, EsSpin sb, const double2* __restrict__ EJ, double2* __restrict__ Ev, int n_v,
+                                                    int n_det, int max_exc, int n_vtot) {
+    const int v = blockIdx.x * 128 + threadIdx.x;
+    if (v >= n_v) return;
+    const int w = v / n_det, d = v - w * n_det;
+    double2 ek = make_double2(0.0, 0.0), e1 = make_double2(0.0, 0.0);
+    const EsSpin sp[2] = {sa, sb};
+    for (int s = 0; s < 2; ++s) {
+        const EsSpin& S = sp[s];
+        for (int c = 0; c < S.n_chunks; ++c) {
+            const double2 a = S.part[((size_t)c * n_vtot + v) * 2];
+            ek.x += a.x; ek.y += a.y;
+        }
+        const signed char* kd = S.kind + (size_t)d * S.n_orb;
+        const int* hi = S.holeIdx + (size_t)d * max_exc;
+        const double2* Hw = S.H + (size_t)w * S.n_orb * 9;
+        const double2* Gv = S.G + (size_t)v * max_exc * S.n_orb;
+        for (int x = 0; x < S.n_orb; ++x) {
+            if (kd[x] < 0) continue;
+            if (kd[x] == 0) { e1.x += Hw[x * 9].x; e1.y += Hw[x * 9].y; }
+            for (int k = 0; k < max_exc && hi[k] >= 0; ++k) {
+                const double2 t1 = cmul(Gv[(size_t)k * S.n_orb + x], Hw[x * 9 + 1 + hi[k]]);
+                e1.x += t1.x; e1.y += t1.y;
+            }
+        }
+    }
+    const double2 ej = EJ[v];
+    Ev[4 * (size_t)v] = make_double2(e1.x + ej.x + ek.x, e1.y + ej.y + ek.y);
+    Ev[4 * (size_t)v + 1] = e1;
+    Ev[4 * (size_t)v + 2] = ej;
+    Ev[4 * (size_t)v + 3] = ek;
+}
+
 }  // namespace
 
 lo_status configure_cas_kernels() {
     cudaError_t e = cudaFuncSetAttribute(k_cas_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<4>::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<6>::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<8>::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_xj, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_cas_*): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
 }
@@ -514,63 +627,110 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const
                                   void* ovlp, int* walker_status, cudaStream_t stream) {
     CasPlan& c = *f->cas;
     const int n_orb = f->n_occ[0], n_v = n_w * c.n_det, ldw0 = 2 * c.W0cap;
+    const bool smw = c.mode != 0, unres = c.has_beta;
     launch_s1(f, n_w, f->ops->dPsi[0], n_orb, c.n_ref, phi, c.dA0, c.dSt0, c.dTh0, 0, ldw0, stream);
     k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[0], n_orb, c.dTh0, (double2*)c.dT, f->N, f->N_pad, c.n_ref, c.n_virt, ldw0);
-    int* stv = c.mode == 0 ? f->dStatus : c.dStV;
+    int* stv = smw ? c.dStV : f->dStatus;
+    int* stvB = smw ? c.dStVB : f->dStatus + f->Wcap;
     k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dT, c.dHoles, c.dParts, c.dCoef, c.dSt0, (double2*)c.dG, (double2*)c.dWd,
-                                                  stv, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb, c.has_beta ? 1 : 0);
-    if (c.has_beta) {
-        // unrestricted trial: the beta strings get their own SMW data; their Theta^d panels follow the alpha panels
+                                                  stv, n_v, c.n_det, c.max_exc, c.n_ref, c.n_virt, n_orb, unres ? 1 : 0);
+    if (unres) {
+        // unrestricted trial: the beta strings get their own SMW data; in the direct mode their Theta^d panels follow the alpha panels
         const int n_orb_b = f->n_occ[1];
         launch_s1(f, n_w, f->ops->dPsi[1], n_orb_b, c.n_ref_b, phi_b, c.dA0B, c.dSt0B, c.dTh0B, 0, ldw0, stream);
         k_cas_T<<<n_w, 256, 0, stream>>>(f->ops->dPsi[1], n_orb_b, c.dTh0B, (double2*)c.dTB, f->N, f->N_pad, c.n_ref_b, c.n_virt_b, ldw0);
         k_cas_coef<<<(n_v + 3) / 4, 128, 0, stream>>>((const double2*)c.dTB, c.dHolesB, c.dPartsB, c.dCoef, c.dSt0B, (double2*)c.dGB,
-                                                      (double2*)c.dWdB, f->dStatus + f->Wcap, n_v, c.n_det, c.max_exc, c.n_ref_b, c.n_virt_b,
-                                                      n_orb_b, 2);
-        dim3 g3b(n_v, n_orb_b, (f->N_pad + 127) / 128);
-        k_cas_theta<<<g3b, 128, 0, stream>>>(c.dTh0B, (const double2*)c.dGB, c.dHolesB, f->dThT, f->N_pad, c.n_ref_b, n_orb_b, c.n_det, c.max_exc,
-                                             ldw0, f->ldw, f->o_base[1]);
+                                                      (double2*)c.dWdB, stvB, n_v, c.n_det, c.max_exc, c.n_ref_b, c.n_virt_b, n_orb_b, 2);
+        if (!smw) {
+            dim3 g3b(n_v, n_orb_b, (f->N_pad + 127) / 128);
+            k_cas_theta<<<g3b, 128, 0, stream>>>(c.dTh0B, (const double2*)c.dGB, c.dHolesB, f->dThT, f->N_pad, c.n_ref_b, n_orb_b, c.n_det, c.max_exc,
+                                                 ldw0, f->ldw, f->o_base[1]);
+        }
     }
-    if (c.mode == 0) {
+    if (!smw) {
         dim3 g3(n_v, n_orb, (f->N_pad + 127) / 128);
         k_cas_theta<<<g3, 128, 0, stream>>>(c.dTh0, (const double2*)c.dG, c.dHoles, f->dThT, f->N_pad, c.n_ref, n_orb, c.n_det, c.max_exc, ldw0, f->ldw, 0);
         lo_status st = launch_s3_s5(f, n_v, nullptr, nullptr, nullptr, nullptr, nullptr, c.dEv, stream);
         if (st != LO_OK) return st;
     } else {
-        // rearranged SMW energy (Eq. 23): S intermediates once per (tile, walker), then small per-determinant forms
+        // rearranged SMW energy (Eq. 23), per spin: S intermediates once per (tile, walker), one-body intermediates, then small
+        // per-determinant forms (exchange, and for a closed-shell trial the compressed Coulomb term)
         const int WB = (n_w + 7) / 8;
-        const long long items = f->n_tiles * WB;
-        const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-        const int* actd = c.dHoleIdx + (size_t)c.n_det * c.max_exc;      // A_set stored behind the hole indices
-        if (c.NP == 4)
-            k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
-        else if (c.NP == 6)
-            k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
-        else
-            k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU, f->tmW, c.tmTh0, f->dWgt, f->dTiles, items, WB, f->N_pad, ldw0, actd, (double2*)c.dS, n_w);
-        const double* hbar = f->ops->dLbar + (size_t)f->n_chol * f->O_tot * f->N_pad;
-        k_cas_H<<<n_w, 256, 0, stream>>>(hbar, c.dTh0, actd, c.n_act, (double2*)c.dH, f->N, f->N_pad, c.n_ref, n_orb, ldw0);
-        const int n_chunks = (int)((f->n_tiles + CE_CH - 1) / CE_CH);
         const int n_vtot = c.max_real * c.n_det;
-        if (n_chunks > 0) {
-            dim3 g4(n_chunks, n_w);
-            const size_t sm4 = (size_t)CE_CH * c.NP * c.NP * 16;
-            if (c.max_exc <= 2)
-                k_cas_energy<2><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
-                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
-            else if (c.max_exc <= 4)
-                k_cas_energy<4><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
-                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
+        const double* hbar0 = f->ops->dLbar + (size_t)f->n_chol * f->O_tot * f->N_pad;
+        for (int s = 0; s < (unres ? 2 : 1); ++s) {
+            const int NP = s ? c.NPB : c.NP, n_act = s ? c.n_actB : c.n_act, n_orb_s = f->n_occ[s], n_ref_s = s ? c.n_ref_b : c.n_ref;
+            const int pan_base = f->o_base[s];
+            const long long nt = c.ntile[s];
+            const ExTile* tiles = f->dTiles + c.tile0[s];
+            const int* hidx = s ? c.dHoleIdxB : c.dHoleIdx;
+            const int* actd = hidx + (size_t)c.n_det * c.max_exc;      // A_set stored behind the hole indices
+            double2* S = (double2*)(s ? c.dSB : c.dS);
+            double* th0 = s ? c.dTh0B : c.dTh0;
+            const CUtensorMap& tm0 = s ? c.tmTh0B : c.tmTh0;
+            const long long items = nt * WB;
+            const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
+            if (NP == 4)
+                k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU, f->tmW, tm0, f->dWgt, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
+            else if (NP == 6)
+                k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU, f->tmW, tm0, f->dWgt, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
             else
-                k_cas_energy<8><<<g4, 128, sm4, stream>>>((const double2*)c.dS, f->dTiles, f->n_tiles, c.dKind, c.dHoleIdx, (const double2*)c.dG,
-                                                          (double2*)c.dPart, n_w, c.n_det, c.max_exc, n_orb, c.NP, n_vtot);
+                k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU, f->tmW, tm0, f->dWgt, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
+            k_cas_H<<<n_w, 256, 0, stream>>>(hbar0 + (size_t)pan_base * f->N_pad, th0, actd, n_act, (double2*)(s ? c.dHB : c.dH), f->N, f->N_pad,
+                                             n_ref_s, n_orb_s, ldw0);
+            const int n_chunks = (int)((nt + CE_CH - 1) / CE_CH);
+            if (n_chunks > 0) {
+                dim3 g4(n_chunks, n_w);
+                const size_t sm4 = (size_t)CE_CH * NP * NP * 16;
+                const signed char* kind = s ? c.dKindB : c.dKind;
+                const double2* G = (const double2*)(s ? c.dGB : c.dG);
+                double2* part = (double2*)(s ? c.dPartB : c.dPart);
+                if (c.max_exc <= 2)
+                    k_cas_energy<2><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base);
+                else if (c.max_exc <= 4)
+                    k_cas_energy<4><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base);
+                else
+                    k_cas_energy<8><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base);
+            }
         }
-        k_cas_e1sum<<<(n_v + 127) / 128, 128, 0, stream>>>((const double2*)c.dPart, n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx,
-                                                           (const double2*)c.dG, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_orb, n_vtot);
+        if (!unres) {
+            k_cas_e1sum<<<(n_v + 127) / 128, 128, 0, stream>>>((const double2*)c.dPart, c.n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx,
+                                                               (const double2*)c.dG, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_orb, n_vtot);
+        } else {
+            // Coulomb term by the Cholesky route (R6, R9): X0 = X0_alpha + X0_beta of the reference from the ordinary kernel on
+            // the reference panels, the Z intermediates of both spins by one DMMA GEMM each, then per (walker, determinant)
+            // E_J^d = 1/2 sum_g (X0^g + SMW corrections)^2  (k_cas_xj)
+            const long long zcols = (long long)f->Xp * f->O_tot;
+            for (int s = 0; s < 2; ++s) {
+                const double* th0 = s ? c.dTh0B : c.dTh0;
+                cudaMemcpy2DAsync(f->dThT + (size_t)f->o_base[s] * f->ldw * f->N_pad, (size_t)f->ldw * f->N_pad * 8, th0, (size_t)ldw0 * f->N_pad * 8,
+                                  (size_t)2 * n_w * f->N_pad * 8, f->n_occ[s], cudaMemcpyDeviceToDevice, stream);
+            }
+            launch_coulomb_x(f, n_w, stream);
+            for (int s = 0; s < 2; ++s) {
+                const int n_act = s ? c.n_actB : c.n_act, na_pad = (s ? c.NPB : c.NP) - 2;
+                const int* hact = s ? c.hActB : c.hAct;
+                const double* th0 = s ? c.dTh0B : c.dTh0;
+                for (int a = 0; a < n_act; ++a)
+                    cudaMemcpyAsync(c.dThAct[s] + (size_t)a * ldw0 * f->N_pad, th0 + (size_t)hact[a] * ldw0 * f->N_pad, (size_t)ldw0 * f->N_pad * 8,
+                                    cudaMemcpyDeviceToDevice, stream);
+                // Z_s[(a, 2w+c)][g * O_tot + o] = Lbar^g_o . Theta0_{s, A_a}
+                launch_gemm_kmajor(c.tmThAct[s], c.tmLbarRows, c.dZ[s], (long long)na_pad * ldw0, zcols, f->N_pad, zcols, f->num_sms, stream);
+            }
+            XjSpin xa = {c.dZ[0], (const double2*)c.dG, c.dHoles, c.dHoleIdx, f->n_occ[0], f->o_base[0], c.n_act};
+            XjSpin xb = {c.dZ[1], (const double2*)c.dGB, c.dHolesB, c.dHoleIdxB, f->n_occ[1], f->o_base[1], c.n_actB};
+            const size_t smx = ((size_t)std::max(c.n_act, 1) * f->n_occ[0] + (size_t)std::max(c.n_actB, 1) * f->n_occ[1]) * 8 * 16;
+            if (smx > 200 * 1024) { set_error("lo_local_energy_cas: active set x orbitals too large for the Coulomb intermediates in shared memory"); return LO_EINVAL; }
+            dim3 gx((c.n_det + 15) / 16, n_w);
+            k_cas_xj<<<gx, 128, smx, stream>>>(xa, xb, f->dXpart, f->ldw, f->n_chol, f->O_tot, zcols, ldw0, c.n_det, c.max_exc, (double2*)c.dEJu);
+            EsSpin ea = {(const double2*)c.dPart, c.n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx, (const double2*)c.dG, f->n_occ[0]};
+            EsSpin eb = {(const double2*)c.dPartB, c.n_chunksB, (const double2*)c.dHB, c.dKindB, c.dHoleIdxB, (const double2*)c.dGB, f->n_occ[1]};
+            k_cas_esum_u<<<(n_v + 127) / 128, 128, 0, stream>>>(ea, eb, (const double2*)c.dEJu, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_vtot);
+        }
     }
     k_cas_combine<<<(n_w + 127) / 128, 128, 0, stream>>>((const double2*)c.dEv, (const double2*)c.dWd, stv, c.dSt0,
-                                                         c.has_beta ? (const double2*)c.dWdB : nullptr, c.has_beta ? f->dStatus + f->Wcap : nullptr,
-                                                         c.has_beta ? c.dSt0B : nullptr, n_w, c.n_det,
+                                                         unres ? (const double2*)c.dWdB : nullptr, unres ? stvB : nullptr,
+                                                         unres ? c.dSt0B : nullptr, n_w, c.n_det,
                                                          (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K, (double2*)ovlp, walker_status);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_error(std::string("lo_local_energy_cas: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }

@@ -108,6 +108,21 @@ struct CasPlan {
     double* dPart = nullptr;                    // [n_chunks][max_real*n_det][2] complex partial (E_K, E_J) sums
     int n_chunks = 0;
     CUtensorMap tmTh0;                          // Theta0^T panels [n_orb*2*W0cap][N_pad], box 16 x 16
+    // ---- rearranged SMW energy with an UNRESTRICTED trial (n_spin == 2): the alpha data are the fields above, the beta
+    // data the *B fields; exchange per spin from that spin's tiles, Coulomb by the Cholesky route from SMW-updated X^g
+    int n_actB = 0, NPB = 0, n_chunksB = 0;
+    int hActB[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int* dHoleIdxB = nullptr;
+    signed char* dKindB = nullptr;
+    double *dSB = nullptr, *dHB = nullptr, *dPartB = nullptr;
+    int* dStVB = nullptr;
+    CUtensorMap tmTh0B;
+    long long tile0[2] = {0, 0}, ntile[2] = {0, 0};   // tile range of each spin inside the factor set's tile list
+    double* dThAct[2] = {nullptr, nullptr};     // gathered active panels [n_act][2*W0cap][N_pad] per spin (A operand of the Z GEMM)
+    double* dZ[2] = {nullptr, nullptr};         // Z[(a, 2w+c)][g*O_tot + o] = Lbar^g_o . Theta0_{A_a}: [n_act*2*W0cap][Xp*O_tot]
+    CUtensorMap tmThAct[2];                     // [n_act*2*W0cap][N_pad], box 128 x 16
+    CUtensorMap tmLbarRows;                     // Lbar as [(Xp*O_tot)][N_pad], box 128 x 16
+    double* dEJu = nullptr;                     // [max_real*n_det] complex: E_J of every (walker, determinant)
 };
 
 // Pair-block SVD (lo_svd.cu)
@@ -201,6 +216,12 @@ void launch_s1(lo_factors* f, int n_w, const double* psi, int ldpsi, int O, cons
                int o_base, int ldw_t, cudaStream_t stream);
 lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream);
 lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStream_t stream);
+// S3 alone on the Theta^T panels: X^g_w into f->dXpart (split-K partials summed into partial 0), E_J / E1 partials as a by-product.
+void launch_coulomb_x(lo_factors* f, int n_w, cudaStream_t stream);
+// out[r][c] = sum_p A[r][p] B[c][p] for K-major fp64 operands given as tensor maps with 128 x 16 boxes (rows, cols multiples
+// of 128; ld_out >= cols): the Coulomb GEMM kernel on another pair of operands (Z intermediates of the unrestricted SMW energy).
+void launch_gemm_kmajor(const CUtensorMap& tmA, const CUtensorMap& tmB, double* out, long long rows, long long cols, int N_pad, long long ld_out,
+                        int num_sms, cudaStream_t stream);
 lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1, void* E_J, void* E_K, void* ovlp,
                                   int* walker_status, cudaStream_t stream);
 // 2D fp64 tensor map over a row-major [rows][inner] array, box [box_rows][16], 128-byte swizzle, zero OOB fill.

@@ -1170,11 +1170,10 @@ lo_status launch_local_energy(lo_factors* f, int n_w, const void* phi_a, const v
     return launch_s3_s5(f, n_w, E_L, E1, E_J, E_K, walker_status, Eout4, stream);
 }
 
-// S2-S5 on the Theta^T panels of n_w (possibly virtual, see lo_local_energy_cas) walkers.
-lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream) {
+// S2 + S3 on the Theta^T panels of n_w walkers: X^g_w (and the hbar row) into f->dXpart, then k_ej.
+void launch_coulomb_x(lo_factors* f, int n_w, cudaStream_t stream) {
     const int N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
     const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
-    // ---- S2 + S3
     const int RB = f->Xp / CO_BM;
     const int ksteps = f->O_tot * (N_pad / KTILE);
     const int nsplit = pick_split((long long)RB * NB, ksteps, f->num_sms);
@@ -1195,6 +1194,25 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         dim3 g2(NB * 2, RB);
         k_ej<<<g2, 256, 0, stream>>>(f->dXpart, EJpart, E1raw, f->Xp, ldw, nsplit, f->n_chol, Wcap);
     }
+}
+
+void launch_gemm_kmajor(const CUtensorMap& tmA, const CUtensorMap& tmB, double* out, long long rows, long long cols, int N_pad, long long ld_out,
+                        int num_sms, cudaStream_t stream) {
+    const int RB = (int)(rows / CO_BM), NB = (int)(cols / 128);
+    const long long items = (long long)RB * NB;
+    const int grid = (int)std::min<long long>(std::max<long long>(items, 1), num_sms);
+    k_coulomb<false, 4><<<grid, 384, CO_SMEM, stream>>>(tmA, tmB, tmB, out, (int)rows, 1, N_pad, (int)ld_out, RB, NB, 1, (int)cols);
+}
+
+// S2-S5 on the Theta^T panels of n_w (possibly virtual, see lo_local_energy_cas) walkers.
+lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, void* E_K, int* walker_status, void* Eout4, cudaStream_t stream) {
+    const int N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
+    const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
+    // ---- S2 + S3
+    launch_coulomb_x(f, n_w, stream);
+    const int RB = f->Xp / CO_BM;
+    double2* EJpart = (double2*)f->dEJpart;
+    double2* E1raw = EJpart + (size_t)RB * Wcap;
     // ---- S4
     int ex_grid = 0;
     {

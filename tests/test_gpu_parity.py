@@ -759,6 +759,41 @@ def test_cas_survey_sizes_200_determinants_rank_6(c1, smw):
         assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
 
 
+def test_cas_unrestricted_smw_200_determinants_rank_6():
+    """The paper's own use of the method -- an open-shell system with a 200-determinant trial, excitation
+    rank up to 6 -- through LO_CAS_SMW_ENERGY on an unrestricted factor set: different alpha / beta strings,
+    6 active occupied x 6 virtual orbitals per spin, 3 walkers; every output against the oracle's definition (each
+    determinant's own LU per spin, w_d = c_d det_a det_b) on the library's factor sets, 1e-10."""
+    torch = torch_cuda()
+    xyz, fns = gen.site_geometry(1)
+    P = gen.make_problem_from_geometry(xyz, fns, (11, 9), 300, seed=41)
+    n_det, n_w = 200, 3
+    Ta = gen.make_cas_trial(P, n_virt=6, n_act_occ=6, n_det=n_det, max_exc=6, spin=0)
+    Tb = gen.make_cas_trial(P, n_virt=6, n_act_occ=6, n_det=n_det, max_exc=6, spin=1)
+    assert ((Ta.holes >= 0).sum(axis=1) != (Tb.holes >= 0).sum(axis=1)).any()
+    F = lo.Factors.setup(P.h, P.L, [Ta.C, Tb.C], 1e-4, device=0, max_walkers=64, gpu_svd=True)
+    F.set_cas_trial(Ta.n_ref, Ta.holes, Ta.parts, Ta.coef, n_w, smw_energy=True)
+    F.set_cas_trial_beta(Tb.n_ref, Tb.holes, Tb.parts)
+    phis = gen.make_walkers(P, n_w)
+    E, st = F.local_energy_cas(torch.from_numpy(phis[0]).cuda(), torch.from_numpy(phis[1]).cuda())
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    assert (st == 0).all()
+    hr = [oracle.half_rotate(P.L, P.h, t.C) for t in (Ta, Tb)]
+    fss = []
+    for s, t in enumerate((Ta, Tb)):
+        n_orb = t.C.shape[1]
+        U, sg, W = F.factor_all(s)
+        pi, pj = oracle.all_pairs(n_orb)
+        fss.append(oracle.make_factor_set(P.N, n_orb, pi, pj, F.ranks(s), U, sg, W))
+    cols = [[t.columns(d) for d in range(n_det)] for t in (Ta, Tb)]
+    for w in range(n_w):
+        Eo = np.array(oracle.local_energy_cas_u([Ta.C, Tb.C], cols, Ta.coef, [a for a, _ in hr], [b for _, b in hr], fss,
+                                                [phis[0][w], phis[1][w]]))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+
+
 def test_cas_smw_edge_cases(c0):
     """One determinant (no excitation) through the SMW-energy mode = the single-determinant energy with the
     compressed Coulomb term; more than 6 distinct hole columns are refused in that mode (and accepted in direct mode)."""
@@ -815,8 +850,22 @@ def test_cas_unrestricted_matches_oracle():
                                                 [phis[0][w], phis[1][w]]))
         assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
         assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+    # the rearranged SMW energy (Eq. 21-23) for the same unrestricted trial: exchange per spin from the S intermediates, Coulomb
+    # by the Cholesky route from SMW-updated X^g (no opposite-spin pair blocks); same oracle, same tolerance
+    F.set_cas_trial(Ta.n_ref, Ta.holes, Ta.parts, Ta.coef, n_w, smw_energy=True)
     with pytest.raises(lo.LoError):
-        F.set_cas_trial(Ta.n_ref, Ta.holes, Ta.parts, Ta.coef, n_w, smw_energy=True)      # SMW-energy mode is closed-shell only
+        F.local_energy_cas(torch.from_numpy(phis[0]).cuda(), torch.from_numpy(phis[1]).cuda())      # beta strings missing
+    F.set_cas_trial_beta(Tb.n_ref, Tb.holes, Tb.parts)
+    Es, sts = F.local_energy_cas(torch.from_numpy(phis[0]).cuda(), torch.from_numpy(phis[1]).cuda())
+    torch.cuda.synchronize()
+    Es, sts = Es.cpu().numpy().T, sts.cpu().numpy()
+    assert (sts == 0).all()
+    assert (np.abs(Es - E).max(axis=1) <= 1e-9 * np.abs(E[:, 0])).all()
+    for w in range(n_w):
+        Eo = np.array(oracle.local_energy_cas_u([Ta.C, Tb.C], cols, Ta.coef, [a for a, _ in hr], [b for _, b in hr], fss,
+                                                [phis[0][w], phis[1][w]]))
+        assert np.abs(Es[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, Es[w], Eo)
+        assert abs(Es[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
 
 
 def test_large_occupation_s1_path():
