@@ -594,22 +594,27 @@ def run_cas_step(args):
     n_det, n_w, smw = args.cas_step, args.walkers or 400, args.cas_mode == "smw"
     P = gen.make_problem(args.config, reading=args.reading)
     T = args.threshold if args.threshold is not None else gen.CONFIGS[args.config].thresholds[0]
-    Tr = gen.make_cas_trial(P, n_virt=6, n_act_occ=args.cas_holes, n_det=n_det, max_exc=args.cas_exc)
-    F = lo.Factors.setup(P.h, P.L, [Tr.C], T, device=0, max_walkers=n_w if smw else n_w * n_det, gpu_svd=True)
+    Trs = [gen.make_cas_trial(P, n_virt=6, n_act_occ=args.cas_holes, n_det=n_det, max_exc=args.cas_exc, spin=s) for s in range(P.n_spin)]
+    Tr = Trs[0]
+    F = lo.Factors.setup(P.h, P.L, [t.C for t in Trs], T, device=0, max_walkers=n_w if smw else n_w * n_det, gpu_svd=True)
     F.set_cas_trial(Tr.n_ref, Tr.holes, Tr.parts, Tr.coef, n_w, smw_energy=smw)
-    phi = torch.from_numpy(gen.make_walkers(P, n_w)[0]).cuda()
+    if P.n_spin == 2:                 # unrestricted trial: different alpha / beta strings
+        F.set_cas_trial_beta(Trs[1].n_ref, Trs[1].holes, Trs[1].parts)
+    phis = [torch.from_numpy(p).cuda() for p in gen.make_walkers(P, n_w)]
+    phi = phis[0] if P.n_spin == 1 else phis
+    call = (lambda: F.local_energy_cas(phi)) if P.n_spin == 1 else (lambda: F.local_energy_cas(phis[0], phis[1]))
     for _ in range(max(args.warmup, 1)):
-        E, st = F.local_energy_cas(phi)
+        E, st = call()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
-        E, st = F.local_energy_cas(phi)
+        E, st = call()
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / args.steps
     info = F.info()
-    print(json.dumps({"cas_step": workload_name(args.config, args.reading, T, n_w), "mode": args.cas_mode, "n_det": n_det,
+    print(json.dumps({"cas_step": workload_name(args.config, args.reading, T, n_w), "mode": args.cas_mode, "n_det": n_det, "n_spin": P.n_spin,
                       "max_exc": args.cas_exc, "active_occupied": args.cas_holes, "tiles": info.n_tiles, "sum_rank": sum(info.sum_rank),
                       "ms_per_step": round(ms, 4), "energies_per_s": round(n_w / (ms * 1e-3), 2),
                       "determinant_energies_per_s": round(n_w * n_det / (ms * 1e-3), 2), "status_ok": bool((st == 0).all()),

@@ -195,10 +195,16 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
 #define LO_CAS_SMW_ENERGY 1
 lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts,
                            const double* coef, int max_real_walkers, int mode);
-/* Unrestricted trial (factor set with n_spin = 2, LO_CAS_DIRECT only): determinant d = |alpha string d> |beta string d>.
+/* Unrestricted trial (factor set with n_spin = 2, either mode): determinant d = |alpha string d> |beta string d>.
  * lo_set_cas_trial gives the alpha strings (reference = the first n_ref columns of psi_a), lo_set_cas_trial_beta the
- * beta strings of the same n_det / max_exc (reference = the first n_ref_b columns of psi_b); w_d = c_d det_a det_b, and
- * every (walker, determinant) is one virtual walker of the unrestricted path (Eq. 10 with explicit spin sums). */
+ * beta strings of the same n_det / max_exc (reference = the first n_ref_b columns of psi_b); w_d = c_d det_a det_b.
+ * LO_CAS_DIRECT: every (walker, determinant) is one virtual walker of the unrestricted path (Eq. 10 with explicit spin
+ * sums).  LO_CAS_SMW_ENERGY (the paper's own use: open-shell systems with 200-determinant trials): the
+ * exchange of each spin from that spin's S intermediates as above; the Coulomb term by the Cholesky route (an
+ * unrestricted factor set holds no opposite-spin pair blocks): X^{g,d}_s = X0^g_s + sum_k sum_x (G_d[k][x] - [x = hole k])
+ * Z_s[hole k][g][x] with Z_s[a][g][x] = Lbar^g_x . Theta0_{s,a} formed once per walker by one GEMM per spin, and
+ * E_J^d = 1/2 sum_g (X^{g,d}_alpha + X^{g,d}_beta)^2; at most 6 distinct hole columns per spin; the Z workspace takes
+ * 8 (n_active padded to 2/4/6) x 2 max_real_walkers(rounded up to 64) x (n_chol padded) x (n_occ[0]+n_occ[1]) bytes per spin. */
 lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, const int* parts_b);
 /* phi_b: device complex128 [n_w][N][n_ref_b] for an unrestricted trial, NULL otherwise. */
 lo_status lo_local_energy_cas(const lo_factors* f, int n_w, const void* phi, const void* phi_b, void* E_L, void* E1,

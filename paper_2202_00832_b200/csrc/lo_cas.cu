@@ -502,9 +502,9 @@ __global__ void k_cas_combine(const double2* __restrict__ Ev, const double2* __r
 //   X^{g,d}_s = sum_x Lbar^g_x . Theta^d_x = X0^g_s + sum_k sum_x G'_s[k][x] Z_s[A-index of hole k][g][x],
 //   G'[k][x] = G_d[k][x] - [x == hole k],   Z_s[a][g][x] = Lbar^g_x . Theta0_{s, A_a}   (one DMMA GEMM per spin and call),
 // and E_J^d = 1/2 sum_g (X^{g,d}_alpha + X^{g,d}_beta)^2  (R6; no opposite-spin pair blocks needed).  X0 = X0_alpha + X0_beta
-// comes from the ordinary Coulomb kernel on the reference panels.  grid (ceil(n_det / 16), n_w), block 128 = 16
-// determinants x 8 Cholesky vectors; the Z rows of 8 Cholesky vectors sit in shared memory while the chunk's
-// determinants use them; sums over g in a fixed order.
+// comes from the ordinary Coulomb kernel on the reference panels.  grid (determinant chunks, n_w), block 128: a thread
+// holds 2, 4 or 8 Cholesky vectors of one determinant; the Z rows of 8 Cholesky vectors sit in shared memory while the
+// block's determinants use them; sums over g in a fixed order.
 struct XjSpin {
     const double* Z;          // [(a * ldw0 + 2w + c)][zcols]
     const double2* G;         // [n_v][max_exc][n_orb]
@@ -512,22 +512,25 @@ struct XjSpin {
     const int* holeIdx;       // [n_det][max_exc]
     int n_orb, o_base, n_act;
 };
+constexpr int XJ_GT = 8;      // Cholesky vectors per shared-memory tile (107 KB at 6 x 70 orbitals per spin: 2 blocks per SM)
+template <int GJ>             // Cholesky vectors per thread (8, 4 or 2 of the tile's 8): a block holds 128 * GJ / 8 determinants
 __global__ void __launch_bounds__(128) k_cas_xj(XjSpin sa, XjSpin sb, const double* __restrict__ X0, int ldx0, int n_chol, int O_tot,
                                                 long long zcols, int ldw0, int n_det, int max_exc, double2* __restrict__ EJ) {
-    extern __shared__ __align__(16) double2 Zs[];      // [spin][a][x][8]
-    const int w = blockIdx.y, tid = threadIdx.x, dl = tid >> 3, gl = tid & 7;
-    const int d = blockIdx.x * 16 + dl;
+    extern __shared__ __align__(16) double2 Zs[];      // [spin][a][Cholesky vector of the tile][x]  (x fastest: conflict-free fill)
+    constexpr int TG = XJ_GT / GJ;                     // threads per determinant
+    const int w = blockIdx.y, tid = threadIdx.x, j0 = (tid % TG) * GJ;
+    const int d = blockIdx.x * (128 / TG) + tid / TG;  // GJ Cholesky vectors of one determinant per thread, in registers
     const bool live = d < n_det;
     const size_t v = (size_t)w * n_det + (live ? d : 0);
     const XjSpin sp[2] = {sa, sb};
-    const int offB = sa.n_act * sa.n_orb * 8;
+    const int offB = sa.n_act * sa.n_orb * XJ_GT;
     double sr = 0.0, si = 0.0;
-    for (int g0 = 0; g0 < n_chol; g0 += 8) {
+    for (int g0 = 0; g0 < n_chol; g0 += XJ_GT) {
         __syncthreads();
         for (int s = 0; s < 2; ++s) {
             const XjSpin& S = sp[s];
             double2* dst = Zs + (s ? offB : 0);
-            const int per = S.n_orb * 8, total = S.n_act * per;
+            const int per = S.n_orb * XJ_GT, total = S.n_act * per;
             for (int e = tid; e < total; e += 128) {
                 const int a = e / per, r = e - a * per, gg = r / S.n_orb, x = r - gg * S.n_orb;
                 double2 z = make_double2(0.0, 0.0);
@@ -536,37 +539,53 @@ __global__ void __launch_bounds__(128) k_cas_xj(XjSpin sa, XjSpin sb, const doub
                     z.x = S.Z[((size_t)a * ldw0 + 2 * w) * zcols + col];
                     z.y = S.Z[((size_t)a * ldw0 + 2 * w + 1) * zcols + col];
                 }
-                dst[(a * S.n_orb + x) * 8 + gg] = z;
+                dst[e] = z;
             }
         }
         __syncthreads();
-        if (live && g0 + gl < n_chol) {
-            double xr = X0[(size_t)(g0 + gl) * ldx0 + 2 * w], xi = X0[(size_t)(g0 + gl) * ldx0 + 2 * w + 1];
-            for (int s = 0; s < 2; ++s) {
-                const XjSpin& S = sp[s];
-                const double2* zs = Zs + (s ? offB : 0);
-                const double2* Gv = S.G + v * max_exc * S.n_orb;
-                for (int k = 0; k < max_exc; ++k) {
-                    const int h = S.holes[(size_t)d * max_exc + k];
-                    if (h < 0) break;
-                    const double2* za = zs + (size_t)S.holeIdx[(size_t)d * max_exc + k] * S.n_orb * 8 + gl;
-                    const double2* gk = Gv + (size_t)k * S.n_orb;
-                    for (int x = 0; x < S.n_orb; ++x) {
-                        double2 c = gk[x];
-                        if (x == h) c.x -= 1.0;
-                        const double2 z = za[x * 8];
-                        xr = fma(c.x, z.x, fma(-c.y, z.y, xr));
-                        xi = fma(c.x, z.y, fma(c.y, z.x, xi));
+        double xr[GJ], xi[GJ];
+#pragma unroll
+        for (int j = 0; j < GJ; ++j) {
+            const bool on = g0 + j0 + j < n_chol;
+            xr[j] = on ? X0[(size_t)(g0 + j0 + j) * ldx0 + 2 * w] : 0.0;
+            xi[j] = on ? X0[(size_t)(g0 + j0 + j) * ldx0 + 2 * w + 1] : 0.0;
+        }
+        for (int s = 0; s < 2 && live; ++s) {
+            const XjSpin& S = sp[s];
+            const double2* zs = Zs + (s ? offB : 0);
+            const double2* Gv = S.G + v * max_exc * S.n_orb;
+            for (int k = 0; k < max_exc; ++k) {
+                const int h = S.holes[(size_t)d * max_exc + k];
+                if (h < 0) break;
+                const double2* za = zs + ((size_t)S.holeIdx[(size_t)d * max_exc + k] * XJ_GT + j0) * S.n_orb;
+                const double2* gk = Gv + (size_t)k * S.n_orb;
+                for (int x0 = 0; x0 < S.n_orb; x0 += 8) {            // 8 independent loads in flight (the loop is latency bound otherwise)
+                    double2 c[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) c[u] = x0 + u < S.n_orb ? __ldg(gk + x0 + u) : make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        if (x0 + u == h) c[u].x -= 1.0;
+                        const int xx = min(x0 + u, S.n_orb - 1);
+#pragma unroll
+                        for (int j = 0; j < GJ; ++j) {
+                            const double2 z = za[j * S.n_orb + xx];    // the same address in every thread with this hole: broadcast
+                            xr[j] = fma(c[u].x, z.x, fma(-c[u].y, z.y, xr[j]));
+                            xi[j] = fma(c[u].x, z.y, fma(c[u].y, z.x, xi[j]));
+                        }
                     }
                 }
             }
-            sr += xr * xr - xi * xi;
-            si += 2.0 * xr * xi;
+        }
+#pragma unroll
+        for (int j = 0; j < GJ; ++j) {            // rows beyond n_chol hold zeros
+            sr += xr[j] * xr[j] - xi[j] * xi[j];
+            si += 2.0 * xr[j] * xi[j];
         }
     }
 #pragma unroll
-    for (int o = 1; o < 8; o <<= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
-    if (live && gl == 0) EJ[v] = make_double2(0.5 * sr, 0.5 * si);
+    for (int o = 1; o < TG; o <<= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
+    if (live && tid % TG == 0) EJ[v] = make_double2(0.5 * sr, 0.5 * si);
 }
 
 // Per virtual walker of an unrestricted trial: E_K^d = alpha + beta chunk partials (the factor weights carry the 1/2 per
@@ -615,7 +634,9 @@ lo_status configure_cas_kernels() {
     cudaError_t e = cudaFuncSetAttribute(k_cas_pairs<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<4>::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<6>::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_pairs<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, CpCfg<8>::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_xj, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_xj<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_xj<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cas_xj<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e != cudaSuccess) { set_error(std::string("cudaFuncSetAttribute(k_cas_*): ") + cudaGetErrorString(e)); return LO_ECUDA; }
     return LO_OK;
 }
@@ -719,10 +740,20 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const
             }
             XjSpin xa = {c.dZ[0], (const double2*)c.dG, c.dHoles, c.dHoleIdx, f->n_occ[0], f->o_base[0], c.n_act};
             XjSpin xb = {c.dZ[1], (const double2*)c.dGB, c.dHolesB, c.dHoleIdxB, f->n_occ[1], f->o_base[1], c.n_actB};
-            const size_t smx = ((size_t)std::max(c.n_act, 1) * f->n_occ[0] + (size_t)std::max(c.n_actB, 1) * f->n_occ[1]) * 8 * 16;
+            const size_t smx = ((size_t)std::max(c.n_act, 1) * f->n_occ[0] + (size_t)std::max(c.n_actB, 1) * f->n_occ[1]) * XJ_GT * 16;
             if (smx > 200 * 1024) { set_error("lo_local_energy_cas: active set x orbitals too large for the Coulomb intermediates in shared memory"); return LO_EINVAL; }
-            dim3 gx((c.n_det + 15) / 16, n_w);
-            k_cas_xj<<<gx, 128, smx, stream>>>(xa, xb, f->dXpart, f->ldw, f->n_chol, f->O_tot, zcols, ldw0, c.n_det, c.max_exc, (double2*)c.dEJu);
+            // as many Cholesky vectors per thread (reuse of every G' entry) as still leaves >= 8 blocks per SM
+            const long long want = 4LL * f->num_sms;
+            if ((long long)n_w * ((c.n_det + 127) / 128) >= want) {
+                dim3 gx((c.n_det + 127) / 128, n_w);
+                k_cas_xj<8><<<gx, 128, smx, stream>>>(xa, xb, f->dXpart, f->ldw, f->n_chol, f->O_tot, zcols, ldw0, c.n_det, c.max_exc, (double2*)c.dEJu);
+            } else if ((long long)n_w * ((c.n_det + 63) / 64) >= want) {
+                dim3 gx((c.n_det + 63) / 64, n_w);
+                k_cas_xj<4><<<gx, 128, smx, stream>>>(xa, xb, f->dXpart, f->ldw, f->n_chol, f->O_tot, zcols, ldw0, c.n_det, c.max_exc, (double2*)c.dEJu);
+            } else {
+                dim3 gx((c.n_det + 31) / 32, n_w);
+                k_cas_xj<2><<<gx, 128, smx, stream>>>(xa, xb, f->dXpart, f->ldw, f->n_chol, f->O_tot, zcols, ldw0, c.n_det, c.max_exc, (double2*)c.dEJu);
+            }
             EsSpin ea = {(const double2*)c.dPart, c.n_chunks, (const double2*)c.dH, c.dKind, c.dHoleIdx, (const double2*)c.dG, f->n_occ[0]};
             EsSpin eb = {(const double2*)c.dPartB, c.n_chunksB, (const double2*)c.dHB, c.dKindB, c.dHoleIdxB, (const double2*)c.dGB, f->n_occ[1]};
             k_cas_esum_u<<<(n_v + 127) / 128, 128, 0, stream>>>(ea, eb, (const double2*)c.dEJu, (double2*)c.dEv, n_v, c.n_det, c.max_exc, n_vtot);
