@@ -340,7 +340,7 @@ void free_cas_plan(CasPlan* c) {
     if (!c) return;
     void* cp[] = {c->dHoles, c->dParts, c->dCoef, c->dTh0, c->dA0, c->dT, c->dG, c->dWd, c->dEv, c->dSt0, c->dHoleIdx, c->dKind, c->dS, c->dH, c->dPart,
                   c->dStV, c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B, c->dHoleIdxB, c->dKindB, c->dSB, c->dHB,
-                  c->dPartB, c->dStVB, c->dThAct[0], c->dThAct[1], c->dZ[0], c->dZ[1], c->dEJu};
+                  c->dPartB, c->dStVB, c->dThAct[0], c->dThAct[1], c->dZ[0], c->dZ[1], c->dEJu, c->dPairs[0], c->dPairs[1]};
     for (void* q : cp)
         if (q) cudaFree(q);
     delete c;
@@ -889,15 +889,17 @@ static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* 
     const int n_act = (int)act.size();
     const int na_pad = n_act <= 2 ? 2 : (n_act <= 4 ? 4 : 6);
     const int NP = 2 + na_pad;
-    // tiles of this spin: the tile list holds spin 0's tiles first (enumerate_blocks)
-    long long t0 = 0, nt = 0;
-    for (const ExTile& t : f->hTiles) {
-        const bool mine = f->n_spin == 1 || (spin == 0 ? t.pi < f->o_base[1] : t.pi >= f->o_base[1]);
-        if (mine) ++nt;
-        else if (spin == 1 && nt == 0) ++t0;
+    // pairs of this spin that have rows, each with its range of <= 4-fragment tiles (consecutive in the tile list)
+    std::vector<CasPair> hp;
+    for (size_t t = 0; t < f->hTiles4.size(); ++t) {
+        const ExTile& T = f->hTiles4[t];
+        const bool mine = f->n_spin == 1 || (spin == 0 ? T.pi < f->o_base[1] : T.pi >= f->o_base[1]);
+        if (!mine) continue;
+        if (!hp.empty() && hp.back().pi == T.pi && hp.back().pj == T.pj && hp.back().t0 + hp.back().nt == (int)t) ++hp.back().nt;
+        else hp.push_back({(int)t, 1, T.pi, T.pj});
     }
-    c->tile0[spin] = spin == 0 ? 0 : t0;
-    c->ntile[spin] = nt;
+    const long long nt = (long long)hp.size();
+    c->npair[spin] = nt;
     std::vector<int> hidx(ne + 8, -1);
     for (size_t k = 0; k < ne; ++k)
         if (holes[k] >= 0) hidx[k] = (int)(std::find(act.begin(), act.end(), holes[k]) - act.begin());
@@ -934,7 +936,9 @@ static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* 
     CK(al((void**)&dPart, (size_t)std::max(n_chunks, 1) * nv * 2 * 16));
     CK(cudaMemcpy(dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(dKind, kind.data(), kind.size(), cudaMemcpyHostToDevice));
-    lo_status st = make_tmap(spin == 0 ? &c->tmTh0 : &c->tmTh0B, dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 16);
+    CK(al((void**)&c->dPairs[spin], std::max<size_t>(hp.size(), 1) * sizeof(CasPair)));
+    if (!hp.empty()) CK(cudaMemcpy(c->dPairs[spin], hp.data(), hp.size() * sizeof(CasPair), cudaMemcpyHostToDevice));
+    lo_status st = make_tmap(spin == 0 ? &c->tmTh0 : &c->tmTh0B, dTh0, f->N_pad, (unsigned long long)n_orb * 2 * c->W0cap, 32);
     if (st != LO_OK) return st;
     if (f->n_spin == 2) {
         // Cholesky-route Coulomb term of the unrestricted SMW energy: gathered active panels and the Z intermediates
@@ -1042,11 +1046,11 @@ lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, 
         return LO_EINVAL;
     }
     void* old[] = {c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B, c->dHoleIdxB, c->dKindB, c->dSB, c->dHB, c->dPartB,
-                   c->dStVB, c->dThAct[1], c->dZ[1]};
+                   c->dStVB, c->dThAct[1], c->dZ[1], c->dPairs[1]};
     for (void* q : old)
         if (q) cudaFree(q);
     c->dHolesB = c->dPartsB = nullptr; c->dTh0B = c->dA0B = c->dTB = c->dGB = c->dWdB = nullptr; c->dSt0B = nullptr;
-    c->dHoleIdxB = nullptr; c->dKindB = nullptr; c->dSB = c->dHB = c->dPartB = nullptr; c->dStVB = nullptr; c->dThAct[1] = c->dZ[1] = nullptr;
+    c->dHoleIdxB = nullptr; c->dKindB = nullptr; c->dSB = c->dHB = c->dPartB = nullptr; c->dStVB = nullptr; c->dThAct[1] = c->dZ[1] = nullptr; c->dPairs[1] = nullptr;
     c->has_beta = false;
     c->n_ref_b = n_ref_b; c->n_virt_b = n_orb_b - n_ref_b;
     const size_t nv = (size_t)c->max_real * c->n_det, ne = (size_t)c->n_det * c->max_exc;

@@ -39,22 +39,61 @@ __global__ void __launch_bounds__(256) k_cas_T(const double* __restrict__ C, int
 // panel set P = [x, y, A_1..A_na] of Theta0 ("Q_L^int = U Phi A_act^-1") serve ALL determinants.  They are
 // contracted over the singular index K at once,
 //     S_t[c][c'] = sum_{K in tile t} wgt_K (U_K . Theta0_c)(W_K . Theta0_c'),     c, c' in P,
-// and a determinant's pair energies are small bilinear forms in S (k_cas_energy).  Work item = (row tile, block of 8
-// walkers); consumer warp m owns row fragment m and all NP panels x 16 real columns; same TMA/mbarrier pipeline.
+// and a determinant's pair energies are small bilinear forms in S (k_cas_energy).  Work item = (row tile, block of 16
+// walkers); work units (row fragment, column tile of 4 walkers) dealt evenly to the consumer warps; same TMA/mbarrier pipeline.
 constexpr int CP_STAGES = 4;
 template <int NP>
 struct CpCfg {
-    static constexpr int STAGE_BYTES = 2 * EX_BM * 128 + NP * 16 * 128;
-    static constexpr int SL = NP * NP + 1;      // slice stride (double2) of one (row group, walker): odd, so the 8 lanes of a
+    static constexpr int STAGE_BYTES = 2 * EX_BM * 128 + NP * 32 * 128;      // U, W (<= 64 rows) + NP panels x 16 walkers
+    static constexpr int SL = NP * NP + 1;      // slice stride (double2) of one (warp, walker): odd, so the 8 lanes of a
                                                 // 128-bit shared access land on distinct 16-byte bank groups
-    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * 8 * SL * 16;
+    static constexpr int SMEM = CP_STAGES * STAGE_BYTES + 1024 + 128 + EX_RING * 16 + 8 * 4 * SL * 16;
 };
 
+// K loop of one (<= 4-fragment) tile for a warp that owns NFW <= 2 row fragments (fg, fg + 2) and one column tile (4
+// walkers): both projections of every fragment onto all NP panels; no padding MMAs (instantiated per NFW).
+template <int NP, int NFW>
+__device__ __forceinline__ void cp_kloop(int KT, uint32_t sbase, uint32_t full, uint32_t empty, int& cslot, uint32_t& cphase, int lane,
+                                         const uint32_t (&xo)[4], uint32_t u_row, uint32_t p_row, double (&accU)[2][NP][2],
+                                         double (&accW)[2][NP][2]) {
+    constexpr int STAGE = CpCfg<NP>::STAGE_BYTES;
+    for (int kt = 0; kt < KT; ++kt) {
+        if (kt) mbar_wait(full + 8 * cslot, cphase);
+        if constexpr (NFW == 0) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + 8 * cslot);
+        } else {
+            const uint32_t st = sbase + cslot * STAGE;
+#pragma unroll
+            for (int ks = 0; ks < KTILE / 4; ++ks) {
+                double a[NFW], w[NFW], bb[NP];
+#pragma unroll
+                for (int j = 0; j < NFW; ++j) {
+                    a[j] = lds_f64(st + u_row + j * 2048 + xo[ks]);
+                    w[j] = lds_f64(st + u_row + EX_BM * 128 + j * 2048 + xo[ks]);
+                }
+#pragma unroll
+                for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 4096 + xo[ks]);
+                if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
+#pragma unroll
+                for (int j = 0; j < NFW; ++j)
+#pragma unroll
+                    for (int c = 0; c < NP; ++c) {
+                        mma884(accU[j][c][0], accU[j][c][1], a[j], bb[c]);
+                        mma884(accW[j][c][0], accW[j][c][1], w[j], bb[c]);
+                    }
+            }
+        }
+        if (++cslot == CP_STAGES) { cslot = 0; cphase ^= 1; }
+    }
+}
+
 template <int NP>
-__global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmW,
+__global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ TmSet tmUs, const __grid_constant__ TmSet tmWs,
                                                       const __grid_constant__ CUtensorMap tmT0, const double* __restrict__ wgt,
-                                                      const ExTile* __restrict__ tiles, long long n_items, int WB, int N_pad, int ldw0,
-                                                      const int* __restrict__ act /* [NP-2] */, double2* __restrict__ S, int n_w,
+                                                      const ExTile* __restrict__ tiles4, const CasPair* __restrict__ pairs, long long n_items,
+                                                      int WB, int N_pad, int ldw0, const int* __restrict__ act /* [NP-2] */,
+                                                      double2* __restrict__ S, int n_w,
                                                       int pan_base /* first orbital of this spin in the factor set's numbering */) {
     constexpr int STAGE = CpCfg<NP>::STAGE_BYTES;
     extern __shared__ unsigned char smem_raw[];
@@ -62,12 +101,11 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
     const uint32_t full = sbase + CP_STAGES * STAGE, empty = full + 8 * CP_STAGES;
     ExTile* ring = reinterpret_cast<ExTile*>(sgen + CP_STAGES * STAGE + 128);
-    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 fragments (warps)][8 walkers][SL]
+    double2* Sacc = reinterpret_cast<double2*>(sgen + CP_STAGES * STAGE + 128 + EX_RING * 16);     // [8 warps][4 walkers][SL]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int KT = N_pad / KTILE;
     if (tid == 0) {
-        prefetch_tmap(&tmU);
-        prefetch_tmap(&tmW);
+        for (int k = 0; k < 8; ++k) { prefetch_tmap(&tmUs.m[k]); prefetch_tmap(&tmWs.m[k]); }
         prefetch_tmap(&tmT0);
         for (int i = 0; i < CP_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 8); }
         fence_barrier_init();
@@ -81,37 +119,40 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
             for (int c = 2; c < NP; ++c) pan[c] = act[c - 2];
             int slot = 0, n = 0;
             uint32_t phase = 0;
-            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-                const ExTile tile = tiles[q / WB];
+            for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
+                const CasPair pr = pairs[q / WB];
                 const int wb = (int)(q % WB);
-                pan[0] = tile.pi - pan_base;
-                pan[1] = tile.pj - pan_base;
-                // whole 64-row boxes of U and W whatever the tile's length (rows past the tile are never read): one TMA each
-                const uint32_t tx = (uint32_t)(2 * EX_BM + NP * 16) * 128;
-                for (int kt = 0; kt < KT; ++kt) {
-                    mbar_wait(empty + 8 * slot, phase ^ 1);
-                    if (kt == 0) ring[n % EX_RING] = tile;
-                    const uint32_t st = sbase + slot * STAGE, bar = full + 8 * slot;
-                    const int k0 = kt * KTILE;
-                    mbar_expect_tx(bar, tx);
-                    tma_load_2d(st, &tmU, k0, tile.row0, bar);
-                    tma_load_2d(st + EX_BM * 128, &tmW, k0, tile.row0, bar);
+                pan[0] = pr.pi - pan_base;
+                pan[1] = pr.pj - pan_base;
+                for (int ts = 0; ts < pr.nt; ++ts, ++n) {         // the pair's tiles, one after the other
+                    const ExTile tile = tiles4[pr.t0 + ts];
+                    const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + NP * 32) * 128;
+                    for (int kt = 0; kt < KT; ++kt) {
+                        mbar_wait(empty + 8 * slot, phase ^ 1);
+                        if (kt == 0) ring[n % EX_RING] = tile;
+                        const uint32_t st = sbase + slot * STAGE, bar = full + 8 * slot;
+                        const int k0 = kt * KTILE;
+                        mbar_expect_tx(bar, tx);
+                        tma_load_2d(st, &tmUs.m[tile.nfrag - 1], k0, tile.row0, bar);
+                        tma_load_2d(st + EX_BM * 128, &tmWs.m[tile.nfrag - 1], k0, tile.row0, bar);
 #pragma unroll
-                    for (int c = 0; c < NP; ++c)        // 16 real rows (8 walkers) of panel c
-                        tma_load_2d(st + 2 * EX_BM * 128 + c * 2048, &tmT0, k0, pan[c] * ldw0 + wb * 16, bar);
-                    if (++slot == CP_STAGES) { slot = 0; phase ^= 1; }
+                        for (int c = 0; c < NP; ++c)        // 32 real rows (16 walkers) of panel c
+                            tma_load_2d(st + 2 * EX_BM * 128 + c * 4096, &tmT0, k0, pan[c] * ldw0 + wb * 32, bar);
+                        if (++slot == CP_STAGES) { slot = 0; phase ^= 1; }
+                    }
                 }
             }
         }
         return;
     }
     reg_inc_consumer();
-    // Work units of an item = (row fragment, column half nf) = 2 * nfrag; consumer warp cw owns units cw and cw + 8, i.e.
-    // fragments cw/2 and 4 + cw/2 of the SAME column half nf = cw & 1 (they share the panel fragments).  The two warps
-    // of a scheduler (cw, cw + 4) then hold at most ceil(nfrag / 2) + ... units: 5 fragments load the four schedulers
-    // 3/3/2/2 instead of 2/1/1/1 whole fragments.
+    // Work item = (pair, block of 16 walkers); its tiles (<= 4 fragments each) run one after the other and S is summed over
+    // them in registers, so S exists once per PAIR.  Work units of a tile = (row fragment, column tile of 4 walkers) =
+    // 4 * nfrag <= 16; consumer warp cw owns column tile cw & 3 and the fragments (cw >> 2), (cw >> 2) + 2: the two warps
+    // of a scheduler (cw, cw + 4) hold nfrag units between them whatever nfrag is, so the four tensor pipes carry equal
+    // loads (round 1 dealt (fragment, column half) units of an 8-walker item: 3/3/2/2 over the schedulers at 5 fragments).
     const int cw = warp - 4, g = lane >> 2, t = lane & 3, ctid = tid - 128;
-    const int nf = cw & 1, fr0 = cw >> 1, fr1 = 4 + (cw >> 1);
+    const int nt = cw & 3, fg = cw >> 2;
     double accU[2][NP][2], accW[2][NP][2];
 #pragma unroll
     for (int j = 0; j < 2; ++j)
@@ -120,71 +161,37 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
     uint32_t xo[4];
 #pragma unroll
     for (int s = 0; s < 4; ++s) xo[s] = frag_off(g, t, s);
-    const uint32_t u_row0 = (uint32_t)(fr0 * 8 + g) * 128, u_row1 = (uint32_t)(fr1 * 8 + g) * 128;
-    const uint32_t p_row = (uint32_t)(2 * EX_BM * 128) + (uint32_t)(nf * 8 + g) * 128;
+    const uint32_t u_row = (uint32_t)(fg * 8 + g) * 128;
+    const uint32_t p_row = (uint32_t)(2 * EX_BM * 128) + (uint32_t)(nt * 8 + g) * 128;
     constexpr int SL = CpCfg<NP>::SL;
+    const bool b0 = g & 1, b1 = g & 2, b2 = g & 4;
+    const int c2own = (b0 ? 4 : 0) + (b1 ? 2 : 0) + (b2 ? 1 : 0);
     int cslot = 0, n = 0;
     uint32_t cphase = 0;
-    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
+    for (long long q = blockIdx.x; q < n_items; q += gridDim.x) {
         const int wb = (int)(q % WB);
-        const long long tix = q / WB;
-        mbar_wait(full + 8 * cslot, cphase);
-        const ExTile tile = ring[n % EX_RING];
-        const int nu = (fr0 < tile.nfrag ? 1 : 0) + (fr1 < tile.nfrag ? 1 : 0);     // warp-uniform: 0, 1 or 2 units
-        for (int kt = 0; kt < KT; ++kt) {
-            if (kt) mbar_wait(full + 8 * cslot, cphase);
-            const uint32_t st = sbase + cslot * STAGE;
-            if (nu == 2) {
+        const long long pix = q / WB;
+        const int n_sub = pairs[pix].nt;
+        double2 sc[NP];                      // this lane's S[c][c2own] of walker 4 nt + t, summed over the pair's rows
 #pragma unroll
-                for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    const double a0 = lds_f64(st + u_row0 + xo[ks]), w0 = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
-                    const double a1 = lds_f64(st + u_row1 + xo[ks]), w1 = lds_f64(st + u_row1 + EX_BM * 128 + xo[ks]);
-                    double bb[NP];
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 2048 + xo[ks]);
-                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) {
-                        mma884(accU[0][c][0], accU[0][c][1], a0, bb[c]);
-                        mma884(accW[0][c][0], accW[0][c][1], w0, bb[c]);
-                        mma884(accU[1][c][0], accU[1][c][1], a1, bb[c]);
-                        mma884(accW[1][c][0], accW[1][c][1], w1, bb[c]);
-                    }
-                }
-            } else if (nu == 1) {
-#pragma unroll
-                for (int ks = 0; ks < KTILE / 4; ++ks) {
-                    const double a0 = lds_f64(st + u_row0 + xo[ks]), w0 = lds_f64(st + u_row0 + EX_BM * 128 + xo[ks]);
-                    double bb[NP];
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) bb[c] = lds_f64(st + p_row + c * 2048 + xo[ks]);
-                    if (ks == KTILE / 4 - 1) release_stage(empty + 8 * cslot, lane);
-#pragma unroll
-                    for (int c = 0; c < NP; ++c) {
-                        mma884(accU[0][c][0], accU[0][c][1], a0, bb[c]);
-                        mma884(accW[0][c][0], accW[0][c][1], w0, bb[c]);
-                    }
-                }
-            } else {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty + 8 * cslot);
+        for (int c = 0; c < NP; ++c) sc[c] = make_double2(0.0, 0.0);
+        for (int ts = 0; ts < n_sub; ++ts, ++n) {
+            mbar_wait(full + 8 * cslot, cphase);
+            const ExTile tile = ring[n % EX_RING];
+            const int nfw = tile.nfrag > fg ? (tile.nfrag - fg + 1) >> 1 : 0;     // warp-uniform, <= 2
+            switch (nfw) {
+                case 0: cp_kloop<NP, 0>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, p_row, accU, accW); break;
+                case 1: cp_kloop<NP, 1>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, p_row, accU, accW); break;
+                default: cp_kloop<NP, 2>(KT, sbase, full, empty, cslot, cphase, lane, xo, u_row, p_row, accU, accW); break;
             }
-            if (++cslot == CP_STAGES) { cslot = 0; cphase ^= 1; }
-        }
-        // epilogue: S[c][c'] of the 4 walkers of this warp's column half, per unit.  For every panel c the lane holds the 8
-        // complex products of its own row g (c' = 0..7, zero beyond NP); a transposing butterfly over the 8 row groups
-        // (each round sends half of the values and keeps the other half: 8+4+2 exchanges instead of 3 per value) leaves
-        // the row sum of column c' = 4 b0 + 2 b1 + b2 (bits of g) in lane g.  Every fragment's S goes to its own slice;
-        // the slices are added in fragment order when the block is written out (fixed order).
-        {
-            const bool b0 = g & 1, b1 = g & 2, b2 = g & 4;
-            const int c2own = (b0 ? 4 : 0) + (b1 ? 2 : 0) + (b2 ? 1 : 0);
+            // S[c][c'] of the 4 walkers of this warp's column tile.  For every panel c the lane holds the 8 complex products
+            // of its own row g (c' = 0..7, zero beyond NP); a transposing butterfly over the 8 row groups (each round sends
+            // half of the values and keeps the other half: 8+4+2 exchanges instead of 3 per value) leaves the row sum of
+            // column c' = 4 b0 + 2 b1 + b2 (bits of g) in lane g.
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                if (j >= nu) break;                     // warp-uniform
-                const int fr = j == 0 ? fr0 : fr1;
-                const double wv = __ldg(wgt + tile.row0 + fr * 8 + g);
-                double2* dst = Sacc + ((fr * 8) + nf * 4 + t) * SL;
+                if (j >= nfw) break;                     // warp-uniform
+                const double wv = __ldg(wgt + tile.row0 + (fg + 2 * j) * 8 + g);
 #pragma unroll
                 for (int c = 0; c < NP; ++c) {
                     const double ur = wv * accU[j][c][0], ui = wv * accU[j][c][1];
@@ -209,19 +216,27 @@ __global__ void __launch_bounds__(384, 1) k_cas_pairs(const __grid_constant__ CU
                         const double snd = b2 ? v[i] : v[i + 2], kp = b2 ? v[i + 2] : v[i];
                         v[i] = kp + __shfl_xor_sync(0xffffffffu, snd, 16);
                     }
-                    if (c2own < NP) dst[c * NP + c2own] = make_double2(v[0], v[1]);
+                    sc[c].x += v[0];
+                    sc[c].y += v[1];
                 }
 #pragma unroll
                 for (int c = 0; c < NP; ++c) accU[j][c][0] = accU[j][c][1] = accW[j][c][0] = accW[j][c][1] = 0.0;
             }
         }
+        // the two warps of a column tile write their slices; they are added in a fixed order when the block is written out
+        {
+            double2* dst = Sacc + (cw * 4 + t) * SL;
+            if (c2own < NP) {
+#pragma unroll
+                for (int c = 0; c < NP; ++c) dst[c * NP + c2own] = sc[c];
+            }
+        }
         bar_sync_consumers();
-        for (int i = ctid; i < 8 * NP * NP; i += 256) {
-            const int wl = i / (NP * NP), wg = wb * 8 + wl;
-            const int is = wl * SL + (i - wl * NP * NP);
-            double2 sum = Sacc[is];
-            for (int fr = 1; fr < tile.nfrag; ++fr) { const double2 v = Sacc[fr * 8 * SL + is]; sum.x += v.x; sum.y += v.y; }
-            if (wg < n_w) S[((size_t)tix * n_w + wg) * NP * NP + (i - wl * NP * NP)] = sum;
+        for (int i = ctid; i < 16 * NP * NP; i += 256) {
+            const int wl = i / (NP * NP), e = i - wl * NP * NP, wg = wb * 16 + wl;      // walker wl of the block: column tile wl / 4, lane t = wl % 4
+            const int s0 = ((wl >> 2) * 4 + (wl & 3)) * SL + e, s1 = (((wl >> 2) + 4) * 4 + (wl & 3)) * SL + e;
+            const double2 x0 = Sacc[s0], x1 = Sacc[s1];
+            if (wg < n_w) S[((size_t)pix * n_w + wg) * NP * NP + e] = make_double2(x0.x + x1.x, x0.y + x1.y);
         }
         bar_sync_consumers();
     }
@@ -255,11 +270,11 @@ __global__ void __launch_bounds__(256) k_cas_H(const double* __restrict__ hbar, 
 // Theta^d_x = s_x Theta0_x + sum_k G_d[k][x] Theta0_{h_k}  (s_x = 1 for a reference non-hole, else 0),
 //   exchange  e = sum_{c in y-list} sum_{c' in x-list} coef_y[c] coef_x[c'] S[c][c'],
 //   Coulomb   j = sum_{c in x-list} sum_{c' in y-list} coef_x[c] coef_y[c'] S[c][c'],
-// lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of CE_CH tiles sits in shared memory, threads
+// lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of CE_CH pairs' S sits in shared memory, threads
 // run over determinants; partial (E_K, E_J) sums per chunk are added in chunk order by k_cas_e1sum.
 constexpr int CE_CH = 16;
 template <int MAXE>     // compile-time bound of the excitation rank: the coefficient lists stay in registers
-__global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const ExTile* __restrict__ tiles, long long n_tiles,
+__global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const CasPair* __restrict__ tiles, long long n_tiles,
                                                     const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
                                                     const double2* __restrict__ G, double2* __restrict__ part, int n_w, int n_det, int max_exc,
                                                     int n_orb, int NP, int n_vtot, int pan_base) {
@@ -676,14 +691,14 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const
     } else {
         // rearranged SMW energy (Eq. 23), per spin: S intermediates once per (tile, walker), one-body intermediates, then small
         // per-determinant forms (exchange, and for a closed-shell trial the compressed Coulomb term)
-        const int WB = (n_w + 7) / 8;
+        const int WB = (n_w + 15) / 16;
         const int n_vtot = c.max_real * c.n_det;
         const double* hbar0 = f->ops->dLbar + (size_t)f->n_chol * f->O_tot * f->N_pad;
         for (int s = 0; s < (unres ? 2 : 1); ++s) {
             const int NP = s ? c.NPB : c.NP, n_act = s ? c.n_actB : c.n_act, n_orb_s = f->n_occ[s], n_ref_s = s ? c.n_ref_b : c.n_ref;
             const int pan_base = f->o_base[s];
-            const long long nt = c.ntile[s];
-            const ExTile* tiles = f->dTiles + c.tile0[s];
+            const long long nt = c.npair[s];               // pairs with rows (S exists once per pair)
+            const CasPair* tiles = c.dPairs[s];
             const int* hidx = s ? c.dHoleIdxB : c.dHoleIdx;
             const int* actd = hidx + (size_t)c.n_det * c.max_exc;      // A_set stored behind the hole indices
             double2* S = (double2*)(s ? c.dSB : c.dS);
@@ -692,11 +707,11 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const
             const long long items = nt * WB;
             const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
             if (NP == 4)
-                k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmU, f->tmW, tm0, f->dWgt, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
+                k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
             else if (NP == 6)
-                k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmU, f->tmW, tm0, f->dWgt, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
+                k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
             else
-                k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmU, f->tmW, tm0, f->dWgt, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
+                k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
             k_cas_H<<<n_w, 256, 0, stream>>>(hbar0 + (size_t)pan_base * f->N_pad, th0, actd, n_act, (double2*)(s ? c.dHB : c.dH), f->N, f->N_pad,
                                              n_ref_s, n_orb_s, ldw0);
             const int n_chunks = (int)((nt + CE_CH - 1) / CE_CH);

@@ -75,6 +75,11 @@ struct GatherRec {
     int r, pad_;
 };
 
+// One pair of the SMW-energy path: its <= 4-fragment tiles are tiles4[t0 .. t0 + nt); S is kept per pair, not per tile.
+struct CasPair {
+    int t0, nt, pi, pj;
+};
+
 // Multi-determinant trial (lo_set_cas_trial): determinants as excitation lists of the reference
 // (= the first n_ref orbitals of the factor set's Psi), workspace for max_real real walkers; the n_det determinants of a
 // real walker are laid out as n_det consecutive VIRTUAL walkers of the ordinary S3-S5 path.
@@ -107,7 +112,7 @@ struct CasPlan {
     double* dH = nullptr;                       // one-body intermediates [W0cap][n_orb][1 + 8] complex (self, A_set)
     double* dPart = nullptr;                    // [n_chunks][max_real*n_det][2] complex partial (E_K, E_J) sums
     int n_chunks = 0;
-    CUtensorMap tmTh0;                          // Theta0^T panels [n_orb*2*W0cap][N_pad], box 16 x 16
+    CUtensorMap tmTh0;                          // Theta0^T panels [n_orb*2*W0cap][N_pad], box 32 x 16 (16 walkers)
     // ---- rearranged SMW energy with an UNRESTRICTED trial (n_spin == 2): the alpha data are the fields above, the beta
     // data the *B fields; exchange per spin from that spin's tiles, Coulomb by the Cholesky route from SMW-updated X^g
     int n_actB = 0, NPB = 0, n_chunksB = 0;
@@ -117,7 +122,8 @@ struct CasPlan {
     double *dSB = nullptr, *dHB = nullptr, *dPartB = nullptr;
     int* dStVB = nullptr;
     CUtensorMap tmTh0B;
-    long long tile0[2] = {0, 0}, ntile[2] = {0, 0};   // tile range of each spin inside the factor set's tile list
+    CasPair* dPairs[2] = {nullptr, nullptr};    // pairs with rows, per spin (tile ranges into the factor set's <= 4-fragment tile list)
+    long long npair[2] = {0, 0};
     double* dThAct[2] = {nullptr, nullptr};     // gathered active panels [n_act][2*W0cap][N_pad] per spin (A operand of the Z GEMM)
     double* dZ[2] = {nullptr, nullptr};         // Z[(a, 2w+c)][g*O_tot + o] = Lbar^g_o . Theta0_{A_a}: [n_act*2*W0cap][Xp*O_tot]
     CUtensorMap tmThAct[2];                     // [n_act*2*W0cap][N_pad], box 128 x 16
