@@ -525,12 +525,19 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
             } else {
                 stats_of_batch.assign(n, SvdStat());
                 std::vector<SvdStat>& stats = stats_of_batch;
+                int oom = 0;       // an allocation failure inside the parallel region must not escape it
 #pragma omp parallel
                 {
-                    std::vector<double> G((size_t)N * N), V((size_t)N * N), sg, rU, rW;
+                    std::vector<double> G, V, sg, rU, rW;
                     std::vector<int> order;
+                    try { G.resize((size_t)N * N); V.resize((size_t)N * N); } catch (const std::bad_alloc&) {
+#pragma omp atomic write
+                        oom = 1;
+                    }
 #pragma omp for schedule(dynamic, 1)
                     for (int x = 0; x < n; ++x) {
+                        if (G.size() != (size_t)N * N || V.size() != (size_t)N * N) continue;
+                        try {
                         host_pair_gram_t(N, n_chol, f->O_tot, Lbar, f->o_base[spin] + bi[x], f->o_base[spin] + bj[x], G.data());
                         if (rsvd_k && host_pair_rsvd(N, rsvd_k, G.data(), sg, rU, rW, &stats[x])) {
                             // the sketch captured the block: its factors are the SVD to working accuracy
@@ -556,8 +563,13 @@ lo_status lo_setup(int N, int n_chol, int n_spin, const int n_occ[2], const doub
                             for (int e = 0; e < N; ++e) pU[x][(size_t)K * N + e] = g[e] * inv;
                             std::memcpy(&pW[x][(size_t)K * N], &V[(size_t)order[K] * N], (size_t)N * 8);
                         }
+                        } catch (const std::bad_alloc&) {
+#pragma omp atomic write
+                            oom = 1;
+                        }
                     }
                 }
+                if (oom) { set_error("lo_setup: out of host memory in the pair SVDs"); st = LO_ENOMEM; break; }
             }
             f->setup_svd_seconds += omp_get_wtime() - t_svd;
             if (!on_gpu)
