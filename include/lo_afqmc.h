@@ -190,7 +190,8 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
  *   over the singular index into S^{xy}[c][c'] = sum_K sigma_K (U_K.Theta0_c)(W_K.Theta0_c'), and each determinant's
  *   exchange AND Coulomb pair energies (Eq. 22: both terms from the compressed factors, as LO_COULOMB_COMPRESSED) are
  *   small bilinear forms in S; E1 likewise from hbar.Theta0 intermediates.  Leading cost (2 + n_active)/2 x the
- *   4-projection single-determinant evaluation, independent of n_det; at most 6 distinct hole columns. */
+ *   4-projection single-determinant evaluation, independent of n_det.  Up to 6 distinct hole columns (active occupied
+ *   orbitals) take one pass; 7..12 are cut into groups of 3 and take one pass per pair of groups (6 passes for 9, 10 for 12). */
 #define LO_CAS_DIRECT 0
 #define LO_CAS_SMW_ENERGY 1
 lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, const int* holes, const int* parts,

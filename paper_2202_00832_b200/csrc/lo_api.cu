@@ -340,7 +340,7 @@ void free_cas_plan(CasPlan* c) {
     if (!c) return;
     void* cp[] = {c->dHoles, c->dParts, c->dCoef, c->dTh0, c->dA0, c->dT, c->dG, c->dWd, c->dEv, c->dSt0, c->dHoleIdx, c->dKind, c->dS, c->dH, c->dPart,
                   c->dStV, c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B, c->dHoleIdxB, c->dKindB, c->dSB, c->dHB,
-                  c->dPartB, c->dStVB, c->dThAct[0], c->dThAct[1], c->dZ[0], c->dZ[1], c->dEJu, c->dPairs[0], c->dPairs[1]};
+                  c->dPartB, c->dStVB, c->dThAct[0], c->dThAct[1], c->dZ[0], c->dZ[1], c->dEJu, c->dPairs[0], c->dPairs[1], c->dPassAct[0], c->dPassAct[1]};
     for (void* q : cp)
         if (q) cudaFree(q);
     delete c;
@@ -900,7 +900,17 @@ static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* 
     };
     const int n_act = (int)act.size();
     const int na_pad = n_act <= 2 ? 2 : (n_act <= 4 ? 4 : 6);
-    const int NP = 2 + na_pad;
+    // up to 6 active columns: one pass on the panel list {x, y, A}; more: groups of 3 and one pass per pair of groups
+    const int gs = n_act <= 6 ? 6 : 3, ng = n_act <= 6 ? 1 : (n_act + 2) / 3, npass = ng * (ng + 1) / 2;
+    const int NP = ng == 1 ? 2 + na_pad : 8;
+    std::vector<int> pass_act((size_t)npass * 6, 0);
+    for (int a = 0, p = 0; a < ng; ++a)
+        for (int b = a; b < ng; ++b, ++p)
+            for (int l = 0; l < 6; ++l) {
+                const int idx = ng == 1 ? l : (l < 3 ? a * 3 + l : b * 3 + (l - 3));
+                pass_act[(size_t)p * 6 + l] = idx < n_act ? act[idx] : 0;
+            }
+    const int ce = std::max(1, std::min(16, (40 * 1024) / (npass * NP * NP * 16)));      // k_cas_energy keeps a chunk in <= 40 KB of shared memory
     // pairs of this spin that have rows, each with its range of <= 4-fragment tiles (consecutive in the tile list)
     std::vector<CasPair> hp;
     for (size_t t = 0; t < f->hTiles4.size(); ++t) {
@@ -912,10 +922,10 @@ static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* 
     }
     const long long nt = (long long)hp.size();
     c->npair[spin] = nt;
-    std::vector<int> hidx(ne + 8, -1);
+    std::vector<int> hidx(ne + 16, -1);
     for (size_t k = 0; k < ne; ++k)
         if (holes[k] >= 0) hidx[k] = (int)(std::find(act.begin(), act.end(), holes[k]) - act.begin());
-    for (int a = 0; a < 8; ++a) {
+    for (int a = 0; a < 16; ++a) {
         hidx[ne + a] = a < n_act ? act[a] : 0;          // A_set (padded with column 0) behind the indices
         (spin == 0 ? c->hAct : c->hActB)[a] = hidx[ne + a];
     }
@@ -929,7 +939,8 @@ static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* 
             }
             kind[(size_t)d * n_orb + x] = kd;
         }
-    const int n_chunks = (int)((nt + 15) / 16);
+    const int n_chunks = (int)((nt + ce - 1) / ce);
+    c->gs[spin] = gs; c->ng[spin] = ng; c->npass[spin] = npass; c->ce[spin] = ce;
     int*& dHoleIdx = spin == 0 ? c->dHoleIdx : c->dHoleIdxB;
     signed char*& dKind = spin == 0 ? c->dKind : c->dKindB;
     int*& dStV = spin == 0 ? c->dStV : c->dStVB;
@@ -943,8 +954,10 @@ static lo_status alloc_smw_spin(lo_factors* f, CasPlan* c, int spin, const int* 
     CK(al((void**)&dHoleIdx, hidx.size() * 4));
     CK(al((void**)&dKind, kind.size()));
     CK(al((void**)&dStV, nv * 4));
-    CK(al((void**)&dS, (size_t)std::max<long long>(nt, 1) * c->max_real * NP * NP * 16));
-    CK(al((void**)&dH, (size_t)c->W0cap * n_orb * 9 * 16));
+    CK(al((void**)&dS, (size_t)npass * std::max<long long>(nt, 1) * c->max_real * NP * NP * 16));
+    CK(al((void**)&dH, (size_t)c->W0cap * n_orb * CAS_HS * 16));
+    CK(al((void**)&c->dPassAct[spin], pass_act.size() * 4));
+    CK(cudaMemcpy(c->dPassAct[spin], pass_act.data(), pass_act.size() * 4, cudaMemcpyHostToDevice));
     CK(al((void**)&dPart, (size_t)std::max(n_chunks, 1) * nv * 2 * 16));
     CK(cudaMemcpy(dHoleIdx, hidx.data(), hidx.size() * 4, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(dKind, kind.data(), kind.size(), cudaMemcpyHostToDevice));
@@ -1013,8 +1026,9 @@ lo_status lo_set_cas_trial(lo_factors* f, int n_ref, int n_det, int max_exc, con
     for (size_t k = 0; k < (size_t)n_det * max_exc; ++k)
         if (holes[k] >= 0 && std::find(act.begin(), act.end(), holes[k]) == act.end()) act.push_back(holes[k]);
     std::sort(act.begin(), act.end());
-    if (mode == LO_CAS_SMW_ENERGY && act.size() > 6) {
-        set_error("lo_set_cas_trial: LO_CAS_SMW_ENERGY supports at most 6 distinct hole columns (active occupied orbitals); use LO_CAS_DIRECT");
+    if (mode == LO_CAS_SMW_ENERGY && (int)act.size() > (f->n_spin == 1 ? CAS_MAX_ACT : 6)) {
+        set_error("lo_set_cas_trial: LO_CAS_SMW_ENERGY supports at most 12 distinct hole columns (active occupied orbitals) for a closed-shell "
+                  "trial and 6 per spin for an unrestricted one; use LO_CAS_DIRECT");
         return LO_EINVAL;
     }
     CK(cudaSetDevice(f->device));
@@ -1058,11 +1072,11 @@ lo_status lo_set_cas_trial_beta(lo_factors* f, int n_ref_b, const int* holes_b, 
         return LO_EINVAL;
     }
     void* old[] = {c->dHolesB, c->dPartsB, c->dTh0B, c->dA0B, c->dTB, c->dGB, c->dWdB, c->dSt0B, c->dHoleIdxB, c->dKindB, c->dSB, c->dHB, c->dPartB,
-                   c->dStVB, c->dThAct[1], c->dZ[1], c->dPairs[1]};
+                   c->dStVB, c->dThAct[1], c->dZ[1], c->dPairs[1], c->dPassAct[1]};
     for (void* q : old)
         if (q) cudaFree(q);
     c->dHolesB = c->dPartsB = nullptr; c->dTh0B = c->dA0B = c->dTB = c->dGB = c->dWdB = nullptr; c->dSt0B = nullptr;
-    c->dHoleIdxB = nullptr; c->dKindB = nullptr; c->dSB = c->dHB = c->dPartB = nullptr; c->dStVB = nullptr; c->dThAct[1] = c->dZ[1] = nullptr; c->dPairs[1] = nullptr;
+    c->dHoleIdxB = nullptr; c->dKindB = nullptr; c->dSB = c->dHB = c->dPartB = nullptr; c->dStVB = nullptr; c->dThAct[1] = c->dZ[1] = nullptr; c->dPairs[1] = nullptr; c->dPassAct[1] = nullptr;
     c->has_beta = false;
     c->n_ref_b = n_ref_b; c->n_virt_b = n_orb_b - n_ref_b;
     const size_t nv = (size_t)c->max_real * c->n_det, ne = (size_t)c->n_det * c->max_exc;

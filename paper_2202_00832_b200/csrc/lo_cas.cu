@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(256) k_cas_H(const double* __restrict__ hbar, 
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, o); si += __shfl_xor_sync(0xffffffffu, si, o); }
         }
-        if (lane == 0) H[((size_t)w * n_orb + x) * 9 + sl] = make_double2(sr, si);
+        if (lane == 0) H[((size_t)w * n_orb + x) * CAS_HS + sl] = make_double2(sr, si);
     }
 }
 
@@ -270,22 +270,25 @@ __global__ void __launch_bounds__(256) k_cas_H(const double* __restrict__ hbar, 
 // Theta^d_x = s_x Theta0_x + sum_k G_d[k][x] Theta0_{h_k}  (s_x = 1 for a reference non-hole, else 0),
 //   exchange  e = sum_{c in y-list} sum_{c' in x-list} coef_y[c] coef_x[c'] S[c][c'],
 //   Coulomb   j = sum_{c in x-list} sum_{c' in y-list} coef_x[c] coef_y[c'] S[c][c'],
-// lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of CE_CH pairs' S sits in shared memory, threads
+// lists = {self, the determinant's holes}.  grid (n_chunks, n_w); a chunk of ce (<= 16) pairs' S sits in shared memory, threads
 // run over determinants; partial (E_K, E_J) sums per chunk are added in chunk order by k_cas_e1sum.
-constexpr int CE_CH = 16;
+// With more than 6 active columns the S intermediates come in passes, one per pair of active groups (a <= b) of gs = 3
+// columns: pass p(a,b) = a ng - a(a-1)/2 + (b-a) holds S on the panel list {x, y, G_a, G_b} (local index 2 + l for a column of
+// G_a, 2 + gs + l for one of G_b); an entry S[c][c'] is read from the pass that contains both columns.  ng = 1 (<= 6 active
+// columns, gs = 6) is the single-pass case.
 template <int MAXE>     // compile-time bound of the excitation rank: the coefficient lists stay in registers
 __global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ S, const CasPair* __restrict__ tiles, long long n_tiles,
                                                     const signed char* __restrict__ kind, const int* __restrict__ holeIdx,
                                                     const double2* __restrict__ G, double2* __restrict__ part, int n_w, int n_det, int max_exc,
-                                                    int n_orb, int NP, int n_vtot, int pan_base) {
-    extern __shared__ __align__(16) double2 Ss[];      // [CE_CH][NP*NP]
-    __shared__ int tx_s[CE_CH], ty_s[CE_CH];
+                                                    int n_orb, int NP, int n_vtot, int pan_base, int gs, int ng, int npass, int ce) {
+    extern __shared__ __align__(16) double2 Ss[];      // [ce pairs][npass][NP*NP]
+    __shared__ int tx_s[16], ty_s[16];
     const int chunk = blockIdx.x, w = blockIdx.y, tid = threadIdx.x;
-    const long long t0 = (long long)chunk * CE_CH;
-    const int nt = (int)min((long long)CE_CH, n_tiles - t0), NP2 = NP * NP;
-    for (int i = tid; i < nt * NP2; i += 128) {
-        const int tl = i / NP2;
-        Ss[i] = S[((size_t)(t0 + tl) * n_w + w) * NP2 + (i - tl * NP2)];
+    const long long t0 = (long long)chunk * ce;
+    const int nt = (int)min((long long)ce, n_tiles - t0), NP2 = NP * NP, PS = npass * NP2;
+    for (int i = tid; i < nt * PS; i += 128) {
+        const int tl = i / PS, r = i - tl * PS, ps = r / NP2, e = r - ps * NP2;
+        Ss[i] = S[(((size_t)ps * n_tiles + (t0 + tl)) * n_w + w) * NP2 + e];
     }
     if (tid < nt) { tx_s[tid] = tiles[t0 + tid].pi - pan_base; ty_s[tid] = tiles[t0 + tid].pj - pan_base; }
     __syncthreads();
@@ -295,32 +298,47 @@ __global__ void __launch_bounds__(128) k_cas_energy(const double2* __restrict__ 
         const int* hi = holeIdx + (size_t)d * max_exc;
         int e = 0;
         while (e < max_exc && hi[e] >= 0) ++e;
+        // entry 0 = self, entries 1..e = the holes: group and local index inside the group
+        int grp[MAXE + 1], loc[MAXE + 1];
+        grp[0] = 0; loc[0] = 0;
+#pragma unroll
+        for (int k = 0; k < MAXE; ++k) {
+            const int ai = k < e ? hi[k] : 0;
+            grp[1 + k] = ai / gs;
+            loc[1 + k] = ai - grp[1 + k] * gs;
+        }
         const double2* Gv = G + v * max_exc * n_orb;
         double2 ek = make_double2(0.0, 0.0), ej = make_double2(0.0, 0.0);
         for (int tl = 0; tl < nt; ++tl) {
             const int x = tx_s[tl], y = ty_s[tl];
             const int kx = kd[x], ky = kd[y];
             if (kx < 0 || ky < 0) continue;
-            const double2* St = Ss + tl * NP2;
-            // coefficient lists: entry 0 = self (index 0 for the x role, 1 for the y role), entries 1..e = the holes
+            const double2* St = Ss + tl * PS;
             double2 cx[MAXE + 1], cy[MAXE + 1];
-            int ix[MAXE + 1], iy[MAXE + 1];
-            cx[0] = make_double2(kx == 0 ? 1.0 : 0.0, 0.0); ix[0] = 0;
-            cy[0] = make_double2(ky == 0 ? 1.0 : 0.0, 0.0); iy[0] = 1;
+            cx[0] = make_double2(kx == 0 ? 1.0 : 0.0, 0.0);
+            cy[0] = make_double2(ky == 0 ? 1.0 : 0.0, 0.0);
 #pragma unroll
             for (int k = 0; k < MAXE; ++k) {
                 const bool on = k < e;
-                cx[1 + k] = on ? Gv[(size_t)k * n_orb + x] : make_double2(0.0, 0.0); ix[1 + k] = on ? 2 + hi[k] : 0;
-                cy[1 + k] = on ? Gv[(size_t)k * n_orb + y] : make_double2(0.0, 0.0); iy[1 + k] = on ? 2 + hi[k] : 0;
+                cx[1 + k] = on ? Gv[(size_t)k * n_orb + x] : make_double2(0.0, 0.0);
+                cy[1 + k] = on ? Gv[(size_t)k * n_orb + y] : make_double2(0.0, 0.0);
             }
 #pragma unroll
-            for (int a = 0; a <= MAXE; ++a) {
+            for (int a = 0; a <= MAXE; ++a) {          // a: column in the y role
                 if (a > e) break;
 #pragma unroll
-                for (int b = 0; b <= MAXE; ++b) {
+                for (int b = 0; b <= MAXE; ++b) {      // b: column in the x role
                     if (b > e) break;
+                    // pass and local indices of (column a as y-role row, column b as x-role column)
+                    int ga = a ? grp[a] : (b ? grp[b] : 0), gb = b ? grp[b] : ga;
+                    int iy = a ? 2 + loc[a] : 1, ix = b ? 2 + loc[b] : 0;
+                    if (a && b && ga != gb) {
+                        if (ga < gb) ix += gs;
+                        else { iy += gs; const int t2 = ga; ga = gb; gb = t2; }
+                    }
+                    const double2* Sp = St + (ga * ng - ga * (ga - 1) / 2 + (gb - ga)) * NP2;
                     const double2 cc = cmul(cy[a], cx[b]);
-                    const double2 se = St[iy[a] * NP + ix[b]], sj = St[ix[b] * NP + iy[a]];
+                    const double2 se = Sp[iy * NP + ix], sj = Sp[ix * NP + iy];
                     const double2 t1 = cmul(cc, se), t2 = cmul(cc, sj);
                     ek.x += t1.x; ek.y += t1.y;
                     ej.x += t2.x; ej.y += t2.y;
@@ -349,13 +367,13 @@ __global__ void __launch_bounds__(128) k_cas_e1sum(const double2* __restrict__ p
     }
     const signed char* kd = kind + (size_t)d * n_orb;
     const int* hi = holeIdx + (size_t)d * max_exc;
-    const double2* Hw = H + (size_t)w * n_orb * 9;
+    const double2* Hw = H + (size_t)w * n_orb * CAS_HS;
     const double2* Gv = G + (size_t)v * max_exc * n_orb;
     for (int x = 0; x < n_orb; ++x) {
         if (kd[x] < 0) continue;
-        if (kd[x] == 0) { e1.x += Hw[x * 9].x; e1.y += Hw[x * 9].y; }
+        if (kd[x] == 0) { e1.x += Hw[x * CAS_HS].x; e1.y += Hw[x * CAS_HS].y; }
         for (int k = 0; k < max_exc && hi[k] >= 0; ++k) {
-            const double2 t1 = cmul(Gv[(size_t)k * n_orb + x], Hw[x * 9 + 1 + hi[k]]);
+            const double2 t1 = cmul(Gv[(size_t)k * n_orb + x], Hw[x * CAS_HS + 1 + hi[k]]);
             e1.x += t1.x; e1.y += t1.y;
         }
     }
@@ -625,13 +643,13 @@ __global__ void __launch_bounds__(128) k_cas_esum_u(EsSpin sa, EsSpin sb, const 
         }
         const signed char* kd = S.kind + (size_t)d * S.n_orb;
         const int* hi = S.holeIdx + (size_t)d * max_exc;
-        const double2* Hw = S.H + (size_t)w * S.n_orb * 9;
+        const double2* Hw = S.H + (size_t)w * S.n_orb * CAS_HS;
         const double2* Gv = S.G + (size_t)v * max_exc * S.n_orb;
         for (int x = 0; x < S.n_orb; ++x) {
             if (kd[x] < 0) continue;
-            if (kd[x] == 0) { e1.x += Hw[x * 9].x; e1.y += Hw[x * 9].y; }
+            if (kd[x] == 0) { e1.x += Hw[x * CAS_HS].x; e1.y += Hw[x * CAS_HS].y; }
             for (int k = 0; k < max_exc && hi[k] >= 0; ++k) {
-                const double2 t1 = cmul(Gv[(size_t)k * S.n_orb + x], Hw[x * 9 + 1 + hi[k]]);
+                const double2 t1 = cmul(Gv[(size_t)k * S.n_orb + x], Hw[x * CAS_HS + 1 + hi[k]]);
                 e1.x += t1.x; e1.y += t1.y;
             }
         }
@@ -706,27 +724,33 @@ lo_status launch_local_energy_cas(lo_factors* f, int n_w, const void* phi, const
             const CUtensorMap& tm0 = s ? c.tmTh0B : c.tmTh0;
             const long long items = nt * WB;
             const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-            if (NP == 4)
-                k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
-            else if (NP == 6)
-                k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
-            else
-                k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, actd, S, n_w, pan_base);
+            // one pass per pair of active groups (a single pass for <= 6 active columns); pass p fills S[p][pair][walker]
+            for (int ps = 0; ps < c.npass[s]; ++ps) {
+                const int* pact = c.dPassAct[s] + (size_t)ps * 6;
+                double2* Sp = S + (size_t)ps * nt * n_w * NP * NP;
+                if (NP == 4)
+                    k_cas_pairs<4><<<grid, 384, CpCfg<4>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, pact, Sp, n_w, pan_base);
+                else if (NP == 6)
+                    k_cas_pairs<6><<<grid, 384, CpCfg<6>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, pact, Sp, n_w, pan_base);
+                else
+                    k_cas_pairs<8><<<grid, 384, CpCfg<8>::SMEM, stream>>>(f->tmUf, f->tmWf, tm0, f->dWgt, f->dTiles4, tiles, items, WB, f->N_pad, ldw0, pact, Sp, n_w, pan_base);
+            }
             k_cas_H<<<n_w, 256, 0, stream>>>(hbar0 + (size_t)pan_base * f->N_pad, th0, actd, n_act, (double2*)(s ? c.dHB : c.dH), f->N, f->N_pad,
                                              n_ref_s, n_orb_s, ldw0);
-            const int n_chunks = (int)((nt + CE_CH - 1) / CE_CH);
+            const int ce = c.ce[s], gs = c.gs[s], ng = c.ng[s], npass = c.npass[s];
+            const int n_chunks = (int)((nt + ce - 1) / ce);
             if (n_chunks > 0) {
                 dim3 g4(n_chunks, n_w);
-                const size_t sm4 = (size_t)CE_CH * NP * NP * 16;
+                const size_t sm4 = (size_t)ce * npass * NP * NP * 16;
                 const signed char* kind = s ? c.dKindB : c.dKind;
                 const double2* G = (const double2*)(s ? c.dGB : c.dG);
                 double2* part = (double2*)(s ? c.dPartB : c.dPart);
                 if (c.max_exc <= 2)
-                    k_cas_energy<2><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base);
+                    k_cas_energy<2><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base, gs, ng, npass, ce);
                 else if (c.max_exc <= 4)
-                    k_cas_energy<4><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base);
+                    k_cas_energy<4><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base, gs, ng, npass, ce);
                 else
-                    k_cas_energy<8><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base);
+                    k_cas_energy<8><<<g4, 128, sm4, stream>>>(S, tiles, nt, kind, hidx, G, part, n_w, c.n_det, c.max_exc, n_orb_s, NP, n_vtot, pan_base, gs, ng, npass, ce);
             }
         }
         if (!unres) {

@@ -84,6 +84,8 @@ struct CasPair {
 // (= the first n_ref orbitals of the factor set's Psi), workspace for max_real real walkers; the n_det determinants of a
 // real walker are laid out as n_det consecutive VIRTUAL walkers of the ordinary S3-S5 path.
 constexpr int CAS_MAX_EXC = 8;
+constexpr int CAS_MAX_ACT = 12;     // distinct hole columns per spin in LO_CAS_SMW_ENERGY (closed shell; 6 for unrestricted trials)
+constexpr int CAS_HS = 1 + CAS_MAX_ACT;   // slots per orbital of the one-body intermediates H
 struct CasPlan {
     int n_ref = 0, n_det = 0, max_exc = 0, n_virt = 0, max_real = 0, W0cap = 0;
     int *dHoles = nullptr, *dParts = nullptr;   // [n_det][max_exc]
@@ -105,23 +107,27 @@ struct CasPlan {
     // ---- rearranged SMW energy (Eq. 23), mode 1
     int mode = 0;                               // 0: direct summation over virtual walkers, 1: SMW energy
     int n_act = 0, NP = 0;                      // active (hole) columns A_set, panel-set size NP = 2 + padded n_act (4, 6 or 8)
-    int hAct[8] = {0, 0, 0, 0, 0, 0, 0, 0};     // A_set (orbital = reference column), padded with 0
+    int hAct[16] = {0};                         // A_set (orbital = reference column), padded with 0
     int* dHoleIdx = nullptr;                    // [n_det][max_exc]: index of hole k in A_set
     signed char* dKind = nullptr;               // [n_det][n_orb]: -1 unoccupied, 0 reference non-hole, 1+m particle m
     double* dS = nullptr;                       // S[tile][w][NP][NP] complex (Eq. 23 intermediates contracted over K)
-    double* dH = nullptr;                       // one-body intermediates [W0cap][n_orb][1 + 8] complex (self, A_set)
+    double* dH = nullptr;                       // one-body intermediates [W0cap][n_orb][CAS_HS] complex (self, A_set)
     double* dPart = nullptr;                    // [n_chunks][max_real*n_det][2] complex partial (E_K, E_J) sums
     int n_chunks = 0;
     CUtensorMap tmTh0;                          // Theta0^T panels [n_orb*2*W0cap][N_pad], box 32 x 16 (16 walkers)
     // ---- rearranged SMW energy with an UNRESTRICTED trial (n_spin == 2): the alpha data are the fields above, the beta
     // data the *B fields; exchange per spin from that spin's tiles, Coulomb by the Cholesky route from SMW-updated X^g
     int n_actB = 0, NPB = 0, n_chunksB = 0;
-    int hActB[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int hActB[16] = {0};
     int* dHoleIdxB = nullptr;
     signed char* dKindB = nullptr;
     double *dSB = nullptr, *dHB = nullptr, *dPartB = nullptr;
     int* dStVB = nullptr;
     CUtensorMap tmTh0B;
+    // more than 6 active columns (closed shell, <= CAS_MAX_ACT): the active set is cut into groups of gs = 3 and k_cas_pairs runs
+    // once per pair of groups (a <= b) on the panel list {x, y, G_a, G_b}; pass p(a,b) = a ng - a(a-1)/2 + (b - a)
+    int gs[2] = {6, 6}, ng[2] = {1, 1}, npass[2] = {1, 1}, ce[2] = {16, 16};   // group size, groups, passes, pairs per k_cas_energy chunk
+    int* dPassAct[2] = {nullptr, nullptr};      // [npass][6] panel (orbital) indices of every pass
     CasPair* dPairs[2] = {nullptr, nullptr};    // pairs with rows, per spin (tile ranges into the factor set's <= 4-fragment tile list)
     long long npair[2] = {0, 0};
     double* dThAct[2] = {nullptr, nullptr};     // gathered active panels [n_act][2*W0cap][N_pad] per spin (A operand of the Z GEMM)

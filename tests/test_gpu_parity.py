@@ -796,7 +796,7 @@ def test_cas_unrestricted_smw_200_determinants_rank_6():
 
 def test_cas_smw_edge_cases(c0):
     """One determinant (no excitation) through the SMW-energy mode = the single-determinant energy with the
-    compressed Coulomb term; more than 6 distinct hole columns are refused in that mode (and accepted in direct mode)."""
+    compressed Coulomb term."""
     torch = torch_cuda()
     T = gen.make_cas_trial(c0, n_virt=3, n_act_occ=3, n_det=4, max_exc=2)
     F = lo.Factors.setup(c0.h, c0.L, [T.C], 1e-8, device=0, max_walkers=64, gpu_svd=True)
@@ -808,14 +808,47 @@ def test_cas_smw_edge_cases(c0):
     F0.set_coulomb_mode(True)
     Es, _ = gpu_energy(F0, [phi])
     assert np.abs(E1d.cpu().numpy().T[:, :4] - Es).max() <= 1e-9 * np.abs(Es[:, 0]).max()
-    # 7 distinct hole columns (c0 has 6 reference columns -> use a wider reference)
-    P = gen.make_problem(1)
-    Tw = gen.make_cas_trial(P, n_virt=4, n_act_occ=9, n_det=40, max_exc=2)
-    assert len(set(Tw.holes[Tw.holes >= 0].tolist())) > 6
-    Fw = lo.Factors.setup(P.h, P.L, [Tw.C], 1e-2, device=0, max_walkers=80, gpu_svd=True)
-    with pytest.raises(lo.LoError):
-        Fw.set_cas_trial(Tw.n_ref, Tw.holes, Tw.parts, Tw.coef, 2, smw_energy=True)
-    Fw.set_cas_trial(Tw.n_ref, Tw.holes, Tw.parts, Tw.coef, 2, smw_energy=False)
+
+
+@pytest.mark.parametrize("n_act,max_exc,n_det", [(9, 2, 40), (12, 4, 60)])
+def test_cas_smw_more_than_six_hole_columns(c1, n_act, max_exc, n_det):
+    """More than 6 distinct hole columns in LO_CAS_SMW_ENERGY (closed shell): the active set is cut into groups of 3 and the
+    S intermediates are formed in one pass per pair of groups (3 groups -> 6 passes, 4 groups -> 10); every output against
+    the oracle's definition with both two-body terms from the factors (Eq. 22), 1e-10, and against the direct-summation
+    mode.  More than 12 hole columns are refused."""
+    torch = torch_cuda()
+    n_w = 5
+    T = gen.make_cas_trial(c1, n_virt=5, n_act_occ=n_act, n_det=n_det, max_exc=max_exc)
+    assert len(set(T.holes[T.holes >= 0].tolist())) == n_act
+    F = lo.Factors.setup(c1.h, c1.L, [T.C], 1e-3, device=0, max_walkers=n_w * n_det, gpu_svd=True)
+    phi = gen.make_walkers(c1, n_w)[0]
+    dphi = torch.from_numpy(phi).cuda()
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w, smw_energy=True)
+    E, st = F.local_energy_cas(dphi)
+    torch.cuda.synchronize()
+    E, st = E.cpu().numpy().T, st.cpu().numpy()
+    assert (st == 0).all()
+    Lbar, hbar = oracle.half_rotate(c1.L, c1.h, T.C)
+    n_orb = T.C.shape[1]
+    U, sg, W = F.factor_all(0)
+    pi, pj = oracle.all_pairs(n_orb)
+    fs = oracle.make_factor_set(c1.N, n_orb, pi, pj, F.ranks(0), U, sg, W)
+    cols = [T.columns(d) for d in range(T.n_det)]
+    for w in (0, n_w - 1):
+        Eo = np.array(oracle.local_energy_cas(T.C, cols, T.coef, Lbar, hbar, fs, phi[w], compressed_coulomb=True))
+        assert np.abs(E[w, :4] - Eo[:4]).max() <= TOL * abs(Eo[0]), (w, E[w], Eo)
+        assert abs(E[w, 4] - Eo[4]) <= TOL * abs(Eo[4])
+    F.set_coulomb_mode(True)
+    F.set_cas_trial(T.n_ref, T.holes, T.parts, T.coef, n_w, smw_energy=False)
+    Ed, _ = F.local_energy_cas(dphi)
+    assert (np.abs(E - Ed.cpu().numpy().T).max(axis=1) <= 1e-9 * np.abs(E[:, 0])).all()
+    if n_act == 12:
+        T13 = gen.make_cas_trial(c1, n_virt=5, n_act_occ=13, n_det=80, max_exc=2)
+        assert len(set(T13.holes[T13.holes >= 0].tolist())) == 13
+        F13 = lo.Factors.setup(c1.h, c1.L, [T13.C], 1.0, device=0, max_walkers=160, gpu_svd=True)
+        with pytest.raises(lo.LoError):
+            F13.set_cas_trial(T13.n_ref, T13.holes, T13.parts, T13.coef, 2, smw_energy=True)
+        F13.set_cas_trial(T13.n_ref, T13.holes, T13.parts, T13.coef, 2, smw_energy=False)
 
 
 def test_cas_unrestricted_matches_oracle():
