@@ -240,6 +240,34 @@ lo_status finish_pack(lo_factors* f) {
     if (!f->hTiles.empty()) CK(cudaMemcpy(f->dTiles, f->hTiles.data(), f->hTiles.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
     CK(cudaMalloc(&f->dTiles4, std::max<size_t>(1, f->hTiles4.size()) * sizeof(ExTile)));
     if (!f->hTiles4.empty()) CK(cudaMemcpy(f->dTiles4, f->hTiles4.data(), f->hTiles4.size() * sizeof(ExTile), cudaMemcpyHostToDevice));
+    {
+        // Static schedule for small problems (a CTA then gets only a handful of items): tiles dealt to num_sms CTAs by
+        // accumulated weight, heaviest first to the least loaded CTA (LPT); weight = fragments + 1/2 (per-item overhead);
+        // every CTA's list in ascending tile order.  Fixed for the factor set: results stay repeatable.
+        const int G = std::max(1, f->num_sms);
+        const size_t nt = f->hTiles.size();
+        std::vector<int> ord(nt), owner(nt), off(G + 1, 0), lst(nt);
+        std::iota(ord.begin(), ord.end(), 0);
+        std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return f->hTiles[a].nfrag > f->hTiles[b].nfrag; });
+        std::vector<std::pair<double, int>> heap;          // (load, cta) min-heap
+        for (int c = 0; c < G; ++c) heap.push_back({0.0, c});
+        auto cmp = [](const std::pair<double, int>& a, const std::pair<double, int>& b) { return a.first != b.first ? a.first > b.first : a.second > b.second; };
+        std::make_heap(heap.begin(), heap.end(), cmp);
+        for (int t : ord) {
+            std::pop_heap(heap.begin(), heap.end(), cmp);
+            heap.back().first += f->hTiles[t].nfrag + 0.5;
+            owner[t] = heap.back().second;
+            std::push_heap(heap.begin(), heap.end(), cmp);
+        }
+        for (size_t t = 0; t < nt; ++t) ++off[owner[t] + 1];
+        for (int c = 0; c < G; ++c) off[c + 1] += off[c];
+        std::vector<int> pos(off.begin(), off.end() - 1);
+        for (size_t t = 0; t < nt; ++t) lst[pos[owner[t]]++] = (int)t;
+        CK(cudaMalloc(&f->dSchedOff, (size_t)(G + 1) * 4));
+        CK(cudaMalloc(&f->dSchedTile, std::max<size_t>(nt, 1) * 4));
+        CK(cudaMemcpy(f->dSchedOff, off.data(), (size_t)(G + 1) * 4, cudaMemcpyHostToDevice));
+        if (nt) CK(cudaMemcpy(f->dSchedTile, lst.data(), nt * 4, cudaMemcpyHostToDevice));
+    }
     st = make_tmap(&f->tmU, f->dU, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmW, f->dW, f->N_pad, rows_alloc, EX_BM);
     if (st == LO_OK) st = make_tmap(&f->tmU8, f->dU, f->N_pad, rows_alloc, 8);
@@ -360,7 +388,7 @@ void free_all(lo_factors* f) {
         for (int c = 0; c < LO_HOST_CHUNKS; ++c)
             if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
         if (f->evEnter) cudaEventDestroy(f->evEnter);
-        void* ptrs[] = {f->dWgt, f->dTiles, f->dTiles4, f->dEJLpart, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
+        void* ptrs[] = {f->dSchedOff, f->dSchedTile, f->dWgt, f->dTiles, f->dTiles4, f->dEJLpart, f->dThT, f->dA[0], f->dA[1], f->dXpart, f->dEJpart, f->dEKpart,
                         f->dStatus, f->dEout, f->dStatusOut, f->dPhi[0], f->dPhi[1], f->dXT, f->dB};
         for (void* p : ptrs)
             if (p) cudaFree(p);

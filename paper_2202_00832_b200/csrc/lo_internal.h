@@ -183,6 +183,7 @@ struct lo_factors {
     double *dU = nullptr, *dW = nullptr, *dWgt = nullptr;
     lo::ExTile* dTiles = nullptr;
     lo::ExTile* dTiles4 = nullptr;
+    int *dSchedOff = nullptr, *dSchedTile = nullptr;   // static schedule of the tiles over num_sms CTAs (small problems), CSR
     CUtensorMap tmU, tmW, tmTheta;       // 2D [rows][N_pad]: boxes 64 x 16 (U, W) and 128 x 16 (Theta^T), 128B swizzle
     CUtensorMap tmU8, tmW8;              // same arrays, boxes 8 x 16 (one row fragment): tiles shorter than 64 rows
     lo::TmSet tmUf, tmWf;                // same arrays, boxes (8 k) x 16 for k = 1..8: one TMA issue per operand for a tile of k fragments

@@ -641,6 +641,30 @@ constexpr int EX_STAGES = 4;
 constexpr int EX_STAGE_BYTES = (2 * EX_BM + 2 * 128) * 128;
 constexpr int EX_SMEM = EX_STAGES * EX_STAGE_BYTES + 1024 + 128 + EX_RING * 16;
 
+// Which (tile, walker block) items a CTA works on, in which order.  Default: round robin over q = tile * NB + nb.  With a
+// static schedule (small problems, where a CTA gets only a handful of items and one item more or less is a 5-15 % imbalance):
+// tiles dealt to the CTAs by accumulated fragment count on the host (longest-processing-time first), CSR lists off / tile;
+// every CTA runs its tiles in list order, all walker blocks of a tile one after the other.  Either way the order is fixed
+// for a factor set and grid: results stay bitwise repeatable.
+struct ExItems {
+    const int* off;      // [gridDim.x + 1] or NULL (round robin)
+    const int* tile;     // [n_tiles]
+    __device__ __forceinline__ long long count(long long n_items, int NB) const {
+        if (off) return (long long)(off[blockIdx.x + 1] - off[blockIdx.x]) * NB;
+        return n_items > (long long)blockIdx.x ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    }
+    __device__ __forceinline__ void at(long long it, int NB, int& tile_idx, int& nb) const {
+        if (off) {
+            tile_idx = tile[off[blockIdx.x] + (int)(it / NB)];
+            nb = (int)(it % NB);
+        } else {
+            const long long q = blockIdx.x + it * gridDim.x;
+            tile_idx = (int)(q / NB);
+            nb = (int)(q % NB);
+        }
+    }
+};
+
 // COUL: also accumulate the two projections of the paper-literal compressed Coulomb term,
 // aJ = U Theta_i and bJ = W Theta_j (Eq. 19/22 first term, "forming the projected vectors must occur four times",
 // PAPER.md:181), from the same staged tiles; tiles are then cut at 4 fragments so the four accumulator sets fit.
@@ -687,7 +711,7 @@ template <bool COUL, bool RAGGED>   // RAGGED: the batch is not a multiple of 64
 __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ TmSet tmUs, const __grid_constant__ TmSet tmWs,
                                                      const __grid_constant__ CUtensorMap tmT, const double* __restrict__ wgt,
                                                      const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
-                                                     double* __restrict__ ekpart, double* __restrict__ ejpart, int Wcap, int n_w) {
+                                                     double* __restrict__ ekpart, double* __restrict__ ejpart, int Wcap, int n_w, ExItems items) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
@@ -715,9 +739,11 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ TmS
         if (warp == 0 && lane == 0) {
             int slot = 0, n = 0;
             uint32_t phase = 0;
-            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-                const ExTile tile = tiles[q / NB];
-                const int nb = (int)(q % NB);
+            const long long my_items = items.count(n_items, NB);
+            for (long long it = 0; it < my_items; ++it, ++n) {
+                int tile_idx, nb;
+                items.at(it, NB, tile_idx, nb);
+                const ExTile tile = tiles[tile_idx];
                 const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + 2 * 128) * 128;
                 for (int kt = 0; kt < KT; ++kt) {
                     mbar_wait(empty + 8 * slot, phase ^ 1);
@@ -755,8 +781,10 @@ __global__ void __launch_bounds__(384, 1) k_exchange(const __grid_constant__ TmS
     const uint32_t tj_row = (uint32_t)(2 * EX_BM + cw * 16 + g) * 128;
     int cslot = 0, n = 0;
     uint32_t cphase = 0;
-    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-        const int nb = (int)(q % NB);
+    const long long my_items = items.count(n_items, NB);
+    for (long long it = 0; it < my_items; ++it, ++n) {
+        int tile_idx, nb;
+        items.at(it, NB, tile_idx, nb);
         // this lane's slice of the CTA partial (lanes with g == 0 own walker cw*8 + nf*4 + t of the block): fetched now,
         // updated after the K loop (same thread wrote it last, so program order makes the previous update visible)
         double2* myp = reinterpret_cast<double2*>(mypart + (size_t)nb * 128 + cw * 16 + 2 * t);
@@ -900,7 +928,7 @@ __device__ __forceinline__ void en_kloop(int KT, uint32_t sbase, uint32_t full, 
 __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constant__ TmSet tmUs, const __grid_constant__ TmSet tmWs,
                                                             const __grid_constant__ CUtensorMap tmT32, const double* __restrict__ wgt,
                                                             const ExTile* __restrict__ tiles, long long n_items, int NB, int N_pad, int ldw,
-                                                            double* __restrict__ ekpart, int Wcap) {
+                                                            double* __restrict__ ekpart, int Wcap, ExItems items) {
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char* sgen = smem_raw + (sbase - smem_u32(smem_raw));
@@ -923,9 +951,11 @@ __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constan
         if (warp == 0 && lane == 0) {
             int slot = 0, n = 0;
             uint32_t phase = 0;
-            for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-                const ExTile tile = tiles[q / NB];
-                const int nb = (int)(q % NB);
+            const long long my_items = items.count(n_items, NB);
+            for (long long it = 0; it < my_items; ++it, ++n) {
+                int tile_idx, nb;
+                items.at(it, NB, tile_idx, nb);
+                const ExTile tile = tiles[tile_idx];
                 const uint32_t tx = (uint32_t)(2 * tile.nfrag * 8 + 2 * 32) * 128;
                 const CUtensorMap* mu = &tmUs.m[tile.nfrag - 1];
                 const CUtensorMap* mw = &tmWs.m[tile.nfrag - 1];
@@ -959,8 +989,10 @@ __global__ void __launch_bounds__(384, 1) k_exchange_narrow(const __grid_constan
     double e0r = 0.0, e0i = 0.0, e1r = 0.0, e1i = 0.0;      // this lane's running sums for walker block 0 / 1
     int cslot = 0, n = 0;
     uint32_t cphase = 0;
-    for (long long q = blockIdx.x; q < n_items; q += gridDim.x, ++n) {
-        const int nb = (int)(q % NB);
+    const long long my_items = items.count(n_items, NB);
+    for (long long it = 0; it < my_items; ++it, ++n) {
+        int tile_idx, nb;
+        items.at(it, NB, tile_idx, nb);
         mbar_wait(full + 8 * cslot, cphase);
         const ExTile tile = ring[n % EX_RING];
         const int nfw = tile.nfrag > fg ? (tile.nfrag - fg + 1) >> 1 : 0;     // warp-uniform
@@ -1221,21 +1253,29 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         long long items = (coul ? f->n_tiles4 : f->n_tiles) * NB;
         ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
         const bool ragged = n_w % WALKER_TILE != 0;
+        // small problems: static LPT schedule of the tiles (grid = all SMs); large ones: round robin in L2-block order
+        const ExItems rr = {nullptr, nullptr}, lpt = {f->dSchedOff, f->dSchedTile};
         if (!coul && n_w <= 32) {
             // narrow batch: 16-walker column blocks, row fragments split over the warps
             const int NB16 = (n_w + 15) / 16;
             items = f->n_tiles * NB16;
-            ex_grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
+            const bool use_lpt = items <= 64LL * f->num_sms && f->n_tiles >= f->num_sms;
+            ex_grid = use_lpt ? f->num_sms : (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
             k_exchange_narrow<<<ex_grid, 384, EN_SMEM, stream>>>(f->tmUf, f->tmWf, f->tmTheta32, f->dWgt, f->dTiles, items, NB16,
-                                                                 N_pad, ldw, f->dEKpart, Wcap);
+                                                                 N_pad, ldw, f->dEKpart, Wcap, use_lpt ? lpt : rr);
         } else
 #define LO_EX_LAUNCH(C_, R_, TILES_, EJ_)                                                                                              \
     k_exchange<C_, R_><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmUf, f->tmWf, f->tmTheta, f->dWgt, TILES_, items, NB, N_pad, ldw, \
-                                                          f->dEKpart, EJ_, Wcap, n_w)
-        if (coul && ragged) LO_EX_LAUNCH(true, true, f->dTiles4, f->dEJLpart);
-        else if (coul) LO_EX_LAUNCH(true, false, f->dTiles4, f->dEJLpart);
-        else if (ragged) LO_EX_LAUNCH(false, true, f->dTiles, nullptr);
-        else LO_EX_LAUNCH(false, false, f->dTiles, nullptr);
+                                                          f->dEKpart, EJ_, Wcap, n_w, IT_)
+        {
+            const bool use_lpt = !coul && items <= 64LL * f->num_sms && f->n_tiles >= f->num_sms;
+            if (use_lpt) ex_grid = f->num_sms;
+            const ExItems IT_ = use_lpt ? lpt : rr;
+            if (coul && ragged) LO_EX_LAUNCH(true, true, f->dTiles4, f->dEJLpart);
+            else if (coul) LO_EX_LAUNCH(true, false, f->dTiles4, f->dEJLpart);
+            else if (ragged) LO_EX_LAUNCH(false, true, f->dTiles, nullptr);
+            else LO_EX_LAUNCH(false, false, f->dTiles, nullptr);
+        }
 #undef LO_EX_LAUNCH
     }
     // ---- S5
