@@ -1259,7 +1259,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
             // narrow batch: 16-walker column blocks, row fragments split over the warps
             const int NB16 = (n_w + 15) / 16;
             items = f->n_tiles * NB16;
-            const bool use_lpt = items <= 64LL * f->num_sms && f->n_tiles >= f->num_sms;
+            const bool use_lpt = items <= 64LL * f->num_sms && f->n_tiles >= 8LL * f->num_sms;     // whole tiles are dealt: needs many tiles per CTA
             ex_grid = use_lpt ? f->num_sms : (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
             k_exchange_narrow<<<ex_grid, 384, EN_SMEM, stream>>>(f->tmUf, f->tmWf, f->tmTheta32, f->dWgt, f->dTiles, items, NB16,
                                                                  N_pad, ldw, f->dEKpart, Wcap, use_lpt ? lpt : rr);
@@ -1268,7 +1268,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
     k_exchange<C_, R_><<<ex_grid, 384, EX_SMEM, stream>>>(f->tmUf, f->tmWf, f->tmTheta, f->dWgt, TILES_, items, NB, N_pad, ldw, \
                                                           f->dEKpart, EJ_, Wcap, n_w, IT_)
         {
-            const bool use_lpt = !coul && items <= 64LL * f->num_sms && f->n_tiles >= f->num_sms;
+            const bool use_lpt = !coul && items <= 64LL * f->num_sms && f->n_tiles >= 8LL * f->num_sms;
             if (use_lpt) ex_grid = f->num_sms;
             const ExItems IT_ = use_lpt ? lpt : rr;
             if (coul && ragged) LO_EX_LAUNCH(true, true, f->dTiles4, f->dEJLpart);
