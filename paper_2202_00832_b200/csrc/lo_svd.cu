@@ -398,12 +398,21 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
                 double acc[10][2];
 #pragma unroll
                 for (int a = 0; a < 10; ++a) acc[a][0] = acc[a][1] = 0.0;
+                // two column chunks of 8 ahead: the loads of chunks k0 + 8 and k0 + 16 are in flight under the MMAs of chunk k0
+                double f[2][4], f1[2][4];
+#pragma unroll
+                for (int h2 = 0; h2 < 2; ++h2)
+#pragma unroll
+                    for (int ti = 0; ti < 4; ++ti) {
+                        f[h2][ti] = okt[ti] ? G[(size_t)rowt[ti] * ld + 4 * h2 + t] : 0.0;
+                        f1[h2][ti] = (okt[ti] && 8 < ld) ? G[(size_t)rowt[ti] * ld + 8 + 4 * h2 + t] : 0.0;
+                    }
                 for (int k0 = 0; k0 < ld; k0 += 8) {
-                    double f[2][4];
+                    double f2[2][4];
 #pragma unroll
                     for (int h2 = 0; h2 < 2; ++h2)
 #pragma unroll
-                        for (int ti = 0; ti < 4; ++ti) f[h2][ti] = okt[ti] ? G[(size_t)rowt[ti] * ld + k0 + 4 * h2 + t] : 0.0;
+                        for (int ti = 0; ti < 4; ++ti) f2[h2][ti] = (okt[ti] && k0 + 16 < ld) ? G[(size_t)rowt[ti] * ld + k0 + 16 + 4 * h2 + t] : 0.0;
 #pragma unroll
                     for (int h2 = 0; h2 < 2; ++h2) {
                         int a = 0;
@@ -412,6 +421,10 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
 #pragma unroll
                             for (int tj = ti; tj < 4; ++tj, ++a) mma884(acc[a][0], acc[a][1], f[h2][ti], f[h2][tj]);
                     }
+#pragma unroll
+                    for (int h2 = 0; h2 < 2; ++h2)
+#pragma unroll
+                        for (int ti = 0; ti < 4; ++ti) { f[h2][ti] = f1[h2][ti]; f1[h2][ti] = f2[h2][ti]; }
                 }
                 {
                     int a = 0;
@@ -470,12 +483,15 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
                 for (int pass = 0; pass < (V ? 2 : 1); ++pass) {
                     double* X = pass == 0 ? G : V;
                     const int ldx = pass == 0 ? ld : ldv;
-                    double bf[8];
+                    double bf[8], b1[8];
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) bf[ks] = okk[ks] ? X[(size_t)rowk[ks] * ldx + g] : 0.0;
+                    for (int ks = 0; ks < 8; ++ks) {
+                        bf[ks] = okk[ks] ? X[(size_t)rowk[ks] * ldx + g] : 0.0;
+                        b1[ks] = (okk[ks] && 8 < ldx) ? X[(size_t)rowk[ks] * ldx + 8 + g] : 0.0;
+                    }
                     for (int c0 = 0; c0 < ldx; c0 += 8) {
                         double nx[8];
-                        const int c1 = c0 + 8;
+                        const int c1 = c0 + 16;
 #pragma unroll
                         for (int ks = 0; ks < 8; ++ks) nx[ks] = (c1 < ldx && okk[ks]) ? X[(size_t)rowk[ks] * ldx + c1 + g] : 0.0;
                         double d[4][2];
@@ -490,7 +506,7 @@ __global__ void __launch_bounds__(SVD_WARPS * 32) k_block_jacobi(double* __restr
                         for (int mt = 0; mt < 4; ++mt)
                             if (okt[mt]) *reinterpret_cast<double2*>(&X[(size_t)rowt[mt] * ldx + c0 + 2 * t]) = make_double2(d[mt][0], d[mt][1]);
 #pragma unroll
-                        for (int ks = 0; ks < 8; ++ks) bf[ks] = nx[ks];
+                        for (int ks = 0; ks < 8; ++ks) { bf[ks] = b1[ks]; b1[ks] = nx[ks]; }
                     }
                 }
             }
