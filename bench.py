@@ -293,6 +293,21 @@ def run_ours(args):
                                      "energies_per_s": round(n_w * args.steps / (c0.elapsed_time(c1) * 1e-3), 2),
                                      "exchange_ms": round(c_ms, 4), "exchange_tflops": round(c_tf, 3), "exchange_frac_of_peak": round(c_tf / peak, 4)}
 
+    # ---- gated experiment (never part of `value` or of the product path): one FP64-accurate GEMM tile from INT8 slices
+    # on tcgen05, against the same tile's cost at the measured DMMA peak
+    if rank == 0:
+        try:
+            p_us, p_err = lo.measure_peak("int8_tile_us", local), lo.measure_peak("int8_tile_err", local)
+            dmma_us = 2.0 * 128 * 128 * 384 / (peak_dmma * 1e12 / torch.cuda.get_device_properties(local).multi_processor_count) * 1e6
+            nxt = dict(nxt or {})
+            nxt["int8_slicing_probe"] = {"what": "128 x 128 x 384 fp64 tile from 6 x 6 INT8 slices (21 digit products, tcgen05.mma kind::i8, TMEM, fp64 "
+                                                 "recombination); operands resident in shared memory: the operand feed is not measured",
+                                         "us_per_tile": round(p_us, 3), "max_err_vs_fp64_rel_to_max": p_err,
+                                         "same_tile_at_measured_dmma_peak_us": round(dmma_us, 3), "ratio": round(dmma_us / p_us, 2)}
+        except lo.LoError as e:
+            nxt = dict(nxt or {})
+            nxt["int8_slicing_probe"] = {"error": str(e)}
+
     # ---- SURVEY 8(f) NEXT-2 (opt-in, outside `value`): multi-determinant trial by direct summation, own factor set
     if args.cas > 0 and info.n_spin == 1:
         n_virt, n_real = 6, max(1, n_w // args.cas)

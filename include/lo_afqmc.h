@@ -79,7 +79,7 @@ enum { LO_K_OVERLAP = 0, LO_K_INVERSE = 1, LO_K_THETA = 2, LO_K_COULOMB = 3, LO_
  *   threshold >= 0 (T_SVD, same units as the integrals).
  *   device >= 0: CUDA device that will hold the factor set and workspace for up to max_walkers walkers.
  *   device <  0: host-only factor set (accessors work; lo_local_energy* return LO_ECUDA).
- *   flags  bit 0 (LO_SETUP_GPU_SVD): run the half-rotation, pair Gram matrices and Jacobi SVDs on the device
+ *   flags  bit 0 (LO_SETUP_GPU_SVD): run the pair Gram matrices and their SVDs (block one-sided Jacobi, DMMA) on the device
  *          (needs device >= 0); otherwise they run on the host with OpenMP.
  * On success *out owns everything; release with lo_free. */
 #define LO_SETUP_GPU_SVD 1
@@ -240,7 +240,12 @@ lo_status lo_flops_per_walker(const lo_factors* f, double flops[LO_K_COUNT]);
 /* In-run roofline denominators (microbenchmarks on `device`):
  *   kind 0: FP64 tensor pipe, register-resident DMMA.8x8x4 loop  -> *value in TFLOP/s
  *   kind 1: FP64 FMA pipe, register-resident DFMA loop           -> *value in TFLOP/s
- *   kind 2: HBM stream copy (read+write bytes)                   -> *value in GB/s */
+ *   kind 2: HBM stream copy (read+write bytes)                   -> *value in GB/s
+ * and one gated experiment that is NOT part of any product path: an FP64-accurate 128 x 128 x 384 GEMM
+ * tile from 6 x 6 signed 7-bit INT8 slices on the 5th-generation tensor cores (tcgen05.mma kind::i8, TMEM accumulators, fp64
+ * recombination), operands resident in shared memory:
+ *   kind 3: microseconds per tile                                -> *value in us
+ *   kind 4: max |C - C_fp64| / max |C_fp64| of that tile         -> *value dimensionless */
 lo_status lo_measure_peak(int device, int kind, double* value);
 
 void lo_free(lo_factors* f);

@@ -95,9 +95,10 @@ def _np(a, dtype):
 
 
 def measure_peak(kind: str, device: int = 0) -> float:
-    """In-run roofline denominators: 'dmma' / 'dfma' in TFLOP/s, 'hbm' in GB/s."""
+    """In-run roofline denominators: 'dmma' / 'dfma' in TFLOP/s, 'hbm' in GB/s; the gated INT8-slicing probe on tcgen05
+    (DESIGN.md 10.1): 'int8_tile_us' (microseconds per 128 x 128 x 384 tile) and 'int8_tile_err' (error against fp64)."""
     v = C.c_double(0)
-    _check(lib().lo_measure_peak(device, {"dmma": 0, "dfma": 1, "hbm": 2}[kind], C.byref(v)))
+    _check(lib().lo_measure_peak(device, {"dmma": 0, "dfma": 1, "hbm": 2, "int8_tile_us": 3, "int8_tile_err": 4}[kind], C.byref(v)))
     return v.value
 
 

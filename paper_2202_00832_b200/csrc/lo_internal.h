@@ -284,5 +284,7 @@ lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table
 
 // microbenchmarks (lo_peak.cu)
 lo_status measure_peak(int device, int kind, double* value);
+// gated experiment (lo_int8_probe.cu): FP64-accurate tile from INT8 slices on tcgen05; time per 128 x 128 x 384 tile, error vs fp64
+lo_status measure_int8_slicing(int device, double* us_per_tile, double* max_err);
 
 }  // namespace lo

@@ -94,8 +94,17 @@ lo_status measure_peak(int device, int kind, double* value) {
         }
         cudaFree(a);
         cudaFree(b);
+    } else if (kind == 3 || kind == 4) {
+        // gated experiment, not a roofline denominator: INT8-sliced tile on tcgen05 (3: microseconds per tile, 4: error vs fp64)
+        double us = 0, err = 0;
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+        lo_status st = measure_int8_slicing(device, &us, &err);
+        if (st != LO_OK) return st;
+        *value = kind == 3 ? us : err;
+        return LO_OK;
     } else {
-        set_error("lo_measure_peak: kind must be 0 (DMMA), 1 (DFMA) or 2 (HBM copy)");
+        set_error("lo_measure_peak: kind must be 0 (DMMA), 1 (DFMA), 2 (HBM copy), 3 / 4 (INT8-slicing probe: us per tile / error)");
         return LO_EINVAL;
     }
     cudaEventDestroy(e0);

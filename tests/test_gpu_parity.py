@@ -941,3 +941,17 @@ def test_cas_singular_reference_overlap_is_flagged(c0, smw):
     assert st.tolist() == [0, 0, 1, 0] and np.isnan(E[2]).all()
     ok = [0, 1, 3]
     assert np.array_equal(E[ok], E_ok[ok])
+
+
+def test_int8_slicing_probe_on_tcgen05():
+    """The gated experiment of DESIGN.md 10.1, NOT on the product path: one FP64-accurate 128 x 128 x 384 GEMM
+    tile from 6 x 6 signed 7-bit INT8 slices (21 digit products, tcgen05.mma kind::i8 into TMEM, fp64 recombination).  Checked
+    here: the result agrees with the fp64 product to 1e-10 of max|C| (the emulation predicts ~2e-11), and the tile takes
+    less than 1/1.3 of what the same tile costs on the DMMA pipe at its measured peak (the gate of the experiment)."""
+    torch_cuda()
+    err = lo.measure_peak("int8_tile_err")
+    us = lo.measure_peak("int8_tile_us")
+    dmma_tflops = lo.measure_peak("dmma")
+    dmma_us = 2.0 * 128 * 128 * 384 / (dmma_tflops * 1e12 / 148) * 1e6          # one SM's share of the measured DMMA peak
+    assert err <= 1e-10, err
+    assert us * 1.3 <= dmma_us, (us, dmma_us)
