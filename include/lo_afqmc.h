@@ -66,6 +66,8 @@ typedef struct {
     long long n_pairs_energy_screened; /* pairs dropped by lo_screen_pairs (m_ij sigma_1 <= energy_screen_cutoff) */
     double energy_screen_cutoff;     /* 0 when no energy screen was applied */
     double energy_screen_bound;      /* cK sum over the dropped pairs of m_ij sigma_1: |dE_K| <= this x max_i |Theta_i|^2 */
+    int exchange_mode;               /* LO_EXCHANGE_DMMA / LO_EXCHANGE_INT8 (lo_set_exchange_mode) */
+    unsigned long long int8_bytes;   /* device memory of the INT8 digit slices (0 until LO_EXCHANGE_INT8 was first set) */
 } lo_info;
 
 /* Kernel indices for lo_timing_get */
@@ -166,6 +168,21 @@ lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld);
 #define LO_COULOMB_CHOLESKY 0
 #define LO_COULOMB_COMPRESSED 1
 lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
+
+/* Exchange arithmetic of every later lo_local_energy* call on this (device-resident) factor set.
+ *   LO_EXCHANGE_DMMA (default): a = U Theta_j, b = W Theta_i as FP64 tensor-pipe GEMMs (mma.sync m8n8k4.f64), Eq. 18 as written.
+ *   LO_EXCHANGE_INT8: the same projections from exact INT8 digit slices on the tcgen05 tensor cores (Ozaki-type splitting:
+ *     every row of U, W and Theta^T is scaled by a power of two and cut into 7 signed 7-bit digits; the 28 digit products
+ *     with digit-index sum <= 6 are exact int32 GEMMs accumulated in TMEM; recombination, sigma weights and the a.b
+ *     reduction in fp64).  Not bit-identical to the DMMA route: the projections carry an absolute error of about
+ *     2^-47 |row|_max |Theta row|_max N, E_K agrees to ~1e-12 relative on the BASELINE configs (the parity
+ *     tests hold it to the same 1e-10 as the default).  The first call slices the factor rows once (extra device memory:
+ *     7/8 of the factor bytes + 7 bytes per Theta^T element, lo_info.int8_bytes) and is synchronous; LO_ENOMEM leaves the
+ *     set in LO_EXCHANGE_DMMA mode.  Ignored while LO_COULOMB_COMPRESSED is set and by lo_local_energy_cas.
+ * Host-only factor sets: LO_EINVAL. */
+#define LO_EXCHANGE_DMMA 0
+#define LO_EXCHANGE_INT8 1
+lo_status lo_set_exchange_mode(lo_factors* f, int mode);
 
 /* SURVEY 8(f) NEXT-2, multi-determinant (CAS-type) trial |Psi_T> = sum_d c_d |d> of closed-shell determinants (the
  * same excitation string in both spins), each at most max_exc (<= 8) excitations from the reference:

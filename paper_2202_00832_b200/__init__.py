@@ -20,7 +20,7 @@ LO_SETUP_RANDOMIZED_SVD = 8
 K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "propagator")
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_screen_pairs", "lo_local_energy",
-           "lo_local_energy_host", "lo_set_cas_trial", "lo_set_cas_trial_beta", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
+           "lo_local_energy_host", "lo_set_cas_trial", "lo_set_cas_trial_beta", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_set_exchange_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
            "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
 
 
@@ -38,7 +38,8 @@ class LoInfo(C.Structure):
                 ("setup_on_gpu", C.c_int), ("n_tiles", C.c_longlong), ("svd_sweeps_max", C.c_int), ("svd_offdiag_max", C.c_double),
                 ("setup_seconds", C.c_double), ("setup_svd_seconds", C.c_double), ("rsvd_sketch", C.c_int),
                 ("n_pairs_rsvd", C.c_longlong), ("n_pairs_prescreened", C.c_longlong),
-                ("n_pairs_energy_screened", C.c_longlong), ("energy_screen_cutoff", C.c_double), ("energy_screen_bound", C.c_double)]
+                ("n_pairs_energy_screened", C.c_longlong), ("energy_screen_cutoff", C.c_double), ("energy_screen_bound", C.c_double),
+                ("exchange_mode", C.c_int), ("int8_bytes", C.c_ulonglong)]
 
 
 _lib = None
@@ -63,6 +64,7 @@ def lib():
         L.lo_coulomb_x.argtypes = [vp, C.POINTER(vp), C.POINTER(ci)]
         L.lo_theta_host.argtypes = [vp, ci, ci, vp]
         L.lo_set_coulomb_mode.argtypes = [vp, ci]
+        L.lo_set_exchange_mode.argtypes = [vp, ci]
         L.lo_set_cas_trial.argtypes = [vp, ci, ci, ci, vp, vp, vp, ci, ci]
         L.lo_set_cas_trial_beta.argtypes = [vp, ci, vp, vp]
         L.lo_local_energy_cas.argtypes = [vp, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -304,6 +306,11 @@ class Factors:
     def set_coulomb_mode(self, compressed: bool):
         """lo_set_coulomb_mode: E_J from the compressed pair factors (Eq. 19/22, paper-literal) or the Cholesky route."""
         _check(lib().lo_set_coulomb_mode(self._h, 1 if compressed else 0))
+
+    def set_exchange_mode(self, int8: bool):
+        """lo_set_exchange_mode: exchange projections from INT8 digit slices on the tcgen05 tensor cores (True) or on the FP64
+        tensor pipe (False, the default).  The first switch to INT8 slices the factor rows (synchronous)."""
+        _check(lib().lo_set_exchange_mode(self._h, 1 if int8 else 0))
 
     def propagator(self, x, stream=None):
         """lo_propagator: x = torch CUDA complex128 [n_w, n_chol] (shifted auxiliary fields); forms

@@ -384,6 +384,7 @@ void free_all(lo_factors* f) {
         f->bW.release();
         free_cas_plan(f->cas);
         f->cas = nullptr;
+        free_exchange_i8(f);
         if (f->copyStream) cudaStreamDestroy(f->copyStream);
         for (int c = 0; c < LO_HOST_CHUNKS; ++c)
             if (f->evCopy[c]) cudaEventDestroy(f->evCopy[c]);
@@ -687,6 +688,8 @@ lo_status lo_info_get(const lo_factors* f, lo_info* info) {
     info->n_pairs_prescreened = f->n_prescreened + f->svd_stat.screened;
     info->n_pairs_energy_screened = f->n_energy_screened; info->energy_screen_cutoff = f->energy_cutoff;
     info->energy_screen_bound = f->energy_bound;
+    info->exchange_mode = f->ex_mode;
+    info->int8_bytes = f->i8_bytes;
     return LO_OK;
 }
 
@@ -898,6 +901,17 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode) {
         return LO_EINVAL;
     }
     f->coulomb_lo = mode == LO_COULOMB_COMPRESSED ? 1 : 0;
+    return LO_OK;
+}
+
+lo_status lo_set_exchange_mode(lo_factors* f, int mode) {
+    if (!f || (mode != LO_EXCHANGE_DMMA && mode != LO_EXCHANGE_INT8)) { set_error("lo_set_exchange_mode: invalid argument"); return LO_EINVAL; }
+    if (mode == LO_EXCHANGE_INT8) {
+        if (f->device < 0) { set_error("lo_set_exchange_mode: LO_EXCHANGE_INT8 needs a device-resident factor set"); return LO_EINVAL; }
+        lo_status st = build_exchange_i8(f);      // slices the factor rows on first use
+        if (st != LO_OK) return st;
+    }
+    f->ex_mode = mode;
     return LO_OK;
 }
 

@@ -1,0 +1,450 @@
+// lo_exchange_i8.cu -- the exchange term (Eq. 18 / 19 / 22 exchange part) on the 5th-generation tensor
+// cores: fp64-accurate projections a = U Theta_j, b = W Theta_i from INT8 digit slices (tcgen05.mma kind::i8, int32
+// accumulators in TMEM), the sigma-weighted complex a.b reduction fused into the TMEM read-out.  Opt-in
+// (lo_set_exchange_mode(f, LO_EXCHANGE_INT8)); the default exchange stays the FP64 DMMA kernel k_exchange.
+//
+// Scheme (Ozaki-type splitting).  A row x of an operand is scaled by a power of two, |x| 2^-e <= 1/2,
+// and cut into XI_S = 7 signed digits of 7 bits,  x = 2^e sum_s d_s 2^-(7 s + 6),  |d_s| <= 64  (exact: the remainder after
+// 7 digits is below 2^(e-49)).  Digit matrices are int8, their products are exact in int32 (|sum| <= 7 * N * 2^12), and
+//     a_K[m] = 2^(e_m + e_K) sum_{g <= 6} 2^-(7 g + 12) D_g[m][K],   D_g = sum_{s + t = g} dTheta_s dU_t^T
+// keeps the 28 digit products with s + t <= 6 in 7 accumulators ("groups").  Rows of Theta^T (walker w, re / im) share one
+// exponent per (orbital, walker), so the complex product a_K b_K carries one power of two per walker.
+//
+// Mapping.  M side (TMEM lanes) = 128 walker rows (64 walkers x re/im) of a Theta^T panel, N side (TMEM columns) = the <= 64
+// factor rows of one exchange tile, K = basis index in blocks of 32.  A work item (tile, walker block) runs two phases,
+// a then b, each streaming K once with all 7 groups live in TMEM (7 x 64 = 448 of the 512 columns).  One CTA per SM,
+// 12 warps: warp 0 (one lane) feeds a 5-stage ring with cp.async.bulk copies of pre-tiled slices (Theta: 7 x 4 KB, factor
+// rows: 7 x 2 KB per stage), warp 1 (one lane) issues the MMAs and commits stages / accumulators to mbarriers, warps 4..11
+// read TMEM (lane quadrant = warp % 4, column half = (warp - 4) / 4), recombine in fp64 and, in phase b, multiply straight
+// into the weighted dot with the a values they hold in registers (own row and the re/im partner row), so b is never stored.
+// Per-CTA partial sums are updated in a fixed order by their owning thread: results are bitwise repeatable.
+//
+// Operand slices in HBM, in the shared-memory layout of a K-major, unswizzled tcgen05 operand (core matrix = 8 rows x 16 bytes):
+//   Thq [(o * NBcap + nb)][kb][s][(r/8)*256 + (k/16)*128 + (r%8)*16 + k%16]   r = 2 (w % 64) + c < 128, k < 32   (per call)
+//   Uq, Wq [tile][kb][s][same with r < 64]                                      rows of the tile, zero beyond them   (setup)
+//   thScale [o][w] = 2^e of the Theta rows,  wq [row] = wgt[row] 2^(eU + eW)   (wgt = -cK m_ij sigma_K, lo_internal.h)
+#include <algorithm>
+#include <cstdlib>
+
+#include "lo_device.cuh"
+
+namespace lo {
+namespace {
+
+constexpr int XI_S = 7;                          // digits per operand
+constexpr int XI_TH_BLK = 128 * 32;              // bytes of one (digit, K block) of a Theta walker block
+constexpr int XI_F_BLK = 64 * 32;                // ... of the factor rows of a tile
+constexpr int XI_TH_STAGE = XI_S * XI_TH_BLK, XI_F_STAGE = XI_S * XI_F_BLK;
+constexpr int XI_STAGE = XI_TH_STAGE + XI_F_STAGE;          // 43008 bytes
+constexpr int XI_STAGES = 5;
+constexpr int XI_SMEM = XI_STAGES * XI_STAGE + 1024;
+constexpr int XI_TMEM_COLS = 512;                // 7 groups x 64 columns = 448, allocation sizes are powers of two
+
+// ---- slicing ---------------------------------------------------------------------------------------------------------
+// 16 consecutive k of one row -> one 16-byte chunk per digit
+__device__ __forceinline__ void slice16(const double* __restrict__ src, double inv, int4 (&out)[XI_S]) {
+    double res[16];
+#pragma unroll
+    for (int i = 0; i < 16; i += 2) {
+        const double2 v = *reinterpret_cast<const double2*>(src + i);
+        res[i] = v.x * inv;
+        res[i + 1] = v.y * inv;
+    }
+#pragma unroll
+    for (int s = 0; s < XI_S; ++s) {
+        const double up = exp2(7.0 * s + 6.0), dn = exp2(-(7.0 * s + 6.0));
+        int w[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            unsigned pk = 0;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const double d = rint(res[4 * q + b] * up);
+                res[4 * q + b] = fma(-d, dn, res[4 * q + b]);          // exact
+                pk |= ((unsigned)(int)d & 0xFFu) << (8 * b);
+            }
+            w[q] = (int)pk;
+        }
+        out[s] = make_int4(w[0], w[1], w[2], w[3]);
+    }
+}
+
+__device__ __forceinline__ int row_exponent(double mx) {
+    // |x| 2^-e <= 1/2 for every |x| <= mx;  rows of zeros and rows holding Inf / NaN (singular walkers, set to NaN by
+    // k_finalize) get e = 0
+    return (mx > 0.0 && mx < 1e300) ? ilogb(mx) + 2 : 0;
+}
+
+// Theta^T panels -> Thq, thScale.  One warp per (orbital, walker): both rows (re, im) share the exponent.
+__global__ void __launch_bounds__(256) k_slice_theta(const double* __restrict__ thT, int8_t* __restrict__ Thq, double* __restrict__ thScale,
+                                                     int O_tot, int ldw, int N_pad, int KB, int NBcap, int Wcap, int n_wpad) {
+    const int lane = threadIdx.x & 31;
+    const long long gw = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int o = (int)(gw / n_wpad), w = (int)(gw % n_wpad);
+    if (o >= O_tot) return;
+    const double* r0 = thT + ((size_t)o * ldw + 2 * w) * N_pad;
+    double mx = 0.0;
+    bool bad = false;
+    for (int i = lane; i < 2 * N_pad; i += 32) {
+        const double a = fabs(r0[i]);
+        bad |= !(a < 1e300);
+        mx = fmax(mx, a);
+    }
+#pragma unroll
+    for (int d = 16; d; d >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+    bad = __any_sync(0xffffffffu, bad);
+    const int e = bad ? 0 : row_exponent(mx);
+    const double inv = bad ? 0.0 : scalbn(1.0, -e);
+    if (lane == 0) thScale[(size_t)o * Wcap + w] = scalbn(1.0, e);
+    const int nch = 2 * KB;                                   // 16-wide chunks per row
+    int8_t* blk = Thq + (size_t)(o * NBcap + w / 64) * KB * XI_TH_STAGE;
+    for (int task = lane; task < 2 * nch; task += 32) {
+        const int c = task / nch, ch = task % nch, k0 = ch * 16, r = 2 * (w % 64) + c;
+        int4 out[XI_S];
+        if (k0 < N_pad && !bad) slice16(r0 + (size_t)c * N_pad + k0, inv, out);
+        else {
+#pragma unroll
+            for (int s = 0; s < XI_S; ++s) out[s] = make_int4(0, 0, 0, 0);
+        }
+        int8_t* dst = blk + (size_t)(ch >> 1) * XI_TH_STAGE + (r >> 3) * 256 + (ch & 1) * 128 + (r & 7) * 16;
+#pragma unroll
+        for (int s = 0; s < XI_S; ++s) *reinterpret_cast<int4*>(dst + s * XI_TH_BLK) = out[s];
+    }
+}
+
+// Factor rows -> Uq / Wq and their exponents.  grid = tiles, 8 warps; warp v handles rows v, v + 8, ... of the tile.
+__global__ void __launch_bounds__(256) k_slice_factors(const double* __restrict__ F, const ExTile* __restrict__ tiles, int8_t* __restrict__ Fq,
+                                                       int* __restrict__ eF, int N_pad, int KB) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const ExTile tile = tiles[blockIdx.x];
+    const int nch = 2 * KB;
+    int8_t* blk = Fq + (size_t)blockIdx.x * KB * XI_F_STAGE;
+    for (int r = warp; r < 64; r += 8) {
+        const bool live = r < tile.nfrag * 8;
+        const double* src = F + (size_t)(tile.row0 + (live ? r : 0)) * N_pad;
+        double mx = 0.0;
+        if (live)
+            for (int i = lane; i < N_pad; i += 32) mx = fmax(mx, fabs(src[i]));
+#pragma unroll
+        for (int d = 16; d; d >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        const int e = row_exponent(mx);
+        const double inv = scalbn(1.0, -e);
+        if (live && lane == 0) eF[tile.row0 + r] = e;
+        for (int ch = lane; ch < nch; ch += 32) {
+            const int k0 = ch * 16;
+            int4 out[XI_S];
+            if (live && k0 < N_pad) slice16(src + k0, inv, out);
+            else {
+#pragma unroll
+                for (int s = 0; s < XI_S; ++s) out[s] = make_int4(0, 0, 0, 0);
+            }
+            int8_t* dst = blk + (size_t)(ch >> 1) * XI_F_STAGE + (r >> 3) * 256 + (ch & 1) * 128 + (r & 7) * 16;
+#pragma unroll
+            for (int s = 0; s < XI_S; ++s) *reinterpret_cast<int4*>(dst + s * XI_F_BLK) = out[s];
+        }
+    }
+}
+
+__global__ void k_i8_weights(const double* __restrict__ wgt, const int* __restrict__ eU, const int* __restrict__ eW, double* __restrict__ wq,
+                             long long rows) {
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < rows) wq[r] = scalbn(wgt[r], eU[r] + eW[r]);
+}
+
+// ---- the exchange kernel ---------------------------------------------------------------------------------------------
+// shared-memory matrix descriptor, K-major, no swizzle: rows 16 bytes apart inside a core matrix, LBO = distance of the two
+// 16-byte K halves, SBO = distance of consecutive 8-row groups; descriptor version 1 (sm_100)
+__device__ __forceinline__ uint64_t xi_desc(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(128u >> 4) << 16) | ((uint64_t)(256u >> 4) << 32) | (1ull << 46);
+}
+// every wait is bounded: a pipeline bug must end in an error code, not in a hung GPU
+__device__ __forceinline__ bool xi_wait(uint32_t bar, uint32_t parity) {
+    for (int spin = 0; spin < (1 << 24); ++spin) {
+        uint32_t ok;
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return true;
+    }
+    return false;
+}
+__device__ __forceinline__ void xi_bulk(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void xi_ld32(uint32_t taddr, int (&v)[32]) {
+#pragma unroll
+    for (int c0 = 0; c0 < 32; c0 += 16)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(v[c0]), "=r"(v[c0 + 1]), "=r"(v[c0 + 2]), "=r"(v[c0 + 3]), "=r"(v[c0 + 4]), "=r"(v[c0 + 5]), "=r"(v[c0 + 6]),
+                       "=r"(v[c0 + 7]), "=r"(v[c0 + 8]), "=r"(v[c0 + 9]), "=r"(v[c0 + 10]), "=r"(v[c0 + 11]), "=r"(v[c0 + 12]),
+                       "=r"(v[c0 + 13]), "=r"(v[c0 + 14]), "=r"(v[c0 + 15])
+                     : "r"(taddr + c0));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+// int32 -> fp64 without I2F: 2^52 + (v + 2^31) is exact in the low mantissa word
+__device__ __forceinline__ double xi_pow2(int e) { return __hiloint2double((1023 + e) << 20, 0); }
+__device__ __forceinline__ double xi_i2d(int v) { return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0; }
+
+__global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict__ Uq, const int8_t* __restrict__ Wq, const int8_t* __restrict__ Thq,
+                                                        const double* __restrict__ wq, const double* __restrict__ thScale,
+                                                        const ExTile* __restrict__ tiles, long long n_items, int NB, int NBcap, int KB, int Wcap,
+                                                        double* __restrict__ ekpart, int* __restrict__ fail) {
+    extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) unsigned long long bar_s[2 * XI_STAGES + 2];      // full[], empty[], acc_full, acc_empty
+    __shared__ uint32_t tmem_base_s;
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t full = smem_u32(&bar_s[0]), empty = full + 8 * XI_STAGES, acc_full = empty + 8 * XI_STAGES, acc_empty = acc_full + 8;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // partial sums: two rows per CTA (one per column half of the epilogue warps), zeroed here, updated by their owners only
+    for (int i = tid; i < 4 * Wcap; i += 384) ekpart[(size_t)blockIdx.x * 4 * Wcap + i] = 0.0;
+    if (tid == 0) {
+        for (int i = 0; i < XI_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 1); }
+        mbar_init(acc_full, 1);
+        mbar_init(acc_empty, 8);            // one arrival per epilogue warp
+        fence_barrier_init();
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"((uint32_t)XI_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = tmem_base_s;
+    const long long my_items = n_items > (long long)blockIdx.x ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    bool ok = true;
+    if (warp < 4) {
+        reg_dec_producer();
+        if (warp == 0 && lane == 0) {
+            // ===== feed: per item two phases (a: U with Theta_pj, b: W with Theta_pi), per phase KB stages
+            int slot = 0;
+            uint32_t phase = 0;
+            for (long long it = 0; it < my_items && ok; ++it) {
+                const long long q = blockIdx.x + it * gridDim.x;
+                const int tile_idx = (int)(q / NB), nb = (int)(q % NB);
+                const ExTile tile = tiles[tile_idx];
+                for (int ph = 0; ph < 2 && ok; ++ph) {
+                    const int8_t* th = Thq + (size_t)((ph ? tile.pi : tile.pj) * NBcap + nb) * KB * XI_TH_STAGE;
+                    const int8_t* fq = (ph ? Wq : Uq) + (size_t)tile_idx * KB * XI_F_STAGE;
+                    for (int kb = 0; kb < KB; ++kb) {
+                        ok = xi_wait(empty + 8 * slot, phase ^ 1);
+                        if (!ok) break;
+                        const uint32_t st = sbase + slot * XI_STAGE, bar = full + 8 * slot;
+                        mbar_expect_tx(bar, XI_STAGE);
+                        xi_bulk(st, th + (size_t)kb * XI_TH_STAGE, XI_TH_STAGE, bar);
+                        xi_bulk(st + XI_TH_STAGE, fq + (size_t)kb * XI_F_STAGE, XI_F_STAGE, bar);
+                        if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
+                    }
+                }
+            }
+            if (!ok) atomicExch(fail, 1);
+        } else if (warp == 1 && lane == 0) {
+            // ===== MMA issue: 28 digit products per K block, group g = s + t accumulates in TMEM columns [64 g, 64 g + N)
+            int slot = 0;
+            uint32_t phase = 0, pe = 1;             // the accumulators start out free
+            for (long long it = 0; it < my_items && ok; ++it) {
+                const long long q = blockIdx.x + it * gridDim.x;
+                const ExTile tile = tiles[(int)(q / NB)];
+                const uint32_t Nmma = (uint32_t)((tile.nfrag * 8 + 15) / 16) * 16;
+                // instruction descriptor: D = S32 (2 << 4), A = B = signed 8 bit (1 << 7, 1 << 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+                const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((Nmma >> 3) << 17) | ((128u >> 4) << 24);
+                for (int ph = 0; ph < 2 && ok; ++ph) {
+                    ok = xi_wait(acc_empty, pe);
+                    if (!ok) break;
+                    pe ^= 1;
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    for (int kb = 0; kb < KB; ++kb) {
+                        ok = xi_wait(full + 8 * slot, phase);
+                        if (!ok) break;
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        const uint32_t st = sbase + slot * XI_STAGE;
+#pragma unroll
+                        for (int s = 0; s < XI_S; ++s) {
+                            const uint64_t da = xi_desc(st + s * XI_TH_BLK);
+                            const uint32_t accum = (kb == 0 && s == 0) ? 0u : 1u;
+#pragma unroll
+                            for (int t = 0; t < XI_S - s; ++t) {
+                                const uint64_t db = xi_desc(st + XI_TH_STAGE + t * XI_F_BLK);
+                                asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }"
+                                             ::"r"(tmem + (uint32_t)(s + t) * 64), "l"(da), "l"(db), "r"(idesc), "r"(accum) : "memory");
+                            }
+                        }
+                        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(empty + 8 * slot) : "memory");
+                        if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(acc_full) : "memory");
+                }
+            }
+            if (!ok) atomicExch(fail, 1);
+        }
+    } else {
+        // ===== epilogue: lane quadrant warp % 4 (walker rows 32 quad .. + 31), column half (warp - 4) / 4 (factor rows 32 half .. + 31)
+        reg_inc_consumer();
+        const int quad = warp & 3, half = (warp - 4) >> 2;
+        const int m = quad * 32 + lane, wl = m >> 1, c = m & 1;       // row of the walker block = 2 wl + c
+        const uint32_t tbase = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)half * 32;
+        double2* mypart = reinterpret_cast<double2*>(ekpart) + (size_t)(2 * blockIdx.x + half) * Wcap;
+        uint32_t pf = 0;
+        for (long long it = 0; it < my_items && ok; ++it) {
+            const long long q = blockIdx.x + it * gridDim.x;
+            const int tile_idx = (int)(q / NB), nb = (int)(q % NB);
+            const ExTile tile = tiles[tile_idx];
+            const int w = nb * 64 + wl, nrow = tile.nfrag * 8 - half * 32;      // live columns of this thread: [0, nrow)
+            double a[32], an[32];
+            // ---- phase a: recombine, weight, fetch the re/im partner row
+            ok = xi_wait(acc_full, pf);
+            ok = __all_sync(0xffffffffu, ok);
+            if (!ok) break;
+            pf ^= 1;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < 32; ++j) a[j] = 0.0;
+#pragma unroll 1
+            for (int g = 0; g < XI_S; ++g) {
+                int v[32];
+                xi_ld32(tbase + (uint32_t)g * 64, v);
+                const double sc = xi_pow2(-(7 * g + 12));
+#pragma unroll
+                for (int j = 0; j < 32; ++j) a[j] = fma(xi_i2d(v[j]), sc, a[j]);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(acc_empty);
+            const double* wrow = wq + tile.row0 + half * 32;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+                a[j] = j < nrow ? a[j] * __ldg(wrow + j) : 0.0;           // columns beyond the tile were never written
+                an[j] = __shfl_xor_sync(0xffffffffu, a[j], 1);
+            }
+            // ---- phase b: p1 = sum a_own b_own, p2 = sum a_partner b_own
+            ok = xi_wait(acc_full, pf);
+            ok = __all_sync(0xffffffffu, ok);
+            if (!ok) break;
+            pf ^= 1;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            double p1 = 0.0, p2 = 0.0;
+#pragma unroll 1
+            for (int g = 0; g < XI_S; ++g) {
+                int v[32];
+                xi_ld32(tbase + (uint32_t)g * 64, v);
+                double q1 = 0.0, q2 = 0.0;
+#pragma unroll
+                for (int j = 0; j < 32; ++j) {
+                    const double b = xi_i2d(v[j]);
+                    q1 = fma(a[j], b, q1);
+                    q2 = fma(an[j], b, q2);
+                }
+                const double sc = xi_pow2(-(7 * g + 12));
+                p1 = fma(q1, sc, p1);
+                p2 = fma(q2, sc, p2);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(acc_empty);
+            // row re (c = 0): p1 = sum a_re b_re, p2 = sum a_im b_re;  row im: p1 = sum a_im b_im, p2 = sum a_re b_im
+            const double sw = thScale[(size_t)tile.pj * Wcap + w] * thScale[(size_t)tile.pi * Wcap + w];
+            const double o1 = __shfl_xor_sync(0xffffffffu, p1, 1), o2 = __shfl_xor_sync(0xffffffffu, p2, 1);
+            if (c == 0) {
+                double2 prev = mypart[w];
+                prev.x = fma(sw, p1 - o1, prev.x);
+                prev.y = fma(sw, p2 + o2, prev.y);
+                mypart[w] = prev;
+            }
+        }
+        if (!ok && lane == 0) atomicExch(fail, 1);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)XI_TMEM_COLS) : "memory");
+}
+
+// a bounded wait expired somewhere: poison the partial sums so that every energy of the call comes out NaN
+__global__ void k_i8_poison(const int* __restrict__ fail, double* __restrict__ ekpart, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (*fail && i < n) ekpart[i] = __longlong_as_double(0x7ff8000000000000LL);
+}
+
+}  // namespace
+
+void free_exchange_i8(lo_factors* f) {
+    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dI8Fail};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    f->dUq = f->dWq = f->dThq = nullptr;
+    f->dWgtQ = f->dThScale = f->dEKq = nullptr;
+    f->dI8Fail = nullptr;
+    f->i8_bytes = 0;
+}
+
+// Slices the packed factor rows once (Uq, Wq, wq) and allocates the per-call buffers (Thq, thScale, partial sums).
+lo_status build_exchange_i8(lo_factors* f) {
+#define CK(call)                                                                                                         \
+    do {                                                                                                                 \
+        cudaError_t e_ = (call);                                                                                         \
+        if (e_ != cudaSuccess) {                                                                                         \
+            set_error(std::string("lo_set_exchange_mode: ") + #call + ": " + cudaGetErrorString(e_));                    \
+            free_exchange_i8(f);                                                                                         \
+            return e_ == cudaErrorMemoryAllocation ? LO_ENOMEM : LO_ECUDA;                                               \
+        }                                                                                                                \
+    } while (0)
+    if (f->dUq) return LO_OK;
+    CK(cudaSetDevice(f->device));
+    static bool configured = false;
+    if (!configured) {
+        CK(cudaFuncSetAttribute(k_exchange_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
+        configured = true;
+    }
+    const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64;
+    const size_t fq_bytes = (size_t)std::max<long long>(f->n_tiles, 1) * KB * XI_F_STAGE;
+    const size_t th_bytes = (size_t)f->O_tot * NBcap * KB * XI_TH_STAGE;
+    const long long rows_al = f->rows + 64;
+    int *eU = nullptr, *eW = nullptr;
+    CK(cudaMalloc(&f->dUq, fq_bytes));
+    CK(cudaMalloc(&f->dWq, fq_bytes));
+    CK(cudaMalloc(&f->dThq, th_bytes));
+    CK(cudaMalloc(&f->dWgtQ, (size_t)rows_al * 8));
+    CK(cudaMalloc(&f->dThScale, (size_t)f->O_tot * f->Wcap * 8));
+    CK(cudaMalloc(&f->dEKq, (size_t)2 * f->num_sms * f->Wcap * 16));
+    CK(cudaMalloc(&f->dI8Fail, 4));
+    CK(cudaMemset(f->dI8Fail, 0, 4));
+    CK(cudaMemset(f->dWgtQ, 0, (size_t)rows_al * 8));
+    CK(cudaMemset(f->dThq, 0, th_bytes));
+    f->i8_bytes = 2 * fq_bytes + th_bytes + (size_t)rows_al * 8;
+    if (f->n_tiles > 0) {
+        cudaError_t e1 = cudaMalloc(&eU, (size_t)rows_al * 4), e2 = cudaMalloc(&eW, (size_t)rows_al * 4);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) {
+            cudaFree(eU); cudaFree(eW);
+            (void)cudaGetLastError();
+            free_exchange_i8(f);
+            set_error("lo_set_exchange_mode: out of device memory for the slicing scratch");
+            return LO_ENOMEM;
+        }
+        cudaMemset(eU, 0, (size_t)rows_al * 4);
+        cudaMemset(eW, 0, (size_t)rows_al * 4);
+        k_slice_factors<<<(unsigned)f->n_tiles, 256>>>(f->dU, f->dTiles, f->dUq, eU, f->N_pad, KB);
+        k_slice_factors<<<(unsigned)f->n_tiles, 256>>>(f->dW, f->dTiles, f->dWq, eW, f->N_pad, KB);
+        k_i8_weights<<<(unsigned)((f->rows + 255) / 256), 256>>>(f->dWgt, eU, eW, f->dWgtQ, f->rows);
+        cudaError_t e = cudaDeviceSynchronize();
+        cudaFree(eU); cudaFree(eW);
+        CK(e);
+    }
+    return LO_OK;
+#undef CK
+}
+
+// S4 in LO_EXCHANGE_INT8 mode: slice the Theta^T panels of this call, run the exchange on the tensor cores; the partial sums
+// land in f->dEKq as 2 * grid rows (*n_part) for k_finalize.
+void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part) {
+    const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64, NB = (n_w + 63) / 64, n_wpad = NB * 64;
+    const long long warps = (long long)f->O_tot * n_wpad;
+    k_slice_theta<<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(f->dThT, f->dThq, f->dThScale, f->O_tot, f->ldw, f->N_pad, KB, NBcap, f->Wcap, n_wpad);
+    const long long items = f->n_tiles * NB;
+    const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
+    k_exchange_i8<<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,
+                                                  f->dI8Fail);
+    const int n = grid * 4 * f->Wcap;
+    k_i8_poison<<<(n + 255) / 256, 256, 0, stream>>>(f->dI8Fail, f->dEKq, n);
+    *part = f->dEKq;
+    *n_part = 2 * grid;
+}
+
+}  // namespace lo

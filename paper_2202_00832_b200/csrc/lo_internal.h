@@ -209,6 +209,15 @@ struct lo_factors {
     unsigned long long factor_bytes = 0, lbar_bytes = 0, workspace_bytes = 0;
     int last_n_w = 0;
     lo::CasPlan* cas = nullptr;
+    // exchange on the tcgen05 tensor cores from INT8 digit slices (lo_set_exchange_mode, lo_exchange_i8.cu)
+    int ex_mode = 0;                       // LO_EXCHANGE_DMMA / LO_EXCHANGE_INT8
+    int8_t *dUq = nullptr, *dWq = nullptr; // [n_tiles][KB][7][64 x 32] digit slices of the factor rows
+    int8_t* dThq = nullptr;                // [O_tot * Wcap/64][KB][7][128 x 32] digit slices of Theta^T, rewritten every call
+    double* dWgtQ = nullptr;               // [rows + 64] wgt * 2^(eU + eW)
+    double* dThScale = nullptr;            // [O_tot][Wcap] 2^e of the Theta rows
+    double* dEKq = nullptr;                // [2 * num_sms][Wcap] complex partial sums
+    int* dI8Fail = nullptr;
+    unsigned long long i8_bytes = 0;
     // timing
     bool timing = false;
     std::vector<lo::TimingEvent> events;
@@ -281,6 +290,11 @@ lo_status gpu_pair_rsvd(const lo_factors* f, int spin, const int* pi, const int*
 bool host_pair_rsvd(int N, int k, const double* G, std::vector<double>& sigma, std::vector<double>& U, std::vector<double>& W, SvdStat* stat);
 // dst[rec.dst_row + K][:] = src[rec.src_row + K][:] for K < rec.r, every rec of the host table (rows of N_pad doubles).
 lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table, int n, int N_pad);
+
+// exchange from INT8 digit slices on tcgen05 (lo_exchange_i8.cu)
+lo_status build_exchange_i8(lo_factors* f);
+void free_exchange_i8(lo_factors* f);
+void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part);
 
 // microbenchmarks (lo_peak.cu)
 lo_status measure_peak(int device, int kind, double* value);

@@ -1247,6 +1247,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
     double2* E1raw = EJpart + (size_t)RB * Wcap;
     // ---- S4
     int ex_grid = 0;
+    const double* ek_part = f->dEKpart;
     {
         Timer tm(f, stream, LO_K_EXCHANGE);
         const bool coul = f->coulomb_lo != 0;
@@ -1255,7 +1256,10 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         const bool ragged = n_w % WALKER_TILE != 0;
         // small problems: static LPT schedule of the tiles (grid = all SMs); large ones: round robin in L2-block order
         const ExItems rr = {nullptr, nullptr}, lpt = {f->dSchedOff, f->dSchedTile};
-        if (!coul && n_w <= 32) {
+        if (!coul && f->ex_mode == LO_EXCHANGE_INT8) {
+            // fp64-accurate projections from INT8 digit slices on the tcgen05 tensor cores (lo_exchange_i8.cu)
+            launch_exchange_i8(f, n_w, stream, &ek_part, &ex_grid);
+        } else if (!coul && n_w <= 32) {
             // narrow batch: 16-walker column blocks, row fragments split over the warps
             const int NB16 = (n_w + 15) / 16;
             items = f->n_tiles * NB16;
@@ -1282,7 +1286,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
     {
         Timer tm(f, stream, LO_K_FINAL);
         const double c1 = f->n_spin == 1 ? 2.0 : 1.0, cJ = f->n_spin == 1 ? 2.0 : 0.5;
-        k_finalize<<<(n_w + 127) / 128, 128, 0, stream>>>(EJpart, RB, E1raw, (const double2*)f->dEKpart, ex_grid, f->dStatus, f->n_spin, Wcap,
+        k_finalize<<<(n_w + 127) / 128, 128, 0, stream>>>(EJpart, RB, E1raw, (const double2*)ek_part, ex_grid, f->dStatus, f->n_spin, Wcap,
                                                           n_w, c1, cJ, (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K,
                                                           walker_status, (double2*)Eout4,
                                                           f->coulomb_lo ? (const double2*)f->dEJLpart : nullptr);
