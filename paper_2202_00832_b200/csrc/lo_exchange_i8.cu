@@ -38,6 +38,7 @@ constexpr int XI_TH_STAGE = XI_S * XI_TH_BLK, XI_F_STAGE = XI_S * XI_F_BLK;
 constexpr int XI_STAGE = XI_TH_STAGE + XI_F_STAGE;          // 43008 bytes
 constexpr int XI_STAGES = 5;
 constexpr int XI_SMEM = XI_STAGES * XI_STAGE + 1024;
+constexpr int XI_CAT = 4;                        // factor digits covered by one MMA (N <= 256)
 constexpr int XI_TMEM_COLS = 512;                // 7 groups x 64 columns = 448, allocation sizes are powers of two
 
 // ---- slicing ---------------------------------------------------------------------------------------------------------
@@ -187,7 +188,7 @@ __device__ __forceinline__ double xi_i2d(int v) { return __hiloint2double(0x4330
 __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict__ Uq, const int8_t* __restrict__ Wq, const int8_t* __restrict__ Thq,
                                                         const double* __restrict__ wq, const double* __restrict__ thScale,
                                                         const ExTile* __restrict__ tiles, long long n_items, int NB, int NBcap, int KB, int Wcap,
-                                                        double* __restrict__ ekpart, int* __restrict__ fail) {
+                                                        double* __restrict__ ekpart, int* __restrict__ fail, int dbg) {
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bar_s[2 * XI_STAGES + 2];      // full[], empty[], acc_full, acc_empty
     __shared__ uint32_t tmem_base_s;
@@ -229,9 +230,12 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                         ok = xi_wait(empty + 8 * slot, phase ^ 1);
                         if (!ok) break;
                         const uint32_t st = sbase + slot * XI_STAGE, bar = full + 8 * slot;
+                        if (dbg & 2) { mbar_arrive(bar); }
+                        else {
                         mbar_expect_tx(bar, XI_STAGE);
                         xi_bulk(st, th + (size_t)kb * XI_TH_STAGE, XI_TH_STAGE, bar);
                         xi_bulk(st + XI_TH_STAGE, fq + (size_t)kb * XI_F_STAGE, XI_F_STAGE, bar);
+                        }
                         if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
                     }
                 }
@@ -246,7 +250,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                 const ExTile tile = tiles[(int)(q / NB)];
                 const uint32_t Nmma = (uint32_t)((tile.nfrag * 8 + 15) / 16) * 16;
                 // instruction descriptor: D = S32 (2 << 4), A = B = signed 8 bit (1 << 7, 1 << 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
-                const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((Nmma >> 3) << 17) | ((128u >> 4) << 24);
+                const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((128u >> 4) << 24);
                 for (int ph = 0; ph < 2 && ok; ++ph) {
                     ok = xi_wait(acc_empty, pe);
                     if (!ok) break;
@@ -257,15 +261,24 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                         if (!ok) break;
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t st = sbase + slot * XI_STAGE;
+                        if (!(dbg & 1)) {
+                            // Theta digit s against the factor digits t = 0 .. 6 - s.  The digit blocks of the factor rows lie one behind the
+                            // other in the stage (64 rows each) and group s + t owns TMEM columns [64 (s + t), + 64), so ONE instruction
+                            // with N = 64 cnt covers cnt consecutive t: its B operand is "rows" t0*64 .. of the stacked digit blocks, its
+                            // accumulator the cnt adjacent groups.  (kind::i8 instructions below N = 128 run at the N = 128 rate.)
 #pragma unroll
-                        for (int s = 0; s < XI_S; ++s) {
-                            const uint64_t da = xi_desc(st + s * XI_TH_BLK);
-                            const uint32_t accum = (kb == 0 && s == 0) ? 0u : 1u;
+                            for (int s = 0; s < XI_S; ++s) {
+                                const uint64_t da = xi_desc(st + s * XI_TH_BLK);
+                                const uint32_t accum = (kb == 0 && s == 0) ? 0u : 1u;
 #pragma unroll
-                            for (int t = 0; t < XI_S - s; ++t) {
-                                const uint64_t db = xi_desc(st + XI_TH_STAGE + t * XI_F_BLK);
-                                asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }"
-                                             ::"r"(tmem + (uint32_t)(s + t) * 64), "l"(da), "l"(db), "r"(idesc), "r"(accum) : "memory");
+                                for (int t0 = 0; t0 < XI_S - s; t0 += XI_CAT) {
+                                    const int cnt = (XI_S - s - t0) < XI_CAT ? (XI_S - s - t0) : XI_CAT;
+                                    const uint32_t Ni = (dbg & 4) ? 64u * cnt : 64u * (cnt - 1) + Nmma;
+                                    const uint32_t id = idesc | ((Ni >> 3) << 17);
+                                    const uint64_t db = xi_desc(st + XI_TH_STAGE + t0 * XI_F_BLK);
+                                    asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }"
+                                                 ::"r"(tmem + (uint32_t)(s + t0) * 64), "l"(da), "l"(db), "r"(id), "r"(accum) : "memory");
+                                }
                             }
                         }
                         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(empty + 8 * slot) : "memory");
@@ -440,7 +453,7 @@ void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const doubl
     const long long items = f->n_tiles * NB;
     const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
     k_exchange_i8<<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,
-                                                  f->dI8Fail);
+                                                  f->dI8Fail, getenv("LO_I8_DBG") ? atoi(getenv("LO_I8_DBG")) : 0);
     const int n = grid * 4 * f->Wcap;
     k_i8_poison<<<(n + 255) / 256, 256, 0, stream>>>(f->dI8Fail, f->dEKq, n);
     *part = f->dEKq;
