@@ -185,10 +185,68 @@ __device__ __forceinline__ void xi_ld32(uint32_t taddr, int (&v)[32]) {
 __device__ __forceinline__ double xi_pow2(int e) { return __hiloint2double((1023 + e) << 20, 0); }
 __device__ __forceinline__ double xi_i2d(int v) { return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0; }
 
+__device__ __forceinline__ void xi_ld16(uint32_t taddr, int (&v)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+                   "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr));
+}
+// the registers of the load are operands of the wait, so that nothing that reads them can be scheduled above it
+__device__ __forceinline__ void xi_ld_wait(int (&v)[16]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]), "+r"(v[8]), "+r"(v[9]),
+                   "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15])
+                 :: "memory");
+}
+// Read-out of the 7 accumulator groups of this thread's row (32 columns each, 16 at a time, the next load in flight while
+// the current one is consumed).  PHASE_B = false: a[j] = sum_g 2^-(7g+12) D_g[j].  PHASE_B = true: p1 += sum_j a[j] b[j],
+// p2 += sum_j an[j] b[j] with b recombined on the fly (linear in the groups), b itself is never stored.
+template <bool PHASE_B>
+__device__ __forceinline__ void xi_readout(uint32_t tbase, double (&a)[32], const double (&an)[32], double& p1, double& p2) {
+    int v0[16], v1[16];
+    xi_ld16(tbase, v0);
+    xi_ld_wait(v0);
+#pragma unroll
+    for (int g = 0; g < XI_S; ++g) {
+        const double sc = xi_pow2(-(7 * g + 12));
+        double q1a = 0.0, q1b = 0.0, q2a = 0.0, q2b = 0.0;
+        xi_ld16(tbase + (uint32_t)g * 64 + 16, v1);
+#pragma unroll
+        for (int j = 0; j < 16; j += 2) {
+            const double b0 = xi_i2d(v0[j]), b1 = xi_i2d(v0[j + 1]);
+            if constexpr (PHASE_B) {
+                q1a = fma(a[j], b0, q1a); q1b = fma(a[j + 1], b1, q1b);
+                q2a = fma(an[j], b0, q2a); q2b = fma(an[j + 1], b1, q2b);
+            } else {
+                a[j] = g ? fma(b0, sc, a[j]) : b0 * sc;
+                a[j + 1] = g ? fma(b1, sc, a[j + 1]) : b1 * sc;
+            }
+        }
+        xi_ld_wait(v1);
+        if (g + 1 < XI_S) xi_ld16(tbase + (uint32_t)(g + 1) * 64, v0);
+#pragma unroll
+        for (int j = 0; j < 16; j += 2) {
+            const double b0 = xi_i2d(v1[j]), b1 = xi_i2d(v1[j + 1]);
+            if constexpr (PHASE_B) {
+                q1a = fma(a[16 + j], b0, q1a); q1b = fma(a[17 + j], b1, q1b);
+                q2a = fma(an[16 + j], b0, q2a); q2b = fma(an[17 + j], b1, q2b);
+            } else {
+                a[16 + j] = g ? fma(b0, sc, a[16 + j]) : b0 * sc;
+                a[17 + j] = g ? fma(b1, sc, a[17 + j]) : b1 * sc;
+            }
+        }
+        if (g + 1 < XI_S) xi_ld_wait(v0);
+        if constexpr (PHASE_B) {
+            p1 = fma(q1a + q1b, sc, p1);
+            p2 = fma(q2a + q2b, sc, p2);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict__ Uq, const int8_t* __restrict__ Wq, const int8_t* __restrict__ Thq,
                                                         const double* __restrict__ wq, const double* __restrict__ thScale,
                                                         const ExTile* __restrict__ tiles, long long n_items, int NB, int NBcap, int KB, int Wcap,
-                                                        double* __restrict__ ekpart, int* __restrict__ fail, int dbg) {
+                                                        double* __restrict__ ekpart, int* __restrict__ fail) {
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bar_s[2 * XI_STAGES + 2];      // full[], empty[], acc_full, acc_empty
     __shared__ uint32_t tmem_base_s;
@@ -223,6 +281,15 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                 const long long q = blockIdx.x + it * gridDim.x;
                 const int tile_idx = (int)(q / NB), nb = (int)(q % NB);
                 const ExTile tile = tiles[tile_idx];
+                if (it + 1 < my_items) {
+                    // the factor digits of the next item come from HBM (every tile is read by NB CTAs at about the same time, once
+                    // per call): ask L2 for them one item ahead
+                    const size_t nxt = (size_t)((q + gridDim.x) / NB) * KB * XI_F_STAGE;
+                    for (int kb = 0; kb < KB; ++kb) {
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(Uq + nxt + (size_t)kb * XI_F_STAGE), "r"((uint32_t)XI_F_STAGE) : "memory");
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(Wq + nxt + (size_t)kb * XI_F_STAGE), "r"((uint32_t)XI_F_STAGE) : "memory");
+                    }
+                }
                 for (int ph = 0; ph < 2 && ok; ++ph) {
                     const int8_t* th = Thq + (size_t)((ph ? tile.pi : tile.pj) * NBcap + nb) * KB * XI_TH_STAGE;
                     const int8_t* fq = (ph ? Wq : Uq) + (size_t)tile_idx * KB * XI_F_STAGE;
@@ -230,12 +297,9 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                         ok = xi_wait(empty + 8 * slot, phase ^ 1);
                         if (!ok) break;
                         const uint32_t st = sbase + slot * XI_STAGE, bar = full + 8 * slot;
-                        if (dbg & 2) { mbar_arrive(bar); }
-                        else {
                         mbar_expect_tx(bar, XI_STAGE);
                         xi_bulk(st, th + (size_t)kb * XI_TH_STAGE, XI_TH_STAGE, bar);
                         xi_bulk(st + XI_TH_STAGE, fq + (size_t)kb * XI_F_STAGE, XI_F_STAGE, bar);
-                        }
                         if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
                     }
                 }
@@ -261,7 +325,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                         if (!ok) break;
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t st = sbase + slot * XI_STAGE;
-                        if (!(dbg & 1)) {
+                        {
                             // Theta digit s against the factor digits t = 0 .. 6 - s.  The digit blocks of the factor rows lie one behind the
                             // other in the stage (64 rows each) and group s + t owns TMEM columns [64 (s + t), + 64), so ONE instruction
                             // with N = 64 cnt covers cnt consecutive t: its B operand is "rows" t0*64 .. of the stacked digit blocks, its
@@ -273,7 +337,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
 #pragma unroll
                                 for (int t0 = 0; t0 < XI_S - s; t0 += XI_CAT) {
                                     const int cnt = (XI_S - s - t0) < XI_CAT ? (XI_S - s - t0) : XI_CAT;
-                                    const uint32_t Ni = (dbg & 4) ? 64u * cnt : 64u * (cnt - 1) + Nmma;
+                                    const uint32_t Ni = 64u * (cnt - 1) + Nmma;
                                     const uint32_t id = idesc | ((Ni >> 3) << 17);
                                     const uint64_t db = xi_desc(st + XI_TH_STAGE + t0 * XI_F_BLK);
                                     asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }"
@@ -302,30 +366,25 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
             const int tile_idx = (int)(q / NB), nb = (int)(q % NB);
             const ExTile tile = tiles[tile_idx];
             const int w = nb * 64 + wl, nrow = tile.nfrag * 8 - half * 32;      // live columns of this thread: [0, nrow)
-            double a[32], an[32];
+            double a[32], an[32], p1 = 0.0, p2 = 0.0;
+            // the weights of this thread's factor rows, fetched before the accumulators are waited for (0 beyond the tile: those
+            // TMEM columns were never written)
+            const double* wrow = wq + tile.row0 + half * 32;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) an[j] = j < nrow ? __ldg(wrow + j) : 0.0;
             // ---- phase a: recombine, weight, fetch the re/im partner row
             ok = xi_wait(acc_full, pf);
             ok = __all_sync(0xffffffffu, ok);
             if (!ok) break;
             pf ^= 1;
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < 32; ++j) a[j] = 0.0;
-#pragma unroll 1
-            for (int g = 0; g < XI_S; ++g) {
-                int v[32];
-                xi_ld32(tbase + (uint32_t)g * 64, v);
-                const double sc = xi_pow2(-(7 * g + 12));
-#pragma unroll
-                for (int j = 0; j < 32; ++j) a[j] = fma(xi_i2d(v[j]), sc, a[j]);
-            }
+            xi_readout<false>(tbase, a, an, p1, p2);
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(acc_empty);
-            const double* wrow = wq + tile.row0 + half * 32;
 #pragma unroll
             for (int j = 0; j < 32; ++j) {
-                a[j] = j < nrow ? a[j] * __ldg(wrow + j) : 0.0;           // columns beyond the tile were never written
+                a[j] *= an[j];
                 an[j] = __shfl_xor_sync(0xffffffffu, a[j], 1);
             }
             // ---- phase b: p1 = sum a_own b_own, p2 = sum a_partner b_own
@@ -334,22 +393,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
             if (!ok) break;
             pf ^= 1;
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            double p1 = 0.0, p2 = 0.0;
-#pragma unroll 1
-            for (int g = 0; g < XI_S; ++g) {
-                int v[32];
-                xi_ld32(tbase + (uint32_t)g * 64, v);
-                double q1 = 0.0, q2 = 0.0;
-#pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const double b = xi_i2d(v[j]);
-                    q1 = fma(a[j], b, q1);
-                    q2 = fma(an[j], b, q2);
-                }
-                const double sc = xi_pow2(-(7 * g + 12));
-                p1 = fma(q1, sc, p1);
-                p2 = fma(q2, sc, p2);
-            }
+            xi_readout<true>(tbase, a, an, p1, p2);
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(acc_empty);
@@ -453,7 +497,7 @@ void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const doubl
     const long long items = f->n_tiles * NB;
     const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
     k_exchange_i8<<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,
-                                                  f->dI8Fail, getenv("LO_I8_DBG") ? atoi(getenv("LO_I8_DBG")) : 0);
+                                                  f->dI8Fail);
     const int n = grid * 4 * f->Wcap;
     k_i8_poison<<<(n + 255) / 256, 256, 0, stream>>>(f->dI8Fail, f->dEKq, n);
     *part = f->dEKq;

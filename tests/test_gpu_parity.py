@@ -955,3 +955,88 @@ def test_int8_slicing_probe_on_tcgen05():
     dmma_us = 2.0 * 128 * 128 * 384 / (dmma_tflops * 1e12 / 148) * 1e6          # one SM's share of the measured DMMA peak
     assert err <= 1e-10, err
     assert us * 1.3 <= dmma_us, (us, dmma_us)
+
+
+# ------------------------------------------------------------------------------------------ exchange from INT8 digit slices (tcgen05)
+def int8_energy(F, phis):
+    """Energies with lo_set_exchange_mode(LO_EXCHANGE_INT8), two calls (bitwise repeatable), the set left in DMMA mode."""
+    F.set_exchange_mode(True)
+    try:
+        assert F.info().exchange_mode == 1 and F.info().int8_bytes > 0
+        Eq, st = gpu_energy(F, phis)
+        Eq2, _ = gpu_energy(F, phis)
+    finally:
+        F.set_exchange_mode(False)
+    assert np.array_equal(Eq, Eq2, equal_nan=True), "INT8 exchange: repeated call differs"
+    return Eq, st
+
+
+@pytest.mark.parametrize("cfg,T,n_w", [(0, 1e-8, 8), (1, 1e-6, 256), (1, 1e-4, 70), (1, 1e-6, 1), (1, 5.0, 33)])
+def test_exchange_int8_mode_matches_oracle(cfg, T, n_w):
+    """lo_set_exchange_mode(LO_EXCHANGE_INT8): the exchange projections from 7 x 7 signed 7-bit digit slices on the tcgen05 tensor
+    cores (28 exact int32 digit products, fp64 recombination).  Every walker against the oracle on the library's factor set at
+    the 1e-10 of the default route; E1 / E_J are the default kernels' and bit-identical; ragged walker counts (70, 1, 33)
+    and tiles of every height (T = 1e-4: ragged ranks; T = 5: every pair truncated away)."""
+    P = gen.make_problem(cfg)
+    phis = gen.make_walkers(P, n_w, seed=7)
+    F = lo.Factors.setup(P.h, P.L, P.psi, T, device=0, max_walkers=max(n_w, 64), gpu_svd=True)
+    Ed, st = gpu_energy(F, phis)
+    Eq, sq = int8_energy(F, phis)
+    Eo, _ = oracle_energy(P, F, phis)
+    assert (st == 0).all() and (sq == 0).all()
+    assert_parity(Eq, Eo)
+    assert np.array_equal(Eq[:, 1:3], Ed[:, 1:3])
+    assert_close(Eq, Ed, "INT8 exchange vs DMMA exchange", tol=1e-10)
+    # back in DMMA mode the default result is reproduced bit for bit
+    Ed2, _ = gpu_energy(F, phis)
+    assert np.array_equal(Ed2, Ed)
+
+
+def test_exchange_int8_mode_unrestricted_and_host_variant():
+    """Same check for an unrestricted trial (two tile lists, panels of both spins) and through lo_local_energy_host (walker
+    chunks of different sizes through the same sliced factor set)."""
+    torch = torch_cuda()
+    xyz, fns = gen.site_geometry(1)
+    P = gen.make_problem_from_geometry(xyz, fns, (9, 7), 300, seed=31)
+    phis = gen.make_walkers(P, 200)
+    F = lo.Factors.setup(P.h, P.L, P.psi, 1e-6, device=0, max_walkers=200, gpu_svd=True)
+    Eq, sq = int8_energy(F, phis)
+    Eo, _ = oracle_energy(P, F, phis)
+    assert (sq == 0).all()
+    assert_parity(Eq, Eo)
+    F.set_exchange_mode(True)
+    Eh, sh = F.local_energy_host([torch.from_numpy(np.ascontiguousarray(p)).pin_memory() for p in phis])
+    F.set_exchange_mode(False)
+    assert_close(Eh, Eq, "host-buffer variant, INT8 exchange")
+
+
+def test_exchange_int8_mode_singular_walker_and_errors(c0):
+    """A singular walker is flagged and NaN, the others are untouched by it (every walker has its own digit exponents);
+    host-only factor sets and unknown modes are refused."""
+    torch = torch_cuda()
+    phis = gen.make_walkers(c0, 4)
+    bad = [p.copy() for p in phis]
+    bad[0][2][:, 1] = 0.0                       # a zero orbital: exactly singular overlap
+    F = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=0, max_walkers=64)
+    Eq, sq = int8_energy(F, bad)
+    Eok, _ = int8_energy(F, phis)
+    assert sq.tolist() == [0, 0, 1, 0] and np.isnan(Eq[2]).all()
+    assert np.array_equal(Eq[[0, 1, 3]], Eok[[0, 1, 3]])
+    with pytest.raises(lo.LoError):
+        lo._check(lo.lib().lo_set_exchange_mode(F._h, 7))
+    Fh = lo.Factors.setup(c0.h, c0.L, c0.psi, 1e-8, device=-1)
+    with pytest.raises(lo.LoError):
+        Fh.set_exchange_mode(True)
+
+
+def test_exchange_int8_mode_c2_full_size(c2_built):
+    """BASELINE.json:configs[2] in bench.py's launch configuration with the INT8 exchange: all 512 walkers, 64 seeded walkers
+    against the oracle on the library's factor set, every walker against the DMMA route."""
+    P, phis, F = c2_built
+    Ed, _ = gpu_energy(F, phis)
+    Eq, sq = int8_energy(F, phis)
+    assert (sq == 0).all() and np.isfinite(Eq).all()
+    idx = np.random.default_rng(12).choice(P.n_w, 64, replace=False)
+    Eo, _ = oracle_energy(P, F, phis, idx)
+    assert_parity(Eq[idx], Eo)
+    assert_close(Eq, Ed, "INT8 exchange vs DMMA exchange, configs[2]", tol=1e-10)
