@@ -35,32 +35,35 @@ NOMINAL_BF16_TFLOPS = 2250.0
 # traffic is then null and `traffic_note` says why.
 TRAFFIC_SIDECAR = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 KERNEL_SOURCES = ("lo_kernels.cu", "lo_device.cuh")
+KERNEL_SOURCES_I8 = ("lo_exchange_i8.cu", "lo_device.cuh")     # rows whose kernel is k_exchange_i8
+NOMINAL_INT8_OVER_BF16 = 2.0   # dense INT8 : bf16 tensor throughput (4.5 : 2.25 POP/s), B200_PROFILING.md nominal table (fp8 row; kind::i8 runs at the fp8 rate)
 
 
-def kernel_sources_sha256():
+def kernel_sources_sha256(names=KERNEL_SOURCES):
     import hashlib
     h = hashlib.sha256()
-    for name in KERNEL_SOURCES:
+    for name in names:
         with open(os.path.join(ROOT, "paper_2202_00832_b200", "csrc", name), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()
 
 
-def ncu_traffic(workload):
-    """(bytes per launch or None, note) for `workload` from profiles/ncu_traffic.csv."""
+def ncu_traffic(workload, int8=False):
+    """(bytes per launch or None, note) for `workload` from profiles/ncu_traffic.csv; int8: the row of k_exchange_i8."""
     import csv
+    names = KERNEL_SOURCES_I8 if int8 else KERNEL_SOURCES
     try:
         with open(TRAFFIC_SIDECAR, newline="") as fh:
-            rows = [r for r in csv.DictReader(fh) if r["workload"] == workload]
+            rows = [r for r in csv.DictReader(fh) if r["workload"] == workload and r["kernel"].startswith("k_exchange_i8") == int8]
     except OSError:
         return None, "no sidecar %s" % os.path.relpath(TRAFFIC_SIDECAR, ROOT)
     if not rows:
         return None, "no ncu --set full capture of this workload in %s" % os.path.relpath(TRAFFIC_SIDECAR, ROOT)
-    sha = kernel_sources_sha256()
+    sha = kernel_sources_sha256(names)
     fresh = [r for r in rows if r["kernel_sources_sha256"] == sha]
     if not fresh:
         return None, "capture of commit %s is stale: %s changed since (sha256 %s.. != %s..)" % (
-            rows[-1]["commit"], "+".join(KERNEL_SOURCES), rows[-1]["kernel_sources_sha256"][:12], sha[:12])
+            rows[-1]["commit"], "+".join(names), rows[-1]["kernel_sources_sha256"][:12], sha[:12])
     r = fresh[-1]
     return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), "%s of %s at commit %s (%s)" % (
         r["kernel"], r["capture"], r["commit"], "dram__bytes_read.sum + dram__bytes_write.sum")
@@ -170,6 +173,37 @@ def run_ours(args):
     peak_dfma = lo.measure_peak("dfma", local)
     peak_hbm = lo.measure_peak("hbm", local)
 
+    # ---- exchange route of the timed step.  "int8" (default): projections from exact INT8 digit slices on the tcgen05 tensor cores
+    # (lo_set_exchange_mode, parity-tested at the same 1e-10); the FP64 DMMA route of the same factor set is timed first, with the
+    # same warm-up and step count, and reported as `dmma_route` (its own roofline against the measured FP64 peak).
+    int8 = args.exchange == "int8"
+    dmma_route = None
+    if int8:
+        for _ in range(max(args.warmup, 3)):
+            F.local_energy(dphi, parts=True)
+        torch.cuda.synchronize()
+        F.timing_enable(True)
+        F.timing_get()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record()
+        for _ in range(args.steps):
+            out_d = F.local_energy(dphi, parts=True)
+        d1.record()
+        torch.cuda.synchronize()
+        tmd = F.timing_get()
+        F.timing_enable(False)
+        d_ms = max_over_ranks(d0.elapsed_time(d1), dev)
+        dx_ms = tmd["exchange"][0] / max(tmd["exchange"][1], 1)
+        dx_tf = fl["exchange"] * n_w / (dx_ms * 1e-3) * 1e-12
+        E_dmma = torch.stack(out_d[:4], dim=1).cpu().numpy()
+        tr_d, tr_d_note = ncu_traffic(workload_name(cfg, reading, T, n_w))
+        dmma_route = {"what": "same step with lo_set_exchange_mode(LO_EXCHANGE_DMMA): k_exchange on the FP64 tensor pipe",
+                      "value": round(world * n_w * args.steps / (d_ms * 1e-3), 2), "unit": UNIT, "ms_per_step": round(d_ms / args.steps, 4),
+                      "roofline": {"bound": "tensor", "kernel": "k_exchange (grouped variable-rank dual DGEMM + fused sigma-weighted a.b)",
+                                   "achieved": round(dx_tf, 3), "peak": round(max(peak_dmma, peak_dfma), 3), "unit": "TFLOP/s",
+                                   "frac": round(dx_tf / max(peak_dmma, peak_dfma), 4), "kernel_ms": round(dx_ms, 4),
+                                   "traffic": tr_d, "traffic_note": tr_d_note}}
+        F.set_exchange_mode(True)
     for _ in range(max(args.warmup, 3)):
         F.local_energy(dphi, parts=True)
     torch.cuda.synchronize()
@@ -197,6 +231,8 @@ def run_ours(args):
     tm = F.timing_get()
     F.timing_enable(False)
     n_kernels = sum(n for _, n in tm.values()) + tm["coulomb"][1]      # the coulomb bracket holds 2 launches (GEMM + k_ej)
+    if int8:
+        n_kernels += 2 * tm["exchange"][1]                             # k_slice_theta + k_exchange_i8 + k_i8_poison
     value = world * n_w * args.steps / (ms_max * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of Phi and D2H of E inside the timed region
@@ -230,17 +266,45 @@ def run_ours(args):
     achieved = ex_flops / (ex_avg * 1e-3) * 1e-12
     peak = max(peak_dmma, peak_dfma)
     mp = measured_peaks()
-    traffic, traffic_note = ncu_traffic(workload_name(cfg, reading, T, n_w))
-    roofline = {"bound": "tensor", "kernel": "k_exchange (grouped variable-rank dual DGEMM + fused sigma-weighted a.b)",
-                "achieved": round(achieved, 3), "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
-                "traffic": traffic, "traffic_note": traffic_note,
-                "peak_source": "in-run register-resident DMMA.8x8x4 / DFMA loops (lo_measure_peak), of measured",
-                "peak_dmma": round(peak_dmma, 3), "peak_dfma": round(peak_dfma, 3),
-                "peak_from_bf16_ratio": round(mp.get("bf16_tflops", 0) * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS, 2) if mp else None,
-                "hbm_gbs_in_run": round(peak_hbm, 1), "hbm_gbs_measured_peaks": mp.get("hbm_gbs"),
-                "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
-                "algorithmic_flops_per_launch": ex_flops,
-                "algorithmic_bytes_per_launch": 16.0 * info.N * sum(info.sum_rank) + 8.0 * sum(info.sum_rank) + 16.0 * info.N * sum(info.n_occ) * n_w}
+    if not int8:
+        traffic, traffic_note = ncu_traffic(workload_name(cfg, reading, T, n_w))
+        roofline = {"bound": "tensor", "kernel": "k_exchange (grouped variable-rank dual DGEMM + fused sigma-weighted a.b)",
+                    "achieved": round(achieved, 3), "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
+                    "traffic": traffic, "traffic_note": traffic_note,
+                    "peak_source": "in-run register-resident DMMA.8x8x4 / DFMA loops (lo_measure_peak), of measured",
+                    "peak_dmma": round(peak_dmma, 3), "peak_dfma": round(peak_dfma, 3),
+                    "peak_from_bf16_ratio": round(mp.get("bf16_tflops", 0) * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS, 2) if mp else None,
+                    "hbm_gbs_in_run": round(peak_hbm, 1), "hbm_gbs_measured_peaks": mp.get("hbm_gbs"),
+                    "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
+                    "algorithmic_flops_per_launch": ex_flops,
+                    "algorithmic_bytes_per_launch": 16.0 * info.N * sum(info.sum_rank) + 8.0 * sum(info.sum_rank) + 16.0 * info.N * sum(info.n_occ) * n_w}
+    else:
+        # k_exchange_i8: every fp64 multiply-add of the two projections becomes 28 INT8 multiply-adds (7 x 7 digits, index sum <= 6)
+        # on the tcgen05 tensor cores.  achieved = those algorithmic integer ops / the exchange bracket (which also holds the
+        # per-call slicing of Theta, k_slice_theta); peak = measured dense bf16 (MEASURED_PEAKS.json, burst) x the nominal
+        # INT8 : bf16 ratio of 2, else the guide's nominal fallback.
+        r_sum = float(sum(info.sum_rank))
+        i8_ops = 28.0 * 8.0 * info.N * r_sum * n_w
+        achieved_i8 = i8_ops / (ex_avg * 1e-3) * 1e-12
+        bf16 = mp.get("bf16_tflops")
+        peak_i8 = (bf16 if bf16 else NOMINAL_BF16_TFLOPS) * NOMINAL_INT8_OVER_BF16
+        traffic, traffic_note = ncu_traffic(workload_name(cfg, reading, T, n_w), int8=True)
+        roofline = {"bound": "tensor", "kernel": "k_exchange_i8 (grouped dual GEMM from 7 x 7 INT8 digit slices, tcgen05.mma kind::i8 into TMEM, fused fp64 "
+                                                 "recombination + sigma-weighted a.b); bracket includes k_slice_theta",
+                    "achieved": round(achieved_i8, 1), "peak": round(peak_i8, 1), "unit": "TFLOP/s", "frac": round(achieved_i8 / peak_i8, 4),
+                    "unit_note": "integer ops (2 per INT8 multiply-add) of the 28 digit products per fp64 multiply-add",
+                    "traffic": traffic, "traffic_note": traffic_note,
+                    "peak_source": ("MEASURED_PEAKS.json bf16_tflops (burst) x 2 (nominal INT8 : bf16)" if bf16 else
+                                    "fallback: nominal dense bf16 2250 TFLOP/s x 2 (B200_PROFILING.md); MEASURED_PEAKS.json absent"),
+                    "peak_bf16_sustained_x2": round(mp["bf16_tflops_sustained"] * NOMINAL_INT8_OVER_BF16, 1) if mp.get("bf16_tflops_sustained") else None,
+                    "fp64_equivalent_tflops": round(achieved, 3), "fp64_equivalent_over_measured_dmma_peak": round(achieved / peak, 4),
+                    "peak_dmma": round(peak_dmma, 3), "peak_dfma": round(peak_dfma, 3),
+                    "hbm_gbs_in_run": round(peak_hbm, 1), "hbm_gbs_measured_peaks": mp.get("hbm_gbs"),
+                    "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
+                    "algorithmic_int8_ops_per_launch": i8_ops, "algorithmic_flops_per_launch_fp64": ex_flops,
+                    "algorithmic_bytes_per_launch": 14.0 * info.N * r_sum + 8.0 * r_sum + (16.0 + 2 * 7.0) * info.N * sum(info.n_occ) * n_w,
+                    "int8_slices_GB": round(info.int8_bytes / 1e9, 3)}
+        dmma_route["max_rel_diff_int8_vs_dmma"] = float((np.abs(E_dev - E_dmma).max(axis=1) / np.abs(E_dmma[:, 0])).max())
     # per STEP (an unrestricted config launches the S1 kernels once per spin; flops_per_walker sums both spins)
     kernels = {k: {"ms": round(m / args.steps, 4), "tflops": round(fl[k] * n_w / (m / args.steps * 1e-3) * 1e-12, 3) if m > 0 else 0.0}
                for k, (m, n) in tm.items()}
@@ -269,6 +333,7 @@ def run_ours(args):
 
     # ---- SURVEY 8(f) NEXT-3 (outside `value`): the paper-literal energy, Coulomb term from the compressed factors too
     if info.n_spin == 1:
+        F.set_exchange_mode(False)      # the compressed-Coulomb kernel is the DMMA exchange kernel with two more projections
         F.set_coulomb_mode(True)
         flc = F.flops_per_walker()
         for _ in range(3):
@@ -366,7 +431,8 @@ def run_ours(args):
     if rank == 0:
         line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                 "ms_per_step": round(ms_max / args.steps, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic",
+                "dtype": "s8 x s8 -> s32 digit products + f64 recombination (exchange), f64 (everything else)" if int8 else "f64",
+                "data": "synthetic",
                 "config": {"workload": workload_name(cfg, reading, T, n_w), "N": info.N, "N_occ": list(info.n_occ)[:info.n_spin],
                            "N_chol": info.n_chol, "N_w_per_gpu": n_w, "T_SVD": T, "sum_rank": sum(info.sum_rank),
                            "compression_pct": round(100 * (1 - sum(info.sum_rank) / (sum(info.n_pairs) * info.N)), 2),
@@ -376,10 +442,11 @@ def run_ours(args):
                            "setup_s": round(setup_s, 1), "lo_setup_s": round(info.setup_seconds, 2), "setup_svd_s": round(info.setup_svd_seconds, 2),
                            "svd_sweeps_max": info.svd_sweeps_max, "pairs_prescreened": int(info.n_pairs_prescreened)},
                 "tflops": round(flops_walker * n_w * world * args.steps / (ms_max * 1e-3) * 1e-12, 3),
+                "tflops_note": "algorithmic complex128 flops of S1-S5 per second (fp64-equivalent when the exchange runs from INT8 slices)",
                 "flops_per_walker": flops_walker, "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu_baseline,
                 "e2e": {"value": round(e2e_value, 2), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "ms_per_step": round(ms_e2e / args.steps, 4), "api": "lo_local_energy_host (C ABI, pinned host buffers)"},
-                "gpu_launches": int(n_kernels), "clocks": clocks, "next": nxt}
+                "gpu_launches": int(n_kernels), "clocks": clocks, "exchange": args.exchange, "dmma_route": dmma_route, "next": nxt}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -683,6 +750,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: pentacene-sized, the headline)")
     ap.add_argument("--reading", default="element", choices=["element", "vector"])
+    ap.add_argument("--exchange", default="int8", choices=["int8", "dmma"],
+                    help="exchange route of the timed step: INT8 digit slices on tcgen05 (default; the DMMA route is timed beside it) or FP64 DMMA only")
     ap.add_argument("--threshold", type=float, default=None)
     ap.add_argument("--walkers", type=int, default=None)
     ap.add_argument("--cpu-walkers", type=int, default=192, help="walkers of the batch the oracle is timed on (cpu_baseline)")
