@@ -265,6 +265,34 @@ lo_status lo_flops_per_walker(const lo_factors* f, double flops[LO_K_COUNT]);
  *   kind 4: max |C - C_fp64| / max |C_fp64| of that tile         -> *value dimensionless */
 lo_status lo_measure_peak(int device, int kind, double* value);
 
+/* Allocation-free S1 for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): Theta = Phi (Psi^T Phi)^-1 (Eq. 15) for a batch of walkers with NO factor set and NO
+ * allocation of any kind -- the same kernels as step S1 of lo_local_energy (k_overlap, k_inverse, k_theta); their
+ * scratch, the overlap matrices A_w = Psi^T Phi_w inverted in place (16 n_w n_occ^2 bytes), lives in a file-scope
+ * `static __device__` array of LO_NOALLOC_SCRATCH_BYTES (4 MiB) that every GPU holds from the moment it loads the library
+ * until the process exits.
+ *   device            CUDA device the pointers belong to
+ *   N, n_occ, n_w     basis functions, occupied orbitals (1 <= n_occ <= N), walkers (>= 1);
+ *                     16 n_w n_occ^2 > LO_NOALLOC_SCRATCH_BYTES is refused with LO_EINVAL (split the batch)
+ *   psi_dev           device fp64 [N][n_occ] row-major (trial orbitals, real)
+ *   phi_dev           device complex128 [n_w][N][n_occ] (walker-major, as lo_local_energy)
+ *   thetaT_dev        OUT, device fp64 [n_occ][ld_w][N_pad], N_pad = N rounded up to a multiple of 16: the Theta^T panel layout
+ *                     of the library, thetaT[(i ld_w + 2 w + c) N_pad + p] = (c ? Im : Re) Theta_w[p][i]; entries
+ *                     p in [N, N_pad) are written as zeros, rows 2 w + c >= 2 n_w are not touched.  ld_w >= 2 n_w, even.
+ *   status_dev        OUT, device int [n_w]: 1 for a walker whose overlap matrix is singular (its Theta is NaN), else 0
+ *   stream            cudaStream_t; the call is asynchronous on it
+ * lo_theta_noalloc_init(device) fetches the device address of the scratch array (cudaGetSymbolAddress) and sets the kernels'
+ * shared-memory attributes; call it once per device BEFORE any stream capture (lo_theta_noalloc calls it itself on first use
+ * otherwise).  Neither function calls cudaMalloc, cudaFree or an allocating library routine.
+ * The scratch array is shared by every call on a device and keeps the last call's contents; nothing in it has to start at
+ * zero (every entry a call reads it has written first), but two calls that overlap on the GPU (different streams, or
+ * concurrent graph launches) race on it: serialise them.
+ * Errors: LO_EINVAL (arguments, size beyond the maximum), LO_ECUDA. */
+#define LO_NOALLOC_SCRATCH_BYTES (4u << 20)
+lo_status lo_theta_noalloc_init(int device);
+lo_status lo_theta_noalloc(int device, int N, int n_occ, int n_w, const double* psi_dev, const void* phi_dev, double* thetaT_dev, int ld_w,
+                           int* status_dev, void* stream);
+
 void lo_free(lo_factors* f);
 const char* lo_last_error(void);
 const char* lo_version(void);

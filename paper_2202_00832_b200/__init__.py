@@ -21,7 +21,7 @@ K_NAMES = ("overlap", "inverse", "theta", "coulomb", "exchange", "finalize", "pr
 _STATUS = {0: "LO_OK", 1: "LO_EINVAL", 2: "LO_ENOMEM", 3: "LO_ECUDA", 5: "LO_EINTERNAL"}
 EXPORTS = ("lo_setup", "lo_info_get", "lo_ranks", "lo_factor_pair", "lo_factor_all", "lo_retruncate", "lo_screen_pairs", "lo_local_energy",
            "lo_local_energy_host", "lo_set_cas_trial", "lo_set_cas_trial_beta", "lo_local_energy_cas", "lo_set_coulomb_mode", "lo_set_exchange_mode", "lo_coulomb_x", "lo_propagator", "lo_propagator_buffer", "lo_propagator_host", "lo_theta_host", "lo_timing_enable", "lo_timing_get", "lo_flops_per_walker",
-           "lo_measure_peak", "lo_free", "lo_last_error", "lo_version")
+           "lo_measure_peak", "lo_theta_noalloc_init", "lo_theta_noalloc", "lo_free", "lo_last_error", "lo_version")
 
 
 class LoError(RuntimeError):
@@ -75,6 +75,8 @@ def lib():
         L.lo_timing_get.argtypes = [vp, C.POINTER(cd), C.POINTER(C.c_longlong)]
         L.lo_flops_per_walker.argtypes = [vp, C.POINTER(cd)]
         L.lo_measure_peak.argtypes = [ci, ci, C.POINTER(cd)]
+        L.lo_theta_noalloc_init.argtypes = [ci]
+        L.lo_theta_noalloc.argtypes = [ci, ci, ci, ci, vp, vp, vp, ci, vp, vp]
         L.lo_free.argtypes = [vp]
         L.lo_free.restype = None
         L.lo_last_error.restype = C.c_char_p
@@ -102,6 +104,33 @@ def measure_peak(kind: str, device: int = 0) -> float:
     v = C.c_double(0)
     _check(lib().lo_measure_peak(device, {"dmma": 0, "dfma": 1, "hbm": 2, "int8_tile_us": 3, "int8_tile_err": 4}[kind], C.byref(v)))
     return v.value
+
+
+LO_NOALLOC_SCRATCH_BYTES = 4 << 20
+
+
+def theta_noalloc_init(device: int = 0):
+    """lo_theta_noalloc_init: fetch the device address of the static scratch array (once per device, before any capture)."""
+    _check(lib().lo_theta_noalloc_init(int(device)))
+
+
+def theta_noalloc(psi, phi, thetaT, status, stream=None):
+    """lo_theta_noalloc: Theta = Phi (Psi^T Phi)^-1 with no allocation (scratch in a static device array of 4 MiB).
+    All arguments are torch CUDA tensors the caller owns: psi float64 [N, n_occ], phi complex128 [n_w, N, n_occ],
+    thetaT float64 [n_occ, ld_w, N_pad] (OUT, Theta^T panels), status int32 [n_w] (OUT).  Asynchronous on `stream`."""
+    import torch
+    if not (psi.is_cuda and phi.is_cuda and thetaT.is_cuda and status.is_cuda):
+        raise ValueError("theta_noalloc: all tensors must be CUDA tensors")
+    if psi.dtype != torch.float64 or phi.dtype != torch.complex128 or thetaT.dtype != torch.float64 or status.dtype != torch.int32:
+        raise ValueError("theta_noalloc: psi/thetaT float64, phi complex128, status int32")
+    if not (psi.is_contiguous() and phi.is_contiguous() and thetaT.is_contiguous() and status.is_contiguous()):
+        raise ValueError("theta_noalloc: tensors must be contiguous")
+    n_w, N, O = phi.shape
+    if tuple(psi.shape) != (N, O) or thetaT.dim() != 3 or thetaT.shape[0] != O or thetaT.shape[2] != (N + 15) // 16 * 16 or status.numel() < n_w:
+        raise ValueError("theta_noalloc: shapes psi [N, O], phi [n_w, N, O], thetaT [O, ld_w, ceil16(N)], status [n_w]")
+    s = torch.cuda.current_stream(phi.device) if stream is None else stream
+    _check(lib().lo_theta_noalloc(phi.device.index, N, O, n_w, C.c_void_p(psi.data_ptr()), C.c_void_p(phi.data_ptr()),
+                                  C.c_void_p(thetaT.data_ptr()), int(thetaT.shape[1]), C.c_void_p(status.data_ptr()), C.c_void_p(s.cuda_stream)))
 
 
 class Factors:

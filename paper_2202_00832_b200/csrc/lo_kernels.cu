@@ -1320,3 +1320,65 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
 }
 
 }  // namespace lo
+
+// ------------------------------------------------------------------------------------------------ allocation-free S1
+// lo_theta_noalloc (include/lo_afqmc.h): step S1 for callers that cannot allocate.  The scratch of the S1 kernels -- the
+// overlap matrices, inverted in place -- is this file-scope array; every GPU that loads the library holds it until exit.
+// In host code the NAME below is a host-side stand-in, not a device address: the kernels get the pointer that
+// cudaGetSymbolAddress returned for the device they run on (fetched once per device, with that device current).
+static __device__ __align__(256) unsigned char lo_noalloc_scratch[LO_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+double* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {nullptr};     // device address of lo_noalloc_scratch, per device
+}  // namespace
+
+extern "C" lo_status lo_theta_noalloc_init(int device) {
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev || device >= NOALLOC_MAX_DEVICES) {
+        (void)cudaGetLastError();
+        lo::set_error("lo_theta_noalloc_init: no such CUDA device");
+        return LO_EINVAL;
+    }
+    if (g_noalloc_ptr[device]) return LO_OK;
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) { lo::set_error(std::string("lo_theta_noalloc_init: cudaSetDevice: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    if (lo::configure_kernels() != LO_OK) return LO_ECUDA;      // shared-memory attributes of the S1 kernels (no allocation)
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, lo_noalloc_scratch);
+    if (e != cudaSuccess || !p) {
+        lo::set_error(std::string("lo_theta_noalloc_init: cudaGetSymbolAddress(lo_noalloc_scratch): ") + cudaGetErrorString(e));
+        return LO_ECUDA;
+    }
+    g_noalloc_ptr[device] = static_cast<double*>(p);
+    return LO_OK;
+}
+
+extern "C" lo_status lo_theta_noalloc(int device, int N, int n_occ, int n_w, const double* psi_dev, const void* phi_dev, double* thetaT_dev,
+                                      int ld_w, int* status_dev, void* stream) {
+    if (N <= 0 || n_occ <= 0 || n_occ > N || n_w <= 0 || !psi_dev || !phi_dev || !thetaT_dev || !status_dev || ld_w < 2 * n_w || (ld_w & 1)) {
+        lo::set_error("lo_theta_noalloc: invalid argument (need 1 <= n_occ <= N, n_w >= 1, non-NULL device pointers, even ld_w >= 2 n_w)");
+        return LO_EINVAL;
+    }
+    const unsigned long long need = 16ull * (unsigned long long)n_w * (unsigned long long)n_occ * (unsigned long long)n_occ;
+    if (need > LO_NOALLOC_SCRATCH_BYTES) {
+        lo::set_error("lo_theta_noalloc: the overlap matrices need " + std::to_string(need) + " bytes of scratch (16 n_w n_occ^2), the static array holds " +
+                      std::to_string((unsigned long long)LO_NOALLOC_SCRATCH_BYTES) + ": split the batch");
+        return LO_EINVAL;
+    }
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES || !g_noalloc_ptr[device]) {
+        lo_status st = lo_theta_noalloc_init(device);       // first use on this device (call it yourself before a stream capture)
+        if (st != LO_OK) return st;
+    }
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) { lo::set_error(std::string("lo_theta_noalloc: cudaSetDevice: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    // the S1 launcher of the ordinary path wants a factor set for N, N_pad and its timers: a blank one on the stack (no device
+    // state, timing off); scratch = the static array, output = the caller's panels
+    lo_factors blank;
+    blank.N = N;
+    blank.N_pad = (N + lo::KTILE - 1) / lo::KTILE * lo::KTILE;
+    lo::launch_s1(&blank, n_w, psi_dev, n_occ, n_occ, phi_dev, g_noalloc_ptr[device], status_dev, thetaT_dev, 0, ld_w, static_cast<cudaStream_t>(stream));
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { lo::set_error(std::string("lo_theta_noalloc: kernel launch failed: ") + cudaGetErrorString(e)); return LO_ECUDA; }
+    return LO_OK;
+}
