@@ -303,7 +303,7 @@ def run_ours(args):
                     "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
                     "algorithmic_int8_ops_per_launch": i8_ops, "algorithmic_flops_per_launch_fp64": ex_flops,
                     "algorithmic_bytes_per_launch": 14.0 * info.N * r_sum + 8.0 * r_sum + (16.0 + 2 * 7.0) * info.N * sum(info.n_occ) * n_w,
-                    "int8_slices_GB": round(info.int8_bytes / 1e9, 3)}
+                    "int8_slices_GB": round(F.info().int8_bytes / 1e9, 3)}
         dmma_route["max_rel_diff_int8_vs_dmma"] = float((np.abs(E_dev - E_dmma).max(axis=1) / np.abs(E_dmma[:, 0])).max())
     # per STEP (an unrestricted config launches the S1 kernels once per spin; flops_per_walker sums both spins)
     kernels = {k: {"ms": round(m / args.steps, 4), "tflops": round(fl[k] * n_w / (m / args.steps * 1e-3) * 1e-12, 3) if m > 0 else 0.0}
