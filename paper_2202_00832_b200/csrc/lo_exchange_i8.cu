@@ -15,7 +15,8 @@
 // a then b, each streaming K once with all 7 groups live in TMEM (7 x 64 = 448 of the 512 columns).  One CTA per SM,
 // 12 warps: warp 0 (one lane) feeds a 5-stage ring with cp.async.bulk copies of pre-tiled slices (Theta: 7 x 4 KB, factor
 // rows: 7 x 2 KB per stage), warp 1 (one lane) issues the MMAs and commits stages / accumulators to mbarriers, warps 4..11
-// read TMEM (lane quadrant = warp % 4, column half = (warp - 4) / 4), recombine in fp64 and, in phase b, multiply straight
+// read TMEM (lane quadrant = warp % 4, column half = (warp - 4) / 4), merge the 7 groups of a column exactly in 64-bit integers, convert
+// the two partial sums to fp64 (the FP64 pipe, 64 FMA / clock / SM, bounds the read-out) and, in phase b, multiply straight
 // into the weighted dot with the a values they hold in registers (own row and the re/im partner row), so b is never stored.
 // Per-CTA partial sums are updated in a fixed order by their owning thread: results are bitwise repeatable.
 //
@@ -185,61 +186,67 @@ __device__ __forceinline__ void xi_ld32(uint32_t taddr, int (&v)[32]) {
 __device__ __forceinline__ double xi_pow2(int e) { return __hiloint2double((1023 + e) << 20, 0); }
 __device__ __forceinline__ double xi_i2d(int v) { return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0; }
 
-__device__ __forceinline__ void xi_ld16(uint32_t taddr, int (&v)[16]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
-                   "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+__device__ __forceinline__ void xi_ld8(uint32_t taddr, int (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
                  : "r"(taddr));
 }
 // the registers of the load are operands of the wait, so that nothing that reads them can be scheduled above it
-__device__ __forceinline__ void xi_ld_wait(int (&v)[16]) {
+__device__ __forceinline__ void xi_ld_wait8(int (&v)[8]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]), "+r"(v[8]), "+r"(v[9]),
-                   "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15])
+                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7])
                  :: "memory");
 }
-// Read-out of the 7 accumulator groups of this thread's row (32 columns each, 16 at a time, the next load in flight while
-// the current one is consumed).  PHASE_B = false: a[j] = sum_g 2^-(7g+12) D_g[j].  PHASE_B = true: p1 += sum_j a[j] b[j],
-// p2 += sum_j an[j] b[j] with b recombined on the fly (linear in the groups), b itself is never stored.
+// int64 -> fp64 without I2F for |s| < 2^51: 2^52 + 2^51 + s is exact in the mantissa
+__device__ __forceinline__ double xi_l2d(long long s) { return __longlong_as_double(s + 0x4338000000000000LL) - 6755399441055744.0; }
+// Read-out of the 7 accumulator groups of this thread's row: 32 columns, 8 at a time; for a column the groups are first merged
+// EXACTLY in 64-bit integers -- hi = D_0 2^21 + D_1 2^14 + D_2 2^7 + D_3, lo = D_4 2^14 + D_5 2^7 + D_6, |hi| <= N 2^33.1 -- and
+// only the two sums go through the FP64 pipe (the read-out is bound by that pipe: 64 FMA / clock / SM),
+//   sum_g 2^-(7g+12) D_g = hi 2^-33 + lo 2^-54.
+// The next 8-column load is in flight while the current one is merged.  PHASE_B = false: a[j] = that value.  PHASE_B = true:
+// p1 += sum_j a[j] b[j], p2 += sum_j an[j] b[j]; b itself is never stored.
 template <bool PHASE_B>
 __device__ __forceinline__ void xi_readout(uint32_t tbase, double (&a)[32], const double (&an)[32], double& p1, double& p2) {
-    int v0[16], v1[16];
-    xi_ld16(tbase, v0);
-    xi_ld_wait(v0);
+    static_assert(XI_S == 7, "the hi / lo split below is written for 7 groups");
+    int v[2][8];
+    xi_ld8(tbase, v[0]);
+    double q1a = 0.0, q1b = 0.0, q2a = 0.0, q2b = 0.0;
+    const double c_hi = xi_pow2(-33), c_lo = xi_pow2(-54);
 #pragma unroll
-    for (int g = 0; g < XI_S; ++g) {
-        const double sc = xi_pow2(-(7 * g + 12));
-        double q1a = 0.0, q1b = 0.0, q2a = 0.0, q2b = 0.0;
-        xi_ld16(tbase + (uint32_t)g * 64 + 16, v1);
+    for (int c = 0; c < 4; ++c) {
+        long long hi[8], lo[8];
 #pragma unroll
-        for (int j = 0; j < 16; j += 2) {
-            const double b0 = xi_i2d(v0[j]), b1 = xi_i2d(v0[j + 1]);
-            if constexpr (PHASE_B) {
-                q1a = fma(a[j], b0, q1a); q1b = fma(a[j + 1], b1, q1b);
-                q2a = fma(an[j], b0, q2a); q2b = fma(an[j + 1], b1, q2b);
-            } else {
-                a[j] = g ? fma(b0, sc, a[j]) : b0 * sc;
-                a[j + 1] = g ? fma(b1, sc, a[j + 1]) : b1 * sc;
+        for (int g = 0; g < XI_S; ++g) {
+            const int n = c * XI_S + g;
+            xi_ld_wait8(v[n & 1]);
+            if (n + 1 < 4 * XI_S) xi_ld8(tbase + (uint32_t)(((n + 1) % XI_S) * 64 + ((n + 1) / XI_S) * 8), v[(n + 1) & 1]);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const long long d = v[n & 1][j];
+                if (g == 0) hi[j] = d * (1LL << 21);
+                else if (g == 1) hi[j] += d * (1LL << 14);
+                else if (g == 2) hi[j] += d * (1LL << 7);
+                else if (g == 3) hi[j] += d;
+                else if (g == 4) lo[j] = d * (1LL << 14);
+                else if (g == 5) lo[j] += d * (1LL << 7);
+                else lo[j] += d;
             }
         }
-        xi_ld_wait(v1);
-        if (g + 1 < XI_S) xi_ld16(tbase + (uint32_t)(g + 1) * 64, v0);
 #pragma unroll
-        for (int j = 0; j < 16; j += 2) {
-            const double b0 = xi_i2d(v1[j]), b1 = xi_i2d(v1[j + 1]);
+        for (int j = 0; j < 8; j += 2) {
+            const double b0 = fma(xi_l2d(hi[j]), c_hi, xi_l2d(lo[j]) * c_lo), b1 = fma(xi_l2d(hi[j + 1]), c_hi, xi_l2d(lo[j + 1]) * c_lo);
             if constexpr (PHASE_B) {
-                q1a = fma(a[16 + j], b0, q1a); q1b = fma(a[17 + j], b1, q1b);
-                q2a = fma(an[16 + j], b0, q2a); q2b = fma(an[17 + j], b1, q2b);
+                q1a = fma(a[c * 8 + j], b0, q1a); q1b = fma(a[c * 8 + j + 1], b1, q1b);
+                q2a = fma(an[c * 8 + j], b0, q2a); q2b = fma(an[c * 8 + j + 1], b1, q2b);
             } else {
-                a[16 + j] = g ? fma(b0, sc, a[16 + j]) : b0 * sc;
-                a[17 + j] = g ? fma(b1, sc, a[17 + j]) : b1 * sc;
+                a[c * 8 + j] = b0;
+                a[c * 8 + j + 1] = b1;
             }
         }
-        if (g + 1 < XI_S) xi_ld_wait(v0);
-        if constexpr (PHASE_B) {
-            p1 = fma(q1a + q1b, sc, p1);
-            p2 = fma(q2a + q2b, sc, p2);
-        }
+    }
+    if constexpr (PHASE_B) {
+        p1 = q1a + q1b;
+        p2 = q2a + q2b;
     }
 }
 
