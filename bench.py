@@ -174,7 +174,8 @@ def run_ours(args):
     peak_hbm = lo.measure_peak("hbm", local)
 
     # ---- exchange route of the timed step.  "int8" (default): projections from exact INT8 digit slices on the tcgen05 tensor cores
-    # (lo_set_exchange_mode, parity-tested at the same 1e-10); the FP64 DMMA route of the same factor set is timed first, with the
+    # and the Coulomb / one-body contraction on the same route (lo_set_exchange_mode, parity-tested at the same 1e-10); the FP64 DMMA
+    # route of the same factor set is timed first, with the
     # same warm-up and step count, and reported as `dmma_route` (its own roofline against the measured FP64 peak).
     int8 = args.exchange == "int8"
     dmma_route = None
@@ -232,7 +233,7 @@ def run_ours(args):
     F.timing_enable(False)
     n_kernels = sum(n for _, n in tm.values()) + tm["coulomb"][1]      # the coulomb bracket holds 2 launches (GEMM + k_ej)
     if int8:
-        n_kernels += 2 * tm["exchange"][1]                             # k_slice_theta + k_exchange_i8 + k_i8_poison
+        n_kernels += tm["coulomb"][1] + tm["exchange"][1]              # + k_slice_theta (coulomb bracket), + k_i8_poison (exchange bracket)
     value = world * n_w * args.steps / (ms_max * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of Phi and D2H of E inside the timed region
@@ -280,8 +281,9 @@ def run_ours(args):
                     "algorithmic_bytes_per_launch": 16.0 * info.N * sum(info.sum_rank) + 8.0 * sum(info.sum_rank) + 16.0 * info.N * sum(info.n_occ) * n_w}
     else:
         # k_exchange_i8: every fp64 multiply-add of the two projections becomes 28 INT8 multiply-adds (7 x 7 digits, index sum <= 6)
-        # on the tcgen05 tensor cores.  achieved = those algorithmic integer ops / the exchange bracket (which also holds the
-        # per-call slicing of Theta, k_slice_theta); peak = measured dense bf16 (MEASURED_PEAKS.json, burst) x the nominal
+        # on the tcgen05 tensor cores.  achieved = those algorithmic integer ops / the exchange bracket (k_exchange_i8 + the
+        # one-block k_i8_poison; the per-call slicing of Theta, k_slice_theta, sits in the coulomb bracket, whose INT8 GEMM
+        # k_coulomb_i8 uses the digits first); peak = measured dense bf16 (MEASURED_PEAKS.json, burst) x the nominal
         # INT8 : bf16 ratio of 2, else the guide's nominal fallback.
         r_sum = float(sum(info.sum_rank))
         i8_ops = 28.0 * 8.0 * info.N * r_sum * n_w
@@ -290,7 +292,7 @@ def run_ours(args):
         peak_i8 = (bf16 if bf16 else NOMINAL_BF16_TFLOPS) * NOMINAL_INT8_OVER_BF16
         traffic, traffic_note = ncu_traffic(workload_name(cfg, reading, T, n_w), int8=True)
         roofline = {"bound": "tensor", "kernel": "k_exchange_i8 (grouped dual GEMM from 7 x 7 INT8 digit slices, tcgen05.mma kind::i8 into TMEM, fused fp64 "
-                                                 "recombination + sigma-weighted a.b); bracket includes k_slice_theta",
+                                                 "recombination + sigma-weighted a.b)",
                     "achieved": round(achieved_i8, 1), "peak": round(peak_i8, 1), "unit": "TFLOP/s", "frac": round(achieved_i8 / peak_i8, 4),
                     "unit_note": "integer ops (2 per INT8 multiply-add) of the 28 digit products per fp64 multiply-add",
                     "traffic": traffic, "traffic_note": traffic_note,
@@ -302,7 +304,7 @@ def run_ours(args):
                     "hbm_gbs_in_run": round(peak_hbm, 1), "hbm_gbs_measured_peaks": mp.get("hbm_gbs"),
                     "kernel_ms": round(ex_avg, 4), "kernel_share_of_step": round(ex_ms / max(sum(m for m, _ in tm.values()), 1e-9), 4),
                     "algorithmic_int8_ops_per_launch": i8_ops, "algorithmic_flops_per_launch_fp64": ex_flops,
-                    "algorithmic_bytes_per_launch": 14.0 * info.N * r_sum + 8.0 * r_sum + (16.0 + 2 * 7.0) * info.N * sum(info.n_occ) * n_w,
+                    "algorithmic_bytes_per_launch": 14.0 * info.N * r_sum + 8.0 * r_sum + 14.0 * info.N * sum(info.n_occ) * n_w,
                     "int8_slices_GB": round(F.info().int8_bytes / 1e9, 3)}
         dmma_route["max_rel_diff_int8_vs_dmma"] = float((np.abs(E_dev - E_dmma).max(axis=1) / np.abs(E_dmma[:, 0])).max())
     # per STEP (an unrestricted config launches the S1 kernels once per spin; flops_per_walker sums both spins)
@@ -431,7 +433,7 @@ def run_ours(args):
     if rank == 0:
         line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                 "ms_per_step": round(ms_max / args.steps, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "s8 x s8 -> s32 digit products + f64 recombination (exchange), f64 (everything else)" if int8 else "f64",
+                "dtype": "s8 x s8 -> s32 digit products + f64 recombination (exchange, Coulomb), f64 (everything else)" if int8 else "f64",
                 "data": "synthetic",
                 "config": {"workload": workload_name(cfg, reading, T, n_w), "N": info.N, "N_occ": list(info.n_occ)[:info.n_spin],
                            "N_chol": info.n_chol, "N_w_per_gpu": n_w, "T_SVD": T, "sum_rank": sum(info.sum_rank),

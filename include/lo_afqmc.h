@@ -169,16 +169,18 @@ lo_status lo_coulomb_x(const lo_factors* f, const void** X_dev, int* ld);
 #define LO_COULOMB_COMPRESSED 1
 lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
 
-/* Exchange arithmetic of every later lo_local_energy* call on this (device-resident) factor set.
- *   LO_EXCHANGE_DMMA (default): a = U Theta_j, b = W Theta_i as FP64 tensor-pipe GEMMs (mma.sync m8n8k4.f64), Eq. 18 as written.
- *   LO_EXCHANGE_INT8: the same projections from exact INT8 digit slices on the tcgen05 tensor cores (Ozaki-type splitting:
- *     every row of U, W and Theta^T is scaled by a power of two and cut into 7 signed 7-bit digits; the 28 digit products
- *     with digit-index sum <= 6 are exact int32 GEMMs accumulated in TMEM; recombination, sigma weights and the a.b
- *     reduction in fp64).  Not bit-identical to the DMMA route: the projections carry an absolute error of about
- *     2^-47 |row|_max |Theta row|_max N, E_K agrees to ~1e-12 relative on the BASELINE configs (the parity
- *     tests hold it to the same 1e-10 as the default).  The first call slices the factor rows once (extra device memory:
- *     7/8 of the factor bytes + 7 bytes per Theta^T element, lo_info.int8_bytes) and is synchronous; LO_ENOMEM leaves the
- *     set in LO_EXCHANGE_DMMA mode.  Ignored while LO_COULOMB_COMPRESSED is set and by lo_local_energy_cas.
+/* Arithmetic of the two heavy contractions of every later lo_local_energy* call on this (device-resident) factor set.
+ *   LO_EXCHANGE_DMMA (default): the exchange projections a = U Theta_j, b = W Theta_i (Eq. 18) and the Coulomb / one-body
+ *     contraction X^g = sum L^g_op Theta_po (Eq. 16) as FP64 tensor-pipe GEMMs (mma.sync m8n8k4.f64), as written.
+ *   LO_EXCHANGE_INT8: the same contractions from exact INT8 digit slices on the tcgen05 tensor cores (Ozaki-type splitting:
+ *     every row of U, W, Lbar (per orbital) and Theta^T is scaled by a power of two and cut into 7 signed 7-bit digits; the 28
+ *     digit products with digit-index sum <= 6 are exact int32 GEMMs accumulated in TMEM; recombination, sigma weights, the a.b
+ *     reduction and E_J = sum_g (X^g)^2 in fp64).  Not bit-identical to the DMMA route: the projections carry an absolute error
+ *     of about 2^-47 |row|_max |Theta row|_max N, the energies agree to ~1e-11 of |E_L| on the BASELINE configs (DESIGN.md
+ *     section 6b; the parity tests hold this route to the same 1e-10 as the default).  The first call slices the factor rows and
+ *     Lbar once (extra device memory: 7/8 of the factor and Lbar bytes + 7 bytes per Theta^T element, lo_info.int8_bytes) and
+ *     is synchronous; LO_ENOMEM leaves the set in LO_EXCHANGE_DMMA mode.  Ignored while LO_COULOMB_COMPRESSED is set and by
+ *     lo_local_energy_cas (both keep their DMMA kernels).
  * Host-only factor sets: LO_EINVAL. */
 #define LO_EXCHANGE_DMMA 0
 #define LO_EXCHANGE_INT8 1

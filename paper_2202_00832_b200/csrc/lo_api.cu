@@ -1161,7 +1161,11 @@ lo_status lo_local_energy_cas(const lo_factors* fc, int n_w, const void* phi, co
     }
     lo_factors* f = const_cast<lo_factors*>(fc);
     CK(cudaSetDevice(f->device));
-    return launch_local_energy_cas(f, n_w, phi, f->n_spin == 2 ? phi_b : nullptr, E_L, E1, E_J, E_K, ovlp, walker_status, (cudaStream_t)stream);
+    const int ex_mode = f->ex_mode;      // the multi-determinant path keeps its DMMA kernels (lo_set_exchange_mode)
+    f->ex_mode = LO_EXCHANGE_DMMA;
+    const lo_status st = launch_local_energy_cas(f, n_w, phi, f->n_spin == 2 ? phi_b : nullptr, E_L, E1, E_J, E_K, ovlp, walker_status, (cudaStream_t)stream);
+    f->ex_mode = ex_mode;
+    return st;
 }
 
 lo_status lo_propagator(const lo_factors* fc, int n_w, const void* x_dev, void* stream) {

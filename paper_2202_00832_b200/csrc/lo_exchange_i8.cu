@@ -250,6 +250,49 @@ __device__ __forceinline__ void xi_readout(uint32_t tbase, double (&a)[32], cons
     }
 }
 
+// The MMAs of one K block (32 basis functions) of a stage at shared address st: Theta digit s (M = 128 rows) against the operand
+// digits t = 0 .. 6 - s.  The operand's digit blocks lie one behind the other in the stage (64 rows each) and group s + t owns TMEM
+// columns [64 (s + t), + 64), so ONE instruction with N = 64 cnt covers cnt consecutive t: its B operand is "rows" t0*64 .. of the
+// stacked digit blocks, its accumulator the cnt adjacent groups (28 digit products in 10 instructions; kind::i8 instructions
+// below N = 128 run at the N = 128 rate).  Nmma = live operand rows rounded up to 16; `first` overwrites the accumulators.
+__device__ __forceinline__ void xi_mma_kblock(uint32_t tmem, uint32_t st, uint32_t Nmma, bool first) {
+    // instruction descriptor: D = S32 (2 << 4), A = B = signed 8 bit (1 << 7, 1 << 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+    const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((128u >> 4) << 24);
+#pragma unroll
+    for (int s = 0; s < XI_S; ++s) {
+        const uint64_t da = xi_desc(st + s * XI_TH_BLK);
+        const uint32_t accum = (first && s == 0) ? 0u : 1u;
+#pragma unroll
+        for (int t0 = 0; t0 < XI_S - s; t0 += XI_CAT) {
+            const int cnt = (XI_S - s - t0) < XI_CAT ? (XI_S - s - t0) : XI_CAT;
+            const uint32_t Ni = 64u * (cnt - 1) + Nmma;
+            const uint32_t id = idesc | ((Ni >> 3) << 17);
+            const uint64_t db = xi_desc(st + XI_TH_STAGE + t0 * XI_F_BLK);
+            asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }"
+                         ::"r"(tmem + (uint32_t)(s + t0) * 64), "l"(da), "l"(db), "r"(id), "r"(accum) : "memory");
+        }
+    }
+}
+
+// CTA set-up shared by the INT8 kernels: mbarriers (full[], empty[], acc_full, acc_empty), 512 TMEM columns; returns the TMEM base
+__device__ __forceinline__ uint32_t xi_cta_setup(uint32_t full, uint32_t* tmem_base_s) {
+    const uint32_t empty = full + 8 * XI_STAGES, acc_full = empty + 8 * XI_STAGES, acc_empty = acc_full + 8;
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < XI_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 1); }
+        mbar_init(acc_full, 1);
+        mbar_init(acc_empty, 8);            // one arrival per epilogue warp
+        fence_barrier_init();
+    }
+    if (threadIdx.x < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_s)), "r"((uint32_t)XI_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    return *tmem_base_s;
+}
+
 __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict__ Uq, const int8_t* __restrict__ Wq, const int8_t* __restrict__ Thq,
                                                         const double* __restrict__ wq, const double* __restrict__ thScale,
                                                         const ExTile* __restrict__ tiles, long long n_items, int NB, int NBcap, int KB, int Wcap,
@@ -262,20 +305,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // partial sums: two rows per CTA (one per column half of the epilogue warps), zeroed here, updated by their owners only
     for (int i = tid; i < 4 * Wcap; i += 384) ekpart[(size_t)blockIdx.x * 4 * Wcap + i] = 0.0;
-    if (tid == 0) {
-        for (int i = 0; i < XI_STAGES; ++i) { mbar_init(full + 8 * i, 1); mbar_init(empty + 8 * i, 1); }
-        mbar_init(acc_full, 1);
-        mbar_init(acc_empty, 8);            // one arrival per epilogue warp
-        fence_barrier_init();
-    }
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"((uint32_t)XI_TMEM_COLS) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t tmem = tmem_base_s;
+    const uint32_t tmem = xi_cta_setup(full, &tmem_base_s);
     const long long my_items = n_items > (long long)blockIdx.x ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     bool ok = true;
     if (warp < 4) {
@@ -320,8 +350,6 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                 const long long q = blockIdx.x + it * gridDim.x;
                 const ExTile tile = tiles[(int)(q / NB)];
                 const uint32_t Nmma = (uint32_t)((tile.nfrag * 8 + 15) / 16) * 16;
-                // instruction descriptor: D = S32 (2 << 4), A = B = signed 8 bit (1 << 7, 1 << 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
-                const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((128u >> 4) << 24);
                 for (int ph = 0; ph < 2 && ok; ++ph) {
                     ok = xi_wait(acc_empty, pe);
                     if (!ok) break;
@@ -332,26 +360,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                         if (!ok) break;
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t st = sbase + slot * XI_STAGE;
-                        {
-                            // Theta digit s against the factor digits t = 0 .. 6 - s.  The digit blocks of the factor rows lie one behind the
-                            // other in the stage (64 rows each) and group s + t owns TMEM columns [64 (s + t), + 64), so ONE instruction
-                            // with N = 64 cnt covers cnt consecutive t: its B operand is "rows" t0*64 .. of the stacked digit blocks, its
-                            // accumulator the cnt adjacent groups.  (kind::i8 instructions below N = 128 run at the N = 128 rate.)
-#pragma unroll
-                            for (int s = 0; s < XI_S; ++s) {
-                                const uint64_t da = xi_desc(st + s * XI_TH_BLK);
-                                const uint32_t accum = (kb == 0 && s == 0) ? 0u : 1u;
-#pragma unroll
-                                for (int t0 = 0; t0 < XI_S - s; t0 += XI_CAT) {
-                                    const int cnt = (XI_S - s - t0) < XI_CAT ? (XI_S - s - t0) : XI_CAT;
-                                    const uint32_t Ni = 64u * (cnt - 1) + Nmma;
-                                    const uint32_t id = idesc | ((Ni >> 3) << 17);
-                                    const uint64_t db = xi_desc(st + XI_TH_STAGE + t0 * XI_F_BLK);
-                                    asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }"
-                                                 ::"r"(tmem + (uint32_t)(s + t0) * 64), "l"(da), "l"(db), "r"(id), "r"(accum) : "memory");
-                                }
-                            }
-                        }
+                        xi_mma_kblock(tmem, st, Nmma, kb == 0);
                         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(empty + 8 * slot) : "memory");
                         if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
                     }
@@ -421,6 +430,155 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)XI_TMEM_COLS) : "memory");
 }
 
+// ---- Coulomb / one-body contraction on the same route -------------------------------------------------------------------------
+// X^g_w = sum_{o,p} Lbar^g_op Theta_w[p][o] (Eq. 16; row n_chol of Lbar is hbar: the one-body term) from the Theta
+// digits of this call and digits of Lbar cut once: Lq [gt][o][kb][7][64 rows x 32 B], rows g = 64 gt .. of Lbar, one power of two
+// per (row g, orbital o) segment (eL).  A work item = (64 rows g, block of 64 walkers, split sp of the orbitals).  The Theta rows carry one exponent
+// per (orbital, walker), so the int32 accumulators are read out after every orbital (12 K blocks at N = 378) and summed in fp64
+// registers with that orbital's scale -- which also keeps every int32 sum far from overflow.  Output: Xpart[sp][g][2 w + c], the
+// layout k_ej reads (it adds the split partials, forms E_J and picks the hbar row).
+__global__ void __launch_bounds__(384, 1) k_coulomb_i8(const int8_t* __restrict__ Lq, const int8_t* __restrict__ Thq, const int* __restrict__ eL,
+                                                       const double* __restrict__ thScale, long long n_items, int NB, int NBcap, int KB, int Wcap,
+                                                       int O_tot, int nsplit, int Xp, int ldw, double* __restrict__ Xpart, int* __restrict__ fail) {
+    extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) unsigned long long bar_s[2 * XI_STAGES + 2];      // full[], empty[], acc_full, acc_empty
+    __shared__ uint32_t tmem_base_s;
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t full = smem_u32(&bar_s[0]), empty = full + 8 * XI_STAGES, acc_full = empty + 8 * XI_STAGES, acc_empty = acc_full + 8;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tmem = xi_cta_setup(full, &tmem_base_s);
+    const long long my_items = n_items > (long long)blockIdx.x ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    bool ok = true;
+    // item q -> (gt, nb, sp), sp fastest: the splits of one (gt, nb) run side by side on neighbouring CTAs
+#define XI_CO_ITEM(q_)                                                              \
+    const int sp = (int)((q_) % nsplit), nb = (int)(((q_) / nsplit) % NB), gt = (int)((q_) / ((long long)nsplit * NB)); \
+    const int o0 = (int)((long long)O_tot * sp / nsplit), o1 = (int)((long long)O_tot * (sp + 1) / nsplit)
+    if (warp < 4) {
+        reg_dec_producer();
+        if (warp == 0 && lane == 0) {
+            int slot = 0;
+            uint32_t phase = 0;
+            for (long long it = 0; it < my_items && ok; ++it) {
+                XI_CO_ITEM(blockIdx.x + it * gridDim.x);
+                for (int o = o0; o < o1 && ok; ++o) {
+                    const int8_t* th = Thq + (size_t)(o * NBcap + nb) * KB * XI_TH_STAGE;
+                    const int8_t* lq = Lq + ((size_t)gt * O_tot + o) * KB * XI_F_STAGE;
+                    for (int kb = 0; kb < KB; ++kb) {
+                        ok = xi_wait(empty + 8 * slot, phase ^ 1);
+                        if (!ok) break;
+                        const uint32_t st = sbase + slot * XI_STAGE, bar = full + 8 * slot;
+                        mbar_expect_tx(bar, XI_STAGE);
+                        xi_bulk(st, th + (size_t)kb * XI_TH_STAGE, XI_TH_STAGE, bar);
+                        xi_bulk(st + XI_TH_STAGE, lq + (size_t)kb * XI_F_STAGE, XI_F_STAGE, bar);
+                        if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
+                    }
+                }
+            }
+            if (!ok) atomicExch(fail, 1);
+        } else if (warp == 1 && lane == 0) {
+            int slot = 0;
+            uint32_t phase = 0, pe = 1;
+            for (long long it = 0; it < my_items && ok; ++it) {
+                XI_CO_ITEM(blockIdx.x + it * gridDim.x);
+                (void)nb; (void)gt;
+                for (int o = o0; o < o1 && ok; ++o) {
+                    ok = xi_wait(acc_empty, pe);
+                    if (!ok) break;
+                    pe ^= 1;
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    for (int kb = 0; kb < KB; ++kb) {
+                        ok = xi_wait(full + 8 * slot, phase);
+                        if (!ok) break;
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        xi_mma_kblock(tmem, sbase + slot * XI_STAGE, 64u, kb == 0);
+                        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(empty + 8 * slot) : "memory");
+                        if (++slot == XI_STAGES) { slot = 0; phase ^= 1; }
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(acc_full) : "memory");
+                }
+            }
+            if (!ok) atomicExch(fail, 1);
+        }
+    } else {
+        reg_inc_consumer();
+        const int quad = warp & 3, half = (warp - 4) >> 2;
+        const int m = quad * 32 + lane;                                // row of the walker block = 2 (w % 64) + c
+        const uint32_t tbase = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)half * 32;
+        uint32_t pf = 0;
+        for (long long it = 0; it < my_items && ok; ++it) {
+            XI_CO_ITEM(blockIdx.x + it * gridDim.x);
+            const int w = nb * 64 + (m >> 1), g0 = gt * 64 + half * 32;
+            double x[32], b[32], d1 = 0.0, d2 = 0.0;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) x[j] = 0.0;
+            for (int o = o0; o < o1; ++o) {
+                const double sw = thScale[(size_t)o * Wcap + w];
+                ok = xi_wait(acc_full, pf);
+                ok = __all_sync(0xffffffffu, ok);
+                if (!ok) break;
+                pf ^= 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                xi_readout<false>(tbase, b, b, d1, d2);
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(acc_empty);
+                const int* el = eL + (size_t)o * Xp + g0;        // the same 128 bytes for every lane: one broadcast line
+#pragma unroll
+                for (int j = 0; j < 32; ++j) x[j] = fma(b[j] * xi_pow2(__ldg(el + j)), sw, x[j]);
+            }
+            if (!ok) break;
+            // a warp stores 32 consecutive doubles of one row g per j: coalesced
+            double* out = Xpart + ((size_t)sp * Xp + g0) * ldw + (size_t)nb * 128 + m;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) out[(size_t)j * ldw] = x[j];
+        }
+        if (!ok && lane == 0) atomicExch(fail, 1);
+    }
+#undef XI_CO_ITEM
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)XI_TMEM_COLS) : "memory");
+}
+
+// Lbar -> exponents eL[o][g] of every (row g, orbital o) segment (one warp each: a localized orbital far from the site of g holds
+// much smaller entries than the row's largest, and the accumulators are read out per orbital anyway) and digits
+// Lq [gt][o][kb][7][64 x 32].
+__global__ void __launch_bounds__(256) k_lbar_exponents(const double* __restrict__ Lbar, int* __restrict__ eL, int Xp, int O_tot, int N_pad) {
+    const int lane = threadIdx.x & 31;
+    const long long seg = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (seg >= (long long)Xp * O_tot) return;
+    const int g = (int)(seg / O_tot), o = (int)(seg % O_tot);
+    const double* src = Lbar + (size_t)seg * N_pad;
+    double mx = 0.0;
+    for (int i = lane; i < N_pad; i += 32) mx = fmax(mx, fabs(src[i]));
+#pragma unroll
+    for (int d = 16; d; d >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+    if (lane == 0) eL[(size_t)o * Xp + g] = row_exponent(mx);
+}
+__global__ void __launch_bounds__(256) k_slice_lbar(const double* __restrict__ Lbar, const int* __restrict__ eL, int8_t* __restrict__ Lq, int O_tot,
+                                                    int N_pad, int KB, int Xp) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gt = blockIdx.x, o = blockIdx.y;
+    const int nch = 2 * KB;
+    int8_t* blk = Lq + ((size_t)gt * O_tot + o) * KB * XI_F_STAGE;
+    for (int r = warp; r < 64; r += 8) {
+        const int g = gt * 64 + r;
+        const double* src = Lbar + ((size_t)g * O_tot + o) * N_pad;
+        const double inv = scalbn(1.0, -eL[(size_t)o * Xp + g]);
+        for (int ch = lane; ch < nch; ch += 32) {
+            const int k0 = ch * 16;
+            int4 out[XI_S];
+            if (k0 < N_pad) slice16(src + k0, inv, out);
+            else {
+#pragma unroll
+                for (int s = 0; s < XI_S; ++s) out[s] = make_int4(0, 0, 0, 0);
+            }
+            int8_t* dst = blk + (size_t)(ch >> 1) * XI_F_STAGE + (r >> 3) * 256 + (ch & 1) * 128 + (r & 7) * 16;
+#pragma unroll
+            for (int s = 0; s < XI_S; ++s) *reinterpret_cast<int4*>(dst + s * XI_F_BLK) = out[s];
+        }
+    }
+}
+
 // a bounded wait expired somewhere: poison the partial sums so that every energy of the call comes out NaN
 __global__ void k_i8_poison(const int* __restrict__ fail, double* __restrict__ ekpart, int n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -430,10 +588,11 @@ __global__ void k_i8_poison(const int* __restrict__ fail, double* __restrict__ e
 }  // namespace
 
 void free_exchange_i8(lo_factors* f) {
-    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dI8Fail};
+    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dI8Fail, f->dLq, f->dELq};
     for (void* p : ptrs)
         if (p) cudaFree(p);
-    f->dUq = f->dWq = f->dThq = nullptr;
+    f->dUq = f->dWq = f->dThq = f->dLq = nullptr;
+    f->dELq = nullptr;
     f->dWgtQ = f->dThScale = f->dEKq = nullptr;
     f->dI8Fail = nullptr;
     f->i8_bytes = 0;
@@ -455,6 +614,7 @@ lo_status build_exchange_i8(lo_factors* f) {
     static bool configured = false;
     if (!configured) {
         CK(cudaFuncSetAttribute(k_exchange_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
+        CK(cudaFuncSetAttribute(k_coulomb_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
         configured = true;
     }
     const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64;
@@ -468,11 +628,21 @@ lo_status build_exchange_i8(lo_factors* f) {
     CK(cudaMalloc(&f->dWgtQ, (size_t)rows_al * 8));
     CK(cudaMalloc(&f->dThScale, (size_t)f->O_tot * f->Wcap * 8));
     CK(cudaMalloc(&f->dEKq, (size_t)2 * f->num_sms * f->Wcap * 16));
+    const size_t lq_bytes = (size_t)(f->Xp / 64) * f->O_tot * KB * XI_F_STAGE;
+    CK(cudaMalloc(&f->dLq, lq_bytes));
+    CK(cudaMalloc(&f->dELq, (size_t)f->Xp * f->O_tot * 4));
     CK(cudaMalloc(&f->dI8Fail, 4));
     CK(cudaMemset(f->dI8Fail, 0, 4));
     CK(cudaMemset(f->dWgtQ, 0, (size_t)rows_al * 8));
     CK(cudaMemset(f->dThq, 0, th_bytes));
-    f->i8_bytes = 2 * fq_bytes + th_bytes + (size_t)rows_al * 8;
+    f->i8_bytes = 2 * fq_bytes + th_bytes + lq_bytes + (size_t)rows_al * 8;
+    {
+        // digits of Lbar (rows g, incl. the hbar row) for the Coulomb / one-body contraction
+        k_lbar_exponents<<<(unsigned)(((long long)f->Xp * f->O_tot + 7) / 8), 256>>>(f->ops->dLbar, f->dELq, f->Xp, f->O_tot, f->N_pad);
+        dim3 gl(f->Xp / 64, f->O_tot);
+        k_slice_lbar<<<gl, 256>>>(f->ops->dLbar, f->dELq, f->dLq, f->O_tot, f->N_pad, KB, f->Xp);
+        CK(cudaDeviceSynchronize());
+    }
     if (f->n_tiles > 0) {
         cudaError_t e1 = cudaMalloc(&eU, (size_t)rows_al * 4), e2 = cudaMalloc(&eW, (size_t)rows_al * 4);
         if (e1 != cudaSuccess || e2 != cudaSuccess) {
@@ -495,12 +665,35 @@ lo_status build_exchange_i8(lo_factors* f) {
 #undef CK
 }
 
-// S4 in LO_EXCHANGE_INT8 mode: slice the Theta^T panels of this call, run the exchange on the tensor cores; the partial sums
-// land in f->dEKq as 2 * grid rows (*n_part) for k_finalize.
-void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part) {
+// INT8 route, per call: digits of the Theta^T panels (used by the Coulomb and the exchange kernels of this call)
+void launch_slice_theta_i8(lo_factors* f, int n_w, cudaStream_t stream) {
     const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64, NB = (n_w + 63) / 64, n_wpad = NB * 64;
     const long long warps = (long long)f->O_tot * n_wpad;
     k_slice_theta<<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(f->dThT, f->dThq, f->dThScale, f->O_tot, f->ldw, f->N_pad, KB, NBcap, f->Wcap, n_wpad);
+}
+
+// S2 + S3 on the INT8 route: X^g_w into f->dXpart as `nsplit` (returned) split partials over the orbitals; the caller runs k_ej
+int launch_coulomb_i8(lo_factors* f, int n_w, cudaStream_t stream) {
+    const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64, NB = (n_w + 63) / 64;
+    const long long base = (long long)(f->Xp / 64) * NB;
+    int nsplit = 1;
+    double best = -1.0;
+    for (int s = 1; s <= std::min(MAX_SPLIT, f->O_tot); ++s) {       // fill the last wave
+        const long long items = base * s, waves = (items + f->num_sms - 1) / f->num_sms;
+        const double eff = (double)items / (double)(waves * f->num_sms);
+        if (eff > best + 0.02) { best = eff; nsplit = s; }
+    }
+    const long long items = base * nsplit;
+    const int grid = (int)std::min<long long>(items, f->num_sms);
+    k_coulomb_i8<<<grid, 384, XI_SMEM, stream>>>(f->dLq, f->dThq, f->dELq, f->dThScale, items, NB, NBcap, KB, f->Wcap, f->O_tot, nsplit, f->Xp, f->ldw,
+                                                 f->dXpart, f->dI8Fail);
+    return nsplit;
+}
+
+// S4 on the INT8 route (the Theta digits of this call are in place: launch_slice_theta_i8); the partial sums land in f->dEKq as
+// 2 * grid rows (*n_part) for k_finalize.
+void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part) {
+    const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64, NB = (n_w + 63) / 64;
     const long long items = f->n_tiles * NB;
     const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
     k_exchange_i8<<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,

@@ -217,6 +217,8 @@ struct lo_factors {
     double* dThScale = nullptr;            // [O_tot][Wcap] 2^e of the Theta rows
     double* dEKq = nullptr;                // [2 * num_sms][Wcap] complex partial sums
     int* dI8Fail = nullptr;
+    int8_t* dLq = nullptr;                 // [Xp/64][O_tot][KB][7][64 x 32] digit slices of Lbar (rows g incl. hbar)
+    int* dELq = nullptr;                   // [O_tot][Xp] exponents of the (row g, orbital o) segments of Lbar
     unsigned long long i8_bytes = 0;
     // timing
     bool timing = false;
@@ -294,6 +296,8 @@ lo_status gpu_gather_rows(const double* src, double* dst, const GatherRec* table
 // exchange from INT8 digit slices on tcgen05 (lo_exchange_i8.cu)
 lo_status build_exchange_i8(lo_factors* f);
 void free_exchange_i8(lo_factors* f);
+void launch_slice_theta_i8(lo_factors* f, int n_w, cudaStream_t stream);
+int launch_coulomb_i8(lo_factors* f, int n_w, cudaStream_t stream);
 void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part);
 
 // microbenchmarks (lo_peak.cu)

@@ -1241,7 +1241,16 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
     const int N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
     const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
     // ---- S2 + S3
-    launch_coulomb_x(f, n_w, stream);
+    const bool i8 = f->ex_mode == LO_EXCHANGE_INT8 && !f->coulomb_lo;
+    if (i8) {
+        // INT8 route (lo_exchange_i8.cu): digits of Theta^T once per call, X^g_w from exact INT8 digit products on tcgen05, then k_ej
+        Timer tm(f, stream, LO_K_COULOMB);
+        launch_slice_theta_i8(f, n_w, stream);
+        const int nsplit = launch_coulomb_i8(f, n_w, stream);
+        dim3 g2(NB * 2, f->Xp / CO_BM);
+        k_ej<<<g2, 256, 0, stream>>>(f->dXpart, (double2*)f->dEJpart, (double2*)f->dEJpart + (size_t)(f->Xp / CO_BM) * Wcap, f->Xp, ldw, nsplit, f->n_chol, Wcap);
+    } else
+        launch_coulomb_x(f, n_w, stream);
     const int RB = f->Xp / CO_BM;
     double2* EJpart = (double2*)f->dEJpart;
     double2* E1raw = EJpart + (size_t)RB * Wcap;
@@ -1256,7 +1265,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         const bool ragged = n_w % WALKER_TILE != 0;
         // small problems: static LPT schedule of the tiles (grid = all SMs); large ones: round robin in L2-block order
         const ExItems rr = {nullptr, nullptr}, lpt = {f->dSchedOff, f->dSchedTile};
-        if (!coul && f->ex_mode == LO_EXCHANGE_INT8) {
+        if (i8) {
             // fp64-accurate projections from INT8 digit slices on the tcgen05 tensor cores (lo_exchange_i8.cu)
             launch_exchange_i8(f, n_w, stream, &ek_part, &ex_grid);
         } else if (!coul && n_w <= 32) {
