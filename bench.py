@@ -317,21 +317,35 @@ def run_ours(args):
         gx = torch.Generator(device=dev).manual_seed(P.seed + rank)
         x = torch.randn((n_w, info.n_chol, 2), dtype=torch.float64, device=dev, generator=gx)
         x = torch.view_as_complex(x).contiguous()
-        for _ in range(3):
-            F.propagator(x)
-        torch.cuda.synchronize()
-        F.timing_enable(True)
-        F.timing_get()
-        for _ in range(args.steps):
-            F.propagator(x)
-        torch.cuda.synchronize()
-        pm, pn = F.timing_get()["propagator"]
-        F.timing_enable(False)
-        p_ms = pm / max(pn, 1)
+        def time_propagator():
+            for _ in range(3):
+                F.propagator(x)
+            torch.cuda.synchronize()
+            F.timing_enable(True)
+            F.timing_get()
+            for _ in range(args.steps):
+                F.propagator(x)
+            torch.cuda.synchronize()
+            pm, pn = F.timing_get()["propagator"]
+            F.timing_enable(False)
+            return pm / max(pn, 1)
+        p_ms = time_propagator()
         p_tf = fl["propagator"] * n_w / (p_ms * 1e-3) * 1e-12
-        nxt = {"propagator": {"what": "B_w = sum_g x^g_w L^g for all walkers, upper triangle (PAPER.md:310), k_pack_x + DMMA GEMM",
-                              "ms": round(p_ms, 4), "tflops": round(p_tf, 3), "frac_of_peak": round(p_tf / peak, 4),
-                              "flops_per_walker": fl["propagator"]}}
+        if int8:
+            # fp64-equivalent rate of the INT8 route (28 digit products per multiply-add), next to the DMMA route of the same call
+            F.set_exchange_mode(False)
+            pd_ms = time_propagator()
+            F.set_exchange_mode(True)
+            pd_tf = fl["propagator"] * n_w / (pd_ms * 1e-3) * 1e-12
+            nxt = {"propagator": {"what": "B_w = sum_g x^g_w L^g for all walkers, upper triangle (PAPER.md:310): k_pack_x + k_slice_theta + k_coulomb_i8 "
+                                          "(INT8 digit slices on tcgen05)",
+                                  "ms": round(p_ms, 4), "fp64_equivalent_tflops": round(p_tf, 3), "fp64_equivalent_over_measured_dmma_peak": round(p_tf / peak, 4),
+                                  "dmma_route_ms": round(pd_ms, 4), "dmma_route_tflops": round(pd_tf, 3), "dmma_route_frac_of_peak": round(pd_tf / peak, 4),
+                                  "flops_per_walker": fl["propagator"]}}
+        else:
+            nxt = {"propagator": {"what": "B_w = sum_g x^g_w L^g for all walkers, upper triangle (PAPER.md:310), k_pack_x + DMMA GEMM",
+                                  "ms": round(p_ms, 4), "tflops": round(p_tf, 3), "frac_of_peak": round(p_tf / peak, 4),
+                                  "flops_per_walker": fl["propagator"]}}
 
     # ---- SURVEY 8(f) NEXT-3 (outside `value`): the paper-literal energy, Coulomb term from the compressed factors too
     if info.n_spin == 1:

@@ -588,11 +588,13 @@ __global__ void k_i8_poison(const int* __restrict__ fail, double* __restrict__ e
 }  // namespace
 
 void free_exchange_i8(lo_factors* f) {
-    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dI8Fail, f->dLq, f->dELq};
+    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dI8Fail, f->dLq, f->dELq, f->dLtq, f->dELt, f->dXq, f->dXScale};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     f->dUq = f->dWq = f->dThq = f->dLq = nullptr;
-    f->dELq = nullptr;
+    f->dELq = f->dELt = nullptr;
+    f->dLtq = f->dXq = nullptr;
+    f->dXScale = nullptr;
     f->dWgtQ = f->dThScale = f->dEKq = nullptr;
     f->dI8Fail = nullptr;
     f->i8_bytes = 0;
@@ -643,6 +645,21 @@ lo_status build_exchange_i8(lo_factors* f) {
         k_slice_lbar<<<gl, 256>>>(f->ops->dLbar, f->dELq, f->dLq, f->O_tot, f->N_pad, KB, f->Xp);
         CK(cudaDeviceSynchronize());
     }
+    if (f->ops->dLt) {
+        // propagator (LO_SETUP_PROPAGATOR): digits of Lt [r(p,q)][g] (one exponent per row) and room for the digits of the fields
+        const int KBx = (f->ops->Xk_pad + 31) / 32;
+        const size_t ltq_bytes = (size_t)(f->ops->tri_pad / 64) * KBx * XI_F_STAGE, xq_bytes = (size_t)NBcap * KBx * XI_TH_STAGE;
+        CK(cudaMalloc(&f->dLtq, ltq_bytes));
+        CK(cudaMalloc(&f->dELt, (size_t)f->ops->tri_pad * 4));
+        CK(cudaMalloc(&f->dXq, xq_bytes));
+        CK(cudaMalloc(&f->dXScale, (size_t)f->Wcap * 8));
+        CK(cudaMemset(f->dXq, 0, xq_bytes));
+        f->i8_bytes += ltq_bytes + xq_bytes;
+        k_lbar_exponents<<<(unsigned)((f->ops->tri_pad + 7) / 8), 256>>>(f->ops->dLt, f->dELt, (int)f->ops->tri_pad, 1, f->ops->Xk_pad);
+        dim3 gl((unsigned)(f->ops->tri_pad / 64), 1);
+        k_slice_lbar<<<gl, 256>>>(f->ops->dLt, f->dELt, f->dLtq, 1, f->ops->Xk_pad, KBx, (int)f->ops->tri_pad);
+        CK(cudaDeviceSynchronize());
+    }
     if (f->n_tiles > 0) {
         cudaError_t e1 = cudaMalloc(&eU, (size_t)rows_al * 4), e2 = cudaMalloc(&eW, (size_t)rows_al * 4);
         if (e1 != cudaSuccess || e2 != cudaSuccess) {
@@ -688,6 +705,19 @@ int launch_coulomb_i8(lo_factors* f, int n_w, cudaStream_t stream) {
     k_coulomb_i8<<<grid, 384, XI_SMEM, stream>>>(f->dLq, f->dThq, f->dELq, f->dThScale, items, NB, NBcap, KB, f->Wcap, f->O_tot, nsplit, f->Xp, f->ldw,
                                                  f->dXpart, f->dI8Fail);
     return nsplit;
+}
+
+// Propagator formation B[r(p,q)][w] = sum_g L^g_pq x^g_w on the INT8 route: the packed fields f->dXT ([2w + c][g],
+// the layout of a one-orbital Theta^T panel with K = g) are cut into digits like Theta, the GEMM is k_coulomb_i8 with one
+// "orbital" segment of ceil(n_chol / 32) K blocks against the digits of Lt; output straight into f->dB.
+void launch_propagator_i8(lo_factors* f, int n_w, cudaStream_t stream) {
+    const int KBx = (f->ops->Xk_pad + 31) / 32, NBcap = f->Wcap / 64, NB = (n_w + 63) / 64, n_wpad = NB * 64;
+    k_slice_theta<<<(unsigned)((n_wpad + 7) / 8), 256, 0, stream>>>(f->dXT, f->dXq, f->dXScale, 1, f->ldw, f->ops->Xk_pad, KBx, NBcap, f->Wcap, n_wpad);
+    const long long items = (long long)(f->ops->tri_pad / 64) * NB;
+    const int grid = (int)std::min<long long>(items, f->num_sms);
+    k_coulomb_i8<<<grid, 384, XI_SMEM, stream>>>(f->dLtq, f->dXq, f->dELt, f->dXScale, items, NB, NBcap, KBx, f->Wcap, 1, 1, (int)f->ops->tri_pad, f->ldw,
+                                                 f->dB, f->dI8Fail);
+    k_i8_poison<<<(f->ldw + 255) / 256, 256, 0, stream>>>(f->dI8Fail, f->dB, f->ldw);      // an expired wait: NaN in row 0 of every walker
 }
 
 // S4 on the INT8 route (the Theta digits of this call are in place: launch_slice_theta_i8); the partial sums land in f->dEKq as

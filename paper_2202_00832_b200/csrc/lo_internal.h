@@ -218,6 +218,10 @@ struct lo_factors {
     double* dEKq = nullptr;                // [2 * num_sms][Wcap] complex partial sums
     int* dI8Fail = nullptr;
     int8_t* dLq = nullptr;                 // [Xp/64][O_tot][KB][7][64 x 32] digit slices of Lbar (rows g incl. hbar)
+    int8_t* dLtq = nullptr;                // propagator: [tri_pad/64][KBx][7][64 x 32] digit slices of Lt (rows r(p,q), K = g)
+    int* dELt = nullptr;                   // [tri_pad] exponents of the Lt rows
+    int8_t* dXq = nullptr;                 // [Wcap/64][KBx][7][128 x 32] digit slices of the packed fields, rewritten every lo_propagator call
+    double* dXScale = nullptr;             // [Wcap] 2^e of the field rows
     int* dELq = nullptr;                   // [O_tot][Xp] exponents of the (row g, orbital o) segments of Lbar
     unsigned long long i8_bytes = 0;
     // timing
@@ -298,6 +302,7 @@ lo_status build_exchange_i8(lo_factors* f);
 void free_exchange_i8(lo_factors* f);
 void launch_slice_theta_i8(lo_factors* f, int n_w, cudaStream_t stream);
 int launch_coulomb_i8(lo_factors* f, int n_w, cudaStream_t stream);
+void launch_propagator_i8(lo_factors* f, int n_w, cudaStream_t stream);
 void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part);
 
 // microbenchmarks (lo_peak.cu)

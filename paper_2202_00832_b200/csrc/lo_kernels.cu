@@ -1318,7 +1318,9 @@ lo_status launch_propagator(lo_factors* f, int n_w, const void* x_dev, cudaStrea
         k_pack_x<<<g1, 128, 0, stream>>>((const double2*)x_dev, f->dXT, f->n_chol, ops.Xk_pad);
         const long long items = (long long)RB * NB;
         const int grid = (int)std::min<long long>(items, f->num_sms);
-        if (n_w % WALKER_TILE)
+        if (f->ex_mode == LO_EXCHANGE_INT8 && f->dLtq)
+            launch_propagator_i8(f, n_w, stream);          // exact INT8 digit products on tcgen05 (lo_exchange_i8.cu)
+        else if (n_w % WALKER_TILE)
             k_coulomb<true, 4><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);
         else
             k_coulomb<false, 4><<<grid, 384, CO_SMEM, stream>>>(ops.tmLt, f->tmXT, f->tmXT, f->dB, (int)ops.tri_pad, 1, ops.Xk_pad, f->ldw, RB, NB, 1, 2 * n_w);

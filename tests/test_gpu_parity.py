@@ -991,6 +991,37 @@ def test_exchange_int8_mode_matches_oracle(cfg, T, n_w):
     assert np.array_equal(Ed2, Ed)
 
 
+@pytest.mark.parametrize("n_w", [5, 130])
+def test_propagator_int8_mode_matches_oracle(c1, n_w):
+    """lo_propagator in LO_EXCHANGE_INT8 mode (digits of Lt and of the fields, k_coulomb_i8 with one K segment): element by element
+    against the oracle's triple loop, 5e-12 of max|B_w| (the digits keep 2^-46 .. 2^-48 of the largest |x^g_w| of the walker and of
+    the largest |L^g_pq| of the row, summed over n_chol terms; here with one field component 1000 x the others), on a ragged batch;
+    switching back reproduces the DMMA result bit for bit."""
+    torch = torch_cuda()
+    F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=n_w, gpu_svd=True, propagator=True)
+    rng = np.random.default_rng(12)
+    x = rng.standard_normal((n_w, c1.n_chol)) + 1j * rng.standard_normal((n_w, c1.n_chol))
+    x[:, 5] *= 1e3                                     # a field component far above the others
+    xd = torch.from_numpy(x).cuda()
+    F.propagator(xd)
+    torch.cuda.synchronize()
+    ws = [0, 3, 4] if n_w == 5 else [0, 63, 64, 129]
+    Bd = [F.propagator_host(w) for w in ws]
+    F.set_exchange_mode(True)
+    F.propagator(xd)
+    torch.cuda.synchronize()
+    for w, B0 in zip(ws, Bd):
+        Bo = oracle.propagator(c1.L, x[w])
+        Bq = F.propagator_host(w)
+        assert np.abs(Bq - Bo).max() <= 5e-12 * np.abs(Bo).max()
+        assert np.abs(Bq - B0).max() <= 5e-12 * np.abs(Bo).max()
+    F.set_exchange_mode(False)
+    F.propagator(xd)
+    torch.cuda.synchronize()
+    for w, B0 in zip(ws, Bd):
+        assert np.array_equal(F.propagator_host(w), B0)
+
+
 def test_exchange_int8_mode_unrestricted_and_host_variant():
     """Same check for an unrestricted trial (two tile lists, panels of both spins) and through lo_local_energy_host (walker
     chunks of different sizes through the same sliced factor set)."""
