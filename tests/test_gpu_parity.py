@@ -398,6 +398,12 @@ def test_c3_full_size_unrestricted_sampled_walkers():
     assert (so == 0).all()
     assert_parity(Eg[idx], Eo)
     assert_all_walkers(P, F, phis, Eg)
+    # the same batch on the INT8 route (exchange of both spins and the Coulomb term summed over both spins from digit slices):
+    # the sampled walkers against the oracle, every walker against the DMMA route
+    Eq, sq = int8_energy(F, phis)
+    assert (sq == 0).all()
+    assert_parity(Eq[idx], Eo)
+    assert_close(Eq, Eg, "INT8 route vs DMMA route, configs[3]", tol=1e-10)
 
 
 def test_c4_threshold_sweep_parity():
