@@ -552,6 +552,41 @@ def run_sweep(args):
                "exchange_tflops": round(fl["exchange"] * n_w / (ex_ms * 1e-3) * 1e-12, 3) if ex_ms > 0 else 0.0,
                "exchange_frac_of_peak": round(fl["exchange"] * n_w / (ex_ms * 1e-3) * 1e-12 / peak, 4) if ex_ms > 0 else 0.0,
                "peak_tflops": round(peak, 3), "setup_s_tightest": round(setup_s, 1), "oracle_exact_s": round(exact_s, 1)}
+        # ---- the same factor set on the INT8 route (exchange + Coulomb from digit slices on tcgen05), when its digits fit beside
+        # what is resident (the sweep keeps the tightest set alive for the re-truncations: run one threshold per invocation,
+        # --threshold T, to get this leg at every threshold of configs[4])
+        if args.exchange == "int8":
+            need = 0.9 * info.factor_bytes + 1.0 * info.lbar_bytes + (2 << 30)
+            free_b = torch.cuda.mem_get_info()[0]
+            if free_b < need:
+                row["int8"] = {"skipped": "digits need %.1f GB, %.1f GB free" % (need / 1e9, free_b / 1e9)}
+            else:
+                E_d = torch.stack(out[:4], dim=1).cpu().numpy()
+                F.set_exchange_mode(True)
+                for _ in range(max(args.warmup, 3)):
+                    out = F.local_energy(dphi, parts=True)
+                torch.cuda.synchronize()
+                F.timing_enable(True)
+                F.timing_get()
+                ev0.record()
+                for _ in range(args.steps):
+                    out = F.local_energy(dphi, parts=True)
+                ev1.record()
+                torch.cuda.synchronize()
+                ms8 = ev0.elapsed_time(ev1) / args.steps
+                tm8 = F.timing_get()
+                F.timing_enable(False)
+                F.set_exchange_mode(False)
+                E_q = torch.stack(out[:4], dim=1).cpu().numpy()
+                ex8 = tm8["exchange"][0] / max(tm8["exchange"][1], 1)
+                EK8 = E_q[:, 3]
+                row["int8"] = {"ms_per_step": round(ms8, 3), "energies_per_s": round(n_w / (ms8 * 1e-3), 2), "exchange_ms": round(ex8, 3),
+                               "coulomb_ms": round(tm8["coulomb"][0] / max(tm8["coulomb"][1], 1), 3),
+                               "exchange_fp64_equivalent_tflops": round(fl["exchange"] * n_w / (ex8 * 1e-3) * 1e-12, 2),
+                               "exchange_int8_pops": round(28.0 * 8.0 * info.N * sum_r * n_w / (ex8 * 1e-3) * 1e-15, 3),
+                               "max_rel_diff_vs_dmma_route": float((np.abs(E_q - E_d).max(axis=1) / np.abs(E_d[:, 0])).max()),
+                               "EK_abs_err_vs_exact_max": float(max(abs(EK8[w] - ek) for (ek, _), w in zip(exact, idx))),
+                               "int8_slices_GB": round(F.info().int8_bytes / 1e9, 2)}
         print(json.dumps(row), flush=True)
         rows.append(row)
         if F is not F0:
