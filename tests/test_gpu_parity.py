@@ -676,12 +676,15 @@ def test_cas_smw_energy_matches_oracle(cfg, n_virt, n_act, n_det, max_exc, n_w, 
     assert (np.abs(E - Ed).max(axis=1) <= 1e-9 * np.abs(Ed[:, 0])).all()
 
 
-def test_local_energy_is_cuda_graph_capturable(c1):
+@pytest.mark.parametrize("int8", [False, True])
+def test_local_energy_is_cuda_graph_capturable(c1, int8):
     """lo_local_energy allocates nothing, does not synchronise and launches only on the caller's stream, so a whole
-    step can be captured in a CUDA graph and replayed on new walker data (launch-bound small configs)."""
+    step can be captured in a CUDA graph and replayed on new walker data (launch-bound small configs); on both routes (the
+    digit slices of the INT8 route are built at the mode switch, before the capture)."""
     torch = torch_cuda()
     n_w = 64
     F = lo.Factors.setup(c1.h, c1.L, c1.psi, 1e-4, device=0, max_walkers=n_w, gpu_svd=True)
+    F.set_exchange_mode(int8)
     phis = gen.make_walkers(c1, n_w)
     E_ref, _ = gpu_energy(F, phis)
     buf = torch.zeros((n_w, c1.N, c1.n_occ[0]), dtype=torch.complex128, device="cuda")
