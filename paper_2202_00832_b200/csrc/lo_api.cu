@@ -908,6 +908,12 @@ lo_status lo_set_exchange_mode(lo_factors* f, int mode) {
     if (!f || (mode != LO_EXCHANGE_DMMA && mode != LO_EXCHANGE_INT8)) { set_error("lo_set_exchange_mode: invalid argument"); return LO_EINVAL; }
     if (mode == LO_EXCHANGE_INT8) {
         if (f->device < 0) { set_error("lo_set_exchange_mode: LO_EXCHANGE_INT8 needs a device-resident factor set"); return LO_EINVAL; }
+        // exact int32 digit sums: 7 products of |digit| <= 64 per multiply-add, over N basis functions (exchange, Coulomb per orbital)
+        // or n_chol fields (propagator): 7 * 4096 * K < 2^31
+        if (f->N_pad > 65536 || (f->ops->dLt && f->ops->Xk_pad > 65536)) {
+            set_error("lo_set_exchange_mode: LO_EXCHANGE_INT8 supports N (and n_chol with the propagator) up to 65536");
+            return LO_EINVAL;
+        }
         lo_status st = build_exchange_i8(f);      // slices the factor rows on first use
         if (st != LO_OK) return st;
     }
