@@ -3,7 +3,7 @@
 // accumulators in TMEM), the sigma-weighted complex a.b reduction fused into the TMEM read-out.  Opt-in
 // (lo_set_exchange_mode(f, LO_EXCHANGE_INT8)); the default exchange stays the FP64 DMMA kernel k_exchange.
 //
-// Scheme (Ozaki-type splitting).  A row x of an operand is scaled by a power of two, |x| 2^-e <= 1/2,
+// Scheme (Ozaki-type splitting).  A row x of an operand is scaled by a power of two, |x| 2^-e < 1,
 // and cut into XI_S = 7 signed digits of 7 bits,  x = 2^e sum_s d_s 2^-(7 s + 6),  |d_s| <= 64  (exact: the remainder after
 // 7 digits is below 2^(e-49)).  Digit matrices are int8, their products are exact in int32 (|sum| <= 7 * N * 2^12), and
 //     a_K[m] = 2^(e_m + e_K) sum_{g <= 6} 2^-(7 g + 12) D_g[m][K],   D_g = sum_{s + t = g} dTheta_s dU_t^T
@@ -72,9 +72,9 @@ __device__ __forceinline__ void slice16(const double* __restrict__ src, double i
 }
 
 __device__ __forceinline__ int row_exponent(double mx) {
-    // |x| 2^-e <= 1/2 for every |x| <= mx;  rows of zeros and rows holding Inf / NaN (singular walkers, set to NaN by
-    // k_finalize) get e = 0
-    return (mx > 0.0 && mx < 1e300) ? ilogb(mx) + 2 : 0;
+    // |x| 2^-e < 1 for every |x| <= mx, so that the leading digit rint(x 2^-e 2^6) lies in [-64, 64] like the others (one bit more
+    // than |x| 2^-e <= 1/2 would keep);  rows of zeros and rows holding Inf / NaN (singular walkers, set to NaN by k_finalize) get e = 0
+    return (mx > 0.0 && mx < 1e300) ? ilogb(mx) + 1 : 0;
 }
 
 // Theta^T panels -> Thq, thScale.  One warp per (orbital, walker): both rows (re, im) share the exponent.
