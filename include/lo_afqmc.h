@@ -176,7 +176,7 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
  *     every row of U, W, Lbar (per orbital) and Theta^T is scaled by a power of two and cut into 7 signed 7-bit digits; the 28
  *     digit products with digit-index sum <= 6 are exact int32 GEMMs accumulated in TMEM; recombination, sigma weights, the a.b
  *     reduction and E_J = sum_g (X^g)^2 in fp64).  Not bit-identical to the DMMA route: the projections carry an absolute error
- *     of about 2^-47 |row|_max |Theta row|_max N, the energies agree to ~1e-11 of |E_L| on the BASELINE configs (DESIGN.md
+ *     of about 2^-47 |row|_max |Theta row|_max N, the energies agree to 1e-12 .. 1e-11 of |E_L| on the BASELINE configs (DESIGN.md
  *     section 6b; the parity tests hold this route to the same 1e-10 as the default).  The first call slices the factor rows and
  *     Lbar once (extra device memory: 7/8 of the factor and Lbar bytes + 7 bytes per Theta^T element, lo_info.int8_bytes) and
  *     is synchronous; LO_ENOMEM leaves the set in LO_EXCHANGE_DMMA mode.  Ignored while LO_COULOMB_COMPRESSED is set and by
