@@ -349,8 +349,7 @@ def run_ours(args):
 
     # ---- SURVEY 8(f) NEXT-3 (outside `value`): the paper-literal energy, Coulomb term from the compressed factors too
     if info.n_spin == 1:
-        F.set_exchange_mode(False)      # the compressed-Coulomb kernel is the DMMA exchange kernel with two more projections
-        F.set_coulomb_mode(True)
+        F.set_coulomb_mode(True)        # in the mode of the timed step: four projections per pair from the INT8 digits, or DMMA
         flc = F.flops_per_walker()
         for _ in range(3):
             F.local_energy(dphi, parts=True)
@@ -369,7 +368,8 @@ def run_ours(args):
         c_ms = cm / max(cn, 1)
         c_tf = flc["exchange"] * n_w / (c_ms * 1e-3) * 1e-12
         nxt = dict(nxt or {})
-        nxt["compressed_coulomb"] = {"what": "lo_set_coulomb_mode(COMPRESSED): E_J and E_K both from the pair factors (Eq. 19/22), 4 projections per pair",
+        nxt["compressed_coulomb"] = {"what": "lo_set_coulomb_mode(COMPRESSED): E_J and E_K both from the pair factors (Eq. 19/22), 4 projections per pair"
+                                             + (" on the INT8 route (exchange_tflops is fp64-equivalent)" if int8 else ""),
                                      "ms_per_step": round(c0.elapsed_time(c1) / args.steps, 4),
                                      "energies_per_s": round(n_w * args.steps / (c0.elapsed_time(c1) * 1e-3), 2),
                                      "exchange_ms": round(c_ms, 4), "exchange_tflops": round(c_tf, 3), "exchange_frac_of_peak": round(c_tf / peak, 4)}

@@ -179,8 +179,8 @@ lo_status lo_set_coulomb_mode(lo_factors* f, int mode);
  *     of about 2^-47 |row|_max |Theta row|_max N, the energies agree to 1e-12 .. 1e-11 of |E_L| on the BASELINE configs (DESIGN.md
  *     section 6b; the parity tests hold this route to the same 1e-10 as the default).  The first call slices the factor rows and
  *     Lbar once (extra device memory: 7/8 of the factor and Lbar bytes + 7 bytes per Theta^T element, lo_info.int8_bytes) and
- *     is synchronous; LO_ENOMEM leaves the set in LO_EXCHANGE_DMMA mode.  Ignored while LO_COULOMB_COMPRESSED is set and by
- *     lo_local_energy_cas (both keep their DMMA kernels).  lo_propagator follows the mode as well (factor sets built with
+ *     is synchronous; LO_ENOMEM leaves the set in LO_EXCHANGE_DMMA mode.  Combines with LO_COULOMB_COMPRESSED (four projections
+ *     per pair from the same digits).  Ignored by lo_local_energy_cas, which keeps its DMMA kernels.  lo_propagator follows the mode as well (factor sets built with
  *     LO_SETUP_PROPAGATOR: the GEMM B = Lt x from digits of Lt, + 7/8 of its bytes, and of the fields).
  * Host-only factor sets: LO_EINVAL. */
 #define LO_EXCHANGE_DMMA 0

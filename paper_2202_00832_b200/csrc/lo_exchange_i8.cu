@@ -293,10 +293,14 @@ __device__ __forceinline__ uint32_t xi_cta_setup(uint32_t full, uint32_t* tmem_b
     return *tmem_base_s;
 }
 
+// COUL (lo_set_coulomb_mode(COMPRESSED)): two more phases per item, aJ = U Theta_i and bJ = W Theta_j (Eq. 19/22
+// first term, "forming the projected vectors must occur four times"), reduced with the same weights into ejpart.
+template <bool COUL>
 __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict__ Uq, const int8_t* __restrict__ Wq, const int8_t* __restrict__ Thq,
                                                         const double* __restrict__ wq, const double* __restrict__ thScale,
                                                         const ExTile* __restrict__ tiles, long long n_items, int NB, int NBcap, int KB, int Wcap,
-                                                        double* __restrict__ ekpart, int* __restrict__ fail) {
+                                                        double* __restrict__ ekpart, double* __restrict__ ejpart, int* __restrict__ fail) {
+    constexpr int NPH = COUL ? 4 : 2;       // phases of an item: (U, Theta_pj), (W, Theta_pi) [, (U, Theta_pi), (W, Theta_pj)]
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bar_s[2 * XI_STAGES + 2];      // full[], empty[], acc_full, acc_empty
     __shared__ uint32_t tmem_base_s;
@@ -304,7 +308,10 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
     const uint32_t full = smem_u32(&bar_s[0]), empty = full + 8 * XI_STAGES, acc_full = empty + 8 * XI_STAGES, acc_empty = acc_full + 8;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // partial sums: two rows per CTA (one per column half of the epilogue warps), zeroed here, updated by their owners only
-    for (int i = tid; i < 4 * Wcap; i += 384) ekpart[(size_t)blockIdx.x * 4 * Wcap + i] = 0.0;
+    for (int i = tid; i < 4 * Wcap; i += 384) {
+        ekpart[(size_t)blockIdx.x * 4 * Wcap + i] = 0.0;
+        if constexpr (COUL) ejpart[(size_t)blockIdx.x * 4 * Wcap + i] = 0.0;
+    }
     const uint32_t tmem = xi_cta_setup(full, &tmem_base_s);
     const long long my_items = n_items > (long long)blockIdx.x ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     bool ok = true;
@@ -327,9 +334,9 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(Wq + nxt + (size_t)kb * XI_F_STAGE), "r"((uint32_t)XI_F_STAGE) : "memory");
                     }
                 }
-                for (int ph = 0; ph < 2 && ok; ++ph) {
-                    const int8_t* th = Thq + (size_t)((ph ? tile.pi : tile.pj) * NBcap + nb) * KB * XI_TH_STAGE;
-                    const int8_t* fq = (ph ? Wq : Uq) + (size_t)tile_idx * KB * XI_F_STAGE;
+                for (int ph = 0; ph < NPH && ok; ++ph) {
+                    const int8_t* th = Thq + (size_t)(((ph == 1 || ph == 2) ? tile.pi : tile.pj) * NBcap + nb) * KB * XI_TH_STAGE;
+                    const int8_t* fq = ((ph & 1) ? Wq : Uq) + (size_t)tile_idx * KB * XI_F_STAGE;
                     for (int kb = 0; kb < KB; ++kb) {
                         ok = xi_wait(empty + 8 * slot, phase ^ 1);
                         if (!ok) break;
@@ -350,7 +357,7 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
                 const long long q = blockIdx.x + it * gridDim.x;
                 const ExTile tile = tiles[(int)(q / NB)];
                 const uint32_t Nmma = (uint32_t)((tile.nfrag * 8 + 15) / 16) * 16;
-                for (int ph = 0; ph < 2 && ok; ++ph) {
+                for (int ph = 0; ph < NPH && ok; ++ph) {
                     ok = xi_wait(acc_empty, pe);
                     if (!ok) break;
                     pe ^= 1;
@@ -376,51 +383,56 @@ __global__ void __launch_bounds__(384, 1) k_exchange_i8(const int8_t* __restrict
         const int m = quad * 32 + lane, wl = m >> 1, c = m & 1;       // row of the walker block = 2 wl + c
         const uint32_t tbase = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)half * 32;
         double2* mypart = reinterpret_cast<double2*>(ekpart) + (size_t)(2 * blockIdx.x + half) * Wcap;
+        double2* mypartJ = COUL ? reinterpret_cast<double2*>(ejpart) + (size_t)(2 * blockIdx.x + half) * Wcap : nullptr;
         uint32_t pf = 0;
         for (long long it = 0; it < my_items && ok; ++it) {
             const long long q = blockIdx.x + it * gridDim.x;
             const int tile_idx = (int)(q / NB), nb = (int)(q % NB);
             const ExTile tile = tiles[tile_idx];
             const int w = nb * 64 + wl, nrow = tile.nfrag * 8 - half * 32;      // live columns of this thread: [0, nrow)
-            double a[32], an[32], p1 = 0.0, p2 = 0.0;
-            // the weights of this thread's factor rows, fetched before the accumulators are waited for (0 beyond the tile: those
-            // TMEM columns were never written)
             const double* wrow = wq + tile.row0 + half * 32;
-#pragma unroll
-            for (int j = 0; j < 32; ++j) an[j] = j < nrow ? __ldg(wrow + j) : 0.0;
-            // ---- phase a: recombine, weight, fetch the re/im partner row
-            ok = xi_wait(acc_full, pf);
-            ok = __all_sync(0xffffffffu, ok);
-            if (!ok) break;
-            pf ^= 1;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            xi_readout<false>(tbase, a, an, p1, p2);
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(acc_empty);
-#pragma unroll
-            for (int j = 0; j < 32; ++j) {
-                a[j] *= an[j];
-                an[j] = __shfl_xor_sync(0xffffffffu, a[j], 1);
-            }
-            // ---- phase b: p1 = sum a_own b_own, p2 = sum a_partner b_own
-            ok = xi_wait(acc_full, pf);
-            ok = __all_sync(0xffffffffu, ok);
-            if (!ok) break;
-            pf ^= 1;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            xi_readout<true>(tbase, a, an, p1, p2);
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(acc_empty);
-            // row re (c = 0): p1 = sum a_re b_re, p2 = sum a_im b_re;  row im: p1 = sum a_im b_im, p2 = sum a_re b_im
             const double sw = thScale[(size_t)tile.pj * Wcap + w] * thScale[(size_t)tile.pi * Wcap + w];
-            const double o1 = __shfl_xor_sync(0xffffffffu, p1, 1), o2 = __shfl_xor_sync(0xffffffffu, p2, 1);
-            if (c == 0) {
-                double2 prev = mypart[w];
-                prev.x = fma(sw, p1 - o1, prev.x);
-                prev.y = fma(sw, p2 + o2, prev.y);
-                mypart[w] = prev;
+#pragma unroll 1
+            for (int pp = 0; pp < NPH / 2; ++pp) {          // pp = 0: exchange projections, pp = 1: compressed-Coulomb projections
+                double a[32], an[32], p1 = 0.0, p2 = 0.0;
+                // the weights of this thread's factor rows, fetched before the accumulators are waited for (0 beyond the tile: those
+                // TMEM columns were never written)
+#pragma unroll
+                for (int j = 0; j < 32; ++j) an[j] = j < nrow ? __ldg(wrow + j) : 0.0;
+                // ---- first phase of the pair: recombine, weight, fetch the re/im partner row
+                ok = xi_wait(acc_full, pf);
+                ok = __all_sync(0xffffffffu, ok);
+                if (!ok) break;
+                pf ^= 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                xi_readout<false>(tbase, a, an, p1, p2);
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(acc_empty);
+#pragma unroll
+                for (int j = 0; j < 32; ++j) {
+                    a[j] *= an[j];
+                    an[j] = __shfl_xor_sync(0xffffffffu, a[j], 1);
+                }
+                // ---- second phase: p1 = sum a_own b_own, p2 = sum a_partner b_own
+                ok = xi_wait(acc_full, pf);
+                ok = __all_sync(0xffffffffu, ok);
+                if (!ok) break;
+                pf ^= 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                xi_readout<true>(tbase, a, an, p1, p2);
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(acc_empty);
+                // row re (c = 0): p1 = sum a_re b_re, p2 = sum a_im b_re;  row im: p1 = sum a_im b_im, p2 = sum a_re b_im
+                const double o1 = __shfl_xor_sync(0xffffffffu, p1, 1), o2 = __shfl_xor_sync(0xffffffffu, p2, 1);
+                if (c == 0) {
+                    double2* dst = (COUL && pp) ? mypartJ : mypart;
+                    double2 prev = dst[w];
+                    prev.x = fma(sw, p1 - o1, prev.x);
+                    prev.y = fma(sw, p2 + o2, prev.y);
+                    dst[w] = prev;
+                }
             }
         }
         if (!ok && lane == 0) atomicExch(fail, 1);
@@ -588,14 +600,14 @@ __global__ void k_i8_poison(const int* __restrict__ fail, double* __restrict__ e
 }  // namespace
 
 void free_exchange_i8(lo_factors* f) {
-    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dI8Fail, f->dLq, f->dELq, f->dLtq, f->dELt, f->dXq, f->dXScale};
+    void* ptrs[] = {f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dEKq, f->dEJq, f->dI8Fail, f->dLq, f->dELq, f->dLtq, f->dELt, f->dXq, f->dXScale};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     f->dUq = f->dWq = f->dThq = f->dLq = nullptr;
     f->dELq = f->dELt = nullptr;
     f->dLtq = f->dXq = nullptr;
     f->dXScale = nullptr;
-    f->dWgtQ = f->dThScale = f->dEKq = nullptr;
+    f->dWgtQ = f->dThScale = f->dEKq = f->dEJq = nullptr;
     f->dI8Fail = nullptr;
     f->i8_bytes = 0;
 }
@@ -615,7 +627,8 @@ lo_status build_exchange_i8(lo_factors* f) {
     CK(cudaSetDevice(f->device));
     static bool configured = false;
     if (!configured) {
-        CK(cudaFuncSetAttribute(k_exchange_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
+        CK(cudaFuncSetAttribute(k_exchange_i8<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
+        CK(cudaFuncSetAttribute(k_exchange_i8<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
         CK(cudaFuncSetAttribute(k_coulomb_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, XI_SMEM));
         configured = true;
     }
@@ -630,6 +643,7 @@ lo_status build_exchange_i8(lo_factors* f) {
     CK(cudaMalloc(&f->dWgtQ, (size_t)rows_al * 8));
     CK(cudaMalloc(&f->dThScale, (size_t)f->O_tot * f->Wcap * 8));
     CK(cudaMalloc(&f->dEKq, (size_t)2 * f->num_sms * f->Wcap * 16));
+    CK(cudaMalloc(&f->dEJq, (size_t)2 * f->num_sms * f->Wcap * 16));
     const size_t lq_bytes = (size_t)(f->Xp / 64) * f->O_tot * KB * XI_F_STAGE;
     CK(cudaMalloc(&f->dLq, lq_bytes));
     CK(cudaMalloc(&f->dELq, (size_t)f->Xp * f->O_tot * 4));
@@ -722,16 +736,21 @@ void launch_propagator_i8(lo_factors* f, int n_w, cudaStream_t stream) {
 
 // S4 on the INT8 route (the Theta digits of this call are in place: launch_slice_theta_i8); the partial sums land in f->dEKq as
 // 2 * grid rows (*n_part) for k_finalize.
-void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part) {
+void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, bool coul, const double** part, int* n_part, const double** partJ) {
     const int KB = (f->N_pad + 31) / 32, NBcap = f->Wcap / 64, NB = (n_w + 63) / 64;
     const long long items = f->n_tiles * NB;
     const int grid = (int)std::min<long long>(std::max<long long>(items, 1), f->num_sms);
-    k_exchange_i8<<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,
-                                                  f->dI8Fail);
+    if (coul)
+        k_exchange_i8<true><<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,
+                                                            f->dEJq, f->dI8Fail);
+    else
+        k_exchange_i8<false><<<grid, 384, XI_SMEM, stream>>>(f->dUq, f->dWq, f->dThq, f->dWgtQ, f->dThScale, f->dTiles, items, NB, NBcap, KB, f->Wcap, f->dEKq,
+                                                             nullptr, f->dI8Fail);
     const int n = grid * 4 * f->Wcap;
     k_i8_poison<<<(n + 255) / 256, 256, 0, stream>>>(f->dI8Fail, f->dEKq, n);
     *part = f->dEKq;
     *n_part = 2 * grid;
+    *partJ = coul ? f->dEJq : nullptr;
 }
 
 }  // namespace lo

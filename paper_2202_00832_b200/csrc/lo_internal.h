@@ -216,6 +216,7 @@ struct lo_factors {
     double* dWgtQ = nullptr;               // [rows + 64] wgt * 2^(eU + eW)
     double* dThScale = nullptr;            // [O_tot][Wcap] 2^e of the Theta rows
     double* dEKq = nullptr;                // [2 * num_sms][Wcap] complex partial sums
+    double* dEJq = nullptr;                // same for the compressed Coulomb term (lo_set_coulomb_mode)
     int* dI8Fail = nullptr;
     int8_t* dLq = nullptr;                 // [Xp/64][O_tot][KB][7][64 x 32] digit slices of Lbar (rows g incl. hbar)
     int8_t* dLtq = nullptr;                // propagator: [tri_pad/64][KBx][7][64 x 32] digit slices of Lt (rows r(p,q), K = g)
@@ -303,7 +304,7 @@ void free_exchange_i8(lo_factors* f);
 void launch_slice_theta_i8(lo_factors* f, int n_w, cudaStream_t stream);
 int launch_coulomb_i8(lo_factors* f, int n_w, cudaStream_t stream);
 void launch_propagator_i8(lo_factors* f, int n_w, cudaStream_t stream);
-void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, const double** part, int* n_part);
+void launch_exchange_i8(lo_factors* f, int n_w, cudaStream_t stream, bool coul, const double** part, int* n_part, const double** partJ);
 
 // microbenchmarks (lo_peak.cu)
 lo_status measure_peak(int device, int kind, double* value);

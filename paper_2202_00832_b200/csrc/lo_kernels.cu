@@ -1241,7 +1241,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
     const int N_pad = f->N_pad, ldw = f->ldw, Wcap = f->Wcap;
     const int NB = (n_w + WALKER_TILE - 1) / WALKER_TILE;
     // ---- S2 + S3
-    const bool i8 = f->ex_mode == LO_EXCHANGE_INT8 && !f->coulomb_lo;
+    const bool i8 = f->ex_mode == LO_EXCHANGE_INT8;
     if (i8) {
         // INT8 route (lo_exchange_i8.cu): digits of Theta^T once per call, X^g_w from exact INT8 digit products on tcgen05, then k_ej
         Timer tm(f, stream, LO_K_COULOMB);
@@ -1257,6 +1257,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
     // ---- S4
     int ex_grid = 0;
     const double* ek_part = f->dEKpart;
+    const double* ejl_part = f->coulomb_lo ? f->dEJLpart : nullptr;
     {
         Timer tm(f, stream, LO_K_EXCHANGE);
         const bool coul = f->coulomb_lo != 0;
@@ -1267,7 +1268,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         const ExItems rr = {nullptr, nullptr}, lpt = {f->dSchedOff, f->dSchedTile};
         if (i8) {
             // fp64-accurate projections from INT8 digit slices on the tcgen05 tensor cores (lo_exchange_i8.cu)
-            launch_exchange_i8(f, n_w, stream, &ek_part, &ex_grid);
+            launch_exchange_i8(f, n_w, stream, coul, &ek_part, &ex_grid, &ejl_part);
         } else if (!coul && n_w <= 32) {
             // narrow batch: 16-walker column blocks, row fragments split over the warps
             const int NB16 = (n_w + 15) / 16;
@@ -1298,7 +1299,7 @@ lo_status launch_s3_s5(lo_factors* f, int n_w, void* E_L, void* E1, void* E_J, v
         k_finalize<<<(n_w + 127) / 128, 128, 0, stream>>>(EJpart, RB, E1raw, (const double2*)ek_part, ex_grid, f->dStatus, f->n_spin, Wcap,
                                                           n_w, c1, cJ, (double2*)E_L, (double2*)E1, (double2*)E_J, (double2*)E_K,
                                                           walker_status, (double2*)Eout4,
-                                                          f->coulomb_lo ? (const double2*)f->dEJLpart : nullptr);
+                                                          (const double2*)ejl_part);
     }
     f->last_n_w = n_w;
     cudaError_t e = cudaGetLastError();

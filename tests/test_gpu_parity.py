@@ -571,6 +571,16 @@ def test_compressed_coulomb_mode(T, reading):
     # the compressed Coulomb term carries a truncation error of the same order as the exchange's
     if T >= 1e-2:
         assert np.abs(E_lo[:, 2] - E_ch[:, 2]).max() > 1e-9 * scale.max()
+    # the same mode on the INT8 route (four projections per pair from the digit slices): every part against the DMMA result
+    # and E_J against the oracle's paper-literal sum
+    Eq, sq = int8_energy(F, phis)
+    assert (sq == 0).all()
+    assert_close(Eq, E_lo, "compressed Coulomb mode, INT8 route vs DMMA route", tol=1e-10)
+    for w in (0, 33, 69):
+        th, _, _ = oracle.theta(P.psi[0], phis[0][w])
+        assert abs(Eq[w, 2] - 2.0 * oracle.coulomb_lo(fs, th)) <= TOL * scale[w]
+    E_lo2, _ = gpu_energy(F, phis)
+    assert np.array_equal(E_lo2, E_lo)
     F.set_coulomb_mode(False)
     E_back, _ = gpu_energy(F, phis)
     assert np.array_equal(E_back, E_ch)
